@@ -1,0 +1,296 @@
+"""oracle/cc.py -- coupled-cluster residuals for the oracle.  TEST INFRASTRUCTURE ONLY.
+
+Three tiers:
+
+tier 0  `fock_space_residuals`: literally the paper's equations.  Jordan-Wigner matrices for the
+        a_p, a_p^dagger on the 2^n-dimensional Fock space; the Hamiltonian of PAPER Eq. (4)
+        (PAPER.md:298), the cluster operators of Eq. (2), the similarity
+        transform and projections of Eq. (3).  Exponentials by their
+        terminating series.  n = o+v <= ~8.
+tier 1a `ccd_residual_unfactorised`: the 10 spin-orbital CCD doubles terms + 1 energy term
+        (= the 11 CCD diagrams of PAPER Table I) as direct sums (numpy.einsum
+        as the library primitive for "sum over these indices").  The paper does not print these
+        (it cites textbooks); they are PINNED to tier 0 in tests/test_oracle_cc.py.
+tier 1b `ccd_residual_program`: the same residual as a list of BINARY tensor operations
+        (two tensors per instruction), every line one oracle.contract /
+        oracle.permsum / oracle.add call.  This is the config-2 workload.  Pinned to tier 1a.
+t3      `t3_term_unfactorised` / `t3_term_program`: the config-4 CCSDT piece
+        X(a,b,c,i,j,k) = sum_d <bc||dk> t_ij^ad ;  R3 += P(k/ij) P(a/bc) X  (9 signed terms),
+        pinned to the tier-0 triples projection of [H, T2]|Phi0>.
+
+Conventions: spinors 0..o-1 occupied, o..o+v-1 virtual.  g[p,q,r,s] = <pq||rs>.
+T2 is stored T[a,b,i,j] = t_ij^ab; integral blocks keep bra-ket order, e.g. oovv[k,l,c,d] = <kl||cd>.
+All arrays are complex128 (relativistic spinor basis: complex, no spin symmetry).
+"""
+import itertools
+
+import numpy as np
+
+import oracle as _o
+
+
+# ------------------------------------------------------------------------------------------
+# tier 0: Fock space
+# ------------------------------------------------------------------------------------------
+def jordan_wigner(n):
+    """a_p = Z^{(x)p} (x) [[0,1],[0,0]] (x) I^{(x)(n-p-1)}; returns list of dense (2^n, 2^n) annihilators."""
+    Z = np.diag([1.0, -1.0])
+    I2 = np.eye(2)
+    low = np.array([[0.0, 1.0], [0.0, 0.0]])
+    ops = []
+    for p in range(n):
+        m = np.array([[1.0]])
+        for q in range(n):
+            m = np.kron(m, Z if q < p else (low if q == p else I2))
+        ops.append(m)
+    return ops
+
+
+class FockSpace:
+    def __init__(self, o, v):
+        self.o, self.v, self.n = o, v, o + v
+        self.a = jordan_wigner(self.n)
+        self.ad = [m.T.copy() for m in self.a]          # real matrices: dagger = transpose
+        vac = np.zeros(2 ** self.n, dtype=np.complex128)
+        vac[0] = 1.0                                     # all sites in state |0> = empty
+        phi = vac
+        for i in reversed(range(o)):                     # |Phi0> = a+_0 a+_1 ... a+_{o-1} |vac>
+            phi = self.ad[i] @ phi
+        self.phi0 = phi
+
+    def apply_H(self, f, g, psi):
+        """H psi, H = sum h_pq a+_p a_q + 1/4 sum <pq||rs> a+_p a+_q a_s a_r   (PAPER Eq. 4),
+        with the bare one-electron part recovered from the Fock matrix: h_pq = f_pq - sum_i <pi||qi>."""
+        n, o = self.n, self.o
+        h = f - np.einsum("piqi->pq", g[:, :o, :, :o])
+        out = np.zeros_like(psi)
+        aq = [self.a[q] @ psi for q in range(n)]
+        for p in range(n):
+            acc = np.zeros_like(psi)
+            for q in range(n):
+                acc += h[p, q] * aq[q]
+            out += self.ad[p] @ acc
+        w = np.zeros((n, n, psi.size), dtype=np.complex128)
+        for r in range(n):
+            for s in range(n):
+                w[r, s] = self.a[s] @ aq[r]              # a_s a_r psi
+        u = np.einsum("pqrs,rsx->pqx", g, w)
+        for p in range(n):
+            for q in range(n):
+                out += 0.25 * (self.ad[p] @ (self.ad[q] @ u[p, q]))
+        return out
+
+    def apply_T(self, t1, t2, psi, t3=None):
+        """T psi with T1 = sum t_i^a a+_a a_i, T2 = 1/4 sum t_ij^ab a+_a a+_b a_j a_i (PAPER Eq. 2).
+        t1[a,i], t2[a,b,i,j] with a,b counted from the first virtual."""
+        o, v = self.o, self.v
+        out = np.zeros_like(psi)
+        if t1 is not None:
+            for a in range(v):
+                for i in range(o):
+                    out += t1[a, i] * (self.ad[o + a] @ (self.a[i] @ psi))
+        if t2 is not None:
+            for i in range(o):
+                ai = self.a[i] @ psi
+                for j in range(o):
+                    aji = self.a[j] @ ai
+                    for a in range(v):
+                        for b in range(v):
+                            if t2[a, b, i, j] != 0:
+                                out += 0.25 * t2[a, b, i, j] * (self.ad[o + a] @ (self.ad[o + b] @ aji))
+        return out
+
+    def exp_T(self, t1, t2, psi, sign=1.0):
+        """exp(sign*T) psi by the terminating series (T is nilpotent on a finite Fock space)."""
+        out = psi.copy()
+        term = psi.copy()
+        for k in range(1, self.n + 2):
+            term = sign * self.apply_T(t1, t2, term) / k
+            if not np.any(term):
+                break
+            out = out + term
+        return out
+
+    def hbar_phi0(self, f, g, t1, t2):
+        """exp(-T) H exp(T) |Phi0>."""
+        return self.exp_T(t1, t2, self.apply_H(f, g, self.exp_T(t1, t2, self.phi0)), sign=-1.0)
+
+    def project_doubles(self, psi):
+        """R[a,b,i,j] = <Phi0| (a+_a a+_b a_j a_i)^dagger |psi>."""
+        o, v = self.o, self.v
+        R = np.zeros((v, v, o, o), dtype=np.complex128)
+        for a, b, i, j in itertools.product(range(v), range(v), range(o), range(o)):
+            ket = self.ad[o + a] @ (self.ad[o + b] @ (self.a[j] @ (self.a[i] @ self.phi0)))
+            R[a, b, i, j] = np.vdot(ket, psi)
+        return R
+
+    def project_singles(self, psi):
+        o, v = self.o, self.v
+        R = np.zeros((v, o), dtype=np.complex128)
+        for a, i in itertools.product(range(v), range(o)):
+            R[a, i] = np.vdot(self.ad[o + a] @ (self.a[i] @ self.phi0), psi)
+        return R
+
+    def project_triples(self, psi):
+        """R3[a,b,c,i,j,k] = <Phi0| (a+_a a+_b a+_c a_k a_j a_i)^dagger |psi>   (tau of PAPER Eq. 2)."""
+        o, v = self.o, self.v
+        R = np.zeros((v, v, v, o, o, o), dtype=np.complex128)
+        for a, b, c, i, j, k in itertools.product(range(v), range(v), range(v), range(o), range(o), range(o)):
+            ket = self.a[k] @ (self.a[j] @ (self.a[i] @ self.phi0))
+            ket = self.ad[o + a] @ (self.ad[o + b] @ (self.ad[o + c] @ ket))
+            R[a, b, c, i, j, k] = np.vdot(ket, psi)
+        return R
+
+
+def fock_space_residuals(o, v, f, g, t2, t1=None):
+    """(E_corr, R1, R2) from PAPER Eq. (3): <Phi0|Hbar|Phi0> - <Phi0|H|Phi0> and <Phi_l|Hbar|Phi0>."""
+    fs = FockSpace(o, v)
+    psi = fs.hbar_phi0(f, g, t1, t2)
+    e_ref = np.vdot(fs.phi0, fs.apply_H(f, g, fs.phi0))
+    e = np.vdot(fs.phi0, psi) - e_ref
+    return e, fs.project_singles(psi), fs.project_doubles(psi)
+
+
+# ------------------------------------------------------------------------------------------
+# integral blocks
+# ------------------------------------------------------------------------------------------
+def blocks(o, f, g):
+    """Slices of f and <pq||rs> in bra-ket order, Fortran-contiguous copies."""
+    O, V = slice(0, o), slice(o, None)
+    F = lambda x: np.asfortranarray(x)
+    return {
+        "foo": F(f[O, O]), "fvv": F(f[V, V]), "fov": F(f[O, V]), "fvo": F(f[V, O]),
+        "vvoo": F(g[V, V, O, O]), "oovv": F(g[O, O, V, V]), "oooo": F(g[O, O, O, O]),
+        "vvvv": F(g[V, V, V, V]), "ovvo": F(g[O, V, V, O]),
+    }
+
+
+# ------------------------------------------------------------------------------------------
+# tier 1a: un-factorised CCD, 10 amplitude terms + energy
+# ------------------------------------------------------------------------------------------
+def _P(X, ax1, ax2):
+    """P(pq) X = X - X(p<->q)."""
+    return X - np.swapaxes(X, ax1, ax2)
+
+
+def ccd_residual_unfactorised(o, f, g, t):
+    """R[a,b,i,j] and E_corr;  t[a,b,i,j] = t_ij^ab.
+
+    R_ij^ab = <ab||ij> + P(ab) f_bc t_ij^ac - P(ij) f_kj t_ik^ab + 1/2 <kl||ij> t_kl^ab
+            + 1/2 <ab||cd> t_ij^cd + P(ij)P(ab) <kb||cj> t_ik^ac + 1/4 <kl||cd> t_ij^cd t_kl^ab
+            + P(ij) <kl||cd> t_ik^ac t_jl^bd - 1/2 P(ij) <kl||cd> t_ik^dc t_lj^ab
+            - 1/2 P(ab) <kl||cd> t_lk^ac t_ij^db ;       E = 1/4 <ij||ab> t_ij^ab
+    """
+    B = blocks(o, f, g)
+    es = np.einsum
+    terms = [
+        B["vvoo"].copy(),
+        _P(es("bc,acij->abij", B["fvv"], t), 0, 1),
+        -_P(es("kj,abik->abij", B["foo"], t), 2, 3),
+        0.5 * es("klij,abkl->abij", B["oooo"], t),
+        0.5 * es("abcd,cdij->abij", B["vvvv"], t),
+        _P(_P(es("kbcj,acik->abij", B["ovvo"], t), 2, 3), 0, 1),
+        0.25 * es("klcd,cdij,abkl->abij", B["oovv"], t, t),
+        _P(es("klcd,acik,bdjl->abij", B["oovv"], t, t), 2, 3),
+        -0.5 * _P(es("klcd,dcik,ablj->abij", B["oovv"], t, t), 2, 3),
+        -0.5 * _P(es("klcd,aclk,dbij->abij", B["oovv"], t, t), 0, 1),
+    ]
+    e_terms = [0.25 * es("ijab,abij->", B["oovv"], t)]
+    return sum(terms), sum(e_terms), len(terms), len(e_terms)
+
+
+# ------------------------------------------------------------------------------------------
+# tier 1b: the factorised program of binary operations (config 2)
+# ------------------------------------------------------------------------------------------
+P_AB = ([[0, 1, 2, 3], [1, 0, 2, 3]], [1, -1])
+P_IJ = ([[0, 1, 2, 3], [0, 1, 3, 2]], [1, -1])
+P_IJ_AB = ([[0, 1, 2, 3], [1, 0, 2, 3], [0, 1, 3, 2], [1, 0, 3, 2]], [1, -1, -1, 1])
+
+
+def ccd_residual_program(B, T, long_double=True):
+    """The CCD residual as binary contractions + permute-sums, each one oracle call.
+
+    B: dict of blocks (see `blocks`), T[a,b,i,j].  Returns (R, list of (name, snorm-free info)).
+    Every line is D (+)= alpha * L * R or D += sum_t c_t X[pi_t].
+    """
+    v, o = T.shape[0], T.shape[2]
+    z = lambda *s: np.zeros(s, dtype=np.complex128, order="F")
+    con = lambda e, D, L, R, a=1.0: _o.contract(e, D, L, R, a, long_double=long_double, want_snorm=False)[0]
+
+    def acc(R, X, PS, s):
+        return _o.permsum(R, X, PS[0], [s * c for c in PS[1]], 1.0)
+
+    R = np.asfortranarray(B["vvoo"]).copy(order="F")                       # driver <ab||ij>
+    X = con("X(a,b,i,j)=T(a,c,i,j)*f(b,c)", z(v, v, o, o), T, B["fvv"])
+    R = acc(R, X, P_AB, +1.0)                                               # + P(ab) f_bc t_ij^ac
+    X = con("X(a,b,i,j)=T(a,b,i,k)*f(k,j)", z(v, v, o, o), T, B["foo"])
+    R = acc(R, X, P_IJ, -1.0)                                               # - P(ij) f_kj t_ik^ab
+    I1 = con("I1(k,l,i,j)+=W(k,l,c,d)*T(c,d,i,j)", B["oooo"], B["oovv"], T, 0.5)
+    R = con("R(a,b,i,j)+=T(a,b,k,l)*I1(k,l,i,j)", R, T, I1, 0.5)           # hh ladder + 1/4 quadratic
+    R = con("R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)", R, B["vvvv"], T, 0.5)     # pp ladder
+    I2 = con("I2(k,b,c,j)+=W(k,l,c,d)*T(b,d,j,l)", B["ovvo"], B["oovv"], T, 0.5)
+    X = con("X(a,b,i,j)=T(a,c,i,k)*I2(k,b,c,j)", z(v, v, o, o), T, I2)
+    R = acc(R, X, P_IJ_AB, +1.0)                                            # ring + quadratic ring
+    I3 = con("I3(l,i)=W(k,l,c,d)*T(d,c,i,k)", z(o, o), B["oovv"], T)
+    X = con("X(a,b,i,j)=T(a,b,l,j)*I3(l,i)", z(v, v, o, o), T, I3)
+    R = acc(R, X, P_IJ, -0.5)
+    I4 = con("I4(a,d)=W(k,l,c,d)*T(a,c,l,k)", z(v, v), B["oovv"], T)
+    X = con("X(a,b,i,j)=I4(a,d)*T(d,b,i,j)", z(v, v, o, o), I4, T)
+    R = acc(R, X, P_AB, -0.5)
+    return R
+
+
+# ------------------------------------------------------------------------------------------
+# config 4: CCSDT piece
+# ------------------------------------------------------------------------------------------
+def _swap(X, p, q):
+    return np.swapaxes(X, p, q)
+
+
+def t3_term_unfactorised(W, T2):
+    """P(k/ij) P(a/bc) sum_d W(b,c,d,k) T2(a,d,i,j);  P(a/bc)F = F - F(a<->b) - F(a<->c),
+    P(k/ij)F = F - F(k<->i) - F(k<->j).   W(b,c,d,k) = <bc||dk>, T2(a,d,i,j) = t_ij^ad."""
+    X = np.einsum("bcdk,adij->abcijk", W, T2)
+    Y = X - _swap(X, 0, 1) - _swap(X, 0, 2)
+    return X, Y - _swap(Y, 5, 3) - _swap(Y, 5, 4)
+
+
+def p9_terms():
+    """The 9 signed index maps of P(k/ij)P(a/bc) in the permsum convention
+    (term: X position m is indexed by D's index number s[m])."""
+    abc = [((0, 1, 2), 1.0), ((1, 0, 2), -1.0), ((2, 1, 0), -1.0)]
+    ijk = [((3, 4, 5), 1.0), ((5, 4, 3), -1.0), ((3, 5, 4), -1.0)]
+    perms, coefs = [], []
+    for (pa, sa) in abc:
+        for (pi, si) in ijk:
+            perms.append(list(pa) + list(pi))
+            coefs.append(sa * si)
+    return perms, coefs
+
+
+def full_antisymmetriser_terms():
+    """All 36 signed (a,b,c) x (i,j,k) permutations."""
+    def sign(p):
+        s, p = 1, list(p)
+        for i in range(len(p)):
+            while p[i] != i:
+                j = p[i]
+                p[i], p[j] = p[j], p[i]
+                s = -s
+        return s
+    perms, coefs = [], []
+    for pa in itertools.permutations(range(3)):
+        for pi in itertools.permutations(range(3)):
+            perms.append(list(pa) + [3 + x for x in pi])
+            coefs.append(float(sign(pa) * sign(pi)))
+    return perms, coefs
+
+
+def t3_term_program(W, T2, R3, long_double=True):
+    """config 4 as library calls: X = W*T2 (one contraction), R3 += P(k/ij)P(a/bc) X (one permute-sum)."""
+    v, o = T2.shape[0], T2.shape[2]
+    X0 = np.zeros((v, v, v, o, o, o), dtype=np.complex128, order="F")
+    X, _ = _o.contract("X(a,b,c,i,j,k)=W(b,c,d,k)*T(a,d,i,j)", X0, W, T2, 1.0,
+                       long_double=long_double, want_snorm=False)
+    perms, coefs = p9_terms()
+    return X, _o.permsum(R3, X, perms, coefs, 1.0)

@@ -1,0 +1,87 @@
+"""Pins for oracle/cc.py.  Tier 0 evaluates PAPER Eqs. (2)-(4) literally on
+the Fock space; the spin-orbital CCD equations (tier 1a) and the factorised binary program (tier 1b,
+config 2) must reproduce it for complex, non-diagonal, Hermitian-consistent inputs."""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import cc
+
+
+def rand_inputs(o, v, seed):
+    rng = np.random.default_rng(seed)
+    n = o + v
+    c = lambda *s: rng.standard_normal(s) + 1j * rng.standard_normal(s)
+    A = c(n, n, n, n)
+    A = A - A.transpose(1, 0, 2, 3)
+    A = A - A.transpose(0, 1, 3, 2)
+    g = 0.5 * (A + A.transpose(2, 3, 0, 1).conj())
+    f = c(n, n)
+    f = f + f.conj().T                         # general (non-diagonal) Hermitian Fock matrix
+    t = c(v, v, o, o)
+    t = t - t.transpose(1, 0, 2, 3)
+    t = t - t.transpose(0, 1, 3, 2)
+    return f, g, t
+
+
+def test_jordan_wigner_anticommutators():
+    a = cc.jordan_wigner(4)
+    for p in range(4):
+        for q in range(4):
+            assert np.array_equal(a[p] @ a[q].T + a[q].T @ a[p], np.eye(16) * (p == q))
+            assert not np.any(a[p] @ a[q] + a[q] @ a[p])
+
+
+@pytest.mark.parametrize("o,v", [(2, 3), (3, 3), (2, 4)])
+def test_ccd_tiers_agree_with_fock_space(o, v):
+    f, g, t = rand_inputs(o, v, 100 * o + v)
+    e0, _, r0 = cc.fock_space_residuals(o, v, f, g, t)
+    r1a, e1a, n_amp, n_en = cc.ccd_residual_unfactorised(o, f, g, t)
+    assert n_amp + n_en == 11                                   # PAPER Table I: CCD = 11 diagrams
+    scale = np.abs(r0).max()
+    assert np.abs(r1a - r0).max() <= 1e-13 * scale
+    assert abs(e1a - e0) <= 1e-13 * abs(e0)
+    r1b = cc.ccd_residual_program(cc.blocks(o, f, g), np.asfortranarray(t))
+    assert np.abs(r1b - r1a).max() <= 1e-13 * scale
+    # residual antisymmetry R(a,b,i,j) = -R(b,a,i,j) = -R(a,b,j,i)
+    assert np.abs(r1b + r1b.transpose(1, 0, 2, 3)).max() <= 1e-13 * scale
+    assert np.abs(r1b + r1b.transpose(0, 1, 3, 2)).max() <= 1e-13 * scale
+
+
+def test_mp2_guess_cancels_driver_and_fock_terms_and_energy_closed_form():
+    o, v = 3, 4
+    _, g, _ = rand_inputs(o, v, 9)
+    rng = np.random.default_rng(10)
+    eo, ev = -2 + 1.5 * rng.random(o), 0.5 + 2.5 * rng.random(v)
+    f = np.diag(np.concatenate([eo, ev])).astype(np.complex128)
+    den = eo[None, None, :, None] + eo[None, None, None, :] - ev[:, None, None, None] - ev[None, :, None, None]
+    vvoo = g[o:, o:, :o, :o]
+    t = vvoo / den
+    # linear-in-f part of the residual + driver vanishes:  <ab||ij> + (e_a+e_b-e_i-e_j) t = 0
+    gz = np.zeros_like(g)
+    gz[o:, o:, :o, :o] = vvoo
+    r, e, _, _ = cc.ccd_residual_unfactorised(o, f, gz, t)
+    assert np.abs(r).max() <= 1e-14 * np.abs(vvoo).max()
+    # MP2 energy: 1/4 sum <ij||ab> t = 1/4 sum |<ab||ij>|^2 / den : real and negative
+    _, e, _, _ = cc.ccd_residual_unfactorised(o, f, g, t)
+    closed = 0.25 * np.sum(np.abs(vvoo) ** 2 / den)
+    assert abs(e - closed) <= 1e-13 * abs(closed) and closed < 0 and abs(e.imag) <= 1e-14 * abs(closed)
+
+
+def test_t3_term_against_fock_space_triples_projection():
+    """<Phi_ijk^abc| [H, T2] |Phi0> = P(k/ij)P(a/bc) sum_d <bc||dk> t_ij^ad - P(i/jk)P(c/ab) sum_l <lc||jk> t_il^ab."""
+    o = v = 3
+    f, g, t = rand_inputs(o, v, 7)
+    fs = cc.FockSpace(o, v)
+    psi = fs.apply_H(f, g, fs.apply_T(None, t, fs.phi0)) - fs.apply_T(None, t, fs.apply_H(f, g, fs.phi0))
+    R3 = fs.project_triples(psi)
+    W = g[o:, o:, o:, :o]
+    X, Y = cc.t3_term_unfactorised(W, t)
+    Z = np.einsum("lcjk,abil->abcijk", g[:o, o:, :o, :o], t)
+    Z = Z - np.swapaxes(Z, 2, 0) - np.swapaxes(Z, 2, 1)
+    Z = Z - np.swapaxes(Z, 3, 4) - np.swapaxes(Z, 3, 5)
+    assert np.abs(R3 - (Y - Z)).max() <= 1e-13 * np.abs(R3).max()
+    # the library-call form (one contraction + one 9-term permute-sum) reproduces the particle part
+    Xp, R3p = cc.t3_term_program(np.asfortranarray(W), np.asfortranarray(t), np.zeros_like(X))
+    assert np.abs(Xp - X).max() <= 1e-13 * np.abs(X).max()
+    assert np.abs(R3p - Y).max() <= 1e-13 * np.abs(Y).max()
