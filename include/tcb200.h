@@ -1,0 +1,150 @@
+/*
+ * tcb200.h -- C ABI of the B200 tensor-contraction backend (libtcb200.so).
+ *
+ * What this boundary is: the calls a tenpi-generated coupled-cluster driver issues to its tensor
+ * library: create / destroy tensors, contract two tensors into a third with a scalar
+ * factor, add, scale, and a barrier.  "Contraction ... includes a list of tensors, a scalar factor and
+ * optionally permutation operators and an output tensor"; only two tensors are
+ * contracted per instruction.  How a contraction is evaluated is the library's business;
+ * the reference scheme is TTGT: bring the operands to matrix form, GEMM, bring the
+ * result to the output's index order.
+ *
+ * Conventions (readings #1, #7, #8, #11, #12)
+ *   - element: complex128 = interleaved (re, im) IEEE doubles, 16 bytes, 16-byte aligned.
+ *   - layout: dense, generalised column-major: in T(a,b,i,j) the FIRST listed index has unit stride
+ *     ("unit-stride index"; tenpi emits Fortran).  offset = sum_k idx_k * prod_{m<k} ext_m.
+ *   - rank 0..6, every extent >= 1.  All tensor data lives in DEVICE memory.
+ *   - expression grammar (white space ignored):
+ *         name '(' [label {',' label}] ')' ('+=' | '=') name '(' ... ')' [ '*' name '(' ... ')' ]
+ *     label = [A-Za-z][A-Za-z0-9_]*  (tenpi prints a,b,i,j or p1,p2,h1,h2 -- PAPER.md:232);
+ *     tensor names are ignored, operands bind by position (D, L, R).  '+=' accumulates into D,
+ *     '=' overwrites D.
+ *   - a valid contraction: every label occurs exactly twice over D, L, R and at most once per tensor
+ *     (no batch/Hadamard index, no trace, no broadcast -> TCB_EUNSUPPORTED).  K = 1 (outer product)
+ *     and fully contracted R (N = 1) are valid.
+ *   - execution: every call validates its arguments, then enqueues work on the context's stream and
+ *     returns; calls execute in issue order (the paper's barrier after each operation, PAPER.md:400,
+ *     becomes stream order).  tcb_sync and tcb_tensor_download block.  On any error return nothing has
+ *     been enqueued and D is untouched.
+ *   - ownership: handles are created and destroyed by the library.  tcb_tensor_wrap borrows caller
+ *     memory and never frees it.  D must not overlap L or R (TCB_EALIAS).
+ *   - no CPU fallback exists: without a CUDA device every compute call returns TCB_ECUDA.
+ *   - not thread-safe per context.
+ *
+ * All functions return 0 (TCB_OK) or a negative tcb_status.
+ */
+#ifndef TCB200_H
+#define TCB200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TCB_MAX_RANK 6
+
+typedef enum {
+    TCB_OK = 0,
+    TCB_EINVAL_EXPR = -1,   /* expression does not parse, or operand count / op does not fit the call */
+    TCB_ESHAPE = -2,        /* ranks or extents of the handles disagree with the expression */
+    TCB_ERANK = -3,         /* rank > TCB_MAX_RANK, or extent < 1 */
+    TCB_EALIAS = -4,        /* D overlaps L or R */
+    TCB_ENOMEM = -5,        /* device allocation or workspace exhausted */
+    TCB_ECUDA = -6,         /* a CUDA call failed (sticky per context); text via tcb_last_error */
+    TCB_EUNSUPPORTED = -7,  /* batch / trace / broadcast index, conjugation, ... */
+    TCB_EINVAL = -8         /* NULL handle, bad option, bad permutation table, ... */
+} tcb_status;
+
+typedef struct tcb_ctx tcb_ctx;       /* device, stream, workspace pool, plan cache */
+typedef struct tcb_tensor tcb_tensor; /* rank, extents, device pointer, owns-memory flag */
+typedef struct { double re, im; } tcb_c128;
+
+/* ---- context ------------------------------------------------------------------------------------ */
+
+/* device: CUDA ordinal.  cuda_stream: a cudaStream_t to enqueue on, or NULL for a stream the context
+ * creates and owns.  workspace_bytes: initial size of the workspace pool used for permuted operands and
+ * split-K partials (0 = grow on demand; growth synchronises the stream). */
+int tcb_ctx_create(tcb_ctx **ctx, int device, void *cuda_stream, size_t workspace_bytes);
+int tcb_ctx_destroy(tcb_ctx *ctx);
+/* keys: "splitk" = "auto" | "off" | <integer number of splits>;  "epilogue" = "auto" | "fused" | "twopass";
+ *       "permute_operands" = "auto" | "always"  (A/B testing of plans);  unknown key -> TCB_EINVAL. */
+int tcb_ctx_set_option(tcb_ctx *ctx, const char *key, const char *value);
+/* Blocks until everything enqueued so far has finished (the paper's barrier). */
+int tcb_sync(tcb_ctx *ctx);
+/* Text of the last error recorded on this context (valid until the next call on it). */
+const char *tcb_last_error(const tcb_ctx *ctx);
+const char *tcb_strerror(int code);
+/* Number of kernels this context has launched so far (all of them this library's own). */
+int64_t tcb_launch_count(const tcb_ctx *ctx);
+
+/* ---- tensors ------------------------------------------------------------------------------------ */
+
+/* Library-owned, zero-filled device tensor.  extents[rank], copied. */
+int tcb_tensor_create(tcb_ctx *ctx, tcb_tensor **t, int rank, const int64_t *extents);
+/* Borrow caller-owned device memory (e.g. torch storage), 16-byte aligned, prod(extents)*16 bytes. */
+int tcb_tensor_wrap(tcb_ctx *ctx, tcb_tensor **t, int rank, const int64_t *extents, void *device_ptr);
+/* Stream-ordered free of library-owned memory; borrowed memory is left alone.  NULL is accepted. */
+int tcb_tensor_destroy(tcb_tensor *t);
+/* Any of rank / extents / device_ptr may be NULL. */
+int tcb_tensor_info(const tcb_tensor *t, int *rank, int64_t extents[TCB_MAX_RANK], void **device_ptr);
+/* HOST <-> device copies of the whole tensor in the layout above.  upload is stream-ordered (the host
+ * buffer must stay valid until tcb_sync unless it is pageable); download blocks until the data is there. */
+int tcb_tensor_upload(tcb_ctx *ctx, tcb_tensor *t, const tcb_c128 *host);
+int tcb_tensor_download(tcb_ctx *ctx, const tcb_tensor *t, tcb_c128 *host);
+/* D[...] = value */
+int tcb_tensor_fill(tcb_ctx *ctx, tcb_tensor *t, tcb_c128 value);
+
+/* ---- the hot path ------------------------------------------------------------------------------- */
+
+/* S1-S5: D(d..) (+)= alpha * L(l..) * R(r..), e.g.
+ *     "R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)".
+ * The planner picks the index grouping (M, N, K), which operands to permute into matrix form (workspace),
+ * the GEMM variant, and scatters alpha*C into D's own index order in the GEMM epilogue. */
+int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor *L, const tcb_tensor *R,
+                 tcb_c128 alpha);
+/* Permuted add, "D(a,b,i,j)+=L(b,a,i,j)":  D = D + alpha * permuted L  ('=' : D = alpha * permuted L). */
+int tcb_add(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor *L, tcb_c128 alpha);
+/* D *= alpha */
+int tcb_scale(tcb_ctx *ctx, tcb_tensor *D, tcb_c128 alpha);
+/* S3, tensor transposition: "D(i,j,a,b)=L(a,b,i,j)", pure data movement, bit-exact. */
+int tcb_permute(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor *L);
+/* S6, fused permute-sum (the generator's unrolled permutation operators):
+ *     D[i] = beta * D[i] + sum_{t<nterms} coefs[t] * X[i_{s_t(0)}, i_{s_t(1)}, ...],   terms added in order t;
+ * perms[t*rank + k] = s_t(k): position k of X is indexed by D's index number s_t(k), so
+ * "D(a,b,i,j) += -1 * X(b,a,i,j)" is s = (1,0,2,3), c = -1.  beta = 0 does not read D.
+ * X must not overlap D.  Each product and each sum is rounded on its own (no FMA contraction). */
+int tcb_permsum(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, int nterms, const int32_t *perms,
+                const tcb_c128 *coefs, tcb_c128 beta);
+/* Sugar over tcb_permsum: spec = "P(a/bc)P(k/ij):D(a,b,c,i,j,k)+=X(a,b,c,i,j,k)".  Each P(x/yz..) stands
+ * for 1 - (x<->y) - (x<->z) - ...; P(xy) for 1 - (x<->y); the product is expanded into signed terms
+ * (first operator outermost).  D = D + alpha * sum of terms. */
+int tcb_antisymmetrize(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *X, tcb_c128 alpha);
+/* JSON description of the plan tcb_contract would use: M, N, K, which operands are permuted, GEMM variant,
+ * split-K, estimated flops and bytes.  Truncated to buflen-1 characters. */
+int tcb_plan_describe(tcb_ctx *ctx, const char *expr, const tcb_tensor *D, const tcb_tensor *L,
+                      const tcb_tensor *R, char *buf, size_t buflen);
+
+/* Host-only planning (no device, no context): the same planner on bare shapes.  options: NULL or
+ * "key=value;key=value" with the keys of tcb_ctx_set_option.  offM / offN (may be NULL) receive the epilogue
+ * offset tables: C[m,n] of the matricised product lands at D[offM[m] + offN[n]]; cap_m / cap_n are the
+ * capacities of the two arrays (TCB_EINVAL if too small). */
+int tcb_plan_describe_host(const char *expr, int rank_d, const int64_t *ext_d, int rank_l, const int64_t *ext_l,
+                           int rank_r, const int64_t *ext_r, const char *options, char *buf, size_t buflen,
+                           int64_t *offM, size_t cap_m, int64_t *offN, size_t cap_n);
+
+/* ---- measurement helpers (not part of the hot path) ----------------------------------------------- */
+
+/* Register-resident mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4) loop on every SM for about `milliseconds`;
+ * returns achieved TFLOP/s (512 flop per warp instruction).  The roofline denominator of the contraction. */
+int tcb_measure_fp64_tensor_peak(tcb_ctx *ctx, double milliseconds, double *tflops);
+/* Milliseconds between two points of the context's stream: tcb_timer_start / tcb_timer_stop bracket the
+ * calls in between with CUDA events on that stream; stop blocks and returns the elapsed time. */
+int tcb_timer_start(tcb_ctx *ctx);
+int tcb_timer_stop(tcb_ctx *ctx, double *milliseconds);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TCB200_H */

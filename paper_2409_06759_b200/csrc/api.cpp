@@ -1,0 +1,708 @@
+// api.cpp -- the C ABI of include/tcb200.h: contexts, tensors, argument validation, plan cache, workspace pool,
+// and the sequencing of kernels for each call.  Everything a call computes runs in this library's own sm_100a
+// kernels; there is no CPU fallback (without a device every compute call returns TCB_ECUDA).
+#include "../../include/tcb200.h"
+
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <memory>
+#include <string>
+#include <vector>
+
+#include "kernels.h"
+#include "parse.h"
+#include "plan.h"
+
+using namespace tcb;
+
+struct CachedPlan {
+    ContractPlan plan;
+    int64_t *d_tables = nullptr;   // device: offM[M] followed by offN[N]
+};
+
+struct tcb_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    bool owns_stream = false;
+    void *ws = nullptr;
+    size_t ws_bytes = 0;
+    std::string last_error;
+    bool sticky_cuda = false;
+    int64_t launches = 0;
+    PlanOptions opt;
+    std::map<std::string, std::unique_ptr<CachedPlan>> plans;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    int64_t live_tensors = 0;
+};
+
+struct tcb_tensor {
+    tcb_ctx *ctx = nullptr;
+    Shape shape;
+    void *ptr = nullptr;
+    bool owns = false;
+    int64_t elems() const { return shape.volume(); }
+};
+
+namespace {
+
+int set_error(tcb_ctx *ctx, int code, const std::string &msg)
+{
+    if (ctx) ctx->last_error = msg;
+    return code;
+}
+
+int cuda_fail(tcb_ctx *ctx, cudaError_t e, const char *where)
+{
+    if (ctx) {
+        ctx->sticky_cuda = true;
+        ctx->last_error = std::string(where) + ": " + cudaGetErrorString(e);
+    }
+    return TCB_ECUDA;
+}
+
+#define TCB_CUDA(ctx, call)                                        \
+    do {                                                           \
+        cudaError_t e__ = (call);                                  \
+        if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call); \
+    } while (0)
+
+int enter(tcb_ctx *ctx)
+{
+    if (!ctx) return TCB_EINVAL;
+    if (ctx->sticky_cuda) return TCB_ECUDA;
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaSetDevice");
+    return TCB_OK;
+}
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+int workspace(tcb_ctx *ctx, size_t bytes, void **out)
+{
+    if (bytes > ctx->ws_bytes) {
+        TCB_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        if (ctx->ws) cudaFree(ctx->ws);
+        ctx->ws = nullptr;
+        ctx->ws_bytes = 0;
+        void *p = nullptr;
+        const size_t want = align_up(bytes, (size_t)1 << 21);
+        cudaError_t e = cudaMalloc(&p, want);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            return set_error(ctx, TCB_ENOMEM, "workspace allocation of " + std::to_string(want) + " bytes failed");
+        }
+        ctx->ws = p;
+        ctx->ws_bytes = want;
+    }
+    *out = ctx->ws;
+    return TCB_OK;
+}
+
+bool overlaps(const tcb_tensor *a, const tcb_tensor *b)
+{
+    const char *a0 = (const char *)a->ptr, *a1 = a0 + a->elems() * 16;
+    const char *b0 = (const char *)b->ptr, *b1 = b0 + b->elems() * 16;
+    return a0 < b1 && b0 < a1;
+}
+
+std::string shape_key(const Shape &s)
+{
+    std::string k = "[";
+    for (int i = 0; i < s.rank; ++i) k += std::to_string(s.ext[i]) + ",";
+    return k + "]";
+}
+
+void strides_of(const Shape &s, int64_t *st)
+{
+    int64_t x = 1;
+    for (int k = 0; k < s.rank; ++k) { st[k] = x; x *= s.ext[k]; }
+}
+
+int find_label(const std::vector<std::string> &v, const std::string &n)
+{
+    for (size_t i = 0; i < v.size(); ++i) if (v[i] == n) return (int)i;
+    return -1;
+}
+
+bool has_dup(const std::vector<std::string> &v)
+{
+    for (size_t a = 0; a < v.size(); ++a)
+        for (size_t b = a + 1; b < v.size(); ++b)
+            if (v[a] == v[b]) return true;
+    return false;
+}
+
+PermuteDesc make_desc(const PermuteShape &s, const void *in, void *out, PermuteOp op, double ar, double ai)
+{
+    PermuteDesc d;
+    d.rank = s.rank;
+    for (int k = 0; k < kMaxRank; ++k) {
+        d.extent[k] = k < s.rank ? s.extent[k] : 1;
+        d.istride[k] = k < s.rank ? s.istride[k] : 0;
+        d.ostride[k] = k < s.rank ? s.ostride[k] : 0;
+    }
+    d.in = in; d.out = out; d.op = op; d.alpha_re = ar; d.alpha_im = ai;
+    return d;
+}
+
+int get_plan(tcb_ctx *ctx, const char *expr, const tcb_tensor *D, const tcb_tensor *L, const tcb_tensor *R,
+             CachedPlan **out)
+{
+    std::string key = std::string(expr) + "|" + shape_key(D->shape) + shape_key(L->shape) + shape_key(R->shape) +
+                      "|" + std::to_string(ctx->opt.splitk) + "," + std::to_string(ctx->opt.epilogue) + "," +
+                      (ctx->opt.permute_always ? "1" : "0");
+    auto it = ctx->plans.find(key);
+    if (it != ctx->plans.end()) { *out = it->second.get(); return TCB_OK; }
+    ParsedExpr e;
+    if (!parse_expression(expr, &e)) return set_error(ctx, TCB_EINVAL_EXPR, std::string("cannot parse: ") + expr);
+    std::unique_ptr<CachedPlan> cp(new CachedPlan());
+    std::string why;
+    int rc = plan_contraction(e, D->shape, L->shape, R->shape, ctx->opt, &cp->plan, &why);
+    if (rc != TCB_OK) return set_error(ctx, rc, why + ": " + expr);
+    const size_t n = cp->plan.offM.size() + cp->plan.offN.size();
+    TCB_CUDA(ctx, cudaMalloc((void **)&cp->d_tables, n * sizeof(int64_t)));
+    // the host vectors live as long as the cache entry, so the stream-ordered copies are safe
+    TCB_CUDA(ctx, cudaMemcpyAsync(cp->d_tables, cp->plan.offM.data(), cp->plan.offM.size() * sizeof(int64_t),
+                                  cudaMemcpyHostToDevice, ctx->stream));
+    TCB_CUDA(ctx, cudaMemcpyAsync(cp->d_tables + cp->plan.offM.size(), cp->plan.offN.data(),
+                                  cp->plan.offN.size() * sizeof(int64_t), cudaMemcpyHostToDevice, ctx->stream));
+    *out = cp.get();
+    ctx->plans[key] = std::move(cp);
+    return TCB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *tcb_strerror(int code)
+{
+    switch (code) {
+    case TCB_OK: return "ok";
+    case TCB_EINVAL_EXPR: return "invalid expression";
+    case TCB_ESHAPE: return "rank or extent mismatch";
+    case TCB_ERANK: return "rank above 6 or extent below 1";
+    case TCB_EALIAS: return "output overlaps an input";
+    case TCB_ENOMEM: return "out of device memory";
+    case TCB_ECUDA: return "CUDA error";
+    case TCB_EUNSUPPORTED: return "unsupported contraction form";
+    case TCB_EINVAL: return "invalid argument";
+    default: return "unknown error";
+    }
+}
+
+const char *tcb_last_error(const tcb_ctx *ctx) { return ctx ? ctx->last_error.c_str() : "null context"; }
+
+int64_t tcb_launch_count(const tcb_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int tcb_ctx_create(tcb_ctx **out, int device, void *cuda_stream, size_t workspace_bytes)
+{
+    if (!out) return TCB_EINVAL;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return TCB_ECUDA;                       // no device: this library has no other way to compute
+    }
+    if (cudaSetDevice(device) != cudaSuccess) return TCB_ECUDA;
+    std::unique_ptr<tcb_ctx> ctx(new tcb_ctx());
+    ctx->device = device;
+    if (cuda_stream) {
+        ctx->stream = (cudaStream_t)cuda_stream;
+    } else {
+        if (cudaStreamCreateWithFlags(&ctx->stream, cudaStreamNonBlocking) != cudaSuccess) return TCB_ECUDA;
+        ctx->owns_stream = true;
+    }
+    {   // tensors are created and destroyed every iteration by generated code: keep freed
+        // blocks in the stream-ordered pool instead of returning them to the driver at every sync
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, device) == cudaSuccess) {
+            unsigned long long keep = ~0ull;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+    }
+    if (cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess) return TCB_ECUDA;
+    if (workspace_bytes) {
+        void *p;
+        int rc = workspace(ctx.get(), workspace_bytes, &p);
+        if (rc != TCB_OK) return rc;
+    }
+    *out = ctx.release();
+    return TCB_OK;
+}
+
+int tcb_ctx_destroy(tcb_ctx *ctx)
+{
+    if (!ctx) return TCB_OK;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    for (auto &kv : ctx->plans)
+        if (kv.second->d_tables) cudaFree(kv.second->d_tables);
+    if (ctx->ws) cudaFree(ctx->ws);
+    if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+    if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    if (ctx->owns_stream) cudaStreamDestroy(ctx->stream);
+    delete ctx;
+    return TCB_OK;
+}
+
+static int apply_option(PlanOptions &opt, const std::string &k, const std::string &v, std::string *why);
+
+int tcb_ctx_set_option(tcb_ctx *ctx, const char *key, const char *value)
+{
+    if (!ctx || !key || !value) return TCB_EINVAL;
+    std::string why;
+    int rc = apply_option(ctx->opt, key, value, &why);
+    return rc ? set_error(ctx, rc, why) : TCB_OK;
+}
+
+int tcb_sync(tcb_ctx *ctx)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    TCB_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return TCB_OK;
+}
+
+// ---- tensors ---------------------------------------------------------------------------------------------
+
+static int make_tensor(tcb_ctx *ctx, tcb_tensor **out, int rank, const int64_t *extents, void *borrowed)
+{
+    if (!out) return TCB_EINVAL;
+    *out = nullptr;
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (rank < 0 || rank > TCB_MAX_RANK) return set_error(ctx, TCB_ERANK, "rank outside 0..6");
+    if (rank > 0 && !extents) return TCB_EINVAL;
+    std::unique_ptr<tcb_tensor> t(new tcb_tensor());
+    t->ctx = ctx;
+    t->shape.rank = rank;
+    for (int k = 0; k < rank; ++k) {
+        if (extents[k] < 1) return set_error(ctx, TCB_ERANK, "extent below 1");
+        t->shape.ext[k] = extents[k];
+    }
+    const size_t bytes = (size_t)t->shape.volume() * 16;
+    if (borrowed) {
+        if (((uintptr_t)borrowed & 15) != 0) return set_error(ctx, TCB_EINVAL, "device pointer not 16-byte aligned");
+        t->ptr = borrowed;
+        t->owns = false;
+    } else {
+        void *p = nullptr;
+        cudaError_t e = cudaMallocAsync(&p, bytes, ctx->stream);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            return set_error(ctx, TCB_ENOMEM, "tensor allocation of " + std::to_string(bytes) + " bytes failed");
+        }
+        t->ptr = p;
+        t->owns = true;
+        TCB_CUDA(ctx, cudaMemsetAsync(p, 0, bytes, ctx->stream));
+    }
+    ++ctx->live_tensors;
+    *out = t.release();
+    return TCB_OK;
+}
+
+int tcb_tensor_create(tcb_ctx *ctx, tcb_tensor **t, int rank, const int64_t *extents)
+{
+    return make_tensor(ctx, t, rank, extents, nullptr);
+}
+
+int tcb_tensor_wrap(tcb_ctx *ctx, tcb_tensor **t, int rank, const int64_t *extents, void *device_ptr)
+{
+    if (!device_ptr) return TCB_EINVAL;
+    return make_tensor(ctx, t, rank, extents, device_ptr);
+}
+
+int tcb_tensor_destroy(tcb_tensor *t)
+{
+    if (!t) return TCB_OK;
+    tcb_ctx *ctx = t->ctx;
+    if (t->owns && t->ptr) {
+        cudaSetDevice(ctx->device);
+        cudaFreeAsync(t->ptr, ctx->stream);      // stream-ordered: pending kernels still see the memory
+    }
+    --ctx->live_tensors;
+    delete t;
+    return TCB_OK;
+}
+
+int tcb_tensor_info(const tcb_tensor *t, int *rank, int64_t extents[TCB_MAX_RANK], void **device_ptr)
+{
+    if (!t) return TCB_EINVAL;
+    if (rank) *rank = t->shape.rank;
+    if (extents) for (int k = 0; k < t->shape.rank; ++k) extents[k] = t->shape.ext[k];
+    if (device_ptr) *device_ptr = t->ptr;
+    return TCB_OK;
+}
+
+int tcb_tensor_upload(tcb_ctx *ctx, tcb_tensor *t, const tcb_c128 *host)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!t || !host) return TCB_EINVAL;
+    TCB_CUDA(ctx, cudaMemcpyAsync(t->ptr, host, (size_t)t->elems() * 16, cudaMemcpyHostToDevice, ctx->stream));
+    return TCB_OK;
+}
+
+int tcb_tensor_download(tcb_ctx *ctx, const tcb_tensor *t, tcb_c128 *host)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!t || !host) return TCB_EINVAL;
+    TCB_CUDA(ctx, cudaMemcpyAsync(host, t->ptr, (size_t)t->elems() * 16, cudaMemcpyDeviceToHost, ctx->stream));
+    TCB_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return TCB_OK;
+}
+
+int tcb_tensor_fill(tcb_ctx *ctx, tcb_tensor *t, tcb_c128 value)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!t) return TCB_EINVAL;
+    TCB_CUDA(ctx, launch_fill(t->ptr, t->elems(), value.re, value.im, ctx->stream, &ctx->launches));
+    return TCB_OK;
+}
+
+// ---- hot path --------------------------------------------------------------------------------------------
+
+int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor *L, const tcb_tensor *R,
+                 tcb_c128 alpha)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!expr || !D || !L || !R) return set_error(ctx, TCB_EINVAL, "null argument");
+    if (overlaps(D, L) || overlaps(D, R)) return set_error(ctx, TCB_EALIAS, "D overlaps L or R");
+    CachedPlan *cp = nullptr;
+    rc = get_plan(ctx, expr, D, L, R, &cp);
+    if (rc) return rc;
+    const ContractPlan &P = cp->plan;
+    const tcb_tensor *TA = P.swapped ? R : L, *TB = P.swapped ? L : R;
+
+    const size_t bytesA = P.a.permuted ? align_up((size_t)P.a.elems * 16, 1024) : 0;
+    const size_t bytesB = P.b.permuted ? align_up((size_t)P.b.elems * 16, 1024) : 0;
+    const size_t bytesP = P.splits > 1 ? align_up((size_t)P.splits * P.M * P.N * 16, 1024) : 0;
+    char *ws = nullptr;
+    if (bytesA + bytesB + bytesP) {
+        void *p;
+        rc = workspace(ctx, bytesA + bytesB + bytesP, &p);
+        if (rc) return rc;
+        ws = (char *)p;
+    }
+    const void *Aptr = TA->ptr, *Bptr = TB->ptr;
+    if (P.a.permuted) {
+        PermuteDesc d = make_desc(P.a.perm, TA->ptr, ws, kPermCopy, 1.0, 0.0);
+        TCB_CUDA(ctx, launch_permute(d, ctx->stream, &ctx->launches));
+        Aptr = ws;
+    }
+    if (P.b.permuted) {
+        PermuteDesc d = make_desc(P.b.perm, TB->ptr, ws + bytesA, kPermCopy, 1.0, 0.0);
+        TCB_CUDA(ctx, launch_permute(d, ctx->stream, &ctx->launches));
+        Bptr = ws + bytesA;
+    }
+    GemmDesc g;
+    g.M = P.M; g.N = P.N; g.K = P.K;
+    g.A = Aptr; g.B = Bptr;
+    g.lda = P.a.ld; g.ldb = P.b.ld;
+    g.a_kmajor = P.a.kmajor; g.b_kmajor = P.b.kmajor;
+    g.D = D->ptr;
+    g.offM = cp->d_tables;
+    g.offN = cp->d_tables + P.offM.size();
+    g.alpha_re = alpha.re; g.alpha_im = alpha.im;
+    g.accumulate = P.accumulate;
+    g.splits = P.splits;
+    g.partial = bytesP ? ws + bytesA + bytesB : nullptr;
+    TCB_CUDA(ctx, launch_zgemm(g, ctx->stream, &ctx->launches));
+    return TCB_OK;
+}
+
+int tcb_plan_describe(tcb_ctx *ctx, const char *expr, const tcb_tensor *D, const tcb_tensor *L,
+                      const tcb_tensor *R, char *buf, size_t buflen)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!expr || !D || !L || !R || !buf || !buflen) return TCB_EINVAL;
+    CachedPlan *cp = nullptr;
+    rc = get_plan(ctx, expr, D, L, R, &cp);
+    if (rc) return rc;
+    const std::string s = cp->plan.describe();
+    std::snprintf(buf, buflen, "%s", s.c_str());
+    return TCB_OK;
+}
+
+static int apply_option(PlanOptions &opt, const std::string &k, const std::string &v, std::string *why)
+{
+    if (k == "splitk") {
+        if (v == "auto") opt.splitk = 0;
+        else if (v == "off") opt.splitk = 1;
+        else {
+            const int n = atoi(v.c_str());
+            if (n < 1) { *why = "splitk: expected auto, off or a positive integer"; return TCB_EINVAL; }
+            opt.splitk = n;
+        }
+        return TCB_OK;
+    }
+    if (k == "epilogue") {
+        if (v == "auto") opt.epilogue = 0;
+        else if (v == "fused") opt.epilogue = 1;
+        else if (v == "twopass") opt.epilogue = 2;
+        else { *why = "epilogue: expected auto, fused or twopass"; return TCB_EINVAL; }
+        return TCB_OK;
+    }
+    if (k == "permute_operands") {
+        if (v == "auto") opt.permute_always = false;
+        else if (v == "always") opt.permute_always = true;
+        else { *why = "permute_operands: expected auto or always"; return TCB_EINVAL; }
+        return TCB_OK;
+    }
+    *why = "unknown option " + k;
+    return TCB_EINVAL;
+}
+
+int tcb_plan_describe_host(const char *expr, int rank_d, const int64_t *ext_d, int rank_l, const int64_t *ext_l,
+                           int rank_r, const int64_t *ext_r, const char *options, char *buf, size_t buflen,
+                           int64_t *offM, size_t cap_m, int64_t *offN, size_t cap_n)
+{
+    if (!expr || !buf || !buflen) return TCB_EINVAL;
+    Shape sh[3];
+    const int ranks[3] = {rank_d, rank_l, rank_r};
+    const int64_t *exts[3] = {ext_d, ext_l, ext_r};
+    for (int t = 0; t < 3; ++t) {
+        if (ranks[t] < 0 || ranks[t] > TCB_MAX_RANK) return TCB_ERANK;
+        sh[t].rank = ranks[t];
+        for (int k = 0; k < ranks[t]; ++k) {
+            if (!exts[t] || exts[t][k] < 1) return TCB_ERANK;
+            sh[t].ext[k] = exts[t][k];
+        }
+    }
+    PlanOptions opt;
+    std::string why;
+    if (options) {
+        std::string o = options;
+        size_t pos = 0;
+        while (pos < o.size()) {
+            size_t end = o.find(';', pos);
+            if (end == std::string::npos) end = o.size();
+            const std::string kv = o.substr(pos, end - pos);
+            pos = end + 1;
+            if (kv.empty()) continue;
+            const size_t eq = kv.find('=');
+            if (eq == std::string::npos) return TCB_EINVAL;
+            int rc = apply_option(opt, kv.substr(0, eq), kv.substr(eq + 1), &why);
+            if (rc) { std::snprintf(buf, buflen, "%s", why.c_str()); return rc; }
+        }
+    }
+    ParsedExpr e;
+    if (!parse_expression(expr, &e)) { std::snprintf(buf, buflen, "cannot parse"); return TCB_EINVAL_EXPR; }
+    ContractPlan P;
+    int rc = plan_contraction(e, sh[0], sh[1], sh[2], opt, &P, &why);
+    if (rc) { std::snprintf(buf, buflen, "%s", why.c_str()); return rc; }
+    std::snprintf(buf, buflen, "%s", P.describe().c_str());
+    if (offM) {
+        if (cap_m < P.offM.size()) return TCB_EINVAL;
+        std::memcpy(offM, P.offM.data(), P.offM.size() * sizeof(int64_t));
+    }
+    if (offN) {
+        if (cap_n < P.offN.size()) return TCB_EINVAL;
+        std::memcpy(offN, P.offN.data(), P.offN.size() * sizeof(int64_t));
+    }
+    return TCB_OK;
+}
+
+// shared by tcb_add and tcb_permute
+static int permuted_op(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor *L, tcb_c128 alpha,
+                       bool pure_copy)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!expr || !D || !L) return set_error(ctx, TCB_EINVAL, "null argument");
+    ParsedExpr e;
+    if (!parse_expression(expr, &e) || e.has_r)
+        return set_error(ctx, TCB_EINVAL_EXPR, std::string("cannot parse as D(..)(+)=L(..): ") + expr);
+    if (pure_copy && e.accumulate) return set_error(ctx, TCB_EINVAL_EXPR, "tcb_permute takes '=', not '+='");
+    if ((int)e.d.size() != D->shape.rank || (int)e.l.size() != L->shape.rank || D->shape.rank != L->shape.rank)
+        return set_error(ctx, TCB_ESHAPE, "rank mismatch");
+    if (has_dup(e.d) || has_dup(e.l)) return set_error(ctx, TCB_EUNSUPPORTED, "label repeated inside one tensor");
+    int64_t sD[kMaxRank], sL[kMaxRank], ext[kMaxRank], is[kMaxRank], os[kMaxRank];
+    strides_of(D->shape, sD);
+    strides_of(L->shape, sL);
+    const int r = L->shape.rank;
+    for (int k = 0; k < r; ++k) {
+        const int pd = find_label(e.d, e.l[k]);
+        if (pd < 0) return set_error(ctx, TCB_EUNSUPPORTED, "label of L missing in D");
+        if (D->shape.ext[pd] != L->shape.ext[k]) return set_error(ctx, TCB_ESHAPE, "extent mismatch");
+        ext[k] = L->shape.ext[k]; is[k] = sL[k]; os[k] = sD[pd];
+    }
+    if (overlaps(D, L)) return set_error(ctx, TCB_EALIAS, "D overlaps L");
+    const PermuteShape ps = canonical_permutation(r, ext, is, os);
+    if (pure_copy) {
+        PermuteDesc d = make_desc(ps, L->ptr, D->ptr, kPermCopy, 1.0, 0.0);
+        TCB_CUDA(ctx, launch_permute(d, ctx->stream, &ctx->launches));
+    } else if (ps.identity) {
+        TCB_CUDA(ctx, launch_axpy(D->ptr, L->ptr, D->elems(), alpha.re, alpha.im, e.accumulate, ctx->stream,
+                                  &ctx->launches));
+    } else {
+        PermuteDesc d = make_desc(ps, L->ptr, D->ptr, e.accumulate ? kPermAccumulate : kPermScale, alpha.re, alpha.im);
+        TCB_CUDA(ctx, launch_permute(d, ctx->stream, &ctx->launches));
+    }
+    return TCB_OK;
+}
+
+int tcb_add(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor *L, tcb_c128 alpha)
+{
+    return permuted_op(ctx, expr, D, L, alpha, false);
+}
+
+int tcb_permute(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor *L)
+{
+    tcb_c128 one = {1.0, 0.0};
+    return permuted_op(ctx, expr, D, L, one, true);
+}
+
+int tcb_scale(tcb_ctx *ctx, tcb_tensor *D, tcb_c128 alpha)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!D) return TCB_EINVAL;
+    TCB_CUDA(ctx, launch_scale(D->ptr, D->elems(), alpha.re, alpha.im, ctx->stream, &ctx->launches));
+    return TCB_OK;
+}
+
+int tcb_permsum(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, int nterms, const int32_t *perms,
+                const tcb_c128 *coefs, tcb_c128 beta)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!D || !X || !perms || !coefs) return set_error(ctx, TCB_EINVAL, "null argument");
+    if (nterms < 1 || nterms > kMaxTerms) return set_error(ctx, TCB_EINVAL, "nterms outside 1..36");
+    const int r = D->shape.rank;
+    if (X->shape.rank != r) return set_error(ctx, TCB_ESHAPE, "rank mismatch");
+    int64_t sX[kMaxRank];
+    strides_of(X->shape, sX);
+    PermSumDesc d;
+    d.rank = r;
+    d.nterms = nterms;
+    for (int k = 0; k < kMaxRank; ++k) d.extent[k] = k < r ? D->shape.ext[k] : 1;
+    for (int t = 0; t < nterms; ++t) {
+        bool seen[kMaxRank] = {false, false, false, false, false, false};
+        for (int k = 0; k < kMaxRank; ++k) d.xstride[t][k] = 0;
+        for (int m = 0; m < r; ++m) {
+            const int s = perms[t * r + m];          // position m of X is indexed by D's index s
+            if (s < 0 || s >= r || seen[s]) return set_error(ctx, TCB_EINVAL, "perms is not a permutation table");
+            seen[s] = true;
+            if (X->shape.ext[m] != D->shape.ext[s]) return set_error(ctx, TCB_ESHAPE, "extent mismatch under a term");
+            d.xstride[t][s] = sX[m];
+        }
+        d.coef_re[t] = coefs[t].re;
+        d.coef_im[t] = coefs[t].im;
+    }
+    if (overlaps(D, X)) return set_error(ctx, TCB_EALIAS, "D overlaps X");
+    d.beta_re = beta.re; d.beta_im = beta.im;
+    d.X = X->ptr; d.D = D->ptr;
+    TCB_CUDA(ctx, launch_permsum(d, ctx->stream, &ctx->launches));
+    return TCB_OK;
+}
+
+int tcb_antisymmetrize(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *X, tcb_c128 alpha)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!spec || !D || !X) return set_error(ctx, TCB_EINVAL, "null argument");
+    std::vector<PermOperator> ops;
+    ParsedExpr e;
+    if (!parse_antisym_spec(spec, &ops, &e)) return set_error(ctx, TCB_EINVAL_EXPR, std::string("cannot parse: ") + spec);
+    const int r = D->shape.rank;
+    if ((int)e.d.size() != r || (int)e.l.size() != r || X->shape.rank != r)
+        return set_error(ctx, TCB_ESHAPE, "rank mismatch");
+    if (has_dup(e.d) || has_dup(e.l)) return set_error(ctx, TCB_EUNSUPPORTED, "label repeated inside one tensor");
+    // operators must act on disjoint label sets (they then commute; all CC operators do)
+    std::vector<std::string> used;
+    for (const PermOperator &op : ops) {
+        std::vector<std::string> mine = op.others;
+        mine.push_back(op.pivot);
+        for (const std::string &s : mine) {
+            if (find_label(e.d, s) < 0) return set_error(ctx, TCB_EINVAL_EXPR, "operator label " + s + " not in D");
+            if (find_label(used, s) >= 0) return set_error(ctx, TCB_EUNSUPPORTED, "operators share label " + s);
+            used.push_back(s);
+        }
+    }
+    // expand the product, first operator outermost
+    struct Term { std::vector<std::string> xl; double sign; };
+    std::vector<Term> terms = {{e.l, 1.0}};
+    for (const PermOperator &op : ops) {
+        std::vector<Term> next;
+        for (const Term &t : terms) {
+            next.push_back(t);
+            for (const std::string &o : op.others) {
+                Term s = t;
+                for (std::string &lab : s.xl) {
+                    if (lab == op.pivot) lab = o;
+                    else if (lab == o) lab = op.pivot;
+                }
+                s.sign = -t.sign;
+                next.push_back(s);
+            }
+        }
+        terms.swap(next);
+    }
+    if ((int)terms.size() > kMaxTerms) return set_error(ctx, TCB_EUNSUPPORTED, "more than 36 terms");
+    std::vector<int32_t> perms(terms.size() * (size_t)std::max(r, 1));
+    std::vector<tcb_c128> coefs(terms.size());
+    for (size_t t = 0; t < terms.size(); ++t) {
+        for (int m = 0; m < r; ++m) {
+            const int s = find_label(e.d, terms[t].xl[m]);
+            if (s < 0) return set_error(ctx, TCB_EUNSUPPORTED, "label of X missing in D");
+            perms[t * r + m] = s;
+        }
+        coefs[t].re = alpha.re * terms[t].sign;
+        coefs[t].im = alpha.im * terms[t].sign;
+    }
+    tcb_c128 beta = {e.accumulate ? 1.0 : 0.0, 0.0};
+    return tcb_permsum(ctx, D, X, (int)terms.size(), perms.data(), coefs.data(), beta);
+}
+
+// used by synth.cu (same shared object): validates the context and exposes its stream and launch counter
+int tcbx_internal_stream(tcb_ctx *ctx, void **stream, int64_t **launches)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    *stream = (void *)ctx->stream;
+    *launches = &ctx->launches;
+    return TCB_OK;
+}
+
+// ---- measurement -------------------------------------------------------------------------------------------
+
+int tcb_measure_fp64_tensor_peak(tcb_ctx *ctx, double milliseconds, double *tflops)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!tflops) return TCB_EINVAL;
+    TCB_CUDA(ctx, run_dmma_peak(milliseconds, tflops, ctx->stream, &ctx->launches));
+    return TCB_OK;
+}
+
+int tcb_timer_start(tcb_ctx *ctx)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    TCB_CUDA(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
+    return TCB_OK;
+}
+
+int tcb_timer_stop(tcb_ctx *ctx, double *milliseconds)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!milliseconds) return TCB_EINVAL;
+    TCB_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
+    TCB_CUDA(ctx, cudaEventSynchronize(ctx->ev1));
+    float ms = 0.f;
+    TCB_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
+    *milliseconds = ms;
+    return TCB_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,78 @@
+// elementwise.cu -- S7: fill, scale, axpy on dense complex128 tensors (north_star "tensor add/scale";
+// the scalar factor of PAPER.md:230).  Memory-bound, one 16-byte access per element, grid-stride.
+#include "kernels.h"
+
+namespace tcb {
+
+namespace {
+
+__global__ void __launch_bounds__(256) fill_kernel(double2 *D, long long n, double re, double im)
+{
+    const double2 v = make_double2(re, im);
+    for (long long i = blockIdx.x * 256LL + threadIdx.x; i < n; i += gridDim.x * 256LL) D[i] = v;
+}
+
+__global__ void __launch_bounds__(256) scale_kernel(double2 *D, long long n, double ar, double ai)
+{
+    for (long long i = blockIdx.x * 256LL + threadIdx.x; i < n; i += gridDim.x * 256LL) {
+        const double2 d = D[i];
+        D[i] = make_double2(__dsub_rn(__dmul_rn(ar, d.x), __dmul_rn(ai, d.y)),
+                            __dadd_rn(__dmul_rn(ar, d.y), __dmul_rn(ai, d.x)));
+    }
+}
+
+template <bool ACC>
+__global__ void __launch_bounds__(256)
+axpy_kernel(double2 *D, const double2 *__restrict__ L, long long n, double ar, double ai)
+{
+    for (long long i = blockIdx.x * 256LL + threadIdx.x; i < n; i += gridDim.x * 256LL) {
+        const double2 x = L[i];
+        double2 y = make_double2(__dsub_rn(__dmul_rn(ar, x.x), __dmul_rn(ai, x.y)),
+                                 __dadd_rn(__dmul_rn(ar, x.y), __dmul_rn(ai, x.x)));
+        if (ACC) {
+            const double2 d = D[i];
+            y.x = __dadd_rn(d.x, y.x);
+            y.y = __dadd_rn(d.y, y.y);
+        }
+        D[i] = y;
+    }
+}
+
+int grid_for(long long n)
+{
+    long long b = (n + 255) / 256;
+    if (b > 148 * 16) b = 148 * 16;
+    return b < 1 ? 1 : (int)b;
+}
+
+}  // namespace
+
+cudaError_t launch_fill(void *D, int64_t n, double re, double im, cudaStream_t s, int64_t *launches)
+{
+    fill_kernel<<<grid_for(n), 256, 0, s>>>((double2 *)D, n, re, im);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && launches) ++*launches;
+    return e;
+}
+
+cudaError_t launch_scale(void *D, int64_t n, double re, double im, cudaStream_t s, int64_t *launches)
+{
+    scale_kernel<<<grid_for(n), 256, 0, s>>>((double2 *)D, n, re, im);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && launches) ++*launches;
+    return e;
+}
+
+cudaError_t launch_axpy(void *D, const void *L, int64_t n, double re, double im, bool accumulate, cudaStream_t s,
+                        int64_t *launches)
+{
+    if (accumulate)
+        axpy_kernel<true><<<grid_for(n), 256, 0, s>>>((double2 *)D, (const double2 *)L, n, re, im);
+    else
+        axpy_kernel<false><<<grid_for(n), 256, 0, s>>>((double2 *)D, (const double2 *)L, n, re, im);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && launches) ++*launches;
+    return e;
+}
+
+}  // namespace tcb

@@ -1,0 +1,77 @@
+// kernels.h -- internal launch interface between the host-side planner/API and the sm_100a kernels.
+// Raw device pointers + stream only; no torch types anywhere in this library.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace tcb {
+
+constexpr int kMaxRank = 6;
+
+// ---- S4 + S5: complex FP64 GEMM on DMMA with the permute-and-accumulate epilogue ---------------------
+// C[m,n] = sum_k A[m,k] * B[k,n];   D[offM[m] + offN[n]] (+)= alpha * C[m,n]
+// Operand layouts ("K-major": k has unit stride, element (row,k) at row*ld + k;
+//                  "M-major": the row index has unit stride, element (row,k) at k*ld + row).
+struct GemmDesc {
+    int64_t M, N, K;
+    const void *A, *B;       // device, complex128
+    int64_t lda, ldb;        // in elements
+    bool a_kmajor, b_kmajor;
+    void *D;                 // device, complex128
+    const int64_t *offM;     // device [M], element offsets into D
+    const int64_t *offN;     // device [N]
+    double alpha_re, alpha_im;
+    bool accumulate;         // true: D += ...; false: D = ...
+    int splits;              // >= 1; > 1 needs `partial`
+    void *partial;           // device, splits * M * N complex128 (split-K partial sums, [z][n][m])
+};
+constexpr int kGemmBM = 64, kGemmBN = 64, kGemmBK = 8;
+cudaError_t launch_zgemm(const GemmDesc &g, cudaStream_t stream, int64_t *launches);
+// Encodes the two TMA descriptors; separated so that the planner can cache them.
+struct GemmTensorMaps { CUtensorMap a, b; };
+cudaError_t encode_gemm_maps(const GemmDesc &g, GemmTensorMaps *maps);
+cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps, cudaStream_t stream,
+                                   int64_t *launches);
+
+// ---- S3: tensor transposition, and the permuted add built on it ------------------------------------------
+// out[sum_d idx_d * ostride[d]] (op)= in[sum_d idx_d * istride[d]]  over idx in [0, extent)
+// The caller passes dims already canonicalised (extent-1 dropped, fusable neighbours fused), sorted by
+// input stride (dim 0 = input unit stride).
+enum PermuteOp { kPermCopy = 0, kPermScale = 1, kPermAccumulate = 2 };   // =, = alpha*, += alpha*
+struct PermuteDesc {
+    int rank;
+    int64_t extent[kMaxRank];
+    int64_t istride[kMaxRank];
+    int64_t ostride[kMaxRank];
+    const void *in;
+    void *out;
+    PermuteOp op;
+    double alpha_re, alpha_im;
+};
+cudaError_t launch_permute(const PermuteDesc &p, cudaStream_t stream, int64_t *launches);
+
+// ---- S6: fused permute-sum -------------------------------------------------------------------------------
+constexpr int kMaxTerms = 36;
+struct PermSumDesc {
+    int rank;
+    int64_t extent[kMaxRank];             // of D
+    int nterms;
+    int64_t xstride[kMaxTerms][kMaxRank]; // stride in X (elements) of D's index k, per term
+    double coef_re[kMaxTerms], coef_im[kMaxTerms];
+    double beta_re, beta_im;
+    const void *X;
+    void *D;
+};
+cudaError_t launch_permsum(const PermSumDesc &p, cudaStream_t stream, int64_t *launches);
+
+// ---- S7: elementwise --------------------------------------------------------------------------------------
+cudaError_t launch_fill(void *D, int64_t n, double re, double im, cudaStream_t stream, int64_t *launches);
+cudaError_t launch_scale(void *D, int64_t n, double re, double im, cudaStream_t stream, int64_t *launches);
+cudaError_t launch_axpy(void *D, const void *L, int64_t n, double re, double im, bool accumulate,
+                        cudaStream_t stream, int64_t *launches);
+
+// ---- measurement -------------------------------------------------------------------------------------------
+cudaError_t run_dmma_peak(double milliseconds, double *tflops, cudaStream_t stream, int64_t *launches);
+
+}  // namespace tcb

@@ -1,0 +1,282 @@
+// plan.cpp -- S2 (host).  "There are different approaches of dealing with tensor transposition ... required
+// for the usage of BLAS GEMM, which depends on a unit-stride index": the planner decides which
+// transpositions of TTGT are really needed.
+//
+//  (i)   extent-1 indices are dropped;
+//  (ii)  the operand that owns D's unit-stride index becomes the GEMM's row side A (its rows run along the
+//        lanes of the epilogue stores), otherwise L and R swap roles;
+//  (iii) an operand is fed IN PLACE when its memory order is [free..][contracted..] ("M-major") or
+//        [contracted..][free..] ("K-major"), in whatever order inside each group: the order of the free
+//        indices is absorbed by the epilogue offset tables offM/offN, and the order of the contracted indices
+//        only has to be common to both operands;
+//  (iv)  otherwise it is permuted into workspace as [contracted in the common order][free in D's order];
+//        if both operands are matrix-shaped but disagree on the contracted order the smaller one is permuted;
+//  (v)   an in-place row operand whose fastest free index is not D's unit-stride index would scatter 16-byte
+//        stores; it is permuted too when it is no larger than D;
+//  (vi)  the result permutation is never a separate pass: alpha*C is scattered by the GEMM epilogue to
+//        D[offM[m] + offN[n]];
+//  (vii) few output tiles and a long K -> split-K with a deterministic second-stage reduction.
+#include "plan.h"
+
+#include <algorithm>
+#include <cstdio>
+#include <map>
+#include <numeric>
+
+#include "../../include/tcb200.h"
+
+namespace tcb {
+
+PermuteShape canonical_permutation(int rank, const int64_t *extent, const int64_t *istride, const int64_t *ostride)
+{
+    struct Dim { int64_t e, is, os; };
+    std::vector<Dim> d;
+    for (int k = 0; k < rank; ++k)
+        if (extent[k] > 1) d.push_back({extent[k], istride[k], ostride[k]});
+    std::sort(d.begin(), d.end(), [](const Dim &a, const Dim &b) { return a.is < b.is; });
+    std::vector<Dim> f;
+    for (const Dim &x : d) {
+        if (!f.empty() && x.is == f.back().is * f.back().e && x.os == f.back().os * f.back().e)
+            f.back().e *= x.e;
+        else
+            f.push_back(x);
+    }
+    PermuteShape p;
+    p.rank = (int)f.size();
+    p.identity = true;
+    p.volume = 1;
+    for (int k = 0; k < p.rank; ++k) {
+        p.extent[k] = f[k].e; p.istride[k] = f[k].is; p.ostride[k] = f[k].os;
+        if (f[k].is != f[k].os) p.identity = false;
+        p.volume *= f[k].e;
+    }
+    return p;
+}
+
+namespace {
+
+struct Lab {
+    std::string name;
+    int64_t ext = 1;
+    int inD = -1, inL = -1, inR = -1;     // positions
+    int64_t sD = 0, sL = 0, sR = 0;       // strides (elements)
+};
+
+void strides_of(const Shape &s, int64_t *st)
+{
+    int64_t x = 1;
+    for (int k = 0; k < s.rank; ++k) { st[k] = x; x *= s.ext[k]; }
+}
+
+bool has_dup(const std::vector<std::string> &v)
+{
+    for (size_t a = 0; a < v.size(); ++a)
+        for (size_t b = a + 1; b < v.size(); ++b)
+            if (v[a] == v[b]) return true;
+    return false;
+}
+
+std::vector<int64_t> offset_table(const std::vector<const Lab *> &order)
+{
+    int64_t n = 1;
+    for (const Lab *l : order) n *= l->ext;
+    std::vector<int64_t> t((size_t)n);
+    std::vector<int64_t> idx(order.size(), 0);
+    int64_t off = 0;
+    for (int64_t i = 0; i < n; ++i) {
+        t[(size_t)i] = off;
+        for (size_t q = 0; q < order.size(); ++q) {
+            off += order[q]->sD;
+            if (++idx[q] < order[q]->ext) break;
+            off -= order[q]->sD * order[q]->ext;
+            idx[q] = 0;
+        }
+    }
+    return t;
+}
+
+std::string join(const std::vector<std::string> &v)
+{
+    std::string s;
+    for (size_t i = 0; i < v.size(); ++i) { if (i) s += ","; s += v[i]; }
+    return s;
+}
+
+}  // namespace
+
+int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const Shape &R, const PlanOptions &opt,
+                     ContractPlan *out, std::string *why)
+{
+    auto fail = [&](int code, const char *msg) { if (why) *why = msg; return code; };
+    if (!e.has_r) return fail(TCB_EINVAL_EXPR, "contraction needs two operands");
+    if ((int)e.d.size() != D.rank || (int)e.l.size() != L.rank || (int)e.r.size() != R.rank)
+        return fail(TCB_ESHAPE, "rank of a handle differs from the expression");
+    if (has_dup(e.d) || has_dup(e.l) || has_dup(e.r))
+        return fail(TCB_EUNSUPPORTED, "label repeated inside one tensor (trace / diagonal)");
+
+    int64_t stD[kMaxRank], stL[kMaxRank], stR[kMaxRank];
+    strides_of(D, stD); strides_of(L, stL); strides_of(R, stR);
+    std::vector<Lab> labs;
+    auto find = [&](const std::string &n) -> Lab * {
+        for (Lab &l : labs) if (l.name == n) return &l;
+        labs.push_back(Lab());
+        labs.back().name = n;
+        return &labs.back();
+    };
+    labs.reserve(3 * kMaxRank);
+    for (int k = 0; k < D.rank; ++k) { Lab *l = find(e.d[k]); l->inD = k; l->sD = stD[k]; l->ext = D.ext[k]; }
+    for (int k = 0; k < L.rank; ++k) {
+        Lab *l = find(e.l[k]);
+        if (l->inD >= 0 && l->ext != L.ext[k]) return fail(TCB_ESHAPE, "extent of an index differs between D and L");
+        l->inL = k; l->sL = stL[k]; l->ext = L.ext[k];
+    }
+    for (int k = 0; k < R.rank; ++k) {
+        Lab *l = find(e.r[k]);
+        if ((l->inD >= 0 || l->inL >= 0) && l->ext != R.ext[k])
+            return fail(TCB_ESHAPE, "extent of an index differs between R and D or L");
+        l->inR = k; l->sR = stR[k]; l->ext = R.ext[k];
+    }
+    for (const Lab &l : labs) {
+        const int n = (l.inD >= 0) + (l.inL >= 0) + (l.inR >= 0);
+        if (n == 3) return fail(TCB_EUNSUPPORTED, "index in D, L and R (batch / Hadamard index)");
+        if (n == 1) return fail(TCB_EUNSUPPORTED, "index in only one tensor (trace / broadcast)");
+    }
+
+    // (ii) row side = owner of D's unit-stride (first non-trivial) index
+    bool swapped = false;
+    for (int k = 0; k < D.rank; ++k) {
+        const Lab *l = find(e.d[k]);
+        if (l->ext > 1) { swapped = (l->inR >= 0); break; }
+    }
+    const std::vector<std::string> &la = swapped ? e.r : e.l, &lb = swapped ? e.l : e.r;
+    auto posA = [&](const Lab *l) { return swapped ? l->inR : l->inL; };
+    auto posB = [&](const Lab *l) { return swapped ? l->inL : l->inR; };
+    auto strA = [&](const Lab *l) { return swapped ? l->sR : l->sL; };
+    auto strB = [&](const Lab *l) { return swapped ? l->sL : l->sR; };
+
+    // memory-order label sequences without extent-1 indices
+    std::vector<const Lab *> seqA, seqB, seqD;
+    for (const std::string &n : la) { const Lab *l = find(n); if (l->ext > 1) seqA.push_back(l); }
+    for (const std::string &n : lb) { const Lab *l = find(n); if (l->ext > 1) seqB.push_back(l); }
+    for (const std::string &n : e.d) { const Lab *l = find(n); if (l->ext > 1) seqD.push_back(l); }
+    auto is_con = [&](const Lab *l) { return l->inD < 0; };
+
+    struct Shape2 { bool mmajor, kmajor; std::vector<const Lab *> free, con; };
+    auto analyse = [&](const std::vector<const Lab *> &seq) {
+        Shape2 s;
+        for (const Lab *l : seq) (is_con(l) ? s.con : s.free).push_back(l);
+        size_t i = 0;
+        while (i < seq.size() && !is_con(seq[i])) ++i;
+        size_t j = i;
+        while (j < seq.size() && is_con(seq[j])) ++j;
+        s.mmajor = (j == seq.size());                 // [free..][con..]
+        i = 0;
+        while (i < seq.size() && is_con(seq[i])) ++i;
+        j = i;
+        while (j < seq.size() && !is_con(seq[j])) ++j;
+        s.kmajor = (j == seq.size());                 // [con..][free..]
+        return s;
+    };
+    Shape2 sa = analyse(seqA), sb = analyse(seqB);
+
+    ContractPlan P;
+    P.swapped = swapped;
+    P.accumulate = e.accumulate;
+    P.M = P.N = P.K = 1;
+    for (const Lab *l : sa.free) P.M *= l->ext;
+    for (const Lab *l : sb.free) P.N *= l->ext;
+    for (const Lab *l : sa.con) P.K *= l->ext;
+    int64_t sizeA = P.M * P.K, sizeB = P.N * P.K, sizeD = P.M * P.N;
+    if (P.M >= (1LL << 30) || P.N >= (1LL << 30) || P.K >= (1LL << 30))
+        return fail(TCB_EUNSUPPORTED, "a matricised extent exceeds 2^30");
+
+    bool inplaceA = (sa.mmajor || sa.kmajor) && !opt.permute_always;
+    bool inplaceB = (sb.mmajor || sb.kmajor) && !opt.permute_always;
+    // (v) row operand whose fastest free index is not D's unit-stride index
+    if (inplaceA && !sa.free.empty() && !seqD.empty() && sa.free[0] != seqD[0] && sizeA <= sizeD) inplaceA = false;
+    // (iv) common contracted order
+    auto same_order = [&](const std::vector<const Lab *> &x, const std::vector<const Lab *> &y) {
+        if (x.size() != y.size()) return false;
+        for (size_t i = 0; i < x.size(); ++i) if (x[i] != y[i]) return false;
+        return true;
+    };
+    std::vector<const Lab *> corder;
+    if (inplaceA && inplaceB && !same_order(sa.con, sb.con)) {
+        if (sizeA <= sizeB) inplaceA = false; else inplaceB = false;
+    }
+    if (inplaceA) corder = sa.con;
+    else if (inplaceB) corder = sb.con;
+    else corder = sa.con.size() ? (sizeA >= sizeB ? sa.con : sb.con) : sb.con;
+
+    // free order: in place -> the operand's own order; permuted -> D's order
+    std::vector<const Lab *> forderA, forderB;
+    if (inplaceA) forderA = sa.free;
+    else for (const Lab *l : seqD) if (posA(l) >= 0) forderA.push_back(l);
+    if (inplaceB) forderB = sb.free;
+    else for (const Lab *l : seqD) if (posB(l) >= 0) forderB.push_back(l);
+
+    auto fill_operand = [&](OperandPlan &o, bool inplace, const Shape2 &s, const std::vector<const Lab *> &seq,
+                            const std::vector<const Lab *> &forder, int64_t rows, auto strX) {
+        o.rows = rows;
+        o.elems = rows * P.K;
+        o.permuted = !inplace;
+        if (inplace) {
+            // K = 1: rows contiguous -> M-major; otherwise prefer what the memory order says
+            if (s.con.empty()) { o.kmajor = false; o.ld = rows; }
+            else if (s.free.empty()) { o.kmajor = true; o.ld = P.K; }
+            else if (s.kmajor) { o.kmajor = true; o.ld = P.K; }
+            else { o.kmajor = false; o.ld = rows; }
+        } else {
+            o.kmajor = true;
+            o.ld = P.K;
+            int64_t ext[2 * kMaxRank], is[2 * kMaxRank], os[2 * kMaxRank];
+            int n = 0;
+            int64_t st = 1;
+            std::map<const Lab *, int64_t> target;
+            for (const Lab *l : corder) { target[l] = st; st *= l->ext; }
+            for (const Lab *l : forder) { target[l] = st; st *= l->ext; }
+            for (const Lab *l : seq) { ext[n] = l->ext; is[n] = strX(l); os[n] = target[l]; ++n; }
+            o.perm = canonical_permutation(n, ext, is, os);
+        }
+    };
+    fill_operand(P.a, inplaceA, sa, seqA, forderA, P.M, strA);
+    fill_operand(P.b, inplaceB, sb, seqB, forderB, P.N, strB);
+
+    P.offM = offset_table(forderA);
+    P.offN = offset_table(forderB);
+    for (const Lab *l : forderA) P.m_labels.push_back(l->name);
+    for (const Lab *l : forderB) P.n_labels.push_back(l->name);
+    for (const Lab *l : corder) P.k_labels.push_back(l->name);
+
+    // (vii) split-K
+    const int64_t tiles = ((P.M + kGemmBM - 1) / kGemmBM) * ((P.N + kGemmBN - 1) / kGemmBN);
+    const int64_t ktiles = (P.K + kGemmBK - 1) / kGemmBK;
+    P.splits = 1;
+    if (opt.splitk > 1) P.splits = (int)std::min<int64_t>(opt.splitk, ktiles);
+    else if (opt.splitk == 0 && tiles <= 148 && ktiles >= 64) {
+        int64_t s = std::min<int64_t>(592 / tiles, ktiles / 16);
+        P.splits = (int)std::max<int64_t>(1, s);
+    }
+
+    P.flops = 8.0 * (double)P.M * (double)P.N * (double)P.K;
+    P.bytes = 16.0 * ((double)sizeA + (double)sizeB + (double)sizeD * (e.accumulate ? 2.0 : 1.0));
+    *out = std::move(P);
+    return TCB_OK;
+}
+
+std::string ContractPlan::describe() const
+{
+    char buf[1024];
+    std::snprintf(buf, sizeof buf,
+                  "{\"M\": %lld, \"N\": %lld, \"K\": %lld, \"m_labels\": \"%s\", \"n_labels\": \"%s\", "
+                  "\"k_labels\": \"%s\", \"row_operand\": \"%s\", \"permute_A\": %s, \"permute_B\": %s, "
+                  "\"A_layout\": \"%s\", \"B_layout\": \"%s\", \"splits\": %d, \"epilogue\": \"fused-scatter\", "
+                  "\"accumulate\": %s, \"flops\": %.6g, \"bytes\": %.6g}",
+                  (long long)M, (long long)N, (long long)K, join(m_labels).c_str(), join(n_labels).c_str(),
+                  join(k_labels).c_str(), swapped ? "R" : "L", a.permuted ? "true" : "false",
+                  b.permuted ? "true" : "false", a.kmajor ? "K-major" : "M-major", b.kmajor ? "K-major" : "M-major",
+                  splits, accumulate ? "true" : "false", flops, bytes);
+    return buf;
+}
+
+}  // namespace tcb

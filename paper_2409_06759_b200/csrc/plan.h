@@ -1,0 +1,58 @@
+// plan.h -- S2: the contraction planner (host).  Chooses the index grouping (M, N, K), which operands are
+// permuted into matrix form, the GEMM variant, split-K, and the epilogue offset tables.
+#pragma once
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "kernels.h"
+#include "parse.h"
+
+namespace tcb {
+
+struct Shape {
+    int rank = 0;
+    int64_t ext[kMaxRank] = {1, 1, 1, 1, 1, 1};
+    int64_t volume() const { int64_t v = 1; for (int k = 0; k < rank; ++k) v *= ext[k]; return v; }
+};
+
+struct PlanOptions {
+    int splitk = 0;               // 0 = auto, 1 = off, n > 1 = forced
+    int epilogue = 0;             // 0 = auto, 1 = fused, 2 = two-pass (reserved)
+    bool permute_always = false;  // A/B testing: permute both operands even when they are matrix-shaped
+};
+
+// canonical transposition descriptor without pointers (extent-1 dropped, neighbours fused, sorted by input stride)
+struct PermuteShape {
+    int rank = 0;
+    int64_t extent[kMaxRank], istride[kMaxRank], ostride[kMaxRank];
+    bool identity = true;        // output order == input order (plain copy)
+    int64_t volume = 1;
+};
+PermuteShape canonical_permutation(int rank, const int64_t *extent, const int64_t *istride, const int64_t *ostride);
+
+struct OperandPlan {
+    bool permuted = false;   // copied into workspace in K-major matrix form first
+    bool kmajor = false;     // layout the GEMM reads
+    int64_t rows = 1, ld = 1, elems = 1;
+    PermuteShape perm;       // valid when permuted
+};
+
+struct ContractPlan {
+    bool swapped = false;    // A := R, B := L (D's unit-stride index lives in R)
+    bool accumulate = false;
+    int64_t M = 1, N = 1, K = 1;
+    OperandPlan a, b;
+    std::vector<int64_t> offM, offN;
+    int splits = 1;
+    std::vector<std::string> m_labels, n_labels, k_labels;
+    double flops = 0, bytes = 0;
+    std::string describe() const;
+};
+
+// returns a tcb_status value (0 = ok)
+int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const Shape &R, const PlanOptions &opt,
+                     ContractPlan *out, std::string *why);
+
+}  // namespace tcb

@@ -54,16 +54,26 @@ def _ln_unit(k53):
     e = np.where(small, e - 1, e) - 53
     s = (m - 1.0) / (m + 1.0)
     s2 = s * s
-    p = np.full_like(s, 1.0 / (2 * (N_LOG_TERMS - 1) + 1))
+    p = np.full_like(s, _LOG_C[-1])
     for k in range(N_LOG_TERMS - 2, -1, -1):
-        p = p * s2 + (1.0 / (2 * k + 1))
+        p = p * s2 + _LOG_C[k]
     lnm = (2.0 * s) * p
     return e.astype(np.float64) * LN2 + lnm
 
 
-_SIN_C = [(-1.0) ** k / float(np.prod(np.arange(1, 2 * k + 2, dtype=np.float64))) for k in range(N_TRIG_TERMS)]
-_COS_C = [(-1.0) ** k / float(np.prod(np.arange(1, 2 * k + 1, dtype=np.float64))) if k else 1.0
-          for k in range(N_TRIG_TERMS)]
+# hex-float literals; csrc/synth.cu carries the same ones
+_SIN_C = [float.fromhex(x) for x in (
+    "0x1.0000000000000p+0", "-0x1.5555555555555p-3", "0x1.1111111111111p-7", "-0x1.a01a01a01a01ap-13",
+    "0x1.71de3a556c734p-19", "-0x1.ae64567f544e4p-26", "0x1.6124613a86d09p-33", "-0x1.ae7f3e733b81fp-41",
+    "0x1.952c77030ad4ap-49", "-0x1.2f49b46814157p-57", "0x1.71b8ef6dcf572p-66", "-0x1.761b413163819p-75")]
+_COS_C = [float.fromhex(x) for x in (
+    "0x1.0000000000000p+0", "-0x1.0000000000000p-1", "0x1.5555555555555p-5", "-0x1.6c16c16c16c17p-10",
+    "0x1.a01a01a01a01ap-16", "-0x1.27e4fb7789f5cp-22", "0x1.1eed8eff8d898p-29", "-0x1.93974a8c07c9dp-37",
+    "0x1.ae7f3e733b81fp-45", "-0x1.6827863b97d97p-53", "0x1.e542ba4020225p-62", "-0x1.0ce396db7f853p-70")]
+_LOG_C = [float.fromhex(x) for x in (
+    "0x1.0000000000000p+0", "0x1.5555555555555p-2", "0x1.999999999999ap-3", "0x1.2492492492492p-3",
+    "0x1.c71c71c71c71cp-4", "0x1.745d1745d1746p-4", "0x1.3b13b13b13b14p-4", "0x1.1111111111111p-4",
+    "0x1.e1e1e1e1e1e1ep-5", "0x1.af286bca1af28p-5", "0x1.8618618618618p-5", "0x1.642c8590b2164p-5")]
 
 
 def _cos_sin_turn(k53):
@@ -94,6 +104,14 @@ def normal_c128(key, idx):
     out = np.empty(idx.shape, dtype=np.complex128)
     out.real = r * c
     out.imag = r * s
+    return out
+
+
+def _scale(z, s):
+    """complex * real, component by component (one rounding each)."""
+    out = np.empty_like(z)
+    out.real = z.real * s
+    out.imag = z.imag * s
     return out
 
 
@@ -156,21 +174,21 @@ def tensor(seed, tensor_id, extents, antisym=(), sigma=1.0, sub=None, hermitian=
         if len(antisym) == 0:
             return g_at(ix)
         if len(antisym) == 1:
-            return 0.5 * (g_at(ix) - g_at(swapped(ix, antisym[0])))
+            return _scale(g_at(ix) - g_at(swapped(ix, antisym[0])), 0.5)
         p, q = antisym
         t1 = g_at(ix) - g_at(swapped(ix, p))
         t2 = g_at(swapped(ix, q)) - g_at(swapped(swapped(ix, p), q))
-        return 0.5 * (t1 - t2)
+        return _scale(t1 - t2, 0.5)
 
     if hermitian:
         assert rank == 4
         A = antisymmetrised(idx)
         Ad = np.conj(antisymmetrised([idx[2], idx[3], idx[0], idx[1]]))
-        val = 0.5 * (A + Ad)
+        val = _scale(A + Ad, 0.5)
     else:
         val = antisymmetrised(idx)
     if sigma != 1.0:
-        val = val * sigma
+        val = _scale(val, sigma)
     shape = [len(s) for s in sub]
     return np.asfortranarray(np.broadcast_to(val, shape)).copy(order="F")
 
@@ -225,7 +243,9 @@ def config_ccd(o, v, config_no=2):
     B["foo"] = np.asfortranarray(np.diag(eo).astype(np.complex128))
     B["fvv"] = np.asfortranarray(np.diag(ev).astype(np.complex128))
     den = (eo[None, None, :, None] + eo[None, None, None, :]) - (ev[:, None, None, None] + ev[None, :, None, None])
-    T = np.asfortranarray(B["vvoo"] / den)
+    T = np.empty(B["vvoo"].shape, dtype=np.complex128, order="F")
+    T.real = B["vvoo"].real / den
+    T.imag = B["vvoo"].imag / den
     return B, T, eo, ev
 
 
