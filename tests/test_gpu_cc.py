@@ -1,0 +1,52 @@
+"""-m gpu: the CC 'generated driver' programs (config 2 CCD residual, config 4 T3 term) run call by call through the
+C ABI, against the same programs evaluated by the oracle, and against the un-factorised equations."""
+import numpy as np
+import pytest
+
+from oracle import cc
+import paper_2409_06759_b200 as pkg
+from paper_2409_06759_b200 import synth, ccd
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    c = pkg.Context(0)
+    yield c
+    c.destroy()
+
+
+@pytest.mark.parametrize("o,v", [(3, 5), (6, 14)])
+def test_ccd_residual_program(ctx, o, v):
+    B, T, eo, ev = synth.config_ccd(o, v)
+    dB = {k: ctx.tensor_from_numpy(x) for k, x in B.items()}
+    dT = ctx.tensor_from_numpy(T)
+    dR = ccd.ccd_residual(ctx, dB, dT)
+    R = ctx.tensor_download(dR)
+    ref = cc.ccd_residual_program(B, T)
+    scale = np.abs(ref).max()
+    assert np.max(np.abs(R - ref)) <= 1e-11 * max(scale, np.abs(B["vvoo"]).max())
+    # invariants: residual antisymmetry (to rounding), driver + Fock terms cancel for the MP2 guess
+    assert np.max(np.abs(R + R.transpose(1, 0, 2, 3))) <= 1e-12 * scale
+    assert np.max(np.abs(R + R.transpose(0, 1, 3, 2))) <= 1e-12 * scale
+    if o <= 3:
+        n = o + v
+        f = np.zeros((n, n), dtype=np.complex128)
+        f[:o, :o], f[o:, o:] = B["foo"], B["fvv"]
+        g = synth.tensor(synth.SEED0 + 2, 1, [n] * 4, antisym=((0, 1), (2, 3)), sigma=0.1, hermitian=True)
+        ref_unf = cc.ccd_residual_unfactorised(o, f, g, T)[0]
+        assert np.max(np.abs(R - ref_unf)) <= 1e-11 * max(np.abs(ref_unf).max(), np.abs(B["vvoo"]).max())
+
+
+def test_t3_term_program(ctx):
+    o, v = 4, 9
+    W, T2 = synth.config_t3(o, v)
+    R3 = synth.config_t3_r3(o, v)
+    dW, dT, dR = ctx.tensor_from_numpy(W), ctx.tensor_from_numpy(T2), ctx.tensor_from_numpy(R3)
+    dX = ctx.tensor_create((v, v, v, o, o, o))
+    ccd.t3_term(ctx, dW, dT, dR, dX)
+    X, ref = cc.t3_term_program(W, T2, R3)
+    gotX, got = ctx.tensor_download(dX), ctx.tensor_download(dR)
+    assert np.max(np.abs(gotX - X)) <= 1e-11 * v * np.abs(W).max() * np.abs(T2).max()
+    assert np.max(np.abs(got - ref)) <= 1e-11 * (np.abs(R3).max() + 9 * np.abs(X).max())
