@@ -69,7 +69,8 @@ typedef struct { double re, im; } tcb_c128;
 int tcb_ctx_create(tcb_ctx **ctx, int device, void *cuda_stream, size_t workspace_bytes);
 int tcb_ctx_destroy(tcb_ctx *ctx);
 /* keys: "splitk" = "auto" | "off" | <integer number of splits>;  "epilogue" = "auto" | "fused" | "twopass";
- *       "permute_operands" = "auto" | "always"  (A/B testing of plans);  unknown key -> TCB_EINVAL. */
+ *       "permute_operands" = "auto" | "always"  (A/B testing of plans);  "kernel_timing" = "on" | "off"
+ *       (see tcb_kernel_stats);  unknown key -> TCB_EINVAL. */
 int tcb_ctx_set_option(tcb_ctx *ctx, const char *key, const char *value);
 /* Blocks until everything enqueued so far has finished (the paper's barrier). */
 int tcb_sync(tcb_ctx *ctx);
@@ -143,6 +144,15 @@ int tcb_measure_fp64_tensor_peak(tcb_ctx *ctx, double milliseconds, double *tflo
  * calls in between with CUDA events on that stream; stop blocks and returns the elapsed time. */
 int tcb_timer_start(tcb_ctx *ctx);
 int tcb_timer_stop(tcb_ctx *ctx, double *milliseconds);
+/* Per-kernel-class device time.  After tcb_ctx_set_option(ctx, "kernel_timing", "on") every kernel launch of
+ * the library is bracketed by a CUDA event pair on the context's stream; tcb_kernel_stats synchronises the
+ * stream and returns the sums since the last reset for kernel = "zgemm" (the GEMM + epilogue launch, with its
+ * split-K reduction when there is one), "permute" (S3 and permuted adds), "permsum" (S6) or "elementwise" (S7).
+ * flops / bytes are the ALGORITHMIC counts of those launches (8 M N K; operands read once, D written once and
+ * read once more for '+='; a transposition moves 2*16 bytes per element). */
+typedef struct { int64_t launches; double milliseconds; double flops; double bytes; } tcb_kernel_stat;
+int tcb_kernel_stats(tcb_ctx *ctx, const char *kernel, tcb_kernel_stat *out);
+int tcb_kernel_stats_reset(tcb_ctx *ctx);
 
 #ifdef __cplusplus
 }

@@ -22,6 +22,11 @@ def _c(z):
     return c128(z.real, z.imag)
 
 
+class kernel_stat(ctypes.Structure):
+    _fields_ = [("launches", ctypes.c_int64), ("milliseconds", ctypes.c_double), ("flops", ctypes.c_double),
+                ("bytes", ctypes.c_double)]
+
+
 class TcbError(RuntimeError):
     def __init__(self, code, text):
         super().__init__(f"tcb error {code}: {text}")
@@ -38,7 +43,7 @@ ABI_SYMBOLS = [
     "tcb_launch_count", "tcb_tensor_create", "tcb_tensor_wrap", "tcb_tensor_destroy", "tcb_tensor_info",
     "tcb_tensor_upload", "tcb_tensor_download", "tcb_tensor_fill", "tcb_contract", "tcb_add", "tcb_scale",
     "tcb_permute", "tcb_permsum", "tcb_antisymmetrize", "tcb_plan_describe", "tcb_measure_fp64_tensor_peak",
-    "tcb_timer_start", "tcb_timer_stop", "tcb_plan_describe_host", "tcbx_synth_normal", "tcbx_synth_index_linear",
+    "tcb_timer_start", "tcb_timer_stop", "tcb_kernel_stats", "tcb_kernel_stats_reset", "tcb_plan_describe_host", "tcbx_synth_normal", "tcbx_synth_index_linear",
     "tcbx_synth_mp2_amplitudes",
 ]
 
@@ -77,6 +82,8 @@ def load_library():
         "tcb_plan_describe_host": [cp, ctypes.c_int, i64p, ctypes.c_int, i64p, ctypes.c_int, i64p, cp, ctypes.c_char_p,
                                    ctypes.c_size_t, i64p, ctypes.c_size_t, i64p, ctypes.c_size_t],
         "tcb_timer_start": [vp],
+        "tcb_kernel_stats": [vp, cp, ctypes.POINTER(kernel_stat)],
+        "tcb_kernel_stats_reset": [vp],
         "tcb_timer_stop": [vp, ctypes.POINTER(ctypes.c_double)],
         "tcbx_synth_normal": [vp, vp, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int, ctypes.POINTER(ctypes.c_int32),
                               ctypes.c_double, ctypes.c_int, i64p, i64p],
@@ -276,6 +283,14 @@ class Context:
         out = ctypes.c_double()
         self._check(self.lib.tcb_measure_fp64_tensor_peak(self.handle, float(milliseconds), ctypes.byref(out)))
         return out.value
+
+    def kernel_stats(self, kernel):
+        out = kernel_stat()
+        self._check(self.lib.tcb_kernel_stats(self.handle, kernel.encode(), ctypes.byref(out)))
+        return {"launches": int(out.launches), "ms": out.milliseconds, "flops": out.flops, "bytes": out.bytes}
+
+    def kernel_stats_reset(self):
+        self._check(self.lib.tcb_kernel_stats_reset(self.handle))
 
     def timer_start(self):
         self._check(self.lib.tcb_timer_start(self.handle))

@@ -36,7 +36,15 @@ struct tcb_ctx {
     std::map<std::string, std::unique_ptr<CachedPlan>> plans;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     int64_t live_tensors = 0;
+    // per-kernel-class device timing ("kernel_timing" = "on"): event pairs around every launch, summed on query
+    bool kernel_timing = false;
+    struct Span { int cls; cudaEvent_t a, b; double flops, bytes; };
+    std::vector<Span> spans;
+    std::vector<cudaEvent_t> free_events;
+    tcb_kernel_stat acc[4];
 };
+
+enum KernelClass { kClsZgemm = 0, kClsPermute = 1, kClsPermsum = 2, kClsElementwise = 3 };
 
 struct tcb_tensor {
     tcb_ctx *ctx = nullptr;
@@ -99,6 +107,50 @@ int workspace(tcb_ctx *ctx, size_t bytes, void **out)
     }
     *out = ctx->ws;
     return TCB_OK;
+}
+
+cudaEvent_t take_event(tcb_ctx *ctx)
+{
+    cudaEvent_t e = nullptr;
+    if (!ctx->free_events.empty()) { e = ctx->free_events.back(); ctx->free_events.pop_back(); }
+    else cudaEventCreate(&e);
+    return e;
+}
+
+// RAII bracket of one kernel-class launch (no-op unless kernel timing is on)
+struct TimedLaunch {
+    tcb_ctx *ctx;
+    tcb_ctx::Span span;
+    bool on;
+    TimedLaunch(tcb_ctx *c, int cls, double flops, double bytes) : ctx(c), on(c->kernel_timing)
+    {
+        if (!on) return;
+        span.cls = cls; span.flops = flops; span.bytes = bytes;
+        span.a = take_event(ctx); span.b = take_event(ctx);
+        cudaEventRecord(span.a, ctx->stream);
+    }
+    ~TimedLaunch()
+    {
+        if (!on) return;
+        cudaEventRecord(span.b, ctx->stream);
+        ctx->spans.push_back(span);
+    }
+};
+
+void fold_spans(tcb_ctx *ctx)
+{
+    if (ctx->spans.empty()) return;
+    cudaStreamSynchronize(ctx->stream);
+    for (const tcb_ctx::Span &s : ctx->spans) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, s.a, s.b) == cudaSuccess) {
+            tcb_kernel_stat &k = ctx->acc[s.cls];
+            k.launches += 1; k.milliseconds += ms; k.flops += s.flops; k.bytes += s.bytes;
+        }
+        ctx->free_events.push_back(s.a);
+        ctx->free_events.push_back(s.b);
+    }
+    ctx->spans.clear();
 }
 
 bool overlaps(const tcb_tensor *a, const tcb_tensor *b)
@@ -210,6 +262,7 @@ int tcb_ctx_create(tcb_ctx **out, int device, void *cuda_stream, size_t workspac
     if (cudaSetDevice(device) != cudaSuccess) return TCB_ECUDA;
     std::unique_ptr<tcb_ctx> ctx(new tcb_ctx());
     ctx->device = device;
+    for (int c = 0; c < 4; ++c) ctx->acc[c] = tcb_kernel_stat{0, 0.0, 0.0, 0.0};
     if (cuda_stream) {
         ctx->stream = (cudaStream_t)cuda_stream;
     } else {
@@ -244,6 +297,8 @@ int tcb_ctx_destroy(tcb_ctx *ctx)
     if (ctx->ws) cudaFree(ctx->ws);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    fold_spans(ctx);
+    for (cudaEvent_t e : ctx->free_events) cudaEventDestroy(e);
     if (ctx->owns_stream) cudaStreamDestroy(ctx->stream);
     delete ctx;
     return TCB_OK;
@@ -255,6 +310,12 @@ int tcb_ctx_set_option(tcb_ctx *ctx, const char *key, const char *value)
 {
     if (!ctx || !key || !value) return TCB_EINVAL;
     std::string why;
+    if (std::string(key) == "kernel_timing") {
+        const std::string v = value;
+        if (v != "on" && v != "off") return set_error(ctx, TCB_EINVAL, "kernel_timing: expected on or off");
+        ctx->kernel_timing = (v == "on");
+        return TCB_OK;
+    }
     int rc = apply_option(ctx->opt, key, value, &why);
     return rc ? set_error(ctx, rc, why) : TCB_OK;
 }
@@ -362,6 +423,7 @@ int tcb_tensor_fill(tcb_ctx *ctx, tcb_tensor *t, tcb_c128 value)
     int rc = enter(ctx);
     if (rc) return rc;
     if (!t) return TCB_EINVAL;
+    TimedLaunch tl(ctx, kClsElementwise, 0.0, 16.0 * (double)t->elems());
     TCB_CUDA(ctx, launch_fill(t->ptr, t->elems(), value.re, value.im, ctx->stream, &ctx->launches));
     return TCB_OK;
 }
@@ -394,11 +456,13 @@ int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor
     const void *Aptr = TA->ptr, *Bptr = TB->ptr;
     if (P.a.permuted) {
         PermuteDesc d = make_desc(P.a.perm, TA->ptr, ws, kPermCopy, 1.0, 0.0);
+        TimedLaunch tl(ctx, kClsPermute, 0.0, 32.0 * (double)P.a.elems);
         TCB_CUDA(ctx, launch_permute(d, ctx->stream, &ctx->launches));
         Aptr = ws;
     }
     if (P.b.permuted) {
         PermuteDesc d = make_desc(P.b.perm, TB->ptr, ws + bytesA, kPermCopy, 1.0, 0.0);
+        TimedLaunch tl(ctx, kClsPermute, 0.0, 32.0 * (double)P.b.elems);
         TCB_CUDA(ctx, launch_permute(d, ctx->stream, &ctx->launches));
         Bptr = ws + bytesA;
     }
@@ -414,6 +478,7 @@ int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor
     g.accumulate = P.accumulate;
     g.splits = P.splits;
     g.partial = bytesP ? ws + bytesA + bytesB : nullptr;
+    TimedLaunch tl(ctx, kClsZgemm, P.flops, P.bytes);
     TCB_CUDA(ctx, launch_zgemm(g, ctx->stream, &ctx->launches));
     return TCB_OK;
 }
@@ -537,13 +602,17 @@ static int permuted_op(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_
     }
     if (overlaps(D, L)) return set_error(ctx, TCB_EALIAS, "D overlaps L");
     const PermuteShape ps = canonical_permutation(r, ext, is, os);
+    const double n16 = 16.0 * (double)D->elems();
     if (pure_copy) {
+        TimedLaunch tl(ctx, kClsPermute, 0.0, 2 * n16);
         PermuteDesc d = make_desc(ps, L->ptr, D->ptr, kPermCopy, 1.0, 0.0);
         TCB_CUDA(ctx, launch_permute(d, ctx->stream, &ctx->launches));
     } else if (ps.identity) {
+        TimedLaunch tl(ctx, kClsElementwise, 0.0, (e.accumulate ? 3 : 2) * n16);
         TCB_CUDA(ctx, launch_axpy(D->ptr, L->ptr, D->elems(), alpha.re, alpha.im, e.accumulate, ctx->stream,
                                   &ctx->launches));
     } else {
+        TimedLaunch tl(ctx, kClsPermute, 0.0, (e.accumulate ? 3 : 2) * n16);
         PermuteDesc d = make_desc(ps, L->ptr, D->ptr, e.accumulate ? kPermAccumulate : kPermScale, alpha.re, alpha.im);
         TCB_CUDA(ctx, launch_permute(d, ctx->stream, &ctx->launches));
     }
@@ -566,6 +635,7 @@ int tcb_scale(tcb_ctx *ctx, tcb_tensor *D, tcb_c128 alpha)
     int rc = enter(ctx);
     if (rc) return rc;
     if (!D) return TCB_EINVAL;
+    TimedLaunch tl(ctx, kClsElementwise, 0.0, 32.0 * (double)D->elems());
     TCB_CUDA(ctx, launch_scale(D->ptr, D->elems(), alpha.re, alpha.im, ctx->stream, &ctx->launches));
     return TCB_OK;
 }
@@ -601,6 +671,8 @@ int tcb_permsum(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, int nterms, co
     if (overlaps(D, X)) return set_error(ctx, TCB_EALIAS, "D overlaps X");
     d.beta_re = beta.re; d.beta_im = beta.im;
     d.X = X->ptr; d.D = D->ptr;
+    const bool reads_d = !(beta.re == 0.0 && beta.im == 0.0);
+    TimedLaunch tl(ctx, kClsPermsum, 0.0, 16.0 * (double)D->elems() * (reads_d ? 3.0 : 2.0));
     TCB_CUDA(ctx, launch_permsum(d, ctx->stream, &ctx->launches));
     return TCB_OK;
 }
@@ -681,6 +753,27 @@ int tcb_measure_fp64_tensor_peak(tcb_ctx *ctx, double milliseconds, double *tflo
     if (rc) return rc;
     if (!tflops) return TCB_EINVAL;
     TCB_CUDA(ctx, run_dmma_peak(milliseconds, tflops, ctx->stream, &ctx->launches));
+    return TCB_OK;
+}
+
+int tcb_kernel_stats(tcb_ctx *ctx, const char *kernel, tcb_kernel_stat *out)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!kernel || !out) return TCB_EINVAL;
+    static const char *names[4] = {"zgemm", "permute", "permsum", "elementwise"};
+    fold_spans(ctx);
+    for (int c = 0; c < 4; ++c)
+        if (std::strcmp(kernel, names[c]) == 0) { *out = ctx->acc[c]; return TCB_OK; }
+    return set_error(ctx, TCB_EINVAL, std::string("unknown kernel class ") + kernel);
+}
+
+int tcb_kernel_stats_reset(tcb_ctx *ctx)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    fold_spans(ctx);
+    for (int c = 0; c < 4; ++c) ctx->acc[c] = tcb_kernel_stat{0, 0.0, 0.0, 0.0};
     return TCB_OK;
 }
 

@@ -1,0 +1,138 @@
+"""-m "not gpu": the C-ABI library loads and exports every symbol include/*.h declares, and the host planner
+(S1 + S2, no device needed) makes the choices DESIGN.md describes.  No compute call is made here."""
+import ctypes
+import glob
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2409_06759_b200 as pkg
+from paper_2409_06759_b200 import binding
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    names = set()
+    for h in glob.glob(os.path.join(ROOT, "include", "*.h")):
+        text = re.sub(r"/\*.*?\*/", "", open(h).read(), flags=re.S)
+        names |= set(re.findall(r"\b(tcbx?_[a-z0-9_]+)\s*\(", text))
+    return names
+
+
+def test_library_exports_every_declared_symbol():
+    lib = pkg.load_library()
+    decl = declared_symbols()
+    assert len(decl) >= 28
+    for name in decl:
+        assert hasattr(lib, name), name
+    assert decl == set(binding.ABI_SYMBOLS), decl ^ set(binding.ABI_SYMBOLS)
+
+
+def test_strerror_and_null_handling():
+    lib = pkg.load_library()
+    assert lib.tcb_strerror(0) == b"ok"
+    assert lib.tcb_strerror(-7) == b"unsupported contraction form"
+    assert lib.tcb_tensor_destroy(None) == 0
+    assert lib.tcb_ctx_destroy(None) == 0
+    assert lib.tcb_sync(None) == binding.TCB_EINVAL
+
+
+def test_no_cpu_fallback_without_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a device is present")
+    with pytest.raises(pkg.TcbError) as ei:
+        pkg.Context(0)
+    assert ei.value.code == binding.TCB_ECUDA
+
+
+def plan(expr, d, l, r, options=None, tables=False):
+    return binding.plan_describe_host(expr, d, l, r, options, want_tables=tables)
+
+
+def test_config3_ladder_needs_no_permutation():
+    o, v = 40, 200
+    p = plan("R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)", (v, v, o, o), (v, v, v, v), (v, v, o, o))
+    assert (p["M"], p["N"], p["K"]) == (40000, 1600, 40000)
+    assert not p["permute_A"] and not p["permute_B"] and p["splits"] == 1
+    assert p["A_layout"] == "M-major" and p["B_layout"] == "K-major" and p["row_operand"] == "L"
+    assert p["flops"] == 8.0 * 40000 * 1600 * 40000
+    # V given as V(c,d,a,b): still in place, K-major
+    p = plan("R(a,b,i,j)+=V(c,d,a,b)*T(c,d,i,j)", (v, v, o, o), (v, v, v, v), (v, v, o, o))
+    assert not p["permute_A"] and p["A_layout"] == "K-major"
+    # T given as T(i,j,c,d): N-major B, still no permutation
+    p = plan("R(a,b,i,j)+=V(a,b,c,d)*T(i,j,c,d)", (v, v, o, o), (v, v, v, v), (o, o, v, v))
+    assert not p["permute_A"] and not p["permute_B"] and p["B_layout"] == "M-major"
+
+
+def test_row_operand_is_owner_of_unit_stride_index_of_D():
+    p = plan("X(a,b,i,j)=I(a,d)*T(d,b,i,j)", (9, 9, 4, 4), (9, 9), (9, 9, 4, 4))
+    assert p["row_operand"] == "L" and p["M"] == 9 and p["N"] == 9 * 16
+    p = plan("X(a,b,i,j)=T(d,b,i,j)*I(a,d)", (9, 9, 4, 4), (9, 9, 4, 4), (9, 9))
+    assert p["row_operand"] == "R" and p["M"] == 9
+
+
+def test_ring_term_permutes_the_smaller_side_only_when_needed():
+    o, v = 6, 14
+    p = plan("X(a,b,i,j)=T(a,c,i,k)*I(k,b,c,j)", (v, v, o, o), (v, v, o, o), (o, v, v, o))
+    assert (p["M"], p["N"], p["K"]) == (o * v, o * v, o * v)
+    assert p["permute_A"] and p["permute_B"]              # neither is matrix-shaped
+
+
+def test_offset_tables_reproduce_the_contraction():
+    """C[m,n] scattered through offM/offN must land where the index string says: checked with numpy on the host."""
+    rng = np.random.default_rng(0)
+    ext = dict(a=5, b=4, c=3, i=2, j=3, k=2)
+    expr = "X(b,i,a,j)=T(a,c,i,k)*I(k,b,c,j)"
+    shp = lambda s: tuple(ext[x] for x in s)
+    p, offM, offN = plan(expr, shp("biaj"), shp("acik"), shp("kbcj"), tables=True)
+    T = rng.standard_normal(shp("acik")) + 1j * rng.standard_normal(shp("acik"))
+    I = rng.standard_normal(shp("kbcj")) + 1j * rng.standard_normal(shp("kbcj"))
+    ref = np.einsum("acik,kbcj->biaj", T, I)
+    m_lab, n_lab, k_lab = p["m_labels"].split(","), p["n_labels"].split(","), p["k_labels"].split(",")
+    rowT, colI = (T, I) if p["row_operand"] == "L" else (I, T)
+    rl, cl = ("acik", "kbcj") if p["row_operand"] == "L" else ("kbcj", "acik")
+    # matricise by hand in the planner's label orders (first label fastest)
+    A = np.transpose(rowT, [rl.index(x) for x in m_lab + k_lab]).reshape(p["M"], p["K"], order="F")
+    Bm = np.transpose(colI, [cl.index(x) for x in k_lab + n_lab]).reshape(p["K"], p["N"], order="F")
+    C = A @ Bm
+    flat = np.zeros(ref.size, dtype=np.complex128)
+    flat[offM[:, None] + offN[None, :]] = C
+    assert np.allclose(flat.reshape(ref.shape, order="F"), ref, atol=1e-12)
+    assert len(set((offM[:, None] + offN[None, :]).ravel().tolist())) == ref.size     # a bijection onto D
+
+
+def test_skinny_contraction_gets_split_k_and_options_override():
+    o, v = 30, 150
+    p = plan("I(l,i)=W(k,l,c,d)*T(d,c,i,k)", (o, o), (o, o, v, v), (v, v, o, o))
+    assert (p["M"], p["N"], p["K"]) == (30, 30, 675000) and p["splits"] > 1
+    p = plan("I(l,i)=W(k,l,c,d)*T(d,c,i,k)", (o, o), (o, o, v, v), (v, v, o, o), "splitk=off")
+    assert p["splits"] == 1
+    p = plan("I(l,i)=W(k,l,c,d)*T(d,c,i,k)", (o, o), (o, o, v, v), (v, v, o, o), "splitk=7")
+    assert p["splits"] == 7
+
+
+@pytest.mark.parametrize("expr,shapes,code", [
+    ("D(m,n)+=L(m,k)*R(k,n", [(2, 2)] * 3, binding.TCB_EINVAL_EXPR),
+    ("D(m,n)+=L(m,k)", [(2, 2)] * 3, binding.TCB_EINVAL_EXPR),
+    ("D(m,n)+=L(m,k)*R(k,n)", [(2, 3), (2, 4), (5, 3)], binding.TCB_ESHAPE),
+    ("D(m,n)+=L(m,k,q)*R(k,n)", [(2, 2)] * 3, binding.TCB_ESHAPE),
+    ("D(m,n)+=L(m,k)*R(k,q)", [(2, 2)] * 3, binding.TCB_EUNSUPPORTED),       # n, q in one tensor only
+    ("D(m,n)+=L(m,n)*R(m,n)", [(2, 2)] * 3, binding.TCB_EUNSUPPORTED),       # Hadamard
+    ("D(m,n)+=L(m,k)*R(k,k)", [(2, 2)] * 3, binding.TCB_EUNSUPPORTED),       # trace
+])
+def test_invalid_contractions_are_rejected(expr, shapes, code):
+    with pytest.raises(pkg.TcbError) as ei:
+        plan(expr, *shapes)
+    assert ei.value.code == code
+
+
+def test_extent_one_indices_are_dropped_and_labels_may_be_long():
+    p = plan("R(p1,x,h1)+=T(p1,e_1,y,h1)*F(e_1,x,y)", (70, 1, 9), (70, 40, 1, 9), (40, 1, 1))
+    assert (p["M"], p["N"], p["K"]) == (630, 1, 40)
+    assert p["permute_A"]                                  # [free][contracted][free]: not matrix-shaped
+    p = plan("R(p1,x,h1)+=T(p1,y,h1,e_1)*F(e_1,x,y)", (70, 1, 9), (70, 1, 9, 40), (40, 1, 1))
+    assert (p["M"], p["N"], p["K"]) == (630, 1, 40) and not p["permute_A"] and p["A_layout"] == "M-major"
