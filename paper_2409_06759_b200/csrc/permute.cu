@@ -3,142 +3,309 @@
 //
 //   out[sum_d idx_d * ostride[d]] (op)= in[sum_d idx_d * istride[d]]
 //
-// One element is one complex128 = one 16-byte vector access (LDG.128 / STG.128), so "vectorised" is per
-// element.  The kernel is a generalised tiled transpose: a tile is a hyper-rectangle of the index space whose
-// extents are chosen on the host so that (a) the leading INPUT dims inside the tile span >= 32 contiguous
-// elements (512-byte read runs) and (b) the leading OUTPUT dims inside the tile span >= 32 contiguous elements
-// of the output (512-byte write runs).  When an extent is small (occupied indices, 6..40) the tile simply
-// spans the next index too (compound runs).  Threads read the tile in input order (coalesced), park it in
-// shared memory, and write it in output order (coalesced); the shared-memory stride of the output-fastest dim
-// is padded to an odd number of 16-byte slots so that the gather side is bank-conflict free.
-// Each thread keeps its tile-local offsets in registers (they are identical for every tile) and the CTA
-// loops over tiles (persistent grid), so the per-element index arithmetic is one add; boundary tiles mask with
-// packed per-dim indices.  All global offsets are 64-bit (V of config 3 is 25.6 GB).
+// One element is one complex128 = 16 bytes.  A tile is a hyper-rectangle of the index space whose extents are
+// chosen on the host so that (a) the leading INPUT dims inside the tile span >= 32 contiguous elements and (b) the
+// leading OUTPUT dims inside the tile span >= 32 contiguous elements of the output (512-byte runs on both sides;
+// when an extent is small -- occupied indices, 6..40 -- the tile spans the next index too).
+//
+// B200 design (measured, profiles/r1b_permute.md): a load->sync->store tile loop cannot keep enough bytes in
+// flight for HBM3e, so the LOAD side is asynchronous bulk copies (cp.async.bulk.shared::cluster.global, SASS
+// UBLKCP): every contiguous input run of a tile ("row" = the tile's extent along the input unit-stride dim) is
+// one bulk copy straight into shared memory, completion counted on an mbarrier; tiles rotate through a ring of
+// 2..4 stages, so each CTA has stages-1 tiles (up to ~100 KB) in flight while it drains one.  Rows are copied to
+// a padded pitch (the stride of the output-fastest dim is odd in 16-byte units), which makes the STORE side --
+// threads gather the tile in output order with LDS.128 and write coalesced STG.128 -- bank-conflict free.
+// A bulk copy costs its issuing warp ~32 cycles, so the rows of a tile are dealt round-robin to all 8 warps.
+// Tile-local offsets are tile-invariant and live in registers; tile coordinates advance by a mixed-radix add
+// (no division in the loop); boundary tiles mask with packed per-dim indices.  All global offsets are 64-bit
+// (V of config 3 is 25.6 GB).
 #include "kernels.h"
 
 #include <algorithm>
+#include <cstdlib>
 
 namespace tcb {
 
 namespace {
 
 constexpr int PT = 256;            // threads per CTA
+constexpr int NW = PT / 32;
 constexpr int kMaxVol = 4096;      // elements per tile (64 KB)
+constexpr int kRowRegs = 2;        // rows per thread whose offsets are kept in registers
+constexpr int kIdxBits = 18;       // packed tile-local index: sum_d ceil(log2 t[d]) <= 18; slot < 2^14
+constexpr int kChunk = 8;          // elements a thread holds in registers at a time
 
 struct PermParams {
     int t[kMaxRank];               // tile extents
     int ntile[kMaxRank];
+    int step[kMaxRank];            // mixed-radix digits of gridDim.x (tile-coordinate increment)
     int q[kMaxRank];               // dims in output order (q[0] = output unit stride)
     int ss[kMaxRank];              // shared-memory strides (elements)
     int sh[kMaxRank];              // bit position of dim d inside a packed tile-local index
     int mk[kMaxRank];              // (1 << bits(d)) - 1
     long long e[kMaxRank], is[kMaxRank], os[kMaxRank];
-    int vol;
+    int vol, rows, stages, tile_bytes;
     long long ntiles;
     const double2 *in;
     double2 *out;
     double ar, ai;
 };
 
-// OffT: type of the tile-local offsets (int when every t[d]*stride[d] sum fits 31 bits, else long long)
-template <int J, int OP, typename OffT>
-__global__ void __launch_bounds__(PT) permute_kernel(const PermParams p)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 {
-    extern __shared__ double2 tile_smem[];
-    const int tid = threadIdx.x;
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "PERM_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra PERM_DONE;\n"
+        "bra PERM_WAIT;\n"
+        "PERM_DONE:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ double2 lds128(uint32_t addr)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
 
-    OffT inoff[J], outoff[J];
-    unsigned inidx[J], outidx[J], sp[J];       // sp = smem slot for the load side | store side << 16
-#pragma unroll
-    for (int j = 0; j < J; ++j) {
-        const int e = tid + PT * j;
-        long long io = 0, oo = 0;
-        unsigned ii = 0, oi = 0;
-        int si = 0, so = 0;
-        int rem = e;
+// tile coordinates of one cursor (the load cursor runs `stages` tiles ahead of the store cursor)
+struct Cursor {
+    int c[kMaxRank];
+    __device__ __forceinline__ void init(const PermParams &p, unsigned tile)   // tile < gridDim.x
+    {
 #pragma unroll
         for (int d = 0; d < kMaxRank; ++d) {
-            const int i = rem % p.t[d];
-            rem /= p.t[d];
-            io += (long long)i * p.is[d];
-            si += i * p.ss[d];
-            ii |= (unsigned)i << p.sh[d];
+            c[d] = (int)(tile % (unsigned)p.ntile[d]);
+            tile /= (unsigned)p.ntile[d];
         }
-        rem = e;
+    }
+    __device__ __forceinline__ void advance(const PermParams &p)
+    {
+        int carry = 0;
+#pragma unroll
+        for (int d = 0; d < kMaxRank; ++d) {
+            int x = c[d] + p.step[d] + carry;
+            carry = x >= p.ntile[d];
+            c[d] = carry ? x - p.ntile[d] : x;
+        }
+    }
+    // base offsets of the tile and the last valid tile-local index per dim
+    __device__ __forceinline__ bool locate(const PermParams &p, const long long *stride, long long *base, int *lim) const
+    {
+        long long b = 0;
+        bool interior = true;
+#pragma unroll
+        for (int d = 0; d < kMaxRank; ++d) {
+            const long long o = (long long)c[d] * p.t[d];
+            b += o * stride[d];
+            const long long l = min((long long)p.t[d], p.e[d] - o);
+            interior = interior && (l == p.t[d]);
+            lim[d] = (int)l - 1;
+        }
+        *base = b;
+        return interior;
+    }
+};
+
+// OffT: type of the tile-local offsets (int when every t[d]*stride[d] sum fits 31 bits, else long long)
+template <int J, int OP, typename OffT>
+__global__ void __launch_bounds__(PT, (J > 8 ? 1 : 2)) permute_kernel(const __grid_constant__ PermParams p)
+{
+    extern __shared__ __align__(128) uint8_t perm_smem[];
+    const uint32_t sbase = smem_u32(perm_smem);
+    const uint32_t bars = sbase + (uint32_t)p.stages * p.tile_bytes;   // full[s] at +8s, empty[s] at +8(stages+s)
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int stages = p.stages;
+
+    if (tid == 0) {
+        for (int s = 0; s < stages; ++s) {
+            mbar_init(bars + 8 * s, NW);
+            mbar_init(bars + 8 * (stages + s), NW);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+
+    // ---- store side: this thread's J elements of a tile, enumerated in OUTPUT order ------------------------
+    // pack[j] = packed tile-local index (low kIdxBits bits) | shared-memory slot << kIdxBits
+    OffT outoff[J];
+    unsigned pack[J];
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+        long long oo = 0;
+        unsigned oi = 0;
+        int so = 0;
+        int rem = tid + PT * j;
 #pragma unroll
         for (int x = 0; x < kMaxRank; ++x) {
             const int d = p.q[x];
+            if (p.t[d] == 1) continue;
             const int i = rem % p.t[d];
             rem /= p.t[d];
             oo += (long long)i * p.os[d];
             so += i * p.ss[d];
             oi |= (unsigned)i << p.sh[d];
         }
-        inoff[j] = (OffT)io; outoff[j] = (OffT)oo; inidx[j] = ii; outidx[j] = oi;
-        sp[j] = (unsigned)si | ((unsigned)so << 16);
+        outoff[j] = (OffT)oo; pack[j] = oi | ((unsigned)so << kIdxBits);
     }
-
-    for (long long tile = blockIdx.x; tile < p.ntiles; tile += gridDim.x) {
-        long long base_in = 0, base_out = 0;
-        int lim[kMaxRank];               // last valid tile-local index per dim
-        bool interior = true;
-        {
-            long long rem = tile;
+    // ---- load side: rows (runs along the input unit-stride dim) dealt round-robin to the warps ---------------
+    // row r of a tile -> thread with lane * NW + warp == r mod PT
+    auto decode_row = [&](int r, long long *goff, int *soff, unsigned *ridx) {
+        long long g = 0;
+        int s = 0;
+        unsigned ii = 0;
 #pragma unroll
-            for (int d = 0; d < kMaxRank; ++d) {
-                const long long tc = rem % p.ntile[d];
-                rem /= p.ntile[d];
-                const long long o = tc * p.t[d];
-                base_in += o * p.is[d];
-                base_out += o * p.os[d];
-                const long long l = min((long long)p.t[d], p.e[d] - o);
-                interior = interior && (l == p.t[d]);
-                lim[d] = (int)l - 1;
-            }
+        for (int d = 1; d < kMaxRank; ++d) {
+            if (p.t[d] == 1) continue;
+            const int i = r % p.t[d];
+            r /= p.t[d];
+            g += (long long)i * p.is[d];
+            s += i * p.ss[d];
+            ii |= (unsigned)i << p.sh[d];
         }
-        auto inside = [&](unsigned idx) {
-            bool ok = true;
+        *goff = g; *soff = s * 16; *ridx = ii;
+    };
+    const int row0 = lane * NW + warp;
+    OffT rgoff[kRowRegs];
+    int rsoff[kRowRegs];
+    unsigned ridx[kRowRegs];
 #pragma unroll
-            for (int d = 0; d < kMaxRank; ++d) ok = ok && ((int)((idx >> p.sh[d]) & p.mk[d]) <= lim[d]);
-            return ok;
-        };
+    for (int k = 0; k < kRowRegs; ++k) {
+        long long g;
+        decode_row(row0 + k * PT, &g, &rsoff[k], &ridx[k]);
+        rgoff[k] = (OffT)g;
+    }
+    const int warp_rows = p.rows > warp ? (p.rows - 1 - warp) / NW + 1 : 0;
+    const unsigned row_bytes = (unsigned)p.t[0] * 16u;
+    __syncthreads();
+
+    auto inside = [&](unsigned idx, const int *lim) {
+        bool ok = true;
+#pragma unroll
+        for (int d = 0; d < kMaxRank; ++d) ok = ok && ((int)((idx >> p.sh[d]) & p.mk[d]) <= lim[d]);
+        return ok;
+    };
+
+    const long long my_n = p.ntiles > blockIdx.x ? (p.ntiles - 1 - blockIdx.x) / gridDim.x + 1 : 0;
+    Cursor lc, sc;
+    lc.init(p, blockIdx.x);
+    sc = lc;
+
+    // issue every row of the load cursor's tile into stage s, then advance the cursor
+    auto issue = [&](int s) {
+        long long base_in;
+        int lim[kMaxRank];
+        const bool interior = lc.locate(p, p.is, &base_in, lim);
+        lc.advance(p);
+        const uint32_t dst = sbase + (uint32_t)s * p.tile_bytes, full = bars + 8 * s;
         const double2 *src = p.in + base_in;
-        double2 *dst = p.out + base_out;
-
-        double2 v[J];
+        if (interior) {
+            if (lane == 0) mbar_expect_tx(full, (unsigned)warp_rows * row_bytes);
+            __syncwarp();
 #pragma unroll
-        for (int j = 0; j < J; ++j) {
-            const bool ok = (tid + PT * j < p.vol) && (interior || inside(inidx[j]));
-            v[j] = ok ? src[inoff[j]] : make_double2(0.0, 0.0);
-        }
-#pragma unroll
-        for (int j = 0; j < J; ++j)
-            if (tid + PT * j < p.vol) tile_smem[sp[j] & 0xffffu] = v[j];
-        __syncthreads();
-        bool okv[J];
-#pragma unroll
-        for (int j = 0; j < J; ++j) {
-            okv[j] = (tid + PT * j < p.vol) && (interior || inside(outidx[j]));
-            if (OP == kPermAccumulate) v[j] = okv[j] ? dst[outoff[j]] : make_double2(0.0, 0.0);
-        }
-#pragma unroll
-        for (int j = 0; j < J; ++j) {
-            if (!okv[j]) continue;
-            const double2 x = tile_smem[sp[j] >> 16];
-            double2 y;
-            if (OP == kPermCopy) {
-                y = x;
-            } else {
-                y.x = __dsub_rn(__dmul_rn(p.ar, x.x), __dmul_rn(p.ai, x.y));
-                y.y = __dadd_rn(__dmul_rn(p.ar, x.y), __dmul_rn(p.ai, x.x));
-                if (OP == kPermAccumulate) {
-                    y.x = __dadd_rn(v[j].x, y.x);
-                    y.y = __dadd_rn(v[j].y, y.y);
-                }
+            for (int k = 0; k < kRowRegs; ++k)
+                if (row0 + k * PT < p.rows) bulk_g2s(dst + rsoff[k], src + rgoff[k], row_bytes, full);
+            for (int r = row0 + kRowRegs * PT; r < p.rows; r += PT) {
+                long long g; int so; unsigned ri;
+                decode_row(r, &g, &so, &ri);
+                bulk_g2s(dst + so, src + g, row_bytes, full);
             }
-            dst[outoff[j]] = y;
+        } else {
+            const unsigned rb = (unsigned)(lim[0] + 1) * 16u;
+            unsigned bytes = 0;
+            for (int r = row0; r < p.rows; r += PT) {
+                long long g; int so; unsigned ri;
+                decode_row(r, &g, &so, &ri);
+                if (inside(ri, lim)) bytes += rb;
+            }
+            bytes = __reduce_add_sync(0xffffffffu, bytes);
+            if (lane == 0) mbar_expect_tx(full, bytes);
+            __syncwarp();
+            for (int r = row0; r < p.rows; r += PT) {
+                long long g; int so; unsigned ri;
+                decode_row(r, &g, &so, &ri);
+                if (inside(ri, lim)) bulk_g2s(dst + so, src + g, rb, full);
+            }
         }
-        __syncthreads();
+    };
+
+    const int npro = (int)min((long long)stages, my_n);
+    for (int s = 0; s < npro; ++s) issue(s);
+
+    int s = 0;
+    uint32_t ph = 0;
+    for (long long k = 0; k < my_n; ++k) {
+        long long base_out;
+        int lim[kMaxRank];
+        const bool interior = sc.locate(p, p.os, &base_out, lim);
+        sc.advance(p);
+        double2 *dst = p.out + base_out;
+        const uint32_t stile = sbase + (uint32_t)s * p.tile_bytes;
+
+        mbar_wait(bars + 8 * s, ph);
+#pragma unroll
+        for (int j0 = 0; j0 < J; j0 += kChunk) {
+            constexpr int C = J < kChunk ? J : kChunk;
+            bool okv[C];
+            double2 v[C], d[C];
+#pragma unroll
+            for (int c = 0; c < C; ++c) {
+                const int j = j0 + c;
+                okv[c] = (tid + PT * j < p.vol) && (interior || inside(pack[j] & ((1u << kIdxBits) - 1), lim));
+                if (OP == kPermAccumulate && okv[c]) d[c] = dst[outoff[j]];
+            }
+#pragma unroll
+            for (int c = 0; c < C; ++c)
+                if (okv[c]) v[c] = lds128(stile + (pack[j0 + c] >> kIdxBits) * 16u);
+            if (j0 + kChunk >= J) {          // last chunk: the stage is drained once these loads have landed
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bars + 8 * (stages + s));
+            }
+#pragma unroll
+            for (int c = 0; c < C; ++c) {
+                if (!okv[c]) continue;
+                const double2 x = v[c];
+                double2 y;
+                if (OP == kPermCopy) {
+                    y = x;
+                } else {
+                    y.x = __dsub_rn(__dmul_rn(p.ar, x.x), __dmul_rn(p.ai, x.y));
+                    y.y = __dadd_rn(__dmul_rn(p.ar, x.y), __dmul_rn(p.ai, x.x));
+                    if (OP == kPermAccumulate) {
+                        y.x = __dadd_rn(d[c].x, y.x);
+                        y.y = __dadd_rn(d[c].y, y.y);
+                    }
+                }
+                dst[outoff[j0 + c]] = y;
+            }
+        }
+        if (k + stages < my_n) {
+            mbar_wait(bars + 8 * (stages + s), ph);      // every warp has drained stage s
+            issue(s);
+        }
+        if (++s == stages) { s = 0; ph ^= 1; }
     }
 }
 
@@ -172,7 +339,7 @@ cudaError_t launch_permute(const PermuteDesc &pd, cudaStream_t stream, int64_t *
     PermParams p;
     const int r = pd.rank;
     for (int d = 0; d < kMaxRank; ++d) {
-        p.t[d] = 1; p.ntile[d] = 1; p.q[d] = d; p.ss[d] = 0; p.sh[d] = 0; p.mk[d] = 0;
+        p.t[d] = 1; p.ntile[d] = 1; p.q[d] = d; p.ss[d] = 0; p.sh[d] = 0; p.mk[d] = 0; p.step[d] = 0;
         p.e[d] = d < r ? pd.extent[d] : 1;
         p.is[d] = d < r ? pd.istride[d] : 0;
         p.os[d] = d < r ? pd.ostride[d] : 0;
@@ -184,38 +351,57 @@ cudaError_t launch_permute(const PermuteDesc &pd, cudaStream_t stream, int64_t *
     for (int d = 0; d < kMaxRank; ++d) p.q[d] = q[d];
 
     const int TI = env_int("TCB_PERM_TI", 32), TO = env_int("TCB_PERM_TO", 32);
-    const int VOL = env_int("TCB_PERM_VOL", 1024);
-    long long prod = 1;
-    for (int d = 0; d < r && prod < TI; ++d) {
-        const long long need = (TI + prod - 1) / prod;
-        p.t[d] = (int)std::max<long long>(p.t[d], std::min<long long>(p.e[d], need));
-        prod *= p.t[d];
-    }
-    prod = 1;
-    for (int x = 0; x < r && prod < TO; ++x) {
-        const int d = q[x];
-        const long long need = (TO + prod - 1) / prod;
-        p.t[d] = (int)std::max<long long>(p.t[d], std::min<long long>(p.e[d], need));
-        prod *= p.t[d];
-    }
-    auto volume = [&] { long long v = 1; for (int d = 0; d < r; ++d) v *= p.t[d]; return v; };
-    // grow (input-leading dims first: longer runs on both sides when dim 0 leads both) up to the volume target
-    for (int d = 0; d < r && volume() < VOL; ++d) {
-        while (p.t[d] < p.e[d] && p.t[d] < 1024 && volume() < VOL) {
-            const long long room = VOL / (volume() / p.t[d]);
-            int nt = (int)std::min<long long>(std::min<long long>(p.e[d], 1024), std::max<long long>(p.t[d] + 1, room));
-            if (volume() / p.t[d] * nt > kMaxVol) break;
-            p.t[d] = nt;
+    const int VOL = std::min(env_int("TCB_PERM_VOL", 2048), kMaxVol);
+    // tile extent for a dim of extent e, between lo and hi: least padding first (ragged last tiles waste a CTA
+    // slot), then 128-byte-aligned cuts (multiples of 8 elements: no cache line shared by two tiles), then
+    // 32-byte-aligned cuts (even: no half-written sector), then the larger tile
+    auto pick_tile = [](long long e, long long lo, long long hi) {
+        hi = std::min(hi, e);
+        lo = std::max<long long>(1, std::min(lo, hi));
+        long long best = lo, best_score = -1;
+        for (long long t = lo; t <= hi; ++t) {
+            const long long padded = (e + t - 1) / t * t;
+            const long long align = (t == e || t % 8 == 0) ? 0 : (t % 2 == 0 ? 1 : 2);
+            const long long score = (padded * 4 + align) * 8192 + (8191 - t);
+            if (best_score < 0 || score < best_score) { best = t; best_score = score; }
         }
+        return best;
+    };
+    // minimal extents: >= ti contiguous elements on the input side, >= to on the output side.  A short leading
+    // dim (<= twice the need: occupied indices) is taken whole rather than cut into two short runs; otherwise
+    // the cut is picked in [need, 1.6 need] (two such sides still fit the volume target).  `plain` is the
+    // fallback that always fits kMaxVol: each side spans < 2 * 32 elements.
+    auto volume = [&] { long long v = 1; for (int d = 0; d < r; ++d) v *= p.t[d]; return v; };
+    auto minimal = [&](int ti, int to, bool plain) {
+        for (int d = 0; d < kMaxRank; ++d) p.t[d] = 1;
+        for (int side = 0; side < 2; ++side) {
+            const int target = side == 0 ? ti : to;
+            long long prod = 1;
+            for (int x = 0; x < r && prod < target; ++x) {
+                const int d = side == 0 ? x : q[x];
+                const long long need = (target + prod - 1) / prod;
+                long long want = std::min<long long>(p.e[d], need);
+                if (!plain && p.e[d] > need)
+                    want = p.e[d] <= 2 * need ? p.e[d] : pick_tile(p.e[d], need, x == 0 ? (8 * need + 4) / 5 : 2 * need - 1);
+                p.t[d] = (int)std::max<long long>(p.t[d], want);
+                prod *= p.t[d];
+            }
+        }
+    };
+    minimal(TI, TO, false);
+    if (volume() > kMaxVol) minimal(std::min(TI, 32), std::min(TO, 32), true);
+    // grow (input-leading dims first: longer runs on both sides when dim 0 leads both) up to the volume target,
+    // never beyond it
+    for (int d = 0; d < r && volume() < VOL; ++d) {
+        const long long others = volume() / p.t[d];
+        const long long room = std::min<long long>(VOL / others, p.e[d]);
+        if (room > p.t[d]) p.t[d] = (int)pick_tile(p.e[d], p.t[d], room);
+        if (p.t[d] < p.e[d]) break;          // a partial dim ends the contiguous run: further dims add rows, not run length
     }
-    // even out the tiles of each dim (e = 60, t = 32 -> 2 tiles of 30)
-    for (int d = 0; d < r; ++d) {
-        const long long n = (p.e[d] + p.t[d] - 1) / p.t[d];
-        p.t[d] = (int)((p.e[d] + n - 1) / n);
-        p.ntile[d] = (int)n;
-    }
+    for (int d = 0; d < r; ++d) p.ntile[d] = (int)((p.e[d] + p.t[d] - 1) / p.t[d]);
     if (volume() > kMaxVol) return cudaErrorInvalidValue;
     p.vol = (int)volume();
+    p.rows = p.vol / p.t[0];
     p.ntiles = 1;
     for (int d = 0; d < r; ++d) p.ntiles *= p.ntile[d];
     // shared-memory strides in input order; the output-fastest dim gets an odd stride
@@ -225,14 +411,25 @@ cudaError_t launch_permute(const PermuteDesc &pd, cudaStream_t stream, int64_t *
         p.ss[d] = s;
         s *= p.t[d];
     }
-    const size_t smem = (size_t)s * sizeof(double2);
+    p.tile_bytes = (int)(((size_t)s * sizeof(double2) + 127) / 128 * 128);
+    // ring depth and CTAs per SM: ~200 KB of shared memory per SM, 2..4 stages per CTA
+    int ctas_per_sm = std::max(1, std::min(4, env_int("TCB_PERM_CTAS", 2)));
+    if (p.vol > 8 * PT) ctas_per_sm = 1;      // the J = 16 instantiation is compiled for one CTA per SM (registers)
+    while (ctas_per_sm > 1 && 2 * p.tile_bytes > 200 * 1024 / ctas_per_sm - 128) --ctas_per_sm;
+    const int budget = 200 * 1024 / ctas_per_sm - 128;
+    p.stages = std::max(2, std::min(env_int("TCB_PERM_STAGES", 4), budget / p.tile_bytes));
+    const size_t smem = (size_t)p.stages * p.tile_bytes + 128;
+    if (smem > 227 * 1024) return cudaErrorInvalidValue;
     p.in = (const double2 *)pd.in;
     p.out = (double2 *)pd.out;
     p.ar = pd.alpha_re; p.ai = pd.alpha_im;
 
     const int J = (p.vol + PT - 1) / PT;
-    const int ctas_per_sm = std::max(1, std::min(8, (int)(200 * 1024 / std::max<size_t>(smem, 8 * 1024))));
-    int blocks = (int)std::min<long long>(p.ntiles, 148LL * env_int("TCB_PERM_CTAS", ctas_per_sm));
+    const int blocks = (int)std::min<long long>(p.ntiles, 148LL * ctas_per_sm);
+    {   // mixed-radix digits of the grid size
+        long long g = blocks;
+        for (int d = 0; d < kMaxRank; ++d) { p.step[d] = (int)(g % p.ntile[d]); g /= p.ntile[d]; }
+    }
     // packed tile-local index: bits(d) = ceil(log2 t[d]); sum <= log2(vol) + rank <= 18
     int bit = 0;
     long long max_in = 0, max_out = 0;
@@ -245,7 +442,7 @@ cudaError_t launch_permute(const PermuteDesc &pd, cudaStream_t stream, int64_t *
         max_in += (long long)(p.t[d] - 1) * p.is[d];
         max_out += (long long)(p.t[d] - 1) * p.os[d];
     }
-    if (bit > 31 || s >= 65536) return cudaErrorInvalidValue;
+    if (bit > kIdxBits || s >= (1 << (32 - kIdxBits))) return cudaErrorInvalidValue;
     const bool small = max_in < (1LL << 31) && max_out < (1LL << 31);
     cudaError_t e;
     if (small) {
