@@ -445,7 +445,7 @@ int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor
 
     const size_t bytesA = P.a.permuted ? align_up((size_t)P.a.elems * 16, 1024) : 0;
     const size_t bytesB = P.b.permuted ? align_up((size_t)P.b.elems * 16, 1024) : 0;
-    const size_t bytesP = P.splits > 1 ? align_up((size_t)P.splits * P.M * P.N * 16, 1024) : 0;
+    const size_t bytesP = align_up(P.partial_bytes, 1024);
     char *ws = nullptr;
     if (bytesA + bytesB + bytesP) {
         void *p;
@@ -476,7 +476,7 @@ int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor
     g.offN = cp->d_tables + P.offM.size();
     g.alpha_re = alpha.re; g.alpha_im = alpha.im;
     g.accumulate = P.accumulate;
-    g.splits = P.splits;
+    g.splitk = P.splitk;
     g.partial = bytesP ? ws + bytesA + bytesB : nullptr;
     TimedLaunch tl(ctx, kClsZgemm, P.flops, P.bytes);
     TCB_CUDA(ctx, launch_zgemm(g, ctx->stream, &ctx->launches));

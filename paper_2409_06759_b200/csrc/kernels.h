@@ -23,9 +23,19 @@ struct GemmDesc {
     const int64_t *offN;     // device [N]
     double alpha_re, alpha_im;
     bool accumulate;         // true: D += ...; false: D = ...
-    int splits;              // >= 1; > 1 needs `partial`
-    void *partial;           // device, splits * M * N complex128 (split-K partial sums, [z][n][m])
+    int splitk;              // 0 = auto (stream-K on the remainder wave), 1 = off, n > 1 = every tile cut n ways
+    void *partial;           // device, gemm_schedule(...).partial_bytes (raw accumulator fragments of cut tiles)
 };
+// How the (tile, k-tile) iteration space is dealt to the persistent grid (2 CTAs per SM): whole tiles
+// data-parallel, the remainder ("stream-K") cut along K into equal chunks, one per CTA, summed by a fix-up kernel.
+struct GemmSchedule {
+    int mt, nt, ktiles, grid;
+    int64_t dp_tiles, sk_tiles, sk_chunks;
+    int sk_q, sk_slots;
+    int splits;              // pieces per tile when every tile is cut (reported by the planner), else 1
+    size_t partial_bytes;
+};
+GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk);
 constexpr int kGemmBM = 64, kGemmBN = 64, kGemmBK = 8;
 cudaError_t launch_zgemm(const GemmDesc &g, cudaStream_t stream, int64_t *launches);
 // Encodes the two TMA descriptors; separated so that the planner can cache them.

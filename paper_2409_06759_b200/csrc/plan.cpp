@@ -248,15 +248,12 @@ int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const 
     for (const Lab *l : forderB) P.n_labels.push_back(l->name);
     for (const Lab *l : corder) P.k_labels.push_back(l->name);
 
-    // (vii) split-K
-    const int64_t tiles = ((P.M + kGemmBM - 1) / kGemmBM) * ((P.N + kGemmBN - 1) / kGemmBN);
-    const int64_t ktiles = (P.K + kGemmBK - 1) / kGemmBK;
-    P.splits = 1;
-    if (opt.splitk > 1) P.splits = (int)std::min<int64_t>(opt.splitk, ktiles);
-    else if (opt.splitk == 0 && tiles <= 148 && ktiles >= 64) {
-        int64_t s = std::min<int64_t>(592 / tiles, ktiles / 16);
-        P.splits = (int)std::max<int64_t>(1, s);
-    }
+    // (vii) schedule: whole tiles data-parallel over the persistent grid, the remainder wave (or, for skinny
+    // M x N with long K, everything) cut along K -- see gemm_schedule in zgemm.cu
+    P.splitk = opt.splitk;
+    const GemmSchedule sc = gemm_schedule(P.M, P.N, P.K, opt.splitk);
+    P.splits = sc.splits;
+    P.partial_bytes = sc.partial_bytes;
 
     P.flops = 8.0 * (double)P.M * (double)P.N * (double)P.K;
     P.bytes = 16.0 * ((double)sizeA + (double)sizeB + (double)sizeD * (e.accumulate ? 2.0 : 1.0));

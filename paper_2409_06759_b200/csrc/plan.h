@@ -45,7 +45,9 @@ struct ContractPlan {
     int64_t M = 1, N = 1, K = 1;
     OperandPlan a, b;
     std::vector<int64_t> offM, offN;
-    int splits = 1;
+    int splits = 1;          // pieces per tile when every tile is cut along K (skinny shapes), else 1
+    int splitk = 0;          // the option the schedule was made with
+    size_t partial_bytes = 0; // workspace for the raw fragments of tiles cut along K
     std::vector<std::string> m_labels, n_labels, k_labels;
     double flops = 0, bytes = 0;
     std::string describe() const;

@@ -32,7 +32,8 @@ namespace tcb {
 namespace {
 
 constexpr int BM = kGemmBM, BN = kGemmBN, BK = kGemmBK;
-constexpr int STAGES = 4;
+constexpr int STAGES = 6;
+constexpr int kNumSMs = 148;            // B200; the persistent grid is 2 CTAs per SM
 constexpr int A_BYTES = BM * BK * 16;   // 8 KB
 constexpr int B_BYTES = BN * BK * 16;   // 8 KB
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
@@ -41,14 +42,19 @@ constexpr int NTHREADS = 128;
 
 struct GemmParams {
     long long M, N, K;
-    int mt, nt, gn;
-    int ktiles, splits, ktiles_per_split;
+    int mblocks, nblocks;          // ceil(M / 8), ceil(N / 8): the 8-row / 8-column DMMA blocks
+    int mt, nt, gn;                // tile grid, column-group width of the tile order
+    int ktiles, klast_steps;       // ceil(K / BK); k-steps of 4 in the last k-tile (1 or 2)
+    long long dp_tiles;            // tiles [0, dp_tiles) are computed whole, tile c + w * grid by CTA c
+    long long sk_tiles;            // tiles [dp_tiles, dp_tiles + sk_tiles): their (tile, k-tile) iterations are cut
+    long long sk_chunks;           //   into sk_chunks chunks of sk_q iterations; chunk ch belongs to CTA ch % grid
+    int sk_q, sk_slots;            // a chunk touches <= sk_slots tiles; partial slot = ch * sk_slots + ordinal
     double2 *D;
     const long long *offM;
     const long long *offN;
     double alpha_re, alpha_im;
     int accumulate;
-    double2 *partial;
+    double2 *partial;              // [slot][32][128] raw accumulator fragments
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -103,154 +109,105 @@ __device__ __forceinline__ double2 lds128(uint32_t addr)
     return v;
 }
 
-template <bool A_KMAJOR, bool B_KMAJOR>
-__global__ void __launch_bounds__(NTHREADS, 2)
-zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-                  const GemmParams p)
-{
-    extern __shared__ uint8_t smem_raw[];
-    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;   // full[s] at +8s, empty[s] at +8(STAGES+s)
-
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int warp_m = warp & 1, warp_n = warp >> 1;
-
-    // tile coordinates: groups of `gn` tile-columns, n fastest inside a group (concurrent CTAs form a
-    // near-square block of the output so that A row panels and B column panels are shared through L2)
-    int tile_m, tile_n;
+// ---- work decomposition ("stream-K": data-parallel full waves, the remainder cut along K) ------------------
+// A segment is a run of k-tiles [kb, ke) of one output tile.  slot < 0: the segment is the whole tile and the
+// CTA writes D itself; otherwise its raw accumulators go to partial slot `slot` and the fix-up kernel sums the
+// tile's slots in k order (fixed order: bit-reproducible, no atomics).
+struct Segment {
+    long long tile, slot;
+    int kb, ke;
+};
+struct SegmentIter {
+    long long w, ch;
+    int sub, phase;
+    __device__ __forceinline__ void init()
     {
-        const int group_sz = p.gn * p.mt;
-        const int g = blockIdx.x / group_sz, rem = blockIdx.x % group_sz;
-        const int n0t = g * p.gn;
-        const int gw = min(p.gn, p.nt - n0t);
-        tile_m = rem / gw;
-        tile_n = n0t + rem % gw;
+        w = blockIdx.x; ch = blockIdx.x; sub = 0; phase = 0;
     }
-    const int m0 = tile_m * BM, n0 = tile_n * BN;
-    const int kt_begin = blockIdx.z * p.ktiles_per_split;
-    const int kt_end = min(p.ktiles, kt_begin + p.ktiles_per_split);
-    const int KT = kt_end - kt_begin;
-
-    if (tid == 0) {
-        for (int s = 0; s < STAGES; ++s) {
-            mbar_init(bar_base + 8 * s, 1);
-            mbar_init(bar_base + 8 * (STAGES + s), NTHREADS / 32);
-        }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
-    }
-    __syncthreads();
-
-    auto issue = [&](int kt_local, int s) {
-        const uint32_t bar = bar_base + 8 * s;
-        const uint32_t sA = smem_base + s * STAGE_BYTES, sB = sA + A_BYTES;
-        const int k0 = (kt_begin + kt_local) * BK;
-        mbar_expect_tx(bar, STAGE_BYTES);
-        if (A_KMAJOR) {
-            tma_load_2d(sA, &tmA, 2 * k0, m0, bar);
-        } else {
-#pragma unroll
-            for (int j = 0; j < BM / 8; ++j) tma_load_2d(sA + j * 1024, &tmA, 2 * (m0 + 8 * j), k0, bar);
-        }
-        if (B_KMAJOR) {
-            tma_load_2d(sB, &tmB, 2 * k0, n0, bar);
-        } else {
-#pragma unroll
-            for (int j = 0; j < BN / 8; ++j) tma_load_2d(sB + j * 1024, &tmB, 2 * (n0 + 8 * j), k0, bar);
-        }
-    };
-
-    if (tid == 0) {
-        const int npro = min(STAGES, KT);
-        for (int s = 0; s < npro; ++s) issue(s, s);
-    }
-
-    // per-lane fragment offsets inside a 1 KB atom, for the two k-steps of a stage
-    const int r = lane >> 2, c = lane & 3;
-    const int rowmap = (r >> 1) + 4 * (r & 1);
-    uint32_t offA[2], offB[2];
-#pragma unroll
-    for (int ks = 0; ks < 2; ++ks) {
-        const int k = ks * 4 + c;
-        offA[ks] = A_KMAJOR ? (rowmap * 128 + ((k ^ rowmap) * 16)) : (k * 128 + ((rowmap ^ k) * 16));
-        offB[ks] = B_KMAJOR ? (rowmap * 128 + ((k ^ rowmap) * 16)) : (k * 128 + ((rowmap ^ k) * 16));
-    }
-
-    double cr[4][4][2], ci[4][4][2];
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            cr[i][j][0] = cr[i][j][1] = 0.0;
-            ci[i][j][0] = ci[i][j][1] = 0.0;
-        }
-
-    for (int kt = 0; kt < KT; ++kt) {
-        const int s = kt % STAGES;
-        if (tid == 0 && kt >= 1 && kt - 1 + STAGES < KT) {
-            // refill the stage consumed in the previous iteration (the other warps had a whole stage to release it)
-            const int sp = (kt - 1) % STAGES;
-            mbar_wait(bar_base + 8 * (STAGES + sp), ((kt - 1) / STAGES) & 1);
-            issue(kt - 1 + STAGES, sp);
-        }
-        mbar_wait(bar_base + 8 * s, (kt / STAGES) & 1);
-        const uint32_t sA = smem_base + s * STAGE_BYTES + (warp_m * 4) * 1024;
-        const uint32_t sB = smem_base + s * STAGE_BYTES + A_BYTES + (warp_n * 4) * 1024;
-#pragma unroll
-        for (int ks = 0; ks < 2; ++ks) {
-            double2 a[4], b[4];
-#pragma unroll
-            for (int i = 0; i < 4; ++i) a[i] = lds128(sA + i * 1024 + offA[ks]);
-#pragma unroll
-            for (int j = 0; j < 4; ++j) b[j] = lds128(sB + j * 1024 + offB[ks]);
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const double nai = neg_exact(a[i].y);
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    dmma(cr[i][j][0], cr[i][j][1], a[i].x, b[j].x);
-                    dmma(ci[i][j][0], ci[i][j][1], a[i].x, b[j].y);
-                    dmma(cr[i][j][0], cr[i][j][1], nai, b[j].y);
-                    dmma(ci[i][j][0], ci[i][j][1], a[i].y, b[j].x);
-                }
+    __device__ __forceinline__ bool next(const GemmParams &p, Segment *s)
+    {
+        if (phase == 0) {
+            if (w < p.dp_tiles) {
+                s->tile = w; s->slot = -1; s->kb = 0; s->ke = p.ktiles;
+                w += gridDim.x;
+                return true;
             }
+            phase = 1;
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + s));
+        const long long total = p.sk_tiles * p.ktiles;
+        while (ch < p.sk_chunks) {
+            const long long it0 = ch * p.sk_q, it1 = min(total, it0 + p.sk_q);
+            const long long first = it0 / p.ktiles, last = (it1 - 1) / p.ktiles;
+            const long long tl = first + sub;
+            if (tl <= last) {
+                const long long base = tl * p.ktiles;
+                s->kb = (int)max(0LL, it0 - base);
+                s->ke = (int)min((long long)p.ktiles, it1 - base);
+                s->tile = p.dp_tiles + tl;
+                s->slot = (s->kb == 0 && s->ke == p.ktiles) ? -1 : ch * p.sk_slots + sub;
+                ++sub;
+                return true;
+            }
+            ch += gridDim.x;
+            sub = 0;
+        }
+        return false;
     }
+};
 
-    // ---- epilogue: lane holds C[m = mb*8 + rowmap][n = nb*8 + c (+4)] for its 4x4 blocks -----------------
-    const long long mw = (long long)m0 + warp_m * 32 + rowmap;
-    const long long nw = (long long)n0 + warp_n * 32 + c;
-    if (p.splits > 1) {
-        double2 *P = p.partial + (long long)blockIdx.z * p.M * p.N;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const long long m = mw + i * 8;
-            if (m >= p.M) continue;
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const long long n = nw + j * 8 + h * 4;
-                    if (n < p.N) P[n * p.M + m] = make_double2(cr[i][j][h], ci[i][j][h]);
-                }
-        }
-        return;
-    }
+// Tile order: groups of `gn` tile-columns, n fastest inside a group (concurrent CTAs form a near-square block of
+// the output, so A row panels and B column panels are shared through L2).  The 8-wide DMMA blocks of M and N are
+// dealt evenly to the tiles (N = 400 -> 7 tiles of 7,7,7,7,7,7,8 blocks instead of six full tiles and a sliver).
+struct TileGeom {
+    int m0, n0;          // element origin
+    int mb, nb;          // blocks in this tile (<= 8 each)
+};
+__device__ __forceinline__ TileGeom tile_geom(const GemmParams &p, long long tile)
+{
+    const long long group_sz = (long long)p.gn * p.mt;
+    const int g = (int)(tile / group_sz), rem = (int)(tile % group_sz);
+    const int n0t = g * p.gn;
+    const int gw = min(p.gn, p.nt - n0t);
+    const int tm = rem / gw, tn = n0t + rem % gw;
+    const int mb0 = (int)((long long)tm * p.mblocks / p.mt), mb1 = (int)((long long)(tm + 1) * p.mblocks / p.mt);
+    const int nb0 = (int)((long long)tn * p.nblocks / p.nt), nb1 = (int)((long long)(tn + 1) * p.nblocks / p.nt);
+    TileGeom t;
+    t.m0 = mb0 * 8; t.n0 = nb0 * 8; t.mb = mb1 - mb0; t.nb = nb1 - nb0;
+    return t;
+}
+// The two warp rows (columns) of a CTA split a tile's blocks ceil/floor; `flip` (the parity of the CTA's wave,
+// i.e. of the other CTA resident on the same SM) hands the larger half to the other pair of sub-partitions.
+struct WarpGeom {
+    int moff, mcnt, noff, ncnt;      // in blocks, relative to the tile origin
+};
+__device__ __forceinline__ WarpGeom warp_geom(const TileGeom &t, int warp_m, int warp_n, int flip)
+{
+    WarpGeom w;
+    const int mh = (t.mb + 1 - flip) / 2, nh = (t.nb + 1 - flip) / 2;      // blocks of warp row / column 0
+    w.moff = warp_m ? mh : 0; w.mcnt = warp_m ? t.mb - mh : mh;
+    w.noff = warp_n ? nh : 0; w.ncnt = warp_n ? t.nb - nh : nh;
+    return w;
+}
+
+// permute-and-accumulate epilogue of one warp fragment: D[offM[m] + offN[n]] (+)= alpha * C[m, n]
+__device__ __forceinline__ void store_fragment(const GemmParams &p, const double (&cr)[4][4][2],
+                                               const double (&ci)[4][4][2], const TileGeom &t, const WarpGeom &w,
+                                               int rowmap, int c)
+{
+    const long long mw = (long long)t.m0 + w.moff * 8 + rowmap;
+    const long long nw = (long long)t.n0 + w.noff * 8 + c;
     long long om[4], on[4][2];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const long long m = mw + i * 8;
-        om[i] = (m < p.M) ? p.offM[m] : -1;
+        om[i] = (i < w.mcnt && m < p.M) ? p.offM[m] : -1;
     }
 #pragma unroll
     for (int j = 0; j < 4; ++j)
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             const long long n = nw + j * 8 + h * 4;
-            on[j][h] = (n < p.N) ? p.offN[n] : -1;
+            on[j][h] = (j < w.ncnt && n < p.N) ? p.offN[n] : -1;
         }
     const double ar = p.alpha_re, ai = p.alpha_im;
 #pragma unroll
@@ -274,25 +231,210 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         }
 }
 
-// deterministic split-K reduction + scatter: D[offM[m]+offN[n]] (+)= alpha * sum_z P[z][n][m]  (z ascending)
-__global__ void __launch_bounds__(256)
-splitk_reduce_kernel(const double2 *__restrict__ P, int splits, long long M, long long N, double2 *D,
-                     const long long *__restrict__ offM, const long long *__restrict__ offN, double ar, double ai,
-                     int accumulate)
+// one k-tile (two k-steps of 4) of a warp tile of MC x NC blocks: complex product = 4 real DMMAs per block pair
+template <int MC, int NC>
+__device__ __forceinline__ void mma_ktile(double (&cr)[4][4][2], double (&ci)[4][4][2], uint32_t sA, uint32_t sB,
+                                          const uint32_t (&offA)[2], const uint32_t (&offB)[2], int nks)
 {
-    const long long total = M * N;
-    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < total;
-         e += (long long)gridDim.x * blockDim.x) {
-        double sr = 0.0, si = 0.0;
-        for (int z = 0; z < splits; ++z) {
-            const double2 v = P[(long long)z * total + e];
-            sr += v.x;
-            si += v.y;
+#pragma unroll
+    for (int ks = 0; ks < 2; ++ks) {
+        if (ks < nks) {
+            double2 a[MC], b[NC];
+#pragma unroll
+            for (int i = 0; i < MC; ++i) a[i] = lds128(sA + i * 1024 + offA[ks]);
+#pragma unroll
+            for (int j = 0; j < NC; ++j) b[j] = lds128(sB + j * 1024 + offB[ks]);
+#pragma unroll
+            for (int i = 0; i < MC; ++i) {
+                const double nai = neg_exact(a[i].y);
+#pragma unroll
+                for (int j = 0; j < NC; ++j) {
+                    dmma(cr[i][j][0], cr[i][j][1], a[i].x, b[j].x);
+                    dmma(ci[i][j][0], ci[i][j][1], a[i].x, b[j].y);
+                    dmma(cr[i][j][0], cr[i][j][1], nai, b[j].y);
+                    dmma(ci[i][j][0], ci[i][j][1], a[i].y, b[j].x);
+                }
+            }
         }
-        const long long m = e % M, n = e / M;
-        double2 *dst = D + offM[m] + offN[n];
-        double2 v = make_double2(ar * sr - ai * si, ar * si + ai * sr);
-        if (accumulate) {
+    }
+}
+
+template <bool A_KMAJOR, bool B_KMAJOR>
+__global__ void __launch_bounds__(NTHREADS, 2)
+zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+                  const __grid_constant__ GemmParams p)
+{
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;   // full[s] at +8s, empty[s] at +8(STAGES+s)
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int warp_m = warp & 1, warp_n = warp >> 1;
+    const int flip = (blockIdx.x / kNumSMs) & 1;
+
+    if (tid == 0) {
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(bar_base + 8 * s, 1);
+            mbar_init(bar_base + 8 * (STAGES + s), NTHREADS / 32);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
+    }
+    __syncthreads();
+
+    // ---- producer (thread 0): walks the same segment list, STAGES k-tiles ahead of the consumers, ACROSS tile
+    // boundaries -- the next tile's operands are already in flight while this tile's epilogue stores drain
+    SegmentIter pit;
+    Segment pseg;
+    int pk = 0, pm0 = 0, pn0 = 0;
+    bool pvalid = false;
+    int pstage = 0;
+    auto producer_advance = [&]() {
+        pvalid = pit.next(p, &pseg);
+        if (pvalid) {
+            const TileGeom t = tile_geom(p, pseg.tile);
+            pm0 = t.m0; pn0 = t.n0; pk = pseg.kb;
+        }
+    };
+    auto issue = [&]() {              // loads k-tile pk of the producer's segment into stage pstage
+        const uint32_t bar = bar_base + 8 * pstage;
+        const uint32_t sA = smem_base + pstage * STAGE_BYTES, sB = sA + A_BYTES;
+        const int k0 = pk * BK;
+        mbar_expect_tx(bar, STAGE_BYTES);
+        if (A_KMAJOR) {
+            tma_load_2d(sA, &tmA, 2 * k0, pm0, bar);
+        } else {
+#pragma unroll
+            for (int j = 0; j < BM / 8; ++j) tma_load_2d(sA + j * 1024, &tmA, 2 * (pm0 + 8 * j), k0, bar);
+        }
+        if (B_KMAJOR) {
+            tma_load_2d(sB, &tmB, 2 * k0, pn0, bar);
+        } else {
+#pragma unroll
+            for (int j = 0; j < BN / 8; ++j) tma_load_2d(sB + j * 1024, &tmB, 2 * (pn0 + 8 * j), k0, bar);
+        }
+        if (++pstage == STAGES) pstage = 0;
+        if (++pk == pseg.ke) producer_advance();
+    };
+    if (tid == 0) {
+        pit.init();
+        producer_advance();
+        for (int s = 0; s < STAGES && pvalid; ++s) issue();
+    }
+
+    // per-lane fragment offsets inside a 1 KB atom, for the two k-steps of a stage
+    const int r = lane >> 2, c = lane & 3;
+    const int rowmap = (r >> 1) + 4 * (r & 1);
+    uint32_t offA[2], offB[2];
+#pragma unroll
+    for (int ks = 0; ks < 2; ++ks) {
+        const int k = ks * 4 + c;
+        offA[ks] = A_KMAJOR ? (rowmap * 128 + ((k ^ rowmap) * 16)) : (k * 128 + ((rowmap ^ k) * 16));
+        offB[ks] = B_KMAJOR ? (rowmap * 128 + ((k ^ rowmap) * 16)) : (k * 128 + ((rowmap ^ k) * 16));
+    }
+
+    SegmentIter cit;
+    Segment seg;
+    cit.init();
+    int stage = 0;
+    uint32_t phase = 0;
+    long long done = 0;                 // k-tiles consumed by this CTA so far
+    while (cit.next(p, &seg)) {
+        const TileGeom tg = tile_geom(p, seg.tile);
+        // tiles cut along K are summed fragment-wise by the fix-up kernel: every CTA must split them alike
+        const WarpGeom wg = warp_geom(tg, warp_m, warp_n, seg.slot < 0 ? flip : 0);
+
+        double cr[4][4][2], ci[4][4][2];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                cr[i][j][0] = cr[i][j][1] = 0.0;
+                ci[i][j][0] = ci[i][j][1] = 0.0;
+            }
+
+        for (int kt = seg.kb; kt < seg.ke; ++kt, ++done) {
+            if (tid == 0 && done >= 1 && pvalid) {
+                // refill the stage consumed in the previous iteration (the other warps had a whole k-tile to release it)
+                const int sp = stage == 0 ? STAGES - 1 : stage - 1;
+                mbar_wait(bar_base + 8 * (STAGES + sp), (stage == 0 ? phase ^ 1 : phase));
+                issue();
+            }
+            mbar_wait(bar_base + 8 * stage, phase);
+            const uint32_t sA = smem_base + stage * STAGE_BYTES + wg.moff * 1024;
+            const uint32_t sB = smem_base + stage * STAGE_BYTES + A_BYTES + wg.noff * 1024;
+            const int nks = (kt == p.ktiles - 1) ? p.klast_steps : 2;
+            switch (wg.mcnt * 5 + wg.ncnt) {      // only the blocks that exist are multiplied (no tensor work on padding)
+#define TCB_CASE(MC, NC) case MC * 5 + NC: mma_ktile<MC, NC>(cr, ci, sA, sB, offA, offB, nks); break;
+                TCB_CASE(4, 4) TCB_CASE(4, 3) TCB_CASE(4, 2) TCB_CASE(4, 1)
+                TCB_CASE(3, 4) TCB_CASE(3, 3) TCB_CASE(3, 2) TCB_CASE(3, 1)
+                TCB_CASE(2, 4) TCB_CASE(2, 3) TCB_CASE(2, 2) TCB_CASE(2, 1)
+                TCB_CASE(1, 4) TCB_CASE(1, 3) TCB_CASE(1, 2) TCB_CASE(1, 1)
+#undef TCB_CASE
+                default: break;                   // a warp without blocks only keeps the barriers moving
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + stage));
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+
+        // ---- epilogue: lane holds C[m = block i, row rowmap][n = block j, column c (+4)] of its warp's blocks -----
+        if (seg.slot < 0) {
+            store_fragment(p, cr, ci, tg, wg, rowmap, c);
+        } else {
+            double2 *P = p.partial + seg.slot * (32LL * NTHREADS) + tid;
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+#pragma unroll
+                    for (int h = 0; h < 2; ++h)
+                        if (i < wg.mcnt && j < wg.ncnt)
+                            P[((i * 4 + j) * 2 + h) * NTHREADS] = make_double2(cr[i][j][h], ci[i][j][h]);
+        }
+    }
+}
+
+// fix-up of the tiles that were cut along K: sums the tile's partial fragments in k order (deterministic) and
+// applies the same permute-and-accumulate epilogue.  grid = (stream-K tiles, 8): CTA y owns fragment column
+// (j, h) = (y >> 1, y & 1) of every warp, same thread <-> element map as the main kernel.
+__global__ void __launch_bounds__(NTHREADS) zgemm_fixup_kernel(const __grid_constant__ GemmParams p)
+{
+    const long long tl = blockIdx.x;
+    const long long base = tl * p.ktiles;
+    const long long ch_lo = base / p.sk_q, ch_hi = (base + p.ktiles - 1) / p.sk_q;
+    if (ch_lo == ch_hi) return;                       // computed whole by one CTA, already in D
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int j = blockIdx.y >> 1, h = blockIdx.y & 1;
+    const TileGeom tg = tile_geom(p, p.dp_tiles + tl);
+    const WarpGeom wg = warp_geom(tg, warp & 1, warp >> 1, 0);
+    if (j >= wg.ncnt) return;
+    double sr[4] = {0.0, 0.0, 0.0, 0.0}, si[4] = {0.0, 0.0, 0.0, 0.0};
+    for (long long ch = ch_lo; ch <= ch_hi; ++ch) {
+        const long long first = (ch * p.sk_q) / p.ktiles;
+        const double2 *P = p.partial + (ch * p.sk_slots + (tl - first)) * (32LL * NTHREADS) + tid;
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+            if (i < wg.mcnt) {
+                const double2 v = P[((i * 4 + j) * 2 + h) * NTHREADS];
+                sr[i] += v.x;
+                si[i] += v.y;
+            }
+    }
+    const int r = lane >> 2, c = lane & 3;
+    const int rowmap = (r >> 1) + 4 * (r & 1);
+    const long long n = (long long)tg.n0 + wg.noff * 8 + c + j * 8 + h * 4;
+    if (n >= p.N) return;
+    const long long on = p.offN[n];
+    const double ar = p.alpha_re, ai = p.alpha_im;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const long long m = (long long)tg.m0 + wg.moff * 8 + rowmap + i * 8;
+        if (i >= wg.mcnt || m >= p.M) continue;
+        double2 *dst = p.D + p.offM[m] + on;
+        double2 v = make_double2(ar * sr[i] - ai * si[i], ar * si[i] + ai * sr[i]);
+        if (p.accumulate) {
             const double2 d = *dst;
             v.x += d.x;
             v.y += d.y;
@@ -346,8 +488,9 @@ cudaError_t encode_operand(CUtensorMap *tm, const void *ptr, int64_t rows, int64
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
+
 template <bool AK, bool BK_>
-cudaError_t launch_variant(const GemmTensorMaps &maps, const GemmParams &p, dim3 grid, cudaStream_t stream)
+cudaError_t launch_variant(const GemmTensorMaps &maps, const GemmParams &p, int grid, cudaStream_t stream)
 {
     auto kern = zgemm_dmma_kernel<AK, BK_>;
     static bool configured = false;
@@ -362,6 +505,42 @@ cudaError_t launch_variant(const GemmTensorMaps &maps, const GemmParams &p, dim3
 
 }  // namespace
 
+GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk)
+{
+    GemmSchedule s;
+    const int64_t mblocks = (M + 7) / 8, nblocks = (N + 7) / 8;
+    s.mt = (int)((mblocks + 7) / 8);
+    s.nt = (int)((nblocks + 7) / 8);
+    s.ktiles = (int)((K + BK - 1) / BK);
+    const int64_t tiles = (int64_t)s.mt * s.nt, KT = s.ktiles;
+    const int64_t slots = 2LL * kNumSMs;                 // resident CTAs
+    s.dp_tiles = tiles; s.sk_tiles = 0; s.sk_chunks = 0; s.sk_q = 1; s.sk_slots = 1; s.splits = 1;
+    if (splitk > 1) {                                    // forced: every tile cut into ~splitk pieces
+        s.dp_tiles = 0; s.sk_tiles = tiles;
+        s.sk_q = (int)std::max<int64_t>(1, (KT + splitk - 1) / splitk);
+        s.splits = (int)((KT + s.sk_q - 1) / s.sk_q);
+    } else if (splitk == 0) {                            // auto: full waves whole, the remainder cut along K
+        const int64_t rem = tiles % slots;
+        // worth it when the remainder wave would leave most of the chip idle for a whole K sweep; a chunk
+        // shorter than 8 k-tiles costs more in fix-up traffic than it saves
+        if (rem > 0 && rem * KT / slots + 8 < KT * 9 / 10) {
+            s.dp_tiles = tiles - rem; s.sk_tiles = rem;
+            const int64_t chunks = std::max<int64_t>(1, std::min<int64_t>(slots, rem * KT / 8));
+            s.sk_q = (int)((rem * KT + chunks - 1) / chunks);
+            if (s.dp_tiles == 0) s.splits = (int)((KT + s.sk_q - 1) / s.sk_q);
+        }
+    }
+    s.partial_bytes = 0;
+    if (s.sk_tiles > 0) {
+        s.sk_chunks = (s.sk_tiles * KT + s.sk_q - 1) / s.sk_q;
+        s.sk_slots = (int)((s.sk_q + KT - 2) / KT + 1);
+        s.partial_bytes = (size_t)s.sk_chunks * s.sk_slots * 32 * NTHREADS * sizeof(double2);
+    }
+    const int64_t units = std::max<int64_t>(std::min<int64_t>(s.dp_tiles, slots), std::min<int64_t>(s.sk_chunks, slots));
+    s.grid = (int)std::max<int64_t>(1, units);
+    return s;
+}
+
 cudaError_t encode_gemm_maps(const GemmDesc &g, GemmTensorMaps *maps)
 {
     // a strided dimension of extent 1 still needs a legal stride: ld >= 1 always holds here
@@ -373,39 +552,35 @@ cudaError_t encode_gemm_maps(const GemmDesc &g, GemmTensorMaps *maps)
 cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps, cudaStream_t stream,
                                    int64_t *launches)
 {
+    const GemmSchedule sc = gemm_schedule(g.M, g.N, g.K, g.splitk);
     GemmParams p;
     p.M = g.M; p.N = g.N; p.K = g.K;
-    p.mt = (int)((g.M + BM - 1) / BM);
-    p.nt = (int)((g.N + BN - 1) / BN);
+    p.mblocks = (int)((g.M + 7) / 8);
+    p.nblocks = (int)((g.N + 7) / 8);
+    p.mt = sc.mt; p.nt = sc.nt;
     p.gn = p.nt <= 24 ? p.nt : 16;
-    p.ktiles = (int)((g.K + BK - 1) / BK);
-    p.splits = g.splits < 1 ? 1 : g.splits;
-    if (p.splits > p.ktiles) p.splits = p.ktiles;
-    p.ktiles_per_split = (p.ktiles + p.splits - 1) / p.splits;
-    p.splits = (p.ktiles + p.ktiles_per_split - 1) / p.ktiles_per_split;   // no empty slices
+    p.ktiles = sc.ktiles;
+    p.klast_steps = (int)((g.K - (int64_t)(sc.ktiles - 1) * BK + 3) / 4);
+    p.dp_tiles = sc.dp_tiles; p.sk_tiles = sc.sk_tiles; p.sk_chunks = sc.sk_chunks;
+    p.sk_q = sc.sk_q; p.sk_slots = sc.sk_slots;
     p.D = (double2 *)g.D;
     p.offM = (const long long *)g.offM;
     p.offN = (const long long *)g.offN;
     p.alpha_re = g.alpha_re; p.alpha_im = g.alpha_im;
     p.accumulate = g.accumulate ? 1 : 0;
     p.partial = (double2 *)g.partial;
-    if (p.splits > 1 && !p.partial) return cudaErrorInvalidValue;
-    dim3 grid((unsigned)((long long)p.mt * p.nt), 1, (unsigned)p.splits);
+    if (sc.partial_bytes && !p.partial) return cudaErrorInvalidValue;
     cudaError_t e;
     if (g.a_kmajor)
-        e = g.b_kmajor ? launch_variant<true, true>(maps, p, grid, stream)
-                       : launch_variant<true, false>(maps, p, grid, stream);
+        e = g.b_kmajor ? launch_variant<true, true>(maps, p, sc.grid, stream)
+                       : launch_variant<true, false>(maps, p, sc.grid, stream);
     else
-        e = g.b_kmajor ? launch_variant<false, true>(maps, p, grid, stream)
-                       : launch_variant<false, false>(maps, p, grid, stream);
+        e = g.b_kmajor ? launch_variant<false, true>(maps, p, sc.grid, stream)
+                       : launch_variant<false, false>(maps, p, sc.grid, stream);
     if (e != cudaSuccess) return e;
     if (launches) ++*launches;
-    if (p.splits > 1) {
-        const long long total = g.M * g.N;
-        int blocks = (int)((total + 255) / 256);
-        if (blocks > 148 * 8) blocks = 148 * 8;
-        splitk_reduce_kernel<<<blocks, 256, 0, stream>>>(p.partial, p.splits, p.M, p.N, p.D, p.offM, p.offN,
-                                                         p.alpha_re, p.alpha_im, p.accumulate);
+    if (sc.sk_tiles > 0) {
+        zgemm_fixup_kernel<<<dim3((unsigned)sc.sk_tiles, 8), NTHREADS, 0, stream>>>(p);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
         if (launches) ++*launches;
