@@ -25,6 +25,8 @@
 //     them in fixed order (deterministic, no atomics) and applies the same scatter.
 #include "kernels.h"
 
+#include <algorithm>
+#include <cstdlib>
 #include <mutex>
 
 namespace tcb {
@@ -32,7 +34,7 @@ namespace tcb {
 namespace {
 
 constexpr int BM = kGemmBM, BN = kGemmBN, BK = kGemmBK;
-constexpr int STAGES = 6;
+constexpr int STAGES = 4;
 constexpr int kNumSMs = 148;            // B200; the persistent grid is 2 CTAs per SM
 constexpr int A_BYTES = BM * BK * 16;   // 8 KB
 constexpr int B_BYTES = BN * BK * 16;   // 8 KB
@@ -43,6 +45,8 @@ constexpr int NTHREADS = 128;
 struct GemmParams {
     long long M, N, K;
     int mblocks, nblocks;          // ceil(M / 8), ceil(N / 8): the 8-row / 8-column DMMA blocks
+    int mpair_base, mpair_extra;   // block pairs per M tile: base, and one more for the first `extra` tiles
+    int npair_base, npair_extra;
     int mt, nt, gn;                // tile grid, column-group width of the tile order
     int ktiles, klast_steps;       // ceil(K / BK); k-steps of 4 in the last k-tile (1 or 2)
     long long dp_tiles;            // tiles [0, dp_tiles) are computed whole, tile c + w * grid by CTA c
@@ -157,33 +161,37 @@ struct SegmentIter {
 
 // Tile order: groups of `gn` tile-columns, n fastest inside a group (concurrent CTAs form a near-square block of
 // the output, so A row panels and B column panels are shared through L2).  The 8-wide DMMA blocks of M and N are
-// dealt evenly to the tiles (N = 400 -> 7 tiles of 7,7,7,7,7,7,8 blocks instead of six full tiles and a sliver).
+// dealt to the tiles evenly and IN PAIRS (N = 400 = 50 blocks -> 7 tiles of 8,8,8,8,6,6,6 blocks instead of six
+// full tiles and a sliver), so that the two warp rows / columns of a CTA get the same number of blocks and the
+// four sub-partitions' DMMA pipes carry the same load.
 struct TileGeom {
     int m0, n0;          // element origin
     int mb, nb;          // blocks in this tile (<= 8 each)
 };
-__device__ __forceinline__ TileGeom tile_geom(const GemmParams &p, long long tile)
+__device__ __forceinline__ TileGeom tile_geom(const GemmParams &p, unsigned tile)
 {
-    const long long group_sz = (long long)p.gn * p.mt;
-    const int g = (int)(tile / group_sz), rem = (int)(tile % group_sz);
-    const int n0t = g * p.gn;
-    const int gw = min(p.gn, p.nt - n0t);
-    const int tm = rem / gw, tn = n0t + rem % gw;
-    const int mb0 = (int)((long long)tm * p.mblocks / p.mt), mb1 = (int)((long long)(tm + 1) * p.mblocks / p.mt);
-    const int nb0 = (int)((long long)tn * p.nblocks / p.nt), nb1 = (int)((long long)(tn + 1) * p.nblocks / p.nt);
+    const unsigned group_sz = (unsigned)p.gn * (unsigned)p.mt;
+    const unsigned g = tile / group_sz, rem = tile - g * group_sz;
+    const int n0t = (int)g * p.gn;
+    const unsigned gw = (unsigned)min(p.gn, p.nt - n0t);
+    const int tm = (int)(rem / gw), tn = n0t + (int)(rem - (rem / gw) * gw);
+    // tile t of a dim owns pairs [t * base + min(t, extra), ...) -- base/extra precomputed on the host
+    const int mp0 = tm * p.mpair_base + min(tm, p.mpair_extra), mp1 = mp0 + p.mpair_base + (tm < p.mpair_extra ? 1 : 0);
+    const int np0 = tn * p.npair_base + min(tn, p.npair_extra), np1 = np0 + p.npair_base + (tn < p.npair_extra ? 1 : 0);
     TileGeom t;
-    t.m0 = mb0 * 8; t.n0 = nb0 * 8; t.mb = mb1 - mb0; t.nb = nb1 - nb0;
+    t.m0 = mp0 * 16; t.n0 = np0 * 16;
+    t.mb = min(2 * mp1, p.mblocks) - 2 * mp0;
+    t.nb = min(2 * np1, p.nblocks) - 2 * np0;
     return t;
 }
-// The two warp rows (columns) of a CTA split a tile's blocks ceil/floor; `flip` (the parity of the CTA's wave,
-// i.e. of the other CTA resident on the same SM) hands the larger half to the other pair of sub-partitions.
+// The two warp rows (columns) of a CTA split a tile's blocks ceil/floor (equal unless the last tile is odd).
 struct WarpGeom {
     int moff, mcnt, noff, ncnt;      // in blocks, relative to the tile origin
 };
-__device__ __forceinline__ WarpGeom warp_geom(const TileGeom &t, int warp_m, int warp_n, int flip)
+__device__ __forceinline__ WarpGeom warp_geom(const TileGeom &t, int warp_m, int warp_n)
 {
     WarpGeom w;
-    const int mh = (t.mb + 1 - flip) / 2, nh = (t.nb + 1 - flip) / 2;      // blocks of warp row / column 0
+    const int mh = (t.mb + 1) / 2, nh = (t.nb + 1) / 2;      // blocks of warp row / column 0
     w.moff = warp_m ? mh : 0; w.mcnt = warp_m ? t.mb - mh : mh;
     w.noff = warp_n ? nh : 0; w.ncnt = warp_n ? t.nb - nh : nh;
     return w;
@@ -209,7 +217,12 @@ __device__ __forceinline__ void store_fragment(const GemmParams &p, const double
             const long long n = nw + j * 8 + h * 4;
             on[j][h] = (j < w.ncnt && n < p.N) ? p.offN[n] : -1;
         }
+    // The plain FP64 pipe shares its datapath with DMMA: every DMUL/DFMA here queues behind the other resident
+    // CTA's tensor work (ncu: 10 % of all stall samples of the K = 60 T3 contraction sat on the alpha multiply).
+    // So the scaling does the least arithmetic alpha allows: none for alpha = 1, one FMA per component for real
+    // alpha (fused with the accumulate), the full complex product only for complex alpha.
     const double ar = p.alpha_re, ai = p.alpha_im;
+    const int mode = (ai != 0.0) ? 2 : (ar != 1.0 ? 1 : 0);
 #pragma unroll
     for (int j = 0; j < 4; ++j)
 #pragma unroll
@@ -220,11 +233,16 @@ __device__ __forceinline__ void store_fragment(const GemmParams &p, const double
                 if (om[i] < 0) continue;
                 double2 *dst = p.D + om[i] + on[j][h];
                 const double xr = cr[i][j][h], xi = ci[i][j][h];
-                double2 v = make_double2(ar * xr - ai * xi, ar * xi + ai * xr);
+                double2 v;
                 if (p.accumulate) {
                     const double2 d = *dst;
-                    v.x += d.x;
-                    v.y += d.y;
+                    if (mode == 0) v = make_double2(d.x + xr, d.y + xi);
+                    else if (mode == 1) v = make_double2(fma(ar, xr, d.x), fma(ar, xi, d.y));
+                    else v = make_double2(fma(ar, xr, fma(-ai, xi, d.x)), fma(ar, xi, fma(ai, xr, d.y)));
+                } else {
+                    if (mode == 0) v = make_double2(xr, xi);
+                    else if (mode == 1) v = make_double2(ar * xr, ar * xi);
+                    else v = make_double2(fma(ar, xr, -ai * xi), fma(ar, xi, ai * xr));
                 }
                 *dst = v;
             }
@@ -270,7 +288,6 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int warp_m = warp & 1, warp_n = warp >> 1;
-    const int flip = (blockIdx.x / kNumSMs) & 1;
 
     if (tid == 0) {
         for (int s = 0; s < STAGES; ++s) {
@@ -290,10 +307,11 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     int pk = 0, pm0 = 0, pn0 = 0;
     bool pvalid = false;
     int pstage = 0;
+    uint32_t pphase = 0;                // parity of the ring round the producer is filling
     auto producer_advance = [&]() {
         pvalid = pit.next(p, &pseg);
         if (pvalid) {
-            const TileGeom t = tile_geom(p, pseg.tile);
+            const TileGeom t = tile_geom(p, (unsigned)pseg.tile);
             pm0 = t.m0; pn0 = t.n0; pk = pseg.kb;
         }
     };
@@ -314,7 +332,7 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 #pragma unroll
             for (int j = 0; j < BN / 8; ++j) tma_load_2d(sB + j * 1024, &tmB, 2 * (pn0 + 8 * j), k0, bar);
         }
-        if (++pstage == STAGES) pstage = 0;
+        if (++pstage == STAGES) { pstage = 0; pphase ^= 1; }
         if (++pk == pseg.ke) producer_advance();
     };
     if (tid == 0) {
@@ -341,9 +359,8 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     uint32_t phase = 0;
     long long done = 0;                 // k-tiles consumed by this CTA so far
     while (cit.next(p, &seg)) {
-        const TileGeom tg = tile_geom(p, seg.tile);
-        // tiles cut along K are summed fragment-wise by the fix-up kernel: every CTA must split them alike
-        const WarpGeom wg = warp_geom(tg, warp_m, warp_n, seg.slot < 0 ? flip : 0);
+        const TileGeom tg = tile_geom(p, (unsigned)seg.tile);
+        const WarpGeom wg = warp_geom(tg, warp_m, warp_n);
 
         double cr[4][4][2], ci[4][4][2];
 #pragma unroll
@@ -356,9 +373,10 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 
         for (int kt = seg.kb; kt < seg.ke; ++kt, ++done) {
             if (tid == 0 && done >= 1 && pvalid) {
-                // refill the stage consumed in the previous iteration (the other warps had a whole k-tile to release it)
-                const int sp = stage == 0 ? STAGES - 1 : stage - 1;
-                mbar_wait(bar_base + 8 * (STAGES + sp), (stage == 0 ? phase ^ 1 : phase));
+                // refill the stage consumed in the previous iteration (the other warps had a whole k-tile to
+                // release it).  A non-blocking variant (mbarrier.test_wait, refill whatever is free) measured 7 %
+                // slower: the wait keeps the four warps of a CTA in step, which the shared DMMA pipe prefers.
+                mbar_wait(bar_base + 8 * (STAGES + pstage), pphase ^ 1);
                 issue();
             }
             mbar_wait(bar_base + 8 * stage, phase);
@@ -407,8 +425,8 @@ __global__ void __launch_bounds__(NTHREADS) zgemm_fixup_kernel(const __grid_cons
     if (ch_lo == ch_hi) return;                       // computed whole by one CTA, already in D
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int j = blockIdx.y >> 1, h = blockIdx.y & 1;
-    const TileGeom tg = tile_geom(p, p.dp_tiles + tl);
-    const WarpGeom wg = warp_geom(tg, warp & 1, warp >> 1, 0);
+    const TileGeom tg = tile_geom(p, (unsigned)(p.dp_tiles + tl));
+    const WarpGeom wg = warp_geom(tg, warp & 1, warp >> 1);
     if (j >= wg.ncnt) return;
     double sr[4] = {0.0, 0.0, 0.0, 0.0}, si[4] = {0.0, 0.0, 0.0, 0.0};
     for (long long ch = ch_lo; ch <= ch_hi; ++ch) {
@@ -558,6 +576,10 @@ cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps
     p.mblocks = (int)((g.M + 7) / 8);
     p.nblocks = (int)((g.N + 7) / 8);
     p.mt = sc.mt; p.nt = sc.nt;
+    if ((int64_t)sc.mt * sc.nt >= (1LL << 31)) return cudaErrorInvalidValue;      // 32-bit tile index
+    const int mpairs = (p.mblocks + 1) / 2, npairs = (p.nblocks + 1) / 2;
+    p.mpair_base = mpairs / sc.mt; p.mpair_extra = mpairs % sc.mt;
+    p.npair_base = npairs / sc.nt; p.npair_extra = npairs % sc.nt;
     p.gn = p.nt <= 24 ? p.nt : 16;
     p.ktiles = sc.ktiles;
     p.klast_steps = (int)((g.K - (int64_t)(sc.ktiles - 1) * BK + 3) / 4);
