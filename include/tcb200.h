@@ -69,8 +69,10 @@ typedef struct { double re, im; } tcb_c128;
 int tcb_ctx_create(tcb_ctx **ctx, int device, void *cuda_stream, size_t workspace_bytes);
 int tcb_ctx_destroy(tcb_ctx *ctx);
 /* keys: "splitk" = "auto" | "off" | <integer number of splits>;  "epilogue" = "auto" | "fused" | "twopass";
- *       "permute_operands" = "auto" | "always"  (A/B testing of plans);  "kernel_timing" = "on" | "off"
- *       (see tcb_kernel_stats);  unknown key -> TCB_EINVAL. */
+ *       "permute_operands" = "auto" | "always"  (A/B testing of plans);  "gemm_deal" = "dynamic" | "static"
+ *       (how the GEMM's tiles and stream-K chunks reach the CTAs: claimed from a counter, or dealt round-robin;
+ *       the result is the same bit for bit);  "kernel_timing" = "on" | "off" (see tcb_kernel_stats);
+ *       unknown key -> TCB_EINVAL. */
 int tcb_ctx_set_option(tcb_ctx *ctx, const char *key, const char *value);
 /* Blocks until everything enqueued so far has finished (the paper's barrier). */
 int tcb_sync(tcb_ctx *ctx);

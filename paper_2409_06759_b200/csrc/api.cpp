@@ -446,10 +446,11 @@ int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor
     const size_t bytesA = P.a.permuted ? align_up((size_t)P.a.elems * 16, 1024) : 0;
     const size_t bytesB = P.b.permuted ? align_up((size_t)P.b.elems * 16, 1024) : 0;
     const size_t bytesP = align_up(P.partial_bytes, 1024);
+    const size_t bytesC = 1024;                 // work counters of the GEMM's dynamic deal
     char *ws = nullptr;
-    if (bytesA + bytesB + bytesP) {
+    {
         void *p;
-        rc = workspace(ctx, bytesA + bytesB + bytesP, &p);
+        rc = workspace(ctx, bytesA + bytesB + bytesP + bytesC, &p);
         if (rc) return rc;
         ws = (char *)p;
     }
@@ -478,6 +479,7 @@ int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor
     g.accumulate = P.accumulate;
     g.splitk = P.splitk;
     g.partial = bytesP ? ws + bytesA + bytesB : nullptr;
+    g.counters = ctx->opt.static_deal ? nullptr : ws + bytesA + bytesB + bytesP;
     TimedLaunch tl(ctx, kClsZgemm, P.flops, P.bytes);
     TCB_CUDA(ctx, launch_zgemm(g, ctx->stream, &ctx->launches));
     return TCB_OK;
@@ -520,6 +522,12 @@ static int apply_option(PlanOptions &opt, const std::string &k, const std::strin
         if (v == "auto") opt.permute_always = false;
         else if (v == "always") opt.permute_always = true;
         else { *why = "permute_operands: expected auto or always"; return TCB_EINVAL; }
+        return TCB_OK;
+    }
+    if (k == "gemm_deal") {
+        if (v == "dynamic") opt.static_deal = false;
+        else if (v == "static") opt.static_deal = true;
+        else { *why = "gemm_deal: expected dynamic or static"; return TCB_EINVAL; }
         return TCB_OK;
     }
     *why = "unknown option " + k;

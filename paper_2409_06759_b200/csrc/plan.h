@@ -21,6 +21,7 @@ struct PlanOptions {
     int splitk = 0;               // 0 = auto, 1 = off, n > 1 = forced
     int epilogue = 0;             // 0 = auto, 1 = fused, 2 = two-pass (reserved)
     bool permute_always = false;  // A/B testing: permute both operands even when they are matrix-shaped
+    bool static_deal = false;     // A/B testing: GEMM work dealt statically (tile c + w * grid) instead of claimed
 };
 
 // canonical transposition descriptor without pointers (extent-1 dropped, neighbours fused, sorted by input stride)

@@ -39,7 +39,8 @@ constexpr int kNumSMs = 148;            // B200; the persistent grid is 2 CTAs p
 constexpr int A_BYTES = BM * BK * 16;   // 8 KB
 constexpr int B_BYTES = BN * BK * 16;   // 8 KB
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 128 /*barriers*/;
+constexpr int kQueue = 8;               // segment queue entries (producer is <= STAGES + 1 segments ahead)
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 128 /*barriers*/ + 256 /*segment queue*/;
 constexpr int NTHREADS = 128;
 
 struct GemmParams {
@@ -59,6 +60,7 @@ struct GemmParams {
     double alpha_re, alpha_im;
     int accumulate;
     double2 *partial;              // [slot][32][128] raw accumulator fragments
+    unsigned long long *counters;  // [2] work counters (whole tiles, stream-K chunks), zero at launch; null: static deal
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -121,22 +123,36 @@ struct Segment {
     long long tile, slot;
     int kb, ke;
 };
+// With work counters the deal is dynamic: a CTA claims its next whole tile, and then its next stream-K chunk, by
+// atomicAdd, one claim ahead of use (the atomic's latency hides behind a whole segment).  Tiles then cost what they
+// cost (ragged tiles are cheaper, SMs differ in speed) and the chip still finishes together; the chunks are small
+// (about three per CTA).  Which CTA computes what changes from run to run, the arithmetic does not: a tile's chunks
+// are fixed k-ranges and are summed in k order.
 struct SegmentIter {
-    long long w, ch;
+    long long w, ch, chn;
     int sub, phase;
-    __device__ __forceinline__ void init()
+    unsigned long long *cnt;
+    __device__ __forceinline__ long long claim(int which, long long fallback)
     {
-        w = blockIdx.x; ch = blockIdx.x; sub = 0; phase = 0;
+        return cnt ? (long long)atomicAdd(cnt + which, 1ULL) : fallback;
+    }
+    __device__ __forceinline__ void init(const GemmParams &p)
+    {
+        cnt = p.counters;
+        w = claim(0, blockIdx.x);
+        ch = -1; chn = -1; sub = 0; phase = 0;
     }
     __device__ __forceinline__ bool next(const GemmParams &p, Segment *s)
     {
         if (phase == 0) {
             if (w < p.dp_tiles) {
                 s->tile = w; s->slot = -1; s->kb = 0; s->ke = p.ktiles;
-                w += gridDim.x;
+                w = claim(0, w + gridDim.x);
                 return true;
             }
             phase = 1;
+            ch = claim(1, blockIdx.x);
+            chn = claim(1, ch + gridDim.x);
         }
         const long long total = p.sk_tiles * p.ktiles;
         while (ch < p.sk_chunks) {
@@ -152,7 +168,8 @@ struct SegmentIter {
                 ++sub;
                 return true;
             }
-            ch += gridDim.x;
+            ch = chn;
+            chn = claim(1, ch + gridDim.x);
             sub = 0;
         }
         return false;
@@ -250,13 +267,15 @@ __device__ __forceinline__ void store_fragment(const GemmParams &p, const double
 }
 
 // one k-tile (two k-steps of 4) of a warp tile of MC x NC blocks: complex product = 4 real DMMAs per block pair
-template <int MC, int NC>
+// (KS = 1: the last k-tile of a K with <= 4 valid entries in it).  Straight-line code: a run-time test on the
+// k-step would end the basic block and keep the second step's LDS from being hoisted over the first step's DMMAs.
+template <int MC, int NC, int KS>
 __device__ __forceinline__ void mma_ktile(double (&cr)[4][4][2], double (&ci)[4][4][2], uint32_t sA, uint32_t sB,
-                                          const uint32_t (&offA)[2], const uint32_t (&offB)[2], int nks)
+                                          const uint32_t (&offA)[2], const uint32_t (&offB)[2])
 {
 #pragma unroll
-    for (int ks = 0; ks < 2; ++ks) {
-        if (ks < nks) {
+    for (int ks = 0; ks < KS; ++ks) {
+        {
             double2 a[MC], b[NC];
 #pragma unroll
             for (int i = 0; i < MC; ++i) a[i] = lds128(sA + i * 1024 + offA[ks]);
@@ -297,6 +316,7 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
+        *reinterpret_cast<volatile int *>(smem_raw + (bar_base - smem_u32(smem_raw)) + 128 + kQueue * sizeof(Segment)) = 0;
     }
     __syncthreads();
 
@@ -308,8 +328,18 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     bool pvalid = false;
     int pstage = 0;
     uint32_t pphase = 0;                // parity of the ring round the producer is filling
+    // segment queue: the producer decides (or claims) what this CTA computes and publishes every segment here
+    // before its first operand load; the consumers pop them in order.  kQueue > STAGES + 1 entries suffice.
+    Segment *q_seg = reinterpret_cast<Segment *>(smem_raw + (bar_base - smem_u32(smem_raw)) + 128);
+    volatile int *q_pub = reinterpret_cast<volatile int *>(q_seg + kQueue);
+    int npub = 0;
     auto producer_advance = [&]() {
         pvalid = pit.next(p, &pseg);
+        Segment out = pseg;
+        if (!pvalid) out.tile = -1;                 // terminator
+        q_seg[npub % kQueue] = out;
+        __threadfence_block();
+        *q_pub = ++npub;
         if (pvalid) {
             const TileGeom t = tile_geom(p, (unsigned)pseg.tile);
             pm0 = t.m0; pn0 = t.n0; pk = pseg.kb;
@@ -336,7 +366,7 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         if (++pk == pseg.ke) producer_advance();
     };
     if (tid == 0) {
-        pit.init();
+        pit.init(p);
         producer_advance();
         for (int s = 0; s < STAGES && pvalid; ++s) issue();
     }
@@ -352,13 +382,17 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         offB[ks] = B_KMAJOR ? (rowmap * 128 + ((k ^ rowmap) * 16)) : (k * 128 + ((rowmap ^ k) * 16));
     }
 
-    SegmentIter cit;
     Segment seg;
-    cit.init();
+    int npop = 0;
     int stage = 0;
     uint32_t phase = 0;
     long long done = 0;                 // k-tiles consumed by this CTA so far
-    while (cit.next(p, &seg)) {
+    for (;;) {
+        while (*q_pub <= npop) { }
+        __threadfence_block();
+        seg = q_seg[npop % kQueue];
+        ++npop;
+        if (seg.tile < 0) break;
         const TileGeom tg = tile_geom(p, (unsigned)seg.tile);
         const WarpGeom wg = warp_geom(tg, warp_m, warp_n);
 
@@ -384,7 +418,10 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             const uint32_t sB = smem_base + stage * STAGE_BYTES + A_BYTES + wg.noff * 1024;
             const int nks = (kt == p.ktiles - 1) ? p.klast_steps : 2;
             switch (wg.mcnt * 5 + wg.ncnt) {      // only the blocks that exist are multiplied (no tensor work on padding)
-#define TCB_CASE(MC, NC) case MC * 5 + NC: mma_ktile<MC, NC>(cr, ci, sA, sB, offA, offB, nks); break;
+#define TCB_CASE(MC, NC) case MC * 5 + NC:                                              \
+    if (nks == 2) mma_ktile<MC, NC, 2>(cr, ci, sA, sB, offA, offB);                        \
+    else mma_ktile<MC, NC, 1>(cr, ci, sA, sB, offA, offB);                                 \
+    break;
                 TCB_CASE(4, 4) TCB_CASE(4, 3) TCB_CASE(4, 2) TCB_CASE(4, 1)
                 TCB_CASE(3, 4) TCB_CASE(3, 3) TCB_CASE(3, 2) TCB_CASE(3, 1)
                 TCB_CASE(2, 4) TCB_CASE(2, 3) TCB_CASE(2, 2) TCB_CASE(2, 1)
@@ -543,7 +580,8 @@ GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk)
         // shorter than 8 k-tiles costs more in fix-up traffic than it saves
         if (rem > 0 && rem * KT / slots + 8 < KT * 9 / 10) {
             s.dp_tiles = tiles - rem; s.sk_tiles = rem;
-            const int64_t chunks = std::max<int64_t>(1, std::min<int64_t>(slots, rem * KT / 8));
+            // about three chunks per CTA: claimed dynamically, they even out what the whole tiles left uneven
+            const int64_t chunks = std::max<int64_t>(1, std::min<int64_t>(3 * slots, rem * KT / 8));
             s.sk_q = (int)((rem * KT + chunks - 1) / chunks);
             if (s.dp_tiles == 0) s.splits = (int)((KT + s.sk_q - 1) / s.sk_q);
         }
@@ -591,6 +629,11 @@ cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps
     p.alpha_re = g.alpha_re; p.alpha_im = g.alpha_im;
     p.accumulate = g.accumulate ? 1 : 0;
     p.partial = (double2 *)g.partial;
+    p.counters = (unsigned long long *)g.counters;
+    if (p.counters) {
+        cudaError_t ce = cudaMemsetAsync(p.counters, 0, 2 * sizeof(unsigned long long), stream);
+        if (ce != cudaSuccess) return ce;
+    }
     if (sc.partial_bytes && !p.partial) return cudaErrorInvalidValue;
     cudaError_t e;
     if (g.a_kmajor)
