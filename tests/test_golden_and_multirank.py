@@ -1,0 +1,81 @@
+"""-m "not gpu": (1) the oracle's CCD equations against the paper's printed diagram count (tests/golden/, PAPER.md
+Table I); (2) the only cross-rank step of bench.py -- max over ranks of the device time, whole-job throughput --
+on two gloo ranks (the path does not shard: DESIGN.md "Multi-GPU: replicas only")."""
+import os
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+GOLDEN = os.path.join(ROOT, "tests", "golden", "paper_table1_diagram_counts.txt")
+
+
+def read_counts():
+    out = {}
+    for line in open(GOLDEN):
+        line = line.strip()
+        if line and not line.startswith("#"):
+            k, v = line.split()
+            out[k] = int(v)
+    return out
+
+
+def test_paper_table1_fixture_is_the_papers():
+    c = read_counts()
+    assert c == {"CCD": 11, "CCSD": 48, "CCSDT": 102, "CCSDTQ": 183, "CCSDTQP": 289}
+
+
+def test_oracle_ccd_term_count_matches_paper_table1():
+    """CCD has 11 diagrams = 10 doubles-amplitude terms + 1 energy term.  A dropped or duplicated term in
+    oracle/cc.py changes the count (and the Fock-space pin in test_oracle_cc.py catches a wrong one)."""
+    from oracle import cc
+    from paper_2409_06759_b200 import synth
+    o, v = 2, 3
+    n = o + v
+    rng = np.random.default_rng(1)
+    f = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+    f = f + f.conj().T
+    g = synth.tensor(7, 1, [n] * 4, antisym=((0, 1), (2, 3)), sigma=0.1, hermitian=True)
+    t = synth.tensor(7, 2, [v, v, o, o], antisym=((0, 1), (2, 3)))
+    _, _, n_amp, n_en = cc.ccd_residual_unfactorised(o, f, g, t)
+    assert n_amp + n_en == read_counts()["CCD"]
+    assert (n_amp, n_en) == (10, 1)
+
+
+def _rank_main(rank, world, port, q):
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    import bench
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    # rank r "measured" (10 + r) ms for the step and (30 - r) ms end to end
+    ms, e2e = bench.max_over_ranks([10.0 + rank, 30.0 - rank], dist, "cpu")
+    dist.barrier()
+    dist.destroy_process_group()
+    q.put((rank, ms, e2e))
+
+
+def test_two_rank_replicas_take_the_slowest_rank_time():
+    import torch.multiprocessing as mp
+    import socket
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_rank_main, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert got == [(0, 11.0, 30.0), (1, 11.0, 30.0)]
+    sys.path.insert(0, ROOT)
+    import bench
+    # whole-job value: both replicas' flops over the slowest rank's time
+    assert bench.job_throughput(2, 1e9, 11.0) == pytest.approx(2 * 1e9 / 11e-3 * 1e-9)
+    assert bench.max_over_ranks([1.0, 2.0], None, "cpu") == [1.0, 2.0]
