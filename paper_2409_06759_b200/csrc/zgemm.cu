@@ -124,13 +124,14 @@ struct Segment {
     int kb, ke;
 };
 // With work counters the deal is dynamic: a CTA claims its next whole tile, and then its next stream-K chunk, by
-// atomicAdd, one claim ahead of use (the atomic's latency hides behind a whole segment).  Tiles then cost what they
+// atomicAdd.  Tiles then cost what they
 // cost (ragged tiles are cheaper, SMs differ in speed) and the chip still finishes together; the chunks are small
 // (about three per CTA).  Which CTA computes what changes from run to run, the arithmetic does not: a tile's chunks
 // are fixed k-ranges and are summed in k order.
 struct SegmentIter {
-    long long w, ch, chn;
+    long long w, wn, ch;
     int sub, phase;
+    bool ahead;                      // claim whole tiles one ahead of use (only when there are plenty)
     unsigned long long *cnt;
     __device__ __forceinline__ long long claim(int which, long long fallback)
     {
@@ -139,20 +140,24 @@ struct SegmentIter {
     __device__ __forceinline__ void init(const GemmParams &p)
     {
         cnt = p.counters;
+        // with many tiles per CTA the claim for the next tile is issued a whole tile early, and its latency never
+        // shows; with few, a tile held in reserve by a busy CTA is a tile an idle CTA cannot take
+        ahead = cnt && p.dp_tiles >= 8LL * gridDim.x;
         w = claim(0, blockIdx.x);
-        ch = -1; chn = -1; sub = 0; phase = 0;
+        wn = ahead ? claim(0, 0) : -1;
+        ch = -1; sub = 0; phase = 0;
     }
     __device__ __forceinline__ bool next(const GemmParams &p, Segment *s)
     {
         if (phase == 0) {
             if (w < p.dp_tiles) {
                 s->tile = w; s->slot = -1; s->kb = 0; s->ke = p.ktiles;
-                w = claim(0, w + gridDim.x);
+                if (ahead) { w = wn; wn = claim(0, 0); }
+                else w = claim(0, w + gridDim.x);
                 return true;
             }
             phase = 1;
             ch = claim(1, blockIdx.x);
-            chn = claim(1, ch + gridDim.x);
         }
         const long long total = p.sk_tiles * p.ktiles;
         while (ch < p.sk_chunks) {
@@ -168,8 +173,7 @@ struct SegmentIter {
                 ++sub;
                 return true;
             }
-            ch = chn;
-            chn = claim(1, ch + gridDim.x);
+            ch = claim(1, ch + gridDim.x);
             sub = 0;
         }
         return false;
@@ -466,16 +470,26 @@ __global__ void __launch_bounds__(NTHREADS) zgemm_fixup_kernel(const __grid_cons
     const WarpGeom wg = warp_geom(tg, warp & 1, warp >> 1);
     if (j >= wg.ncnt) return;
     double sr[4] = {0.0, 0.0, 0.0, 0.0}, si[4] = {0.0, 0.0, 0.0, 0.0};
-    for (long long ch = ch_lo; ch <= ch_hi; ++ch) {
-        const long long first = (ch * p.sk_q) / p.ktiles;
-        const double2 *P = p.partial + (ch * p.sk_slots + (tl - first)) * (32LL * NTHREADS) + tid;
+    // chunks in k order, four at a time: the 16 loads of a batch are independent, the additions keep their order
+    for (long long ch0 = ch_lo; ch0 <= ch_hi; ch0 += 4) {
+        double2 v[4][4];
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
-            if (i < wg.mcnt) {
-                const double2 v = P[((i * 4 + j) * 2 + h) * NTHREADS];
-                sr[i] += v.x;
-                si[i] += v.y;
-            }
+        for (int u = 0; u < 4; ++u) {
+            const long long ch = ch0 + u;
+            const long long first = (ch * p.sk_q) / p.ktiles;
+            const double2 *P = p.partial + (ch * p.sk_slots + (tl - first)) * (32LL * NTHREADS) + tid;
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                if (ch <= ch_hi && i < wg.mcnt) v[u][i] = P[((i * 4 + j) * 2 + h) * NTHREADS];
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                if (ch0 + u <= ch_hi && i < wg.mcnt) {
+                    sr[i] += v[u][i].x;
+                    si[i] += v[u][i].y;
+                }
     }
     const int r = lane >> 2, c = lane & 3;
     const int rowmap = (r >> 1) + 4 * (r & 1);
@@ -580,8 +594,11 @@ GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk)
         // shorter than 8 k-tiles costs more in fix-up traffic than it saves
         if (rem > 0 && rem * KT / slots + 8 < KT * 9 / 10) {
             s.dp_tiles = tiles - rem; s.sk_tiles = rem;
-            // about three chunks per CTA: claimed dynamically, they even out what the whole tiles left uneven
-            const int64_t chunks = std::max<int64_t>(1, std::min<int64_t>(3 * slots, rem * KT / 8));
+            // about three chunks per CTA when whole tiles came first: claimed dynamically, they even out what the
+            // tiles left uneven.  With nothing but chunks (skinny M x N) one per CTA is already even, and a tile's
+            // chunks are summed one after the other by the fix-up: the fewer the better.
+            const int64_t per_cta = tiles >= slots ? 3 : 1;
+            const int64_t chunks = std::max<int64_t>(1, std::min<int64_t>(per_cta * slots, rem * KT / 8));
             s.sk_q = (int)((rem * KT + chunks - 1) / chunks);
             if (s.dp_tiles == 0) s.splits = (int)((KT + s.sk_q - 1) / s.sk_q);
         }
