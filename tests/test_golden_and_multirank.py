@@ -79,3 +79,16 @@ def test_two_rank_replicas_take_the_slowest_rank_time():
     # whole-job value: both replicas' flops over the slowest rank's time
     assert bench.job_throughput(2, 1e9, 11.0) == pytest.approx(2 * 1e9 / 11e-3 * 1e-9)
     assert bench.max_over_ranks([1.0, 2.0], None, "cpu") == [1.0, 2.0]
+
+
+def test_transpose_benchmark_sample_holds_the_required_permutations():
+    """BASELINE.json configs[4]: 48 sampled rank-6 permutations; the sample is seeded and always contains the identity,
+    the reversal, the half swap and the six transpositions of P(a/bc), P(k/ij)."""
+    from paper_2409_06759_b200 import transpose_bench as tb
+    s = tb.rank6_sample()
+    assert len(s) == 48 and len(set(s)) == 48 and s == tb.rank6_sample()
+    assert all(sorted(p) == list(range(6)) for p in s)
+    for need in [(0, 1, 2, 3, 4, 5), (5, 4, 3, 2, 1, 0), (3, 4, 5, 0, 1, 2), (1, 0, 2, 3, 4, 5), (2, 1, 0, 3, 4, 5),
+                 (0, 1, 2, 5, 4, 3), (0, 1, 2, 3, 5, 4)]:
+        assert need in s
+    assert tb.expression((1, 0, 2, 3)) == "D(b,a,c,d)=L(a,b,c,d)"
