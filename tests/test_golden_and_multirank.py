@@ -92,3 +92,21 @@ def test_transpose_benchmark_sample_holds_the_required_permutations():
                  (0, 1, 2, 5, 4, 3), (0, 1, 2, 3, 5, 4)]:
         assert need in s
     assert tb.expression((1, 0, 2, 3)) == "D(b,a,c,d)=L(a,b,c,d)"
+
+
+def test_ccsd_contraction_list_is_well_formed():
+    """configs[4]: every expression of the CCSD stand-in list is a valid binary contraction for the host planner (labels
+    twice overall, extents by index type), and the permutation operators unroll into the signed output orders."""
+    from paper_2409_06759_b200 import ccsd_contractions as cl, binding
+    o, v = 3, 5
+    calls = cl.all_calls(o, v)
+    assert len(calls) == sum(2 ** len([p for p in ops.split(",") if p]) for _, ops in cl.CONTRACTIONS)
+    for e, sign, sd, sl, sr in calls:
+        plan = binding.plan_describe_host(e, sd, sl, sr)
+        d, _, l, r = cl.split(e)
+        assert plan["M"] * plan["N"] == int(np.prod(sd)) and sign in (1.0, -1.0)
+    orders = cl.output_orders("R2(a,b,i,j)+=T2(a,e,i,m)*Wmbej(m,b,e,j)", "ij,ab")
+    assert [(x[:12], s) for x, s in orders] == [("R2(a,b,i,j)+", 1.0), ("R2(a,b,j,i)+", -1.0), ("R2(b,a,i,j)+", -1.0),
+                                                ("R2(b,a,j,i)+", 1.0)]
+    kinds = {(p["K"] == 1, p["N"] == 1) for p in (binding.plan_describe_host(e, sd, sl, sr) for e, _, sd, sl, sr in calls)}
+    assert (True, False) in kinds and (False, True) in kinds          # the list holds an outer product and N = 1 cases

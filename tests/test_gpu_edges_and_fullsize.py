@@ -120,3 +120,24 @@ def test_fullsize_ccd_pp_ladder_sampled_columns(ctx):
     assert worst <= TOL
     for t in (V, T, R0):
         t.destroy()
+
+
+@pytest.mark.parametrize("o,v", [(3, 5), (4, 9)])
+def test_every_ccsd_contraction_in_every_emitted_output_order(ctx, o, v):
+    """BASELINE.json configs[4] (first half) at oracle-sized extents: all 32 binary contractions of the CCSD list, each in
+    every output index order its permutation operators unroll into (rank 2-4, K = 1 and N = 1 included)."""
+    from paper_2409_06759_b200 import ccsd_contractions as cl
+    rng = np.random.default_rng(o * 100 + v)
+    worst = 0.0
+    for e, sign, sd, sl, sr in cl.all_calls(o, v):
+        D, L, R = rc(rng, *sd), rc(rng, *sl), rc(rng, *sr)
+        dD, dL, dR = ctx.tensor_from_numpy(D), ctx.tensor_from_numpy(L), ctx.tensor_from_numpy(R)
+        ctx.contract(e, dD, dL, dR, 0.5 * sign)
+        got = ctx.tensor_download(dD)
+        ref, sn = oracle.contract(e, D, L, R, 0.5 * sign)
+        err = parity_error(got, ref, sn)
+        assert err <= TOL, (e, err)
+        worst = max(worst, err)
+        for t in (dD, dL, dR):
+            t.destroy()
+    assert worst <= TOL
