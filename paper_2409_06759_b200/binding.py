@@ -247,6 +247,12 @@ class Context:
         self._check(self.lib.tcb_tensor_download(self.handle, t.handle, out.ctypes.data_as(ctypes.c_void_p)))
         return out
 
+    def tensor_device_ptr(self, t):
+        """Device address of the tensor's storage (tcb_tensor_info)."""
+        ptr = ctypes.c_void_p()
+        self._check(self.lib.tcb_tensor_info(t.handle, None, None, ctypes.byref(ptr)))
+        return ptr.value
+
     def tensor_fill(self, t, value):
         self._check(self.lib.tcb_tensor_fill(self.handle, t.handle, _c(value)))
 
