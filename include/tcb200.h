@@ -142,6 +142,9 @@ int tcb_plan_describe_host(const char *expr, int rank_d, const int64_t *ext_d, i
 /* Register-resident mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4) loop on every SM for about `milliseconds`;
  * returns achieved TFLOP/s (512 flop per warp instruction).  The roofline denominator of the contraction. */
 int tcb_measure_fp64_tensor_peak(tcb_ctx *ctx, double milliseconds, double *tflops);
+/* The same for the plain FP64 pipe (register-resident DFMA chains, 2 flop per FMA and lane): on B200 the vector and
+ * the tensor FP64 rates are nominally equal; the pair of numbers shows what the tensor path buys. */
+int tcb_measure_fp64_vector_peak(tcb_ctx *ctx, double milliseconds, double *tflops);
 /* Milliseconds between two points of the context's stream: tcb_timer_start / tcb_timer_stop bracket the
  * calls in between with CUDA events on that stream; stop blocks and returns the elapsed time. */
 int tcb_timer_start(tcb_ctx *ctx);

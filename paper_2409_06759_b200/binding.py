@@ -42,7 +42,7 @@ ABI_SYMBOLS = [
     "tcb_ctx_create", "tcb_ctx_destroy", "tcb_ctx_set_option", "tcb_sync", "tcb_last_error", "tcb_strerror",
     "tcb_launch_count", "tcb_tensor_create", "tcb_tensor_wrap", "tcb_tensor_destroy", "tcb_tensor_info",
     "tcb_tensor_upload", "tcb_tensor_download", "tcb_tensor_fill", "tcb_contract", "tcb_add", "tcb_scale",
-    "tcb_permute", "tcb_permsum", "tcb_antisymmetrize", "tcb_plan_describe", "tcb_measure_fp64_tensor_peak",
+    "tcb_permute", "tcb_permsum", "tcb_antisymmetrize", "tcb_plan_describe", "tcb_measure_fp64_tensor_peak", "tcb_measure_fp64_vector_peak",
     "tcb_timer_start", "tcb_timer_stop", "tcb_kernel_stats", "tcb_kernel_stats_reset", "tcb_plan_describe_host", "tcbx_synth_normal", "tcbx_synth_index_linear",
     "tcbx_synth_mp2_amplitudes",
 ]
@@ -79,6 +79,7 @@ def load_library():
         "tcb_antisymmetrize": [vp, cp, vp, vp, c128],
         "tcb_plan_describe": [vp, cp, vp, vp, vp, ctypes.c_char_p, ctypes.c_size_t],
         "tcb_measure_fp64_tensor_peak": [vp, ctypes.c_double, ctypes.POINTER(ctypes.c_double)],
+        "tcb_measure_fp64_vector_peak": [vp, ctypes.c_double, ctypes.POINTER(ctypes.c_double)],
         "tcb_plan_describe_host": [cp, ctypes.c_int, i64p, ctypes.c_int, i64p, ctypes.c_int, i64p, cp, ctypes.c_char_p,
                                    ctypes.c_size_t, i64p, ctypes.c_size_t, i64p, ctypes.c_size_t],
         "tcb_timer_start": [vp],
@@ -288,6 +289,11 @@ class Context:
     def measure_fp64_tensor_peak(self, milliseconds=200.0):
         out = ctypes.c_double()
         self._check(self.lib.tcb_measure_fp64_tensor_peak(self.handle, float(milliseconds), ctypes.byref(out)))
+        return out.value
+
+    def measure_fp64_vector_peak(self, milliseconds=200.0):
+        out = ctypes.c_double()
+        self._check(self.lib.tcb_measure_fp64_vector_peak(self.handle, float(milliseconds), ctypes.byref(out)))
         return out.value
 
     def kernel_stats(self, kernel):

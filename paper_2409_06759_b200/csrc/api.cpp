@@ -764,6 +764,15 @@ int tcb_measure_fp64_tensor_peak(tcb_ctx *ctx, double milliseconds, double *tflo
     return TCB_OK;
 }
 
+int tcb_measure_fp64_vector_peak(tcb_ctx *ctx, double milliseconds, double *tflops)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!tflops) return TCB_EINVAL;
+    TCB_CUDA(ctx, run_dfma_peak(milliseconds, tflops, ctx->stream, &ctx->launches));
+    return TCB_OK;
+}
+
 int tcb_kernel_stats(tcb_ctx *ctx, const char *kernel, tcb_kernel_stat *out)
 {
     int rc = enter(ctx);

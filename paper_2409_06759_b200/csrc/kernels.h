@@ -84,5 +84,6 @@ cudaError_t launch_axpy(void *D, const void *L, int64_t n, double re, double im,
 
 // ---- measurement -------------------------------------------------------------------------------------------
 cudaError_t run_dmma_peak(double milliseconds, double *tflops, cudaStream_t stream, int64_t *launches);
+cudaError_t run_dfma_peak(double milliseconds, double *tflops, cudaStream_t stream, int64_t *launches);
 
 }  // namespace tcb
