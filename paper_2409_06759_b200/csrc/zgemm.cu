@@ -630,10 +630,11 @@ GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk)
         // shorter than 8 k-tiles costs more in fix-up traffic than it saves
         if (rem > 0 && rem * KT / slots + 8 < KT * 9 / 10) {
             s.dp_tiles = tiles - rem; s.sk_tiles = rem;
-            // about three chunks per CTA when whole tiles came first: claimed dynamically, they even out what the
-            // tiles left uneven.  With nothing but chunks (skinny M x N) one per CTA is already even, and a tile's
-            // chunks are summed one after the other by the fix-up: the fewer the better.
-            const int64_t per_cta = tiles >= slots ? 3 : 1;
+            // about three chunks per CTA, claimed dynamically: they even out what whole tiles left uneven and what
+            // ragged tiles make uneven among the chunks themselves (a 6 x 6-block tile costs half an 8 x 8 one).
+            // With very few tiles (skinny M x N) one chunk per CTA: a tile's chunks are summed one after the other
+            // by the fix-up, the fewer the better.
+            const int64_t per_cta = tiles >= 16 ? 3 : 1;      // <= ~55 chunks per tile for the fix-up to sum
             const int64_t chunks = std::max<int64_t>(1, std::min<int64_t>(per_cta * slots, rem * KT / 8));
             s.sk_q = (int)((rem * KT + chunks - 1) / chunks);
             if (s.dp_tiles == 0) s.splits = (int)((KT + s.sk_q - 1) / s.sk_q);
