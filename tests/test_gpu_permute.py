@@ -164,3 +164,46 @@ def test_device_generator_matches_host_generator(ctx):
     dI = ctx.tensor_create((7, 3, 5))
     ctx.synth_index_linear(dI)
     assert ctx.tensor_download(dI).tobytes() == synth.index_linear_tensor((7, 3, 5)).tobytes()
+
+
+@pytest.mark.parametrize("shape,spec,nterms", [
+    ((12, 12, 12, 6, 6, 6), "P(a/bc)P(k/ij):R(a,b,c,i,j,k)+=X(a,b,c,i,j,k)", 9),     # cube 4 x 4 x 2, 9 terms
+    ((12, 12, 12, 6, 6, 6), "P(a/bc):R(a,b,c,i,j,k)+=X(a,b,c,i,j,k)", 3),            # 3 terms inside a slab
+    ((12, 12, 12, 6, 6, 6), "P(k/ij):R(a,b,c,i,j,k)=X(a,b,c,i,j,k)", 3),             # one unit-stride index, beta = 0
+    ((64, 64, 8, 8), "P(ij)P(ab):R(a,b,i,j)+=X(a,b,i,j)", 4),                        # cube 8 x 4, all 32 lanes
+    ((30, 30, 18, 18), "P(ab):R(a,b,i,j)+=X(a,b,i,j)", 2),                           # cube 6 x 5, two idle lanes
+    ((66, 66, 8, 8), "P(ij)P(ab):R(a,b,i,j)+=X(a,b,i,j)", 4),                        # 66 = 2*3*11: cube 6 x 3 < 24 lanes -> generic
+])
+def test_permsum_cube_path_is_bit_identical_to_the_oracle(ctx, shape, spec, nterms):
+    """Tensors of >= 2^18 elements take permsum_cube_kernel (warp = micro-cube, running offsets); same term order and
+    rounding as the oracle -> identical bits for unit coefficients, 1e-14 for a complex alpha."""
+    rng = np.random.default_rng(len(shape) * 1000 + nterms)
+    D, X = rc(rng, *shape), rc(rng, *shape)
+    dX = ctx.tensor_from_numpy(X)
+    # the spec's own expansion, replayed for the oracle through tcb_permsum's (perms, coefs) form
+    import re
+    ops = re.findall(r"P\(([^)]*)\)", spec.split(":")[0])
+    labels = re.findall(r"\(([^()]*)\)", spec.split(":")[1])[0].split(",")
+    terms = [(list(labels), 1.0)]
+    for op in ops:
+        pivot, others = (op.split("/")[0], list(op.split("/")[1])) if "/" in op else (op[0], [op[1]])
+        nxt = []
+        for lab, sg in terms:
+            nxt.append((lab, sg))
+            for o_ in others:
+                nxt.append(([o_ if t == pivot else pivot if t == o_ else t for t in lab], -sg))
+        terms = nxt
+    assert len(terms) == nterms
+    perms = [[labels.index(t) for t in lab] for lab, _ in terms]
+    coefs = [sg for _, sg in terms]
+    beta = 1.0 if "+=" in spec else 0.0
+    dD = ctx.tensor_from_numpy(D)
+    ctx.antisymmetrize(spec, dD, dX, 1.0)
+    assert ctx.tensor_download(dD).tobytes() == oracle.permsum(D, X, perms, coefs, beta).tobytes()
+    dD2 = ctx.tensor_from_numpy(D)
+    alpha = 0.5 - 0.25j
+    ctx.antisymmetrize(spec, dD2, dX, alpha)
+    ref = oracle.permsum(D, X, perms, [alpha * c for c in coefs], beta)
+    assert np.max(np.abs(ctx.tensor_download(dD2) - ref)) <= 1e-14 * (np.abs(D).max() + nterms * np.abs(X).max())
+    for t in (dD, dD2, dX):
+        t.destroy()
