@@ -214,8 +214,18 @@ int get_plan(tcb_ctx *ctx, const char *expr, const tcb_tensor *D, const tcb_tens
     std::string why;
     int rc = plan_contraction(e, D->shape, L->shape, R->shape, ctx->opt, &cp->plan, &why);
     if (rc != TCB_OK) return set_error(ctx, rc, why + ": " + expr);
-    const size_t n = cp->plan.offM.size() + cp->plan.offN.size();
+    const ContractPlan &pl = cp->plan;
+    const size_t n = pl.offM.size() + pl.offN.size() + pl.offAm.size() + pl.offAk.size() + pl.offBk.size();
     TCB_CUDA(ctx, cudaMalloc((void **)&cp->d_tables, n * sizeof(int64_t)));
+    {   // GEMV tables behind offM and offN: offAm, offAk, offBk
+        size_t at = pl.offM.size() + pl.offN.size();
+        for (const std::vector<int64_t> *t : {&pl.offAm, &pl.offAk, &pl.offBk}) {
+            if (!t->empty())
+                TCB_CUDA(ctx, cudaMemcpyAsync(cp->d_tables + at, t->data(), t->size() * sizeof(int64_t),
+                                              cudaMemcpyHostToDevice, ctx->stream));
+            at += t->size();
+        }
+    }
     // the host vectors live as long as the cache entry, so the stream-ordered copies are safe
     TCB_CUDA(ctx, cudaMemcpyAsync(cp->d_tables, cp->plan.offM.data(), cp->plan.offM.size() * sizeof(int64_t),
                                   cudaMemcpyHostToDevice, ctx->stream));
@@ -442,6 +452,28 @@ int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor
     if (rc) return rc;
     const ContractPlan &P = cp->plan;
     const tcb_tensor *TA = P.swapped ? R : L, *TB = P.swapped ? L : R;
+    if (P.gemv) {
+        const size_t bytesPg = align_up(P.partial_bytes, 1024);
+        void *wsg = nullptr;
+        if (bytesPg) {
+            rc = workspace(ctx, bytesPg, &wsg);
+            if (rc) return rc;
+        }
+        GemvDesc g;
+        g.M = P.M; g.K = P.K;
+        g.A = TA->ptr; g.B = TB->ptr; g.D = D->ptr;
+        g.offD = cp->d_tables;
+        g.offAm = cp->d_tables + P.offM.size() + P.offN.size();
+        g.offAk = g.offAm + P.offAm.size();
+        g.offBk = g.offAk + P.offAk.size();
+        g.kfast = P.gemv_kfast;
+        g.alpha_re = alpha.re; g.alpha_im = alpha.im;
+        g.accumulate = P.accumulate;
+        g.partial = wsg;
+        TimedLaunch tl(ctx, kClsZgemm, P.flops, P.bytes);
+        TCB_CUDA(ctx, launch_gemv(g, ctx->stream, &ctx->launches));
+        return TCB_OK;
+    }
 
     const size_t bytesA = P.a.permuted ? align_up((size_t)P.a.elems * 16, 1024) : 0;
     const size_t bytesB = P.b.permuted ? align_up((size_t)P.b.elems * 16, 1024) : 0;

@@ -1,0 +1,162 @@
+// gemv.cu -- S2 regime "GEMV": contractions in which one operand is contracted away completely (N = 1), e.g.
+//   Fae(a,e) += ovvv(m,a,f,e) * T1(f,m)      R1(a,i) += T2(a,e,i,m) * Fme(m,e)        (CCSD: still binary)
+// As a GEMM these waste 63 of 64 tile columns and, worse, first permute the big operand into matrix form (1.6 GB for
+// ovvv at v = 150).  But a tensor's element offset is a SUM over its indices, so any operand is a matrix with a row table
+// and a column table:  A[m,k] = L[offAm[m] + offAk[k]].  This kernel reads the big operand once, in place, in its own
+// memory order:
+//   D[offD[m]] (+)= alpha * sum_k L[offAm[m] + offAk[k]] * R[offBk[k]]
+// m-fast (L's unit-stride index is free): one thread per m, consecutive threads read consecutive addresses, the R values
+//   and column offsets of a k-tile are staged in shared memory;
+// k-fast (L's unit-stride index is contracted): one warp per m, lanes along k, shuffle reduction in a fixed tree.
+// K can be cut into `ksplit` chunks (few rows, long K): partial sums are written per chunk and added in chunk order by
+// gemv_reduce_kernel -- deterministic, no atomics.  HBM-bound: algorithmic bytes = 16 (M K + K + M (2 if += else 1)).
+#include "kernels.h"
+
+#include <algorithm>
+
+namespace tcb {
+
+namespace {
+
+constexpr int GT = 256;        // threads per CTA
+constexpr int KT = 256;        // k-tile staged in shared memory (m-fast)
+
+struct GemvParams {
+    long long M, K, kchunk;
+    const double2 *A, *B;
+    double2 *D, *partial;        // partial: [ksplit][M] when ksplit > 1
+    const long long *offAm, *offAk, *offBk, *offD;
+    double ar, ai;
+    int accumulate, ksplit;
+};
+
+__device__ __forceinline__ void cmac(double2 &acc, const double2 a, const double2 b)
+{
+    acc.x = fma(a.x, b.x, fma(-a.y, b.y, acc.x));
+    acc.y = fma(a.x, b.y, fma(a.y, b.x, acc.y));
+}
+
+__device__ __forceinline__ void finish(const GemvParams &p, long long m, double2 acc)
+{
+    if (p.ksplit > 1) {
+        p.partial[(long long)blockIdx.y * p.M + m] = acc;
+        return;
+    }
+    double2 v = make_double2(p.ar * acc.x - p.ai * acc.y, p.ar * acc.y + p.ai * acc.x);
+    double2 *dst = p.D + p.offD[m];
+    if (p.accumulate) { const double2 d = *dst; v.x += d.x; v.y += d.y; }
+    *dst = v;
+}
+
+__global__ void __launch_bounds__(GT) gemv_mfast_kernel(const __grid_constant__ GemvParams p)
+{
+    __shared__ double2 s_b[KT];
+    __shared__ long long s_o[KT];
+    const long long m = (long long)blockIdx.x * GT + threadIdx.x;
+    const long long k0 = (long long)blockIdx.y * p.kchunk, k1 = min(p.K, k0 + p.kchunk);
+    const double2 *row = p.A + (m < p.M ? p.offAm[m] : 0);
+    double2 acc = make_double2(0.0, 0.0);
+    for (long long kb = k0; kb < k1; kb += KT) {
+        const int nk = (int)min((long long)KT, k1 - kb);
+        __syncthreads();
+        if (threadIdx.x < nk) {
+            s_b[threadIdx.x] = p.B[p.offBk[kb + threadIdx.x]];
+            s_o[threadIdx.x] = p.offAk[kb + threadIdx.x];
+        }
+        __syncthreads();
+        if (m < p.M) {
+            int k = 0;
+            for (; k + 4 <= nk; k += 4) {              // four independent loads in flight per thread
+                const double2 a0 = row[s_o[k]], a1 = row[s_o[k + 1]], a2 = row[s_o[k + 2]], a3 = row[s_o[k + 3]];
+                cmac(acc, a0, s_b[k]); cmac(acc, a1, s_b[k + 1]); cmac(acc, a2, s_b[k + 2]); cmac(acc, a3, s_b[k + 3]);
+            }
+            for (; k < nk; ++k) cmac(acc, row[s_o[k]], s_b[k]);
+        }
+    }
+    if (m < p.M) finish(p, m, acc);
+}
+
+__global__ void __launch_bounds__(GT) gemv_kfast_kernel(const __grid_constant__ GemvParams p)
+{
+    const int lane = threadIdx.x & 31;
+    const long long m = (long long)blockIdx.x * (GT / 32) + (threadIdx.x >> 5);
+    if (m >= p.M) return;
+    const long long k0 = (long long)blockIdx.y * p.kchunk, k1 = min(p.K, k0 + p.kchunk);
+    const double2 *row = p.A + p.offAm[m];
+    double2 acc[2] = {make_double2(0.0, 0.0), make_double2(0.0, 0.0)};
+    long long k = k0 + lane;
+    for (; k + 32 < k1; k += 64) {                      // two independent chains per lane
+        const double2 a0 = row[p.offAk[k]], a1 = row[p.offAk[k + 32]];
+        cmac(acc[0], a0, p.B[p.offBk[k]]);
+        cmac(acc[1], a1, p.B[p.offBk[k + 32]]);
+    }
+    if (k < k1) cmac(acc[0], row[p.offAk[k]], p.B[p.offBk[k]]);
+    double2 s = make_double2(acc[0].x + acc[1].x, acc[0].y + acc[1].y);
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) {                 // fixed tree: bit-reproducible
+        s.x += __shfl_down_sync(0xffffffffu, s.x, d);
+        s.y += __shfl_down_sync(0xffffffffu, s.y, d);
+    }
+    if (lane == 0) finish(p, m, s);
+}
+
+__global__ void __launch_bounds__(GT) gemv_reduce_kernel(const __grid_constant__ GemvParams p)
+{
+    const long long m = (long long)blockIdx.x * GT + threadIdx.x;
+    if (m >= p.M) return;
+    double2 acc = make_double2(0.0, 0.0);
+    for (int s = 0; s < p.ksplit; ++s) {                // chunk order
+        const double2 v = p.partial[(long long)s * p.M + m];
+        acc.x += v.x; acc.y += v.y;
+    }
+    double2 v = make_double2(p.ar * acc.x - p.ai * acc.y, p.ar * acc.y + p.ai * acc.x);
+    double2 *dst = p.D + p.offD[m];
+    if (p.accumulate) { const double2 d = *dst; v.x += d.x; v.y += d.y; }
+    *dst = v;
+}
+
+}  // namespace
+
+int gemv_ksplit(int64_t M, int64_t K, bool kfast)
+{
+    const int64_t ctas_m = kfast ? (M + GT / 32 - 1) / (GT / 32) : (M + GT - 1) / GT;
+    const int64_t min_chunk = kfast ? 512 : 256;
+    int64_t s = (4 * 148 + ctas_m - 1) / ctas_m;
+    s = std::min<int64_t>(s, K / min_chunk);
+    return (int)std::max<int64_t>(1, std::min<int64_t>(s, 64));
+}
+
+cudaError_t launch_gemv(const GemvDesc &g, cudaStream_t stream, int64_t *launches)
+{
+    GemvParams p;
+    p.M = g.M; p.K = g.K;
+    p.A = (const double2 *)g.A; p.B = (const double2 *)g.B; p.D = (double2 *)g.D;
+    p.partial = (double2 *)g.partial;
+    p.offAm = (const long long *)g.offAm; p.offAk = (const long long *)g.offAk;
+    p.offBk = (const long long *)g.offBk; p.offD = (const long long *)g.offD;
+    p.ar = g.alpha_re; p.ai = g.alpha_im;
+    p.accumulate = g.accumulate ? 1 : 0;
+    p.ksplit = gemv_ksplit(g.M, g.K, g.kfast);
+    if (p.ksplit > 1 && !p.partial) return cudaErrorInvalidValue;
+    p.kchunk = (g.K + p.ksplit - 1) / p.ksplit;
+    p.kchunk = (p.kchunk + 63) / 64 * 64;
+    p.ksplit = (int)((g.K + p.kchunk - 1) / p.kchunk);
+    if (g.kfast) {
+        dim3 grid((unsigned)((g.M + GT / 32 - 1) / (GT / 32)), (unsigned)p.ksplit);
+        gemv_kfast_kernel<<<grid, GT, 0, stream>>>(p);
+    } else {
+        dim3 grid((unsigned)((g.M + GT - 1) / GT), (unsigned)p.ksplit);
+        gemv_mfast_kernel<<<grid, GT, 0, stream>>>(p);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if (launches) ++*launches;
+    if (p.ksplit > 1) {
+        gemv_reduce_kernel<<<(unsigned)((g.M + GT - 1) / GT), GT, 0, stream>>>(p);
+        e = cudaGetLastError();
+        if (e == cudaSuccess && launches) ++*launches;
+    }
+    return e;
+}
+
+}  // namespace tcb

@@ -45,6 +45,21 @@ cudaError_t encode_gemm_maps(const GemmDesc &g, GemmTensorMaps *maps);
 cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps, cudaStream_t stream,
                                    int64_t *launches);
 
+// ---- S2 regime "GEMV": one operand contracted away completely (N = 1); the other is read in place through offset tables
+//   D[offD[m]] (+)= alpha * sum_k A[offAm[m] + offAk[k]] * B[offBk[k]]
+struct GemvDesc {
+    int64_t M, K;
+    const void *A, *B;       // device, complex128: the operand with free indices, the fully contracted one
+    void *D;
+    const int64_t *offAm, *offAk, *offBk, *offD;   // device tables (element offsets)
+    bool kfast;              // A's unit-stride index is contracted (warp per row) / free (thread per row)
+    double alpha_re, alpha_im;
+    bool accumulate;
+    void *partial;           // device, gemv_ksplit(M, K, kfast) * M complex128 when the split is > 1
+};
+int gemv_ksplit(int64_t M, int64_t K, bool kfast);
+cudaError_t launch_gemv(const GemvDesc &g, cudaStream_t stream, int64_t *launches);
+
 // ---- S3: tensor transposition, and the permuted add built on it ------------------------------------------
 // out[sum_d idx_d * ostride[d]] (op)= in[sum_d idx_d * istride[d]]  over idx in [0, extent)
 // The caller passes dims already canonicalised (extent-1 dropped, fusable neighbours fused), sorted by

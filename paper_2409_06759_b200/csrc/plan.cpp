@@ -76,8 +76,11 @@ bool has_dup(const std::vector<std::string> &v)
     return false;
 }
 
-std::vector<int64_t> offset_table(const std::vector<const Lab *> &order)
+// offsets of the multi-index enumerated over `order` (first label fastest) in the tensor whose strides `which` picks:
+// 0 = D, 1 = L, 2 = R
+std::vector<int64_t> offset_table(const std::vector<const Lab *> &order, int which = 0)
 {
+    auto stride = [which](const Lab *l) { return which == 0 ? l->sD : which == 1 ? l->sL : l->sR; };
     int64_t n = 1;
     for (const Lab *l : order) n *= l->ext;
     std::vector<int64_t> t((size_t)n);
@@ -86,9 +89,9 @@ std::vector<int64_t> offset_table(const std::vector<const Lab *> &order)
     for (int64_t i = 0; i < n; ++i) {
         t[(size_t)i] = off;
         for (size_t q = 0; q < order.size(); ++q) {
-            off += order[q]->sD;
+            off += stride(order[q]);
             if (++idx[q] < order[q]->ext) break;
-            off -= order[q]->sD * order[q]->ext;
+            off -= stride(order[q]) * order[q]->ext;
             idx[q] = 0;
         }
     }
@@ -190,6 +193,31 @@ int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const 
     if (P.M >= (1LL << 30) || P.N >= (1LL << 30) || P.K >= (1LL << 30))
         return fail(TCB_EUNSUPPORTED, "a matricised extent exceeds 2^30");
 
+    // (vii) GEMV route: B is contracted away completely.  A tensor's offset is a sum over its indices, so A is a matrix
+    // with a row table and a column table whatever its index order: no operand is permuted, A is read once in place.
+    if (sb.free.empty() && P.M > 1 && P.K > 1 && !opt.permute_always) {
+        P.gemv = true;
+        P.gemv_kfast = is_con(seqA[0]);
+        const int wa = swapped ? 2 : 1, wb = swapped ? 1 : 2;
+        P.offM = offset_table(sa.free, 0);              // rows enumerated in A's own memory order
+        P.offAm = offset_table(sa.free, wa);
+        P.offAk = offset_table(sa.con, wa);
+        P.offBk = offset_table(sa.con, wb);
+        P.offN.assign(1, 0);
+        P.a.permuted = P.b.permuted = false;
+        P.a.rows = P.M; P.b.rows = 1; P.a.elems = sizeA; P.b.elems = sizeB;
+        P.a.kmajor = P.gemv_kfast; P.b.kmajor = true;
+        for (const Lab *l : sa.free) P.m_labels.push_back(l->name);
+        for (const Lab *l : sa.con) P.k_labels.push_back(l->name);
+        P.splitk = opt.splitk;
+        P.splits = gemv_ksplit(P.M, P.K, P.gemv_kfast);
+        P.partial_bytes = P.splits > 1 ? (size_t)P.splits * (size_t)P.M * 16 : 0;
+        P.flops = 8.0 * (double)P.M * (double)P.K;
+        P.bytes = 16.0 * ((double)sizeA + (double)sizeB + (double)sizeD * (e.accumulate ? 2.0 : 1.0));
+        *out = std::move(P);
+        return TCB_OK;
+    }
+
     bool inplaceA = (sa.mmajor || sa.kmajor) && !opt.permute_always;
     bool inplaceB = (sb.mmajor || sb.kmajor) && !opt.permute_always;
     // (v) row operand whose fastest free index is not D's unit-stride index
@@ -267,12 +295,12 @@ std::string ContractPlan::describe() const
     std::snprintf(buf, sizeof buf,
                   "{\"M\": %lld, \"N\": %lld, \"K\": %lld, \"m_labels\": \"%s\", \"n_labels\": \"%s\", "
                   "\"k_labels\": \"%s\", \"row_operand\": \"%s\", \"permute_A\": %s, \"permute_B\": %s, "
-                  "\"A_layout\": \"%s\", \"B_layout\": \"%s\", \"splits\": %d, \"epilogue\": \"fused-scatter\", "
+                  "\"A_layout\": \"%s\", \"B_layout\": \"%s\", \"splits\": %d, \"route\": \"%s\", \"epilogue\": \"fused-scatter\", "
                   "\"accumulate\": %s, \"flops\": %.6g, \"bytes\": %.6g}",
                   (long long)M, (long long)N, (long long)K, join(m_labels).c_str(), join(n_labels).c_str(),
                   join(k_labels).c_str(), swapped ? "R" : "L", a.permuted ? "true" : "false",
                   b.permuted ? "true" : "false", a.kmajor ? "K-major" : "M-major", b.kmajor ? "K-major" : "M-major",
-                  splits, accumulate ? "true" : "false", flops, bytes);
+                  splits, gemv ? "gemv" : "gemm", accumulate ? "true" : "false", flops, bytes);
     return buf;
 }
 

@@ -46,6 +46,9 @@ struct ContractPlan {
     int64_t M = 1, N = 1, K = 1;
     OperandPlan a, b;
     std::vector<int64_t> offM, offN;
+    // GEMV route (N = 1: one operand fully contracted): the other operand is read in place through these tables
+    bool gemv = false, gemv_kfast = false;
+    std::vector<int64_t> offAm, offAk, offBk;
     int splits = 1;          // pieces per tile when every tile is cut along K (skinny shapes), else 1
     int splitk = 0;          // the option the schedule was made with
     size_t partial_bytes = 0; // workspace for the raw fragments of tiles cut along K

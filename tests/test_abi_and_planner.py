@@ -133,6 +133,10 @@ def test_invalid_contractions_are_rejected(expr, shapes, code):
 def test_extent_one_indices_are_dropped_and_labels_may_be_long():
     p = plan("R(p1,x,h1)+=T(p1,e_1,y,h1)*F(e_1,x,y)", (70, 1, 9), (70, 40, 1, 9), (40, 1, 1))
     assert (p["M"], p["N"], p["K"]) == (630, 1, 40)
-    assert p["permute_A"]                                  # [free][contracted][free]: not matrix-shaped
+    # [free][contracted][free] is not matrix-shaped, but N = 1 takes the GEMV route: T is read in place through its row
+    # and column offset tables, nothing is permuted
+    assert p["route"] == "gemv" and not p["permute_A"] and not p["permute_B"]
+    p = plan("R(p1,x,h1,q)+=T(p1,e_1,y,h1)*F(e_1,x,q,y)", (70, 1, 9, 3), (70, 40, 1, 9), (40, 1, 3, 1))
+    assert (p["M"], p["N"], p["K"]) == (630, 3, 40) and p["route"] == "gemm" and p["permute_A"]
     p = plan("R(p1,x,h1)+=T(p1,y,h1,e_1)*F(e_1,x,y)", (70, 1, 9), (70, 1, 9, 40), (40, 1, 1))
     assert (p["M"], p["N"], p["K"]) == (630, 1, 40) and not p["permute_A"] and p["A_layout"] == "M-major"

@@ -141,3 +141,28 @@ def test_every_ccsd_contraction_in_every_emitted_output_order(ctx, o, v):
         for t in (dD, dL, dR):
             t.destroy()
     assert worst <= TOL
+
+
+@pytest.mark.parametrize("expr,ext", [
+    ("D(a,e)+=L(m,a,f,e)*R(f,m)", dict(a=13, e=11, m=5, f=7)),            # k-fast: L's unit-stride index is contracted
+    ("D(a,i)=L(a,e,i,m)*R(m,e)", dict(a=40, i=9, e=17, m=6)),             # m-fast: L's unit-stride index is free
+    ("D(i)+=R(k,j)*L(j,i,k)", dict(i=3, j=300, k=301)),                   # few rows, long K: K cut, operands swapped
+    ("D(a,b)+=L(a,k,b)*R(k)", dict(a=700, b=3, k=2500)),                  # m-fast with the K cut
+])
+def test_gemv_route_reads_the_operand_in_place(ctx, expr, ext):
+    """N = 1 (one operand contracted away): no permutation, tables of row / column offsets, deterministic K split"""
+    from gpu_util import split_expr
+    rng = np.random.default_rng(sum(ext.values()))
+    dl, ll, rl = split_expr(expr)
+    D, L, R = rc(rng, *[ext[x] for x in dl]), rc(rng, *[ext[x] for x in ll]), rc(rng, *[ext[x] for x in rl])
+    dD, dL, dR = ctx.tensor_from_numpy(D), ctx.tensor_from_numpy(L), ctx.tensor_from_numpy(R)
+    plan = ctx.plan_describe(expr, dD, dL, dR)
+    assert plan["route"] == "gemv" and not plan["permute_A"] and not plan["permute_B"]
+    alpha = 0.75 - 0.5j
+    ctx.contract(expr, dD, dL, dR, alpha)
+    got = ctx.tensor_download(dD)
+    ref, sn = oracle.contract(expr, D, L, R, alpha)
+    assert parity_error(got, ref, sn) <= TOL
+    dD2 = ctx.tensor_from_numpy(D)
+    ctx.contract(expr, dD2, dL, dR, alpha)
+    assert ctx.tensor_download(dD2).tobytes() == got.tobytes()           # run-to-run identical
