@@ -4,7 +4,7 @@
 //   D[offM[m] + offN[n]] (+)= alpha * C[m,n]   ("Transpose result array to obtain C", PAPER.md:91 -- done
 //                                               here as a scatter through offset tables, no extra pass)
 //
-// B200 facts this design rests on (measured, profiles/r1_fp64_peak.txt): tcgen05 has no FP64 kind, the
+// B200 facts this design rests on (measured, profiles/r1b_fp64_peak.md): tcgen05 has no FP64 kind, the
 // native FP64 tensor op is SASS DMMA.8x8x4 (mma.sync.m8n8k4.f64): one per 16 cycles per SM sub-partition =
 // 128 flop/clk/SM = 37.0 TFLOP/s; its latency (~26 cycles) needs >= 2 independent accumulators per
 // sub-partition.  The pipe is slow relative to shared memory (one 32x32 complex warp tile needs 8 LDS.128
@@ -21,8 +21,17 @@
 //     row ^ k), i.e. fragment loads are bank-conflict free without padding.
 //   * complex product = 4 real DMMAs: Cr += Ar*Br; Cr += (-Ai)*Bi; Ci += Ar*Bi; Ci += Ai*Br  (the sign flip
 //     is an exact XOR on the high word).
-//   * split-K (skinny M,N with huge K): grid.z slices of K write raw partial tiles, a second kernel sums
-//     them in fixed order (deterministic, no atomics) and applies the same scatter.
+//   * persistent grid (2 CTAs per SM) with a stream-K schedule: whole tiles one CTA each while they fill the grid, the
+//     remainder wave -- or everything, for skinny M x N with long K -- cut along K into chunks whose raw accumulator
+//     fragments go to a workspace; zgemm_fixup_kernel sums a tile's chunks in k order (deterministic, no atomics on
+//     data) and applies the same scatter.  Tiles and chunks are claimed from two counters (dynamic deal).
+//   * the producer (thread 0) walks the CTA's segment list 4 k-tiles ahead of the consumers and ACROSS tile
+//     boundaries; segments reach the other warps through a small shared-memory queue.
+//   * no tensor work on padding: the 8-wide blocks of M and N are dealt to the tiles in pairs, a warp multiplies only
+//     the blocks it has (mma_ktile<MC, NC, KS>), the last k-tile of a K with <= 4 entries left does one k-step.
+//   * epilogue: read-modify-write software-pipelined one fragment column ahead; no FP64 multiplies for alpha = 1
+//     (the plain FP64 pipe shares its datapath with DMMA).
+// Measured history and the ncu evidence for each of these: DESIGN.md 6.2, profiles/r1b_zgemm_ncu_full.md.
 #include "kernels.h"
 
 #include <algorithm>
