@@ -58,6 +58,14 @@ def ccd_residual(ctx, B, T, R=None):
     return R
 
 
+def ccd_energy(ctx, B, T):
+    """E_corr = 1/4 sum_ijab <ij||ab> t_ij^ab -- the energy diagram (the 11th of the paper's 11 CCD diagrams,
+    PAPER.md:276), a contraction into a rank-0 tensor.  Returns the rank-0 device tensor E (download it to read it)."""
+    E = ctx.tensor_create(())
+    ctx.contract("E()=W(i,j,a,b)*T(a,b,i,j)", E, B["oovv"], T, 0.25)
+    return E
+
+
 CCD_FLOPS = lambda o, v: 8.0 * (                 # 8 real flop per complex multiply-add
     v * v * o * o * v                            # Fock vv
     + v * v * o * o * o                          # Fock oo

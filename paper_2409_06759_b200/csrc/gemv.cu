@@ -100,15 +100,23 @@ __global__ void __launch_bounds__(GT) gemv_kfast_kernel(const __grid_constant__ 
     if (lane == 0) finish(p, m, s);
 }
 
+// chunk partials -> D: one warp per row, lanes stride over the chunks in order, then a fixed shuffle tree (deterministic)
 __global__ void __launch_bounds__(GT) gemv_reduce_kernel(const __grid_constant__ GemvParams p)
 {
-    const long long m = (long long)blockIdx.x * GT + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    const long long m = (long long)blockIdx.x * (GT / 32) + (threadIdx.x >> 5);
     if (m >= p.M) return;
     double2 acc = make_double2(0.0, 0.0);
-    for (int s = 0; s < p.ksplit; ++s) {                // chunk order
+    for (int s = lane; s < p.ksplit; s += 32) {
         const double2 v = p.partial[(long long)s * p.M + m];
         acc.x += v.x; acc.y += v.y;
     }
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) {
+        acc.x += __shfl_down_sync(0xffffffffu, acc.x, d);
+        acc.y += __shfl_down_sync(0xffffffffu, acc.y, d);
+    }
+    if (lane != 0) return;
     double2 v = make_double2(p.ar * acc.x - p.ai * acc.y, p.ar * acc.y + p.ai * acc.x);
     double2 *dst = p.D + p.offD[m];
     if (p.accumulate) { const double2 d = *dst; v.x += d.x; v.y += d.y; }
@@ -123,7 +131,7 @@ int gemv_ksplit(int64_t M, int64_t K, bool kfast)
     const int64_t min_chunk = kfast ? 512 : 256;
     int64_t s = (4 * 148 + ctas_m - 1) / ctas_m;
     s = std::min<int64_t>(s, K / min_chunk);
-    return (int)std::max<int64_t>(1, std::min<int64_t>(s, 64));
+    return (int)std::max<int64_t>(1, std::min<int64_t>(s, kfast ? 8 * 4 * 148 : 64));   // a dot product: one warp per chunk
 }
 
 cudaError_t launch_gemv(const GemvDesc &g, cudaStream_t stream, int64_t *launches)
@@ -152,7 +160,7 @@ cudaError_t launch_gemv(const GemvDesc &g, cudaStream_t stream, int64_t *launche
     if (e != cudaSuccess) return e;
     if (launches) ++*launches;
     if (p.ksplit > 1) {
-        gemv_reduce_kernel<<<(unsigned)((g.M + GT - 1) / GT), GT, 0, stream>>>(p);
+        gemv_reduce_kernel<<<(unsigned)((g.M + GT / 32 - 1) / (GT / 32)), GT, 0, stream>>>(p);
         e = cudaGetLastError();
         if (e == cudaSuccess && launches) ++*launches;
     }

@@ -195,7 +195,9 @@ int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const 
 
     // (vii) GEMV route: B is contracted away completely.  A tensor's offset is a sum over its indices, so A is a matrix
     // with a row table and a column table whatever its index order: no operand is permuted, A is read once in place.
-    if (sb.free.empty() && P.M > 1 && P.K > 1 && !opt.permute_always) {
+    // Both operands contracted away (rank-0 D: the correlation energy E = 1/4 <ij||ab> t_ij^ab, the 11th CCD diagram of
+    // PAPER.md:276) is the same route with a single row.
+    if (sb.free.empty() && P.K > 1 && (P.M > 1 || sa.free.empty()) && !seqA.empty() && !opt.permute_always) {
         P.gemv = true;
         P.gemv_kfast = is_con(seqA[0]);
         const int wa = swapped ? 2 : 1, wb = swapped ? 1 : 2;

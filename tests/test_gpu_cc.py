@@ -50,3 +50,38 @@ def test_t3_term_program(ctx):
     gotX, got = ctx.tensor_download(dX), ctx.tensor_download(dR)
     assert np.max(np.abs(gotX - X)) <= 1e-11 * v * np.abs(W).max() * np.abs(T2).max()
     assert np.max(np.abs(got - ref)) <= 1e-11 * (np.abs(R3).max() + 9 * np.abs(X).max())
+
+
+@pytest.mark.parametrize("o,v", [(3, 5), (20, 80)])
+def test_ccd_energy_is_a_rank0_contraction(ctx, o, v):
+    """E = 1/4 sum <ij||ab> t_ij^ab (the 11th CCD diagram): both operands contracted away, D of rank 0.
+    At (20, 80) -- the bench size -- the inputs come from the device twin of the generator and are downloaded."""
+    import oracle
+    if o <= 6:
+        B, T, eo, ev = synth.config_ccd(o, v)
+        W, Th = B["oovv"], T
+        dW, dT = ctx.tensor_from_numpy(W), ctx.tensor_from_numpy(Th)
+    else:
+        dW, dT = ctx.tensor_create((o, o, v, v)), ctx.tensor_create((v, v, o, o))
+        ctx.synth_normal(dW, synth.SEED0 + 2, 1, antisym=((0, 1), (2, 3)), sigma=0.1)
+        ctx.synth_normal(dT, synth.SEED0 + 2, 2, antisym=((0, 1), (2, 3)))
+        W, Th = ctx.tensor_download(dW), ctx.tensor_download(dT)
+    dE = ccd.ccd_energy(ctx, {"oovv": dW}, dT)
+    got = ctx.tensor_download(dE)
+    ref, sn = oracle.contract("E()=W(i,j,a,b)*T(a,b,i,j)", np.zeros(()), W, Th, 0.25)
+    assert got.shape == ()
+    assert abs(complex(got) - complex(np.asarray(ref).reshape(-1)[0])) <= 1e-11 * float(np.asarray(sn).reshape(-1)[0])
+    plan = ctx.plan_describe("E()=W(i,j,a,b)*T(a,b,i,j)", dE, dW, dT)
+    assert plan["route"] == "gemv" and (plan["M"], plan["N"]) == (1, 1) and not plan["permute_A"] and not plan["permute_B"]
+    # accumulate form and determinism
+    ctx.contract("E()+=W(i,j,a,b)*T(a,b,i,j)", dE, dW, dT, 0.25)
+    twice = complex(ctx.tensor_download(dE))
+    assert abs(twice - 2 * complex(got)) <= 1e-11 * float(np.asarray(sn).reshape(-1)[0])
+    if o <= 6:
+        # and it is the oracle's CCD energy (tier 1a)
+        n = o + v
+        f = np.zeros((n, n), dtype=np.complex128)
+        f[:o, :o], f[o:, o:] = B["foo"], B["fvv"]
+        g = synth.tensor(synth.SEED0 + 2, 1, [n] * 4, antisym=((0, 1), (2, 3)), sigma=0.1, hermitian=True)
+        e_ref = cc.ccd_residual_unfactorised(o, f, g, T)[1]
+        assert abs(complex(got) - complex(e_ref)) <= 1e-11 * float(np.asarray(sn).reshape(-1)[0])
