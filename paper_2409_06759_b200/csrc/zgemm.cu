@@ -639,11 +639,13 @@ GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk)
         // shorter than 8 k-tiles costs more in fix-up traffic than it saves
         if (rem > 0 && rem * KT / slots + 8 < KT * 9 / 10) {
             s.dp_tiles = tiles - rem; s.sk_tiles = rem;
-            // about three chunks per CTA, claimed dynamically: they even out what whole tiles left uneven and what
+            // three to six chunks per CTA, claimed dynamically: they even out what whole tiles left uneven and what
             // ragged tiles make uneven among the chunks themselves (a 6 x 6-block tile costs half an 8 x 8 one).
             // With very few tiles (skinny M x N) one chunk per CTA: a tile's chunks are summed one after the other
             // by the fix-up, the fewer the better.
-            const int64_t per_cta = tiles >= 16 ? 3 : 1;      // <= ~55 chunks per tile for the fix-up to sum
+            // measured: 6 per CTA behind whole tiles (pp ladder 33.1 -> 33.7 TFLOP/s: the tail is half a chunk), 3 when
+            // everything is chunks (more only lengthens the fix-up's sums)
+            const int64_t per_cta = tiles >= slots ? 6 : tiles >= 16 ? 3 : 1;
             const int64_t chunks = std::max<int64_t>(1, std::min<int64_t>(per_cta * slots, rem * KT / 8));
             s.sk_q = (int)((rem * KT + chunks - 1) / chunks);
             if (s.dp_tiles == 0) s.splits = (int)((KT + s.sk_q - 1) / s.sk_q);
