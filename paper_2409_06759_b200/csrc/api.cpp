@@ -88,8 +88,11 @@ int enter(tcb_ctx *ctx)
 
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+constexpr size_t kWsHeader = 1024;      // head of the workspace: persistent work counters (see zgemm.cu)
+
 int workspace(tcb_ctx *ctx, size_t bytes, void **out)
 {
+    bytes += kWsHeader;
     if (bytes > ctx->ws_bytes) {
         TCB_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
         if (ctx->ws) cudaFree(ctx->ws);
@@ -104,8 +107,10 @@ int workspace(tcb_ctx *ctx, size_t bytes, void **out)
         }
         ctx->ws = p;
         ctx->ws_bytes = want;
+        // the first kWsHeader bytes hold the GEMM's work counters: zero once here, every kernel leaves them zero
+        TCB_CUDA(ctx, cudaMemsetAsync(p, 0, kWsHeader, ctx->stream));
     }
-    *out = ctx->ws;
+    *out = (char *)ctx->ws + kWsHeader;
     return TCB_OK;
 }
 
@@ -478,11 +483,10 @@ int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor
     const size_t bytesA = P.a.permuted ? align_up((size_t)P.a.elems * 16, 1024) : 0;
     const size_t bytesB = P.b.permuted ? align_up((size_t)P.b.elems * 16, 1024) : 0;
     const size_t bytesP = align_up(P.partial_bytes, 1024);
-    const size_t bytesC = 1024;                 // work counters of the GEMM's dynamic deal
     char *ws = nullptr;
     {
         void *p;
-        rc = workspace(ctx, bytesA + bytesB + bytesP + bytesC, &p);
+        rc = workspace(ctx, bytesA + bytesB + bytesP, &p);
         if (rc) return rc;
         ws = (char *)p;
     }
@@ -511,7 +515,7 @@ int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor
     g.accumulate = P.accumulate;
     g.splitk = P.splitk;
     g.partial = bytesP ? ws + bytesA + bytesB : nullptr;
-    g.counters = ctx->opt.static_deal ? nullptr : ws + bytesA + bytesB + bytesP;
+    g.counters = ctx->opt.static_deal ? nullptr : (char *)ctx->ws;      // the workspace header
     TimedLaunch tl(ctx, kClsZgemm, P.flops, P.bytes);
     TCB_CUDA(ctx, launch_zgemm(g, ctx->stream, &ctx->launches));
     return TCB_OK;

@@ -25,7 +25,7 @@ struct GemmDesc {
     bool accumulate;         // true: D += ...; false: D = ...
     int splitk;              // 0 = auto (stream-K on the remainder wave), 1 = off, n > 1 = every tile cut n ways
     void *partial;           // device, gemm_schedule(...).partial_bytes (raw accumulator fragments of cut tiles)
-    void *counters = nullptr; // device, 16 bytes, 8-byte aligned: work counters of the dynamic deal (null: static deal)
+    void *counters = nullptr; // device, 24 bytes, 8-byte aligned, ZERO on entry (the kernel leaves them zero): work counters of the dynamic deal (null: static deal)
 };
 // How the (tile, k-tile) iteration space is dealt to the persistent grid (2 CTAs per SM): whole tiles
 // data-parallel, the remainder ("stream-K") cut along K into equal chunks, one per CTA, summed by a fix-up kernel.

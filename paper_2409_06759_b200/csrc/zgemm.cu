@@ -69,7 +69,7 @@ struct GemmParams {
     double alpha_re, alpha_im;
     int accumulate;
     double2 *partial;              // [slot][32][128] raw accumulator fragments
-    unsigned long long *counters;  // [2] work counters (whole tiles, stream-K chunks), zero at launch; null: static deal
+    unsigned long long *counters;  // [3] whole tiles claimed, stream-K chunks claimed, CTAs done; zero at launch; null: static deal
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -498,6 +498,15 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                             P[((i * 4 + j) * 2 + h) * NTHREADS] = make_double2(cr[i][j][h], ci[i][j][h]);
         }
     }
+    // counters[2] counts the CTAs that are done claiming; the last one leaves all three at zero for the next launch
+    // (no memset node between contractions)
+    if (tid == 0 && p.counters) {
+        __threadfence();
+        if (atomicAdd(p.counters + 2, 1ULL) == gridDim.x - 1) {
+            p.counters[0] = 0; p.counters[1] = 0; p.counters[2] = 0;
+            __threadfence();
+        }
+    }
 }
 
 // fix-up of the tiles that were cut along K: sums the tile's partial fragments in k order (deterministic) and
@@ -694,11 +703,7 @@ cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps
     p.alpha_re = g.alpha_re; p.alpha_im = g.alpha_im;
     p.accumulate = g.accumulate ? 1 : 0;
     p.partial = (double2 *)g.partial;
-    p.counters = (unsigned long long *)g.counters;
-    if (p.counters) {
-        cudaError_t ce = cudaMemsetAsync(p.counters, 0, 2 * sizeof(unsigned long long), stream);
-        if (ce != cudaSuccess) return ce;
-    }
+    p.counters = (unsigned long long *)g.counters;      // zero on entry; the last CTA to leave zeroes them again
     if (sc.partial_bytes && !p.partial) return cudaErrorInvalidValue;
     cudaError_t e;
     if (g.a_kmajor)
