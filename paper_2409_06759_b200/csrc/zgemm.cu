@@ -276,39 +276,25 @@ __device__ __forceinline__ void store_fragment(const GemmParams &p, const double
             }
         return;
     }
-    if (p.accumulate) {
-        // read-modify-write, software-pipelined: the 4 loads of column (j,h)+1 are issued before the 4 stores of
-        // column (j,h).  Written load-then-store per element the compiler may not hoist a load over the previous
-        // store (it cannot rule out aliasing), and a tile's 32 accesses per thread were 32 serial DRAM round trips:
-        // K <= 150 contractions into large D ran at 1.3 TB/s.
-        auto ldcol = [&](int jh, double2 (&d)[4]) {
-            const long long o = on[jh >> 1][jh & 1];
+    if (p.accumulate) {            // A/B fallback (TCB_GEMM_RED=0): plain read-modify-write, one element in flight
 #pragma unroll
-            for (int i = 0; i < 4; ++i)
-                if (o >= 0 && om[i] >= 0) d[i] = p.D[om[i] + o];
-        };
-        double2 dcur[4], dnext[4];
-        ldcol(0, dcur);
+        for (int j = 0; j < 4; ++j)
 #pragma unroll
-        for (int jh = 0; jh < 8; ++jh) {
-            const int j = jh >> 1, h = jh & 1;
-            if (jh + 1 < 8) ldcol(jh + 1, dnext);
-            if (on[j][h] >= 0) {
+            for (int h = 0; h < 2; ++h) {
+                if (on[j][h] < 0) continue;
 #pragma unroll
                 for (int i = 0; i < 4; ++i) {
                     if (om[i] < 0) continue;
                     const double xr = cr[i][j][h], xi = ci[i][j][h];
-                    const double2 d = dcur[i];
+                    double2 *dst = p.D + om[i] + on[j][h];
+                    const double2 d = *dst;
                     double2 v;
                     if (mode == 0) v = make_double2(d.x + xr, d.y + xi);
                     else if (mode == 1) v = make_double2(fma(ar, xr, d.x), fma(ar, xi, d.y));
                     else v = make_double2(fma(ar, xr, fma(-ai, xi, d.x)), fma(ar, xi, fma(ai, xr, d.y)));
-                    p.D[om[i] + on[j][h]] = v;
+                    *dst = v;
                 }
             }
-#pragma unroll
-            for (int i = 0; i < 4; ++i) dcur[i] = dnext[i];
-        }
         return;
     }
 #pragma unroll
