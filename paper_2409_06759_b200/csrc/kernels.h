@@ -90,6 +90,9 @@ struct PermSumDesc {
     void *D;
 };
 cudaError_t launch_permsum(const PermSumDesc &p, cudaStream_t stream, int64_t *launches);
+// fast path (permsum_orbit.cu): terms that permute three leading indices of equal extent among themselves; *handled =
+// false when the call is of another kind
+cudaError_t launch_permsum_orbit(const PermSumDesc &p, cudaStream_t stream, int64_t *launches, bool *handled);
 
 // ---- S7: elementwise --------------------------------------------------------------------------------------
 cudaError_t launch_fill(void *D, int64_t n, double re, double im, cudaStream_t stream, int64_t *launches);

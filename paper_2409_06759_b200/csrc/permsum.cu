@@ -211,6 +211,11 @@ bool try_cube(const PermSumDesc &d, cudaStream_t stream, cudaError_t *err)
 cudaError_t launch_permsum(const PermSumDesc &d, cudaStream_t stream, int64_t *launches)
 {
     {
+        bool handled = false;
+        cudaError_t oe = launch_permsum_orbit(d, stream, launches, &handled);
+        if (oe != cudaSuccess || handled) return oe;
+    }
+    {
         cudaError_t ce = cudaSuccess;
         if (try_cube(d, stream, &ce)) {
             if (ce == cudaSuccess && launches) ++*launches;

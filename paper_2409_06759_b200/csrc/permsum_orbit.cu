@@ -1,0 +1,556 @@
+// permsum_orbit.cu -- S6 fast path for antisymmetrisers over THREE leading indices of equal extent:
+//   D = beta D + sum_t c_t X[pi_t(.)],  every pi_t permuting the leading indices {0,1,2} among themselves and the
+//   remaining ("outer") indices among themselves -- the unrolled P(a/bc), P(a/bc)P(k/ij) of a CCSDT residual
+//   (PAPER.md:194, 230, 284).
+//
+// Why (profiles/r1b_permsum.md): the gather kernels read every term straight from L2; with 9 terms that is 9 x 16
+// bytes per element through l1tex, 10-16 cache lines per warp gather (tag stage 75 % busy), X fetched 4.9x from DRAM.
+// Here the leading indices are cut into 6 x 6 x 6 cubes.  A permutation of the leading indices maps cubes to cubes, the
+// cubes reachable from one another form an orbit of <= 6.  One work item = one orbit at one value of the outer indices:
+//   * a producer warp loads the orbit's cubes of X, once per distinct outer permutation (k/ij: 3), with ONE tiled TMA
+//     load per cube (cp.async.bulk.tensor.4d over the map {a, b, c, outer slab}, box 6 x 6 x 6 x 1, SASS UTMALDG) into
+//     a 3-stage mbarrier ring -- L2 -> SM traffic 3 x X instead of 9 x X, no per-row copy instructions;
+//   * 18 consumer warps produce the orbit's cubes of D from shared memory: a quarter-warp is a 2 x 2 x 2 micro-cube,
+//     whose eight 16-byte reads fall in eight different bank groups under EVERY permutation of (a,b,c) because the cube
+//     strides 1, 6, 36 are 1, 6, 4 mod 8; a warp covers a full 96-byte row of a, so D moves in whole sectors;
+//   * items are ordered so that the (<= 6) outer slabs that are permutations of one another are processed together
+//     by one CTA for one orbit: each cube of X comes from DRAM once.
+// Terms are added in the caller's order with separately rounded products and sums: bit-identical to the generic
+// kernel and to the oracle.
+#include "kernels.h"
+
+#include <algorithm>
+#include <cstdlib>
+#include <map>
+#include <mutex>
+#include <numeric>
+#include <vector>
+
+namespace tcb {
+
+namespace {
+
+constexpr int T6 = 6;                       // cube edge
+constexpr int kCube = T6 * T6 * T6;         // 216 elements, 3456 bytes = 27 x 128
+constexpr int kCubeBytes = kCube * 16;
+constexpr int kConsumerWarps = 18;          // 54 warp tasks (6 cubes x 9 (b,c) micro-rows) = 3 rounds
+constexpr int kThreads = (kConsumerWarps + 1) * 32;
+constexpr int kRounds = 3;
+constexpr int kMaxOmega = 6;                // cubes per orbit
+constexpr int kMaxTau = 6;                  // distinct outer permutations
+constexpr int kMaxStages = 4;
+constexpr int kOrbTerms = 9;
+
+struct alignas(4) OrbitEntry {              // one orbit of cube coordinates
+    unsigned char n, pad;                            // cubes in the orbit
+    unsigned char coord[kMaxOmega][3];               // block coordinates
+    unsigned char src[kMaxOmega][kOrbTerms];         // cube of X that term t reads for cube w of D
+};
+static_assert(sizeof(OrbitEntry) == 76, "OrbitEntry is copied word by word");
+
+struct OrbitParams {
+    int nterms, ntau, nO, stages, eI, ragged, beta_zero;
+    int eO[3];                               // outer extents (dims 3..)
+    long long dsI[3], dsO[3];                // strides of the leading / outer dims (D and X have the same shape)
+    long long slab_elems;                    // eI^3
+    long long xsO[kMaxTau][3];               // stride in X of D's outer index k under outer class u
+    int sstr[kOrbTerms][3];                  // shared-memory stride of D's leading index k under term t (1, 6 or 36)
+    unsigned char tau[kOrbTerms];            // outer class of term t
+    double cr[kOrbTerms], ci[kOrbTerms], br, bi;
+    unsigned norbits, ngroups;
+    const OrbitEntry *orbits;
+    const unsigned *slab_order;              // slabs, group by group
+    const unsigned *group_start;             // [ngroups + 1] into slab_order
+    double2 *D;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "ORB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra ORB_DONE;\n"
+        "bra ORB_WAIT;\n"
+        "ORB_DONE:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap *tm, int c0, int c1, int c2, int c3,
+                                            uint32_t bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+        ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar)
+        : "memory");
+}
+
+struct alignas(16) StageMeta {               // written by the producer warp before it arms the stage's barrier
+    long long cube[kMaxOmega];               // D offset of cube w
+    int slot[kMaxOmega][12];                 // element offset (in the stage) of the cube term t reads for cube w
+    int n;
+    unsigned char coord[kMaxOmega][4];
+    unsigned ob[sizeof(OrbitEntry) / 4];     // producer scratch: the item's orbit entry
+};
+
+// Items: for group g of outer slabs (slabs that are permutations of one another), for orbit o: the group's slabs.
+// CTA b takes the (g, o) pairs b, b + grid, ...; producer and consumers walk the same sequence.
+struct ItemCursor {
+    unsigned long long pair, npairs;
+    unsigned s, s_end, orbit;
+    __device__ __forceinline__ void init(const OrbitParams &p)
+    {
+        npairs = (unsigned long long)p.ngroups * p.norbits;
+        pair = blockIdx.x;
+        load(p);
+    }
+    __device__ __forceinline__ void load(const OrbitParams &p)
+    {
+        if (pair < npairs) {
+            const unsigned g = (unsigned)(pair / p.norbits);
+            orbit = (unsigned)(pair - (unsigned long long)g * p.norbits);
+            s = p.group_start[g];
+            s_end = p.group_start[g + 1];
+        }
+    }
+    __device__ __forceinline__ bool valid() const { return pair < npairs; }
+    __device__ __forceinline__ void advance(const OrbitParams &p)
+    {
+        if (++s == s_end) {
+            pair += gridDim.x;
+            load(p);
+        }
+    }
+};
+
+__global__ void __launch_bounds__(kThreads, 1)
+permsum_orbit_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ OrbitParams p)
+{
+    extern __shared__ __align__(128) uint8_t orb_smem[];
+    __shared__ __align__(8) unsigned long long s_bar[2 * kMaxStages];
+    __shared__ StageMeta s_meta[kMaxStages];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t bar0 = smem_u32(s_bar);
+    const uint32_t data0 = smem_u32(orb_smem);
+    const uint32_t stage_bytes = (uint32_t)(kMaxOmega * p.ntau * kCubeBytes);
+    if (tid == 0) {
+        for (int s = 0; s < p.stages; ++s) {
+            mbar_init(bar0 + 8 * s, 1);                                  // full: the producer's arrive + the bytes
+            mbar_init(bar0 + 8 * (kMaxStages + s), kConsumerWarps);      // empty: one arrive per consumer warp
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmX) : "memory");
+    }
+    __syncthreads();
+    ItemCursor cur;
+    cur.init(p);
+    if (warp == kConsumerWarps) {
+        // ================= producer warp =================
+        unsigned it = 0;
+        for (; cur.valid(); cur.advance(p), ++it) {
+            const int st = (int)(it % (unsigned)p.stages);
+            const uint32_t par = (it / (unsigned)p.stages) & 1u;
+            StageMeta &m = s_meta[st];
+            mbar_wait(bar0 + 8 * (kMaxStages + st), par ^ 1u);          // consumers are done with the stage
+            {   // the item's orbit entry, word by word
+                const unsigned *src = reinterpret_cast<const unsigned *>(p.orbits + cur.orbit);
+                if (lane < (int)(sizeof(OrbitEntry) / 4)) m.ob[lane] = src[lane];
+            }
+            unsigned slab = p.slab_order[cur.s];
+            long long doffO = 0, xoffO[kMaxTau];
+#pragma unroll
+            for (int u = 0; u < kMaxTau; ++u) xoffO[u] = 0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k)
+                if (k < p.nO) {
+                    const long long v = slab % (unsigned)p.eO[k];
+                    slab /= (unsigned)p.eO[k];
+                    doffO += v * p.dsO[k];
+#pragma unroll
+                    for (int u = 0; u < kMaxTau; ++u)
+                        if (u < p.ntau) xoffO[u] += v * p.xsO[u][k];
+                }
+            __syncwarp();
+            const OrbitEntry &ob = *reinterpret_cast<const OrbitEntry *>(m.ob);
+            const int n = ob.n;
+            for (int idx = lane; idx < kMaxOmega * kOrbTerms; idx += 32) {
+                const int w = idx / kOrbTerms, t = idx - w * kOrbTerms;
+                if (w < n && t < p.nterms) m.slot[w][t] = (ob.src[w][t] * p.ntau + p.tau[t]) * kCube;
+            }
+            if (lane < n) {
+                m.cube[lane] = doffO + (long long)ob.coord[lane][0] * T6 * p.dsI[0] +
+                               (long long)ob.coord[lane][1] * T6 * p.dsI[1] + (long long)ob.coord[lane][2] * T6 * p.dsI[2];
+                m.coord[lane][0] = ob.coord[lane][0];
+                m.coord[lane][1] = ob.coord[lane][1];
+                m.coord[lane][2] = ob.coord[lane][2];
+            }
+            if (lane == 0) m.n = n;
+            __syncwarp();
+            const uint32_t full = bar0 + 8 * st;
+            if (lane == 0) mbar_expect_tx(full, (uint32_t)(n * p.ntau * kCubeBytes));
+            __syncwarp();
+            for (int idx = lane; idx < n * p.ntau; idx += 32) {
+                const int g = idx / p.ntau, u = idx - g * p.ntau;
+                long long xo = xoffO[0];
+#pragma unroll
+                for (int uu = 1; uu < kMaxTau; ++uu)
+                    if (uu == u) xo = xoffO[uu];
+                tma_load_4d(data0 + st * stage_bytes + (uint32_t)idx * kCubeBytes, &tmX, ob.coord[g][0] * (2 * T6),
+                            ob.coord[g][1] * T6, ob.coord[g][2] * T6, (int)(xo / p.slab_elems), full);
+            }
+        }
+        return;
+    }
+    // ================= consumer warps =================
+    // per thread, once: its element of every round (cube w, local coordinates) -- the same for every item
+    const int qw = lane >> 3, bits = lane & 7;
+    const bool lane_on = qw < 3;
+    int ew[kRounds], soff[kRounds][kOrbTerms], lpack[kRounds];
+    long long dloc[kRounds];
+#pragma unroll
+    for (int j = 0; j < kRounds; ++j) {
+        const int wt = warp + kConsumerWarps * j;            // warp task: cube wt / 9, micro-row (m1, m2) = wt % 9
+        ew[j] = wt / 9;
+        const int mr = wt - ew[j] * 9, m2 = mr / 3, m1 = mr - m2 * 3;
+        const int l0 = 2 * (qw % 3) + (bits & 1), l1 = 2 * m1 + ((bits >> 1) & 1), l2 = 2 * m2 + (bits >> 2);
+        lpack[j] = l0 | (l1 << 8) | (l2 << 16);
+        dloc[j] = l0 * p.dsI[0] + l1 * p.dsI[1] + l2 * p.dsI[2];
+#pragma unroll
+        for (int t = 0; t < kOrbTerms; ++t) soff[j][t] = l0 * p.sstr[t][0] + l1 * p.sstr[t][1] + l2 * p.sstr[t][2];
+    }
+    unsigned it = 0;
+    for (; cur.valid(); cur.advance(p), ++it) {
+        const int st = (int)(it % (unsigned)p.stages);
+        const uint32_t par = (it / (unsigned)p.stages) & 1u;
+        const StageMeta &m = s_meta[st];
+        mbar_wait(bar0 + 8 * st, par);
+        const int n = m.n;
+        const double2 *cubes = reinterpret_cast<const double2 *>(orb_smem + (size_t)st * stage_bytes);
+        bool ok[kRounds];
+        long long doff[kRounds];
+        double2 dv[kRounds];
+#pragma unroll
+        for (int j = 0; j < kRounds; ++j) {
+            ok[j] = lane_on && ew[j] < n;
+            if (ok[j] && p.ragged) {
+#pragma unroll
+                for (int k = 0; k < 3; ++k)
+                    ok[j] = ok[j] && (m.coord[ew[j]][k] * T6 + ((lpack[j] >> (8 * k)) & 255) < p.eI);
+            }
+            doff[j] = ok[j] ? m.cube[ew[j]] + dloc[j] : 0;
+            if (ok[j] && !p.beta_zero) dv[j] = p.D[doff[j]];
+        }
+#pragma unroll
+        for (int j = 0; j < kRounds; ++j) {
+            if (!ok[j]) continue;
+            double ar = 0.0, ai = 0.0;
+            if (!p.beta_zero) {
+                ar = __dsub_rn(__dmul_rn(p.br, dv[j].x), __dmul_rn(p.bi, dv[j].y));
+                ai = __dadd_rn(__dmul_rn(p.br, dv[j].y), __dmul_rn(p.bi, dv[j].x));
+            }
+            int sl[12];
+            {
+                const int4 *sv = reinterpret_cast<const int4 *>(m.slot[ew[j]]);
+#pragma unroll
+                for (int q = 0; q < 3; ++q) {
+                    const int4 v = sv[q];
+                    sl[4 * q] = v.x; sl[4 * q + 1] = v.y; sl[4 * q + 2] = v.z; sl[4 * q + 3] = v.w;
+                }
+            }
+#pragma unroll
+            for (int t0 = 0; t0 < kOrbTerms; t0 += 3) {           // three conflict-free LDS.128 in flight, then their arithmetic
+                double2 x[3];
+#pragma unroll
+                for (int u = 0; u < 3; ++u)
+                    if (t0 + u < p.nterms) x[u] = cubes[sl[t0 + u] + soff[j][t0 + u]];
+#pragma unroll
+                for (int u = 0; u < 3; ++u)
+                    if (t0 + u < p.nterms) {
+                        const double cr = p.cr[t0 + u], ci = p.ci[t0 + u];
+                        ar = __dadd_rn(ar, __dsub_rn(__dmul_rn(cr, x[u].x), __dmul_rn(ci, x[u].y)));
+                        ai = __dadd_rn(ai, __dadd_rn(__dmul_rn(cr, x[u].y), __dmul_rn(ci, x[u].x)));
+                    }
+            }
+            p.D[doff[j]] = make_double2(ar, ai);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar0 + 8 * (kMaxStages + st));      // this warp no longer reads the stage
+    }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+EncodeTiledFn orbit_encode_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        void *ptr = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)ptr;
+    });
+    return fn;
+}
+
+// Everything about a call that does not depend on pointers and coefficients: built once per (shape, term set).
+struct OrbitPlan {
+    bool eligible = false;
+    OrbitParams p;
+    size_t smem = 0;
+    long long nslabs = 1;
+    int grid = 0;
+};
+
+std::vector<long long> plan_key(const PermSumDesc &d)
+{
+    std::vector<long long> k;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    k.push_back(dev);
+    k.push_back(d.rank);
+    k.push_back(d.nterms);
+    for (int s = 0; s < d.rank; ++s) k.push_back(d.extent[s]);
+    for (int t = 0; t < d.nterms; ++t)
+        for (int s = 0; s < d.rank; ++s) k.push_back(d.xstride[t][s]);
+    return k;
+}
+
+// Fills plan (tables on the device, allocated once and kept).  plan.eligible stays false when the term set is not of
+// the "leading three equal-extent indices permuted among themselves" kind.
+cudaError_t build_plan(const PermSumDesc &d, OrbitPlan &plan)
+{
+    const int r = d.rank;
+    if (r < 3 || d.nterms < 2 || d.nterms > kOrbTerms) return cudaSuccess;
+    long long n = 1, ds[kMaxRank];
+    for (int k = 0; k < r; ++k) {
+        if (d.extent[k] < 2) return cudaSuccess;             // extent-1 indices: X strides are ambiguous
+        ds[k] = n;
+        n *= d.extent[k];
+    }
+    if (n < (1LL << 16)) return cudaSuccess;                 // small tensors: launch latency decides, keep the simple kernels
+    // position in X of D's index s under term t (X strides are distinct: all extents >= 2)
+    std::vector<std::vector<int>> pos(d.nterms, std::vector<int>(r));
+    for (int t = 0; t < d.nterms; ++t)
+        for (int s = 0; s < r; ++s) {
+            int m = 0;
+            for (int s2 = 0; s2 < r; ++s2) m += d.xstride[t][s2] < d.xstride[t][s] ? 1 : 0;
+            pos[t][s] = m;
+            if (d.extent[m] != d.extent[s] || d.xstride[t][s] != ds[m]) return cudaSuccess;   // X has D's shape
+            if ((s < 3) != (m < 3)) return cudaSuccess;      // leading indices stay among the leading three
+        }
+    if (d.extent[0] != d.extent[1] || d.extent[0] != d.extent[2]) return cudaSuccess;
+    {   // all three leading indices must really move (else the cube kernel is already coalesced and cheaper)
+        bool moved[3] = {false, false, false};
+        for (int t = 0; t < d.nterms; ++t)
+            for (int s = 0; s < 3; ++s) moved[s] = moved[s] || pos[t][s] != s;
+        if (!(moved[0] && moved[1] && moved[2])) return cudaSuccess;
+    }
+    OrbitParams &p = plan.p;
+    p.nterms = d.nterms;
+    p.eI = (int)d.extent[0];
+    if (p.eI < T6 || d.extent[0] > 255 * T6) return cudaSuccess;
+    p.ragged = p.eI % T6 ? 1 : 0;
+    const int nb = (p.eI + T6 - 1) / T6;
+    p.nO = r - 3;
+    long long nslabs = 1;
+    for (int k = 0; k < 3; ++k) {
+        p.dsI[k] = ds[k];
+        p.eO[k] = k < p.nO ? (int)d.extent[3 + k] : 1;
+        p.dsO[k] = k < p.nO ? ds[3 + k] : 0;
+        nslabs *= p.eO[k];
+    }
+    if (nslabs > (1LL << 22)) return cudaSuccess;
+    p.slab_elems = ds[2] * d.extent[2];
+    // outer-permutation classes
+    std::map<std::vector<int>, int> classes;
+    const int q[3] = {1, T6, T6 * T6};
+    for (int t = 0; t < d.nterms; ++t) {
+        std::vector<int> key;
+        for (int k = 0; k < p.nO; ++k) key.push_back(pos[t][3 + k]);
+        auto it = classes.find(key);
+        if (it == classes.end()) {
+            if ((int)classes.size() == kMaxTau) return cudaSuccess;
+            const int u = (int)classes.size();
+            it = classes.emplace(key, u).first;
+            for (int k = 0; k < 3; ++k) p.xsO[u][k] = k < p.nO ? d.xstride[t][3 + k] : 0;
+        }
+        p.tau[t] = (unsigned char)it->second;
+        for (int k = 0; k < 3; ++k) p.sstr[t][k] = q[pos[t][k]];
+    }
+    for (int t = d.nterms; t < kOrbTerms; ++t) {
+        p.tau[t] = 0;
+        for (int k = 0; k < 3; ++k) p.sstr[t][k] = 0;
+    }
+    p.ntau = (int)classes.size();
+    for (int u = p.ntau; u < kMaxTau; ++u)
+        for (int k = 0; k < 3; ++k) p.xsO[u][k] = 0;
+    const size_t stage_bytes = (size_t)kMaxOmega * p.ntau * kCubeBytes;
+    p.stages = (int)std::min<size_t>(kMaxStages, (200 * 1024) / stage_bytes);
+    if (p.stages < 2) return cudaSuccess;
+    plan.smem = stage_bytes * p.stages;
+    // ---- orbits of the cube coordinates under the terms ------------------------------------------------------------
+    const int ncubes = nb * nb * nb;
+    auto decode = [&](int id, int *c) { for (int k = 0; k < 3; ++k) { c[k] = id % nb; id /= nb; } };
+    auto encode = [&](const int *c) { return (c[2] * nb + c[1]) * nb + c[0]; };
+    auto image = [&](int id, int t) {          // cube of X that term t reads for cube `id` of D
+        int c[3], g[3];
+        decode(id, c);
+        for (int k = 0; k < 3; ++k) g[pos[t][k]] = c[k];
+        return encode(g);
+    };
+    std::vector<int> orbit_of((size_t)ncubes, -1);
+    std::vector<OrbitEntry> orbits;
+    for (int id = 0; id < ncubes; ++id) {
+        if (orbit_of[(size_t)id] >= 0) continue;
+        std::vector<int> members = {id};
+        orbit_of[(size_t)id] = (int)orbits.size();
+        for (size_t h = 0; h < members.size(); ++h)
+            for (int t = 0; t < d.nterms; ++t) {
+                const int g = image(members[h], t);
+                if (orbit_of[(size_t)g] < 0) {
+                    if ((int)members.size() == kMaxOmega) return cudaSuccess;
+                    orbit_of[(size_t)g] = (int)orbits.size();
+                    members.push_back(g);
+                }
+            }
+        OrbitEntry e;
+        std::fill((unsigned char *)&e, (unsigned char *)&e + sizeof e, (unsigned char)0);
+        e.n = (unsigned char)members.size();
+        for (size_t w = 0; w < members.size(); ++w) {
+            int c[3];
+            decode(members[w], c);
+            for (int k = 0; k < 3; ++k) e.coord[w][k] = (unsigned char)c[k];
+            for (int t = 0; t < d.nterms; ++t) {
+                const int g = image(members[w], t);
+                e.src[w][t] = (unsigned char)(std::find(members.begin(), members.end(), g) - members.begin());
+            }
+        }
+        orbits.push_back(e);
+    }
+    // ---- groups of outer slabs that are permutations of one another (union-find over the outer classes) --------------
+    std::vector<unsigned> order((size_t)nslabs), parent((size_t)nslabs);
+    std::iota(order.begin(), order.end(), 0u);
+    std::iota(parent.begin(), parent.end(), 0u);
+    auto find = [&](unsigned a) {
+        while (parent[a] != a) { parent[a] = parent[parent[a]]; a = parent[a]; }
+        return a;
+    };
+    for (unsigned s = 0; s < (unsigned)nslabs; ++s) {
+        long long v[3] = {0, 0, 0};
+        unsigned rem = s;
+        for (int k = 0; k < p.nO; ++k) { v[k] = rem % (unsigned)p.eO[k]; rem /= (unsigned)p.eO[k]; }
+        for (int u = 0; u < p.ntau; ++u) {
+            long long xo = 0;
+            for (int k = 0; k < p.nO; ++k) xo += v[k] * p.xsO[u][k];
+            const unsigned a = find(s), b = find((unsigned)(xo / p.slab_elems));
+            if (a != b) parent[std::max(a, b)] = std::min(a, b);
+        }
+    }
+    std::vector<unsigned> root((size_t)nslabs);
+    for (unsigned s = 0; s < (unsigned)nslabs; ++s) root[s] = find(s);
+    std::stable_sort(order.begin(), order.end(), [&](unsigned a, unsigned b) { return root[a] < root[b]; });
+    std::vector<unsigned> group_start;
+    for (unsigned i = 0; i < (unsigned)nslabs; ++i)
+        if (i == 0 || root[order[i]] != root[order[i - 1]]) group_start.push_back(i);
+    p.ngroups = (unsigned)group_start.size();
+    group_start.push_back((unsigned)nslabs);
+    p.norbits = (unsigned)orbits.size();
+    // ---- tables to the device, kept for the life of the process ----------------------------------------------------
+    const size_t b0 = orbits.size() * sizeof(OrbitEntry), b1 = order.size() * 4, b2 = group_start.size() * 4;
+    const size_t o1 = (b0 + 15) / 16 * 16, o2 = o1 + (b1 + 15) / 16 * 16;
+    char *tables = nullptr;
+    cudaError_t e = cudaMalloc((void **)&tables, o2 + b2);
+    if (e != cudaSuccess) return e;
+    e = cudaMemcpy(tables, orbits.data(), b0, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(tables + o1, order.data(), b1, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(tables + o2, group_start.data(), b2, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaFree(tables); return e; }
+    p.orbits = reinterpret_cast<const OrbitEntry *>(tables);
+    p.slab_order = reinterpret_cast<const unsigned *>(tables + o1);
+    p.group_start = reinterpret_cast<const unsigned *>(tables + o2);
+    plan.nslabs = nslabs;
+    plan.grid = (int)std::min<unsigned long long>((unsigned long long)p.ngroups * p.norbits, 148ULL);
+    plan.eligible = true;
+    return cudaSuccess;
+}
+
+}  // namespace
+
+// Returns cudaSuccess with *handled = false when the call is not of this kernel's kind (the caller then runs the
+// gather kernels).
+cudaError_t launch_permsum_orbit(const PermSumDesc &d, cudaStream_t stream, int64_t *launches, bool *handled)
+{
+    *handled = false;
+    if (getenv("TCB_PERMSUM_GENERIC") || getenv("TCB_PERMSUM_NO_ORBIT")) return cudaSuccess;
+    EncodeTiledFn fn = orbit_encode_fn();
+    if (!fn) return cudaSuccess;
+    static std::mutex mu;
+    static std::map<std::vector<long long>, OrbitPlan> plans;
+    OrbitPlan plan;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        const std::vector<long long> key = plan_key(d);
+        auto it = plans.find(key);
+        if (it == plans.end()) {
+            OrbitPlan fresh;
+            cudaError_t e = build_plan(d, fresh);
+            if (e != cudaSuccess) return e;
+            it = plans.emplace(key, fresh).first;
+        }
+        plan = it->second;
+    }
+    if (!plan.eligible) return cudaSuccess;
+    OrbitParams p = plan.p;
+    if ((reinterpret_cast<uintptr_t>(d.X) & 15) != 0) return cudaSuccess;
+    for (int t = 0; t < kOrbTerms; ++t) {
+        p.cr[t] = t < d.nterms ? d.coef_re[t] : 0.0;
+        p.ci[t] = t < d.nterms ? d.coef_im[t] : 0.0;
+    }
+    p.br = d.beta_re; p.bi = d.beta_im;
+    p.beta_zero = (d.beta_re == 0.0 && d.beta_im == 0.0) ? 1 : 0;
+    p.D = (double2 *)d.D;
+    CUtensorMap tm;
+    {
+        const cuuint64_t e = (cuuint64_t)p.eI;
+        cuuint64_t dims[4] = {2 * e, e, e, (cuuint64_t)plan.nslabs};
+        cuuint64_t strides[3] = {e * 16, e * e * 16, e * e * e * 16};
+        cuuint32_t box[4] = {2 * T6, T6, T6, 1}, estr[4] = {1, 1, 1, 1};
+        CUresult r = fn(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void *>(d.X), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return cudaSuccess;              // a shape the map cannot express: the gather kernels
+    }
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(permsum_orbit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    permsum_orbit_kernel<<<plan.grid, kThreads, plan.smem, stream>>>(tm, p);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if (launches) ++*launches;
+    *handled = true;
+    return cudaSuccess;
+}
+
+}  // namespace tcb

@@ -167,15 +167,21 @@ def test_device_generator_matches_host_generator(ctx):
 
 
 @pytest.mark.parametrize("shape,spec,nterms", [
-    ((12, 12, 12, 6, 6, 6), "P(a/bc)P(k/ij):R(a,b,c,i,j,k)+=X(a,b,c,i,j,k)", 9),     # cube 4 x 4 x 2, 9 terms
-    ((12, 12, 12, 6, 6, 6), "P(a/bc):R(a,b,c,i,j,k)+=X(a,b,c,i,j,k)", 3),            # 3 terms inside a slab
+    ((12, 12, 12, 6, 6, 6), "P(a/bc)P(k/ij):R(a,b,c,i,j,k)+=X(a,b,c,i,j,k)", 9),     # orbit kernel, 9 terms, 3 outer classes
+    ((12, 12, 12, 6, 6, 6), "P(a/bc):R(a,b,c,i,j,k)+=X(a,b,c,i,j,k)", 3),            # orbit kernel, 3 terms inside a slab
+    ((14, 14, 14, 3, 3, 3), "P(a/bc)P(k/ij):R(a,b,c,i,j,k)+=X(a,b,c,i,j,k)", 9),     # orbit kernel, ragged cubes (14 = 2*6 + 2)
+    ((14, 14, 14, 3, 3, 3), "P(a/bc)P(k/ij):R(a,b,c,i,j,k)=X(a,b,c,i,j,k)", 9),      # ... beta = 0
+    ((42, 42, 42), "P(a/bc):R(a,b,c)+=X(a,b,c)", 3),                                 # orbit kernel, no outer index
+    ((18, 18, 18, 13), "P(c/ab):R(a,b,c,i)+=X(a,b,c,i)", 3),                         # orbit kernel, one outer index
+    ((12, 12, 12, 6, 6, 6), "P(ab)P(k/ij):R(a,b,c,i,j,k)+=X(a,b,c,i,j,k)", 6),       # c stays put: cube kernel
     ((12, 12, 12, 6, 6, 6), "P(k/ij):R(a,b,c,i,j,k)=X(a,b,c,i,j,k)", 3),             # one unit-stride index, beta = 0
     ((64, 64, 8, 8), "P(ij)P(ab):R(a,b,i,j)+=X(a,b,i,j)", 4),                        # cube 8 x 4, all 32 lanes
     ((30, 30, 18, 18), "P(ab):R(a,b,i,j)+=X(a,b,i,j)", 2),                           # cube 6 x 5, two idle lanes
     ((66, 66, 8, 8), "P(ij)P(ab):R(a,b,i,j)+=X(a,b,i,j)", 4),                        # 66 = 2*3*11: cube 6 x 3 < 24 lanes -> generic
 ])
 def test_permsum_cube_path_is_bit_identical_to_the_oracle(ctx, shape, spec, nterms):
-    """Tensors of >= 2^18 elements take permsum_cube_kernel (warp = micro-cube, running offsets); same term order and
+    """Term sets that permute three leading indices among themselves take permsum_orbit_kernel (TMA-staged orbit cubes),
+    other tensors of >= 2^18 elements permsum_cube_kernel (warp = micro-cube, running offsets); same term order and
     rounding as the oracle -> identical bits for unit coefficients, 1e-14 for a complex alpha."""
     rng = np.random.default_rng(len(shape) * 1000 + nterms)
     D, X = rc(rng, *shape), rc(rng, *shape)
@@ -205,5 +211,14 @@ def test_permsum_cube_path_is_bit_identical_to_the_oracle(ctx, shape, spec, nter
     ctx.antisymmetrize(spec, dD2, dX, alpha)
     ref = oracle.permsum(D, X, perms, [alpha * c for c in coefs], beta)
     assert np.max(np.abs(ctx.tensor_download(dD2) - ref)) <= 1e-14 * (np.abs(D).max() + nterms * np.abs(X).max())
-    for t in (dD, dD2, dX):
+    # the gather kernels give the same bits (the option is read per call)
+    import os
+    os.environ["TCB_PERMSUM_NO_ORBIT"] = "1"
+    try:
+        dD3 = ctx.tensor_from_numpy(D)
+        ctx.antisymmetrize(spec, dD3, dX, alpha)
+        assert ctx.tensor_download(dD3).tobytes() == ctx.tensor_download(dD2).tobytes()
+    finally:
+        del os.environ["TCB_PERMSUM_NO_ORBIT"]
+    for t in (dD, dD2, dD3, dX):
         t.destroy()
