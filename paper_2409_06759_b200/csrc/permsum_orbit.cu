@@ -33,8 +33,8 @@ namespace {
 constexpr int T6 = 6;                       // cube edge
 constexpr int kCube = T6 * T6 * T6;         // 216 elements, 3456 bytes = 27 x 128
 constexpr int kCubeBytes = kCube * 16;
-constexpr int kConsumerWarps = 18;          // 54 warp tasks (6 cubes x 9 (b,c) micro-rows) = 3 rounds
-constexpr int kThreads = (kConsumerWarps + 1) * 32;
+constexpr int kConsumerWarps = 14;          // 162 micro-cubes per orbit = 3 rounds of 14 warps x 4 quarter-warps
+constexpr int kThreads = (kConsumerWarps + 2) * 32;   // + the X producer warp and the D load/store warp
 constexpr int kRounds = 3;
 constexpr int kMaxOmega = 6;                // cubes per orbit
 constexpr int kMaxTau = 6;                  // distinct outer permutations
@@ -49,9 +49,8 @@ struct alignas(4) OrbitEntry {              // one orbit of cube coordinates
 static_assert(sizeof(OrbitEntry) == 76, "OrbitEntry is copied word by word");
 
 struct OrbitParams {
-    int nterms, ntau, nO, stages, eI, ragged, beta_zero;
+    int nterms, ntau, nO, stages, eI, beta_zero;
     int eO[3];                               // outer extents (dims 3..)
-    long long dsI[3], dsO[3];                // strides of the leading / outer dims (D and X have the same shape)
     long long slab_elems;                    // eI^3
     long long xsO[kMaxTau][3];               // stride in X of D's outer index k under outer class u
     int sstr[kOrbTerms][3];                  // shared-memory stride of D's leading index k under term t (1, 6 or 36)
@@ -100,16 +99,21 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap *tm,
         : "memory");
 }
 
-struct alignas(16) StageMeta {               // written by the producer warp before it arms the stage's barrier
-    long long cube[kMaxOmega];               // D offset of cube w
+__device__ __forceinline__ void tma_store_4d(const CUtensorMap *tm, int c0, int c1, int c2, int c3, uint32_t src)
+{
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%1, %2, %3, %4}], [%5];" ::"l"(tm),
+                 "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(src)
+                 : "memory");
+}
+
+struct alignas(16) StageMeta {               // written by the X producer warp before it arms the stage's barrier
     int slot[kMaxOmega][12];                 // element offset (in the stage) of the cube term t reads for cube w
     int n;
-    unsigned char coord[kMaxOmega][4];
     unsigned ob[sizeof(OrbitEntry) / 4];     // producer scratch: the item's orbit entry
 };
 
 // Items: for group g of outer slabs (slabs that are permutations of one another), for orbit o: the group's slabs.
-// CTA b takes the (g, o) pairs b, b + grid, ...; producer and consumers walk the same sequence.
+// CTA b takes the (g, o) pairs b, b + grid, ...; the two producer warps and the consumers walk the same sequence.
 struct ItemCursor {
     unsigned long long pair, npairs;
     unsigned s, s_end, orbit;
@@ -138,41 +142,54 @@ struct ItemCursor {
     }
 };
 
+// barrier indices
+constexpr int kXFull = 0, kXEmpty = kMaxStages, kDFull = 2 * kMaxStages, kDReady = 2 * kMaxStages + 2;
+constexpr int kNumBars = 2 * kMaxStages + 4;
+
 __global__ void __launch_bounds__(kThreads, 1)
-permsum_orbit_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ OrbitParams p)
+permsum_orbit_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmD,
+                     const __grid_constant__ OrbitParams p)
 {
     extern __shared__ __align__(128) uint8_t orb_smem[];
-    __shared__ __align__(8) unsigned long long s_bar[2 * kMaxStages];
+    __shared__ __align__(8) unsigned long long s_bar[kNumBars];
     __shared__ StageMeta s_meta[kMaxStages];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t bar0 = smem_u32(s_bar);
-    const uint32_t data0 = smem_u32(orb_smem);
     const uint32_t stage_bytes = (uint32_t)(kMaxOmega * p.ntau * kCubeBytes);
+    const uint32_t dbuf_bytes = kMaxOmega * kCubeBytes;
+    // shared memory: [2 D buffers of 6 cubes][stages x (6 * ntau cubes of X)]
+    const uint32_t dbuf0 = smem_u32(orb_smem);
+    const uint32_t data0 = dbuf0 + 2 * dbuf_bytes;
     if (tid == 0) {
         for (int s = 0; s < p.stages; ++s) {
-            mbar_init(bar0 + 8 * s, 1);                                  // full: the producer's arrive + the bytes
-            mbar_init(bar0 + 8 * (kMaxStages + s), kConsumerWarps);      // empty: one arrive per consumer warp
+            mbar_init(bar0 + 8 * (kXFull + s), 1);                  // the producer's arrive + the bytes
+            mbar_init(bar0 + 8 * (kXEmpty + s), kConsumerWarps);    // one arrive per consumer warp
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(bar0 + 8 * (kDFull + b), 1);                  // D cubes loaded (or, beta = 0, buffer free)
+            mbar_init(bar0 + 8 * (kDReady + b), kConsumerWarps);    // results written: the buffer may be stored
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmX) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmD) : "memory");
     }
     __syncthreads();
     ItemCursor cur;
     cur.init(p);
     if (warp == kConsumerWarps) {
-        // ================= producer warp =================
+        // ================= X producer warp =================
         unsigned it = 0;
         for (; cur.valid(); cur.advance(p), ++it) {
             const int st = (int)(it % (unsigned)p.stages);
             const uint32_t par = (it / (unsigned)p.stages) & 1u;
             StageMeta &m = s_meta[st];
-            mbar_wait(bar0 + 8 * (kMaxStages + st), par ^ 1u);          // consumers are done with the stage
+            mbar_wait(bar0 + 8 * (kXEmpty + st), par ^ 1u);          // consumers are done with the stage
             {   // the item's orbit entry, word by word
                 const unsigned *src = reinterpret_cast<const unsigned *>(p.orbits + cur.orbit);
                 if (lane < (int)(sizeof(OrbitEntry) / 4)) m.ob[lane] = src[lane];
             }
             unsigned slab = p.slab_order[cur.s];
-            long long doffO = 0, xoffO[kMaxTau];
+            long long xoffO[kMaxTau];
 #pragma unroll
             for (int u = 0; u < kMaxTau; ++u) xoffO[u] = 0;
 #pragma unroll
@@ -180,7 +197,6 @@ permsum_orbit_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
                 if (k < p.nO) {
                     const long long v = slab % (unsigned)p.eO[k];
                     slab /= (unsigned)p.eO[k];
-                    doffO += v * p.dsO[k];
 #pragma unroll
                     for (int u = 0; u < kMaxTau; ++u)
                         if (u < p.ntau) xoffO[u] += v * p.xsO[u][k];
@@ -192,16 +208,9 @@ permsum_orbit_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
                 const int w = idx / kOrbTerms, t = idx - w * kOrbTerms;
                 if (w < n && t < p.nterms) m.slot[w][t] = (ob.src[w][t] * p.ntau + p.tau[t]) * kCube;
             }
-            if (lane < n) {
-                m.cube[lane] = doffO + (long long)ob.coord[lane][0] * T6 * p.dsI[0] +
-                               (long long)ob.coord[lane][1] * T6 * p.dsI[1] + (long long)ob.coord[lane][2] * T6 * p.dsI[2];
-                m.coord[lane][0] = ob.coord[lane][0];
-                m.coord[lane][1] = ob.coord[lane][1];
-                m.coord[lane][2] = ob.coord[lane][2];
-            }
             if (lane == 0) m.n = n;
             __syncwarp();
-            const uint32_t full = bar0 + 8 * st;
+            const uint32_t full = bar0 + 8 * (kXFull + st);
             if (lane == 0) mbar_expect_tx(full, (uint32_t)(n * p.ntau * kCubeBytes));
             __syncwarp();
             for (int idx = lane; idx < n * p.ntau; idx += 32) {
@@ -216,20 +225,62 @@ permsum_orbit_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
         }
         return;
     }
+    if (warp == kConsumerWarps + 1) {
+        // ================= D warp: loads the orbit's cubes of D two items ahead, stores the finished ones ==============
+        // lane w < n owns cube w of the item: one tiled TMA load, one tiled TMA store (bulk groups are per thread)
+        ItemCursor ld = cur;                                          // runs two items ahead of `cur`
+        auto load_item = [&](const ItemCursor &c, int b) {
+            const uint32_t full = bar0 + 8 * (kDFull + b);
+            if (p.beta_zero) {                                       // nothing to read: just hand the buffer over
+                if (lane == 0) mbar_arrive(full);
+                return;
+            }
+            const OrbitEntry *ob = p.orbits + c.orbit;
+            const int n = ob->n;
+            if (lane == 0) mbar_expect_tx(full, (uint32_t)(n * kCubeBytes));
+            __syncwarp();
+            if (lane < n)
+                tma_load_4d(dbuf0 + b * dbuf_bytes + lane * kCubeBytes, &tmD, ob->coord[lane][0] * (2 * T6),
+                            ob->coord[lane][1] * T6, ob->coord[lane][2] * T6, (int)p.slab_order[c.s], full);
+        };
+        for (int b = 0; b < 2; ++b)
+            if (ld.valid()) {
+                load_item(ld, b);
+                ld.advance(p);
+            }
+        unsigned it = 0;
+        for (; cur.valid(); cur.advance(p), ++it) {
+            const int b = (int)(it & 1u);
+            mbar_wait(bar0 + 8 * (kDReady + b), (it >> 1) & 1u);     // every consumer warp has written its results
+            const OrbitEntry *ob = p.orbits + cur.orbit;
+            if (lane < ob->n) {
+                tma_store_4d(&tmD, ob->coord[lane][0] * (2 * T6), ob->coord[lane][1] * T6, ob->coord[lane][2] * T6,
+                             (int)p.slab_order[cur.s], dbuf0 + b * dbuf_bytes + lane * kCubeBytes);
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory read: buffer reusable
+            }
+            __syncwarp();
+            if (ld.valid()) {
+                load_item(ld, b);
+                ld.advance(p);
+            }
+        }
+        asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+        return;
+    }
     // ================= consumer warps =================
-    // per thread, once: its element of every round (cube w, local coordinates) -- the same for every item
+    // A quarter-warp is a 2 x 2 x 2 micro-cube (conflict-free LDS.128 / STS.128 under every permutation of the three
+    // indices); a cube has 27 of them, an orbit <= 162 = 3 rounds of 14 warps x 4.  Element <-> thread is the same for
+    // every item.
     const int qw = lane >> 3, bits = lane & 7;
-    const bool lane_on = qw < 3;
-    int ew[kRounds], soff[kRounds][kOrbTerms], lpack[kRounds];
-    long long dloc[kRounds];
+    int ew[kRounds], soff[kRounds][kOrbTerms], dl[kRounds];
 #pragma unroll
     for (int j = 0; j < kRounds; ++j) {
-        const int wt = warp + kConsumerWarps * j;            // warp task: cube wt / 9, micro-row (m1, m2) = wt % 9
-        ew[j] = wt / 9;
-        const int mr = wt - ew[j] * 9, m2 = mr / 3, m1 = mr - m2 * 3;
-        const int l0 = 2 * (qw % 3) + (bits & 1), l1 = 2 * m1 + ((bits >> 1) & 1), l2 = 2 * m2 + (bits >> 2);
-        lpack[j] = l0 | (l1 << 8) | (l2 << 16);
-        dloc[j] = l0 * p.dsI[0] + l1 * p.dsI[1] + l2 * p.dsI[2];
+        const int q = warp * 4 + qw + kConsumerWarps * 4 * j;
+        ew[j] = q / 27;
+        const int mc = q - ew[j] * 27, m2 = mc / 9, m1 = (mc - m2 * 9) / 3, m0 = mc - m2 * 9 - m1 * 3;
+        const int l0 = 2 * m0 + (bits & 1), l1 = 2 * m1 + ((bits >> 1) & 1), l2 = 2 * m2 + (bits >> 2);
+        dl[j] = ew[j] * kCube + l0 + T6 * l1 + T6 * T6 * l2;
 #pragma unroll
         for (int t = 0; t < kOrbTerms; ++t) soff[j][t] = l0 * p.sstr[t][0] + l1 * p.sstr[t][1] + l2 * p.sstr[t][2];
     }
@@ -237,31 +288,21 @@ permsum_orbit_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
     for (; cur.valid(); cur.advance(p), ++it) {
         const int st = (int)(it % (unsigned)p.stages);
         const uint32_t par = (it / (unsigned)p.stages) & 1u;
+        const int b = (int)(it & 1u);
         const StageMeta &m = s_meta[st];
-        mbar_wait(bar0 + 8 * st, par);
+        mbar_wait(bar0 + 8 * (kXFull + st), par);
+        mbar_wait(bar0 + 8 * (kDFull + b), (it >> 1) & 1u);
         const int n = m.n;
-        const double2 *cubes = reinterpret_cast<const double2 *>(orb_smem + (size_t)st * stage_bytes);
-        bool ok[kRounds];
-        long long doff[kRounds];
-        double2 dv[kRounds];
+        const double2 *cubes = reinterpret_cast<const double2 *>(orb_smem + 2 * dbuf_bytes + (size_t)st * stage_bytes);
+        double2 *dcube = reinterpret_cast<double2 *>(orb_smem + (size_t)b * dbuf_bytes);
 #pragma unroll
         for (int j = 0; j < kRounds; ++j) {
-            ok[j] = lane_on && ew[j] < n;
-            if (ok[j] && p.ragged) {
-#pragma unroll
-                for (int k = 0; k < 3; ++k)
-                    ok[j] = ok[j] && (m.coord[ew[j]][k] * T6 + ((lpack[j] >> (8 * k)) & 255) < p.eI);
-            }
-            doff[j] = ok[j] ? m.cube[ew[j]] + dloc[j] : 0;
-            if (ok[j] && !p.beta_zero) dv[j] = p.D[doff[j]];
-        }
-#pragma unroll
-        for (int j = 0; j < kRounds; ++j) {
-            if (!ok[j]) continue;
+            if (ew[j] >= n) continue;
             double ar = 0.0, ai = 0.0;
             if (!p.beta_zero) {
-                ar = __dsub_rn(__dmul_rn(p.br, dv[j].x), __dmul_rn(p.bi, dv[j].y));
-                ai = __dadd_rn(__dmul_rn(p.br, dv[j].y), __dmul_rn(p.bi, dv[j].x));
+                const double2 dv = dcube[dl[j]];
+                ar = __dsub_rn(__dmul_rn(p.br, dv.x), __dmul_rn(p.bi, dv.y));
+                ai = __dadd_rn(__dmul_rn(p.br, dv.y), __dmul_rn(p.bi, dv.x));
             }
             int sl[12];
             {
@@ -286,10 +327,14 @@ permsum_orbit_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
                         ai = __dadd_rn(ai, __dadd_rn(__dmul_rn(cr, x[u].y), __dmul_rn(ci, x[u].x)));
                     }
             }
-            p.D[doff[j]] = make_double2(ar, ai);
+            dcube[dl[j]] = make_double2(ar, ai);
         }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // results visible to the TMA store
         __syncwarp();
-        if (lane == 0) mbar_arrive(bar0 + 8 * (kMaxStages + st));      // this warp no longer reads the stage
+        if (lane == 0) {
+            mbar_arrive(bar0 + 8 * (kDReady + b));                    // this warp's results are in the D buffer
+            mbar_arrive(bar0 + 8 * (kXEmpty + st));                   // this warp no longer reads the stage
+        }
     }
 }
 
@@ -368,14 +413,11 @@ cudaError_t build_plan(const PermSumDesc &d, OrbitPlan &plan)
     p.nterms = d.nterms;
     p.eI = (int)d.extent[0];
     if (p.eI < T6 || d.extent[0] > 255 * T6) return cudaSuccess;
-    p.ragged = p.eI % T6 ? 1 : 0;
     const int nb = (p.eI + T6 - 1) / T6;
     p.nO = r - 3;
     long long nslabs = 1;
     for (int k = 0; k < 3; ++k) {
-        p.dsI[k] = ds[k];
         p.eO[k] = k < p.nO ? (int)d.extent[3 + k] : 1;
-        p.dsO[k] = k < p.nO ? ds[3 + k] : 0;
         nslabs *= p.eO[k];
     }
     if (nslabs > (1LL << 22)) return cudaSuccess;
@@ -404,9 +446,10 @@ cudaError_t build_plan(const PermSumDesc &d, OrbitPlan &plan)
     for (int u = p.ntau; u < kMaxTau; ++u)
         for (int k = 0; k < 3; ++k) p.xsO[u][k] = 0;
     const size_t stage_bytes = (size_t)kMaxOmega * p.ntau * kCubeBytes;
-    p.stages = (int)std::min<size_t>(kMaxStages, (200 * 1024) / stage_bytes);
+    const size_t dbufs = 2 * (size_t)kMaxOmega * kCubeBytes, budget = 227 * 1024 - 4096;   // static: barriers, stage tables
+    p.stages = (int)std::min<size_t>(kMaxStages, (budget - dbufs) / stage_bytes);
     if (p.stages < 2) return cudaSuccess;
-    plan.smem = stage_bytes * p.stages;
+    plan.smem = dbufs + stage_bytes * p.stages;
     // ---- orbits of the cube coordinates under the terms ------------------------------------------------------------
     const int ncubes = nb * nb * nb;
     auto decode = [&](int id, int *c) { for (int k = 0; k < 3; ++k) { c[k] = id % nb; id /= nb; } };
@@ -528,24 +571,28 @@ cudaError_t launch_permsum_orbit(const PermSumDesc &d, cudaStream_t stream, int6
     p.br = d.beta_re; p.bi = d.beta_im;
     p.beta_zero = (d.beta_re == 0.0 && d.beta_im == 0.0) ? 1 : 0;
     p.D = (double2 *)d.D;
-    CUtensorMap tm;
+    if ((reinterpret_cast<uintptr_t>(d.D) & 15) != 0) return cudaSuccess;
+    CUtensorMap tmX, tmD;
     {
         const cuuint64_t e = (cuuint64_t)p.eI;
         cuuint64_t dims[4] = {2 * e, e, e, (cuuint64_t)plan.nslabs};
         cuuint64_t strides[3] = {e * 16, e * e * 16, e * e * e * 16};
         cuuint32_t box[4] = {2 * T6, T6, T6, 1}, estr[4] = {1, 1, 1, 1};
-        CUresult r = fn(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void *>(d.X), dims, strides, box, estr,
+        CUresult r = fn(&tmX, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void *>(d.X), dims, strides, box, estr,
                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) return cudaSuccess;              // a shape the map cannot express: the gather kernels
+        if (r == CUDA_SUCCESS)
+            r = fn(&tmD, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, d.D, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return cudaSuccess;              // a shape the maps cannot express: the gather kernels
     }
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(permsum_orbit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(permsum_orbit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 4096);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    permsum_orbit_kernel<<<plan.grid, kThreads, plan.smem, stream>>>(tm, p);
+    permsum_orbit_kernel<<<plan.grid, kThreads, plan.smem, stream>>>(tmX, tmD, p);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (launches) ++*launches;
