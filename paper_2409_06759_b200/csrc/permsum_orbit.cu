@@ -38,7 +38,7 @@ constexpr int kThreads = (kConsumerWarps + 2) * 32;   // + the X producer warp a
 constexpr int kRounds = 3;
 constexpr int kMaxOmega = 6;                // cubes per orbit
 constexpr int kMaxTau = 6;                  // distinct outer permutations
-constexpr int kMaxStages = 4;
+constexpr int kMaxStages = 8;
 constexpr int kOrbTerms = 9;
 
 struct alignas(4) OrbitEntry {              // one orbit of cube coordinates
@@ -183,12 +183,13 @@ permsum_orbit_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
             const int st = (int)(it % (unsigned)p.stages);
             const uint32_t par = (it / (unsigned)p.stages) & 1u;
             StageMeta &m = s_meta[st];
+            // the item's orbit entry (word by word) and slab: fetched before the wait, so their latency hides behind it
+            unsigned ob_word = 0;
+            if (lane < (int)(sizeof(OrbitEntry) / 4))
+                ob_word = __ldg(reinterpret_cast<const unsigned *>(p.orbits + cur.orbit) + lane);
+            unsigned slab = __ldg(p.slab_order + cur.s);
             mbar_wait(bar0 + 8 * (kXEmpty + st), par ^ 1u);          // consumers are done with the stage
-            {   // the item's orbit entry, word by word
-                const unsigned *src = reinterpret_cast<const unsigned *>(p.orbits + cur.orbit);
-                if (lane < (int)(sizeof(OrbitEntry) / 4)) m.ob[lane] = src[lane];
-            }
-            unsigned slab = p.slab_order[cur.s];
+            if (lane < (int)(sizeof(OrbitEntry) / 4)) m.ob[lane] = ob_word;
             long long xoffO[kMaxTau];
 #pragma unroll
             for (int u = 0; u < kMaxTau; ++u) xoffO[u] = 0;
@@ -229,39 +230,48 @@ permsum_orbit_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
         // ================= D warp: loads the orbit's cubes of D two items ahead, stores the finished ones ==============
         // lane w < n owns cube w of the item: one tiled TMA load, one tiled TMA store (bulk groups are per thread)
         ItemCursor ld = cur;                                          // runs two items ahead of `cur`
-        auto load_item = [&](const ItemCursor &c, int b) {
+        auto cube_coords = [&](const ItemCursor &c, int *n, int *c0, int *c1, int *c2, int *c3) {
+            const OrbitEntry *ob = p.orbits + c.orbit;
+            *n = __ldg(&ob->n);
+            const int w = lane < kMaxOmega ? lane : 0;
+            *c0 = __ldg(&ob->coord[w][0]) * (2 * T6);
+            *c1 = __ldg(&ob->coord[w][1]) * T6;
+            *c2 = __ldg(&ob->coord[w][2]) * T6;
+            *c3 = (int)__ldg(p.slab_order + c.s);
+        };
+        auto load_item = [&](int b, int n, int c0, int c1, int c2, int c3) {
             const uint32_t full = bar0 + 8 * (kDFull + b);
             if (p.beta_zero) {                                       // nothing to read: just hand the buffer over
                 if (lane == 0) mbar_arrive(full);
                 return;
             }
-            const OrbitEntry *ob = p.orbits + c.orbit;
-            const int n = ob->n;
             if (lane == 0) mbar_expect_tx(full, (uint32_t)(n * kCubeBytes));
             __syncwarp();
-            if (lane < n)
-                tma_load_4d(dbuf0 + b * dbuf_bytes + lane * kCubeBytes, &tmD, ob->coord[lane][0] * (2 * T6),
-                            ob->coord[lane][1] * T6, ob->coord[lane][2] * T6, (int)p.slab_order[c.s], full);
+            if (lane < n) tma_load_4d(dbuf0 + b * dbuf_bytes + lane * kCubeBytes, &tmD, c0, c1, c2, c3, full);
         };
         for (int b = 0; b < 2; ++b)
             if (ld.valid()) {
-                load_item(ld, b);
+                int n, c0, c1, c2, c3;
+                cube_coords(ld, &n, &c0, &c1, &c2, &c3);
+                load_item(b, n, c0, c1, c2, c3);
                 ld.advance(p);
             }
         unsigned it = 0;
         for (; cur.valid(); cur.advance(p), ++it) {
             const int b = (int)(it & 1u);
+            int sn, s0, s1, s2, s3, ln = 0, l0 = 0, l1 = 0, l2 = 0, l3 = 0;
+            cube_coords(cur, &sn, &s0, &s1, &s2, &s3);               // fetched before the wait
+            const bool more = ld.valid();
+            if (more) cube_coords(ld, &ln, &l0, &l1, &l2, &l3);
             mbar_wait(bar0 + 8 * (kDReady + b), (it >> 1) & 1u);     // every consumer warp has written its results
-            const OrbitEntry *ob = p.orbits + cur.orbit;
-            if (lane < ob->n) {
-                tma_store_4d(&tmD, ob->coord[lane][0] * (2 * T6), ob->coord[lane][1] * T6, ob->coord[lane][2] * T6,
-                             (int)p.slab_order[cur.s], dbuf0 + b * dbuf_bytes + lane * kCubeBytes);
+            if (lane < sn) {
+                tma_store_4d(&tmD, s0, s1, s2, s3, dbuf0 + b * dbuf_bytes + lane * kCubeBytes);
                 asm volatile("cp.async.bulk.commit_group;" ::: "memory");
                 asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory read: buffer reusable
             }
             __syncwarp();
-            if (ld.valid()) {
-                load_item(ld, b);
+            if (more) {
+                load_item(b, ln, l0, l1, l2, l3);
                 ld.advance(p);
             }
         }
@@ -371,6 +381,7 @@ std::vector<long long> plan_key(const PermSumDesc &d)
     int dev = 0;
     cudaGetDevice(&dev);
     k.push_back(dev);
+    k.push_back(getenv("TCB_PERMSUM_ORBIT") ? 1 : 0);
     k.push_back(d.rank);
     k.push_back(d.nterms);
     for (int s = 0; s < d.rank; ++s) k.push_back(d.extent[s]);
@@ -384,7 +395,10 @@ std::vector<long long> plan_key(const PermSumDesc &d)
 cudaError_t build_plan(const PermSumDesc &d, OrbitPlan &plan)
 {
     const int r = d.rank;
-    if (r < 3 || d.nterms < 2 || d.nterms > kOrbTerms) return cudaSuccess;
+    // measured on (60,60,60,12,12,12): 9 terms 4.3 ms here against 8.5 ms for the cube kernel; 3 terms 3.7 against 3.6 (both
+    // near what HBM gives for 96-byte rows) -> the gather kernel keeps the short sums unless the caller forces this one
+    const bool always = getenv("TCB_PERMSUM_ORBIT") != nullptr;
+    if (r < 3 || d.nterms < (always ? 2 : 4) || d.nterms > kOrbTerms) return cudaSuccess;
     long long n = 1, ds[kMaxRank];
     for (int k = 0; k < r; ++k) {
         if (d.extent[k] < 2) return cudaSuccess;             // extent-1 indices: X strides are ambiguous
@@ -448,6 +462,7 @@ cudaError_t build_plan(const PermSumDesc &d, OrbitPlan &plan)
     const size_t stage_bytes = (size_t)kMaxOmega * p.ntau * kCubeBytes;
     const size_t dbufs = 2 * (size_t)kMaxOmega * kCubeBytes, budget = 227 * 1024 - 4096;   // static: barriers, stage tables
     p.stages = (int)std::min<size_t>(kMaxStages, (budget - dbufs) / stage_bytes);
+    if (getenv("TCB_ORBIT_STAGES")) p.stages = std::min(p.stages, atoi(getenv("TCB_ORBIT_STAGES")));
     if (p.stages < 2) return cudaSuccess;
     plan.smem = dbufs + stage_bytes * p.stages;
     // ---- orbits of the cube coordinates under the terms ------------------------------------------------------------
@@ -573,17 +588,18 @@ cudaError_t launch_permsum_orbit(const PermSumDesc &d, cudaStream_t stream, int6
     p.D = (double2 *)d.D;
     if ((reinterpret_cast<uintptr_t>(d.D) & 15) != 0) return cudaSuccess;
     CUtensorMap tmX, tmD;
+    static const CUtensorMapL2promotion kPromo = getenv("TCB_ORBIT_PROMO") ? (CUtensorMapL2promotion)atoi(getenv("TCB_ORBIT_PROMO")) : CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
     {
         const cuuint64_t e = (cuuint64_t)p.eI;
         cuuint64_t dims[4] = {2 * e, e, e, (cuuint64_t)plan.nslabs};
         cuuint64_t strides[3] = {e * 16, e * e * 16, e * e * e * 16};
         cuuint32_t box[4] = {2 * T6, T6, T6, 1}, estr[4] = {1, 1, 1, 1};
         CUresult r = fn(&tmX, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void *>(d.X), dims, strides, box, estr,
-                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, kPromo,
                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r == CUDA_SUCCESS)
             r = fn(&tmD, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, d.D, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                   CU_TENSOR_MAP_SWIZZLE_NONE, kPromo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return cudaSuccess;              // a shape the maps cannot express: the gather kernels
     }
     static bool configured = false;

@@ -220,5 +220,13 @@ def test_permsum_cube_path_is_bit_identical_to_the_oracle(ctx, shape, spec, nter
         assert ctx.tensor_download(dD3).tobytes() == ctx.tensor_download(dD2).tobytes()
     finally:
         del os.environ["TCB_PERMSUM_NO_ORBIT"]
-    for t in (dD, dD2, dD3, dX):
+    # ... and so does the orbit kernel where it is not the default (fewer than 4 terms); a no-op for other term sets
+    os.environ["TCB_PERMSUM_ORBIT"] = "1"
+    try:
+        dD4 = ctx.tensor_from_numpy(D)
+        ctx.antisymmetrize(spec, dD4, dX, 1.0)
+        assert ctx.tensor_download(dD4).tobytes() == ctx.tensor_download(dD).tobytes()
+    finally:
+        del os.environ["TCB_PERMSUM_ORBIT"]
+    for t in (dD, dD2, dD3, dD4, dX):
         t.destroy()
