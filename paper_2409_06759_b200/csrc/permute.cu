@@ -12,7 +12,7 @@
 // flight for HBM3e, so the LOAD side is asynchronous bulk copies (cp.async.bulk.shared::cluster.global, SASS
 // UBLKCP): every contiguous input run of a tile ("row" = the tile's extent along the input unit-stride dim) is
 // one bulk copy straight into shared memory, completion counted on an mbarrier; tiles rotate through a ring of
-// 2..4 stages, so each CTA has stages-1 tiles (up to ~100 KB) in flight while it drains one.  Rows are copied to
+// 2 stages (TCB_PERM_STAGES: up to 4), so each CTA has one tile (~33 KB) in flight while it drains one.  Rows are copied to
 // a padded pitch (the stride of the output-fastest dim is odd in 16-byte units), which makes the STORE side --
 // threads gather the tile in output order with LDS.128 and write coalesced STG.128 -- bank-conflict free.
 // A bulk copy costs its issuing warp ~32 cycles, so the rows of a tile are dealt round-robin to all 8 warps.
@@ -417,7 +417,9 @@ cudaError_t launch_permute(const PermuteDesc &pd, cudaStream_t stream, int64_t *
     if (p.vol > 8 * PT) ctas_per_sm = 1;      // the J = 16 instantiation is compiled for one CTA per SM (registers)
     while (ctas_per_sm > 1 && 2 * p.tile_bytes > 200 * 1024 / ctas_per_sm - 128) --ctas_per_sm;
     const int budget = 200 * 1024 / ctas_per_sm - 128;
-    p.stages = std::max(2, std::min(env_int("TCB_PERM_STAGES", 4), budget / p.tile_bytes));
+    // measured (r1c sweep): 2 stages beat 3-4 on every shape from 324 MB up (medians 4.9 -> 5.3, 5.2 -> 5.55, 5.6 -> 6.0 TB/s):
+    // one tile in flight per CTA is enough with two CTAs per SM, and the shared memory not taken stays L1
+    p.stages = std::max(2, std::min(env_int("TCB_PERM_STAGES", 2), budget / p.tile_bytes));
     const size_t smem = (size_t)p.stages * p.tile_bytes + 128;
     if (smem > 227 * 1024) return cudaErrorInvalidValue;
     p.in = (const double2 *)pd.in;
