@@ -111,6 +111,14 @@ int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor
 int tcb_add(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor *L, tcb_c128 alpha);
 /* D *= alpha */
 int tcb_scale(tcb_ctx *ctx, tcb_tensor *D, tcb_c128 alpha);
+/* Next row 8(f)-3, the solver around the residual: the Jacobi step with orbital-energy denominators ("adding energy
+ * denominators to selected terms"; one such step per CC iteration):
+ *     T[i0,i1,..] += alpha * R[i0,i1,..] / (eps[0][i0] + eps[1][i1] + ...)      energies summed in index order
+ * eps: HOST array of rank pointers; eps[k] = extent_k real doubles, or NULL when index k does not enter the
+ * denominator (at least one must be given).  For t_ij^ab stored T(a,b,i,j): eps = {-e_virt, -e_virt, +e_occ, +e_occ}.
+ * T and R have the same shape and must not overlap.  The energies are copied before the call returns.  A zero
+ * denominator is not detected (the quotient is IEEE inf/nan).  Errors: TCB_EINVAL, TCB_ESHAPE, TCB_EALIAS, TCB_ECUDA. */
+int tcb_denominator_update(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, const double *const *eps, tcb_c128 alpha);
 /* S3, tensor transposition: "D(i,j,a,b)=L(a,b,i,j)", pure data movement, bit-exact. */
 int tcb_permute(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor *L);
 /* S6, fused permute-sum (the generator's unrolled permutation operators):

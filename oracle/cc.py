@@ -241,6 +241,45 @@ def ccd_residual_program(B, T, long_double=True):
 
 
 # ------------------------------------------------------------------------------------------
+# next row 8(f)-3: the Jacobi iteration around the residual (energy denominators; a "CC iteration",
+# PAPER.md:406-410).  The paper does not print the update; it is the textbook fixed-point step, PINNED in
+# tests/test_oracle_cc.py: the first step from T = 0 is the MP2 amplitude closed form, and the converged
+# amplitudes zero the tier-0 (Fock-space) doubles projection.
+# ------------------------------------------------------------------------------------------
+def denominator_update(T, R, eps, alpha=1.0):
+    """T[i0,i1,..] + alpha * R[i0,i1,..] / (eps[0][i0] + eps[1][i1] + ...), energies summed in index order,
+    real and imaginary parts divided separately.  eps[k] = None: index k does not enter."""
+    d = np.zeros(T.shape, dtype=np.float64, order="F")
+    for k, e in enumerate(eps):
+        if e is not None:
+            shape = [1] * T.ndim
+            shape[k] = T.shape[k]
+            d = d + np.asarray(e, dtype=np.float64).reshape(shape)
+    q = (R.real / d) + 1j * (R.imag / d)
+    return np.asfortranarray(T + alpha * q)
+
+
+def ccd_energy(B, T):
+    """E_corr = 1/4 sum <ij||ab> t_ij^ab"""
+    return complex(np.asarray(_o.contract("E()=W(i,j,a,b)*T(a,b,i,j)", np.zeros(()), B["oovv"], T, 0.25,
+                                          want_snorm=False)[0]).reshape(-1)[0])
+
+
+def ccd_jacobi(B, e_occ, e_virt, iterations, T0=None):
+    """T <- T + R(T) / (e_i + e_j - e_a - e_b), `iterations` times from T0 (default 0).  R contains the full Fock terms,
+    so the fixed point has R = 0 whatever diagonal is used as denominator.  Returns (T, [E_corr after each step])."""
+    v, o = B["vvoo"].shape[0], B["vvoo"].shape[2]
+    T = np.zeros((v, v, o, o), dtype=np.complex128, order="F") if T0 is None else np.asfortranarray(T0).copy(order="F")
+    ev, eo = -np.asarray(e_virt, dtype=np.float64), np.asarray(e_occ, dtype=np.float64)
+    energies = []
+    for _ in range(iterations):
+        R = ccd_residual_program(B, T)
+        T = denominator_update(T, R, [ev, ev, eo, eo], 1.0)
+        energies.append(ccd_energy(B, T))
+    return T, energies
+
+
+# ------------------------------------------------------------------------------------------
 # config 4: CCSDT piece
 # ------------------------------------------------------------------------------------------
 def _swap(X, p, q):

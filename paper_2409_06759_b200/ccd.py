@@ -66,6 +66,28 @@ def ccd_energy(ctx, B, T):
     return E
 
 
+def ccd_solve(ctx, B, e_occ, e_virt, iterations, T=None):
+    """Jacobi iterations of the CCD amplitude equations (PAPER.md:212 energy denominators, 406-410 "CC
+    iteration"):  T <- T + R(T) / (e_i + e_j - e_a - e_b), from T (default: a zero tensor, whose first step is the MP2
+    guess).  Every step is `ccd_residual` + one `tcb_denominator_update` + the rank-0 energy contraction; only the
+    16-byte energy comes back to the host per iteration.  Returns (T, [E_corr after each step])."""
+    import numpy as np
+    v, _, o, _ = B["vvoo"].extents
+    if T is None:
+        T = ctx.tensor_create((v, v, o, o))
+    ev, eo = -np.asarray(e_virt, dtype=np.float64), np.asarray(e_occ, dtype=np.float64)
+    R = ctx.tensor_create((v, v, o, o))
+    energies = []
+    for _ in range(iterations):
+        ccd_residual(ctx, B, T, R)
+        ctx.denominator_update(T, R, [ev, ev, eo, eo], 1.0)
+        E = ccd_energy(ctx, B, T)
+        energies.append(complex(ctx.tensor_download(E)))
+        E.destroy()
+    R.destroy()
+    return T, energies
+
+
 CCD_FLOPS = lambda o, v: 8.0 * (                 # 8 real flop per complex multiply-add
     v * v * o * o * v                            # Fock vv
     + v * v * o * o * o                          # Fock oo

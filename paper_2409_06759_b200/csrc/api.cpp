@@ -684,6 +684,43 @@ int tcb_scale(tcb_ctx *ctx, tcb_tensor *D, tcb_c128 alpha)
     return TCB_OK;
 }
 
+int tcb_denominator_update(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, const double *const *eps, tcb_c128 alpha)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!T || !R || !eps) return set_error(ctx, TCB_EINVAL, "null argument");
+    const int r = T->shape.rank;
+    if (R->shape.rank != r) return set_error(ctx, TCB_ESHAPE, "rank mismatch");
+    for (int k = 0; k < r; ++k)
+        if (R->shape.ext[k] != T->shape.ext[k]) return set_error(ctx, TCB_ESHAPE, "T and R differ in shape");
+    if (overlaps(T, R)) return set_error(ctx, TCB_EALIAS, "T overlaps R");
+    std::vector<double> host;
+    int at[kMaxRank];
+    bool any = false;
+    for (int k = 0; k < kMaxRank; ++k) {
+        at[k] = -1;
+        if (k < r && eps[k]) {
+            at[k] = (int)host.size();
+            host.insert(host.end(), eps[k], eps[k] + T->shape.ext[k]);
+            any = true;
+        }
+    }
+    if (!any) return set_error(ctx, TCB_EINVAL, "no index carries orbital energies: the denominator would be zero");
+    // the energies travel with the call: a few hundred doubles, stream-ordered allocation (pageable source: the copy
+    // is staged before cudaMemcpyAsync returns)
+    double *dev = nullptr;
+    TCB_CUDA(ctx, cudaMallocAsync((void **)&dev, host.size() * sizeof(double), ctx->stream));
+    cudaError_t e = cudaMemcpyAsync(dev, host.data(), host.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) {
+        TimedLaunch tl(ctx, kClsElementwise, 0.0, 48.0 * (double)T->elems());
+        e = launch_denominator_update(T->ptr, R->ptr, r, T->shape.ext, dev, at, alpha.re, alpha.im, ctx->stream,
+                                      &ctx->launches);
+    }
+    cudaFreeAsync(dev, ctx->stream);
+    TCB_CUDA(ctx, e);
+    return TCB_OK;
+}
+
 int tcb_permsum(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, int nterms, const int32_t *perms,
                 const tcb_c128 *coefs, tcb_c128 beta)
 {

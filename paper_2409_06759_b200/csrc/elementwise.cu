@@ -75,4 +75,60 @@ cudaError_t launch_axpy(void *D, const void *L, int64_t n, double re, double im,
     return e;
 }
 
+// T[idx] += alpha * R[idx] / (sum_k eps_k[idx_k])  -- the Jacobi step of a CC solver (orbital-energy denominators)
+struct DenomParams {
+    int rank;
+    long long e[kMaxRank];
+    int eps_at[kMaxRank];            // start of dim k's energies in `eps`, -1: the index does not enter the denominator
+    const double *eps;
+    double2 *T;
+    const double2 *R;
+    long long n;
+    double ar, ai;
+};
+
+__global__ void __launch_bounds__(256) denominator_update_kernel(const __grid_constant__ DenomParams p)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < p.n; i += stride) {
+        unsigned long long rem = (unsigned long long)i;
+        double d = 0.0;
+#pragma unroll
+        for (int k = 0; k < kMaxRank; ++k)
+            if (k < p.rank) {
+                const unsigned long long q = rem / (unsigned long long)p.e[k];
+                const long long ik = (long long)(rem - q * (unsigned long long)p.e[k]);
+                rem = q;
+                if (p.eps_at[k] >= 0) d = __dadd_rn(d, p.eps[p.eps_at[k] + ik]);      // summed in index order
+            }
+        const double2 r = p.R[i];
+        const double qr = __ddiv_rn(r.x, d), qi = __ddiv_rn(r.y, d);
+        double2 t = p.T[i];
+        t.x = __dadd_rn(t.x, __dsub_rn(__dmul_rn(p.ar, qr), __dmul_rn(p.ai, qi)));
+        t.y = __dadd_rn(t.y, __dadd_rn(__dmul_rn(p.ar, qi), __dmul_rn(p.ai, qr)));
+        p.T[i] = t;
+    }
+}
+
+cudaError_t launch_denominator_update(void *T, const void *R, int rank, const int64_t *extent, const double *eps_dev,
+                                      const int *eps_at, double re, double im, cudaStream_t s, int64_t *launches)
+{
+    DenomParams p;
+    p.rank = rank;
+    p.n = 1;
+    for (int k = 0; k < kMaxRank; ++k) {
+        p.e[k] = k < rank ? extent[k] : 1;
+        p.eps_at[k] = k < rank ? eps_at[k] : -1;
+        p.n *= p.e[k];
+    }
+    p.eps = eps_dev;
+    p.T = (double2 *)T;
+    p.R = (const double2 *)R;
+    p.ar = re; p.ai = im;
+    denominator_update_kernel<<<grid_for(p.n), 256, 0, s>>>(p);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && launches) ++*launches;
+    return e;
+}
+
 }  // namespace tcb

@@ -85,3 +85,46 @@ def test_ccd_energy_is_a_rank0_contraction(ctx, o, v):
         g = synth.tensor(synth.SEED0 + 2, 1, [n] * 4, antisym=((0, 1), (2, 3)), sigma=0.1, hermitian=True)
         e_ref = cc.ccd_residual_unfactorised(o, f, g, T)[1]
         assert abs(complex(got) - complex(e_ref)) <= 1e-11 * float(np.asarray(sn).reshape(-1)[0])
+
+
+@pytest.mark.parametrize("shape,eps_on,alpha", [
+    ((5, 5, 3, 3), (1, 1, 1, 1), 1.0),
+    ((7, 3, 5), (1, 0, 1), 0.5 - 2.0j),
+    ((4, 4, 4, 3, 3, 3), (1, 1, 1, 1, 1, 1), -1.0),
+    ((300, 7), (0, 1), 1.0j),
+])
+def test_denominator_update_matches_the_oracle(ctx, shape, eps_on, alpha):
+    """tcb_denominator_update: T += alpha * R / (sum_k eps_k[i_k]), energies summed in index order, components divided
+    separately -- the same roundings as the oracle, so the bound is a few ulp."""
+    rng = np.random.default_rng(sum(shape))
+    T = np.asfortranarray(rng.standard_normal(shape) + 1j * rng.standard_normal(shape))
+    R = np.asfortranarray(rng.standard_normal(shape) + 1j * rng.standard_normal(shape))
+    eps = [rng.uniform(0.5, 2.0, e) if on else None for e, on in zip(shape, eps_on)]
+    dT, dR = ctx.tensor_from_numpy(T), ctx.tensor_from_numpy(R)
+    ctx.denominator_update(dT, dR, eps, alpha)
+    got, ref = ctx.tensor_download(dT), cc.denominator_update(T, R, eps, alpha)
+    assert np.max(np.abs(got - ref)) <= 4e-16 * (np.abs(T).max() + abs(alpha) * np.abs(R).max() / 0.5)
+    with pytest.raises(pkg.TcbError):
+        ctx.denominator_update(dT, dR, [None] * len(shape), 1.0)          # no energies at all
+    with pytest.raises(pkg.TcbError):
+        ctx.denominator_update(dT, dT, eps, 1.0)                           # T aliases R
+    for t in (dT, dR):
+        t.destroy()
+
+
+def test_ccd_jacobi_iterations_follow_the_oracle(ctx):
+    """Five CC iterations (residual program + denominator update + rank-0 energy) on the GPU against the same five on
+    the oracle; the converged run zeroes the residual (whose Fock-space pin is in tests/test_oracle_cc.py)."""
+    o, v = 3, 5
+    B, T_mp2, eo, ev = synth.config_ccd(o, v)
+    dB = {k: ctx.tensor_from_numpy(x) for k, x in B.items()}
+    dT, energies = ccd.ccd_solve(ctx, dB, eo, ev, 5)
+    T_ref, e_ref = cc.ccd_jacobi(B, eo, ev, 5)
+    assert np.max(np.abs(ctx.tensor_download(dT) - T_ref)) <= 1e-11 * np.abs(T_ref).max()
+    for e, r in zip(energies, e_ref):
+        assert abs(e - r) <= 1e-11 * abs(r)
+    dT, energies = ccd.ccd_solve(ctx, dB, eo, ev, 35, dT)
+    dR = ccd.ccd_residual(ctx, dB, dT)
+    assert np.max(np.abs(ctx.tensor_download(dR))) <= 1e-11 * np.abs(B["vvoo"]).max()
+    assert abs(energies[-1] - energies[-2]) <= 1e-12 * abs(energies[-1])
+    assert abs(energies[-1] - cc.ccd_jacobi(B, eo, ev, 40)[1][-1]) <= 1e-11 * abs(energies[-1])

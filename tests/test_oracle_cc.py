@@ -85,3 +85,52 @@ def test_t3_term_against_fock_space_triples_projection():
     Xp, R3p = cc.t3_term_program(np.asfortranarray(W), np.asfortranarray(t), np.zeros_like(X))
     assert np.abs(Xp - X).max() <= 1e-13 * np.abs(X).max()
     assert np.abs(R3p - Y).max() <= 1e-13 * np.abs(Y).max()
+
+
+def _ccd_problem(o, v):
+    """config_ccd blocks plus the full f and g they were cut from (the generator is keyed by global spinor labels)"""
+    from paper_2409_06759_b200 import synth
+    B, T_mp2, eo, ev = synth.config_ccd(o, v)
+    n = o + v
+    f = np.zeros((n, n), dtype=np.complex128)
+    f[:o, :o], f[o:, o:] = B["foo"], B["fvv"]
+    g = synth.tensor(synth.SEED0 + 2, 1, [n] * 4, antisym=((0, 1), (2, 3)), sigma=0.1, hermitian=True)
+    return B, T_mp2, eo, ev, f, g
+
+
+def test_jacobi_first_step_from_zero_is_the_mp2_closed_form():
+    """T = 0: R = <ab||ij>, so one step gives t = <ab||ij> / (e_i + e_j - e_a - e_b) -- the generator's own MP2
+    amplitudes, written there from the closed form -- and E = 1/4 sum |<ab||ij>|^2 / (e_i + e_j - e_a - e_b) < 0."""
+    B, T_mp2, eo, ev, f, g = _ccd_problem(3, 4)
+    T, energies = cc.ccd_jacobi(B, eo, ev, 1)
+    assert np.abs(T - T_mp2).max() <= 1e-14 * np.abs(T_mp2).max()
+    d = eo[None, None, :, None] + eo[None, None, None, :] - ev[:, None, None, None] - ev[None, :, None, None]
+    e_closed = 0.25 * np.sum(np.abs(B["vvoo"]) ** 2 / d)
+    assert e_closed < 0 and abs(energies[0] - e_closed) <= 1e-13 * abs(e_closed)
+    assert abs(energies[0].imag) <= 1e-15 * abs(e_closed)
+
+
+def test_denominator_update_closed_form_and_skipped_indices():
+    rng = np.random.default_rng(5)
+    T = np.asfortranarray(rng.standard_normal((3, 4, 2)) + 1j * rng.standard_normal((3, 4, 2)))
+    R = np.asfortranarray(rng.standard_normal((3, 4, 2)) + 1j * rng.standard_normal((3, 4, 2)))
+    e0, e2 = rng.uniform(1, 2, 3), rng.uniform(1, 2, 2)
+    got = cc.denominator_update(T, R, [e0, None, e2], 0.5 - 2j)
+    for i in range(3):
+        for j in range(4):
+            for k in range(2):
+                assert abs(got[i, j, k] - (T[i, j, k] + (0.5 - 2j) * R[i, j, k] / (e0[i] + e2[k]))) <= 1e-15 * 8
+
+
+@pytest.mark.parametrize("o,v", [(2, 3), (3, 3)])
+def test_converged_jacobi_amplitudes_zero_the_fock_space_projection(o, v):
+    """The fixed point of the iteration solves PAPER Eq. (3): <Phi_ij^ab| exp(-T) H exp(T) |Phi0> = 0, evaluated on the
+    Fock space (tier 0) -- which shares nothing with the factorised program the iteration runs on -- and the energy of
+    the last step is the tier-0 <Phi0| exp(-T) H exp(T) |Phi0> - <Phi0|H|Phi0>."""
+    B, T_mp2, eo, ev, f, g = _ccd_problem(o, v)
+    T, energies = cc.ccd_jacobi(B, eo, ev, 40)
+    e0, _, r0 = cc.fock_space_residuals(o, v, f, g, T)
+    assert np.abs(r0).max() <= 1e-12 * np.abs(B["vvoo"]).max()
+    assert abs(energies[-1] - e0) <= 1e-12 * abs(e0)
+    assert abs(energies[-1] - energies[-2]) <= 1e-13 * abs(e0)
+    assert np.abs(T - T_mp2).max() > 1e-3 * np.abs(T_mp2).max()          # it did move away from the MP2 guess
