@@ -241,6 +241,127 @@ def ccd_residual_program(B, T, long_double=True):
 
 
 # ------------------------------------------------------------------------------------------
+# CCSD (next row 8(f)-3; the paper's scaling benchmark is a CCSD iteration).  The paper prints only
+# Eqs. (1)-(4); these are the textbook intermediates (Stanton et al. form, refs. at PAPER.md:216) in residual form (full
+# Fock matrix, no denominators), PINNED to tier 0 in tests/test_oracle_cc.py.  t1[a,i] = t_i^a.
+# ------------------------------------------------------------------------------------------
+def block(o, g, name):
+    """<pq||rs> block by letters, e.g. 'ovvo' -> g[O,V,V,O] (bra-ket order), Fortran-contiguous."""
+    rng = {"o": slice(0, o), "v": slice(o, None)}
+    return np.asfortranarray(g[tuple(rng[c] for c in name)])
+
+
+CCSD_BLOCKS = ("vvoo", "oovv", "oooo", "vvvv", "ovvo", "ooov", "ovvv", "vovv", "oovo", "ovov", "vvvo", "ovoo")
+
+
+def ccsd_blocks(o, f, g):
+    B = {name: block(o, g, name) for name in CCSD_BLOCKS}
+    O, V = slice(0, o), slice(o, None)
+    for name, sl in (("foo", (O, O)), ("fvv", (V, V)), ("fov", (O, V)), ("fvo", (V, O))):
+        B[name] = np.asfortranarray(f[sl])
+    return B
+
+
+def ccsd_residual_unfactorised(o, f, g, t1, t2):
+    """(E_corr, R1[a,i], R2[a,b,i,j]) of spin-orbital CCSD:
+    tau~ = t2 + 1/2 (t1 t1 - a<->b), tau = t2 + t1 t1 - a<->b
+    Fae = f_ae - 1/2 f_me t_m^a + t_m^f <ma||fe> - 1/2 tau~_mn^af <mn||ef>
+    Fmi = f_mi + 1/2 t_i^e f_me + t_n^e <mn||ie> + 1/2 tau~_in^ef <mn||ef>;   Fme = f_me + t_n^f <mn||ef>
+    Wmnij = <mn||ij> + P(ij) t_j^e <mn||ie> + 1/4 tau_ij^ef <mn||ef>
+    Wabef = <ab||ef> - P(ab) t_m^b <am||ef> + 1/4 tau_mn^ab <mn||ef>
+    Wmbej = <mb||ej> + t_j^f <mb||ef> - t_n^b <mn||ej> - (1/2 t_jn^fb + t_j^f t_n^b) <mn||ef>
+    R1 = f_ai + t_i^e Fae - t_m^a Fmi + t_im^ae Fme - t_n^f <na||if> - 1/2 t_im^ef <ma||ef> - 1/2 t_mn^ae <nm||ei>
+    R2 = <ab||ij> + P(ab) t_ij^ae (Fbe - 1/2 t_m^b Fme) - P(ij) t_im^ab (Fmj + 1/2 t_j^e Fme) + 1/2 tau_mn^ab Wmnij
+         + 1/2 tau_ij^ef Wabef + P(ij)P(ab) (t_im^ae Wmbej - t_i^e t_m^a <mb||ej>) + P(ij) t_i^e <ab||ej> - P(ab) t_m^a <mb||ij>
+    E = f_ia t_i^a + 1/4 <ij||ab> t_ij^ab + 1/2 <ij||ab> t_i^a t_j^b"""
+    B = ccsd_blocks(o, f, g)
+    es = np.einsum
+    tt = es("ai,bj->abij", t1, t1)
+    tau_t = t2 + 0.5 * (tt - tt.transpose(1, 0, 2, 3))
+    tau = t2 + tt - tt.transpose(1, 0, 2, 3)
+    Fae = (B["fvv"] - 0.5 * es("me,am->ae", B["fov"], t1) + es("fm,mafe->ae", t1, B["ovvv"])
+           - 0.5 * es("afmn,mnef->ae", tau_t, B["oovv"]))
+    Fmi = (B["foo"] + 0.5 * es("ei,me->mi", t1, B["fov"]) + es("en,mnie->mi", t1, B["ooov"])
+           + 0.5 * es("efin,mnef->mi", tau_t, B["oovv"]))
+    Fme = B["fov"] + es("fn,mnef->me", t1, B["oovv"])
+    Wmnij = B["oooo"] + _P(es("ej,mnie->mnij", t1, B["ooov"]), 2, 3) + 0.25 * es("efij,mnef->mnij", tau, B["oovv"])
+    Wabef = B["vvvv"] - _P(es("bm,amef->abef", t1, B["vovv"]), 0, 1) + 0.25 * es("abmn,mnef->abef", tau, B["oovv"])
+    Wmbej = (B["ovvo"] + es("fj,mbef->mbej", t1, B["ovvv"]) - es("bn,mnej->mbej", t1, B["oovo"])
+             - es("fbjn,mnef->mbej", 0.5 * t2 + es("fj,bn->fbjn", t1, t1), B["oovv"]))
+    R1 = (B["fvo"] + es("ei,ae->ai", t1, Fae) - es("am,mi->ai", t1, Fmi) + es("aeim,me->ai", t2, Fme)
+          - es("fn,naif->ai", t1, B["ovov"]) - 0.5 * es("efim,maef->ai", t2, B["ovvv"])
+          - 0.5 * es("aemn,nmei->ai", t2, B["oovo"]))
+    R2 = (B["vvoo"]
+          + _P(es("aeij,be->abij", t2, Fae - 0.5 * es("bm,me->be", t1, Fme)), 0, 1)
+          - _P(es("abim,mj->abij", t2, Fmi + 0.5 * es("ej,me->mj", t1, Fme)), 2, 3)
+          + 0.5 * es("abmn,mnij->abij", tau, Wmnij) + 0.5 * es("efij,abef->abij", tau, Wabef)
+          + _P(_P(es("aeim,mbej->abij", t2, Wmbej) - es("ei,am,mbej->abij", t1, t1, B["ovvo"]), 2, 3), 0, 1)
+          + _P(es("ei,abej->abij", t1, B["vvvo"]), 2, 3) - _P(es("am,mbij->abij", t1, B["ovoo"]), 0, 1))
+    E = es("ia,ai->", B["fov"], t1) + 0.25 * es("ijab,abij->", B["oovv"], t2) + 0.5 * es("ijab,ai,bj->", B["oovv"], t1, t1)
+    return E, R1, R2
+
+
+def ccsd_residual_program(B, T1, T2, long_double=True):
+    """The CCSD residuals as BINARY tensor operations, every line one oracle.contract / oracle.add /
+    oracle.permsum call -- the same list of operations `paper_2409_06759_b200.ccd.ccsd_residual` issues to the library.
+    B: `ccsd_blocks`; T1[a,i], T2[a,b,i,j].  Returns (E, R1, R2).  Pinned to `ccsd_residual_unfactorised`."""
+    v, o = T1.shape
+    z = lambda *s: np.zeros(s, dtype=np.complex128, order="F")
+    cp = lambda x: np.asfortranarray(x).copy(order="F")
+    con = lambda e, D, L, R, a=1.0: _o.contract(e, D, L, R, a, long_double=long_double, want_snorm=False)[0]
+
+    def acc(D, X, PS, s):
+        return _o.permsum(D, X, PS[0], [s * c for c in PS[1]], 1.0)
+
+    tt = con("tt(a,b,i,j)=T1(a,i)*T1(b,j)", z(v, v, o, o), T1, T1)
+    taut = acc(cp(T2), tt, P_AB, 0.5)
+    tau = acc(cp(T2), tt, P_AB, 1.0)
+    Fae = con("F(a,e)+=T1(a,m)*f(m,e)", cp(B["fvv"]), T1, B["fov"], -0.5)
+    Fae = con("F(a,e)+=W(m,a,f,e)*T1(f,m)", Fae, B["ovvv"], T1, 1.0)
+    Fae = con("F(a,e)+=t(a,f,m,n)*W(m,n,e,f)", Fae, taut, B["oovv"], -0.5)
+    Fmi = con("F(m,i)+=f(m,e)*T1(e,i)", cp(B["foo"]), B["fov"], T1, 0.5)
+    Fmi = con("F(m,i)+=W(m,n,i,e)*T1(e,n)", Fmi, B["ooov"], T1, 1.0)
+    Fmi = con("F(m,i)+=W(m,n,e,f)*t(e,f,i,n)", Fmi, B["oovv"], taut, 0.5)
+    Fme = con("F(m,e)+=W(m,n,e,f)*T1(f,n)", cp(B["fov"]), B["oovv"], T1, 1.0)
+    X = con("X(m,n,i,j)=W(m,n,i,e)*T1(e,j)", z(o, o, o, o), B["ooov"], T1)
+    Wmnij = acc(cp(B["oooo"]), X, P_IJ, 1.0)
+    Wmnij = con("W(m,n,i,j)+=V(m,n,e,f)*t(e,f,i,j)", Wmnij, B["oovv"], tau, 0.25)
+    X = con("X(a,b,e,f)=V(a,m,e,f)*T1(b,m)", z(v, v, v, v), B["vovv"], T1)
+    Wabef = acc(cp(B["vvvv"]), X, P_AB, -1.0)
+    Wabef = con("W(a,b,e,f)+=t(a,b,m,n)*V(m,n,e,f)", Wabef, tau, B["oovv"], 0.25)
+    Q = _o.add("Q(f,b,j,n)+=t(f,b,j,n)", _o.add("Q(f,b,j,n)+=T2(f,b,j,n)", z(v, v, o, o), T2, 0.5), tt, 1.0)
+    Wmbej = con("W(m,b,e,j)+=V(m,b,e,f)*T1(f,j)", cp(B["ovvo"]), B["ovvv"], T1, 1.0)
+    Wmbej = con("W(m,b,e,j)+=V(m,n,e,j)*T1(b,n)", Wmbej, B["oovo"], T1, -1.0)
+    Wmbej = con("W(m,b,e,j)+=V(m,n,e,f)*Q(f,b,j,n)", Wmbej, B["oovv"], Q, -1.0)
+    R1 = con("R(a,i)+=F(a,e)*T1(e,i)", cp(B["fvo"]), Fae, T1, 1.0)
+    R1 = con("R(a,i)+=T1(a,m)*F(m,i)", R1, T1, Fmi, -1.0)
+    R1 = con("R(a,i)+=T2(a,e,i,m)*F(m,e)", R1, T2, Fme, 1.0)
+    R1 = con("R(a,i)+=V(n,a,i,f)*T1(f,n)", R1, B["ovov"], T1, -1.0)
+    R1 = con("R(a,i)+=V(m,a,e,f)*T2(e,f,i,m)", R1, B["ovvv"], T2, -0.5)
+    R1 = con("R(a,i)+=T2(a,e,m,n)*V(n,m,e,i)", R1, T2, B["oovo"], -0.5)
+    G = con("G(b,e)+=T1(b,m)*F(m,e)", cp(Fae), T1, Fme, -0.5)
+    X = con("X(a,b,i,j)=T2(a,e,i,j)*G(b,e)", z(v, v, o, o), T2, G)
+    R2 = acc(cp(B["vvoo"]), X, P_AB, 1.0)
+    Gm = con("G(m,j)+=F(m,e)*T1(e,j)", cp(Fmi), Fme, T1, 0.5)
+    X = con("X(a,b,i,j)=T2(a,b,i,m)*G(m,j)", z(v, v, o, o), T2, Gm)
+    R2 = acc(R2, X, P_IJ, -1.0)
+    R2 = con("R(a,b,i,j)+=t(a,b,m,n)*W(m,n,i,j)", R2, tau, Wmnij, 0.5)
+    R2 = con("R(a,b,i,j)+=W(a,b,e,f)*t(e,f,i,j)", R2, Wabef, tau, 0.5)
+    X = con("X(a,b,i,j)=T2(a,e,i,m)*W(m,b,e,j)", z(v, v, o, o), T2, Wmbej)
+    Z = con("Z(m,b,i,j)=V(m,b,e,j)*T1(e,i)", z(o, v, o, o), B["ovvo"], T1)
+    X = con("X(a,b,i,j)+=T1(a,m)*Z(m,b,i,j)", X, T1, Z, -1.0)
+    R2 = acc(R2, X, P_IJ_AB, 1.0)
+    X = con("X(a,b,i,j)=V(a,b,e,j)*T1(e,i)", z(v, v, o, o), B["vvvo"], T1)
+    R2 = acc(R2, X, P_IJ, 1.0)
+    X = con("X(a,b,i,j)=T1(a,m)*V(m,b,i,j)", z(v, v, o, o), T1, B["ovoo"])
+    R2 = acc(R2, X, P_AB, -1.0)
+    E = con("E()=f(i,a)*T1(a,i)", np.zeros(()), B["fov"], T1, 1.0)
+    E = con("E()+=V(i,j,a,b)*T2(a,b,i,j)", E, B["oovv"], T2, 0.25)
+    E = con("E()+=V(i,j,a,b)*t(a,b,i,j)", E, B["oovv"], tt, 0.5)
+    return complex(np.asarray(E).reshape(-1)[0]), R1, R2
+
+
+# ------------------------------------------------------------------------------------------
 # next row 8(f)-3: the Jacobi iteration around the residual (energy denominators, PAPER.md:212; a "CC iteration",
 # PAPER.md:406-410).  The paper does not print the update; it is the textbook fixed-point step, PINNED in
 # tests/test_oracle_cc.py: the first step from T = 0 is the MP2 amplitude closed form, and the converged

@@ -66,6 +66,109 @@ def ccd_energy(ctx, B, T):
     return E
 
 
+CCSD_BLOCKS = ("vvoo", "oovv", "oooo", "vvvv", "ovvo", "ooov", "ovvv", "vovv", "oovo", "ovov", "vvvo", "ovoo",
+               "foo", "fvv", "fov", "fvo")
+
+
+def ccsd_residual(ctx, B, T1, T2, R1=None, R2=None):
+    """Spin-orbital CCSD residuals (the paper's benchmark iteration) as the binary tensor operations a
+    generated driver issues: 35 contractions, 11 permute-sums, 12 adds; intermediates are created and destroyed around
+    their use (PAPER.md:212).  B: dict of device tensors `CCSD_BLOCKS` (<pq||rs> blocks in bra-ket order, f blocks);
+    T1 (v,o) = t_i^a, T2 (v,v,o,o) = t_ij^ab.  Returns (E rank-0 tensor, R1, R2).  Equations: DESIGN.md / oracle/cc.py
+    `ccsd_residual_unfactorised` (pinned to PAPER Eq. (3) on the Fock space)."""
+    v, o = T1.extents
+    new = ctx.tensor_create
+    con, add, asym = ctx.contract, ctx.add, ctx.antisymmetrize
+
+    def copy(src, shape, label):
+        D = new(shape)
+        add(f"D({label})=S({label})", D, src, 1.0)
+        return D
+
+    tt = new((v, v, o, o))
+    con("tt(a,b,i,j)=T1(a,i)*T1(b,j)", tt, T1, T1, 1.0)
+    taut = copy(T2, (v, v, o, o), "a,b,i,j")
+    asym("P(ab):t(a,b,i,j)+=tt(a,b,i,j)", taut, tt, 0.5)
+    tau = copy(T2, (v, v, o, o), "a,b,i,j")
+    asym("P(ab):t(a,b,i,j)+=tt(a,b,i,j)", tau, tt, 1.0)
+    Fae = copy(B["fvv"], (v, v), "a,e")
+    con("F(a,e)+=T1(a,m)*f(m,e)", Fae, T1, B["fov"], -0.5)
+    con("F(a,e)+=W(m,a,f,e)*T1(f,m)", Fae, B["ovvv"], T1, 1.0)
+    con("F(a,e)+=t(a,f,m,n)*W(m,n,e,f)", Fae, taut, B["oovv"], -0.5)
+    Fmi = copy(B["foo"], (o, o), "m,i")
+    con("F(m,i)+=f(m,e)*T1(e,i)", Fmi, B["fov"], T1, 0.5)
+    con("F(m,i)+=W(m,n,i,e)*T1(e,n)", Fmi, B["ooov"], T1, 1.0)
+    con("F(m,i)+=W(m,n,e,f)*t(e,f,i,n)", Fmi, B["oovv"], taut, 0.5)
+    taut.destroy()
+    Fme = copy(B["fov"], (o, v), "m,e")
+    con("F(m,e)+=W(m,n,e,f)*T1(f,n)", Fme, B["oovv"], T1, 1.0)
+    X = new((o, o, o, o))
+    con("X(m,n,i,j)=W(m,n,i,e)*T1(e,j)", X, B["ooov"], T1, 1.0)
+    Wmnij = copy(B["oooo"], (o, o, o, o), "m,n,i,j")
+    asym("P(ij):W(m,n,i,j)+=X(m,n,i,j)", Wmnij, X, 1.0)
+    X.destroy()
+    con("W(m,n,i,j)+=V(m,n,e,f)*t(e,f,i,j)", Wmnij, B["oovv"], tau, 0.25)
+    X = new((v, v, v, v))
+    con("X(a,b,e,f)=V(a,m,e,f)*T1(b,m)", X, B["vovv"], T1, 1.0)
+    Wabef = copy(B["vvvv"], (v, v, v, v), "a,b,e,f")
+    asym("P(ab):W(a,b,e,f)+=X(a,b,e,f)", Wabef, X, -1.0)
+    X.destroy()
+    con("W(a,b,e,f)+=t(a,b,m,n)*V(m,n,e,f)", Wabef, tau, B["oovv"], 0.25)
+    Q = new((v, v, o, o))
+    add("Q(f,b,j,n)=T2(f,b,j,n)", Q, T2, 0.5)
+    add("Q(f,b,j,n)+=t(f,b,j,n)", Q, tt, 1.0)
+    Wmbej = copy(B["ovvo"], (o, v, v, o), "m,b,e,j")
+    con("W(m,b,e,j)+=V(m,b,e,f)*T1(f,j)", Wmbej, B["ovvv"], T1, 1.0)
+    con("W(m,b,e,j)+=V(m,n,e,j)*T1(b,n)", Wmbej, B["oovo"], T1, -1.0)
+    con("W(m,b,e,j)+=V(m,n,e,f)*Q(f,b,j,n)", Wmbej, B["oovv"], Q, -1.0)
+    Q.destroy()
+    if R1 is None:
+        R1 = new((v, o))
+    add("R(a,i)=f(a,i)", R1, B["fvo"], 1.0)
+    con("R(a,i)+=F(a,e)*T1(e,i)", R1, Fae, T1, 1.0)
+    con("R(a,i)+=T1(a,m)*F(m,i)", R1, T1, Fmi, -1.0)
+    con("R(a,i)+=T2(a,e,i,m)*F(m,e)", R1, T2, Fme, 1.0)
+    con("R(a,i)+=V(n,a,i,f)*T1(f,n)", R1, B["ovov"], T1, -1.0)
+    con("R(a,i)+=V(m,a,e,f)*T2(e,f,i,m)", R1, B["ovvv"], T2, -0.5)
+    con("R(a,i)+=T2(a,e,m,n)*V(n,m,e,i)", R1, T2, B["oovo"], -0.5)
+    if R2 is None:
+        R2 = new((v, v, o, o))
+    add("R(a,b,i,j)=W(a,b,i,j)", R2, B["vvoo"], 1.0)
+    X = new((v, v, o, o))
+    con("G(b,e)+=T1(b,m)*F(m,e)", Fae, T1, Fme, -0.5)                 # Fae is not needed any more: it becomes G
+    con("X(a,b,i,j)=T2(a,e,i,j)*G(b,e)", X, T2, Fae, 1.0)
+    asym("P(ab):R(a,b,i,j)+=X(a,b,i,j)", R2, X, 1.0)
+    Fae.destroy()
+    con("G(m,j)+=F(m,e)*T1(e,j)", Fmi, Fme, T1, 0.5)                   # likewise Fmi becomes Gm
+    con("X(a,b,i,j)=T2(a,b,i,m)*G(m,j)", X, T2, Fmi, 1.0)
+    asym("P(ij):R(a,b,i,j)+=X(a,b,i,j)", R2, X, -1.0)
+    Fmi.destroy()
+    Fme.destroy()
+    con("R(a,b,i,j)+=t(a,b,m,n)*W(m,n,i,j)", R2, tau, Wmnij, 0.5)
+    Wmnij.destroy()
+    con("R(a,b,i,j)+=W(a,b,e,f)*t(e,f,i,j)", R2, Wabef, tau, 0.5)
+    Wabef.destroy()
+    tau.destroy()
+    con("X(a,b,i,j)=T2(a,e,i,m)*W(m,b,e,j)", X, T2, Wmbej, 1.0)
+    Wmbej.destroy()
+    Z = new((o, v, o, o))
+    con("Z(m,b,i,j)=V(m,b,e,j)*T1(e,i)", Z, B["ovvo"], T1, 1.0)
+    con("X(a,b,i,j)+=T1(a,m)*Z(m,b,i,j)", X, T1, Z, -1.0)
+    Z.destroy()
+    asym("P(ij)P(ab):R(a,b,i,j)+=X(a,b,i,j)", R2, X, 1.0)
+    con("X(a,b,i,j)=V(a,b,e,j)*T1(e,i)", X, B["vvvo"], T1, 1.0)
+    asym("P(ij):R(a,b,i,j)+=X(a,b,i,j)", R2, X, 1.0)
+    con("X(a,b,i,j)=T1(a,m)*V(m,b,i,j)", X, T1, B["ovoo"], 1.0)
+    asym("P(ab):R(a,b,i,j)+=X(a,b,i,j)", R2, X, -1.0)
+    X.destroy()
+    E = new(())
+    con("E()=f(i,a)*T1(a,i)", E, B["fov"], T1, 1.0)
+    con("E()+=V(i,j,a,b)*T2(a,b,i,j)", E, B["oovv"], T2, 0.25)
+    con("E()+=V(i,j,a,b)*t(a,b,i,j)", E, B["oovv"], tt, 0.5)
+    tt.destroy()
+    return E, R1, R2
+
+
 def ccd_solve(ctx, B, e_occ, e_virt, iterations, T=None):
     """Jacobi iterations of the CCD amplitude equations (PAPER.md:212 energy denominators, 406-410 "CC
     iteration"):  T <- T + R(T) / (e_i + e_j - e_a - e_b), from T (default: a zero tensor, whose first step is the MP2

@@ -128,3 +128,39 @@ def test_ccd_jacobi_iterations_follow_the_oracle(ctx):
     assert np.max(np.abs(ctx.tensor_download(dR))) <= 1e-11 * np.abs(B["vvoo"]).max()
     assert abs(energies[-1] - energies[-2]) <= 1e-12 * abs(energies[-1])
     assert abs(energies[-1] - cc.ccd_jacobi(B, eo, ev, 40)[1][-1]) <= 1e-11 * abs(energies[-1])
+
+
+@pytest.mark.parametrize("o,v", [(3, 4), (5, 11)])
+def test_ccsd_residual_program(ctx, o, v):
+    """The CCSD residuals (singles, doubles, energy) as ~60 ABI calls against the oracle's program of the same binary
+    operations; at (3,4) also against the unfactorised tier (itself pinned to the Fock space)."""
+    n = o + v
+    rng = np.random.default_rng(o * 100 + v)
+    c = lambda *s: rng.standard_normal(s) + 1j * rng.standard_normal(s)
+    g = synth.tensor(synth.SEED0 + 5, 1, [n] * 4, antisym=((0, 1), (2, 3)), sigma=0.1, hermitian=True)
+    f = c(n, n) * 0.1
+    f = f + f.conj().T + np.diag(np.concatenate([np.linspace(-2, -0.5, o), np.linspace(0.5, 3, v)]))
+    t2 = c(v, v, o, o) * 0.2
+    t2 = t2 - t2.transpose(1, 0, 2, 3)
+    t2 = np.asfortranarray(t2 - t2.transpose(0, 1, 3, 2))
+    t1 = np.asfortranarray(c(v, o) * 0.2)
+    B = cc.ccsd_blocks(o, f, g)
+    assert set(B) == set(ccd.CCSD_BLOCKS)
+    dB = {k: ctx.tensor_from_numpy(x) for k, x in B.items()}
+    dT1, dT2 = ctx.tensor_from_numpy(t1), ctx.tensor_from_numpy(t2)
+    live = ctx.launch_count()
+    dE, dR1, dR2 = ccd.ccsd_residual(ctx, dB, dT1, dT2)
+    assert ctx.launch_count() - live >= 58
+    E, R1, R2 = complex(ctx.tensor_download(dE)), ctx.tensor_download(dR1), ctx.tensor_download(dR2)
+    e_ref, r1_ref, r2_ref = cc.ccsd_residual_program(B, t1, t2)
+    assert abs(E - e_ref) <= 1e-11 * abs(e_ref)
+    assert np.max(np.abs(R1 - r1_ref)) <= 1e-11 * np.abs(r1_ref).max()
+    assert np.max(np.abs(R2 - r2_ref)) <= 1e-11 * np.abs(r2_ref).max()
+    assert np.max(np.abs(R2 + R2.transpose(1, 0, 2, 3))) <= 1e-12 * np.abs(r2_ref).max()
+    if o <= 3:
+        e_u, r1_u, r2_u = cc.ccsd_residual_unfactorised(o, f, g, t1, t2)
+        assert abs(E - e_u) <= 1e-11 * abs(e_u)
+        assert np.max(np.abs(R1 - r1_u)) <= 1e-11 * np.abs(r1_u).max()
+        assert np.max(np.abs(R2 - r2_u)) <= 1e-11 * np.abs(r2_u).max()
+    for t in list(dB.values()) + [dT1, dT2, dE, dR1, dR2]:
+        t.destroy()

@@ -134,3 +134,36 @@ def test_converged_jacobi_amplitudes_zero_the_fock_space_projection(o, v):
     assert abs(energies[-1] - e0) <= 1e-12 * abs(e0)
     assert abs(energies[-1] - energies[-2]) <= 1e-13 * abs(e0)
     assert np.abs(T - T_mp2).max() > 1e-3 * np.abs(T_mp2).max()          # it did move away from the MP2 guess
+
+
+@pytest.mark.parametrize("o,v", [(2, 3), (3, 3), (2, 4)])
+def test_ccsd_unfactorised_agrees_with_fock_space(o, v):
+    """The textbook CCSD intermediates, in residual form with a general complex non-diagonal Hermitian f, against
+    PAPER Eq. (3) on the Fock space: singles and doubles projections and the energy."""
+    f, g, t2 = rand_inputs(o, v, 300 * o + v)
+    rng = np.random.default_rng(7 * o + v)
+    t1 = rng.standard_normal((v, o)) + 1j * rng.standard_normal((v, o))
+    t2, t1 = 0.3 * t2, 0.3 * t1
+    e0, r1_0, r2_0 = cc.fock_space_residuals(o, v, f, g, t2, t1)
+    e, r1, r2 = cc.ccsd_residual_unfactorised(o, f, g, t1, t2)
+    assert abs(e - e0) <= 1e-13 * abs(e0)
+    assert np.abs(r1 - r1_0).max() <= 1e-13 * np.abs(r1_0).max()
+    assert np.abs(r2 - r2_0).max() <= 1e-13 * np.abs(r2_0).max()
+    # t1 = 0 reduces to CCD
+    e_d, r1_d, r2_d = cc.ccsd_residual_unfactorised(o, f, g, 0 * t1, t2)
+    assert np.abs(r2_d - cc.ccd_residual_unfactorised(o, f, g, t2)[0]).max() <= 1e-13 * np.abs(r2_d).max()
+
+
+@pytest.mark.parametrize("o,v", [(2, 3), (3, 4)])
+def test_ccsd_program_of_binary_operations_agrees_with_the_unfactorised_tier(o, v):
+    f, g, t2 = rand_inputs(o, v, 500 * o + v)
+    rng = np.random.default_rng(11 * o + v)
+    t1 = np.asfortranarray(0.3 * (rng.standard_normal((v, o)) + 1j * rng.standard_normal((v, o))))
+    t2 = np.asfortranarray(0.3 * t2)
+    e, r1, r2 = cc.ccsd_residual_unfactorised(o, f, g, t1, t2)
+    ep, r1p, r2p = cc.ccsd_residual_program(cc.ccsd_blocks(o, f, g), t1, t2)
+    assert abs(ep - e) <= 1e-13 * abs(e)
+    assert np.abs(r1p - r1).max() <= 1e-13 * np.abs(r1).max()
+    assert np.abs(r2p - r2).max() <= 1e-13 * np.abs(r2).max()
+    assert np.abs(r2p + r2p.transpose(1, 0, 2, 3)).max() <= 1e-13 * np.abs(r2).max()
+    assert np.abs(r2p + r2p.transpose(0, 1, 3, 2)).max() <= 1e-13 * np.abs(r2).max()
