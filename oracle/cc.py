@@ -400,6 +400,25 @@ def ccd_jacobi(B, e_occ, e_virt, iterations, T0=None):
     return T, energies
 
 
+def ccsd_jacobi(B, e_occ, e_virt, iterations):
+    """t1 <- t1 + R1 / (e_i - e_a), t2 <- t2 + R2 / (e_i + e_j - e_a - e_b) from zero amplitudes, both residuals
+    evaluated at the same (old) amplitudes.  Returns (T1, T2, [E_corr of the amplitudes after each step])."""
+    v, o = B["fvo"].shape
+    T1 = np.zeros((v, o), dtype=np.complex128, order="F")
+    T2 = np.zeros((v, v, o, o), dtype=np.complex128, order="F")
+    ev, eo = -np.asarray(e_virt, dtype=np.float64), np.asarray(e_occ, dtype=np.float64)
+    energies = []
+    for it in range(iterations + 1):
+        E, R1, R2 = ccsd_residual_program(B, T1, T2)
+        if it > 0:
+            energies.append(E)                  # the energy comes with the residuals of the NEXT evaluation
+        if it == iterations:
+            break
+        T1 = denominator_update(T1, R1, [ev, eo], 1.0)
+        T2 = denominator_update(T2, R2, [ev, ev, eo, eo], 1.0)
+    return T1, T2, energies
+
+
 # ------------------------------------------------------------------------------------------
 # config 4: CCSDT piece
 # ------------------------------------------------------------------------------------------

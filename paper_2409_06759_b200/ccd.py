@@ -191,6 +191,31 @@ def ccd_solve(ctx, B, e_occ, e_virt, iterations, T=None):
     return T, energies
 
 
+def ccsd_solve(ctx, B, e_occ, e_virt, iterations):
+    """Jacobi iterations of the CCSD amplitude equations from zero amplitudes: t1 += R1 / (e_i - e_a),
+    t2 += R2 / (e_i + e_j - e_a - e_b), both residuals evaluated at the old amplitudes.  One iteration = `ccsd_residual`
+    + two `tcb_denominator_update`; the energy of the updated amplitudes is produced by the next residual evaluation
+    (so `iterations` updates cost iterations + 1 evaluations).  Returns (T1, T2, [E_corr after each step])."""
+    import numpy as np
+    v, o = B["fvo"].extents
+    T1, T2 = ctx.tensor_create((v, o)), ctx.tensor_create((v, v, o, o))
+    R1, R2 = ctx.tensor_create((v, o)), ctx.tensor_create((v, v, o, o))
+    ev, eo = -np.asarray(e_virt, dtype=np.float64), np.asarray(e_occ, dtype=np.float64)
+    energies = []
+    for it in range(iterations + 1):
+        E, _, _ = ccsd_residual(ctx, B, T1, T2, R1, R2)
+        if it > 0:
+            energies.append(complex(ctx.tensor_download(E)))
+        E.destroy()
+        if it == iterations:
+            break
+        ctx.denominator_update(T1, R1, [ev, eo], 1.0)
+        ctx.denominator_update(T2, R2, [ev, ev, eo, eo], 1.0)
+    R1.destroy()
+    R2.destroy()
+    return T1, T2, energies
+
+
 CCD_FLOPS = lambda o, v: 8.0 * (                 # 8 real flop per complex multiply-add
     v * v * o * o * v                            # Fock vv
     + v * v * o * o * o                          # Fock oo

@@ -164,3 +164,27 @@ def test_ccsd_residual_program(ctx, o, v):
         assert np.max(np.abs(R2 - r2_u)) <= 1e-11 * np.abs(r2_u).max()
     for t in list(dB.values()) + [dT1, dT2, dE, dR1, dR2]:
         t.destroy()
+
+
+def test_ccsd_jacobi_iterations_follow_the_oracle(ctx):
+    """Four CCSD iterations on the GPU (residual program + two denominator updates each) against the oracle's."""
+    o, v = 3, 4
+    rng = np.random.default_rng(77)
+    n = o + v
+    c = lambda *s: rng.standard_normal(s) + 1j * rng.standard_normal(s)
+    g = synth.tensor(synth.SEED0 + 6, 1, [n] * 4, antisym=((0, 1), (2, 3)), sigma=0.05, hermitian=True)
+    e = np.concatenate([np.linspace(-2.0, -0.5, o), np.linspace(0.5, 3.0, v)])
+    f = 0.05 * c(n, n)
+    f = f + f.conj().T
+    f[np.diag_indices(n)] = e
+    B = cc.ccsd_blocks(o, f, g)
+    dB = {k: ctx.tensor_from_numpy(x) for k, x in B.items()}
+    dT1, dT2, energies = ccd.ccsd_solve(ctx, dB, e[:o], e[o:], 4)
+    T1, T2, e_ref = cc.ccsd_jacobi(B, e[:o], e[o:], 4)
+    assert np.max(np.abs(ctx.tensor_download(dT1) - T1)) <= 1e-11 * np.abs(T1).max()
+    assert np.max(np.abs(ctx.tensor_download(dT2) - T2)) <= 1e-11 * np.abs(T2).max()
+    assert len(energies) == 4
+    for x, y in zip(energies, e_ref):
+        assert abs(x - y) <= 1e-11 * abs(y)
+    for t in list(dB.values()) + [dT1, dT2]:
+        t.destroy()

@@ -167,3 +167,30 @@ def test_ccsd_program_of_binary_operations_agrees_with_the_unfactorised_tier(o, 
     assert np.abs(r2p - r2).max() <= 1e-13 * np.abs(r2).max()
     assert np.abs(r2p + r2p.transpose(1, 0, 2, 3)).max() <= 1e-13 * np.abs(r2).max()
     assert np.abs(r2p + r2p.transpose(0, 1, 3, 2)).max() <= 1e-13 * np.abs(r2).max()
+
+
+def _ccsd_problem(o, v, seed):
+    """weakly coupled Hermitian problem with a non-zero occupied-virtual Fock block (so that t1 does not vanish)"""
+    rng = np.random.default_rng(seed)
+    n = o + v
+    c = lambda *s: rng.standard_normal(s) + 1j * rng.standard_normal(s)
+    A = c(n, n, n, n)
+    A = A - A.transpose(1, 0, 2, 3)
+    A = A - A.transpose(0, 1, 3, 2)
+    g = 0.05 * 0.5 * (A + A.transpose(2, 3, 0, 1).conj())
+    f = 0.05 * c(n, n)
+    e = np.concatenate([np.linspace(-2.0, -0.5, o), np.linspace(0.5, 3.0, v)])
+    f = f + f.conj().T
+    f[np.diag_indices(n)] = e
+    return f, g, e[:o], e[o:]
+
+
+@pytest.mark.parametrize("o,v", [(2, 3), (3, 3)])
+def test_converged_ccsd_jacobi_zeroes_the_fock_space_singles_and_doubles(o, v):
+    f, g, eo, ev = _ccsd_problem(o, v, 40 + o + v)
+    T1, T2, energies = cc.ccsd_jacobi(cc.ccsd_blocks(o, f, g), eo, ev, 60)
+    e0, r1, r2 = cc.fock_space_residuals(o, v, f, g, T2, T1)
+    scale = np.abs(g).max()
+    assert np.abs(r1).max() <= 1e-12 * scale and np.abs(r2).max() <= 1e-12 * scale
+    assert abs(energies[-1] - e0) <= 1e-12 * abs(e0)
+    assert np.abs(T1).max() > 1e-3 and np.abs(T2).max() > 1e-3
