@@ -119,6 +119,12 @@ int tcb_scale(tcb_ctx *ctx, tcb_tensor *D, tcb_c128 alpha);
  * T and R have the same shape and must not overlap.  The energies are copied before the call returns.  A zero
  * denominator is not detected (the quotient is IEEE inf/nan).  Errors: TCB_EINVAL, TCB_ESHAPE, TCB_EALIAS, TCB_ECUDA. */
 int tcb_denominator_update(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, const double *const *eps, tcb_c128 alpha);
+/* Inner product into a rank-0 tensor (what a DIIS extrapolation around the iteration needs; the bilinear form is also
+ * reachable as a full contraction "E()=X(..)*Y(..)", the sesquilinear one only here):
+ *     D = alpha * sum_i (conjugate_x ? conj(X[i]) : X[i]) * Y[i]
+ * X and Y have the same shape (any rank), D has rank 0 and overlaps neither.  Deterministic (fixed summation order).
+ * Stream-ordered like every other call: download D to read it.  Errors: TCB_EINVAL, TCB_ESHAPE, TCB_EALIAS, TCB_ECUDA. */
+int tcb_dot(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, const tcb_tensor *Y, int conjugate_x, tcb_c128 alpha);
 /* S3, tensor transposition: "D(i,j,a,b)=L(a,b,i,j)", pure data movement, bit-exact. */
 int tcb_permute(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor *L);
 /* S6, fused permute-sum (the generator's unrolled permutation operators):

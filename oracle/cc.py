@@ -400,6 +400,40 @@ def ccd_jacobi(B, e_occ, e_virt, iterations, T0=None):
     return T, energies
 
 
+def diis_coefficients(Bm):
+    """min |sum_i c_i e_i|^2 subject to sum_i c_i = 1, Bm[i,j] = <e_i|e_j> (Pulay):  [[B, 1], [1^T, 0]] [c; lam] = [0; 1]."""
+    m = Bm.shape[0]
+    A = np.zeros((m + 1, m + 1), dtype=np.complex128)
+    A[:m, :m] = Bm
+    A[:m, m] = A[m, :m] = 1.0
+    rhs = np.zeros(m + 1, dtype=np.complex128)
+    rhs[m] = 1.0
+    return np.linalg.solve(A, rhs)[:m]
+
+
+def ccd_diis(B, e_occ, e_virt, iterations, depth=6):
+    """The CCD iteration with DIIS extrapolation: error vector e_k = R(T_k) / D (the Jacobi step), trial vector
+    T_k + e_k; the next T is the combination of the last `depth` trial vectors that minimises |sum c_i e_i|.
+    Returns (T, [E_corr after each step], [|e_k| of each step])."""
+    v, o = B["vvoo"].shape[0], B["vvoo"].shape[2]
+    T = np.zeros((v, v, o, o), dtype=np.complex128, order="F")
+    ev, eo = -np.asarray(e_virt, dtype=np.float64), np.asarray(e_occ, dtype=np.float64)
+    trial, err, energies, norms = [], [], [], []
+    for _ in range(iterations):
+        R = ccd_residual_program(B, T)
+        e = denominator_update(np.zeros_like(T), R, [ev, ev, eo, eo], 1.0)
+        trial.append(np.asfortranarray(T + e))
+        err.append(e)
+        trial, err = trial[-depth:], err[-depth:]
+        m = len(err)
+        Bm = np.array([[np.vdot(err[i], err[j]) for j in range(m)] for i in range(m)])
+        norms.append(float(np.sqrt(abs(Bm[m - 1, m - 1]))))
+        c = diis_coefficients(Bm) if m > 1 else np.ones(1)
+        T = np.asfortranarray(sum(ci * t for ci, t in zip(c, trial)))
+        energies.append(ccd_energy(B, T))
+    return T, energies, norms
+
+
 def ccsd_jacobi(B, e_occ, e_virt, iterations):
     """t1 <- t1 + R1 / (e_i - e_a), t2 <- t2 + R2 / (e_i + e_j - e_a - e_b) from zero amplitudes, both residuals
     evaluated at the same (old) amplitudes.  Returns (T1, T2, [E_corr of the amplitudes after each step])."""

@@ -191,6 +191,64 @@ def ccd_solve(ctx, B, e_occ, e_virt, iterations, T=None):
     return T, energies
 
 
+def ccd_solve_diis(ctx, B, e_occ, e_virt, iterations, depth=6):
+    """The CCD iteration with DIIS extrapolation (Pulay): error vector e_k = R(T_k) / D, trial vector T_k + e_k, next T =
+    the combination of the last `depth` trial vectors minimising |sum c_i e_i|.  Tensors, inner products (`tcb_dot`,
+    one new row of <e_i|e_j> per iteration) and linear combinations (`tcb_add`) live on the device; only the
+    depth x depth system is solved on the host.  Returns (T, [E_corr after each step], [|e_k| of each step])."""
+    import numpy as np
+    v, _, o, _ = B["vvoo"].extents
+    shape = (v, v, o, o)
+    T, R = ctx.tensor_create(shape), ctx.tensor_create(shape)
+    ev, eo = -np.asarray(e_virt, dtype=np.float64), np.asarray(e_occ, dtype=np.float64)
+    trial, err, energies, norms = [], [], [], []
+    Bm = np.zeros((0, 0), dtype=np.complex128)
+    s = ctx.tensor_create(())
+    for _ in range(iterations):
+        ccd_residual(ctx, B, T, R)
+        if len(err) == depth:                      # the oldest pair leaves; its tensors are reused
+            e, t = err.pop(0), trial.pop(0)
+            Bm = Bm[1:, 1:]
+            ctx.tensor_fill(e, 0.0)
+        else:
+            e, t = ctx.tensor_create(shape), ctx.tensor_create(shape)
+        ctx.denominator_update(e, R, [ev, ev, eo, eo], 1.0)
+        ctx.add("t(a,b,i,j)=T(a,b,i,j)", t, T, 1.0)
+        ctx.add("t(a,b,i,j)+=e(a,b,i,j)", t, e, 1.0)
+        err.append(e)
+        trial.append(t)
+        m = len(err)
+        row = np.zeros(m, dtype=np.complex128)
+        for i in range(m):                         # <e_i|e_new>; the matrix is Hermitian
+            ctx.dot(s, err[i], e, True, 1.0)
+            row[i] = complex(ctx.tensor_download(s))
+        Bn = np.zeros((m, m), dtype=np.complex128)
+        Bn[:m - 1, :m - 1] = Bm
+        Bn[:, m - 1] = row
+        Bn[m - 1, :] = row.conj()
+        Bn[m - 1, m - 1] = row[m - 1]
+        Bm = Bn
+        norms.append(float(np.sqrt(abs(Bm[m - 1, m - 1]))))
+        if m > 1:
+            A = np.zeros((m + 1, m + 1), dtype=np.complex128)
+            A[:m, :m] = Bm
+            A[:m, m] = A[m, :m] = 1.0
+            rhs = np.zeros(m + 1, dtype=np.complex128)
+            rhs[m] = 1.0
+            c = np.linalg.solve(A, rhs)[:m]
+        else:
+            c = np.ones(1, dtype=np.complex128)
+        ctx.add("T(a,b,i,j)=t(a,b,i,j)", T, trial[0], complex(c[0]))
+        for ci, ti in zip(c[1:], trial[1:]):
+            ctx.add("T(a,b,i,j)+=t(a,b,i,j)", T, ti, complex(ci))
+        E = ccd_energy(ctx, B, T)
+        energies.append(complex(ctx.tensor_download(E)))
+        E.destroy()
+    for x in err + trial + [R, s]:
+        x.destroy()
+    return T, energies, norms
+
+
 def ccsd_solve(ctx, B, e_occ, e_virt, iterations):
     """Jacobi iterations of the CCSD amplitude equations from zero amplitudes: t1 += R1 / (e_i - e_a),
     t2 += R2 / (e_i + e_j - e_a - e_b), both residuals evaluated at the old amplitudes.  One iteration = `ccsd_residual`

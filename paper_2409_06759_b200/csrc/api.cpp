@@ -684,6 +684,31 @@ int tcb_scale(tcb_ctx *ctx, tcb_tensor *D, tcb_c128 alpha)
     return TCB_OK;
 }
 
+int tcb_dot(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, const tcb_tensor *Y, int conjugate_x, tcb_c128 alpha)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!D || !X || !Y) return set_error(ctx, TCB_EINVAL, "null argument");
+    if (D->shape.rank != 0) return set_error(ctx, TCB_ESHAPE, "D must have rank 0");
+    if (X->shape.rank != Y->shape.rank) return set_error(ctx, TCB_ESHAPE, "rank mismatch");
+    for (int k = 0; k < X->shape.rank; ++k)
+        if (X->shape.ext[k] != Y->shape.ext[k]) return set_error(ctx, TCB_ESHAPE, "X and Y differ in shape");
+    if (overlaps(D, X) || overlaps(D, Y)) return set_error(ctx, TCB_EALIAS, "D overlaps X or Y");
+    const int64_t n = X->elems();
+    const int nblocks = (int)std::max<int64_t>(1, std::min<int64_t>(kDotBlocks, (n + 255) / 256));
+    void *partial = nullptr;
+    TCB_CUDA(ctx, cudaMallocAsync(&partial, (size_t)nblocks * 16, ctx->stream));
+    cudaError_t e;
+    {
+        TimedLaunch tl(ctx, kClsElementwise, 8.0 * (double)n, 32.0 * (double)n);
+        e = launch_dot(D->ptr, X->ptr, Y->ptr, n, conjugate_x != 0, alpha.re, alpha.im, partial, nblocks, ctx->stream,
+                       &ctx->launches);
+    }
+    cudaFreeAsync(partial, ctx->stream);
+    TCB_CUDA(ctx, e);
+    return TCB_OK;
+}
+
 int tcb_denominator_update(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, const double *const *eps, tcb_c128 alpha)
 {
     int rc = enter(ctx);

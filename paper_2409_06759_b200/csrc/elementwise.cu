@@ -75,6 +75,56 @@ cudaError_t launch_axpy(void *D, const void *L, int64_t n, double re, double im,
     return e;
 }
 
+// D = alpha * sum_i (conj?) X[i] * Y[i] -- the inner product a DIIS extrapolation needs.  Two deterministic stages:
+// every block sums its grid-stride share in a fixed order (thread-sequential, then a fixed shuffle / shared-memory
+// tree), then one block sums the per-block partials in index order.
+template <bool CONJ>
+__global__ void __launch_bounds__(256)
+dot_partial_kernel(const double2 *__restrict__ X, const double2 *__restrict__ Y, long long n, double2 *partial)
+{
+    double sr = 0.0, si = 0.0;
+    for (long long i = blockIdx.x * 256LL + threadIdx.x; i < n; i += gridDim.x * 256LL) {
+        const double2 x = X[i], y = Y[i];
+        const double xi = CONJ ? -x.y : x.y;
+        // products rounded separately (no FMA contraction): <x|x> then has an exactly zero imaginary part
+        sr = __dadd_rn(sr, __dsub_rn(__dmul_rn(x.x, y.x), __dmul_rn(xi, y.y)));
+        si = __dadd_rn(si, __dadd_rn(__dmul_rn(x.x, y.y), __dmul_rn(xi, y.x)));
+    }
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) {
+        sr += __shfl_down_sync(0xffffffffu, sr, d);
+        si += __shfl_down_sync(0xffffffffu, si, d);
+    }
+    __shared__ double wr[8], wi[8];
+    if ((threadIdx.x & 31) == 0) { wr[threadIdx.x >> 5] = sr; wi[threadIdx.x >> 5] = si; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) { sr += wr[w]; si += wi[w]; }
+        partial[blockIdx.x] = make_double2(sr, si);
+    }
+}
+
+__global__ void __launch_bounds__(32) dot_final_kernel(const double2 *partial, int nblocks, double2 *D, double ar, double ai)
+{
+    if (threadIdx.x != 0) return;
+    double sr = 0.0, si = 0.0;
+    for (int b = 0; b < nblocks; ++b) { sr += partial[b].x; si += partial[b].y; }
+    *D = make_double2(ar * sr - ai * si, ar * si + ai * sr);
+}
+
+cudaError_t launch_dot(void *D, const void *X, const void *Y, int64_t n, bool conj_x, double re, double im, void *partial,
+                       int nblocks, cudaStream_t s, int64_t *launches)
+{
+    if (conj_x) dot_partial_kernel<true><<<nblocks, 256, 0, s>>>((const double2 *)X, (const double2 *)Y, n, (double2 *)partial);
+    else dot_partial_kernel<false><<<nblocks, 256, 0, s>>>((const double2 *)X, (const double2 *)Y, n, (double2 *)partial);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    dot_final_kernel<<<1, 32, 0, s>>>((const double2 *)partial, nblocks, (double2 *)D, re, im);
+    e = cudaGetLastError();
+    if (e == cudaSuccess && launches) *launches += 2;
+    return e;
+}
+
 // T[idx] += alpha * R[idx] / (sum_k eps_k[idx_k])  -- the Jacobi step of a CC solver (orbital-energy denominators)
 struct DenomParams {
     int rank;

@@ -188,3 +188,40 @@ def test_ccsd_jacobi_iterations_follow_the_oracle(ctx):
         assert abs(x - y) <= 1e-11 * abs(y)
     for t in list(dB.values()) + [dT1, dT2]:
         t.destroy()
+
+
+@pytest.mark.parametrize("shape,conj", [((7, 5, 3), True), ((7, 5, 3), False), ((300, 41, 9), True), ((), True)])
+def test_dot_matches_numpy(ctx, shape, conj):
+    rng = np.random.default_rng(len(shape) + int(conj))
+    X = np.asfortranarray(rng.standard_normal(shape) + 1j * rng.standard_normal(shape))
+    Y = np.asfortranarray(rng.standard_normal(shape) + 1j * rng.standard_normal(shape))
+    dX, dY, dD = ctx.tensor_from_numpy(X), ctx.tensor_from_numpy(Y), ctx.tensor_create(())
+    alpha = 0.5 - 1.5j
+    ctx.dot(dD, dX, dY, conj, alpha)
+    ref = alpha * (np.vdot(X, Y) if conj else np.sum(X * Y))
+    assert abs(complex(ctx.tensor_download(dD)) - ref) <= 1e-13 * abs(alpha) * np.sum(np.abs(X) * np.abs(Y))
+    ctx.dot(dD, dX, dX, True, 1.0)
+    got = complex(ctx.tensor_download(dD))
+    assert got.imag == 0.0 and abs(got.real - np.sum(np.abs(X) ** 2)) <= 1e-13 * np.sum(np.abs(X) ** 2)
+    with pytest.raises(pkg.TcbError):
+        ctx.dot(dX, dX, dY, True, 1.0) if len(shape) else ctx.dot(dD, dD, dY, True, 1.0)
+    for t in (dX, dY, dD):
+        t.destroy()
+
+
+def test_ccd_diis_follows_the_oracle_and_converges(ctx):
+    o, v = 3, 5
+    B, T_mp2, eo, ev = synth.config_ccd(o, v)
+    dB = {k: ctx.tensor_from_numpy(x) for k, x in B.items()}
+    dT, energies, norms = ccd.ccd_solve_diis(ctx, dB, eo, ev, 4)
+    T_ref, e_ref, n_ref = cc.ccd_diis(B, eo, ev, 4)
+    # the small linear system amplifies rounding differences of the inner products: 1e-9, not 1e-11
+    assert np.max(np.abs(ctx.tensor_download(dT) - T_ref)) <= 1e-9 * np.abs(T_ref).max()
+    for x, y in zip(energies, e_ref):
+        assert abs(x - y) <= 1e-9 * abs(y)
+    dT2, energies2, norms2 = ccd.ccd_solve_diis(ctx, dB, eo, ev, 16)
+    dR = ccd.ccd_residual(ctx, dB, dT2)
+    assert np.max(np.abs(ctx.tensor_download(dR))) <= 1e-11 * np.abs(B["vvoo"]).max()
+    assert norms2[-1] <= 1e-11 * norms2[0]
+    # same fixed point as the plain iteration
+    assert abs(energies2[-1] - cc.ccd_jacobi(B, eo, ev, 40)[1][-1]) <= 1e-11 * abs(energies2[-1])

@@ -194,3 +194,27 @@ def test_converged_ccsd_jacobi_zeroes_the_fock_space_singles_and_doubles(o, v):
     assert np.abs(r1).max() <= 1e-12 * scale and np.abs(r2).max() <= 1e-12 * scale
     assert abs(energies[-1] - e0) <= 1e-12 * abs(e0)
     assert np.abs(T1).max() > 1e-3 and np.abs(T2).max() > 1e-3
+
+
+def test_diis_reaches_the_same_fixed_point_in_fewer_steps():
+    """DIIS changes the path, not the solution: its amplitudes zero the Fock-space projection as well, the error vector of
+    the 6th DIIS step is far below that of the 6th Jacobi step, and the coefficients sum to one."""
+    o, v = 3, 3
+    B, T_mp2, eo, ev, f, g = _ccd_problem(o, v)
+    T, energies, norms = cc.ccd_diis(B, eo, ev, 14)
+    e0, _, r0 = cc.fock_space_residuals(o, v, f, g, T)
+    assert np.abs(r0).max() <= 1e-12 * np.abs(B["vvoo"]).max()
+    assert abs(energies[-1] - e0) <= 1e-12 * abs(e0)
+    Tj, _ = cc.ccd_jacobi(B, eo, ev, 5)
+    rj = cc.ccd_residual_program(B, Tj)
+    d = eo[None, None, :, None] + eo[None, None, None, :] - ev[:, None, None, None] - ev[None, :, None, None]
+    assert norms[5] < 0.1 * np.linalg.norm(rj / d)
+    assert abs(norms[0] - np.linalg.norm(B["vvoo"] / d)) <= 1e-13 * norms[0]      # first error vector = MP2 amplitudes
+    Bm = np.array([[2.0, 0.5j], [-0.5j, 1.0]])
+    c = cc.diis_coefficients(Bm)
+    assert abs(c.sum() - 1) <= 1e-15
+    # the constrained minimum: any other c' with sum 1 gives a larger c'^H B c'
+    best = np.vdot(c, Bm @ c).real
+    for t in (-0.3, 0.2, 0.7, 1.4):
+        cp = np.array([t, 1 - t])
+        assert np.vdot(cp, Bm @ cp).real >= best - 1e-15
