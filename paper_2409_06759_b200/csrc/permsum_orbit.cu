@@ -49,7 +49,7 @@ struct alignas(4) OrbitEntry {              // one orbit of cube coordinates
 static_assert(sizeof(OrbitEntry) == 76, "OrbitEntry is copied word by word");
 
 struct OrbitParams {
-    int nterms, ntau, nO, stages, eI, beta_zero;
+    int nterms, ntau, nO, stages, dbufs, eI, beta_zero;
     int eO[3];                               // outer extents (dims 3..)
     long long slab_elems;                    // eI^3
     long long xsO[kMaxTau][3];               // stride in X of D's outer index k under outer class u
@@ -143,8 +143,9 @@ struct ItemCursor {
 };
 
 // barrier indices
-constexpr int kXFull = 0, kXEmpty = kMaxStages, kDFull = 2 * kMaxStages, kDReady = 2 * kMaxStages + 2;
-constexpr int kNumBars = 2 * kMaxStages + 4;
+constexpr int kMaxDBufs = 6;
+constexpr int kXFull = 0, kXEmpty = kMaxStages, kDFull = 2 * kMaxStages, kDReady = 2 * kMaxStages + kMaxDBufs;
+constexpr int kNumBars = 2 * kMaxStages + 2 * kMaxDBufs;
 
 __global__ void __launch_bounds__(kThreads, 1)
 permsum_orbit_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmD,
@@ -159,13 +160,13 @@ permsum_orbit_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
     const uint32_t dbuf_bytes = kMaxOmega * kCubeBytes;
     // shared memory: [2 D buffers of 6 cubes][stages x (6 * ntau cubes of X)]
     const uint32_t dbuf0 = smem_u32(orb_smem);
-    const uint32_t data0 = dbuf0 + 2 * dbuf_bytes;
+    const uint32_t data0 = dbuf0 + p.dbufs * dbuf_bytes;
     if (tid == 0) {
         for (int s = 0; s < p.stages; ++s) {
             mbar_init(bar0 + 8 * (kXFull + s), 1);                  // the producer's arrive + the bytes
             mbar_init(bar0 + 8 * (kXEmpty + s), kConsumerWarps);    // one arrive per consumer warp
         }
-        for (int b = 0; b < 2; ++b) {
+        for (int b = 0; b < p.dbufs; ++b) {
             mbar_init(bar0 + 8 * (kDFull + b), 1);                  // D cubes loaded (or, beta = 0, buffer free)
             mbar_init(bar0 + 8 * (kDReady + b), kConsumerWarps);    // results written: the buffer may be stored
         }
@@ -249,7 +250,7 @@ permsum_orbit_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
             __syncwarp();
             if (lane < n) tma_load_4d(dbuf0 + b * dbuf_bytes + lane * kCubeBytes, &tmD, c0, c1, c2, c3, full);
         };
-        for (int b = 0; b < 2; ++b)
+        for (int b = 0; b < p.dbufs; ++b)
             if (ld.valid()) {
                 int n, c0, c1, c2, c3;
                 cube_coords(ld, &n, &c0, &c1, &c2, &c3);
@@ -258,12 +259,12 @@ permsum_orbit_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
             }
         unsigned it = 0;
         for (; cur.valid(); cur.advance(p), ++it) {
-            const int b = (int)(it & 1u);
+            const int b = (int)(it % (unsigned)p.dbufs);
             int sn, s0, s1, s2, s3, ln = 0, l0 = 0, l1 = 0, l2 = 0, l3 = 0;
             cube_coords(cur, &sn, &s0, &s1, &s2, &s3);               // fetched before the wait
             const bool more = ld.valid();
             if (more) cube_coords(ld, &ln, &l0, &l1, &l2, &l3);
-            mbar_wait(bar0 + 8 * (kDReady + b), (it >> 1) & 1u);     // every consumer warp has written its results
+            mbar_wait(bar0 + 8 * (kDReady + b), (it / (unsigned)p.dbufs) & 1u);     // every consumer warp has written its results
             if (lane < sn) {
                 tma_store_4d(&tmD, s0, s1, s2, s3, dbuf0 + b * dbuf_bytes + lane * kCubeBytes);
                 asm volatile("cp.async.bulk.commit_group;" ::: "memory");
@@ -298,12 +299,12 @@ permsum_orbit_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_const
     for (; cur.valid(); cur.advance(p), ++it) {
         const int st = (int)(it % (unsigned)p.stages);
         const uint32_t par = (it / (unsigned)p.stages) & 1u;
-        const int b = (int)(it & 1u);
+        const int b = (int)(it % (unsigned)p.dbufs);
         const StageMeta &m = s_meta[st];
         mbar_wait(bar0 + 8 * (kXFull + st), par);
-        mbar_wait(bar0 + 8 * (kDFull + b), (it >> 1) & 1u);
+        mbar_wait(bar0 + 8 * (kDFull + b), (it / (unsigned)p.dbufs) & 1u);
         const int n = m.n;
-        const double2 *cubes = reinterpret_cast<const double2 *>(orb_smem + 2 * dbuf_bytes + (size_t)st * stage_bytes);
+        const double2 *cubes = reinterpret_cast<const double2 *>(orb_smem + (size_t)p.dbufs * dbuf_bytes + (size_t)st * stage_bytes);
         double2 *dcube = reinterpret_cast<double2 *>(orb_smem + (size_t)b * dbuf_bytes);
 #pragma unroll
         for (int j = 0; j < kRounds; ++j) {
@@ -460,7 +461,9 @@ cudaError_t build_plan(const PermSumDesc &d, OrbitPlan &plan)
     for (int u = p.ntau; u < kMaxTau; ++u)
         for (int k = 0; k < 3; ++k) p.xsO[u][k] = 0;
     const size_t stage_bytes = (size_t)kMaxOmega * p.ntau * kCubeBytes;
-    const size_t dbufs = 2 * (size_t)kMaxOmega * kCubeBytes, budget = 227 * 1024 - 4096;   // static: barriers, stage tables
+    const size_t budget = 227 * 1024 - 4096;                       // static: barriers, stage tables
+    p.dbufs = getenv("TCB_ORBIT_DBUFS") ? std::max(2, std::min(kMaxDBufs, atoi(getenv("TCB_ORBIT_DBUFS")))) : 2;
+    const size_t dbufs = (size_t)p.dbufs * kMaxOmega * kCubeBytes;
     p.stages = (int)std::min<size_t>(kMaxStages, (budget - dbufs) / stage_bytes);
     if (getenv("TCB_ORBIT_STAGES")) p.stages = std::min(p.stages, atoi(getenv("TCB_ORBIT_STAGES")));
     if (p.stages < 2) return cudaSuccess;
