@@ -507,3 +507,53 @@ def t3_term_program(W, T2, R3, long_double=True):
                        long_double=long_double, want_snorm=False)
     perms, coefs = p9_terms()
     return X, _o.permsum(R3, X, perms, coefs, 1.0)
+
+
+# ------------------------------------------------------------------------------------------
+# next row 8(f)-3, outlook of the paper (CCSD(T)): the [T] triples correction from doubles.
+#   R3(a,b,c,i,j,k) = <Phi_ijk^abc| [H, T2] |Phi0>
+#                   = P(k/ij)P(a/bc) sum_d <bc||dk> t_ij^ad - P(i/jk)P(c/ab) sum_l <lc||jk> t_il^ab
+#   t3 = R3 / D3,  D3 = e_i + e_j + e_k - e_a - e_b - e_c ;   E[T] = 1/36 sum conj(t3) D3 t3 = 1/36 <t3|R3>
+# The connected-triples formula is pinned to the tier-0 triples projection, the 1/36 to a sum over unique triples.
+# ------------------------------------------------------------------------------------------
+def p9_terms_second():
+    """The 9 signed index maps of P(i/jk)P(c/ab) in the permsum convention."""
+    abc = [((0, 1, 2), 1.0), ((2, 1, 0), -1.0), ((0, 2, 1), -1.0)]      # 1 - (c<->a) - (c<->b)
+    ijk = [((3, 4, 5), 1.0), ((4, 3, 5), -1.0), ((5, 4, 3), -1.0)]      # 1 - (i<->j) - (i<->k)
+    perms, coefs = [], []
+    for (pa, sa) in abc:
+        for (pi, si) in ijk:
+            perms.append(list(pa) + list(pi))
+            coefs.append(sa * si)
+    return perms, coefs
+
+
+def triples_unfactorised(o, g, t2, e_occ, e_virt):
+    """(R3, E[T]) by direct sums."""
+    W, U = g[o:, o:, o:, :o], g[:o, o:, :o, :o]                          # <bc||dk>, <lc||jk>
+    _, Y = t3_term_unfactorised(W, t2)
+    Z = np.einsum("lcjk,abil->abcijk", U, t2)
+    Z = Z - _swap(Z, 2, 0) - _swap(Z, 2, 1)
+    Z = Z - _swap(Z, 3, 4) - _swap(Z, 3, 5)
+    R3 = Y - Z
+    eo, ev = np.asarray(e_occ), np.asarray(e_virt)
+    D3 = (eo[None, None, None, :, None, None] + eo[None, None, None, None, :, None] + eo[None, None, None, None, None, :]
+          - ev[:, None, None, None, None, None] - ev[None, :, None, None, None, None] - ev[None, None, :, None, None, None])
+    return R3, np.sum(np.conj(R3) * R3 / D3) / 36.0
+
+
+def triples_program(W, U, T2, e_occ, e_virt, long_double=True):
+    """The same as library calls: two contractions into rank-6 tensors, two 9-term permute-sums, one denominator
+    update, one inner product.  W(b,c,d,k) = <bc||dk>, U(l,c,j,k) = <lc||jk>.  Returns (R3, t3, E[T])."""
+    v, o = T2.shape[0], T2.shape[2]
+    z6 = lambda: np.zeros((v, v, v, o, o, o), dtype=np.complex128, order="F")
+    con = lambda e, D, L, R, a=1.0: _o.contract(e, D, L, R, a, long_double=long_double, want_snorm=False)[0]
+    X = con("X(a,b,c,i,j,k)=W(b,c,d,k)*T(a,d,i,j)", z6(), W, T2)
+    p1, c1 = p9_terms()
+    R3 = _o.permsum(z6(), X, p1, c1, 0.0)
+    Z = con("Z(a,b,c,i,j,k)=T(a,b,i,l)*U(l,c,j,k)", z6(), T2, U)
+    p2, c2 = p9_terms_second()
+    R3 = _o.permsum(R3, Z, p2, [-c for c in c2], 1.0)
+    ev, eo = -np.asarray(e_virt, dtype=np.float64), np.asarray(e_occ, dtype=np.float64)
+    t3 = denominator_update(z6(), R3, [ev, ev, ev, eo, eo, eo], 1.0)
+    return R3, t3, np.vdot(t3, R3) / 36.0

@@ -191,6 +191,32 @@ def ccd_solve(ctx, B, e_occ, e_virt, iterations, T=None):
     return T, energies
 
 
+def triples_correction(ctx, W, U, T2, e_occ, e_virt, keep=False):
+    """The [T] triples correction from doubles (the paper's outlook, CCSD(T): PAPER.md:386, 452), all rank-6 work on the
+    device:  R3 = P(k/ij)P(a/bc) sum_d <bc||dk> t_ij^ad - P(i/jk)P(c/ab) sum_l <lc||jk> t_il^ab   (two contractions into
+    6 GB-class tensors, two 9-term antisymmetrisers),  t3 = R3 / (e_i + e_j + e_k - e_a - e_b - e_c)
+    (`tcb_denominator_update`),  E[T] = 1/36 <t3|R3> (`tcb_dot`).  W (v,v,v,o) = <bc||dk>, U (o,v,o,o) = <lc||jk>.
+    Returns the rank-0 tensor E (and R3, t3 when keep=True)."""
+    import numpy as np
+    v, _, o, _ = T2.extents
+    shape = (v, v, v, o, o, o)
+    X, R3 = ctx.tensor_create(shape), ctx.tensor_create(shape)
+    ctx.contract("X(a,b,c,i,j,k)=W(b,c,d,k)*T(a,d,i,j)", X, W, T2, 1.0)
+    ctx.antisymmetrize("P(a/bc)P(k/ij):R(a,b,c,i,j,k)=X(a,b,c,i,j,k)", R3, X, 1.0)
+    ctx.contract("X(a,b,c,i,j,k)=T(a,b,i,l)*U(l,c,j,k)", X, T2, U, 1.0)
+    ctx.antisymmetrize("P(c/ab)P(i/jk):R(a,b,c,i,j,k)+=X(a,b,c,i,j,k)", R3, X, -1.0)
+    ctx.tensor_fill(X, 0.0)                                            # X becomes t3
+    ev, eo = -np.asarray(e_virt, dtype=np.float64), np.asarray(e_occ, dtype=np.float64)
+    ctx.denominator_update(X, R3, [ev, ev, ev, eo, eo, eo], 1.0)
+    E = ctx.tensor_create(())
+    ctx.dot(E, X, R3, True, 1.0 / 36.0)
+    if keep:
+        return E, R3, X
+    X.destroy()
+    R3.destroy()
+    return E
+
+
 def ccd_solve_diis(ctx, B, e_occ, e_virt, iterations, depth=6):
     """The CCD iteration with DIIS extrapolation (Pulay): error vector e_k = R(T_k) / D, trial vector T_k + e_k, next T =
     the combination of the last `depth` trial vectors minimising |sum c_i e_i|.  Tensors, inner products (`tcb_dot`,

@@ -2,6 +2,8 @@
 // the scalar factor of PAPER.md:230).  Memory-bound, one 16-byte access per element, grid-stride.
 #include "kernels.h"
 
+#include <algorithm>
+
 namespace tcb {
 
 namespace {
@@ -126,37 +128,79 @@ cudaError_t launch_dot(void *D, const void *X, const void *Y, int64_t n, bool co
 }
 
 // T[idx] += alpha * R[idx] / (sum_k eps_k[idx_k])  -- the Jacobi step of a CC solver (orbital-energy denominators)
+// A CTA takes a slab (the leading `ninner` dims, >= 2048 elements when the tensor has them) at a time: the outer
+// indices and their energies are decoded once per slab, an element costs ninner - 1 32-bit divisions (the first
+// version decoded every element with six 64-bit divisions: 4.9 ms on a 6 GB rank-6 tensor, 3.7 TB/s).
 struct DenomParams {
-    int rank;
+    int rank, ninner;
     long long e[kMaxRank];
     int eps_at[kMaxRank];            // start of dim k's energies in `eps`, -1: the index does not enter the denominator
     const double *eps;
     double2 *T;
     const double2 *R;
-    long long n;
+    long long nslabs;
+    unsigned slab;                   // elements per slab
     double ar, ai;
 };
 
 __global__ void __launch_bounds__(256) denominator_update_kernel(const __grid_constant__ DenomParams p)
 {
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < p.n; i += stride) {
-        unsigned long long rem = (unsigned long long)i;
-        double d = 0.0;
+    for (long long sl = blockIdx.x; sl < p.nslabs; sl += gridDim.x) {
+        // energies of the outer indices, added in index order AFTER the inner ones (so the sum keeps index order)
+        double outer[kMaxRank];
+        unsigned long long rem = (unsigned long long)sl;
 #pragma unroll
-        for (int k = 0; k < kMaxRank; ++k)
-            if (k < p.rank) {
+        for (int k = 0; k < kMaxRank; ++k) {
+            outer[k] = 0.0;
+            if (k >= p.ninner && k < p.rank) {
                 const unsigned long long q = rem / (unsigned long long)p.e[k];
                 const long long ik = (long long)(rem - q * (unsigned long long)p.e[k]);
                 rem = q;
-                if (p.eps_at[k] >= 0) d = __dadd_rn(d, p.eps[p.eps_at[k] + ik]);      // summed in index order
+                if (p.eps_at[k] >= 0) outer[k] = p.eps[p.eps_at[k] + ik];
             }
-        const double2 r = p.R[i];
-        const double qr = __ddiv_rn(r.x, d), qi = __ddiv_rn(r.y, d);
-        double2 t = p.T[i];
-        t.x = __dadd_rn(t.x, __dsub_rn(__dmul_rn(p.ar, qr), __dmul_rn(p.ai, qi)));
-        t.y = __dadd_rn(t.y, __dadd_rn(__dmul_rn(p.ar, qi), __dmul_rn(p.ai, qr)));
-        p.T[i] = t;
+        }
+        const long long base = sl * (long long)p.slab;
+        // four elements per thread and round: all eight loads are issued before the first division
+        for (unsigned j0 = threadIdx.x; j0 < p.slab; j0 += 4 * 256) {
+            double2 x[4], t[4];
+            double d[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const unsigned j = j0 + u * 256;
+                if (j < p.slab) {
+                    x[u] = p.R[base + j];
+                    t[u] = p.T[base + j];
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                unsigned r = j0 + u * 256;
+                d[u] = 0.0;
+#pragma unroll
+                for (int k = 0; k < kMaxRank; ++k)
+                    if (k < p.rank) {
+                        if (k < p.ninner) {
+                            const unsigned ek = (unsigned)p.e[k];
+                            const unsigned q = k + 1 < p.ninner ? r / ek : 0u;
+                            const unsigned ik = min(r - q * ek, ek - 1);      // (a lane past the slab reads a valid slot)
+                            r = q;
+                            if (p.eps_at[k] >= 0) d[u] = __dadd_rn(d[u], p.eps[p.eps_at[k] + ik]);
+                        } else if (p.eps_at[k] >= 0) {
+                            d[u] = __dadd_rn(d[u], outer[k]);
+                        }
+                    }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const unsigned j = j0 + u * 256;
+                if (j < p.slab) {
+                    const double qr = __ddiv_rn(x[u].x, d[u]), qi = __ddiv_rn(x[u].y, d[u]);
+                    t[u].x = __dadd_rn(t[u].x, __dsub_rn(__dmul_rn(p.ar, qr), __dmul_rn(p.ai, qi)));
+                    t[u].y = __dadd_rn(t[u].y, __dadd_rn(__dmul_rn(p.ar, qi), __dmul_rn(p.ai, qr)));
+                    p.T[base + j] = t[u];
+                }
+            }
+        }
     }
 }
 
@@ -165,17 +209,26 @@ cudaError_t launch_denominator_update(void *T, const void *R, int rank, const in
 {
     DenomParams p;
     p.rank = rank;
-    p.n = 1;
+    long long n = 1, slab = 1;
+    p.ninner = 0;
     for (int k = 0; k < kMaxRank; ++k) {
         p.e[k] = k < rank ? extent[k] : 1;
         p.eps_at[k] = k < rank ? eps_at[k] : -1;
-        p.n *= p.e[k];
+        n *= p.e[k];
+        if (k < rank && (slab < 2048 || p.ninner == 0) && slab * p.e[k] <= (1LL << 30)) {
+            slab *= p.e[k];
+            p.ninner = k + 1;
+        }
     }
+    if (p.ninner == 0) { p.ninner = rank; slab = n; }       // rank 0 never gets here (no energies); keeps the kernel total
+    p.slab = (unsigned)slab;
+    p.nslabs = n / slab;
     p.eps = eps_dev;
     p.T = (double2 *)T;
     p.R = (const double2 *)R;
     p.ar = re; p.ai = im;
-    denominator_update_kernel<<<grid_for(p.n), 256, 0, s>>>(p);
+    const int blocks = (int)std::max<long long>(1, std::min<long long>(p.nslabs, 148LL * 8));
+    denominator_update_kernel<<<blocks, 256, 0, s>>>(p);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess && launches) ++*launches;
     return e;

@@ -225,3 +225,30 @@ def test_ccd_diis_follows_the_oracle_and_converges(ctx):
     assert norms2[-1] <= 1e-11 * norms2[0]
     # same fixed point as the plain iteration
     assert abs(energies2[-1] - cc.ccd_jacobi(B, eo, ev, 40)[1][-1]) <= 1e-11 * abs(energies2[-1])
+
+
+@pytest.mark.parametrize("o,v", [(3, 4), (4, 12)])
+def test_triples_correction_program(ctx, o, v):
+    """[T] from doubles: two rank-6 contractions, two 9-term antisymmetrisers (the second one is P(c/ab)P(i/jk)), the
+    rank-6 denominator update and the inner product, against the oracle's program of the same calls."""
+    n = o + v
+    g = synth.tensor(synth.SEED0 + 7, 1, [n] * 4, antisym=((0, 1), (2, 3)), sigma=0.3, hermitian=True)
+    rng = np.random.default_rng(o + v)
+    t2 = rng.standard_normal((v, v, o, o)) + 1j * rng.standard_normal((v, v, o, o))
+    t2 = t2 - t2.transpose(1, 0, 2, 3)
+    t2 = np.asfortranarray(t2 - t2.transpose(0, 1, 3, 2))
+    eo, ev = np.linspace(-2.0, -0.5, o), np.linspace(0.5, 3.0, v)
+    W, U = np.asfortranarray(g[o:, o:, o:, :o]), np.asfortranarray(g[:o, o:, :o, :o])
+    dW, dU, dT = ctx.tensor_from_numpy(W), ctx.tensor_from_numpy(U), ctx.tensor_from_numpy(t2)
+    dE, dR3, dt3 = ccd.triples_correction(ctx, dW, dU, dT, eo, ev, keep=True)
+    R3, t3, E = cc.triples_program(W, U, t2, eo, ev)
+    scale = np.abs(R3).max()
+    assert np.max(np.abs(ctx.tensor_download(dR3) - R3)) <= 1e-11 * scale
+    assert np.max(np.abs(ctx.tensor_download(dt3) - t3)) <= 1e-11 * np.abs(t3).max()
+    got = complex(ctx.tensor_download(dE))
+    assert abs(got - E) <= 1e-11 * abs(E) and got.real < 0
+    if o == 3:
+        R3u, Eu = cc.triples_unfactorised(o, g, t2, eo, ev)
+        assert abs(got - Eu) <= 1e-11 * abs(Eu)
+    for t in (dW, dU, dT, dE, dR3, dt3):
+        t.destroy()

@@ -218,3 +218,33 @@ def test_diis_reaches_the_same_fixed_point_in_fewer_steps():
     for t in (-0.3, 0.2, 0.7, 1.4):
         cp = np.array([t, 1 - t])
         assert np.vdot(cp, Bm @ cp).real >= best - 1e-15
+
+
+def test_triples_correction_against_the_fock_space_and_unique_triples():
+    """R3 of the [T] correction is the tier-0 projection <Phi_ijk^abc|[H,T2]|Phi0>; the energy's 1/36 is checked by
+    summing |R3|^2 / D3 over unique triples a<b<c, i<j<k; the program of library calls reproduces both."""
+    o = v = 3
+    f, g, t = rand_inputs(o, v, 21)
+    eo, ev = np.linspace(-2.0, -0.5, o), np.linspace(0.5, 3.0, v)
+    fs = cc.FockSpace(o, v)
+    psi = fs.apply_H(f, g, fs.apply_T(None, t, fs.phi0)) - fs.apply_T(None, t, fs.apply_H(f, g, fs.phi0))
+    R3_0 = fs.project_triples(psi)
+    R3, E = cc.triples_unfactorised(o, g, t, eo, ev)
+    assert np.abs(R3 - R3_0).max() <= 1e-13 * np.abs(R3_0).max()
+    e_unique = 0.0
+    for a in range(v):
+        for b in range(a + 1, v):
+            for c in range(b + 1, v):
+                for i in range(o):
+                    for j in range(i + 1, o):
+                        for k in range(j + 1, o):
+                            e_unique += abs(R3_0[a, b, c, i, j, k]) ** 2 / (eo[i] + eo[j] + eo[k] - ev[a] - ev[b] - ev[c])
+    assert e_unique < 0 and abs(E - e_unique) <= 1e-13 * abs(e_unique) and abs(E.imag) <= 1e-15 * abs(e_unique)
+    W = np.asfortranarray(g[o:, o:, o:, :o])
+    U = np.asfortranarray(g[:o, o:, :o, :o])
+    R3p, t3p, Ep = cc.triples_program(W, U, np.asfortranarray(t), eo, ev)
+    assert np.abs(R3p - R3).max() <= 1e-13 * np.abs(R3).max()
+    assert abs(Ep - E) <= 1e-13 * abs(E)
+    # antisymmetry of the triples amplitudes in (a,b,c) and (i,j,k)
+    assert np.abs(t3p + t3p.transpose(1, 0, 2, 3, 4, 5)).max() <= 1e-13 * np.abs(t3p).max()
+    assert np.abs(t3p + t3p.transpose(0, 1, 2, 3, 5, 4)).max() <= 1e-13 * np.abs(t3p).max()
