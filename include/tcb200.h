@@ -119,6 +119,9 @@ int tcb_scale(tcb_ctx *ctx, tcb_tensor *D, tcb_c128 alpha);
  * T and R have the same shape and must not overlap.  The energies are copied before the call returns.  A zero
  * denominator is not detected (the quotient is IEEE inf/nan).  Errors: TCB_EINVAL, TCB_ESHAPE, TCB_EALIAS, TCB_ECUDA. */
 int tcb_denominator_update(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, const double *const *eps, tcb_c128 alpha);
+/* The '=' form of the same operation:  T[i0,i1,..] = alpha * R[i0,i1,..] / (eps[0][i0] + eps[1][i1] + ...); T is not
+ * read (first-order amplitudes from a residual, e.g. t3 = R3 / D3 of the triples correction).  Same arguments, same errors. */
+int tcb_denominator_divide(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, const double *const *eps, tcb_c128 alpha);
 /* Inner product into a rank-0 tensor (what a DIIS extrapolation around the iteration needs; the bilinear form is also
  * reachable as a full contraction "E()=X(..)*Y(..)", the sesquilinear one only here):
  *     D = alpha * sum_i (conjugate_x ? conj(X[i]) : X[i]) * Y[i]

@@ -42,7 +42,7 @@ ABI_SYMBOLS = [
     "tcb_ctx_create", "tcb_ctx_destroy", "tcb_ctx_set_option", "tcb_sync", "tcb_last_error", "tcb_strerror",
     "tcb_launch_count", "tcb_tensor_create", "tcb_tensor_wrap", "tcb_tensor_destroy", "tcb_tensor_info",
     "tcb_tensor_upload", "tcb_tensor_download", "tcb_tensor_fill", "tcb_contract", "tcb_add", "tcb_scale",
-    "tcb_denominator_update", "tcb_dot",
+    "tcb_denominator_update", "tcb_denominator_divide", "tcb_dot",
     "tcb_permute", "tcb_permsum", "tcb_antisymmetrize", "tcb_plan_describe", "tcb_measure_fp64_tensor_peak", "tcb_measure_fp64_vector_peak",
     "tcb_timer_start", "tcb_timer_stop", "tcb_kernel_stats", "tcb_kernel_stats_reset", "tcb_plan_describe_host", "tcbx_synth_normal", "tcbx_synth_index_linear",
     "tcbx_synth_mp2_amplitudes",
@@ -76,6 +76,7 @@ def load_library():
         "tcb_add": [vp, cp, vp, vp, c128],
         "tcb_scale": [vp, vp, c128],
         "tcb_denominator_update": [vp, vp, vp, ctypes.POINTER(ctypes.POINTER(ctypes.c_double)), c128],
+        "tcb_denominator_divide": [vp, vp, vp, ctypes.POINTER(ctypes.POINTER(ctypes.c_double)), c128],
         "tcb_dot": [vp, vp, vp, vp, ctypes.c_int, c128],
         "tcb_permute": [vp, cp, vp, vp],
         "tcb_permsum": [vp, vp, vp, ctypes.c_int, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(c128), c128],
@@ -270,13 +271,20 @@ class Context:
     def scale(self, D, alpha):
         self._check(self.lib.tcb_scale(self.handle, D.handle, _c(alpha)))
 
-    def denominator_update(self, T, R, eps, alpha=1.0):
-        """T[i0,i1,..] += alpha * R[i0,i1,..] / (eps[0][i0] + eps[1][i1] + ...); eps: one real vector (or None) per index."""
+    def _denominator(self, fn, T, R, eps, alpha):
         import numpy as np
         keep = [None if e is None else np.ascontiguousarray(e, dtype=np.float64) for e in eps]
         dp = ctypes.POINTER(ctypes.c_double)
         arr = (dp * len(keep))(*[ctypes.cast(None, dp) if e is None else e.ctypes.data_as(dp) for e in keep])
-        self._check(self.lib.tcb_denominator_update(self.handle, T.handle, R.handle, arr, _c(alpha)))
+        self._check(fn(self.handle, T.handle, R.handle, arr, _c(alpha)))
+
+    def denominator_update(self, T, R, eps, alpha=1.0):
+        """T[i0,i1,..] += alpha * R[i0,i1,..] / (eps[0][i0] + eps[1][i1] + ...); eps: one real vector (or None) per index."""
+        self._denominator(self.lib.tcb_denominator_update, T, R, eps, alpha)
+
+    def denominator_divide(self, T, R, eps, alpha=1.0):
+        """T[i0,i1,..] = alpha * R[i0,i1,..] / (eps[0][i0] + eps[1][i1] + ...); T is not read."""
+        self._denominator(self.lib.tcb_denominator_divide, T, R, eps, alpha)
 
     def dot(self, D, X, Y, conjugate_x=True, alpha=1.0):
         """D (rank 0) = alpha * sum conj?(X) * Y"""

@@ -195,7 +195,7 @@ def triples_correction(ctx, W, U, T2, e_occ, e_virt, keep=False):
     """The [T] triples correction from doubles (the paper's outlook, CCSD(T): PAPER.md:386, 452), all rank-6 work on the
     device:  R3 = P(k/ij)P(a/bc) sum_d <bc||dk> t_ij^ad - P(i/jk)P(c/ab) sum_l <lc||jk> t_il^ab   (two contractions into
     6 GB-class tensors, two 9-term antisymmetrisers),  t3 = R3 / (e_i + e_j + e_k - e_a - e_b - e_c)
-    (`tcb_denominator_update`),  E[T] = 1/36 <t3|R3> (`tcb_dot`).  W (v,v,v,o) = <bc||dk>, U (o,v,o,o) = <lc||jk>.
+    (`tcb_denominator_divide`),  E[T] = 1/36 <t3|R3> (`tcb_dot`).  W (v,v,v,o) = <bc||dk>, U (o,v,o,o) = <lc||jk>.
     Returns the rank-0 tensor E (and R3, t3 when keep=True)."""
     import numpy as np
     v, _, o, _ = T2.extents
@@ -205,9 +205,8 @@ def triples_correction(ctx, W, U, T2, e_occ, e_virt, keep=False):
     ctx.antisymmetrize("P(a/bc)P(k/ij):R(a,b,c,i,j,k)=X(a,b,c,i,j,k)", R3, X, 1.0)
     ctx.contract("X(a,b,c,i,j,k)=T(a,b,i,l)*U(l,c,j,k)", X, T2, U, 1.0)
     ctx.antisymmetrize("P(c/ab)P(i/jk):R(a,b,c,i,j,k)+=X(a,b,c,i,j,k)", R3, X, -1.0)
-    ctx.tensor_fill(X, 0.0)                                            # X becomes t3
     ev, eo = -np.asarray(e_virt, dtype=np.float64), np.asarray(e_occ, dtype=np.float64)
-    ctx.denominator_update(X, R3, [ev, ev, ev, eo, eo, eo], 1.0)
+    ctx.denominator_divide(X, R3, [ev, ev, ev, eo, eo, eo], 1.0)       # X becomes t3
     E = ctx.tensor_create(())
     ctx.dot(E, X, R3, True, 1.0 / 36.0)
     if keep:
@@ -235,10 +234,9 @@ def ccd_solve_diis(ctx, B, e_occ, e_virt, iterations, depth=6):
         if len(err) == depth:                      # the oldest pair leaves; its tensors are reused
             e, t = err.pop(0), trial.pop(0)
             Bm = Bm[1:, 1:]
-            ctx.tensor_fill(e, 0.0)
         else:
             e, t = ctx.tensor_create(shape), ctx.tensor_create(shape)
-        ctx.denominator_update(e, R, [ev, ev, eo, eo], 1.0)
+        ctx.denominator_divide(e, R, [ev, ev, eo, eo], 1.0)
         ctx.add("t(a,b,i,j)=T(a,b,i,j)", t, T, 1.0)
         ctx.add("t(a,b,i,j)+=e(a,b,i,j)", t, e, 1.0)
         err.append(e)

@@ -709,7 +709,8 @@ int tcb_dot(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, const tcb_tensor *
     return TCB_OK;
 }
 
-int tcb_denominator_update(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, const double *const *eps, tcb_c128 alpha)
+static int denominator_op(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, const double *const *eps, tcb_c128 alpha,
+                          bool accumulate)
 {
     int rc = enter(ctx);
     if (rc) return rc;
@@ -737,13 +738,23 @@ int tcb_denominator_update(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, con
     TCB_CUDA(ctx, cudaMallocAsync((void **)&dev, host.size() * sizeof(double), ctx->stream));
     cudaError_t e = cudaMemcpyAsync(dev, host.data(), host.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) {
-        TimedLaunch tl(ctx, kClsElementwise, 0.0, 48.0 * (double)T->elems());
-        e = launch_denominator_update(T->ptr, R->ptr, r, T->shape.ext, dev, at, alpha.re, alpha.im, ctx->stream,
-                                      &ctx->launches);
+        TimedLaunch tl(ctx, kClsElementwise, 0.0, (accumulate ? 48.0 : 32.0) * (double)T->elems());
+        e = launch_denominator_update(T->ptr, R->ptr, r, T->shape.ext, dev, at, alpha.re, alpha.im, accumulate,
+                                      ctx->stream, &ctx->launches);
     }
     cudaFreeAsync(dev, ctx->stream);
     TCB_CUDA(ctx, e);
     return TCB_OK;
+}
+
+int tcb_denominator_update(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, const double *const *eps, tcb_c128 alpha)
+{
+    return denominator_op(ctx, T, R, eps, alpha, true);
+}
+
+int tcb_denominator_divide(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, const double *const *eps, tcb_c128 alpha)
+{
+    return denominator_op(ctx, T, R, eps, alpha, false);
 }
 
 int tcb_permsum(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, int nterms, const int32_t *perms,

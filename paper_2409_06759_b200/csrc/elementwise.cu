@@ -143,6 +143,7 @@ struct DenomParams {
     double ar, ai;
 };
 
+template <bool ACC>
 __global__ void __launch_bounds__(256) denominator_update_kernel(const __grid_constant__ DenomParams p)
 {
     for (long long sl = blockIdx.x; sl < p.nslabs; sl += gridDim.x) {
@@ -169,7 +170,7 @@ __global__ void __launch_bounds__(256) denominator_update_kernel(const __grid_co
                 const unsigned j = j0 + u * 256;
                 if (j < p.slab) {
                     x[u] = p.R[base + j];
-                    t[u] = p.T[base + j];
+                    t[u] = ACC ? p.T[base + j] : make_double2(0.0, 0.0);
                 }
             }
 #pragma unroll
@@ -195,8 +196,10 @@ __global__ void __launch_bounds__(256) denominator_update_kernel(const __grid_co
                 const unsigned j = j0 + u * 256;
                 if (j < p.slab) {
                     const double qr = __ddiv_rn(x[u].x, d[u]), qi = __ddiv_rn(x[u].y, d[u]);
-                    t[u].x = __dadd_rn(t[u].x, __dsub_rn(__dmul_rn(p.ar, qr), __dmul_rn(p.ai, qi)));
-                    t[u].y = __dadd_rn(t[u].y, __dadd_rn(__dmul_rn(p.ar, qi), __dmul_rn(p.ai, qr)));
+                    const double ur = __dsub_rn(__dmul_rn(p.ar, qr), __dmul_rn(p.ai, qi));
+                    const double ui = __dadd_rn(__dmul_rn(p.ar, qi), __dmul_rn(p.ai, qr));
+                    t[u].x = ACC ? __dadd_rn(t[u].x, ur) : ur;
+                    t[u].y = ACC ? __dadd_rn(t[u].y, ui) : ui;
                     p.T[base + j] = t[u];
                 }
             }
@@ -205,7 +208,8 @@ __global__ void __launch_bounds__(256) denominator_update_kernel(const __grid_co
 }
 
 cudaError_t launch_denominator_update(void *T, const void *R, int rank, const int64_t *extent, const double *eps_dev,
-                                      const int *eps_at, double re, double im, cudaStream_t s, int64_t *launches)
+                                      const int *eps_at, double re, double im, bool accumulate, cudaStream_t s,
+                                      int64_t *launches)
 {
     DenomParams p;
     p.rank = rank;
@@ -228,7 +232,8 @@ cudaError_t launch_denominator_update(void *T, const void *R, int rank, const in
     p.R = (const double2 *)R;
     p.ar = re; p.ai = im;
     const int blocks = (int)std::max<long long>(1, std::min<long long>(p.nslabs, 148LL * 8));
-    denominator_update_kernel<<<blocks, 256, 0, s>>>(p);
+    if (accumulate) denominator_update_kernel<true><<<blocks, 256, 0, s>>>(p);
+    else denominator_update_kernel<false><<<blocks, 256, 0, s>>>(p);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess && launches) ++*launches;
     return e;

@@ -104,9 +104,10 @@ cudaError_t launch_axpy(void *D, const void *L, int64_t n, double re, double im,
 constexpr int kDotBlocks = 148 * 4;
 cudaError_t launch_dot(void *D, const void *X, const void *Y, int64_t n, bool conj_x, double re, double im, void *partial,
                        int nblocks, cudaStream_t stream, int64_t *launches);
-// T[idx] += alpha * R[idx] / (sum_k eps[eps_at[k] + idx_k]) over the dims with eps_at[k] >= 0 (eps: device doubles)
+// T[idx] (+)= alpha * R[idx] / (sum_k eps[eps_at[k] + idx_k]) over the dims with eps_at[k] >= 0 (eps: device doubles)
 cudaError_t launch_denominator_update(void *T, const void *R, int rank, const int64_t *extent, const double *eps_dev,
-                                      const int *eps_at, double re, double im, cudaStream_t stream, int64_t *launches);
+                                      const int *eps_at, double re, double im, bool accumulate, cudaStream_t stream,
+                                      int64_t *launches);
 
 // ---- measurement -------------------------------------------------------------------------------------------
 cudaError_t run_dmma_peak(double milliseconds, double *tflops, cudaStream_t stream, int64_t *launches);

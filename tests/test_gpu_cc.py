@@ -104,6 +104,9 @@ def test_denominator_update_matches_the_oracle(ctx, shape, eps_on, alpha):
     ctx.denominator_update(dT, dR, eps, alpha)
     got, ref = ctx.tensor_download(dT), cc.denominator_update(T, R, eps, alpha)
     assert np.max(np.abs(got - ref)) <= 4e-16 * (np.abs(T).max() + abs(alpha) * np.abs(R).max() / 0.5)
+    ctx.denominator_divide(dT, dR, eps, alpha)                            # the '=' form does not read T
+    ref0 = cc.denominator_update(np.zeros_like(T), R, eps, alpha)
+    assert np.max(np.abs(ctx.tensor_download(dT) - ref0)) <= 4e-16 * abs(alpha) * np.abs(R).max() / 0.5
     with pytest.raises(pkg.TcbError):
         ctx.denominator_update(dT, dR, [None] * len(shape), 1.0)          # no energies at all
     with pytest.raises(pkg.TcbError):
