@@ -100,6 +100,19 @@ class FockSpace:
                                 out += 0.25 * t2[a, b, i, j] * (self.ad[o + a] @ (self.ad[o + b] @ aji))
         return out
 
+    def apply_T3(self, t3, psi):
+        """T3 psi, T3 = 1/36 sum t_ijk^abc a+_a a+_b a+_c a_k a_j a_i (PAPER Eq. 2); t3[a,b,c,i,j,k]."""
+        o, v = self.o, self.v
+        out = np.zeros_like(psi)
+        for i, j, k in itertools.product(range(o), repeat=3):
+            low = self.a[k] @ (self.a[j] @ (self.a[i] @ psi))
+            if not np.any(low):
+                continue
+            for a, b, c in itertools.product(range(v), repeat=3):
+                if t3[a, b, c, i, j, k] != 0:
+                    out += t3[a, b, c, i, j, k] / 36.0 * (self.ad[o + a] @ (self.ad[o + b] @ (self.ad[o + c] @ low)))
+        return out
+
     def exp_T(self, t1, t2, psi, sign=1.0):
         """exp(sign*T) psi by the terminating series (T is nilpotent on a finite Fock space)."""
         out = psi.copy()
@@ -557,3 +570,13 @@ def triples_program(W, U, T2, e_occ, e_virt, long_double=True):
     ev, eo = -np.asarray(e_virt, dtype=np.float64), np.asarray(e_occ, dtype=np.float64)
     t3 = denominator_update(z6(), R3, [ev, ev, ev, eo, eo, eo], 1.0)
     return R3, t3, np.vdot(t3, R3) / 36.0
+
+
+def triples_singles_term(t1, oovv, t3, long_double=True):
+    """The singles term that turns [T] into (T):  E_ST = <Phi0| T1^+ H T3 |Phi0> = 1/4 sum conj(t_i^a) <jk||bc> t_ijk^abc,
+    as library calls: Y(a,i) = t3(a,b,c,i,j,k) * <jk||bc> (a rank-6 tensor contracted down to rank 2), E_ST = 1/4 <t1|Y>.
+    Pinned to the Fock-space matrix element in tests/test_oracle_cc.py."""
+    v, o = t1.shape
+    Y = _o.contract("Y(a,i)=T(a,b,c,i,j,k)*W(j,k,b,c)", np.zeros((v, o), dtype=np.complex128, order="F"), t3, oovv, 1.0,
+                    long_double=long_double, want_snorm=False)[0]
+    return Y, 0.25 * np.vdot(t1, Y)

@@ -191,12 +191,14 @@ def ccd_solve(ctx, B, e_occ, e_virt, iterations, T=None):
     return T, energies
 
 
-def triples_correction(ctx, W, U, T2, e_occ, e_virt, keep=False):
+def triples_correction(ctx, W, U, T2, e_occ, e_virt, keep=False, T1=None, oovv=None):
     """The [T] triples correction from doubles (the paper's outlook, CCSD(T): PAPER.md:386, 452), all rank-6 work on the
     device:  R3 = P(k/ij)P(a/bc) sum_d <bc||dk> t_ij^ad - P(i/jk)P(c/ab) sum_l <lc||jk> t_il^ab   (two contractions into
     6 GB-class tensors, two 9-term antisymmetrisers),  t3 = R3 / (e_i + e_j + e_k - e_a - e_b - e_c)
     (`tcb_denominator_divide`),  E[T] = 1/36 <t3|R3> (`tcb_dot`).  W (v,v,v,o) = <bc||dk>, U (o,v,o,o) = <lc||jk>.
-    Returns the rank-0 tensor E (and R3, t3 when keep=True)."""
+    With T1 (v,o) and oovv given, also the singles term of (T):  Y(a,i) = t3(a,b,c,i,j,k) <jk||bc> (the rank-6 tensor
+    read once, in place), E_ST = 1/4 <t1|Y>.
+    Returns the rank-0 tensor E[T]; with T1, (E[T], E_ST); with keep=True, additionally R3 and t3."""
     import numpy as np
     v, _, o, _ = T2.extents
     shape = (v, v, v, o, o, o)
@@ -209,11 +211,18 @@ def triples_correction(ctx, W, U, T2, e_occ, e_virt, keep=False):
     ctx.denominator_divide(X, R3, [ev, ev, ev, eo, eo, eo], 1.0)       # X becomes t3
     E = ctx.tensor_create(())
     ctx.dot(E, X, R3, True, 1.0 / 36.0)
+    out = [E]
+    if T1 is not None:
+        Y, Est = ctx.tensor_create((v, o)), ctx.tensor_create(())
+        ctx.contract("Y(a,i)=T(a,b,c,i,j,k)*W(j,k,b,c)", Y, X, oovv, 1.0)
+        ctx.dot(Est, T1, Y, True, 0.25)
+        Y.destroy()
+        out.append(Est)
     if keep:
-        return E, R3, X
+        return tuple(out) + (R3, X)
     X.destroy()
     R3.destroy()
-    return E
+    return out[0] if T1 is None else tuple(out)
 
 
 def ccd_solve_diis(ctx, B, e_occ, e_virt, iterations, depth=6):

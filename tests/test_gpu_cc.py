@@ -253,5 +253,15 @@ def test_triples_correction_program(ctx, o, v):
     if o == 3:
         R3u, Eu = cc.triples_unfactorised(o, g, t2, eo, ev)
         assert abs(got - Eu) <= 1e-11 * abs(Eu)
-    for t in (dW, dU, dT, dE, dR3, dt3):
+    # (T): the singles term, the rank-6 amplitudes contracted down to rank 2 in place (GEMV route)
+    t1 = np.asfortranarray(rng.standard_normal((v, o)) + 1j * rng.standard_normal((v, o)))
+    oovv = np.asfortranarray(g[:o, :o, o:, o:])
+    dT1, dV = ctx.tensor_from_numpy(t1), ctx.tensor_from_numpy(oovv)
+    dE2, dEst = ccd.triples_correction(ctx, dW, dU, dT, eo, ev, T1=dT1, oovv=dV)
+    _, est_ref = cc.triples_singles_term(t1, oovv, t3)
+    assert abs(complex(ctx.tensor_download(dEst)) - est_ref) <= 1e-11 * abs(est_ref)
+    assert complex(ctx.tensor_download(dE2)) == got                       # deterministic: the same bits twice
+    plan = ctx.plan_describe("Y(a,i)=T(a,b,c,i,j,k)*W(j,k,b,c)", dT1, dt3, dV)
+    assert plan["route"] == "gemv" and not plan["permute_A"]
+    for t in (dW, dU, dT, dE, dR3, dt3, dT1, dV, dE2, dEst):
         t.destroy()

@@ -248,3 +248,21 @@ def test_triples_correction_against_the_fock_space_and_unique_triples():
     # antisymmetry of the triples amplitudes in (a,b,c) and (i,j,k)
     assert np.abs(t3p + t3p.transpose(1, 0, 2, 3, 4, 5)).max() <= 1e-13 * np.abs(t3p).max()
     assert np.abs(t3p + t3p.transpose(0, 1, 2, 3, 5, 4)).max() <= 1e-13 * np.abs(t3p).max()
+
+
+def test_triples_singles_term_against_the_fock_space_matrix_element():
+    """E_ST = <T1 Phi0| H |T3 Phi0> on the Fock space (T3 from PAPER Eq. 2) against 1/4 sum conj(t1) <jk||bc> t3."""
+    o = v = 3
+    f, g, t2 = rand_inputs(o, v, 33)
+    eo, ev = np.linspace(-2.0, -0.5, o), np.linspace(0.5, 3.0, v)
+    rng = np.random.default_rng(3)
+    t1 = np.asfortranarray(rng.standard_normal((v, o)) + 1j * rng.standard_normal((v, o)))
+    W, U = np.asfortranarray(g[o:, o:, o:, :o]), np.asfortranarray(g[:o, o:, :o, :o])
+    _, t3, _ = cc.triples_program(W, U, np.asfortranarray(t2), eo, ev)
+    fs = cc.FockSpace(o, v)
+    e0 = np.vdot(fs.apply_T(t1, None, fs.phi0), fs.apply_H(f, g, fs.apply_T3(t3, fs.phi0)))
+    Y, e = cc.triples_singles_term(t1, cc.block(o, g, "oovv"), t3)
+    assert abs(e - e0) <= 1e-13 * abs(e0)
+    assert abs(e - 0.25 * np.einsum("ai,jkbc,abcijk->", t1.conj(), g[:o, :o, o:, o:], t3)) <= 1e-13 * abs(e0)
+    # T3 Phi0 has the right norm: 1/36 of the sum over all index tuples = sum over unique triples
+    assert abs(np.vdot(fs.apply_T3(t3, fs.phi0), fs.apply_T3(t3, fs.phi0)) - np.sum(np.abs(t3) ** 2) / 36.0) <= 1e-13 * np.sum(np.abs(t3) ** 2)
