@@ -86,6 +86,9 @@ int64_t tcb_launch_count(const tcb_ctx *ctx);
 
 /* Library-owned, zero-filled device tensor.  extents[rank], copied. */
 int tcb_tensor_create(tcb_ctx *ctx, tcb_tensor **t, int rank, const int64_t *extents);
+/* The same without the zero fill: contents are undefined until written.  For intermediates whose first use is an '='
+ * operation (generated code creates and destroys them around every use); a 6 GB tensor saves 1 ms. */
+int tcb_tensor_alloc(tcb_ctx *ctx, tcb_tensor **t, int rank, const int64_t *extents);
 /* Borrow caller-owned device memory (e.g. torch storage), 16-byte aligned, prod(extents)*16 bytes. */
 int tcb_tensor_wrap(tcb_ctx *ctx, tcb_tensor **t, int rank, const int64_t *extents, void *device_ptr);
 /* Stream-ordered free of library-owned memory; borrowed memory is left alone.  NULL is accepted. */

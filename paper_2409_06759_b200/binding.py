@@ -40,7 +40,7 @@ def library_path():
 # every symbol include/tcb200.h and include/tcb200_synth.h declare
 ABI_SYMBOLS = [
     "tcb_ctx_create", "tcb_ctx_destroy", "tcb_ctx_set_option", "tcb_sync", "tcb_last_error", "tcb_strerror",
-    "tcb_launch_count", "tcb_tensor_create", "tcb_tensor_wrap", "tcb_tensor_destroy", "tcb_tensor_info",
+    "tcb_launch_count", "tcb_tensor_create", "tcb_tensor_alloc", "tcb_tensor_wrap", "tcb_tensor_destroy", "tcb_tensor_info",
     "tcb_tensor_upload", "tcb_tensor_download", "tcb_tensor_fill", "tcb_contract", "tcb_add", "tcb_scale",
     "tcb_denominator_update", "tcb_denominator_divide", "tcb_dot",
     "tcb_permute", "tcb_permsum", "tcb_antisymmetrize", "tcb_plan_describe", "tcb_measure_fp64_tensor_peak", "tcb_measure_fp64_vector_peak",
@@ -66,6 +66,7 @@ def load_library():
         "tcb_ctx_set_option": [vp, cp, cp],
         "tcb_sync": [vp],
         "tcb_tensor_create": [vp, ctypes.POINTER(vp), ctypes.c_int, i64p],
+        "tcb_tensor_alloc": [vp, ctypes.POINTER(vp), ctypes.c_int, i64p],
         "tcb_tensor_wrap": [vp, ctypes.POINTER(vp), ctypes.c_int, i64p, vp],
         "tcb_tensor_destroy": [vp],
         "tcb_tensor_info": [vp, ctypes.POINTER(ctypes.c_int), i64p, ctypes.POINTER(vp)],
@@ -211,10 +212,12 @@ class Context:
         return int(self.lib.tcb_launch_count(self.handle))
 
     # ---- tensors ----
-    def tensor_create(self, extents):
+    def tensor_create(self, extents, zero=True):
+        """zero=False: tcb_tensor_alloc, contents undefined until written (for targets of '=' operations)"""
         e, r = _ext(extents)
         h = ctypes.c_void_p()
-        self._check(self.lib.tcb_tensor_create(self.handle, ctypes.byref(h), r, e))
+        fn = self.lib.tcb_tensor_create if zero else self.lib.tcb_tensor_alloc
+        self._check(fn(self.handle, ctypes.byref(h), r, e))
         return self._track(Tensor(self, h, extents))
 
     def tensor_wrap(self, extents, device_ptr, keepalive=None):

@@ -25,31 +25,31 @@ def ccd_residual(ctx, B, T, R=None):
     Returns the residual tensor R (v,v,o,o); all work is enqueued on the context's stream."""
     v, _, o, _ = T.extents
     if R is None:
-        R = ctx.tensor_create((v, v, o, o))
-    X = ctx.tensor_create((v, v, o, o))
+        R = ctx.tensor_create((v, v, o, o), zero=False)
+    X = ctx.tensor_create((v, v, o, o), zero=False)          # every intermediate below is first written by an '=' call
     ctx.add("R(a,b,i,j)=W(a,b,i,j)", R, B["vvoo"], 1.0)
     ctx.contract("X(a,b,i,j)=T(a,c,i,j)*f(b,c)", X, T, B["fvv"], 1.0)
     ctx.antisymmetrize("P(ab):R(a,b,i,j)+=X(a,b,i,j)", R, X, 1.0)
     ctx.contract("X(a,b,i,j)=T(a,b,i,k)*f(k,j)", X, T, B["foo"], 1.0)
     ctx.antisymmetrize("P(ij):R(a,b,i,j)+=X(a,b,i,j)", R, X, -1.0)
-    I1 = ctx.tensor_create((o, o, o, o))
+    I1 = ctx.tensor_create((o, o, o, o), zero=False)
     ctx.add("I1(k,l,i,j)=W(k,l,i,j)", I1, B["oooo"], 1.0)
     ctx.contract("I1(k,l,i,j)+=W(k,l,c,d)*T(c,d,i,j)", I1, B["oovv"], T, 0.5)
     ctx.contract("R(a,b,i,j)+=T(a,b,k,l)*I1(k,l,i,j)", R, T, I1, 0.5)
     I1.destroy()
     ctx.contract("R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)", R, B["vvvv"], T, 0.5)
-    I2 = ctx.tensor_create((o, v, v, o))
+    I2 = ctx.tensor_create((o, v, v, o), zero=False)
     ctx.add("I2(k,b,c,j)=W(k,b,c,j)", I2, B["ovvo"], 1.0)
     ctx.contract("I2(k,b,c,j)+=W(k,l,c,d)*T(b,d,j,l)", I2, B["oovv"], T, 0.5)
     ctx.contract("X(a,b,i,j)=T(a,c,i,k)*I2(k,b,c,j)", X, T, I2, 1.0)
     I2.destroy()
     ctx.antisymmetrize("P(ij)P(ab):R(a,b,i,j)+=X(a,b,i,j)", R, X, 1.0)
-    I3 = ctx.tensor_create((o, o))
+    I3 = ctx.tensor_create((o, o), zero=False)
     ctx.contract("I3(l,i)=W(k,l,c,d)*T(d,c,i,k)", I3, B["oovv"], T, 1.0)
     ctx.contract("X(a,b,i,j)=T(a,b,l,j)*I3(l,i)", X, T, I3, 1.0)
     I3.destroy()
     ctx.antisymmetrize("P(ij):R(a,b,i,j)+=X(a,b,i,j)", R, X, -0.5)
-    I4 = ctx.tensor_create((v, v))
+    I4 = ctx.tensor_create((v, v), zero=False)
     ctx.contract("I4(a,d)=W(k,l,c,d)*T(a,c,l,k)", I4, B["oovv"], T, 1.0)
     ctx.contract("X(a,b,i,j)=I4(a,d)*T(d,b,i,j)", X, I4, T, 1.0)
     I4.destroy()
@@ -77,7 +77,7 @@ def ccsd_residual(ctx, B, T1, T2, R1=None, R2=None):
     T1 (v,o) = t_i^a, T2 (v,v,o,o) = t_ij^ab.  Returns (E rank-0 tensor, R1, R2).  Equations: DESIGN.md / oracle/cc.py
     `ccsd_residual_unfactorised` (pinned to PAPER Eq. (3) on the Fock space)."""
     v, o = T1.extents
-    new = ctx.tensor_create
+    new = lambda shape: ctx.tensor_create(shape, zero=False)      # every tensor below is first written by an '=' call
     con, add, asym = ctx.contract, ctx.add, ctx.antisymmetrize
 
     def copy(src, shape, label):
@@ -202,7 +202,7 @@ def triples_correction(ctx, W, U, T2, e_occ, e_virt, keep=False, T1=None, oovv=N
     import numpy as np
     v, _, o, _ = T2.extents
     shape = (v, v, v, o, o, o)
-    X, R3 = ctx.tensor_create(shape), ctx.tensor_create(shape)
+    X, R3 = ctx.tensor_create(shape, zero=False), ctx.tensor_create(shape, zero=False)    # both first written by '='
     ctx.contract("X(a,b,c,i,j,k)=W(b,c,d,k)*T(a,d,i,j)", X, W, T2, 1.0)
     ctx.antisymmetrize("P(a/bc)P(k/ij):R(a,b,c,i,j,k)=X(a,b,c,i,j,k)", R3, X, 1.0)
     ctx.contract("X(a,b,c,i,j,k)=T(a,b,i,l)*U(l,c,j,k)", X, T2, U, 1.0)

@@ -345,7 +345,8 @@ int tcb_sync(tcb_ctx *ctx)
 
 // ---- tensors ---------------------------------------------------------------------------------------------
 
-static int make_tensor(tcb_ctx *ctx, tcb_tensor **out, int rank, const int64_t *extents, void *borrowed)
+static int make_tensor(tcb_ctx *ctx, tcb_tensor **out, int rank, const int64_t *extents, void *borrowed,
+                       bool zero = true)
 {
     if (!out) return TCB_EINVAL;
     *out = nullptr;
@@ -374,7 +375,7 @@ static int make_tensor(tcb_ctx *ctx, tcb_tensor **out, int rank, const int64_t *
         }
         t->ptr = p;
         t->owns = true;
-        TCB_CUDA(ctx, cudaMemsetAsync(p, 0, bytes, ctx->stream));
+        if (zero) TCB_CUDA(ctx, cudaMemsetAsync(p, 0, bytes, ctx->stream));
     }
     ++ctx->live_tensors;
     *out = t.release();
@@ -384,6 +385,11 @@ static int make_tensor(tcb_ctx *ctx, tcb_tensor **out, int rank, const int64_t *
 int tcb_tensor_create(tcb_ctx *ctx, tcb_tensor **t, int rank, const int64_t *extents)
 {
     return make_tensor(ctx, t, rank, extents, nullptr);
+}
+
+int tcb_tensor_alloc(tcb_ctx *ctx, tcb_tensor **t, int rank, const int64_t *extents)
+{
+    return make_tensor(ctx, t, rank, extents, nullptr, false);
 }
 
 int tcb_tensor_wrap(tcb_ctx *ctx, tcb_tensor **t, int rank, const int64_t *extents, void *device_ptr)
