@@ -251,7 +251,7 @@ def run_ours(args, rank, world, local_rank):
         "vs_baseline": None, "dtype": "complex128 (f64)", "data": "synthetic",
         "config": {"workload": WORKLOAD, "o": O, "v": V, "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "l2": "inputs larger than L2 (vvvv 655 MB, working set 0.9 GB vs 126 MB L2), no flush",
-                   "calls_per_step": "11 tcb_contract + 6 tcb_antisymmetrize + 3 tcb_add"},
+                   "calls_per_step": "11 tcb_contract + 5 tcb_antisymmetrize + 3 tcb_add"},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "GFLOP/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_ms / e2e_steps, "steps": e2e_steps, "residual_norm": r_norm,
@@ -495,7 +495,7 @@ def run_extras(ctx):
         E.destroy()
         classes = {k: ctx.kernel_stats(k) for k in ("zgemm", "permute", "permsum", "elementwise")}
         ctx.set_option("kernel_timing", "off")
-        out.append({"workload": "CCSD residual (R1, R2, E) o=30 v=150: 35 contractions + 11 permute-sums + 12 adds, "
+        out.append({"workload": "CCSD residual (R1, R2, E) o=30 v=150: 35 contractions + 9 permute-sums + 12 adds, "
                                 "vvvv and Wabef 8.1 GB each",
                     "ms": b, "ms_median": float(np.median(ts)), "contractions": Counting.calls, "launches": launches,
                     "tflops": Counting.flops / b * 1e-9,

@@ -72,7 +72,7 @@ CCSD_BLOCKS = ("vvoo", "oovv", "oooo", "vvvv", "ovvo", "ooov", "ovvv", "vovv", "
 
 def ccsd_residual(ctx, B, T1, T2, R1=None, R2=None):
     """Spin-orbital CCSD residuals (the paper's benchmark iteration) as the binary tensor operations a
-    generated driver issues: 35 contractions, 11 permute-sums, 12 adds; intermediates are created and destroyed around
+    generated driver issues: 35 contractions, 9 permute-sums, 12 adds; intermediates are created and destroyed around
     their use (PAPER.md:212).  B: dict of device tensors `CCSD_BLOCKS` (<pq||rs> blocks in bra-ket order, f blocks);
     T1 (v,o) = t_i^a, T2 (v,v,o,o) = t_ij^ab.  Returns (E rank-0 tensor, R1, R2).  Equations: DESIGN.md / oracle/cc.py
     `ccsd_residual_unfactorised` (pinned to PAPER Eq. (3) on the Fock space)."""

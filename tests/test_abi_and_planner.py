@@ -140,3 +140,69 @@ def test_extent_one_indices_are_dropped_and_labels_may_be_long():
     assert (p["M"], p["N"], p["K"]) == (630, 3, 40) and p["route"] == "gemm" and p["permute_A"]
     p = plan("R(p1,x,h1)+=T(p1,y,h1,e_1)*F(e_1,x,y)", (70, 1, 9), (70, 1, 9, 40), (40, 1, 1))
     assert (p["M"], p["N"], p["K"]) == (630, 1, 40) and not p["permute_A"] and p["A_layout"] == "M-major"
+
+
+class _RecordingContext:
+    """Duck-typed stand-in for Context: records the library calls a driver of ccd.py issues (no device, no arithmetic)."""
+
+    class _T:
+        def __init__(self, extents):
+            self.extents = tuple(int(e) for e in extents)
+
+        def destroy(self):
+            pass
+
+    def __init__(self):
+        self.contractions, self.antisym, self.adds, self.other = [], [], [], []
+
+    def tensor_create(self, extents, zero=True):
+        return self._T(extents)
+
+    def contract(self, expr, D, L, R, alpha=1.0):
+        self.contractions.append((expr, D.extents, L.extents, R.extents))
+
+    def antisymmetrize(self, spec, D, X, alpha=1.0):
+        assert D.extents == X.extents
+        self.antisym.append(spec)
+
+    def add(self, expr, D, L, alpha=1.0):
+        self.adds.append(expr)
+
+    def denominator_divide(self, T, R, eps, alpha=1.0):
+        assert T.extents == R.extents and len(eps) == len(T.extents)
+        self.other.append("divide")
+
+    def dot(self, D, X, Y, conj=True, alpha=1.0):
+        assert D.extents == () and X.extents == Y.extents
+        self.other.append("dot")
+
+
+def test_every_contraction_of_the_driver_programs_is_planned_on_the_host():
+    """The CCD, CCSD and (T) programs of ccd.py, replayed against a recording context: every contraction string goes
+    through the host planner (tcb_plan_describe_host, no device) with the shapes the program gives it; the counts are the
+    documented ones and the big operands are never permuted."""
+    from paper_2409_06759_b200 import ccd
+    o, v = 6, 14
+    ext = lambda name: tuple(o if c == "o" else v for c in name)
+    rec = _RecordingContext()
+    B = {k: rec._T(ext(k[-2:]) if k[0] == "f" else ext(k)) for k in ccd.CCSD_BLOCKS}
+    T1, T2 = rec._T((v, o)), rec._T((v, v, o, o))
+    ccd.ccd_residual(rec, B, T2)
+    n_ccd = len(rec.contractions)
+    assert (n_ccd, len(rec.antisym), len(rec.adds)) == (11, 5, 3)
+    ccd.ccsd_residual(rec, B, T1, T2)
+    assert len(rec.contractions) - n_ccd == 35 and len(rec.antisym) - 5 == 9
+    n_before = len(rec.contractions)
+    ccd.triples_correction(rec, rec._T((v, v, v, o)), rec._T((o, v, o, o)), T2, [0.0] * o, [0.0] * v,
+                           T1=T1, oovv=B["oovv"])
+    assert len(rec.contractions) - n_before == 3 and rec.other == ["divide", "dot", "dot"]
+    routes = {}
+    for expr, d, l, r in rec.contractions:
+        p = plan(expr, d, l, r)
+        flops = 8.0 * p["M"] * p["N"] * p["K"]
+        assert abs(p["flops"] - flops) <= 1e-5 * flops          # the description prints six significant digits
+        routes[p["route"]] = routes.get(p["route"], 0) + 1
+        big = max(np.prod(l), np.prod(r))
+        if np.prod(l) == big and big >= v ** 4:
+            assert not p["permute_A" if p["row_operand"] == "L" else "permute_B"], expr     # vvvv-sized operands in place
+    assert routes.get("gemv", 0) >= 6 and routes.get("gemm", 0) >= 35

@@ -135,7 +135,7 @@ def test_ccd_jacobi_iterations_follow_the_oracle(ctx):
 
 @pytest.mark.parametrize("o,v", [(3, 4), (5, 11)])
 def test_ccsd_residual_program(ctx, o, v):
-    """The CCSD residuals (singles, doubles, energy) as ~60 ABI calls against the oracle's program of the same binary
+    """The CCSD residuals (singles, doubles, energy) as 56 ABI calls against the oracle's program of the same binary
     operations; at (3,4) also against the unfactorised tier (itself pinned to the Fock space)."""
     n = o + v
     rng = np.random.default_rng(o * 100 + v)
