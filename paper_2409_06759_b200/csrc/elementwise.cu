@@ -224,7 +224,10 @@ cudaError_t launch_denominator_update(void *T, const void *R, int rank, const in
             p.ninner = k + 1;
         }
     }
-    if (p.ninner == 0) { p.ninner = rank; slab = n; }       // rank 0 never gets here (no energies); keeps the kernel total
+    if (p.ninner == 0) {                                    // a leading extent above 2^30 (rank 0 never gets here)
+        if (n > (1LL << 31)) return cudaErrorInvalidValue;
+        p.ninner = rank; slab = n;
+    }
     p.slab = (unsigned)slab;
     p.nslabs = n / slab;
     p.eps = eps_dev;
