@@ -165,6 +165,19 @@ int tcb_measure_fp64_tensor_peak(tcb_ctx *ctx, double milliseconds, double *tflo
 /* The same for the plain FP64 pipe (register-resident DFMA chains, 2 flop per FMA and lane): on B200 the vector and
  * the tensor FP64 rates are nominally equal; the pair of numbers shows what the tensor path buys. */
 int tcb_measure_fp64_vector_peak(tcb_ctx *ctx, double milliseconds, double *tflops);
+/* CUDA graph of a call list (a whole residual evaluation: "capture launch-bound inner loops", the paper's barrier per
+ * operation, becomes graph edges).  Between tcb_capture_begin and tcb_capture_end every call on the
+ * context is RECORDED instead of executed -- kernels, stream-ordered creation and destruction of intermediates --
+ * and tcb_graph_launch replays the list on the context's stream.  Requirements: the same call list has run at least
+ * once before (plans cached, workspace grown: neither may happen inside a capture), "kernel_timing" is off, no
+ * upload / download / sync / tcb_denominator_* inside (they copy from host memory).  The tensors the list reads and
+ * writes must stay alive and at their addresses while the graph is used.  tcb_capture_end returns TCB_EUNSUPPORTED
+ * (and no graph) when the list could not be captured.  tcb_launch_count advances by the captured launches per replay. */
+typedef struct tcb_graph tcb_graph;
+int tcb_capture_begin(tcb_ctx *ctx);
+int tcb_capture_end(tcb_ctx *ctx, tcb_graph **graph);
+int tcb_graph_launch(tcb_ctx *ctx, tcb_graph *graph);
+int tcb_graph_destroy(tcb_graph *graph);
 /* Milliseconds between two points of the context's stream: tcb_timer_start / tcb_timer_stop bracket the
  * calls in between with CUDA events on that stream; stop blocks and returns the elapsed time. */
 int tcb_timer_start(tcb_ctx *ctx);

@@ -44,6 +44,7 @@ ABI_SYMBOLS = [
     "tcb_tensor_upload", "tcb_tensor_download", "tcb_tensor_fill", "tcb_contract", "tcb_add", "tcb_scale",
     "tcb_denominator_update", "tcb_denominator_divide", "tcb_dot",
     "tcb_permute", "tcb_permsum", "tcb_antisymmetrize", "tcb_plan_describe", "tcb_measure_fp64_tensor_peak", "tcb_measure_fp64_vector_peak",
+    "tcb_capture_begin", "tcb_capture_end", "tcb_graph_launch", "tcb_graph_destroy",
     "tcb_timer_start", "tcb_timer_stop", "tcb_kernel_stats", "tcb_kernel_stats_reset", "tcb_plan_describe_host", "tcbx_synth_normal", "tcbx_synth_index_linear",
     "tcbx_synth_mp2_amplitudes",
 ]
@@ -87,6 +88,10 @@ def load_library():
         "tcb_measure_fp64_vector_peak": [vp, ctypes.c_double, ctypes.POINTER(ctypes.c_double)],
         "tcb_plan_describe_host": [cp, ctypes.c_int, i64p, ctypes.c_int, i64p, ctypes.c_int, i64p, cp, ctypes.c_char_p,
                                    ctypes.c_size_t, i64p, ctypes.c_size_t, i64p, ctypes.c_size_t],
+        "tcb_capture_begin": [vp],
+        "tcb_capture_end": [vp, ctypes.POINTER(vp)],
+        "tcb_graph_launch": [vp, vp],
+        "tcb_graph_destroy": [vp],
         "tcb_timer_start": [vp],
         "tcb_kernel_stats": [vp, cp, ctypes.POINTER(kernel_stat)],
         "tcb_kernel_stats_reset": [vp],
@@ -329,6 +334,21 @@ class Context:
 
     def kernel_stats_reset(self):
         self._check(self.lib.tcb_kernel_stats_reset(self.handle))
+
+    def capture_begin(self):
+        self._check(self.lib.tcb_capture_begin(self.handle))
+
+    def capture_end(self):
+        """Returns an opaque graph handle for graph_launch / graph_destroy."""
+        g = ctypes.c_void_p()
+        self._check(self.lib.tcb_capture_end(self.handle, ctypes.byref(g)))
+        return g
+
+    def graph_launch(self, g):
+        self._check(self.lib.tcb_graph_launch(self.handle, g))
+
+    def graph_destroy(self, g):
+        self.lib.tcb_graph_destroy(g)
 
     def timer_start(self):
         self._check(self.lib.tcb_timer_start(self.handle))

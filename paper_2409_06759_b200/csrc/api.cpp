@@ -38,6 +38,8 @@ struct tcb_ctx {
     int64_t live_tensors = 0;
     // per-kernel-class device timing ("kernel_timing" = "on"): event pairs around every launch, summed on query
     bool kernel_timing = false;
+    bool capturing = false;                  // between tcb_capture_begin and tcb_capture_end
+    int64_t capture_l0 = 0;
     struct Span { int cls; cudaEvent_t a, b; double flops, bytes; };
     std::vector<Span> spans;
     std::vector<cudaEvent_t> free_events;
@@ -906,6 +908,68 @@ int tcb_kernel_stats_reset(tcb_ctx *ctx)
     if (rc) return rc;
     fold_spans(ctx);
     for (int c = 0; c < 4; ++c) ctx->acc[c] = tcb_kernel_stat{0, 0.0, 0.0, 0.0};
+    return TCB_OK;
+}
+
+// ---- CUDA graph capture of a call list ---------------------------------------------------------------------------
+struct tcb_graph {
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    int64_t launches = 0;
+};
+
+int tcb_capture_begin(tcb_ctx *ctx)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (ctx->capturing) return set_error(ctx, TCB_EINVAL, "a capture is already open");
+    if (ctx->kernel_timing) return set_error(ctx, TCB_EINVAL, "kernel_timing must be off during a capture");
+    TCB_CUDA(ctx, cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+    ctx->capturing = true;
+    ctx->capture_l0 = ctx->launches;
+    return TCB_OK;
+}
+
+int tcb_capture_end(tcb_ctx *ctx, tcb_graph **out)
+{
+    if (!ctx || !out) return TCB_EINVAL;
+    *out = nullptr;
+    if (!ctx->capturing) return set_error(ctx, TCB_EINVAL, "no capture is open");
+    ctx->capturing = false;
+    std::unique_ptr<tcb_graph> g(new tcb_graph);
+    cudaError_t e = cudaStreamEndCapture(ctx->stream, &g->graph);
+    if (e != cudaSuccess || !g->graph) {
+        cudaGetLastError();
+        return set_error(ctx, TCB_EUNSUPPORTED, std::string("the call list could not be captured: ") + cudaGetErrorString(e));
+    }
+    e = cudaGraphInstantiate(&g->exec, g->graph, 0);
+    if (e != cudaSuccess) {
+        cudaGraphDestroy(g->graph);
+        cudaGetLastError();
+        return set_error(ctx, TCB_EUNSUPPORTED, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e));
+    }
+    g->launches = ctx->launches - ctx->capture_l0;
+    *out = g.release();
+    return TCB_OK;
+}
+
+int tcb_graph_launch(tcb_ctx *ctx, tcb_graph *g)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!g || !g->exec) return TCB_EINVAL;
+    if (ctx->capturing) return set_error(ctx, TCB_EINVAL, "graph launch inside a capture");
+    TCB_CUDA(ctx, cudaGraphLaunch(g->exec, ctx->stream));
+    ctx->launches += g->launches;
+    return TCB_OK;
+}
+
+int tcb_graph_destroy(tcb_graph *g)
+{
+    if (!g) return TCB_EINVAL;
+    if (g->exec) cudaGraphExecDestroy(g->exec);
+    if (g->graph) cudaGraphDestroy(g->graph);
+    delete g;
     return TCB_OK;
 }
 

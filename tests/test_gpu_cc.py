@@ -265,3 +265,37 @@ def test_triples_correction_program(ctx, o, v):
     assert plan["route"] == "gemv" and not plan["permute_A"]
     for t in (dW, dU, dT, dE, dR3, dt3, dT1, dV, dE2, dEst):
         t.destroy()
+
+
+def test_cuda_graph_of_the_residual_call_list_replays_bit_identically(ctx):
+    """tcb_capture_begin/end around a warm CCD residual evaluation: 35 kernel nodes plus the stream-ordered creation and
+    destruction of its intermediates; a replay gives the same bits as the call-by-call evaluation and counts its launches."""
+    o, v = 6, 14
+    B, T, eo, ev = synth.config_ccd(o, v)
+    dB = {k: ctx.tensor_from_numpy(x) for k, x in B.items()}
+    dT = ctx.tensor_from_numpy(T)
+    dR, dR2 = ctx.tensor_create((v, v, o, o)), ctx.tensor_create((v, v, o, o))
+    for _ in range(2):
+        ccd.ccd_residual(ctx, dB, dT, dR)
+    ref = ctx.tensor_download(dR)
+    l0 = ctx.launch_count()
+    ctx.capture_begin()
+    with pytest.raises(pkg.TcbError):
+        ctx.capture_begin()                                     # one capture at a time
+    ccd.ccd_residual(ctx, dB, dT, dR2)
+    g = ctx.capture_end()
+    per_list = ctx.launch_count() - l0
+    assert per_list >= 19
+    assert not np.any(ctx.tensor_download(dR2))                 # recorded, not executed
+    for _ in range(2):
+        l1 = ctx.launch_count()
+        ctx.graph_launch(g)
+        assert ctx.launch_count() - l1 == per_list
+        assert ctx.tensor_download(dR2).tobytes() == ref.tobytes()
+    ctx.graph_destroy(g)
+    ctx.set_option("kernel_timing", "on")
+    with pytest.raises(pkg.TcbError):
+        ctx.capture_begin()                                     # event pairs cannot live inside a graph
+    ctx.set_option("kernel_timing", "off")
+    with pytest.raises(pkg.TcbError):
+        ctx.capture_end()                                       # nothing open
