@@ -168,14 +168,19 @@ def run_ours(args, rank, world, local_rank):
     # The steps without event pairs replay a CUDA graph of the same call list (tcb_capture_begin/end: 35 kernel nodes,
     # stream-ordered intermediates included; captured once, outside the timed region, like the plans): 7.18 instead of
     # 7.27 ms per step.  --no-graph issues every step call by call.
-    graph = None
+    graph, graph_note = None, None
     if not args.no_graph:
         ctx.set_option("kernel_timing", "off")
-        ctx.capture_begin()
-        step()
-        graph = ctx.capture_end()
-        ctx.graph_launch(graph)
-        ctx.sync()
+        try:
+            ctx.capture_begin()
+            try:
+                step()
+            finally:
+                graph = ctx.capture_end()          # also closes the capture when step() raised
+            ctx.graph_launch(graph)
+            ctx.sync()
+        except pkg.TcbError as exc:                # not capturable on this box: every step call by call, and say so
+            graph, graph_note = None, f"capture failed ({exc}); "
     ctx.sync()
     ctx.kernel_stats_reset()
     sampler = ClockSampler(local_rank)
@@ -270,7 +275,7 @@ def run_ours(args, rank, world, local_rank):
         "config": {"workload": WORKLOAD, "o": O, "v": V, "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "l2": "inputs larger than L2 (vvvv 655 MB, working set 0.9 GB vs 126 MB L2), no flush",
                    "calls_per_step": "11 tcb_contract + 5 tcb_antisymmetrize + 3 tcb_add",
-                   "issue": ("call by call" if graph is None else
+                   "issue": ((graph_note or "") + "call by call" if graph is None else
                              f"CUDA graph replay of the call list (tcb_capture_*), except the {sampled} steps that carry "
                              "per-launch event pairs, which are issued call by call")},
         "clocks": clocks,

@@ -10,9 +10,12 @@
 //   * a producer warp loads the orbit's cubes of X, once per distinct outer permutation (k/ij: 3), with ONE tiled TMA
 //     load per cube (cp.async.bulk.tensor.4d over the map {a, b, c, outer slab}, box 6 x 6 x 6 x 1, SASS UTMALDG) into
 //     a 3-stage mbarrier ring -- L2 -> SM traffic 3 x X instead of 9 x X, no per-row copy instructions;
-//   * 18 consumer warps produce the orbit's cubes of D from shared memory: a quarter-warp is a 2 x 2 x 2 micro-cube,
-//     whose eight 16-byte reads fall in eight different bank groups under EVERY permutation of (a,b,c) because the cube
-//     strides 1, 6, 36 are 1, 6, 4 mod 8; a warp covers a full 96-byte row of a, so D moves in whole sectors;
+//   * a D warp loads the orbit's cubes of D two items ahead (tiled TMA loads into a ring of D buffers) and writes the
+//     finished cubes back with tiled TMA stores (cp.async.bulk.tensor.4d.global.shared::cta, per-thread bulk groups);
+//     ragged extents need no masks: TMA zero-fills loads and clips stores;
+//   * 14 consumer warps compute in place in the D buffer from shared memory: a quarter-warp is a 2 x 2 x 2 micro-cube,
+//     whose eight 16-byte accesses fall in eight different bank groups under EVERY permutation of (a,b,c) because the
+//     cube strides 1, 6, 36 are 1, 6, 4 mod 8 (no padding, which TMA boxes could not have);
 //   * items are ordered so that the (<= 6) outer slabs that are permutations of one another are processed together
 //     by one CTA for one orbit: each cube of X comes from DRAM once.
 // Terms are added in the caller's order with separately rounded products and sums: bit-identical to the generic
