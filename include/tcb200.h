@@ -68,14 +68,34 @@ typedef struct { double re, im; } tcb_c128;
  * split-K partials (0 = grow on demand; growth synchronises the stream). */
 int tcb_ctx_create(tcb_ctx **ctx, int device, void *cuda_stream, size_t workspace_bytes);
 int tcb_ctx_destroy(tcb_ctx *ctx);
-/* keys: "splitk" = "auto" | "off" | <integer number of splits>;  "epilogue" = "auto" | "fused" | "twopass";
- *       "permute_operands" = "auto" | "always"  (A/B testing of plans);  "gemm_deal" = "dynamic" | "static"
- *       (how the GEMM's tiles and stream-K chunks reach the CTAs: claimed from a counter, or dealt round-robin;
- *       the result is the same bit for bit);  "kernel_timing" = "on" | "off" (see tcb_kernel_stats);
- *       unknown key -> TCB_EINVAL. */
+/* keys: "splitk" = "auto" | "off" | <integer number of splits>;
+ *       "epilogue" = "auto" | "fused" (alpha*C scattered into D's index order by the GEMM epilogue: no third TTGT pass)
+ *                  | "twopass" (PAPER.md:91 literally: the GEMM writes a plain M x N matrix into workspace, a
+ *                    permute-accumulate pass brings it into D; kept for A/B tests, "auto" never picks it);
+ *       "operand_loads" = "auto" (cost model: per operand the cheapest of reading it in place by TMA, reading it in place
+ *                    through offset tables, or permuting it into workspace first) | "gather" (never permute) | "permute"
+ *                    (never gather: TTGT as in PAPER.md:88-89);
+ *       "permute_operands" = "auto" | "always"  (A/B testing of plans: both operands always permuted);
+ *       "gemm_deal" = "dynamic" | "static" (how the GEMM's tiles and stream-K chunks reach the CTAs: claimed from a counter,
+ *                    or dealt round-robin; the result is the same bit for bit);
+ *       "kernel_timing" = "on" | "off" (see tcb_kernel_stats);   unknown key -> TCB_EINVAL. */
 int tcb_ctx_set_option(tcb_ctx *ctx, const char *key, const char *value);
-/* Blocks until everything enqueued so far has finished (the paper's barrier). */
+/* Blocks until everything enqueued so far -- on every lane -- has finished (the paper's barrier). */
 int tcb_sync(tcb_ctx *ctx);
+/* Lanes: concurrency between independent contractions.  Generated code puts a barrier after every tensor
+ * operation, which the paper measures as its serial fraction; DLTC-style layering lets
+ * operations without a data dependence run side by side.  A context has tcb_lane_count() lanes; each is a stream with its
+ * own workspace.  Lane 0 is the context's stream and the default.
+ *   tcb_lane_set(ctx, l)      : every following call (tensor creation and destruction included) is enqueued on lane l;
+ *   tcb_lane_wait(ctx, l, m)  : what is enqueued on lane l from now on starts after everything enqueued on lane m so far.
+ * Calls on ONE lane execute in issue order; calls on different lanes are unordered unless a tcb_lane_wait orders them --
+ * that is the caller's statement that they are independent (no output of one is an operand or output of the other, and a
+ * tensor is destroyed on a lane that has waited for its last user).  Inside tcb_capture_begin/end the lanes become
+ * parallel branches of the graph: a lane joins the capture at its first use there (it then starts after what lane 0 held
+ * at that point) and is joined back into lane 0 by tcb_capture_end.  Errors: TCB_EINVAL (lane out of range), TCB_ECUDA. */
+int tcb_lane_count(void);
+int tcb_lane_set(tcb_ctx *ctx, int lane);
+int tcb_lane_wait(tcb_ctx *ctx, int lane, int on_lane);
 /* Text of the last error recorded on this context (valid until the next call on it). */
 const char *tcb_last_error(const tcb_ctx *ctx);
 const char *tcb_strerror(int code);
@@ -168,15 +188,21 @@ int tcb_measure_fp64_vector_peak(tcb_ctx *ctx, double milliseconds, double *tflo
 /* CUDA graph of a call list (a whole residual evaluation: "capture launch-bound inner loops", the paper's barrier per
  * operation, becomes graph edges).  Between tcb_capture_begin and tcb_capture_end every call on the
  * context is RECORDED instead of executed -- kernels, stream-ordered creation and destruction of intermediates --
- * and tcb_graph_launch replays the list on the context's stream.  Requirements: the same call list has run at least
- * once before (plans cached, workspace grown: neither may happen inside a capture), "kernel_timing" is off, no
- * upload / download / sync / tcb_denominator_* inside (they copy from host memory).  The tensors the list reads and
- * writes must stay alive and at their addresses while the graph is used.  tcb_capture_end returns TCB_EUNSUPPORTED
- * (and no graph) when the list could not be captured.  tcb_launch_count advances by the captured launches per replay. */
+ * and tcb_graph_launch replays the list on the context's stream (lane 0; calls issued on other lanes inside the capture
+ * become parallel branches).  Requirements: the same call list has run at least once before (plans cached, workspace
+ * grown, lanes created: none of it may happen inside a capture), "kernel_timing" is off, no upload / download / sync /
+ * tcb_denominator_* inside (they copy from host memory).  A call that breaks a requirement returns TCB_EUNSUPPORTED
+ * WITHOUT touching the device, the context stays usable, and tcb_capture_end then returns TCB_EUNSUPPORTED and no graph:
+ * issue the list call by call instead.  The tensors the list reads and writes must stay alive and at their addresses
+ * while the graph is used; so must the context's workspace: tcb_graph_launch returns TCB_EINVAL when a later call has
+ * made the workspace grow (its old block, whose address the graph carries, is gone) -- capture again.
+ * tcb_launch_count advances by the captured launches per replay.  tcb_graph_info: nodes and dependency edges of the
+ * graph (a chain has edges = nodes - 1; parallel branches show as more) and the kernel launches per replay. */
 typedef struct tcb_graph tcb_graph;
 int tcb_capture_begin(tcb_ctx *ctx);
 int tcb_capture_end(tcb_ctx *ctx, tcb_graph **graph);
 int tcb_graph_launch(tcb_ctx *ctx, tcb_graph *graph);
+int tcb_graph_info(const tcb_graph *graph, int64_t *nodes, int64_t *edges, int64_t *kernel_launches);
 int tcb_graph_destroy(tcb_graph *graph);
 /* Milliseconds between two points of the context's stream: tcb_timer_start / tcb_timer_stop bracket the
  * calls in between with CUDA events on that stream; stop blocks and returns the elapsed time. */

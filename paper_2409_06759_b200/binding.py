@@ -44,7 +44,8 @@ ABI_SYMBOLS = [
     "tcb_tensor_upload", "tcb_tensor_download", "tcb_tensor_fill", "tcb_contract", "tcb_add", "tcb_scale",
     "tcb_denominator_update", "tcb_denominator_divide", "tcb_dot",
     "tcb_permute", "tcb_permsum", "tcb_antisymmetrize", "tcb_plan_describe", "tcb_measure_fp64_tensor_peak", "tcb_measure_fp64_vector_peak",
-    "tcb_capture_begin", "tcb_capture_end", "tcb_graph_launch", "tcb_graph_destroy",
+    "tcb_capture_begin", "tcb_capture_end", "tcb_graph_launch", "tcb_graph_info", "tcb_graph_destroy",
+    "tcb_lane_count", "tcb_lane_set", "tcb_lane_wait",
     "tcb_timer_start", "tcb_timer_stop", "tcb_kernel_stats", "tcb_kernel_stats_reset", "tcb_plan_describe_host", "tcbx_synth_normal", "tcbx_synth_index_linear",
     "tcbx_synth_mp2_amplitudes",
 ]
@@ -92,6 +93,10 @@ def load_library():
         "tcb_capture_end": [vp, ctypes.POINTER(vp)],
         "tcb_graph_launch": [vp, vp],
         "tcb_graph_destroy": [vp],
+        "tcb_graph_info": [vp, i64p, i64p, i64p],
+        "tcb_lane_count": [],
+        "tcb_lane_set": [vp, ctypes.c_int],
+        "tcb_lane_wait": [vp, ctypes.c_int, ctypes.c_int],
         "tcb_timer_start": [vp],
         "tcb_kernel_stats": [vp, cp, ctypes.POINTER(kernel_stat)],
         "tcb_kernel_stats_reset": [vp],
@@ -346,6 +351,21 @@ class Context:
 
     def graph_launch(self, g):
         self._check(self.lib.tcb_graph_launch(self.handle, g))
+
+    def graph_info(self, g):
+        """{'nodes', 'edges', 'launches'} of a captured graph"""
+        n, e, k = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
+        self._check(self.lib.tcb_graph_info(g, ctypes.byref(n), ctypes.byref(e), ctypes.byref(k)))
+        return {"nodes": n.value, "edges": e.value, "launches": k.value}
+
+    def lane_count(self):
+        return int(self.lib.tcb_lane_count())
+
+    def lane_set(self, lane):
+        self._check(self.lib.tcb_lane_set(self.handle, int(lane)))
+
+    def lane_wait(self, lane, on_lane):
+        self._check(self.lib.tcb_lane_wait(self.handle, int(lane), int(on_lane)))
 
     def graph_destroy(self, g):
         self.lib.tcb_graph_destroy(g)

@@ -4,7 +4,9 @@
 #include "../../include/tcb200.h"
 
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
 
+#include <algorithm>
 #include <cstdio>
 #include <cstring>
 #include <map>
@@ -20,15 +22,31 @@ using namespace tcb;
 
 struct CachedPlan {
     ContractPlan plan;
-    int64_t *d_tables = nullptr;   // device: offM[M] followed by offN[N]
+    int64_t *d_tables = nullptr;   // device: offM[M], offN[N], then the GEMV tables or the gather tables of A and B
+    const int64_t *d_aux[4] = {nullptr, nullptr, nullptr, nullptr};   // gemv: offAm, offAk, offBk; gemm: gather row/k of A, of B
+    // the two TMA descriptors of the GEMM, valid for operands at map_a / map_b (re-encoded when a pointer changes)
+    GemmTensorMaps maps;
+    const void *map_a = nullptr, *map_b = nullptr;
+    bool maps_valid = false;
 };
 
-struct tcb_ctx {
-    int device = 0;
+// A lane = one stream with its own workspace (permuted operands, split-K partials, the GEMM's work counters).  Lane 0 is the
+// context's stream; independent branches of a call list go to other lanes (tcb_lane_set / tcb_lane_wait).
+constexpr int kMaxLanes = 4;
+struct Lane {
     cudaStream_t stream = nullptr;
     bool owns_stream = false;
     void *ws = nullptr;
     size_t ws_bytes = 0;
+    cudaEvent_t ev = nullptr;        // records "everything enqueued on this lane so far" for tcb_lane_wait
+    bool in_capture = false;         // forked into the open capture
+};
+
+struct tcb_ctx {
+    int device = 0;
+    Lane lanes[kMaxLanes];
+    int cur = 0;                     // the lane calls are enqueued on
+    uint64_t ws_generation = 0;      // bumped whenever a workspace block is reallocated (captured graphs bake addresses in)
     std::string last_error;
     bool sticky_cuda = false;
     int64_t launches = 0;
@@ -39,6 +57,7 @@ struct tcb_ctx {
     // per-kernel-class device timing ("kernel_timing" = "on"): event pairs around every launch, summed on query
     bool kernel_timing = false;
     bool capturing = false;                  // between tcb_capture_begin and tcb_capture_end
+    bool capture_failed = false;             // a call inside the capture was refused: tcb_capture_end returns no graph
     int64_t capture_l0 = 0;
     struct Span { int cls; cudaEvent_t a, b; double flops, bytes; };
     std::vector<Span> spans;
@@ -64,14 +83,49 @@ int set_error(tcb_ctx *ctx, int code, const std::string &msg)
     return code;
 }
 
+inline cudaStream_t cur_stream(tcb_ctx *ctx) { return ctx->lanes[ctx->cur].stream; }
+
+bool is_capture_error(cudaError_t e)
+{
+    return e >= cudaErrorStreamCaptureUnsupported && e <= cudaErrorStreamCaptureWrongThread;
+}
+
 int cuda_fail(tcb_ctx *ctx, cudaError_t e, const char *where)
 {
+    if (e == cudaErrorNotSupported) {
+        // a launcher refused a shape it cannot tile: decided on the host before anything was enqueued; the context lives on
+        cudaGetLastError();
+        if (ctx) ctx->last_error = std::string(where) + ": shape not supported by this kernel";
+        return TCB_EUNSUPPORTED;
+    }
+    if (ctx && is_capture_error(e)) {
+        // an operation that cannot be recorded was issued inside tcb_capture_begin/end: the capture is lost, the context
+        // is not (tcb_capture_end returns TCB_EUNSUPPORTED and the list can be issued call by call)
+        cudaGetLastError();
+        ctx->capture_failed = true;
+        ctx->last_error = std::string(where) + ": " + cudaGetErrorString(e);
+        return TCB_EUNSUPPORTED;
+    }
     if (ctx) {
         ctx->sticky_cuda = true;
         ctx->last_error = std::string(where) + ": " + cudaGetErrorString(e);
     }
     return TCB_ECUDA;
 }
+
+// calls that copy from host memory, synchronise, allocate with cudaMalloc or plan for the first time cannot be recorded
+int refuse_in_capture(tcb_ctx *ctx, const char *what)
+{
+    if (!ctx->capturing) return TCB_OK;
+    ctx->capture_failed = true;
+    ctx->last_error = std::string(what) + " is not allowed between tcb_capture_begin and tcb_capture_end";
+    return TCB_EUNSUPPORTED;
+}
+
+struct NvtxRange {                          // one NVTX range per ABI call (tracing)
+    explicit NvtxRange(const char *name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
 
 #define TCB_CUDA(ctx, call)                                        \
     do {                                                           \
@@ -90,16 +144,21 @@ int enter(tcb_ctx *ctx)
 
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-constexpr size_t kWsHeader = 1024;      // head of the workspace: persistent work counters (see zgemm.cu)
+constexpr size_t kWsHeader = 8192;      // head of the workspace: persistent work counters (kGemmCounterBytes, see zgemm.cu)
+static_assert(kWsHeader >= kGemmCounterBytes, "workspace header too small for the GEMM counters");
 
 int workspace(tcb_ctx *ctx, size_t bytes, void **out)
 {
+    Lane &ln = ctx->lanes[ctx->cur];
     bytes += kWsHeader;
-    if (bytes > ctx->ws_bytes) {
-        TCB_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-        if (ctx->ws) cudaFree(ctx->ws);
-        ctx->ws = nullptr;
-        ctx->ws_bytes = 0;
+    if (bytes > ln.ws_bytes) {
+        int rc = refuse_in_capture(ctx, "growing the workspace (run the call list once before capturing it)");
+        if (rc) return rc;
+        TCB_CUDA(ctx, cudaStreamSynchronize(ln.stream));
+        if (ln.ws) cudaFree(ln.ws);
+        ln.ws = nullptr;
+        ln.ws_bytes = 0;
+        ++ctx->ws_generation;
         void *p = nullptr;
         const size_t want = align_up(bytes, (size_t)1 << 21);
         cudaError_t e = cudaMalloc(&p, want);
@@ -107,12 +166,12 @@ int workspace(tcb_ctx *ctx, size_t bytes, void **out)
             cudaGetLastError();
             return set_error(ctx, TCB_ENOMEM, "workspace allocation of " + std::to_string(want) + " bytes failed");
         }
-        ctx->ws = p;
-        ctx->ws_bytes = want;
+        ln.ws = p;
+        ln.ws_bytes = want;
         // the first kWsHeader bytes hold the GEMM's work counters: zero once here, every kernel leaves them zero
-        TCB_CUDA(ctx, cudaMemsetAsync(p, 0, kWsHeader, ctx->stream));
+        TCB_CUDA(ctx, cudaMemsetAsync(p, 0, kWsHeader, ln.stream));
     }
-    *out = (char *)ctx->ws + kWsHeader;
+    *out = (char *)ln.ws + kWsHeader;
     return TCB_OK;
 }
 
@@ -134,12 +193,12 @@ struct TimedLaunch {
         if (!on) return;
         span.cls = cls; span.flops = flops; span.bytes = bytes;
         span.a = take_event(ctx); span.b = take_event(ctx);
-        cudaEventRecord(span.a, ctx->stream);
+        cudaEventRecord(span.a, cur_stream(ctx));
     }
     ~TimedLaunch()
     {
         if (!on) return;
-        cudaEventRecord(span.b, ctx->stream);
+        cudaEventRecord(span.b, cur_stream(ctx));
         ctx->spans.push_back(span);
     }
 };
@@ -147,7 +206,7 @@ struct TimedLaunch {
 void fold_spans(tcb_ctx *ctx)
 {
     if (ctx->spans.empty()) return;
-    cudaStreamSynchronize(ctx->stream);
+    for (Lane &ln : ctx->lanes) if (ln.stream) cudaStreamSynchronize(ln.stream);
     for (const tcb_ctx::Span &s : ctx->spans) {
         float ms = 0.f;
         if (cudaEventElapsedTime(&ms, s.a, s.b) == cudaSuccess) {
@@ -212,9 +271,13 @@ int get_plan(tcb_ctx *ctx, const char *expr, const tcb_tensor *D, const tcb_tens
 {
     std::string key = std::string(expr) + "|" + shape_key(D->shape) + shape_key(L->shape) + shape_key(R->shape) +
                       "|" + std::to_string(ctx->opt.splitk) + "," + std::to_string(ctx->opt.epilogue) + "," +
-                      (ctx->opt.permute_always ? "1" : "0");
+                      (ctx->opt.permute_always ? "1" : "0") + "," + std::to_string(ctx->opt.operand_loads);
     auto it = ctx->plans.find(key);
     if (it != ctx->plans.end()) { *out = it->second.get(); return TCB_OK; }
+    {
+        int rcc = refuse_in_capture(ctx, "planning a contraction for the first time (run the call list once before capturing it)");
+        if (rcc) return rcc;
+    }
     ParsedExpr e;
     if (!parse_expression(expr, &e)) return set_error(ctx, TCB_EINVAL_EXPR, std::string("cannot parse: ") + expr);
     std::unique_ptr<CachedPlan> cp(new CachedPlan());
@@ -222,22 +285,28 @@ int get_plan(tcb_ctx *ctx, const char *expr, const tcb_tensor *D, const tcb_tens
     int rc = plan_contraction(e, D->shape, L->shape, R->shape, ctx->opt, &cp->plan, &why);
     if (rc != TCB_OK) return set_error(ctx, rc, why + ": " + expr);
     const ContractPlan &pl = cp->plan;
-    const size_t n = pl.offM.size() + pl.offN.size() + pl.offAm.size() + pl.offAk.size() + pl.offBk.size();
+    // one device block: offM, offN, then the GEMV tables (offAm, offAk, offBk) or the gather tables (row, k of A; row, k of B).
+    // The host vectors live as long as the cache entry, so the stream-ordered copies are safe.
+    const std::vector<int64_t> *aux[4] = {&pl.offAm, &pl.offAk, &pl.offBk, nullptr};
+    if (!pl.gemv) { aux[0] = &pl.a.gather_row; aux[1] = &pl.a.gather_k; aux[2] = &pl.b.gather_row; aux[3] = &pl.b.gather_k; }
+    size_t n = pl.offM.size() + pl.offN.size();
+    for (const std::vector<int64_t> *t : aux) if (t) n += t->size();
     TCB_CUDA(ctx, cudaMalloc((void **)&cp->d_tables, n * sizeof(int64_t)));
-    {   // GEMV tables behind offM and offN: offAm, offAk, offBk
-        size_t at = pl.offM.size() + pl.offN.size();
-        for (const std::vector<int64_t> *t : {&pl.offAm, &pl.offAk, &pl.offBk}) {
-            if (!t->empty())
-                TCB_CUDA(ctx, cudaMemcpyAsync(cp->d_tables + at, t->data(), t->size() * sizeof(int64_t),
-                                              cudaMemcpyHostToDevice, ctx->stream));
-            at += t->size();
-        }
+    size_t at = 0;
+    auto put = [&](const std::vector<int64_t> &t) -> cudaError_t {
+        cudaError_t e = t.empty() ? cudaSuccess
+                                  : cudaMemcpyAsync(cp->d_tables + at, t.data(), t.size() * sizeof(int64_t),
+                                                    cudaMemcpyHostToDevice, cur_stream(ctx));
+        at += t.size();
+        return e;
+    };
+    TCB_CUDA(ctx, put(pl.offM));
+    TCB_CUDA(ctx, put(pl.offN));
+    for (int q = 0; q < 4; ++q) {
+        if (!aux[q]) continue;
+        cp->d_aux[q] = aux[q]->empty() ? nullptr : cp->d_tables + at;
+        TCB_CUDA(ctx, put(*aux[q]));
     }
-    // the host vectors live as long as the cache entry, so the stream-ordered copies are safe
-    TCB_CUDA(ctx, cudaMemcpyAsync(cp->d_tables, cp->plan.offM.data(), cp->plan.offM.size() * sizeof(int64_t),
-                                  cudaMemcpyHostToDevice, ctx->stream));
-    TCB_CUDA(ctx, cudaMemcpyAsync(cp->d_tables + cp->plan.offM.size(), cp->plan.offN.data(),
-                                  cp->plan.offN.size() * sizeof(int64_t), cudaMemcpyHostToDevice, ctx->stream));
     *out = cp.get();
     ctx->plans[key] = std::move(cp);
     return TCB_OK;
@@ -281,11 +350,12 @@ int tcb_ctx_create(tcb_ctx **out, int device, void *cuda_stream, size_t workspac
     ctx->device = device;
     for (int c = 0; c < 4; ++c) ctx->acc[c] = tcb_kernel_stat{0, 0.0, 0.0, 0.0};
     if (cuda_stream) {
-        ctx->stream = (cudaStream_t)cuda_stream;
+        ctx->lanes[0].stream = (cudaStream_t)cuda_stream;
     } else {
-        if (cudaStreamCreateWithFlags(&ctx->stream, cudaStreamNonBlocking) != cudaSuccess) return TCB_ECUDA;
-        ctx->owns_stream = true;
+        if (cudaStreamCreateWithFlags(&ctx->lanes[0].stream, cudaStreamNonBlocking) != cudaSuccess) return TCB_ECUDA;
+        ctx->lanes[0].owns_stream = true;
     }
+    if (cudaEventCreateWithFlags(&ctx->lanes[0].ev, cudaEventDisableTiming) != cudaSuccess) return TCB_ECUDA;
     {   // tensors are created and destroyed every iteration by generated code: keep freed
         // blocks in the stream-ordered pool instead of returning them to the driver at every sync
         cudaMemPool_t pool;
@@ -308,15 +378,18 @@ int tcb_ctx_destroy(tcb_ctx *ctx)
 {
     if (!ctx) return TCB_OK;
     cudaSetDevice(ctx->device);
-    cudaStreamSynchronize(ctx->stream);
+    for (Lane &ln : ctx->lanes) if (ln.stream) cudaStreamSynchronize(ln.stream);
     for (auto &kv : ctx->plans)
         if (kv.second->d_tables) cudaFree(kv.second->d_tables);
-    if (ctx->ws) cudaFree(ctx->ws);
+    for (Lane &ln : ctx->lanes) if (ln.ws) cudaFree(ln.ws);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     fold_spans(ctx);
     for (cudaEvent_t e : ctx->free_events) cudaEventDestroy(e);
-    if (ctx->owns_stream) cudaStreamDestroy(ctx->stream);
+    for (Lane &ln : ctx->lanes) {
+        if (ln.ev) cudaEventDestroy(ln.ev);
+        if (ln.owns_stream && ln.stream) cudaStreamDestroy(ln.stream);
+    }
     delete ctx;
     return TCB_OK;
 }
@@ -341,7 +414,69 @@ int tcb_sync(tcb_ctx *ctx)
 {
     int rc = enter(ctx);
     if (rc) return rc;
-    TCB_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    rc = refuse_in_capture(ctx, "tcb_sync");
+    if (rc) return rc;
+    for (Lane &ln : ctx->lanes)
+        if (ln.stream) TCB_CUDA(ctx, cudaStreamSynchronize(ln.stream));
+    return TCB_OK;
+}
+
+// ---- lanes: concurrency between independent contractions (DLTC layers; the barrier after every
+// tensor operation is the measured serial fraction of PAPER.md:400) --------------------------------------------------------
+static int lane_ready(tcb_ctx *ctx, int lane)
+{
+    Lane &ln = ctx->lanes[lane];
+    if (!ln.stream) {
+        int rc = refuse_in_capture(ctx, "the first use of a lane (use every lane once before capturing)");
+        if (rc) return rc;
+        TCB_CUDA(ctx, cudaStreamCreateWithFlags(&ln.stream, cudaStreamNonBlocking));
+        ln.owns_stream = true;
+        TCB_CUDA(ctx, cudaEventCreateWithFlags(&ln.ev, cudaEventDisableTiming));
+    }
+    return TCB_OK;
+}
+
+// inside a capture a lane joins the graph by depending on the capture's origin (lane 0): done once, at its first use
+static int lane_fork_into_capture(tcb_ctx *ctx, int lane)
+{
+    Lane &ln = ctx->lanes[lane];
+    if (!ctx->capturing || lane == 0 || ln.in_capture) return TCB_OK;
+    TCB_CUDA(ctx, cudaEventRecord(ctx->lanes[0].ev, ctx->lanes[0].stream));
+    TCB_CUDA(ctx, cudaStreamWaitEvent(ln.stream, ctx->lanes[0].ev, 0));
+    ln.in_capture = true;
+    return TCB_OK;
+}
+
+int tcb_lane_count(void) { return kMaxLanes; }
+
+int tcb_lane_set(tcb_ctx *ctx, int lane)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (lane < 0 || lane >= kMaxLanes) return set_error(ctx, TCB_EINVAL, "lane outside 0..3");
+    rc = lane_ready(ctx, lane);
+    if (rc) return rc;
+    rc = lane_fork_into_capture(ctx, lane);
+    if (rc) return rc;
+    ctx->cur = lane;
+    return TCB_OK;
+}
+
+int tcb_lane_wait(tcb_ctx *ctx, int lane, int on_lane)
+{
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (lane < 0 || lane >= kMaxLanes || on_lane < 0 || on_lane >= kMaxLanes)
+        return set_error(ctx, TCB_EINVAL, "lane outside 0..3");
+    if (lane == on_lane) return TCB_OK;
+    rc = lane_ready(ctx, lane);
+    if (!rc) rc = lane_ready(ctx, on_lane);
+    if (!rc) rc = lane_fork_into_capture(ctx, on_lane);
+    if (rc) return rc;
+    Lane &a = ctx->lanes[lane], &b = ctx->lanes[on_lane];
+    TCB_CUDA(ctx, cudaEventRecord(b.ev, b.stream));
+    TCB_CUDA(ctx, cudaStreamWaitEvent(a.stream, b.ev, 0));
+    if (ctx->capturing) a.in_capture = true;
     return TCB_OK;
 }
 
@@ -370,14 +505,14 @@ static int make_tensor(tcb_ctx *ctx, tcb_tensor **out, int rank, const int64_t *
         t->owns = false;
     } else {
         void *p = nullptr;
-        cudaError_t e = cudaMallocAsync(&p, bytes, ctx->stream);
+        cudaError_t e = cudaMallocAsync(&p, bytes, cur_stream(ctx));
         if (e != cudaSuccess) {
             cudaGetLastError();
             return set_error(ctx, TCB_ENOMEM, "tensor allocation of " + std::to_string(bytes) + " bytes failed");
         }
         t->ptr = p;
         t->owns = true;
-        if (zero) TCB_CUDA(ctx, cudaMemsetAsync(p, 0, bytes, ctx->stream));
+        if (zero) TCB_CUDA(ctx, cudaMemsetAsync(p, 0, bytes, cur_stream(ctx)));
     }
     ++ctx->live_tensors;
     *out = t.release();
@@ -406,7 +541,7 @@ int tcb_tensor_destroy(tcb_tensor *t)
     tcb_ctx *ctx = t->ctx;
     if (t->owns && t->ptr) {
         cudaSetDevice(ctx->device);
-        cudaFreeAsync(t->ptr, ctx->stream);      // stream-ordered: pending kernels still see the memory
+        cudaFreeAsync(t->ptr, cur_stream(ctx));      // stream-ordered: pending kernels still see the memory
     }
     --ctx->live_tensors;
     delete t;
@@ -427,7 +562,9 @@ int tcb_tensor_upload(tcb_ctx *ctx, tcb_tensor *t, const tcb_c128 *host)
     int rc = enter(ctx);
     if (rc) return rc;
     if (!t || !host) return TCB_EINVAL;
-    TCB_CUDA(ctx, cudaMemcpyAsync(t->ptr, host, (size_t)t->elems() * 16, cudaMemcpyHostToDevice, ctx->stream));
+    rc = refuse_in_capture(ctx, "tcb_tensor_upload");
+    if (rc) return rc;
+    TCB_CUDA(ctx, cudaMemcpyAsync(t->ptr, host, (size_t)t->elems() * 16, cudaMemcpyHostToDevice, cur_stream(ctx)));
     return TCB_OK;
 }
 
@@ -436,18 +573,21 @@ int tcb_tensor_download(tcb_ctx *ctx, const tcb_tensor *t, tcb_c128 *host)
     int rc = enter(ctx);
     if (rc) return rc;
     if (!t || !host) return TCB_EINVAL;
-    TCB_CUDA(ctx, cudaMemcpyAsync(host, t->ptr, (size_t)t->elems() * 16, cudaMemcpyDeviceToHost, ctx->stream));
-    TCB_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    rc = refuse_in_capture(ctx, "tcb_tensor_download");
+    if (rc) return rc;
+    TCB_CUDA(ctx, cudaMemcpyAsync(host, t->ptr, (size_t)t->elems() * 16, cudaMemcpyDeviceToHost, cur_stream(ctx)));
+    TCB_CUDA(ctx, cudaStreamSynchronize(cur_stream(ctx)));
     return TCB_OK;
 }
 
 int tcb_tensor_fill(tcb_ctx *ctx, tcb_tensor *t, tcb_c128 value)
 {
+    NvtxRange nvtx_range("tcb_tensor_fill");
     int rc = enter(ctx);
     if (rc) return rc;
     if (!t) return TCB_EINVAL;
     TimedLaunch tl(ctx, kClsElementwise, 0.0, 16.0 * (double)t->elems());
-    TCB_CUDA(ctx, launch_fill(t->ptr, t->elems(), value.re, value.im, ctx->stream, &ctx->launches));
+    TCB_CUDA(ctx, launch_fill(t->ptr, t->elems(), value.re, value.im, cur_stream(ctx), &ctx->launches));
     return TCB_OK;
 }
 
@@ -456,6 +596,7 @@ int tcb_tensor_fill(tcb_ctx *ctx, tcb_tensor *t, tcb_c128 value)
 int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor *L, const tcb_tensor *R,
                  tcb_c128 alpha)
 {
+    NvtxRange nvtx_range("tcb_contract");
     int rc = enter(ctx);
     if (rc) return rc;
     if (!expr || !D || !L || !R) return set_error(ctx, TCB_EINVAL, "null argument");
@@ -484,48 +625,78 @@ int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor
         g.accumulate = P.accumulate;
         g.partial = wsg;
         TimedLaunch tl(ctx, kClsZgemm, P.flops, P.bytes);
-        TCB_CUDA(ctx, launch_gemv(g, ctx->stream, &ctx->launches));
+        TCB_CUDA(ctx, launch_gemv(g, cur_stream(ctx), &ctx->launches));
         return TCB_OK;
     }
 
     const size_t bytesA = P.a.permuted ? align_up((size_t)P.a.elems * 16, 1024) : 0;
     const size_t bytesB = P.b.permuted ? align_up((size_t)P.b.elems * 16, 1024) : 0;
     const size_t bytesP = align_up(P.partial_bytes, 1024);
+    const size_t bytesC = P.twopass ? align_up((size_t)P.M * (size_t)P.N * 16, 1024) : 0;
+    // everything that can refuse is decided before the first launch (on an error return nothing has been enqueued)
+    PermuteDesc dA, dB, dC;
+    if (P.a.permuted) {
+        dA = make_desc(P.a.perm, TA->ptr, nullptr, kPermCopy, 1.0, 0.0);
+        TCB_CUDA(ctx, launch_permute(dA, nullptr, nullptr, true));
+    }
+    if (P.b.permuted) {
+        dB = make_desc(P.b.perm, TB->ptr, nullptr, kPermCopy, 1.0, 0.0);
+        TCB_CUDA(ctx, launch_permute(dB, nullptr, nullptr, true));
+    }
+    if (P.twopass) {
+        dC = make_desc(P.c_perm, nullptr, D->ptr, P.accumulate ? kPermAccumulate : kPermScale, alpha.re, alpha.im);
+        TCB_CUDA(ctx, launch_permute(dC, nullptr, nullptr, true));
+    }
     char *ws = nullptr;
     {
         void *p;
-        rc = workspace(ctx, bytesA + bytesB + bytesP, &p);
+        rc = workspace(ctx, bytesA + bytesB + bytesP + bytesC, &p);
         if (rc) return rc;
         ws = (char *)p;
     }
     const void *Aptr = TA->ptr, *Bptr = TB->ptr;
     if (P.a.permuted) {
-        PermuteDesc d = make_desc(P.a.perm, TA->ptr, ws, kPermCopy, 1.0, 0.0);
+        dA.out = ws;
         TimedLaunch tl(ctx, kClsPermute, 0.0, 32.0 * (double)P.a.elems);
-        TCB_CUDA(ctx, launch_permute(d, ctx->stream, &ctx->launches));
+        TCB_CUDA(ctx, launch_permute(dA, cur_stream(ctx), &ctx->launches));
         Aptr = ws;
     }
     if (P.b.permuted) {
-        PermuteDesc d = make_desc(P.b.perm, TB->ptr, ws + bytesA, kPermCopy, 1.0, 0.0);
+        dB.out = ws + bytesA;
         TimedLaunch tl(ctx, kClsPermute, 0.0, 32.0 * (double)P.b.elems);
-        TCB_CUDA(ctx, launch_permute(d, ctx->stream, &ctx->launches));
+        TCB_CUDA(ctx, launch_permute(dB, cur_stream(ctx), &ctx->launches));
         Bptr = ws + bytesA;
     }
+    char *Cws = ws + bytesA + bytesB + bytesP;
     GemmDesc g;
     g.M = P.M; g.N = P.N; g.K = P.K;
     g.A = Aptr; g.B = Bptr;
     g.lda = P.a.ld; g.ldb = P.b.ld;
     g.a_kmajor = P.a.kmajor; g.b_kmajor = P.b.kmajor;
-    g.D = D->ptr;
+    if (P.a.gather) { g.gatherAm = cp->d_aux[0]; g.gatherAk = cp->d_aux[1]; g.a_mfast = P.a.mfast; }
+    if (P.b.gather) { g.gatherBn = cp->d_aux[2]; g.gatherBk = cp->d_aux[3]; g.b_mfast = P.b.mfast; }
+    g.D = P.twopass ? (void *)Cws : D->ptr;
     g.offM = cp->d_tables;
     g.offN = cp->d_tables + P.offM.size();
-    g.alpha_re = alpha.re; g.alpha_im = alpha.im;
-    g.accumulate = P.accumulate;
+    g.alpha_re = P.twopass ? 1.0 : alpha.re; g.alpha_im = P.twopass ? 0.0 : alpha.im;
+    g.accumulate = P.twopass ? false : P.accumulate;
     g.splitk = P.splitk;
     g.partial = bytesP ? ws + bytesA + bytesB : nullptr;
-    g.counters = ctx->opt.static_deal ? nullptr : (char *)ctx->ws;      // the workspace header
-    TimedLaunch tl(ctx, kClsZgemm, P.flops, P.bytes);
-    TCB_CUDA(ctx, launch_zgemm(g, ctx->stream, &ctx->launches));
+    g.counters = ctx->opt.static_deal ? nullptr : ctx->lanes[ctx->cur].ws;      // the workspace header
+    // the two TMA descriptors are kept beside the plan: re-encoded only when an operand sits somewhere else
+    if (!cp->maps_valid || cp->map_a != Aptr || cp->map_b != Bptr) {
+        TCB_CUDA(ctx, encode_gemm_maps(g, &cp->maps));
+        cp->map_a = Aptr; cp->map_b = Bptr; cp->maps_valid = true;
+    }
+    {
+        TimedLaunch tl(ctx, kClsZgemm, P.flops, P.bytes);
+        TCB_CUDA(ctx, launch_zgemm_with_maps(g, cp->maps, cur_stream(ctx), &ctx->launches));
+    }
+    if (P.twopass) {
+        dC.in = Cws;
+        TimedLaunch tl(ctx, kClsPermute, 0.0, 16.0 * (double)P.M * (double)P.N * (P.accumulate ? 3.0 : 2.0));
+        TCB_CUDA(ctx, launch_permute(dC, cur_stream(ctx), &ctx->launches));
+    }
     return TCB_OK;
 }
 
@@ -566,6 +737,13 @@ static int apply_option(PlanOptions &opt, const std::string &k, const std::strin
         if (v == "auto") opt.permute_always = false;
         else if (v == "always") opt.permute_always = true;
         else { *why = "permute_operands: expected auto or always"; return TCB_EINVAL; }
+        return TCB_OK;
+    }
+    if (k == "operand_loads") {
+        if (v == "auto") opt.operand_loads = 0;
+        else if (v == "gather") opt.operand_loads = 1;
+        else if (v == "permute") opt.operand_loads = 2;
+        else { *why = "operand_loads: expected auto, gather or permute"; return TCB_EINVAL; }
         return TCB_OK;
     }
     if (k == "gemm_deal") {
@@ -632,6 +810,7 @@ int tcb_plan_describe_host(const char *expr, int rank_d, const int64_t *ext_d, i
 static int permuted_op(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor *L, tcb_c128 alpha,
                        bool pure_copy)
 {
+    NvtxRange nvtx_range(pure_copy ? "tcb_permute" : "tcb_add");
     int rc = enter(ctx);
     if (rc) return rc;
     if (!expr || !D || !L) return set_error(ctx, TCB_EINVAL, "null argument");
@@ -658,15 +837,15 @@ static int permuted_op(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_
     if (pure_copy) {
         TimedLaunch tl(ctx, kClsPermute, 0.0, 2 * n16);
         PermuteDesc d = make_desc(ps, L->ptr, D->ptr, kPermCopy, 1.0, 0.0);
-        TCB_CUDA(ctx, launch_permute(d, ctx->stream, &ctx->launches));
+        TCB_CUDA(ctx, launch_permute(d, cur_stream(ctx), &ctx->launches));
     } else if (ps.identity) {
         TimedLaunch tl(ctx, kClsElementwise, 0.0, (e.accumulate ? 3 : 2) * n16);
-        TCB_CUDA(ctx, launch_axpy(D->ptr, L->ptr, D->elems(), alpha.re, alpha.im, e.accumulate, ctx->stream,
+        TCB_CUDA(ctx, launch_axpy(D->ptr, L->ptr, D->elems(), alpha.re, alpha.im, e.accumulate, cur_stream(ctx),
                                   &ctx->launches));
     } else {
         TimedLaunch tl(ctx, kClsPermute, 0.0, (e.accumulate ? 3 : 2) * n16);
         PermuteDesc d = make_desc(ps, L->ptr, D->ptr, e.accumulate ? kPermAccumulate : kPermScale, alpha.re, alpha.im);
-        TCB_CUDA(ctx, launch_permute(d, ctx->stream, &ctx->launches));
+        TCB_CUDA(ctx, launch_permute(d, cur_stream(ctx), &ctx->launches));
     }
     return TCB_OK;
 }
@@ -684,16 +863,18 @@ int tcb_permute(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor 
 
 int tcb_scale(tcb_ctx *ctx, tcb_tensor *D, tcb_c128 alpha)
 {
+    NvtxRange nvtx_range("tcb_scale");
     int rc = enter(ctx);
     if (rc) return rc;
     if (!D) return TCB_EINVAL;
     TimedLaunch tl(ctx, kClsElementwise, 0.0, 32.0 * (double)D->elems());
-    TCB_CUDA(ctx, launch_scale(D->ptr, D->elems(), alpha.re, alpha.im, ctx->stream, &ctx->launches));
+    TCB_CUDA(ctx, launch_scale(D->ptr, D->elems(), alpha.re, alpha.im, cur_stream(ctx), &ctx->launches));
     return TCB_OK;
 }
 
 int tcb_dot(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, const tcb_tensor *Y, int conjugate_x, tcb_c128 alpha)
 {
+    NvtxRange nvtx_range("tcb_dot");
     int rc = enter(ctx);
     if (rc) return rc;
     if (!D || !X || !Y) return set_error(ctx, TCB_EINVAL, "null argument");
@@ -703,16 +884,16 @@ int tcb_dot(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, const tcb_tensor *
         if (X->shape.ext[k] != Y->shape.ext[k]) return set_error(ctx, TCB_ESHAPE, "X and Y differ in shape");
     if (overlaps(D, X) || overlaps(D, Y)) return set_error(ctx, TCB_EALIAS, "D overlaps X or Y");
     const int64_t n = X->elems();
-    const int nblocks = (int)std::max<int64_t>(1, std::min<int64_t>(kDotBlocks, (n + 255) / 256));
+    const int nblocks = (int)std::max<int64_t>(1, std::min<int64_t>(std::min(kDotBlocks, 4 * sm_count()), (n + 255) / 256));
     void *partial = nullptr;
-    TCB_CUDA(ctx, cudaMallocAsync(&partial, (size_t)nblocks * 16, ctx->stream));
+    TCB_CUDA(ctx, cudaMallocAsync(&partial, (size_t)nblocks * 16, cur_stream(ctx)));
     cudaError_t e;
     {
         TimedLaunch tl(ctx, kClsElementwise, 8.0 * (double)n, 32.0 * (double)n);
-        e = launch_dot(D->ptr, X->ptr, Y->ptr, n, conjugate_x != 0, alpha.re, alpha.im, partial, nblocks, ctx->stream,
+        e = launch_dot(D->ptr, X->ptr, Y->ptr, n, conjugate_x != 0, alpha.re, alpha.im, partial, nblocks, cur_stream(ctx),
                        &ctx->launches);
     }
-    cudaFreeAsync(partial, ctx->stream);
+    cudaFreeAsync(partial, cur_stream(ctx));
     TCB_CUDA(ctx, e);
     return TCB_OK;
 }
@@ -720,9 +901,12 @@ int tcb_dot(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, const tcb_tensor *
 static int denominator_op(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, const double *const *eps, tcb_c128 alpha,
                           bool accumulate)
 {
+    NvtxRange nvtx_range("tcb_denominator_update/divide");
     int rc = enter(ctx);
     if (rc) return rc;
     if (!T || !R || !eps) return set_error(ctx, TCB_EINVAL, "null argument");
+    rc = refuse_in_capture(ctx, "tcb_denominator_update / tcb_denominator_divide (they copy the energies from host memory)");
+    if (rc) return rc;
     const int r = T->shape.rank;
     if (R->shape.rank != r) return set_error(ctx, TCB_ESHAPE, "rank mismatch");
     for (int k = 0; k < r; ++k)
@@ -743,14 +927,14 @@ static int denominator_op(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, cons
     // the energies travel with the call: a few hundred doubles, stream-ordered allocation (pageable source: the copy
     // is staged before cudaMemcpyAsync returns)
     double *dev = nullptr;
-    TCB_CUDA(ctx, cudaMallocAsync((void **)&dev, host.size() * sizeof(double), ctx->stream));
-    cudaError_t e = cudaMemcpyAsync(dev, host.data(), host.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
+    TCB_CUDA(ctx, cudaMallocAsync((void **)&dev, host.size() * sizeof(double), cur_stream(ctx)));
+    cudaError_t e = cudaMemcpyAsync(dev, host.data(), host.size() * sizeof(double), cudaMemcpyHostToDevice, cur_stream(ctx));
     if (e == cudaSuccess) {
         TimedLaunch tl(ctx, kClsElementwise, 0.0, (accumulate ? 48.0 : 32.0) * (double)T->elems());
         e = launch_denominator_update(T->ptr, R->ptr, r, T->shape.ext, dev, at, alpha.re, alpha.im, accumulate,
-                                      ctx->stream, &ctx->launches);
+                                      cur_stream(ctx), &ctx->launches);
     }
-    cudaFreeAsync(dev, ctx->stream);
+    cudaFreeAsync(dev, cur_stream(ctx));
     TCB_CUDA(ctx, e);
     return TCB_OK;
 }
@@ -768,6 +952,7 @@ int tcb_denominator_divide(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, con
 int tcb_permsum(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, int nterms, const int32_t *perms,
                 const tcb_c128 *coefs, tcb_c128 beta)
 {
+    NvtxRange nvtx_range("tcb_permsum");
     int rc = enter(ctx);
     if (rc) return rc;
     if (!D || !X || !perms || !coefs) return set_error(ctx, TCB_EINVAL, "null argument");
@@ -798,12 +983,13 @@ int tcb_permsum(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, int nterms, co
     d.X = X->ptr; d.D = D->ptr;
     const bool reads_d = !(beta.re == 0.0 && beta.im == 0.0);
     TimedLaunch tl(ctx, kClsPermsum, 0.0, 16.0 * (double)D->elems() * (reads_d ? 3.0 : 2.0));
-    TCB_CUDA(ctx, launch_permsum(d, ctx->stream, &ctx->launches));
+    TCB_CUDA(ctx, launch_permsum(d, cur_stream(ctx), &ctx->launches));
     return TCB_OK;
 }
 
 int tcb_antisymmetrize(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *X, tcb_c128 alpha)
 {
+    NvtxRange nvtx_range("tcb_antisymmetrize");
     int rc = enter(ctx);
     if (rc) return rc;
     if (!spec || !D || !X) return set_error(ctx, TCB_EINVAL, "null argument");
@@ -865,7 +1051,7 @@ int tcbx_internal_stream(tcb_ctx *ctx, void **stream, int64_t **launches)
 {
     int rc = enter(ctx);
     if (rc) return rc;
-    *stream = (void *)ctx->stream;
+    *stream = (void *)cur_stream(ctx);
     *launches = &ctx->launches;
     return TCB_OK;
 }
@@ -877,7 +1063,7 @@ int tcb_measure_fp64_tensor_peak(tcb_ctx *ctx, double milliseconds, double *tflo
     int rc = enter(ctx);
     if (rc) return rc;
     if (!tflops) return TCB_EINVAL;
-    TCB_CUDA(ctx, run_dmma_peak(milliseconds, tflops, ctx->stream, &ctx->launches));
+    TCB_CUDA(ctx, run_dmma_peak(milliseconds, tflops, cur_stream(ctx), &ctx->launches));
     return TCB_OK;
 }
 
@@ -886,7 +1072,7 @@ int tcb_measure_fp64_vector_peak(tcb_ctx *ctx, double milliseconds, double *tflo
     int rc = enter(ctx);
     if (rc) return rc;
     if (!tflops) return TCB_EINVAL;
-    TCB_CUDA(ctx, run_dfma_peak(milliseconds, tflops, ctx->stream, &ctx->launches));
+    TCB_CUDA(ctx, run_dfma_peak(milliseconds, tflops, cur_stream(ctx), &ctx->launches));
     return TCB_OK;
 }
 
@@ -916,6 +1102,8 @@ struct tcb_graph {
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
     int64_t launches = 0;
+    uint64_t ws_generation = 0;      // the workspace blocks whose addresses the kernels of this graph carry
+    size_t nodes = 0, edges = 0;
 };
 
 int tcb_capture_begin(tcb_ctx *ctx)
@@ -924,8 +1112,12 @@ int tcb_capture_begin(tcb_ctx *ctx)
     if (rc) return rc;
     if (ctx->capturing) return set_error(ctx, TCB_EINVAL, "a capture is already open");
     if (ctx->kernel_timing) return set_error(ctx, TCB_EINVAL, "kernel_timing must be off during a capture");
-    TCB_CUDA(ctx, cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+    if (ctx->cur != 0) return set_error(ctx, TCB_EINVAL, "a capture starts on lane 0");
+    TCB_CUDA(ctx, cudaStreamBeginCapture(ctx->lanes[0].stream, cudaStreamCaptureModeThreadLocal));
     ctx->capturing = true;
+    ctx->capture_failed = false;
+    for (Lane &ln : ctx->lanes) ln.in_capture = false;
+    ctx->lanes[0].in_capture = true;
     ctx->capture_l0 = ctx->launches;
     return TCB_OK;
 }
@@ -935,12 +1127,28 @@ int tcb_capture_end(tcb_ctx *ctx, tcb_graph **out)
     if (!ctx || !out) return TCB_EINVAL;
     *out = nullptr;
     if (!ctx->capturing) return set_error(ctx, TCB_EINVAL, "no capture is open");
+    cudaSetDevice(ctx->device);
+    // every lane that was forked into the capture joins lane 0 again (a capture must end with one open path)
+    for (int l = 1; l < kMaxLanes && !ctx->capture_failed; ++l) {
+        Lane &ln = ctx->lanes[l];
+        if (!ln.in_capture) continue;
+        if (cudaEventRecord(ln.ev, ln.stream) != cudaSuccess ||
+            cudaStreamWaitEvent(ctx->lanes[0].stream, ln.ev, 0) != cudaSuccess) {
+            cudaGetLastError();
+            ctx->capture_failed = true;
+        }
+    }
     ctx->capturing = false;
+    ctx->cur = 0;
+    for (Lane &ln : ctx->lanes) ln.in_capture = false;
     std::unique_ptr<tcb_graph> g(new tcb_graph);
-    cudaError_t e = cudaStreamEndCapture(ctx->stream, &g->graph);
-    if (e != cudaSuccess || !g->graph) {
+    cudaError_t e = cudaStreamEndCapture(ctx->lanes[0].stream, &g->graph);
+    if (e != cudaSuccess || !g->graph || ctx->capture_failed) {
         cudaGetLastError();
-        return set_error(ctx, TCB_EUNSUPPORTED, std::string("the call list could not be captured: ") + cudaGetErrorString(e));
+        if (g->graph) cudaGraphDestroy(g->graph);
+        const std::string why = ctx->capture_failed ? ctx->last_error : std::string(cudaGetErrorString(e));
+        ctx->capture_failed = false;
+        return set_error(ctx, TCB_EUNSUPPORTED, "the call list could not be captured: " + why);
     }
     e = cudaGraphInstantiate(&g->exec, g->graph, 0);
     if (e != cudaSuccess) {
@@ -948,19 +1156,35 @@ int tcb_capture_end(tcb_ctx *ctx, tcb_graph **out)
         cudaGetLastError();
         return set_error(ctx, TCB_EUNSUPPORTED, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e));
     }
+    cudaGraphGetNodes(g->graph, nullptr, &g->nodes);
+    cudaGraphGetEdges(g->graph, nullptr, nullptr, &g->edges);
     g->launches = ctx->launches - ctx->capture_l0;
+    g->ws_generation = ctx->ws_generation;
     *out = g.release();
     return TCB_OK;
 }
 
 int tcb_graph_launch(tcb_ctx *ctx, tcb_graph *g)
 {
+    NvtxRange nvtx_range("tcb_graph_launch");
     int rc = enter(ctx);
     if (rc) return rc;
     if (!g || !g->exec) return TCB_EINVAL;
     if (ctx->capturing) return set_error(ctx, TCB_EINVAL, "graph launch inside a capture");
-    TCB_CUDA(ctx, cudaGraphLaunch(g->exec, ctx->stream));
+    if (g->ws_generation != ctx->ws_generation)
+        return set_error(ctx, TCB_EINVAL, "the workspace was reallocated after this graph was captured (a later call needed a "
+                                          "larger one): capture the call list again");
+    TCB_CUDA(ctx, cudaGraphLaunch(g->exec, ctx->lanes[0].stream));
     ctx->launches += g->launches;
+    return TCB_OK;
+}
+
+int tcb_graph_info(const tcb_graph *g, int64_t *nodes, int64_t *edges, int64_t *kernel_launches)
+{
+    if (!g) return TCB_EINVAL;
+    if (nodes) *nodes = (int64_t)g->nodes;
+    if (edges) *edges = (int64_t)g->edges;
+    if (kernel_launches) *kernel_launches = g->launches;
     return TCB_OK;
 }
 
@@ -977,7 +1201,7 @@ int tcb_timer_start(tcb_ctx *ctx)
 {
     int rc = enter(ctx);
     if (rc) return rc;
-    TCB_CUDA(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
+    TCB_CUDA(ctx, cudaEventRecord(ctx->ev0, cur_stream(ctx)));
     return TCB_OK;
 }
 
@@ -986,7 +1210,7 @@ int tcb_timer_stop(tcb_ctx *ctx, double *milliseconds)
     int rc = enter(ctx);
     if (rc) return rc;
     if (!milliseconds) return TCB_EINVAL;
-    TCB_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
+    TCB_CUDA(ctx, cudaEventRecord(ctx->ev1, cur_stream(ctx)));
     TCB_CUDA(ctx, cudaEventSynchronize(ctx->ev1));
     float ms = 0.f;
     TCB_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));

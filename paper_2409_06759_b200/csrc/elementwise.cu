@@ -43,7 +43,7 @@ axpy_kernel(double2 *D, const double2 *__restrict__ L, long long n, double ar, d
 int grid_for(long long n)
 {
     long long b = (n + 255) / 256;
-    if (b > 148 * 16) b = 148 * 16;
+    if (b > sm_count() * 16LL) b = sm_count() * 16LL;
     return b < 1 ? 1 : (int)b;
 }
 
@@ -234,7 +234,7 @@ cudaError_t launch_denominator_update(void *T, const void *R, int rank, const in
     p.T = (double2 *)T;
     p.R = (const double2 *)R;
     p.ar = re; p.ai = im;
-    const int blocks = (int)std::max<long long>(1, std::min<long long>(p.nslabs, 148LL * 8));
+    const int blocks = (int)std::max<long long>(1, std::min<long long>(p.nslabs, sm_count() * 8LL));
     if (accumulate) denominator_update_kernel<true><<<blocks, 256, 0, s>>>(p);
     else denominator_update_kernel<false><<<blocks, 256, 0, s>>>(p);
     cudaError_t e = cudaGetLastError();

@@ -129,9 +129,10 @@ int gemv_ksplit(int64_t M, int64_t K, bool kfast)
 {
     const int64_t ctas_m = kfast ? (M + GT / 32 - 1) / (GT / 32) : (M + GT - 1) / GT;
     const int64_t min_chunk = kfast ? 512 : 256;
-    int64_t s = (4 * 148 + ctas_m - 1) / ctas_m;
+    const int64_t sms = sm_count();
+    int64_t s = (4 * sms + ctas_m - 1) / ctas_m;
     s = std::min<int64_t>(s, K / min_chunk);
-    return (int)std::max<int64_t>(1, std::min<int64_t>(s, kfast ? 8 * 4 * 148 : 64));   // a dot product: one warp per chunk
+    return (int)std::max<int64_t>(1, std::min<int64_t>(s, kfast ? 8 * 4 * sms : 64));   // a dot product: one warp per chunk
 }
 
 cudaError_t launch_gemv(const GemvDesc &g, cudaStream_t stream, int64_t *launches)

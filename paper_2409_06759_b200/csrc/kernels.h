@@ -9,6 +9,13 @@ namespace tcb {
 
 constexpr int kMaxRank = 6;
 
+// Number of SMs of the current device (cudaDevAttrMultiProcessorCount, cached per device); 148 -- a B200 -- when no
+// device can be asked (the host-only planner).  Every persistent grid is sized from this.
+int sm_count();
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is per device: true when `tag` (one per kernel instantiation) has not
+// been configured on the current device yet (and marks it configured)
+bool first_use_on_device(const void *tag);
+
 // ---- S4 + S5: complex FP64 GEMM on DMMA with the permute-and-accumulate epilogue ---------------------
 // C[m,n] = sum_k A[m,k] * B[k,n];   D[offM[m] + offN[n]] (+)= alpha * C[m,n]
 // Operand layouts ("K-major": k has unit stride, element (row,k) at row*ld + k;
@@ -25,8 +32,17 @@ struct GemmDesc {
     bool accumulate;         // true: D += ...; false: D = ...
     int splitk;              // 0 = auto (stream-K on the remainder wave), 1 = off, n > 1 = every tile cut n ways
     void *partial;           // device, gemm_schedule(...).partial_bytes (raw accumulator fragments of cut tiles)
-    void *counters = nullptr; // device, 24 bytes, 8-byte aligned, ZERO on entry (the kernel leaves them zero): work counters of the dynamic deal (null: static deal)
+    void *counters = nullptr; // device, kGemmCounterBytes, 8-byte aligned, ZERO on entry (the kernel leaves them zero): work
+                              // counters of the dynamic deal + arrival counters of the cut tiles (null: static deal, fix-up kernel)
+    // Permutation-free operand loads: when gatherAm is set, A is not a matrix in memory and is read in place
+    // as A[m,k] = A[gatherAm[m] + gatherAk[k]] (device tables, element offsets; lda / a_kmajor unused); a_mfast: the operand's
+    // unit-stride index is a row (free) index, so lanes run along m, else along k.  Same for B.
+    const int64_t *gatherAm = nullptr, *gatherAk = nullptr, *gatherBn = nullptr, *gatherBk = nullptr;
+    bool a_mfast = false, b_mfast = false;
 };
+constexpr int kGemmTileCounterOffset = 64;                 // bytes into `counters`
+constexpr int kGemmTileCounters = 1000;                    // cut tiles whose fix-up can run inside the main kernel
+constexpr size_t kGemmCounterBytes = kGemmTileCounterOffset + 4 * kGemmTileCounters + 32;
 // How the (tile, k-tile) iteration space is dealt to the persistent grid (2 CTAs per SM): whole tiles
 // data-parallel, the remainder ("stream-K") cut along K into equal chunks, one per CTA, summed by a fix-up kernel.
 struct GemmSchedule {
@@ -75,7 +91,8 @@ struct PermuteDesc {
     PermuteOp op;
     double alpha_re, alpha_im;
 };
-cudaError_t launch_permute(const PermuteDesc &p, cudaStream_t stream, int64_t *launches);
+// dry_run: only decide whether the shape can be tiled (cudaErrorNotSupported if not) -- nothing is launched
+cudaError_t launch_permute(const PermuteDesc &p, cudaStream_t stream, int64_t *launches, bool dry_run = false);
 
 // ---- S6: fused permute-sum -------------------------------------------------------------------------------
 constexpr int kMaxTerms = 36;
@@ -101,7 +118,7 @@ cudaError_t launch_axpy(void *D, const void *L, int64_t n, double re, double im,
                         cudaStream_t stream, int64_t *launches);
 
 // D[0] = alpha * sum_i (conj_x ? conj(X[i]) : X[i]) * Y[i]; partial: device, nblocks complex128 (nblocks <= kDotBlocks)
-constexpr int kDotBlocks = 148 * 4;
+constexpr int kDotBlocks = 1024;      // upper bound of the first-stage grid (4 blocks per SM)
 cudaError_t launch_dot(void *D, const void *X, const void *Y, int64_t n, bool conj_x, double re, double im, void *partial,
                        int nblocks, cudaStream_t stream, int64_t *launches);
 // T[idx] (+)= alpha * R[idx] / (sum_k eps[eps_at[k] + idx_k]) over the dims with eps_at[k] >= 0 (eps: device doubles)

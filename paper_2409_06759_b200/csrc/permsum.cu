@@ -199,7 +199,7 @@ bool try_cube(const PermSumDesc &d, cudaStream_t stream, cudaError_t *err)
     // on configs[3]; 9.4-11 with 3-4), the 4-term one (64 registers) with 4
     static const int env_ctas = getenv("TCB_PERMSUM_CTAS") ? atoi(getenv("TCB_PERMSUM_CTAS")) : 0;
     const int ctas = env_ctas > 0 ? env_ctas : (d.nterms <= 4 ? 4 : 2);
-    const unsigned blocks = (unsigned)std::min<long long>((units + 7) / 8, 148LL * ctas);
+    const unsigned blocks = (unsigned)std::min<long long>((units + 7) / 8, (long long)sm_count() * ctas);
     if (d.nterms <= 4) permsum_cube_kernel<4><<<blocks, 256, 0, stream>>>(p);
     else permsum_cube_kernel<9><<<blocks, 256, 0, stream>>>(p);
     *err = cudaGetLastError();
@@ -240,7 +240,7 @@ cudaError_t launch_permsum(const PermSumDesc &d, cudaStream_t stream, int64_t *l
     p.X = (const double2 *)d.X;
     p.D = (double2 *)d.D;
     long long blocks = (p.n + 255) / 256;
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > sm_count() * 16LL) blocks = sm_count() * 16LL;
     if (blocks < 1) blocks = 1;
     permsum_kernel<<<(int)blocks, 256, 0, stream>>>(p);
     cudaError_t e = cudaGetLastError();

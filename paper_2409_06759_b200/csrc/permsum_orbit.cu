@@ -552,7 +552,7 @@ cudaError_t build_plan(const PermSumDesc &d, OrbitPlan &plan)
     p.slab_order = reinterpret_cast<const unsigned *>(tables + o1);
     p.group_start = reinterpret_cast<const unsigned *>(tables + o2);
     plan.nslabs = nslabs;
-    plan.grid = (int)std::min<unsigned long long>((unsigned long long)p.ngroups * p.norbits, 148ULL);
+    plan.grid = (int)std::min<unsigned long long>((unsigned long long)p.ngroups * p.norbits, (unsigned long long)sm_count());
     plan.eligible = true;
     return cudaSuccess;
 }
@@ -608,11 +608,9 @@ cudaError_t launch_permsum_orbit(const PermSumDesc &d, cudaStream_t stream, int6
                    CU_TENSOR_MAP_SWIZZLE_NONE, kPromo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return cudaSuccess;              // a shape the maps cannot express: the gather kernels
     }
-    static bool configured = false;
-    if (!configured) {
+    if (first_use_on_device((const void *)permsum_orbit_kernel)) {
         cudaError_t e = cudaFuncSetAttribute(permsum_orbit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 4096);
         if (e != cudaSuccess) return e;
-        configured = true;
     }
     permsum_orbit_kernel<<<plan.grid, kThreads, plan.smem, stream>>>(tmX, tmD, p);
     cudaError_t e = cudaGetLastError();

@@ -334,7 +334,7 @@ int env_int(const char *name, int dflt)
 
 }  // namespace
 
-cudaError_t launch_permute(const PermuteDesc &pd, cudaStream_t stream, int64_t *launches)
+cudaError_t launch_permute(const PermuteDesc &pd, cudaStream_t stream, int64_t *launches, bool dry_run)
 {
     PermParams p;
     const int r = pd.rank;
@@ -399,7 +399,7 @@ cudaError_t launch_permute(const PermuteDesc &pd, cudaStream_t stream, int64_t *
         if (p.t[d] < p.e[d]) break;          // a partial dim ends the contiguous run: further dims add rows, not run length
     }
     for (int d = 0; d < r; ++d) p.ntile[d] = (int)((p.e[d] + p.t[d] - 1) / p.t[d]);
-    if (volume() > kMaxVol) return cudaErrorInvalidValue;
+    if (volume() > kMaxVol) return cudaErrorNotSupported;
     p.vol = (int)volume();
     p.rows = p.vol / p.t[0];
     p.ntiles = 1;
@@ -421,13 +421,13 @@ cudaError_t launch_permute(const PermuteDesc &pd, cudaStream_t stream, int64_t *
     // one tile in flight per CTA is enough with two CTAs per SM, and the shared memory not taken stays L1
     p.stages = std::max(2, std::min(env_int("TCB_PERM_STAGES", 2), budget / p.tile_bytes));
     const size_t smem = (size_t)p.stages * p.tile_bytes + 128;
-    if (smem > 227 * 1024) return cudaErrorInvalidValue;
+    if (smem > 227 * 1024) return cudaErrorNotSupported;
     p.in = (const double2 *)pd.in;
     p.out = (double2 *)pd.out;
     p.ar = pd.alpha_re; p.ai = pd.alpha_im;
 
     const int J = (p.vol + PT - 1) / PT;
-    const int blocks = (int)std::min<long long>(p.ntiles, 148LL * ctas_per_sm);
+    const int blocks = (int)std::min<long long>(p.ntiles, (long long)sm_count() * ctas_per_sm);
     {   // mixed-radix digits of the grid size
         long long g = blocks;
         for (int d = 0; d < kMaxRank; ++d) { p.step[d] = (int)(g % p.ntile[d]); g /= p.ntile[d]; }
@@ -444,7 +444,8 @@ cudaError_t launch_permute(const PermuteDesc &pd, cudaStream_t stream, int64_t *
         max_in += (long long)(p.t[d] - 1) * p.is[d];
         max_out += (long long)(p.t[d] - 1) * p.os[d];
     }
-    if (bit > kIdxBits || s >= (1 << (32 - kIdxBits))) return cudaErrorInvalidValue;
+    if (bit > kIdxBits || s >= (1 << (32 - kIdxBits))) return cudaErrorNotSupported;
+    if (dry_run) return cudaSuccess;          // every check that can refuse the shape has passed; nothing is launched
     const bool small = max_in < (1LL << 31) && max_out < (1LL << 31);
     cudaError_t e;
     if (small) {

@@ -216,46 +216,98 @@ int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const 
         P.partial_bytes = P.splits > 1 ? (size_t)P.splits * (size_t)P.M * 16 : 0;
         P.flops = 8.0 * (double)P.M * (double)P.K;
         P.bytes = 16.0 * ((double)sizeA + (double)sizeB + (double)sizeD * (e.accumulate ? 2.0 : 1.0));
+        P.est_seconds = std::max(P.flops / (37.2e12 * 0.92), P.bytes / 6.0e12) + 4e-6;
         *out = std::move(P);
         return TCB_OK;
     }
 
-    bool inplaceA = (sa.mmajor || sa.kmajor) && !opt.permute_always;
-    bool inplaceB = (sb.mmajor || sb.kmajor) && !opt.permute_always;
-    // (v) row operand whose fastest free index is not D's unit-stride index
-    if (inplaceA && !sa.free.empty() && !seqD.empty() && sa.free[0] != seqD[0] && sizeA <= sizeD) inplaceA = false;
-    // (iv) common contracted order
+    // (iii)-(viii) how each operand reaches the GEMM, decided by a cost model.  Per operand three feeds exist:
+    //   tma     : read in place by 2-D TMA boxes -- needs a matrix-shaped memory order whose contracted order is the common one;
+    //   gather  : read in place through a row table and a column table (any index order);
+    //   permute : copied into workspace as [contracted in the common order][free in D's order] first (TTGT).
+    // The common contracted order is A's or B's own.  A candidate costs  sum over passes of max(flops / peak, bytes / BW)
+    // (SURVEY 8(a) S2 (viii)); bytes count twice where only 16 of a 32-byte sector are used (no contiguous direction for the
+    // lanes of a gathered operand; epilogue stores that do not run along D's unit-stride index).
     auto same_order = [&](const std::vector<const Lab *> &x, const std::vector<const Lab *> &y) {
         if (x.size() != y.size()) return false;
         for (size_t i = 0; i < x.size(); ++i) if (x[i] != y[i]) return false;
         return true;
     };
+    std::vector<const Lab *> dorderA, dorderB;            // the free labels in D's order
+    for (const Lab *l : seqD) if (posA(l) >= 0) dorderA.push_back(l);
+    for (const Lab *l : seqD) if (posB(l) >= 0) dorderB.push_back(l);
+    struct Feed { int kind; std::vector<const Lab *> forder; bool mfast; double waste; };   // kind: 0 tma, 1 gather, 2 permute
+    auto feeds_of = [&](const Shape2 &s, const std::vector<const Lab *> &seq, const std::vector<const Lab *> &dorder,
+                        const std::vector<const Lab *> &corder, bool is_a) {
+        std::vector<Feed> f;
+        const bool matrix = (s.mmajor || s.kmajor) && same_order(s.con, corder);
+        if (matrix && !opt.permute_always) f.push_back({0, s.free, false, 1.0});
+        if (!opt.permute_always && opt.operand_loads != 2) {
+            const Lab *u = seq.empty() ? nullptr : seq[0];           // the operand's unit-stride index
+            auto gather = [&](const std::vector<const Lab *> &forder) {
+                bool mfast = false;
+                int64_t run = 1;
+                if (u && !is_con(u)) { mfast = !forder.empty() && forder[0] == u; run = mfast ? u->ext : 1; }
+                else if (u) run = (!corder.empty() && corder[0] == u) ? std::min<int64_t>(u->ext, 8) : 1;
+                f.push_back({1, forder, mfast, run >= 2 ? 1.0 : 2.0});
+            };
+            gather(is_a ? dorder : s.free);                          // A: rows in D's order (contiguous epilogue stores)
+            if (is_a && !same_order(dorder, s.free)) gather(s.free);  //    or in its own (contiguous loads)
+        }
+        if (opt.operand_loads != 1 || opt.permute_always) f.push_back({2, dorder, false, 1.0});
+        return f;
+    };
+    // achievable rates on a B200: 0.92 of the FP64 tensor peak, 5.5 TB/s for a transposition pass
+    const double kPeak = 37.2e12 * 0.92, kBw = 6.0e12, kBwPerm = 5.5e12, kLaunch = 4e-6;
+    // what the address arithmetic and the 4 x LDGSTS per thread and k-tile of a gathered operand cost the tensor pipe
+    const double kGatherCost = 1.005;
+    const double flops = 8.0 * (double)P.M * (double)P.N * (double)P.K;
+    const double bytesD = 16.0 * (double)sizeD * (e.accumulate ? 2.0 : 1.0);
+    std::vector<std::vector<const Lab *>> corders;
+    corders.push_back(sa.con);
+    if (!same_order(sa.con, sb.con)) corders.push_back(sb.con);
+    double best = -1.0;
+    Feed fa, fb;
     std::vector<const Lab *> corder;
-    if (inplaceA && inplaceB && !same_order(sa.con, sb.con)) {
-        if (sizeA <= sizeB) inplaceA = false; else inplaceB = false;
-    }
-    if (inplaceA) corder = sa.con;
-    else if (inplaceB) corder = sb.con;
-    else corder = sa.con.size() ? (sizeA >= sizeB ? sa.con : sb.con) : sb.con;
+    for (const auto &co : corders)
+        for (const Feed &ca : feeds_of(sa, seqA, dorderA, co, true))
+            for (const Feed &cb : feeds_of(sb, seqB, dorderB, co, false)) {
+                const double wd = (seqD.empty() || (!ca.forder.empty() && ca.forder[0] == seqD[0])) ? 1.0 : 2.0;
+                double fl = flops / kPeak;
+                if (ca.kind == 1) fl *= kGatherCost;
+                if (cb.kind == 1) fl *= kGatherCost;
+                const double by = (16.0 * (double)sizeA * ca.waste + 16.0 * (double)sizeB * cb.waste + bytesD * wd) / kBw;
+                double t = std::max(fl, by) + kLaunch;
+                // 16-byte scattered epilogue stores are not hidden behind the tensor work (one sector per lane instead of
+                // four lines per warp instruction): they cost their traffic on top (measured in round 1: permuting a row
+                // operand no larger than D first paid off)
+                if (wd > 1.0) t += bytesD / kBw;
+                if (ca.kind == 2) t += 32.0 * (double)sizeA / kBwPerm + kLaunch;
+                if (cb.kind == 2) t += 32.0 * (double)sizeB / kBwPerm + kLaunch;
+                if (best < 0 || t < best * (1.0 - 1e-9)) { best = t; fa = ca; fb = cb; corder = co; }
+            }
+    if (best < 0) return fail(TCB_EUNSUPPORTED, "no way to feed the operands under the given options");
+    P.est_seconds = best;
+    const std::vector<const Lab *> &forderA = fa.forder, &forderB = fb.forder;
 
-    // free order: in place -> the operand's own order; permuted -> D's order
-    std::vector<const Lab *> forderA, forderB;
-    if (inplaceA) forderA = sa.free;
-    else for (const Lab *l : seqD) if (posA(l) >= 0) forderA.push_back(l);
-    if (inplaceB) forderB = sb.free;
-    else for (const Lab *l : seqD) if (posB(l) >= 0) forderB.push_back(l);
-
-    auto fill_operand = [&](OperandPlan &o, bool inplace, const Shape2 &s, const std::vector<const Lab *> &seq,
-                            const std::vector<const Lab *> &forder, int64_t rows, auto strX) {
+    auto fill_operand = [&](OperandPlan &o, const Feed &f, const Shape2 &s, const std::vector<const Lab *> &seq,
+                            int64_t rows, auto strX, int which) {
         o.rows = rows;
         o.elems = rows * P.K;
-        o.permuted = !inplace;
-        if (inplace) {
+        o.permuted = f.kind == 2;
+        o.gather = f.kind == 1;
+        o.mfast = f.mfast;
+        if (f.kind == 0) {
             // K = 1: rows contiguous -> M-major; otherwise prefer what the memory order says
             if (s.con.empty()) { o.kmajor = false; o.ld = rows; }
             else if (s.free.empty()) { o.kmajor = true; o.ld = P.K; }
             else if (s.kmajor) { o.kmajor = true; o.ld = P.K; }
             else { o.kmajor = false; o.ld = rows; }
+        } else if (f.kind == 1) {
+            o.kmajor = true;                   // the layout the gathered k-tile has in shared memory
+            o.ld = P.K;
+            o.gather_row = offset_table(f.forder, which);
+            o.gather_k = offset_table(corder, which);
         } else {
             o.kmajor = true;
             o.ld = P.K;
@@ -264,16 +316,32 @@ int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const 
             int64_t st = 1;
             std::map<const Lab *, int64_t> target;
             for (const Lab *l : corder) { target[l] = st; st *= l->ext; }
-            for (const Lab *l : forder) { target[l] = st; st *= l->ext; }
+            for (const Lab *l : f.forder) { target[l] = st; st *= l->ext; }
             for (const Lab *l : seq) { ext[n] = l->ext; is[n] = strX(l); os[n] = target[l]; ++n; }
             o.perm = canonical_permutation(n, ext, is, os);
         }
     };
-    fill_operand(P.a, inplaceA, sa, seqA, forderA, P.M, strA);
-    fill_operand(P.b, inplaceB, sb, seqB, forderB, P.N, strB);
+    fill_operand(P.a, fa, sa, seqA, P.M, strA, swapped ? 2 : 1);
+    fill_operand(P.b, fb, sb, seqB, P.N, strB, swapped ? 1 : 2);
+
+    // (vi) epilogue: fused scatter (default), or -- "epilogue" = "twopass", the third pass of TTGT kept for
+    // A/B tests -- the GEMM writes a plain M x N matrix into workspace and a permute-accumulate pass brings it into D
+    P.twopass = opt.epilogue == 2;
+    if (P.twopass) {
+        int64_t ext[2 * kMaxRank], is[2 * kMaxRank], os[2 * kMaxRank];
+        int n = 0;
+        int64_t st = 1;
+        for (const Lab *l : forderA) { ext[n] = l->ext; is[n] = st; os[n] = l->sD; st *= l->ext; ++n; }
+        for (const Lab *l : forderB) { ext[n] = l->ext; is[n] = st; os[n] = l->sD; st *= l->ext; ++n; }
+        P.c_perm = canonical_permutation(n, ext, is, os);
+    }
 
     P.offM = offset_table(forderA);
     P.offN = offset_table(forderB);
+    if (P.twopass) {                       // C[m + n * M]
+        for (size_t m = 0; m < P.offM.size(); ++m) P.offM[m] = (int64_t)m;
+        for (size_t n = 0; n < P.offN.size(); ++n) P.offN[n] = (int64_t)n * P.M;
+    }
     for (const Lab *l : forderA) P.m_labels.push_back(l->name);
     for (const Lab *l : forderB) P.n_labels.push_back(l->name);
     for (const Lab *l : corder) P.k_labels.push_back(l->name);
@@ -293,16 +361,19 @@ int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const 
 
 std::string ContractPlan::describe() const
 {
-    char buf[1024];
+    char buf[1280];
+    auto feed = [&](const OperandPlan &o) { return gemv ? "table" : o.permuted ? "permute" : o.gather ? "gather" : "tma"; };
     std::snprintf(buf, sizeof buf,
                   "{\"M\": %lld, \"N\": %lld, \"K\": %lld, \"m_labels\": \"%s\", \"n_labels\": \"%s\", "
                   "\"k_labels\": \"%s\", \"row_operand\": \"%s\", \"permute_A\": %s, \"permute_B\": %s, "
-                  "\"A_layout\": \"%s\", \"B_layout\": \"%s\", \"splits\": %d, \"route\": \"%s\", \"epilogue\": \"fused-scatter\", "
-                  "\"accumulate\": %s, \"flops\": %.6g, \"bytes\": %.6g}",
+                  "\"A_layout\": \"%s\", \"B_layout\": \"%s\", \"feed_A\": \"%s\", \"feed_B\": \"%s\", \"splits\": %d, "
+                  "\"route\": \"%s\", \"epilogue\": \"%s\", \"accumulate\": %s, \"flops\": %.6g, \"bytes\": %.6g, "
+                  "\"est_us\": %.4g}",
                   (long long)M, (long long)N, (long long)K, join(m_labels).c_str(), join(n_labels).c_str(),
                   join(k_labels).c_str(), swapped ? "R" : "L", a.permuted ? "true" : "false",
                   b.permuted ? "true" : "false", a.kmajor ? "K-major" : "M-major", b.kmajor ? "K-major" : "M-major",
-                  splits, gemv ? "gemv" : "gemm", accumulate ? "true" : "false", flops, bytes);
+                  feed(a), feed(b), splits, gemv ? "gemv" : "gemm", twopass ? "twopass" : "fused-scatter",
+                  accumulate ? "true" : "false", flops, bytes, est_seconds * 1e6);
     return buf;
 }
 

@@ -19,7 +19,8 @@ struct Shape {
 
 struct PlanOptions {
     int splitk = 0;               // 0 = auto, 1 = off, n > 1 = forced
-    int epilogue = 0;             // 0 = auto, 1 = fused, 2 = two-pass (reserved)
+    int epilogue = 0;             // 0 = auto, 1 = fused, 2 = two-pass (GEMM into workspace + permute-accumulate pass)
+    int operand_loads = 0;        // 0 = auto (cost model), 1 = never permute (gather whatever TMA cannot read), 2 = never gather
     bool permute_always = false;  // A/B testing: permute both operands even when they are matrix-shaped
     bool static_deal = false;     // A/B testing: GEMM work dealt statically (tile c + w * grid) instead of claimed
 };
@@ -35,6 +36,9 @@ PermuteShape canonical_permutation(int rank, const int64_t *extent, const int64_
 
 struct OperandPlan {
     bool permuted = false;   // copied into workspace in K-major matrix form first
+    bool gather = false;     // read in place through gather_row / gather_k (element offsets into the operand)
+    bool mfast = false;      // gather: lanes run along the rows (the operand's unit-stride index leads the row order)
+    std::vector<int64_t> gather_row, gather_k;
     bool kmajor = false;     // layout the GEMM reads
     int64_t rows = 1, ld = 1, elems = 1;
     PermuteShape perm;       // valid when permuted
@@ -54,6 +58,9 @@ struct ContractPlan {
     size_t partial_bytes = 0; // workspace for the raw fragments of tiles cut along K
     std::vector<std::string> m_labels, n_labels, k_labels;
     double flops = 0, bytes = 0;
+    double est_seconds = 0;   // the cost model's estimate for the chosen candidate
+    bool twopass = false;     // epilogue: GEMM into a plain M x N workspace matrix, then c_perm brings it into D
+    PermuteShape c_perm;
     std::string describe() const;
 };
 

@@ -160,7 +160,7 @@ synth_mp2_kernel(double2 *T, const double2 *__restrict__ W, const double *__rest
 int grid_for(long long n)
 {
     long long b = (n + 255) / 256;
-    if (b > 148 * 16) b = 148 * 16;
+    if (b > tcb::sm_count() * 16LL) b = tcb::sm_count() * 16LL;
     return b < 1 ? 1 : (int)b;
 }
 

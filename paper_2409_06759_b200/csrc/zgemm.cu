@@ -23,19 +23,29 @@
 //     is an exact XOR on the high word).
 //   * persistent grid (2 CTAs per SM) with a stream-K schedule: whole tiles one CTA each while they fill the grid, the
 //     remainder wave -- or everything, for skinny M x N with long K -- cut along K into chunks whose raw accumulator
-//     fragments go to a workspace; zgemm_fixup_kernel sums a tile's chunks in k order (deterministic, no atomics on
-//     data) and applies the same scatter.  Tiles and chunks are claimed from two counters (dynamic deal).
+//     fragments go to a workspace; the CTA that delivers a tile's LAST chunk (a per-tile arrival counter) sums the
+//     tile's chunks in k order (deterministic, no atomics on data) and applies the same scatter, inside the same launch
+//     (zgemm_fixup_kernel remains for the static deal and for forced split-K with more cut tiles than counters).
+//     Tiles and chunks are claimed from two counters (dynamic deal).
 //   * the producer (thread 0) walks the CTA's segment list 4 k-tiles ahead of the consumers and ACROSS tile
 //     boundaries; segments reach the other warps through a small shared-memory queue.
 //   * no tensor work on padding: the 8-wide blocks of M and N are dealt to the tiles in pairs, a warp multiplies only
 //     the blocks it has (mma_ktile<MC, NC, KS>), the last k-tile of a K with <= 4 entries left does one k-step.
-//   * epilogue: read-modify-write software-pipelined one fragment column ahead; no FP64 multiplies for alpha = 1
-//     (the plain FP64 pipe shares its datapath with DMMA).
+//   * epilogue: '+=' is two red.global.add.f64 per element (the add happens in L2, the SM never waits for D; every
+//     element is touched by one thread, so the sum stays deterministic); no FP64 multiplies for alpha = 1 (the plain
+//     FP64 pipe shares its datapath with DMMA).
+//   * permutation-free operand loads (BSMTC / GETT): an operand that is not matrix-shaped
+//     in memory is NOT copied into a workspace first.  A tensor's element offset is a sum over its indices, so any
+//     operand is a matrix with a row table and a column table, A[m,k] = L[rowA[m] + colA[k]]; all 128 threads fetch
+//     their share of the k-tile with 16-byte cp.async (LDGSTS, zero-fill for the tails) straight into the same swizzled
+//     atoms the TMA path fills, completion counted on the same mbarrier (cp.async.mbarrier.arrive.noinc), so the
+//     consumer side does not know the difference.  Lanes run along whichever of m / k is contiguous in memory.
 // Measured history and the ncu evidence for each of these: DESIGN.md 6.2, profiles/r1b_zgemm_ncu_full.md.
 #include "kernels.h"
 
 #include <algorithm>
 #include <cstdlib>
+#include <cstring>
 #include <mutex>
 
 namespace tcb {
@@ -44,7 +54,6 @@ namespace {
 
 constexpr int BM = kGemmBM, BN = kGemmBN, BK = kGemmBK;
 constexpr int STAGES = 4;
-constexpr int kNumSMs = 148;            // B200; the persistent grid is 2 CTAs per SM
 constexpr int A_BYTES = BM * BK * 16;   // 8 KB
 constexpr int B_BYTES = BN * BK * 16;   // 8 KB
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
@@ -70,7 +79,13 @@ struct GemmParams {
     int accumulate, use_red;
     double2 *partial;              // [slot][32][128] raw accumulator fragments
     unsigned long long *counters;  // [3] whole tiles claimed, stream-K chunks claimed, CTAs done; zero at launch; null: static deal
+    unsigned *tile_cnt;            // [sk_tiles] chunks delivered per cut tile (zero at launch, left zero); null: fix-up kernel
+    // gathered operands (mode kGather): X[row, k] = base[rowtab[row] + ktab[k]]
+    const double2 *gA, *gB;
+    const long long *gAm, *gAk, *gBn, *gBk;
+    int a_mfast, b_mfast;          // lanes run along the rows (the operand's unit-stride index is free) or along k
 };
+enum { kTmaK = 0, kTmaM = 1, kGather = 2 };   // how an operand reaches shared memory
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -106,6 +121,49 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *tm,
         "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
         ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(bar)
         : "memory");
+}
+// 16-byte asynchronous copy global -> shared (LDGSTS), src_bytes = 0 writes zeros (tails)
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src, int src_bytes)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+// the mbarrier receives one arrival when all cp.async issued so far by this thread have landed
+__device__ __forceinline__ void cp_async_arrive(uint32_t bar)
+{
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
+// rows [row0, row0 + rows_in_tile) x k-tile k0 of a gathered operand into a stage, K-major atoms: element (m, k) of the
+// tile at (m >> 3) * 1024 + (m & 7) * 128 + ((k ^ (m & 7)) * 16) -- the layout a SWIZZLE_128B K-major TMA box produces
+__device__ __forceinline__ void gather_ktile(uint32_t sX, const double2 *base, const long long *rowtab, long long row0,
+                                             int rows_in_tile, long long rows_total, const long long *ktab, long long k0,
+                                             long long K, bool mfast, int tid)
+{
+    if (mfast) {
+        const int m = tid & 63;
+        if (m >= rows_in_tile) return;
+        const bool rok = row0 + m < rows_total;
+        const long long ro = rok ? __ldg(rowtab + row0 + m) : 0;
+        const uint32_t drow = sX + (m >> 3) * 1024 + (m & 7) * 128;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int kk = (tid >> 6) + 2 * j;
+            const bool ok = rok && k0 + kk < K;
+            const long long ko = ok ? __ldg(ktab + k0 + kk) : 0;
+            cp_async16(drow + ((kk ^ (m & 7)) * 16), base + ro + ko, ok ? 16 : 0);
+        }
+    } else {
+        const int kk = tid & 7;
+        const bool kok = k0 + kk < K;
+        const long long ko = kok ? __ldg(ktab + k0 + kk) : 0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int m = (tid >> 3) + 16 * j;
+            if (m >= rows_in_tile) continue;
+            const bool ok = kok && row0 + m < rows_total;
+            const long long ro = ok ? __ldg(rowtab + row0 + m) : 0;
+            cp_async16(sX + (m >> 3) * 1024 + (m & 7) * 128 + ((kk ^ (m & 7)) * 16), base + ro + ko, ok ? 16 : 0);
+        }
+    }
 }
 __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b)
 {
@@ -345,11 +403,45 @@ __device__ __forceinline__ void mma_ktile(double (&cr)[4][4][2], double (&ci)[4]
     }
 }
 
-template <bool A_KMAJOR, bool B_KMAJOR>
+// sums the chunks of cut tile `tl` in k order into the accumulator registers (same thread <-> element map as the
+// partial stores) -- shared by the in-kernel fix-up and, element-wise, by zgemm_fixup_kernel
+__device__ __forceinline__ void sum_tile_chunks(const GemmParams &p, long long tl, const WarpGeom &wg, int tid,
+                                                double (&cr)[4][4][2], double (&ci)[4][4][2])
+{
+    const long long base = tl * p.ktiles;
+    const long long ch_lo = base / p.sk_q, ch_hi = (base + p.ktiles - 1) / p.sk_q;
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            cr[i][j][0] = cr[i][j][1] = 0.0;
+            ci[i][j][0] = ci[i][j][1] = 0.0;
+        }
+    for (long long ch = ch_lo; ch <= ch_hi; ++ch) {
+        const long long first = (ch * p.sk_q) / p.ktiles;
+        const double2 *P = p.partial + (ch * p.sk_slots + (tl - first)) * (32LL * NTHREADS) + tid;
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+#pragma unroll
+                for (int h = 0; h < 2; ++h)
+                    if (i < wg.mcnt && j < wg.ncnt) {
+                        const double2 v = __ldcg(P + ((i * 4 + j) * 2 + h) * NTHREADS);     // written by other SMs: L2
+                        cr[i][j][h] += v.x;
+                        ci[i][j][h] += v.y;
+                    }
+    }
+}
+
+template <int AMODE, int BMODE>
 __global__ void __launch_bounds__(NTHREADS, 2)
 zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                   const __grid_constant__ GemmParams p)
 {
+    constexpr bool kAnyTma = AMODE != kGather || BMODE != kGather;
+    constexpr bool kAnyGather = AMODE == kGather || BMODE == kGather;
+    constexpr uint32_t kTmaBytes = (AMODE != kGather ? A_BYTES : 0) + (BMODE != kGather ? B_BYTES : 0);
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;   // full[s] at +8s, empty[s] at +8(STAGES+s)
@@ -359,12 +451,13 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 
     if (tid == 0) {
         for (int s = 0; s < STAGES; ++s) {
-            mbar_init(bar_base + 8 * s, 1);
+            // full: thread 0's expect_tx arrival for the TMA part + one cp.async arrival per thread for the gathered part
+            mbar_init(bar_base + 8 * s, (kAnyTma ? 1 : 0) + (kAnyGather ? NTHREADS : 0));
             mbar_init(bar_base + 8 * (STAGES + s), NTHREADS / 32);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
+        if (AMODE != kGather) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
+        if (BMODE != kGather) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
         *reinterpret_cast<volatile int *>(smem_raw + (bar_base - smem_u32(smem_raw)) + 128 + kQueue * sizeof(Segment)) = 0;
     }
     __syncthreads();
@@ -381,6 +474,7 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     // before its first operand load; the consumers pop them in order.  kQueue > STAGES + 1 entries suffice.
     Segment *q_seg = reinterpret_cast<Segment *>(smem_raw + (bar_base - smem_u32(smem_raw)) + 128);
     volatile int *q_pub = reinterpret_cast<volatile int *>(q_seg + kQueue);
+    volatile int *s_flag = q_pub + 1;   // "this CTA delivered the tile's last chunk" (in-kernel fix-up)
     int npub = 0;
     auto producer_advance = [&]() {
         pvalid = pit.next(p, &pseg);
@@ -394,30 +488,61 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             pm0 = t.m0; pn0 = t.n0; pk = pseg.kb;
         }
     };
-    auto issue = [&]() {              // loads k-tile pk of the producer's segment into stage pstage
-        const uint32_t bar = bar_base + 8 * pstage;
-        const uint32_t sA = smem_base + pstage * STAGE_BYTES, sB = sA + A_BYTES;
-        const int k0 = pk * BK;
-        mbar_expect_tx(bar, STAGE_BYTES);
-        if (A_KMAJOR) {
-            tma_load_2d(sA, &tmA, 2 * k0, pm0, bar);
-        } else {
+    auto issue = [&]() {              // loads k-tile pk of the producer's segment into stage pstage (TMA operands)
+        if (kAnyTma) {
+            const uint32_t bar = bar_base + 8 * pstage;
+            const uint32_t sA = smem_base + pstage * STAGE_BYTES, sB = sA + A_BYTES;
+            const int k0 = pk * BK;
+            mbar_expect_tx(bar, kTmaBytes);
+            if (AMODE == kTmaK) {
+                tma_load_2d(sA, &tmA, 2 * k0, pm0, bar);
+            } else if (AMODE == kTmaM) {
 #pragma unroll
-            for (int j = 0; j < BM / 8; ++j) tma_load_2d(sA + j * 1024, &tmA, 2 * (pm0 + 8 * j), k0, bar);
-        }
-        if (B_KMAJOR) {
-            tma_load_2d(sB, &tmB, 2 * k0, pn0, bar);
-        } else {
+                for (int j = 0; j < BM / 8; ++j) tma_load_2d(sA + j * 1024, &tmA, 2 * (pm0 + 8 * j), k0, bar);
+            }
+            if (BMODE == kTmaK) {
+                tma_load_2d(sB, &tmB, 2 * k0, pn0, bar);
+            } else if (BMODE == kTmaM) {
 #pragma unroll
-            for (int j = 0; j < BN / 8; ++j) tma_load_2d(sB + j * 1024, &tmB, 2 * (pn0 + 8 * j), k0, bar);
+                for (int j = 0; j < BN / 8; ++j) tma_load_2d(sB + j * 1024, &tmB, 2 * (pn0 + 8 * j), k0, bar);
+            }
         }
         if (++pstage == STAGES) { pstage = 0; pphase ^= 1; }
         if (++pk == pseg.ke) producer_advance();
+    };
+    // ---- gathered operands: EVERY thread walks the published segment list with its own cursor, in step with thread 0's,
+    // and fetches its share (4 x 16 bytes per operand and k-tile) of the same k-tile into the same stage
+    int gq = 0, gk = 0, gke = 0, gstage = 0, gm0 = 0, gn0 = 0, gmr = 0, gnr = 0;
+    uint32_t gphase = 0;
+    bool gvalid = false;
+    auto gather_enter = [&]() {       // moves the cursor into published segment gq
+        while (*q_pub <= gq) { }
+        __threadfence_block();
+        const Segment sg = q_seg[gq % kQueue];
+        gvalid = sg.tile >= 0;
+        if (gvalid) {
+            const TileGeom t = tile_geom(p, (unsigned)sg.tile);
+            gm0 = t.m0; gn0 = t.n0; gmr = t.mb * 8; gnr = t.nb * 8;
+            gk = sg.kb; gke = sg.ke;
+        }
+    };
+    auto gather_issue = [&]() {
+        const uint32_t sA = smem_base + gstage * STAGE_BYTES, sB = sA + A_BYTES;
+        const long long k0 = (long long)gk * BK;
+        if (AMODE == kGather) gather_ktile(sA, p.gA, p.gAm, gm0, gmr, p.M, p.gAk, k0, p.K, p.a_mfast != 0, tid);
+        if (BMODE == kGather) gather_ktile(sB, p.gB, p.gBn, gn0, gnr, p.N, p.gBk, k0, p.K, p.b_mfast != 0, tid);
+        cp_async_arrive(bar_base + 8 * gstage);
+        if (++gstage == STAGES) { gstage = 0; gphase ^= 1; }
+        if (++gk == gke) { ++gq; gather_enter(); }
     };
     if (tid == 0) {
         pit.init(p);
         producer_advance();
         for (int s = 0; s < STAGES && pvalid; ++s) issue();
+    }
+    if (kAnyGather) {
+        gather_enter();
+        for (int s = 0; s < STAGES && gvalid; ++s) gather_issue();
     }
 
     // per-lane fragment offsets inside a 1 KB atom, for the two k-steps of a stage
@@ -427,8 +552,8 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 #pragma unroll
     for (int ks = 0; ks < 2; ++ks) {
         const int k = ks * 4 + c;
-        offA[ks] = A_KMAJOR ? (rowmap * 128 + ((k ^ rowmap) * 16)) : (k * 128 + ((rowmap ^ k) * 16));
-        offB[ks] = B_KMAJOR ? (rowmap * 128 + ((k ^ rowmap) * 16)) : (k * 128 + ((rowmap ^ k) * 16));
+        offA[ks] = AMODE != kTmaM ? (rowmap * 128 + ((k ^ rowmap) * 16)) : (k * 128 + ((rowmap ^ k) * 16));
+        offB[ks] = BMODE != kTmaM ? (rowmap * 128 + ((k ^ rowmap) * 16)) : (k * 128 + ((rowmap ^ k) * 16));
     }
 
     Segment seg;
@@ -463,6 +588,11 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 // slower: the wait keeps the four warps of a CTA in step, which the shared DMMA pipe prefers.
                 mbar_wait(bar_base + 8 * (STAGES + pstage), pphase ^ 1);
                 issue();
+            }
+            if (kAnyGather && done >= 1 && gvalid) {
+                // the same refill for the gathered part (every thread waits for the stage to be drained)
+                mbar_wait(bar_base + 8 * (STAGES + gstage), gphase ^ 1);
+                gather_issue();
             }
             mbar_wait(bar_base + 8 * stage, phase);
             const uint32_t sA = smem_base + stage * STAGE_BYTES + wg.moff * 1024;
@@ -505,6 +635,27 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                     for (int h = 0; h < 2; ++h)
                         if (i < wg.mcnt && j < wg.ncnt)
                             P[((i * 4 + j) * 2 + h) * NTHREADS] = make_double2(cr[i][j][h], ci[i][j][h]);
+            if (p.tile_cnt) {
+                // in-kernel fix-up: the CTA that delivers the LAST chunk of a cut tile sums all of the tile's chunks in k
+                // order (fixed k-ranges, fixed order: the result does not depend on who that CTA is) and writes D
+                const long long tl = seg.tile - p.dp_tiles;
+                __threadfence();
+                __syncthreads();
+                if (tid == 0) {
+                    const long long base = tl * p.ktiles;
+                    const unsigned nch = (unsigned)((base + p.ktiles - 1) / p.sk_q - base / p.sk_q + 1);
+                    const unsigned old = atomicAdd(p.tile_cnt + tl, 1u);
+                    *s_flag = (old == nch - 1) ? 1 : 0;
+                    if (old == nch - 1) p.tile_cnt[tl] = 0;          // left zero for the next launch
+                }
+                __syncthreads();
+                if (*s_flag) {
+                    __threadfence();
+                    sum_tile_chunks(p, tl, wg, tid, cr, ci);
+                    store_fragment(p, cr, ci, tg, wg, rowmap, c);
+                }
+                __syncthreads();                                     // s_flag is reused by the next cut segment
+            }
         }
     }
     // counters[2] counts the CTAs that are done claiming; the last one leaves all three at zero for the next launch
@@ -621,18 +772,26 @@ cudaError_t encode_operand(CUtensorMap *tm, const void *ptr, int64_t rows, int64
 }
 
 
-template <bool AK, bool BK_>
+template <int AM, int BM_>
 cudaError_t launch_variant(const GemmTensorMaps &maps, const GemmParams &p, int grid, cudaStream_t stream)
 {
-    auto kern = zgemm_dmma_kernel<AK, BK_>;
-    static bool configured = false;
-    if (!configured) {
+    auto kern = zgemm_dmma_kernel<AM, BM_>;
+    if (first_use_on_device((const void *)kern)) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
         if (e != cudaSuccess) return e;
-        configured = true;
     }
     kern<<<grid, NTHREADS, SMEM_BYTES, stream>>>(maps.a, maps.b, p);
     return cudaGetLastError();
+}
+
+template <int AM>
+cudaError_t launch_b(int bmode, const GemmTensorMaps &maps, const GemmParams &p, int grid, cudaStream_t stream)
+{
+    switch (bmode) {
+    case kTmaK: return launch_variant<AM, kTmaK>(maps, p, grid, stream);
+    case kTmaM: return launch_variant<AM, kTmaM>(maps, p, grid, stream);
+    default: return launch_variant<AM, kGather>(maps, p, grid, stream);
+    }
 }
 
 }  // namespace
@@ -645,7 +804,7 @@ GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk)
     s.nt = (int)((nblocks + 7) / 8);
     s.ktiles = (int)((K + BK - 1) / BK);
     const int64_t tiles = (int64_t)s.mt * s.nt, KT = s.ktiles;
-    const int64_t slots = 2LL * kNumSMs;                 // resident CTAs
+    const int64_t slots = 2LL * sm_count();              // resident CTAs: the persistent grid is 2 per SM
     s.dp_tiles = tiles; s.sk_tiles = 0; s.sk_chunks = 0; s.sk_q = 1; s.sk_slots = 1; s.splits = 1;
     if (splitk > 1) {                                    // forced: every tile cut into ~splitk pieces
         s.dp_tiles = 0; s.sk_tiles = tiles;
@@ -682,10 +841,14 @@ GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk)
 
 cudaError_t encode_gemm_maps(const GemmDesc &g, GemmTensorMaps *maps)
 {
-    // a strided dimension of extent 1 still needs a legal stride: ld >= 1 always holds here
-    cudaError_t e = encode_operand(&maps->a, g.A, g.M, g.K, g.lda, g.a_kmajor, BM);
-    if (e != cudaSuccess) return e;
-    return encode_operand(&maps->b, g.B, g.N, g.K, g.ldb, g.b_kmajor, BN);
+    // a strided dimension of extent 1 still needs a legal stride: ld >= 1 always holds here; a gathered operand has no map
+    std::memset(maps, 0, sizeof *maps);
+    if (!g.gatherAm) {
+        cudaError_t e = encode_operand(&maps->a, g.A, g.M, g.K, g.lda, g.a_kmajor, BM);
+        if (e != cudaSuccess) return e;
+    }
+    if (!g.gatherBn) return encode_operand(&maps->b, g.B, g.N, g.K, g.ldb, g.b_kmajor, BN);
+    return cudaSuccess;
 }
 
 cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps, cudaStream_t stream,
@@ -717,16 +880,24 @@ cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps
     p.partial = (double2 *)g.partial;
     p.counters = (unsigned long long *)g.counters;      // zero on entry; the last CTA to leave zeroes them again
     if (sc.partial_bytes && !p.partial) return cudaErrorInvalidValue;
+    // the in-kernel fix-up needs the dynamic deal's counter block and one arrival counter per cut tile
+    p.tile_cnt = (p.counters && sc.sk_tiles > 0 && sc.sk_tiles <= kGemmTileCounters)
+                     ? reinterpret_cast<unsigned *>(reinterpret_cast<char *>(p.counters) + kGemmTileCounterOffset) : nullptr;
+    p.gA = (const double2 *)g.A; p.gB = (const double2 *)g.B;
+    p.gAm = (const long long *)g.gatherAm; p.gAk = (const long long *)g.gatherAk;
+    p.gBn = (const long long *)g.gatherBn; p.gBk = (const long long *)g.gatherBk;
+    p.a_mfast = g.a_mfast ? 1 : 0; p.b_mfast = g.b_mfast ? 1 : 0;
+    const int amode = g.gatherAm ? kGather : (g.a_kmajor ? kTmaK : kTmaM);
+    const int bmode = g.gatherBn ? kGather : (g.b_kmajor ? kTmaK : kTmaM);
     cudaError_t e;
-    if (g.a_kmajor)
-        e = g.b_kmajor ? launch_variant<true, true>(maps, p, sc.grid, stream)
-                       : launch_variant<true, false>(maps, p, sc.grid, stream);
-    else
-        e = g.b_kmajor ? launch_variant<false, true>(maps, p, sc.grid, stream)
-                       : launch_variant<false, false>(maps, p, sc.grid, stream);
+    switch (amode) {
+    case kTmaK: e = launch_b<kTmaK>(bmode, maps, p, sc.grid, stream); break;
+    case kTmaM: e = launch_b<kTmaM>(bmode, maps, p, sc.grid, stream); break;
+    default: e = launch_b<kGather>(bmode, maps, p, sc.grid, stream); break;
+    }
     if (e != cudaSuccess) return e;
     if (launches) ++*launches;
-    if (sc.sk_tiles > 0) {
+    if (sc.sk_tiles > 0 && !p.tile_cnt) {
         zgemm_fixup_kernel<<<dim3((unsigned)sc.sk_tiles, 8), NTHREADS, 0, stream>>>(p);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;

@@ -75,11 +75,40 @@ def test_row_operand_is_owner_of_unit_stride_index_of_D():
     assert p["row_operand"] == "R" and p["M"] == 9
 
 
-def test_ring_term_permutes_the_smaller_side_only_when_needed():
+def test_ring_term_reads_both_operands_in_place_through_offset_tables():
+    """neither operand of the ring term is matrix-shaped; TTGT would transpose both, the
+    cost model reads both in place (gather); "operand_loads=permute" gives the TTGT plan back for A/B tests."""
     o, v = 6, 14
-    p = plan("X(a,b,i,j)=T(a,c,i,k)*I(k,b,c,j)", (v, v, o, o), (v, v, o, o), (o, v, v, o))
+    e, shapes = "X(a,b,i,j)=T(a,c,i,k)*I(k,b,c,j)", ((v, v, o, o), (v, v, o, o), (o, v, v, o))
+    p = plan(e, *shapes)
     assert (p["M"], p["N"], p["K"]) == (o * v, o * v, o * v)
-    assert p["permute_A"] and p["permute_B"]              # neither is matrix-shaped
+    assert not p["permute_A"] and not p["permute_B"] and p["feed_A"] == "gather" and p["feed_B"] == "gather"
+    assert p["m_labels"] == "a,i"                          # rows in D's order: contiguous epilogue stores
+    p = plan(e, *shapes, "operand_loads=permute")
+    assert p["permute_A"] and p["permute_B"] and p["feed_A"] == "permute"
+    q = plan(e, *shapes, "operand_loads=gather")
+    assert q["feed_A"] == "gather" and q["est_us"] < p["est_us"]
+
+
+def test_cost_model_picks_per_operand_feeds():
+    """S2 (viii): candidates cost max(flops / peak, bytes / BW) per pass; matrix-shaped operands stay on TMA, a non-matrix
+    operand is gathered, and nothing is ever permuted under "auto" at CC sizes (o=30, v=150)."""
+    from paper_2409_06759_b200 import ccsd_contractions as cl
+    o, v = 30, 150
+    seen = set()
+    for e, sign, sd, sl, sr in cl.all_calls(o, v):
+        p = plan(e, sd, sl, sr)
+        assert not p["permute_A"] and not p["permute_B"], (e, p)
+        assert p["est_us"] > 0
+        seen.add((p["feed_A"], p["feed_B"]))
+    assert ("tma", "tma") in seen and any("gather" in fb for fb in seen)
+    # pp ladder: both in place by TMA, cost = the tensor-bound GEMM
+    p = plan("R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)", (v, v, o, o), (v, v, v, v), (v, v, o, o))
+    assert p["feed_A"] == "tma" and p["feed_B"] == "tma"
+    assert abs(p["est_us"] - 8.0 * 22500 * 900 * 22500 / (37.2e12 * 0.92) * 1e6) < 0.02 * p["est_us"]
+    # the two-pass epilogue is an option, never the default
+    assert p["epilogue"] == "fused-scatter"
+    assert plan("R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)", (v, v, o, o), (v, v, v, v), (v, v, o, o), "epilogue=twopass")["epilogue"] == "twopass"
 
 
 def test_offset_tables_reproduce_the_contraction():
@@ -137,7 +166,7 @@ def test_extent_one_indices_are_dropped_and_labels_may_be_long():
     # and column offset tables, nothing is permuted
     assert p["route"] == "gemv" and not p["permute_A"] and not p["permute_B"]
     p = plan("R(p1,x,h1,q)+=T(p1,e_1,y,h1)*F(e_1,x,q,y)", (70, 1, 9, 3), (70, 40, 1, 9), (40, 1, 3, 1))
-    assert (p["M"], p["N"], p["K"]) == (630, 3, 40) and p["route"] == "gemm" and p["permute_A"]
+    assert (p["M"], p["N"], p["K"]) == (630, 3, 40) and p["route"] == "gemm" and p["feed_A"] == "gather"
     p = plan("R(p1,x,h1)+=T(p1,y,h1,e_1)*F(e_1,x,y)", (70, 1, 9), (70, 1, 9, 40), (40, 1, 1))
     assert (p["M"], p["N"], p["K"]) == (630, 1, 40) and not p["permute_A"] and p["A_layout"] == "M-major"
 
