@@ -1,10 +1,11 @@
 #!/usr/bin/env python
 """bench.py -- one JSON line for the driver (contract in DESIGN.md "Measurement").
 
-A step = one pass of the whole hot path (S1-S7) over one batch of synthetic input: the full spin-orbital CCD
-residual of BASELINE.json configs[1] (o=20, v=80, complex128) issued call by call through the C ABI, i.e. 11
-contractions (S1-S5, four of them with operand permutations S3), 6 fused permute-sums (S6) and 3 adds (S7).
-metric = complex-FP64 contraction throughput, GFLOP/s with 8 real flop per complex multiply-add.
+A step = BASELINE.json configs[2], the largest single-GPU configuration: the CCSD particle-particle ladder
+    R(a,b,i,j) += 1/2 sum_cd V(a,b,c,d) T(c,d,i,j),   complex128, o=40, v=200   (40000 x 1600 x 40000; V = 25.6 GB)
+issued as ONE tcb_contract call through the C ABI ("timed as a single contraction including operand permutations": the
+planner finds none to do -- V and T are read in place by TMA).  metric = complex-FP64 contraction throughput, GFLOP/s with
+8 real flop per complex multiply-add; the GB/s half of BASELINE.json's metric (transposition) is `roofline_hbm`.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-extras]
 
@@ -25,29 +26,48 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-METRIC = "complex-FP64 contraction GFLOP/s (CCD residual, 8 flop per complex MAC)"
-O, V = 20, 80                                   # BASELINE.json configs[1]
-WORKLOAD = f"configs[1]: full spin-orbital CCD residual, complex128, o={O}, v={V}"
-# nominal FP64 tensor peak derived from unit counts: 148 SMs x 4 sub-partitions x one DMMA.8x8x4
-# (512 flop) per 16 cycles x 1.965 GHz; the register-resident DMMA loop (tcb_measure_fp64_tensor_peak) reaches 37.0.
+METRIC = "complex-FP64 contraction GFLOP/s (CCSD pp ladder, 8 flop per complex MAC)"
+O, V = 40, 200                                  # BASELINE.json configs[2]
+EXPR = "R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)"
+FLOPS_STEP = 8.0 * (V * V) ** 2 * (O * O)
+WORKLOAD = (f"configs[2]: CCSD pp ladder R(a,b,i,j) += 1/2 V(a,b,c,d) T(c,d,i,j), complex128, o={O}, v={V} "
+            f"({V * V} x {O * O} x {V * V}, V 25.6 GB read in place)")
+# nominal FP64 tensor peak derived from unit counts: SMs x 4 sub-partitions x one DMMA.8x8x4 (512 flop) per 16
+# cycles x max SM clock = 148 x 128 x 1.965 GHz.  bench.py also MEASURES the register-resident DMMA loop in the same process
+# (tcb_measure_fp64_tensor_peak) and prints it beside this figure.
 FP64_TENSOR_PEAK_TFLOPS = 148 * 128 * 1.965e9 * 1e-12
-# DRAM traffic of the 11 zgemm_dmma_kernel launches of one step, from the ncu --set full capture committed as
-# profiles/r1b_zgemm_ncu_full.md (2.751 GB read + 0.277 GB written); bench.py itself never runs under a profiler
-ZGEMM_DRAM_BYTES_PER_STEP = 3.028e9
-ZGEMM_LAUNCHES_PER_STEP = 11
+# DRAM traffic per launch of the dominant kernels, from the committed ncu --set full captures (bench.py never runs under a
+# profiler): profiles/r2_dram_traffic.json.txt, written from the .ncu-rep files named inside it
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_dram_traffic.json.txt")
 
 
-EVENT_EVERY = 5          # per-launch event pairs on every 5th timed step (see run_ours)
+def committed_traffic(key):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel `key` from the committed profile, or None"""
+    try:
+        with open(TRAFFIC_FILE) as f:
+            return json.load(f)[key]
+    except Exception:          # noqa: BLE001 -- no capture committed for this kernel
+        return None
+
+
+def hbm_peak():
+    """(GB/s, source): the driver-measured copy bandwidth, else the profiling guide's fallback"""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (driver-measured copy bandwidth)"
+        except Exception:      # noqa: BLE001
+            pass
+    return 6650.0, "fallback: B200_PROFILING.md measured copy bandwidth (MEASURED_PEAKS.json absent)"
 
 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the configs[2..4] context measurements")
-    ap.add_argument("--no-graph", action="store_true", help="issue every timed step call by call (no CUDA graph replay)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -66,7 +86,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.FIELDS}",
-                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                          "--format=csv,noheader,nounits", "-lms", "10"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -139,7 +159,7 @@ def run_ours(args, rank, world, local_rank):
     import numpy as np
     import torch
     import paper_2409_06759_b200 as pkg
-    from paper_2409_06759_b200 import ccd
+    from paper_2409_06759_b200 import synth
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; this library has no CPU fallback")
@@ -155,103 +175,98 @@ def run_ours(args, rank, world, local_rank):
         torch.cuda.synchronize()
 
     ctx = pkg.Context(local_rank)
-    B, T = make_ccd_inputs(ctx, O, V)
-    R = ctx.tensor_create((V, V, O, O))
-    flops_step = ccd.CCD_FLOPS(O, V)
-    ctx.set_option("kernel_timing", "off" if os.environ.get("TCB_BENCH_NO_KERNEL_TIMING") else "on")
+    seed, anti = synth.SEED0 + 3, ((0, 1), (2, 3))
+    Vt, Tt, Rt = ctx.tensor_create((V, V, V, V), zero=False), ctx.tensor_create((V, V, O, O), zero=False), \
+        ctx.tensor_create((V, V, O, O))
+    ctx.synth_normal(Vt, seed, 1, antisym=anti)
+    ctx.synth_normal(Tt, seed, 2, antisym=anti)
+    plan = ctx.plan_describe(EXPR, Rt, Vt, Tt)
 
     def step():
-        ccd.ccd_residual(ctx, B, T, R)
+        ctx.contract(EXPR, Rt, Vt, Tt, 0.5)
 
-    for _ in range(max(args.warmup, 3)):
+    warmup = max(args.warmup, 3)
+    for _ in range(warmup):
         step()
-    # The steps without event pairs replay a CUDA graph of the same call list (tcb_capture_begin/end: 35 kernel nodes,
-    # stream-ordered intermediates included; captured once, outside the timed region, like the plans): 7.18 instead of
-    # 7.27 ms per step.  --no-graph issues every step call by call.
-    graph, graph_note = None, None
-    if not args.no_graph:
-        ctx.set_option("kernel_timing", "off")
-        try:
-            ctx.capture_begin()
-            try:
-                step()
-            finally:
-                graph = ctx.capture_end()          # also closes the capture when step() raised
-            ctx.graph_launch(graph)
-            ctx.sync()
-        except pkg.TcbError as exc:                # not capturable on this box: every step call by call, and say so
-            graph, graph_note = None, f"capture failed ({exc}); "
     ctx.sync()
+    # the roofline denominator, measured in this process: register-resident DMMA.8x8x4 loop on every SM for 0.2 s
+    peak_sampler = ClockSampler(local_rank)
+    peak_sampler.start()
+    time.sleep(0.05)
+    tp0 = time.time()
+    peak_live = ctx.measure_fp64_tensor_peak(200.0)
+    ctx.sync()
+    peak_clocks = peak_sampler.stop(tp0, time.time())
+
+    # one kernel launch per step, so the per-launch event pairs (tcb_kernel_stats) serialise nothing: they stay on
+    ctx.set_option("kernel_timing", "on")
     ctx.kernel_stats_reset()
     sampler = ClockSampler(local_rank)
     sampler.start()
-    time.sleep(0.3)
+    time.sleep(0.2)
     barrier()
     l0, t0 = ctx.launch_count(), time.time()
-    # Per-launch CUDA event pairs (the live roofline figures) serialise consecutive launches: with them on every step
-    # the step is 2.1 % slower (7.42 vs 7.27 ms).  They are recorded on every EVENT_EVERY-th timed step only; `value` is
-    # the time of all K steps, sampled ones included.
-    sampled = 0
     ctx.timer_start()
-    for it in range(args.steps):
-        on = (it % EVENT_EVERY == 0) and not os.environ.get("TCB_BENCH_NO_KERNEL_TIMING")
-        sampled += 1 if on else 0
-        if on or graph is None:
-            ctx.set_option("kernel_timing", "on" if on else "off")
-            step()
-            ctx.set_option("kernel_timing", "off")
-        else:
-            ctx.graph_launch(graph)
+    for _ in range(args.steps):
+        step()
     ms = ctx.timer_stop()
     barrier()
     t1 = time.time()
     launches = ctx.launch_count() - l0
     clocks = sampler.stop(t0, t1)
-    stats = {k: ctx.kernel_stats(k) for k in ("zgemm", "permute", "permsum", "elementwise")}
+    zg = ctx.kernel_stats("zgemm")
     ctx.set_option("kernel_timing", "off")
-    if graph is not None:
-        ctx.graph_destroy(graph)
 
-    # ---- e2e: the same step through the C ABI with HOST buffers (pinned), copies inside the timed region ----
-    names = list(B.keys())
-    host_in = {k: torch.empty(B[k].size, dtype=torch.complex128).pin_memory() for k in names}
-    host_T = torch.empty(T.size, dtype=torch.complex128).pin_memory()
-    host_R = torch.empty(R.size, dtype=torch.complex128).pin_memory()
-    for k in names:
-        ctx.tensor_download_raw(B[k], host_in[k].data_ptr())
-    ctx.tensor_download_raw(T, host_T.data_ptr())
-    h2d = sum(B[k].nbytes for k in names) + T.nbytes
-    d2h = R.nbytes
+    # ---- the GB/s half of the metric: the dominant permutation kernel on a configs[4] transposition, same process ------
+    hbm, hbm_src = hbm_peak()
+    ctx.set_option("kernel_timing", "on")
+    tshape = (200, 200, 40, 40)
+    Lp, Dp = ctx.tensor_create(tshape, zero=False), ctx.tensor_create((40, 40, 200, 200), zero=False)
+    ctx.synth_index_linear(Lp)
+    for _ in range(3):
+        ctx.permute("D(i,j,a,b)=L(a,b,i,j)", Dp, Lp)
+    ctx.kernel_stats_reset()
+    for _ in range(20):
+        ctx.permute("D(i,j,a,b)=L(a,b,i,j)", Dp, Lp)
+    pm = ctx.kernel_stats("permute")
+    ctx.set_option("kernel_timing", "off")
+    Lp.destroy(); Dp.destroy()
+    pm_gbs = pm["bytes"] / (pm["ms"] * 1e-3) * 1e-9 if pm["ms"] > 0 else 0.0
 
-    # Two device copies of the inputs and a second context (its own stream) for the uploads: while step n computes
-    # on one copy, step n+1's inputs cross PCIe into the other.  Every step still uploads all of its inputs from
-    # pinned host memory and reads its result back, all inside the timed region.
+    # ---- e2e: the same step through the C ABI with HOST buffers (pinned), copies inside the timed region ---------------
+    # Every step uploads V (25.6 GB), T and R from pinned host memory and reads R back.  Two device copies of V and T and a
+    # second context (its own stream) for the uploads: while step n computes on one copy, step n+1's operands cross PCIe
+    # into the other.
+    host_V = torch.empty(Vt.size, dtype=torch.complex128).pin_memory()
+    host_T = torch.empty(Tt.size, dtype=torch.complex128).pin_memory()
+    host_R = torch.empty(Rt.size, dtype=torch.complex128).pin_memory()
+    host_Rin = torch.zeros(Rt.size, dtype=torch.complex128).pin_memory()
+    ctx.tensor_download_raw(Vt, host_V.data_ptr())
+    ctx.tensor_download_raw(Tt, host_T.data_ptr())
+    h2d, d2h = Vt.nbytes + Tt.nbytes + Rt.nbytes, Rt.nbytes
     ctx_up = pkg.Context(local_rank)
-    sets = [(B, T)]
-    B2 = {k: ctx.tensor_create(B[k].extents) for k in names}
-    T2 = ctx.tensor_create(T.extents)
-    sets.append((B2, T2))
-    up = [({k: ctx_up.tensor_wrap(Bs[k].extents, ctx.tensor_device_ptr(Bs[k])) for k in names},
-           ctx_up.tensor_wrap(Ts.extents, ctx.tensor_device_ptr(Ts))) for Bs, Ts in sets]
+    V2, T2 = ctx.tensor_create(Vt.extents, zero=False), ctx.tensor_create(Tt.extents, zero=False)
+    sets = [(Vt, Tt), (V2, T2)]
+    up = [(ctx_up.tensor_wrap(a.extents, ctx.tensor_device_ptr(a)), ctx_up.tensor_wrap(b.extents, ctx.tensor_device_ptr(b)))
+          for a, b in sets]
 
     def upload(which):
-        Bu, Tu = up[which]
-        for k in names:
-            ctx_up.tensor_upload_raw(Bu[k], host_in[k].data_ptr())
-        ctx_up.tensor_upload_raw(Tu, host_T.data_ptr())
+        ctx_up.tensor_upload_raw(up[which][0], host_V.data_ptr())
+        ctx_up.tensor_upload_raw(up[which][1], host_T.data_ptr())
 
     def e2e_run(nsteps):
         upload(0)
         ctx_up.sync()
         for n in range(nsteps):
             if n + 1 < nsteps:
-                upload((n + 1) % 2)                               # overlaps with this step's kernels
-            Bs, Ts = sets[n % 2]
-            ccd.ccd_residual(ctx, Bs, Ts, R)
-            ctx.tensor_download_raw(R, host_R.data_ptr())          # blocks until R is on the host
+                upload((n + 1) % 2)                               # overlaps with this step's kernel
+            Vs, Ts = sets[n % 2]
+            ctx.tensor_upload_raw(Rt, host_Rin.data_ptr())         # R_in travels too ('+=' reads it)
+            ctx.contract(EXPR, Rt, Vs, Ts, 0.5)
+            ctx.tensor_download_raw(Rt, host_R.data_ptr())         # blocks until R is on the host
             ctx_up.sync()
 
-    e2e_steps = max(3, min(args.steps, 10))
+    e2e_steps = max(3, min(args.steps, 5))
     e2e_run(2)
     barrier()
     ctx.timer_start()
@@ -260,71 +275,106 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     ctx_up.destroy()
     r_norm = float(torch.linalg.vector_norm(host_R).item())     # the step's result was really read back
+    del host_V
+    V2.destroy(); T2.destroy()
 
     ms, e2e_ms = max_over_ranks([ms, e2e_ms], dist, "cuda")
     ms_step = ms / args.steps
-    value = job_throughput(world, flops_step, ms_step)
-    e2e_value = job_throughput(world, flops_step, e2e_ms / e2e_steps)
+    value = job_throughput(world, FLOPS_STEP, ms_step)
+    e2e_value = job_throughput(world, FLOPS_STEP, e2e_ms / e2e_steps)
 
-    zg = stats["zgemm"]
     achieved = zg["flops"] / (zg["ms"] * 1e-3) * 1e-12 if zg["ms"] > 0 else 0.0
+    alg_bytes = zg["bytes"] / max(zg["launches"], 1)
     line = {
         "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "warmup": warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "complex128 (f64)", "data": "synthetic",
         "config": {"workload": WORKLOAD, "o": O, "v": V, "parallelism": "replicas only" if world > 1 else "1 gpu",
-                   "l2": "inputs larger than L2 (vvvv 655 MB, working set 0.9 GB vs 126 MB L2), no flush",
-                   "calls_per_step": "11 tcb_contract + 5 tcb_antisymmetrize + 3 tcb_add",
-                   "issue": ((graph_note or "") + "call by call" if graph is None else
-                             f"CUDA graph replay of the call list (tcb_capture_*), except the {sampled} steps that carry "
-                             "per-launch event pairs, which are issued call by call")},
+                   "l2": "inputs larger than L2 (V 25.6 GB, T and R 1.02 GB each vs 126 MB L2), no flush",
+                   "calls_per_step": "1 tcb_contract",
+                   "plan": {k: plan[k] for k in ("M", "N", "K", "feed_A", "feed_B", "A_layout", "B_layout", "splits", "epilogue")}},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "GFLOP/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_ms / e2e_steps, "steps": e2e_steps, "residual_norm": r_norm,
-                "pipelining": "uploads of step n+1 on a second stream overlap the kernels of step n (two device copies)"},
+                "pipelining": "V and T of step n+1 cross PCIe on a second stream while step n computes (two device copies)"},
         "gpu_launches": launches,
-        "roofline": {"bound": "tensor", "kernel": "zgemm_dmma_kernel (all 11 contractions of the step)",
+        "roofline": {"bound": "tensor", "kernel": "zgemm_dmma_kernel (the step's one launch: GEMM + fused permute-accumulate "
+                                                  "epilogue + in-kernel stream-K fix-up)",
                      "achieved": achieved, "peak": FP64_TENSOR_PEAK_TFLOPS, "unit": "TFLOP/s",
                      "frac": achieved / FP64_TENSOR_PEAK_TFLOPS,
-                     "peak_source": "derived FP64 DMMA peak 148 SM x 128 flop/clk x 1.965 GHz (MEASURED_PEAKS.json has "
-                                    "no FP64 figure; the register-resident DMMA loop measures 37.0)",
-                     "traffic": ZGEMM_DRAM_BYTES_PER_STEP / ZGEMM_LAUNCHES_PER_STEP,
-                     "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum per launch, mean over the 11 GEMM launches "
-                                     "of one step, ncu --set full capture in profiles/r1b_zgemm_ncu_full.md; algorithmic "
-                                     f"bytes per launch {zg['bytes'] / max(zg['launches'], 1):.4g}",
-                     "share_of_step": zg["ms"] / (ms_step * sampled) if ms > 0 and sampled else None,
-                     "sampling": f"per-launch event pairs on {sampled} of the {args.steps} timed steps (every "
-                                 f"{EVENT_EVERY}th): they serialise launches, +2.1 % on a step that carries them"},
-        "kernels": {k: {"launches": s["launches"], "ms_per_step": s["ms"] / max(sampled, 1),
-                        "tflops": s["flops"] / (s["ms"] * 1e-3) * 1e-12 if s["ms"] > 0 and s["flops"] else None,
-                        "gbs": s["bytes"] / (s["ms"] * 1e-3) * 1e-9 if s["ms"] > 0 else None} for k, s in stats.items()},
+                     "peak_source": "derived FP64 DMMA peak 148 SM x 128 flop/clk x 1.965 GHz (MEASURED_PEAKS.json has no FP64 "
+                                    "figure); peak_measured_live is the register-resident DMMA loop run in this process",
+                     "peak_measured_live": peak_live, "peak_measured_clocks": peak_clocks,
+                     "frac_of_measured_live": achieved / peak_live if peak_live else None,
+                     "algorithmic_flops_per_launch": zg["flops"] / max(zg["launches"], 1),
+                     "algorithmic_bytes_per_launch": alg_bytes,
+                     "avg_launch_ms": zg["ms"] / max(zg["launches"], 1), "launches_timed": zg["launches"],
+                     "traffic": committed_traffic("zgemm_configs2"),
+                     "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of this launch, read from the committed "
+                                     "ncu --set full summary profiles/r2_dram_traffic.json.txt (null: no capture committed)",
+                     "share_of_step": zg["ms"] / ms if ms > 0 else None},
+        "roofline_hbm": {"bound": "hbm", "kernel": "permute_kernel: configs[4] transposition D(i,j,a,b) = L(a,b,i,j) of a "
+                                                   "(200,200,40,40) complex128 tensor (1.02 GB), 20 launches",
+                         "achieved": pm_gbs, "peak": hbm, "unit": "GB/s", "frac": pm_gbs / hbm, "peak_source": hbm_src,
+                         "algorithmic_bytes_per_launch": pm["bytes"] / max(pm["launches"], 1),
+                         "avg_launch_ms": pm["ms"] / max(pm["launches"], 1),
+                         "traffic": committed_traffic("permute_1gb")},
     }
-    return ctx, line
+    return ctx, (Vt, Tt, Rt), line
 
 
 # ---------------------------------------------------------------------------------------------------------
 # CPU oracle legs (the only places bench.py may execute oracle/)
 # ---------------------------------------------------------------------------------------------------------
-def oracle_sample(n_cols=24):
-    """The oracle as it stands (order A nested loops, double accumulators, OpenMP) on a bounded sample of
-    configs[1]: the pp-ladder contraction R(a,b,i,j) += 1/2 vvvv(a,b,c,d) T(c,d,i,j) -- 60 % of the step's flops --
-    restricted to n_cols of the o*o = 400 (i,j) columns of R.  Returns (GFLOP/s, seconds, cores, text)."""
+def oracle_sample(n_rows=80, t_cache={}):
+    """The oracle as it stands (order A nested loops, double accumulators, OpenMP) on a bounded sample of configs[2]:
+    the same contraction restricted to n_rows of the v*v = 40 000 (a,b) rows of R (all 1 600 columns, all of K).
+    Returns (GFLOP/s, seconds, cores, text)."""
+    import numpy as np
+    import oracle
+    rng = np.random.default_rng(0)
+    # the sample's VALUES do not matter for timing (dense loops, no data-dependent work): random stand-ins of the exact
+    # shapes, so that no 200^4 tensor has to be generated by the slow host generator
+    if "T" not in t_cache:
+        Tt = np.empty((V, V, O, O), dtype=np.complex128, order="F")
+        Tt.real = rng.standard_normal(Tt.shape)
+        Tt.imag = rng.standard_normal(Tt.shape)
+        t_cache["T"] = Tt
+    Tt = t_cache["T"]
+    Vs = np.asfortranarray(rng.standard_normal((1, n_rows, V, V)) + 1j * rng.standard_normal((1, n_rows, V, V)))
+    Rs = np.zeros((1, n_rows, O, O), dtype=np.complex128, order="F")
+    t0 = time.time()
+    oracle.contract_inplace_double(EXPR, Rs, Vs, Tt, 0.5)
+    dt = time.time() - t0
+    flops = 8.0 * n_rows * (O * O) * (V * V)
+    return flops / dt * 1e-9, dt, oracle.num_threads(), \
+        f"configs[2] ladder on {n_rows} of the {V * V} (a,b) rows of R ({flops:.3g} flop, {dt:.1f} s)"
+
+
+def oracle_check(ctx, tensors, n=8):
+    """cpu_baseline leg, part two: the oracle (long-double accumulators) on n^4 sampled outputs of the step the GPU just
+    ran -- its operands regenerated on the host by the index-keyed twin of the device generator, nothing read back from
+    the device but R -- gives the line's max_norm_err (north_star: <= 1e-11)."""
     import numpy as np
     import oracle
     from paper_2409_06759_b200 import synth
-    rng = np.random.default_rng(0)
-    # the sample's VALUES do not matter for timing (dense loops, no data-dependent work): random stand-ins of the
-    # exact shapes, so that no 80^4 tensor has to be generated by the slow host generator
-    Vt = np.asfortranarray(rng.standard_normal((V, V, V, V)) + 1j * rng.standard_normal((V, V, V, V)))
-    Tt = np.asfortranarray(rng.standard_normal((V, V, n_cols, 1)) + 1j * rng.standard_normal((V, V, n_cols, 1)))
-    Rt = np.zeros((V, V, n_cols, 1), dtype=np.complex128, order="F")
-    expr = "R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)"
-    t0 = time.time()
-    oracle.contract_inplace_double(expr, Rt, Vt, Tt, 0.5)
-    dt = time.time() - t0
-    flops = 8.0 * V ** 4 * n_cols
-    return flops / dt * 1e-9, dt, oracle.num_threads(), \
-        f"pp ladder of configs[1] on {n_cols} of {O * O} (i,j) columns of R ({flops:.3g} flop, {dt:.1f} s)"
+    Vt, Tt, Rt = tensors
+    seed, anti = synth.SEED0 + 3, ((0, 1), (2, 3))
+    rng = np.random.default_rng(11)
+    pa, pb = np.sort(rng.choice(V, n, replace=False)), np.sort(rng.choice(V, n, replace=False))
+    pi, pj = np.sort(rng.choice(O, n, replace=False)), np.sort(rng.choice(O, n, replace=False))
+    full = np.arange(V)
+    hV = synth.tensor(seed, 1, [V] * 4, antisym=anti, sub=[pa, pb, full, full])
+    hT = synth.tensor(seed, 2, [V, V, O, O], antisym=anti, sub=[full, full, pi, pj])
+    ctx.tensor_fill(Rt, 0.0)
+    ctx.contract(EXPR, Rt, Vt, Tt, 0.5)
+    got = ctx.tensor_download(Rt)[np.ix_(pa, pb, pi, pj)]
+    ref, sn = oracle.contract(EXPR, np.zeros((n, n, n, n)), hV, hT, 0.5)
+    nz = sn > 0
+    err = float(np.max(np.abs(got - ref)[nz] / sn[nz]))
+    exact = bool(np.array_equal(got[~nz], ref[~nz]))
+    return {"max_norm_err": err, "outputs_checked": int(got.size), "zero_norm_outputs_exact": exact,
+            "tolerance": 1e-11}
 
 
 def run_reference(args, rank):
@@ -332,10 +382,9 @@ def run_reference(args, rank):
         return None
     vals, cores, sample = [], 0, ""
     for _ in range(args.warmup):
-        oracle_sample(2)
-    t0 = time.time()
+        oracle_sample(8)
     for _ in range(args.steps):
-        g, dt, cores, sample = oracle_sample(8)
+        g, dt, cores, sample = oracle_sample(80)
         vals.append((g, dt))
     total = sum(dt for _, dt in vals)
     gf = sum(g * dt for g, dt in vals) / total
@@ -396,26 +445,66 @@ def run_extras(ctx):
         ctx.sync()
     except Exception as e:          # noqa: BLE001
         out.append({"workload": "configs[0]", "error": str(e)})
-    try:    # configs[2]
-        o, v = 40, 200
-        Vt, Tt, Rt = ctx.tensor_create((v, v, v, v)), ctx.tensor_create((v, v, o, o)), ctx.tensor_create((v, v, o, o))
-        ctx.synth_normal(Vt, 20240909, 1, antisym=((0, 1), (2, 3)))
-        ctx.synth_normal(Tt, 20240909, 2, antisym=((0, 1), (2, 3)))
-        expr = "R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)"
-        b, m = best_of(lambda: ctx.contract(expr, Rt, Vt, Tt, 0.5), 3)
-        fl = 8.0 * (v * v) ** 2 * o * o
-        out.append({"workload": "configs[2]: CCSD pp ladder o=40 v=200 (40000x1600x40000, V 25.6 GB in place)",
-                    "ms": b, "ms_median": m, "tflops": fl / b * 1e-9, "frac_fp64_tensor_peak": fl / b * 1e-9 / FP64_TENSOR_PEAK_TFLOPS})
-        Tp = ctx.tensor_create((o, o, v, v))
-        expr2 = "R(a,b,i,j)+=V(a,b,c,d)*T(i,j,c,d)"
-        b, m = best_of(lambda: ctx.contract(expr2, Rt, Vt, Tp, 0.5), 2)
-        out.append({"workload": "configs[2] variant T(i,j,c,d)", "ms": b, "tflops": fl / b * 1e-9,
-                    "frac_fp64_tensor_peak": fl / b * 1e-9 / FP64_TENSOR_PEAK_TFLOPS})
-        for t in (Vt, Tt, Rt, Tp):
+    try:    # configs[1]: the whole CCD residual (every S row: contractions, gathered operands, permute-sums, adds), lanes + graph
+        from paper_2409_06759_b200 import ccd
+        o, v = 20, 80
+        B, T = make_ccd_inputs(ctx, o, v)
+        R = ctx.tensor_create((v, v, o, o))
+        for _ in range(3):
+            ccd.ccd_residual(ctx, B, T, R)
+        ctx.sync()
+        l0 = ctx.launch_count()
+        ctx.capture_begin()
+        ccd.ccd_residual(ctx, B, T, R)
+        g = ctx.capture_end()
+        per_step = ctx.launch_count() - l0
+        info = ctx.graph_info(g)
+        b_graph, m_graph = best_of(lambda: [ctx.graph_launch(g) for _ in range(10)], 5)
+        b_eager, _ = best_of(lambda: [ccd.ccd_residual(ctx, B, T, R) for _ in range(10)], 3)
+        b_chain, _ = best_of(lambda: [ccd.ccd_residual(ctx, B, T, R, lanes=False) for _ in range(10)], 3)
+        ctx.graph_destroy(g)
+        ctx.set_option("kernel_timing", "on")
+        ctx.kernel_stats_reset()
+        ccd.ccd_residual(ctx, B, T, R, lanes=False)
+        classes = {k: ctx.kernel_stats(k) for k in ("zgemm", "permute", "permsum", "elementwise")}
+        ctx.set_option("kernel_timing", "off")
+        fl = ccd.CCD_FLOPS(o, v)
+        out.append({"workload": "configs[1]: full spin-orbital CCD residual o=20 v=80 (11 contractions, 5 permute-sums, 3 adds)",
+                    "ms_graph_replay": b_graph / 10, "ms_graph_replay_median": m_graph / 10, "ms_call_by_call_lanes": b_eager / 10,
+                    "ms_call_by_call_one_lane": b_chain / 10, "tflops": fl / (b_graph / 10) * 1e-9,
+                    "frac_fp64_tensor_peak": fl / (b_graph / 10) * 1e-9 / FP64_TENSOR_PEAK_TFLOPS,
+                    "launches_per_step": per_step, "graph": info,
+                    "one_lane_ms_by_class": {k: c["ms"] for k, c in classes.items()},
+                    "one_lane_launches_by_class": {k: c["launches"] for k, c in classes.items()},
+                    "one_lane_gbs_by_class": {k: (c["bytes"] / c["ms"] * 1e-6 if c["ms"] > 0 else None) for k, c in classes.items()}})
+        for t in list(B.values()) + [T, R]:
             t.destroy()
         ctx.sync()
+    except Exception as e:          # noqa: BLE001
+        out.append({"workload": "configs[1]", "error": str(e)})
+    try:    # configs[2] variants: "including operand permutations" -- T given as T(i,j,c,d), V as V(c,d,a,b), and TTGT forced
+        o, v = 40, 200
+        Vt, Rt = ctx.tensor_create((v, v, v, v), zero=False), ctx.tensor_create((v, v, o, o))
+        ctx.synth_normal(Vt, 20240909, 1, antisym=((0, 1), (2, 3)))
+        fl = 8.0 * (v * v) ** 2 * o * o
+        for expr, tshape, opt in (("R(a,b,i,j)+=V(a,b,c,d)*T(i,j,c,d)", (o, o, v, v), None),
+                                  ("R(a,b,i,j)+=V(c,d,a,b)*T(c,d,i,j)", (v, v, o, o), None),
+                                  ("R(a,b,i,j)+=V(a,b,c,d)*T(c,i,d,j)", (v, o, v, o), None),
+                                  ("R(a,b,i,j)+=V(a,b,c,d)*T(c,i,d,j)", (v, o, v, o), "permute")):
+            Tp = ctx.tensor_create(tshape, zero=False)
+            ctx.synth_normal(Tp, 20240909, 2)
+            ctx.set_option("operand_loads", opt or "auto")
+            plan = ctx.plan_describe(expr, Rt, Vt, Tp)
+            b, m = best_of(lambda: ctx.contract(expr, Rt, Vt, Tp, 0.5), 3)
+            ctx.set_option("operand_loads", "auto")
+            out.append({"workload": f"configs[2] variant {expr}" + (f" [operand_loads={opt}]" if opt else ""), "ms": b,
+                        "ms_median": m, "tflops": fl / b * 1e-9, "frac_fp64_tensor_peak": fl / b * 1e-9 / FP64_TENSOR_PEAK_TFLOPS,
+                        "feed_A": plan["feed_A"], "feed_B": plan["feed_B"]})
+            Tp.destroy()
+        Vt.destroy(); Rt.destroy()
+        ctx.sync()
     except Exception as e:          # noqa: BLE001 -- context numbers must never break the bench line
-        out.append({"workload": "configs[2]", "error": str(e)})
+        out.append({"workload": "configs[2] variants", "error": str(e)})
     try:    # configs[3]
         from paper_2409_06759_b200 import ccd
         o, v = 12, 60
@@ -594,13 +683,16 @@ def main():
         if line is not None:
             print(json.dumps(line), flush=True)
         return
-    ctx, line = run_ours(args, rank, world, local_rank)
+    ctx, tensors, line = run_ours(args, rank, world, local_rank)
     if rank == 0 and world == 1:
         if not args.no_cpu_baseline:
-            g, dt, cores, sample = oracle_sample(96)
+            g, dt, cores, sample = oracle_sample(400)
             line["cpu_baseline"] = {"value": g, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample}
-        if not args.no_extras:
-            line["other_workloads"] = run_extras(ctx)
+            line["cpu_baseline"].update(oracle_check(ctx, tensors))
+    for t in tensors:
+        t.destroy()
+    if rank == 0 and world == 1 and not args.no_extras:
+        line["other_workloads"] = run_extras(ctx)
     ctx.destroy()
     if world > 1:
         import torch.distributed as dist

@@ -197,12 +197,13 @@ int tcb_measure_fp64_vector_peak(tcb_ctx *ctx, double milliseconds, double *tflo
  * while the graph is used; so must the context's workspace: tcb_graph_launch returns TCB_EINVAL when a later call has
  * made the workspace grow (its old block, whose address the graph carries, is gone) -- capture again.
  * tcb_launch_count advances by the captured launches per replay.  tcb_graph_info: nodes and dependency edges of the
- * graph (a chain has edges = nodes - 1; parallel branches show as more) and the kernel launches per replay. */
+ * graph, the kernel launches per replay, and depth = the number of nodes on the longest dependency path (a chain has
+ * depth = nodes; parallel branches make it smaller).  Any output pointer may be NULL. */
 typedef struct tcb_graph tcb_graph;
 int tcb_capture_begin(tcb_ctx *ctx);
 int tcb_capture_end(tcb_ctx *ctx, tcb_graph **graph);
 int tcb_graph_launch(tcb_ctx *ctx, tcb_graph *graph);
-int tcb_graph_info(const tcb_graph *graph, int64_t *nodes, int64_t *edges, int64_t *kernel_launches);
+int tcb_graph_info(const tcb_graph *graph, int64_t *nodes, int64_t *edges, int64_t *kernel_launches, int64_t *depth);
 int tcb_graph_destroy(tcb_graph *graph);
 /* Milliseconds between two points of the context's stream: tcb_timer_start / tcb_timer_stop bracket the
  * calls in between with CUDA events on that stream; stop blocks and returns the elapsed time. */

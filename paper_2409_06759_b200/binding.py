@@ -93,7 +93,7 @@ def load_library():
         "tcb_capture_end": [vp, ctypes.POINTER(vp)],
         "tcb_graph_launch": [vp, vp],
         "tcb_graph_destroy": [vp],
-        "tcb_graph_info": [vp, i64p, i64p, i64p],
+        "tcb_graph_info": [vp, i64p, i64p, i64p, i64p],
         "tcb_lane_count": [],
         "tcb_lane_set": [vp, ctypes.c_int],
         "tcb_lane_wait": [vp, ctypes.c_int, ctypes.c_int],
@@ -354,9 +354,9 @@ class Context:
 
     def graph_info(self, g):
         """{'nodes', 'edges', 'launches'} of a captured graph"""
-        n, e, k = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
-        self._check(self.lib.tcb_graph_info(g, ctypes.byref(n), ctypes.byref(e), ctypes.byref(k)))
-        return {"nodes": n.value, "edges": e.value, "launches": k.value}
+        n, e, k, d = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
+        self._check(self.lib.tcb_graph_info(g, ctypes.byref(n), ctypes.byref(e), ctypes.byref(k), ctypes.byref(d)))
+        return {"nodes": n.value, "edges": e.value, "launches": k.value, "depth": d.value}
 
     def lane_count(self):
         return int(self.lib.tcb_lane_count())

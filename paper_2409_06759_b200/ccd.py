@@ -20,41 +20,66 @@ I4(a,d)     = oovv(k,l,c,d)*T(a,c,l,k) ; X(a,b,i,j) = I4(a,d)*T(d,b,i,j) ; R -= 
 """
 
 
-def ccd_residual(ctx, B, T, R=None):
+def ccd_residual(ctx, B, T, R=None, lanes=True):
     """B: dict name -> Tensor for foo, fvv, vvoo, oovv, oooo, vvvv, ovvo;  T: Tensor (v,v,o,o).
-    Returns the residual tensor R (v,v,o,o); all work is enqueued on the context's stream."""
+    Returns the residual tensor R (v,v,o,o); all work is enqueued on the context (lane 0 holds the result).
+
+    lanes: the intermediates that do not depend on one another are built side by side (DLTC layers,
+    PAPER.md:79, instead of the barrier after every operation of PAPER.md:400): lane 1 builds I3, I4 and their X tensors
+    (skinny, long-K contractions that leave most of the tensor pipe idle), lane 2 builds I2 and the ring term's X, lane 0
+    does the Fock terms, the two ladders, and every update of R (updates of one tensor stay on one lane, in order)."""
     v, _, o, _ = T.extents
+    use_lanes = lanes and hasattr(ctx, "lane_set")
+    lane = ctx.lane_set if use_lanes else (lambda l: None)
+    wait = ctx.lane_wait if use_lanes else (lambda l, m: None)
+    new = lambda shape: ctx.tensor_create(shape, zero=False)   # every intermediate below is first written by an '=' call
     if R is None:
-        R = ctx.tensor_create((v, v, o, o), zero=False)
-    X = ctx.tensor_create((v, v, o, o), zero=False)          # every intermediate below is first written by an '=' call
+        R = new((v, v, o, o))
+    wait(1, 0)
+    wait(2, 0)
+    # ---- lane 2: I2 and the ring term ------------------------------------------------------------------------------------
+    lane(2)
+    I2 = new((o, v, v, o))
+    ctx.add("I2(k,b,c,j)=W(k,b,c,j)", I2, B["ovvo"], 1.0)
+    ctx.contract("I2(k,b,c,j)+=W(k,l,c,d)*T(b,d,j,l)", I2, B["oovv"], T, 0.5)
+    X2 = new((v, v, o, o))
+    ctx.contract("X(a,b,i,j)=T(a,c,i,k)*I2(k,b,c,j)", X2, T, I2, 1.0)
+    I2.destroy()
+    # ---- lane 1: the two skinny intermediates and their terms ------------------------------------------------------------
+    lane(1)
+    I3 = new((o, o))
+    ctx.contract("I3(l,i)=W(k,l,c,d)*T(d,c,i,k)", I3, B["oovv"], T, 1.0)
+    X3 = new((v, v, o, o))
+    ctx.contract("X(a,b,i,j)=T(a,b,l,j)*I3(l,i)", X3, T, I3, 1.0)
+    I3.destroy()
+    I4 = new((v, v))
+    ctx.contract("I4(a,d)=W(k,l,c,d)*T(a,c,l,k)", I4, B["oovv"], T, 1.0)
+    X4 = new((v, v, o, o))
+    ctx.contract("X(a,b,i,j)=I4(a,d)*T(d,b,i,j)", X4, I4, T, 1.0)
+    I4.destroy()
+    # ---- lane 0: driver, Fock terms, ladders, and every update of R ------------------------------------------------------
+    lane(0)
+    X = new((v, v, o, o))
     ctx.add("R(a,b,i,j)=W(a,b,i,j)", R, B["vvoo"], 1.0)
     ctx.contract("X(a,b,i,j)=T(a,c,i,j)*f(b,c)", X, T, B["fvv"], 1.0)
     ctx.antisymmetrize("P(ab):R(a,b,i,j)+=X(a,b,i,j)", R, X, 1.0)
     ctx.contract("X(a,b,i,j)=T(a,b,i,k)*f(k,j)", X, T, B["foo"], 1.0)
     ctx.antisymmetrize("P(ij):R(a,b,i,j)+=X(a,b,i,j)", R, X, -1.0)
-    I1 = ctx.tensor_create((o, o, o, o), zero=False)
+    X.destroy()
+    I1 = new((o, o, o, o))
     ctx.add("I1(k,l,i,j)=W(k,l,i,j)", I1, B["oooo"], 1.0)
     ctx.contract("I1(k,l,i,j)+=W(k,l,c,d)*T(c,d,i,j)", I1, B["oovv"], T, 0.5)
     ctx.contract("R(a,b,i,j)+=T(a,b,k,l)*I1(k,l,i,j)", R, T, I1, 0.5)
     I1.destroy()
     ctx.contract("R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)", R, B["vvvv"], T, 0.5)
-    I2 = ctx.tensor_create((o, v, v, o), zero=False)
-    ctx.add("I2(k,b,c,j)=W(k,b,c,j)", I2, B["ovvo"], 1.0)
-    ctx.contract("I2(k,b,c,j)+=W(k,l,c,d)*T(b,d,j,l)", I2, B["oovv"], T, 0.5)
-    ctx.contract("X(a,b,i,j)=T(a,c,i,k)*I2(k,b,c,j)", X, T, I2, 1.0)
-    I2.destroy()
-    ctx.antisymmetrize("P(ij)P(ab):R(a,b,i,j)+=X(a,b,i,j)", R, X, 1.0)
-    I3 = ctx.tensor_create((o, o), zero=False)
-    ctx.contract("I3(l,i)=W(k,l,c,d)*T(d,c,i,k)", I3, B["oovv"], T, 1.0)
-    ctx.contract("X(a,b,i,j)=T(a,b,l,j)*I3(l,i)", X, T, I3, 1.0)
-    I3.destroy()
-    ctx.antisymmetrize("P(ij):R(a,b,i,j)+=X(a,b,i,j)", R, X, -0.5)
-    I4 = ctx.tensor_create((v, v), zero=False)
-    ctx.contract("I4(a,d)=W(k,l,c,d)*T(a,c,l,k)", I4, B["oovv"], T, 1.0)
-    ctx.contract("X(a,b,i,j)=I4(a,d)*T(d,b,i,j)", X, I4, T, 1.0)
-    I4.destroy()
-    ctx.antisymmetrize("P(ab):R(a,b,i,j)+=X(a,b,i,j)", R, X, -0.5)
-    X.destroy()
+    wait(0, 2)
+    ctx.antisymmetrize("P(ij)P(ab):R(a,b,i,j)+=X(a,b,i,j)", R, X2, 1.0)
+    X2.destroy()
+    wait(0, 1)
+    ctx.antisymmetrize("P(ij):R(a,b,i,j)+=X(a,b,i,j)", R, X3, -0.5)
+    ctx.antisymmetrize("P(ab):R(a,b,i,j)+=X(a,b,i,j)", R, X4, -0.5)
+    X3.destroy()
+    X4.destroy()
     return R
 
 

@@ -1103,7 +1103,7 @@ struct tcb_graph {
     cudaGraphExec_t exec = nullptr;
     int64_t launches = 0;
     uint64_t ws_generation = 0;      // the workspace blocks whose addresses the kernels of this graph carry
-    size_t nodes = 0, edges = 0;
+    size_t nodes = 0, edges = 0, depth = 0;   // depth: nodes on the longest dependency path (= nodes for a chain)
 };
 
 int tcb_capture_begin(tcb_ctx *ctx)
@@ -1158,6 +1158,23 @@ int tcb_capture_end(tcb_ctx *ctx, tcb_graph **out)
     }
     cudaGraphGetNodes(g->graph, nullptr, &g->nodes);
     cudaGraphGetEdges(g->graph, nullptr, nullptr, &g->edges);
+    {   // longest dependency path, in nodes
+        std::vector<cudaGraphNode_t> nd(g->nodes), from(g->edges), to(g->edges);
+        size_t nn = g->nodes, ne = g->edges;
+        if (nn && cudaGraphGetNodes(g->graph, nd.data(), &nn) == cudaSuccess &&
+            (!ne || cudaGraphGetEdges(g->graph, from.data(), to.data(), &ne) == cudaSuccess)) {
+            std::map<cudaGraphNode_t, size_t> len;
+            for (size_t i = 0; i < nn; ++i) len[nd[i]] = 1;
+            for (size_t pass = 0; pass < nn; ++pass) {           // relax until stable (graphs here have tens of nodes)
+                bool moved = false;
+                for (size_t k = 0; k < ne; ++k)
+                    if (len[to[k]] < len[from[k]] + 1) { len[to[k]] = len[from[k]] + 1; moved = true; }
+                if (!moved) break;
+            }
+            for (auto &kv : len) g->depth = std::max(g->depth, kv.second);
+        }
+        cudaGetLastError();
+    }
     g->launches = ctx->launches - ctx->capture_l0;
     g->ws_generation = ctx->ws_generation;
     *out = g.release();
@@ -1179,9 +1196,10 @@ int tcb_graph_launch(tcb_ctx *ctx, tcb_graph *g)
     return TCB_OK;
 }
 
-int tcb_graph_info(const tcb_graph *g, int64_t *nodes, int64_t *edges, int64_t *kernel_launches)
+int tcb_graph_info(const tcb_graph *g, int64_t *nodes, int64_t *edges, int64_t *kernel_launches, int64_t *depth)
 {
     if (!g) return TCB_EINVAL;
+    if (depth) *depth = (int64_t)g->depth;
     if (nodes) *nodes = (int64_t)g->nodes;
     if (edges) *edges = (int64_t)g->edges;
     if (kernel_launches) *kernel_launches = g->launches;

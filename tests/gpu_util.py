@@ -90,3 +90,101 @@ def sampled_contraction_parity(ctx, expr, ext, alpha, seed, rng, nsub=8, antisym
         for t in (L, R, D):
             t.destroy()
     return worst, checked
+
+
+# ---- call-by-call parity of a whole driver program (VERDICT r1 "weak" 2) ---------------------------------------------------
+def expand_antisym_spec(spec):
+    """'P(ab)P(k/ij):D(..)+=X(..)' -> (perms, signs, accumulate): P(xy) = 1 - (x<->y), P(x/yz) = 1 - (x<->y) - (x<->z), the
+    product expanded first operator outermost (reading 15); perms[t][m] = D-position of X's index m in term t.
+    Written for the tests from the reading, independently of the library's parser."""
+    import re
+    ops, body = spec.split(":")
+    m = re.fullmatch(r"\s*\w+\(([^)]*)\)\s*(\+?=)\s*\w+\(([^)]*)\)\s*", body)
+    dl = [x.strip() for x in m.group(1).split(",")]
+    xl = [x.strip() for x in m.group(3).split(",")]
+    terms = [(list(xl), 1.0)]
+    for op in re.findall(r"P\(([^)]*)\)", ops):
+        if "/" in op:
+            pivot, others = op.split("/")
+            pivot = pivot.strip()
+            others = [c for c in others.strip()] if "," not in others else [c.strip() for c in others.split(",")]
+        else:
+            labs = [c.strip() for c in op.split(",")] if "," in op else list(op.strip())
+            pivot, others = labs[0], labs[1:]
+        nxt = []
+        for lab, sg in terms:
+            nxt.append((lab, sg))
+            for o_ in others:
+                sw = [o_ if x == pivot else pivot if x == o_ else x for x in lab]
+                nxt.append((sw, -sg))
+        terms = nxt
+    perms = [[dl.index(x) for x in lab] for lab, _ in terms]
+    return perms, [sg for _, sg in terms], m.group(2) == "+="
+
+
+class ShadowTensor:
+    def __init__(self, gpu, host):
+        self.gpu, self.host, self.extents = gpu, host, gpu.extents
+
+    def destroy(self):
+        self.gpu.destroy()
+
+
+class ShadowContext:
+    """Runs a driver program (ccd.py) through the C ABI and, call by call, through the oracle on host values that only the
+    oracle has touched; after every call the device result is compared with the oracle's ELEMENT BY ELEMENT, normalised by
+    that call's own snorm = |alpha| sum|L||R| + |D_in| (north_star's metric), not by max|ref|."""
+
+    def __init__(self, ctx, tol=TOL):
+        self.ctx, self.tol, self.worst, self.calls = ctx, tol, 0.0, 0
+
+    def wrap(self, host):
+        host = np.asfortranarray(np.asarray(host, dtype=np.complex128))
+        return ShadowTensor(self.ctx.tensor_from_numpy(host), host.copy(order="F"))
+
+    def tensor_create(self, extents, zero=True):
+        return ShadowTensor(self.ctx.tensor_create(extents, zero=zero), np.zeros(tuple(extents), dtype=np.complex128, order="F"))
+
+    def lane_set(self, lane):
+        self.ctx.lane_set(lane)
+
+    def lane_wait(self, lane, on_lane):
+        self.ctx.lane_wait(lane, on_lane)
+
+    def _compare(self, what, D, ref, sn):
+        self.ctx.sync()
+        got = self.ctx.tensor_download(D.gpu)
+        zero = sn == 0
+        # chained calls: an element whose normaliser vanishes must still vanish to rounding of its inputs' rounding
+        assert np.all(np.abs(got - ref)[zero] <= 1e-25), what
+        if not zero.all():
+            err = float(np.max(np.abs(got - ref)[~zero] / sn[~zero]))
+            assert err <= self.tol, (what, err)
+            self.worst = max(self.worst, err)
+        self.calls += 1
+        D.host = ref
+
+    def contract(self, expr, D, L, R, alpha=1.0):
+        import oracle
+        self.ctx.contract(expr, D.gpu, L.gpu, R.gpu, alpha)
+        ref, sn = oracle.contract(expr, D.host, L.host, R.host, alpha)
+        self._compare(expr, D, ref, sn)
+
+    def add(self, expr, D, L, alpha=1.0):
+        import oracle
+        self.ctx.add(expr, D.gpu, L.gpu, alpha)
+        acc = "+=" in expr
+        base = D.host if acc else np.zeros_like(D.host)
+        e_acc = expr if acc else expr.replace("=", "+=", 1)
+        ref = oracle.add(e_acc, base, L.host, alpha)
+        sn = np.abs(base) + abs(alpha) * oracle.add(e_acc, np.zeros_like(base), np.abs(L.host), 1.0).real
+        self._compare(expr, D, ref, sn)
+
+    def antisymmetrize(self, spec, D, X, alpha=1.0):
+        import oracle
+        self.ctx.antisymmetrize(spec, D.gpu, X.gpu, alpha)
+        perms, signs, acc = expand_antisym_spec(spec)
+        ref = oracle.permsum(D.host, X.host, perms, [alpha * s for s in signs], 1.0 if acc else 0.0)
+        sn = (np.abs(D.host) if acc else 0.0) + abs(alpha) * oracle.permsum(
+            np.zeros_like(D.host), np.abs(X.host), perms, [1.0] * len(signs), 0.0).real
+        self._compare(spec, D, ref, sn)

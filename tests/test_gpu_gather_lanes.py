@@ -46,7 +46,7 @@ GATHER_CASES = [
     ("F(m,i)+=V(m,n,e,f)*T(e,f,i,n)", dict(m=6, i=5, n=7, e=31, f=29)),
     ("F(a,e)+=T(a,f,m,n)*V(m,n,e,f)", dict(a=20, e=18, f=41, m=6, n=5)),
     # extent-1 indices and a K tail of 1
-    ("D(a,x,b)+=L(a,c,y,b2)*R(c,b,b2)", dict(a=8, x=1, b=9, c=3, y=1, b2=3)),
+    ("D(a,x,b)+=L(a,c,y,b2)*R(c,x,b,y,b2)", dict(a=8, x=1, b=9, c=3, y=1, b2=3)),
 ]
 
 
@@ -139,7 +139,7 @@ def test_lanes_eager_and_captured_as_parallel_graph_branches(ctx):
     g = ctx.capture_end()
     info = ctx.graph_info(g)
     assert info["launches"] == 3 and info["nodes"] >= 3
-    assert info["edges"] >= info["nodes"], info              # a chain has nodes - 1 edges; fork + join adds at least one
+    assert info["depth"] < info["nodes"], info               # a chain has depth = nodes: two of the three run side by side
     ctx.graph_launch(g)
     assert ctx.tensor_download(R).tobytes() == eager.tobytes()
     ctx.graph_destroy(g)
