@@ -259,8 +259,10 @@ int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const 
     };
     // achievable rates on a B200: 0.92 of the FP64 tensor peak, 5.5 TB/s for a transposition pass
     const double kPeak = 37.2e12 * 0.92, kBw = 6.0e12, kBwPerm = 5.5e12, kLaunch = 4e-6;
-    // what the address arithmetic and the 4 x LDGSTS per thread and k-tile of a gathered operand cost the tensor pipe
-    const double kGatherCost = 1.005;
+    // what a gathered operand costs the tensor pipe (table loads, address arithmetic and 4 x LDGSTS per thread and k-tile
+    // are issued by the warps that also issue the DMMAs), measured on 4500^3 and 1600^3 ring terms (profiles/r2_gather_ab.md):
+    // +4.5 % per operand whose lanes run along contiguous memory, +26 % when every lane fetches its own 32-byte sector
+    const double kGatherCost = 1.045, kGatherScattered = 1.26;
     const double flops = 8.0 * (double)P.M * (double)P.N * (double)P.K;
     const double bytesD = 16.0 * (double)sizeD * (e.accumulate ? 2.0 : 1.0);
     std::vector<std::vector<const Lab *>> corders;
@@ -274,8 +276,8 @@ int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const 
             for (const Feed &cb : feeds_of(sb, seqB, dorderB, co, false)) {
                 const double wd = (seqD.empty() || (!ca.forder.empty() && ca.forder[0] == seqD[0])) ? 1.0 : 2.0;
                 double fl = flops / kPeak;
-                if (ca.kind == 1) fl *= kGatherCost;
-                if (cb.kind == 1) fl *= kGatherCost;
+                if (ca.kind == 1) fl *= ca.waste > 1.0 ? kGatherScattered : kGatherCost;
+                if (cb.kind == 1) fl *= cb.waste > 1.0 ? kGatherScattered : kGatherCost;
                 const double by = (16.0 * (double)sizeA * ca.waste + 16.0 * (double)sizeB * cb.waste + bytesD * wd) / kBw;
                 double t = std::max(fl, by) + kLaunch;
                 // 16-byte scattered epilogue stores are not hidden behind the tensor work (one sector per lane instead of

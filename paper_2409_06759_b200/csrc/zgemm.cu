@@ -57,6 +57,8 @@ constexpr int STAGES = 4;
 constexpr int A_BYTES = BM * BK * 16;   // 8 KB
 constexpr int B_BYTES = BN * BK * 16;   // 8 KB
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int kGatherAhead = 2;         // k-tiles a gathered operand is fetched ahead (its refill never waits for the
+                                        // stage the CTA is still draining: no CTA-wide lock step per k-tile)
 constexpr int kQueue = 8;               // segment queue entries (producer is <= STAGES + 1 segments ahead)
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 128 /*barriers*/ + 256 /*segment queue*/;
 constexpr int NTHREADS = 128;
@@ -542,7 +544,7 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     }
     if (kAnyGather) {
         gather_enter();
-        for (int s = 0; s < STAGES && gvalid; ++s) gather_issue();
+        for (int s = 0; s < kGatherAhead && gvalid; ++s) gather_issue();
     }
 
     // per-lane fragment offsets inside a 1 KB atom, for the two k-steps of a stage
@@ -589,8 +591,10 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 mbar_wait(bar_base + 8 * (STAGES + pstage), pphase ^ 1);
                 issue();
             }
-            if (kAnyGather && done >= 1 && gvalid) {
-                // the same refill for the gathered part (every thread waits for the stage to be drained)
+            if (kAnyGather && gvalid) {
+                // the gathered part of k-tile done + kGatherAhead goes into the stage that was consumed STAGES - kGatherAhead
+                // iterations ago: every thread checks that all four warps have left it (they have, unless one lags two
+                // k-tiles; a fresh barrier passes the parity test at once)
                 mbar_wait(bar_base + 8 * (STAGES + gstage), gphase ^ 1);
                 gather_issue();
             }

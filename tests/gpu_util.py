@@ -155,8 +155,10 @@ class ShadowContext:
         self.ctx.sync()
         got = self.ctx.tensor_download(D.gpu)
         zero = sn == 0
-        # chained calls: an element whose normaliser vanishes must still vanish to rounding of its inputs' rounding
-        assert np.all(np.abs(got - ref)[zero] <= 1e-25), what
+        # An element whose normaliser vanishes in the ORACLE's chain (a = b of an antisymmetric operand) is an exact zero
+        # there; on the device the operand of a chained call is antisymmetric only to rounding (the DMMA complex product
+        # rounds ar*bi + ai*br in issue order, so t_a t_b - t_b t_a leaves an ulp), hence: noise level of the call, not 0
+        assert np.all(np.abs(got - ref)[zero] <= 1e-13 * (sn.max() if sn.size else 0.0)), what
         if not zero.all():
             err = float(np.max(np.abs(got - ref)[~zero] / sn[~zero]))
             assert err <= self.tol, (what, err)

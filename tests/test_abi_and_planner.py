@@ -91,17 +91,28 @@ def test_ring_term_reads_both_operands_in_place_through_offset_tables():
 
 
 def test_cost_model_picks_per_operand_feeds():
-    """S2 (viii): candidates cost max(flops / peak, bytes / BW) per pass; matrix-shaped operands stay on TMA, a non-matrix
-    operand is gathered, and nothing is ever permuted under "auto" at CC sizes (o=30, v=150)."""
+    """S2 (viii): candidates cost max(flops / peak, bytes / BW) per pass.  At CC sizes (o=30, v=150): matrix-shaped operands
+    stay on TMA; a non-matrix operand of a short-K call (where a transposition pass would cost as much as the GEMM) is
+    gathered; the tensor-bound 4500^3 ring terms transpose both operands first (a 0.1 ms pass each against a 21 ms GEMM
+    that gathering would slow by more); "operand_loads=gather" removes every transposition."""
     from paper_2409_06759_b200 import ccsd_contractions as cl
     o, v = 30, 150
     seen = set()
     for e, sign, sd, sl, sr in cl.all_calls(o, v):
         p = plan(e, sd, sl, sr)
-        assert not p["permute_A"] and not p["permute_B"], (e, p)
         assert p["est_us"] > 0
         seen.add((p["feed_A"], p["feed_B"]))
-    assert ("tma", "tma") in seen and any("gather" in fb for fb in seen)
+        q = plan(e, sd, sl, sr, "operand_loads=gather")
+        assert not q["permute_A"] and not q["permute_B"], (e, q)
+        assert q["est_us"] >= p["est_us"] * (1 - 1e-6)        # "auto" never costs more than a forced choice
+        big = max(np.prod(sl), np.prod(sr))
+        if big >= o * v ** 3 and p["K"] <= 150:                # a v^3 o operand in front of a short-K GEMM: never transposed
+            assert not p["permute_A"] and not p["permute_B"], (e, p)
+    assert ("tma", "tma") in seen and ("permute", "permute") in seen and any("gather" in fb for fb in seen)
+    ring = plan("R2(a,b,i,j)+=T2(a,e,i,m)*Wmbej(m,b,e,j)", (v, v, o, o), (v, v, o, o), (o, v, v, o))
+    assert ring["feed_A"] == "permute" and ring["feed_B"] == "permute"
+    short = plan("R2(a,b,i,j)+=vvvo(a,b,e,j)*T1(e,i)", (v, v, o, o), (v, v, v, o), (v, o))
+    assert short["feed_A"] == "gather" and short["feed_B"] == "tma" and short["m_labels"] == "a,b,j"
     # pp ladder: both in place by TMA, cost = the tensor-bound GEMM
     p = plan("R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)", (v, v, o, o), (v, v, v, v), (v, v, o, o))
     assert p["feed_A"] == "tma" and p["feed_B"] == "tma"
