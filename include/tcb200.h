@@ -164,6 +164,25 @@ int tcb_permsum(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, int nterms, co
  * for 1 - (x<->y) - (x<->z) - ...; P(xy) for 1 - (x<->y); the product is expanded into signed terms
  * (first operator outermost).  D = D + alpha * sum of terms. */
 int tcb_antisymmetrize(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *X, tcb_c128 alpha);
+/* Index-permutation-symmetric (antisymmetric) packed storage, SURVEY 8(f)-2.  The paper lists index-permutation symmetry as
+ * what its generated code does not exploit yet (outlook 440, 452); it gives no storage scheme, so this is
+ * a reading (reading 16): a group a<b (or a<b<c) of labels of equal extent n, in which the tensor is antisymmetric,
+ * is stored as ONE packed index running over the strictly increasing tuples, first label fastest:
+ *     pairs (0,1) (0,2) (1,2) (0,3) ..   p = b(b-1)/2 + a;      triples (0,1,2) (0,1,3) (0,2,3) (1,2,3) ..
+ * of extent tcb_packed_extent(n, 2) = n(n-1)/2, tcb_packed_extent(n, 3) = n(n-1)(n-2)/6.  A packed tensor is an ordinary
+ * handle (create it with those extents); contractions over whole groups are plain tcb_contract calls on the packed indices:
+ *     Vp(a<b,c<d) = V(a,b,c,d);  Tp(c<d,i<j) = T(c,d,i,j);  "Rp(x,y)+=Vp(x,z)*Tp(z,y)" with alpha = 1;  R(a,b,i,j) += Rp(a<b,i<j)
+ * is the pp ladder R += 1/2 V T at 1/8 of the flops (the c<d sum visits each unordered pair once: no factor 1/2).
+ *   tcb_pack   spec "Vp(a<b,c<d)=V(a,b,c,d)": Dp[.., p, ..] = L[.., a, .., b, ..]; pure data movement, bit-exact; groups of
+ *              1..3 labels, in any order and at any dense positions; '=' only.
+ *   tcb_unpack spec "R(a,b,i,j)+=Rp(a<b,i<j)" (or '='): D[.., a, .., b, ..] (+)= alpha * sign * Lp[.., p(sorted a, b), ..],
+ *              sign = parity of the sorting permutation, 0 when two labels of a group coincide.  With alpha = 1 and '=' an
+ *              exactly antisymmetric tensor comes back bit for bit.
+ * Errors: TCB_EINVAL_EXPR (syntax, no group, '+=' in tcb_pack, labels not matching), TCB_ESHAPE (ranks, unequal extents in a
+ * group, packed extent not n choose k), TCB_EUNSUPPORTED (groups of more than 3 labels, repeated label), TCB_EALIAS. */
+int tcb_pack(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *L);
+int tcb_unpack(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *L, tcb_c128 alpha);
+int64_t tcb_packed_extent(int64_t n, int k);      /* n choose k for k = 1, 2, 3; -1 otherwise */
 /* JSON description of the plan tcb_contract would use: M, N, K, which operands are permuted, GEMM variant,
  * split-K, estimated flops and bytes.  Truncated to buflen-1 characters. */
 int tcb_plan_describe(tcb_ctx *ctx, const char *expr, const tcb_tensor *D, const tcb_tensor *L,

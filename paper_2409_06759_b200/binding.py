@@ -45,7 +45,7 @@ ABI_SYMBOLS = [
     "tcb_denominator_update", "tcb_denominator_divide", "tcb_dot",
     "tcb_permute", "tcb_permsum", "tcb_antisymmetrize", "tcb_plan_describe", "tcb_measure_fp64_tensor_peak", "tcb_measure_fp64_vector_peak",
     "tcb_capture_begin", "tcb_capture_end", "tcb_graph_launch", "tcb_graph_info", "tcb_graph_destroy",
-    "tcb_lane_count", "tcb_lane_set", "tcb_lane_wait",
+    "tcb_lane_count", "tcb_lane_set", "tcb_lane_wait", "tcb_pack", "tcb_unpack", "tcb_packed_extent",
     "tcb_timer_start", "tcb_timer_stop", "tcb_kernel_stats", "tcb_kernel_stats_reset", "tcb_plan_describe_host", "tcbx_synth_normal", "tcbx_synth_index_linear",
     "tcbx_synth_mp2_amplitudes",
 ]
@@ -95,6 +95,8 @@ def load_library():
         "tcb_graph_destroy": [vp],
         "tcb_graph_info": [vp, i64p, i64p, i64p, i64p],
         "tcb_lane_count": [],
+        "tcb_pack": [vp, cp, vp, vp],
+        "tcb_unpack": [vp, cp, vp, vp, c128],
         "tcb_lane_set": [vp, ctypes.c_int],
         "tcb_lane_wait": [vp, ctypes.c_int, ctypes.c_int],
         "tcb_timer_start": [vp],
@@ -115,6 +117,8 @@ def load_library():
     lib.tcb_last_error.restype = ctypes.c_char_p
     lib.tcb_strerror.argtypes = [ctypes.c_int]
     lib.tcb_strerror.restype = ctypes.c_char_p
+    lib.tcb_packed_extent.argtypes = [ctypes.c_int64, ctypes.c_int]
+    lib.tcb_packed_extent.restype = ctypes.c_int64
     lib.tcb_launch_count.argtypes = [vp]
     lib.tcb_launch_count.restype = ctypes.c_int64
     _lib = lib
@@ -315,6 +319,17 @@ class Context:
 
     def antisymmetrize(self, spec, D, X, alpha=1.0):
         self._check(self.lib.tcb_antisymmetrize(self.handle, spec.encode(), D.handle, X.handle, _c(alpha)))
+
+    def pack(self, spec, D, L):
+        """'Vp(a<b,c<d)=V(a,b,c,d)': antisymmetric index groups stored as one packed index each (tcb_pack)"""
+        self._check(self.lib.tcb_pack(self.handle, spec.encode(), D.handle, L.handle))
+
+    def unpack(self, spec, D, L, alpha=1.0):
+        """'R(a,b,i,j)+=Rp(a<b,i<j)': D (+)= alpha * sign * Lp[packed position] (tcb_unpack)"""
+        self._check(self.lib.tcb_unpack(self.handle, spec.encode(), D.handle, L.handle, _c(alpha)))
+
+    def packed_extent(self, n, k):
+        return int(self.lib.tcb_packed_extent(int(n), int(k)))
 
     def plan_describe(self, expr, D, L, R):
         buf = ctypes.create_string_buffer(2048)

@@ -42,6 +42,12 @@ struct Lane {
     bool in_capture = false;         // forked into the open capture
 };
 
+struct SymTables {
+    std::vector<int64_t> host;      // the tables of all packed dims, one after the other
+    int64_t *dev = nullptr;
+    size_t at[kMaxRank] = {0, 0, 0, 0, 0, 0};
+};
+
 struct tcb_ctx {
     int device = 0;
     Lane lanes[kMaxLanes];
@@ -52,6 +58,7 @@ struct tcb_ctx {
     int64_t launches = 0;
     PlanOptions opt;
     std::map<std::string, std::unique_ptr<CachedPlan>> plans;
+    std::map<std::string, std::unique_ptr<struct SymTables>> sym_tables;   // tcb_pack offset tables per (spec, extents)
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     int64_t live_tensors = 0;
     // per-kernel-class device timing ("kernel_timing" = "on"): event pairs around every launch, summed on query
@@ -381,6 +388,8 @@ int tcb_ctx_destroy(tcb_ctx *ctx)
     for (Lane &ln : ctx->lanes) if (ln.stream) cudaStreamSynchronize(ln.stream);
     for (auto &kv : ctx->plans)
         if (kv.second->d_tables) cudaFree(kv.second->d_tables);
+    for (auto &kv : ctx->sym_tables)
+        if (kv.second->dev) cudaFree(kv.second->dev);
     for (Lane &ln : ctx->lanes) if (ln.ws) cudaFree(ln.ws);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
@@ -1044,6 +1053,142 @@ int tcb_antisymmetrize(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_
     }
     tcb_c128 beta = {e.accumulate ? 1.0 : 0.0, 0.0};
     return tcb_permsum(ctx, D, X, (int)terms.size(), perms.data(), coefs.data(), beta);
+}
+
+// ---- index-permutation-symmetric packed storage ------------------------------------------------------------
+namespace {
+
+int64_t choose(int64_t n, int k)
+{
+    if (k == 1) return n;
+    if (k == 2) return n * (n - 1) / 2;
+    return n * (n - 1) * (n - 2) / 6;
+}
+
+// validates a pack / unpack spec against the two handles; dense_pos[g][s] = position in the dense tensor of label s of group g
+int bind_sym_spec(tcb_ctx *ctx, const std::vector<std::vector<std::string>> &packed, const std::vector<std::vector<std::string>> &dense,
+                  const tcb_tensor *P, const tcb_tensor *Dn, int dense_pos[kMaxRank][3])
+{
+    if ((int)packed.size() != P->shape.rank || (int)dense.size() != Dn->shape.rank)
+        return set_error(ctx, TCB_ESHAPE, "rank of a handle differs from the spec");
+    std::vector<std::string> dl;
+    for (const auto &g : dense) {
+        if (g.size() != 1) return set_error(ctx, TCB_EINVAL_EXPR, "a<b groups on both sides");
+        dl.push_back(g[0]);
+    }
+    if (has_dup(dl)) return set_error(ctx, TCB_EUNSUPPORTED, "label repeated inside the dense tensor");
+    size_t used = 0;
+    bool any_group = false;
+    for (size_t g = 0; g < packed.size(); ++g) {
+        const auto &grp = packed[g];
+        if (grp.size() > 3) return set_error(ctx, TCB_EUNSUPPORTED, "groups of more than three labels");
+        any_group = any_group || grp.size() > 1;
+        int64_t n = -1;
+        for (size_t s = 0; s < grp.size(); ++s) {
+            const int pos = find_label(dl, grp[s]);
+            if (pos < 0) return set_error(ctx, TCB_EINVAL_EXPR, "label " + grp[s] + " missing in the dense tensor");
+            for (size_t g2 = 0; g2 <= g; ++g2)
+                for (size_t s2 = 0; s2 < (g2 == g ? s : packed[g2].size()); ++s2)
+                    if (packed[g2][s2] == grp[s]) return set_error(ctx, TCB_EUNSUPPORTED, "label repeated inside the packed tensor");
+            dense_pos[g][s] = pos;
+            if (n >= 0 && Dn->shape.ext[pos] != n) return set_error(ctx, TCB_ESHAPE, "labels of one group differ in extent");
+            n = Dn->shape.ext[pos];
+            ++used;
+        }
+        if (P->shape.ext[g] != choose(n, (int)grp.size()))
+            return set_error(ctx, TCB_ESHAPE, "packed extent is not n(n-1)/2 (n(n-1)(n-2)/6) of the group's dense extent");
+    }
+    if (used != dl.size()) return set_error(ctx, TCB_EINVAL_EXPR, "a dense label is missing in the packed tensor");
+    if (!any_group) return set_error(ctx, TCB_EINVAL_EXPR, "no a<b group in the spec (use tcb_permute)");
+    return TCB_OK;
+}
+
+}  // namespace
+
+int tcb_pack(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *L)
+{
+    NvtxRange nvtx_range("tcb_pack");
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!spec || !D || !L) return set_error(ctx, TCB_EINVAL, "null argument");
+    SymSpec sp;
+    if (!parse_sym_spec(spec, &sp)) return set_error(ctx, TCB_EINVAL_EXPR, std::string("cannot parse: ") + spec);
+    if (sp.accumulate) return set_error(ctx, TCB_EINVAL_EXPR, "tcb_pack takes '=', not '+='");
+    int pos[kMaxRank][3];
+    rc = bind_sym_spec(ctx, sp.lhs, sp.rhs, D, L, pos);
+    if (rc) return rc;
+    if (overlaps(D, L)) return set_error(ctx, TCB_EALIAS, "D overlaps L");
+    const std::string key = std::string(spec) + "|" + shape_key(D->shape) + shape_key(L->shape);
+    auto it = ctx->sym_tables.find(key);
+    if (it == ctx->sym_tables.end()) {
+        rc = refuse_in_capture(ctx, "the first tcb_pack of a spec (run the call list once before capturing it)");
+        if (rc) return rc;
+        std::unique_ptr<SymTables> st(new SymTables());
+        int64_t sL[kMaxRank];
+        strides_of(L->shape, sL);
+        for (size_t g = 0; g < sp.lhs.size(); ++g) {
+            st->at[g] = st->host.size();
+            const int k = (int)sp.lhs[g].size();
+            const int64_t n = L->shape.ext[pos[g][0]];
+            const int64_t s0 = sL[pos[g][0]], s1 = k > 1 ? sL[pos[g][1]] : 0, s2 = k > 2 ? sL[pos[g][2]] : 0;
+            // strictly increasing tuples, first label fastest
+            if (k == 1) for (int64_t a = 0; a < n; ++a) st->host.push_back(a * s0);
+            else if (k == 2) { for (int64_t b = 0; b < n; ++b) for (int64_t a = 0; a < b; ++a) st->host.push_back(a * s0 + b * s1); }
+            else for (int64_t c = 0; c < n; ++c) for (int64_t b = 0; b < c; ++b) for (int64_t a = 0; a < b; ++a)
+                     st->host.push_back(a * s0 + b * s1 + c * s2);
+        }
+        TCB_CUDA(ctx, cudaMalloc((void **)&st->dev, std::max<size_t>(1, st->host.size()) * sizeof(int64_t)));
+        TCB_CUDA(ctx, cudaMemcpyAsync(st->dev, st->host.data(), st->host.size() * sizeof(int64_t), cudaMemcpyHostToDevice,
+                                      cur_stream(ctx)));
+        it = ctx->sym_tables.emplace(key, std::move(st)).first;
+    }
+    PackDesc d;
+    d.rank = D->shape.rank;
+    for (int k = 0; k < kMaxRank; ++k) {
+        d.extent[k] = k < d.rank ? D->shape.ext[k] : 1;
+        d.tab[k] = k < d.rank ? it->second->dev + it->second->at[k] : nullptr;
+    }
+    d.in = L->ptr; d.out = D->ptr;
+    TimedLaunch tl(ctx, kClsPermute, 0.0, 32.0 * (double)D->elems());
+    TCB_CUDA(ctx, launch_pack(d, cur_stream(ctx), &ctx->launches));
+    return TCB_OK;
+}
+
+int tcb_unpack(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *L, tcb_c128 alpha)
+{
+    NvtxRange nvtx_range("tcb_unpack");
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!spec || !D || !L) return set_error(ctx, TCB_EINVAL, "null argument");
+    SymSpec sp;
+    if (!parse_sym_spec(spec, &sp)) return set_error(ctx, TCB_EINVAL_EXPR, std::string("cannot parse: ") + spec);
+    int pos[kMaxRank][3];
+    rc = bind_sym_spec(ctx, sp.rhs, sp.lhs, L, D, pos);
+    if (rc) return rc;
+    if (overlaps(D, L)) return set_error(ctx, TCB_EALIAS, "D overlaps L");
+    UnpackDesc d;
+    d.rank = D->shape.rank;
+    d.ngroups = L->shape.rank;
+    int64_t sP[kMaxRank];
+    strides_of(L->shape, sP);
+    for (int k = 0; k < kMaxRank; ++k) d.extent[k] = k < d.rank ? D->shape.ext[k] : 1;
+    for (int g = 0; g < kMaxRank; ++g) {
+        d.glen[g] = g < d.ngroups ? (int)sp.rhs[g].size() : 1;
+        d.pstride[g] = g < d.ngroups ? sP[g] : 0;
+        for (int s = 0; s < 3; ++s) d.gpos[g][s] = (g < d.ngroups && s < d.glen[g]) ? pos[g][s] : 0;
+    }
+    d.alpha_re = alpha.re; d.alpha_im = alpha.im;
+    d.accumulate = sp.accumulate;
+    d.in = L->ptr; d.out = D->ptr;
+    TimedLaunch tl(ctx, kClsPermute, 0.0, 16.0 * ((double)D->elems() * (sp.accumulate ? 2.0 : 1.0) + (double)L->elems()));
+    TCB_CUDA(ctx, launch_unpack(d, cur_stream(ctx), &ctx->launches));
+    return TCB_OK;
+}
+
+int64_t tcb_packed_extent(int64_t n, int k)
+{
+    if (n < 0 || k < 1 || k > 3) return -1;
+    return choose(n, k);
 }
 
 // used by synth.cu (same shared object): validates the context and exposes its stream and launch counter

@@ -111,6 +111,31 @@ cudaError_t launch_permsum(const PermSumDesc &p, cudaStream_t stream, int64_t *l
 // false when the call is of another kind
 cudaError_t launch_permsum_orbit(const PermSumDesc &p, cudaStream_t stream, int64_t *launches, bool *handled);
 
+// ---- index-permutation-symmetric packed storage (sympack.cu) ---------------------------------
+// pack: out[packed linear index] = in[sum_d tab[d][i_d]]  (tab[d]: device table over the values of packed index d)
+struct PackDesc {
+    int rank;
+    int64_t extent[kMaxRank];
+    const int64_t *tab[kMaxRank];
+    const void *in;
+    void *out;
+};
+cudaError_t launch_pack(const PackDesc &d, cudaStream_t stream, int64_t *launches);
+// unpack: out[dense index] (+)= alpha * sign * in[sum_g p(sorted labels of group g) * pstride[g]]
+struct UnpackDesc {
+    int rank;                       // dense rank
+    int64_t extent[kMaxRank];       // dense extents
+    int ngroups;                    // = rank of the packed tensor
+    int glen[kMaxRank];             // labels per group (1..3)
+    int gpos[kMaxRank][3];          // dense positions of the group's labels, in the group's order
+    int64_t pstride[kMaxRank];      // stride of the packed index in the packed tensor
+    double alpha_re, alpha_im;
+    bool accumulate;
+    const void *in;
+    void *out;
+};
+cudaError_t launch_unpack(const UnpackDesc &d, cudaStream_t stream, int64_t *launches);
+
 // ---- S7: elementwise --------------------------------------------------------------------------------------
 cudaError_t launch_fill(void *D, int64_t n, double re, double im, cudaStream_t stream, int64_t *launches);
 cudaError_t launch_scale(void *D, int64_t n, double re, double im, cudaStream_t stream, int64_t *launches);

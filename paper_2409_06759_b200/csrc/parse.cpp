@@ -41,6 +41,28 @@ bool tensor(Cursor &c, std::vector<std::string> *labels)
     }
 }
 
+bool sym_tensor(Cursor &c, std::vector<std::vector<std::string>> *items)
+{
+    if (!ident(c, nullptr)) return false;
+    if (!c.eat('(')) return false;
+    items->clear();
+    if (c.eat(')')) return true;
+    for (;;) {
+        std::vector<std::string> group;
+        for (;;) {
+            std::string lab;
+            c.ws();
+            if (!std::isalpha((unsigned char)*c.p)) return false;
+            if (!ident(c, &lab)) return false;
+            group.push_back(lab);
+            if (!c.eat('<')) break;
+        }
+        items->push_back(group);
+        if (c.eat(',')) continue;
+        return c.eat(')');
+    }
+}
+
 bool expression(Cursor &c, ParsedExpr *e)
 {
     if (!tensor(c, &e->d)) return false;
@@ -104,6 +126,20 @@ bool parse_antisym_spec(const char *text, std::vector<PermOperator> *ops, Parsed
         ops->push_back(op);
     }
     return expression(c, expr) && !expr->has_r;
+}
+
+bool parse_sym_spec(const char *text, SymSpec *out)
+{
+    if (!text || !out) return false;
+    Cursor c{text};
+    if (!sym_tensor(c, &out->lhs)) return false;
+    c.ws();
+    if (c.p[0] == '+' && c.p[1] == '=') { out->accumulate = true; c.p += 2; }
+    else if (c.p[0] == '=') { out->accumulate = false; c.p += 1; }
+    else return false;
+    if (!sym_tensor(c, &out->rhs)) return false;
+    c.ws();
+    return *c.p == 0;
 }
 
 }  // namespace tcb

@@ -21,4 +21,12 @@ struct PermOperator {
 };
 bool parse_antisym_spec(const char *text, std::vector<PermOperator> *ops, ParsedExpr *expr);
 
+// "Vp(a<b,c<d)=V(a,b,c,d)" / "R(a,b,i,j)+=Rp(a<b,i<j)": each index position is a group of one or more labels joined by '<'
+// (index-permutation-symmetric packed storage, tcb_pack / tcb_unpack)
+struct SymSpec {
+    std::vector<std::vector<std::string>> lhs, rhs;
+    bool accumulate = false;
+};
+bool parse_sym_spec(const char *text, SymSpec *out);
+
 }  // namespace tcb

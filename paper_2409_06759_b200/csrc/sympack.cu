@@ -1,0 +1,206 @@
+// sympack.cu -- index-permutation-symmetric (antisymmetric) packed storage: tcb_pack / tcb_unpack.
+//
+// The paper names index-permutation symmetry as the feature its production code does not exploit yet (PAPER.md:202, 264,
+// 440, 452).  Reading taken (reading 16, oracle/sym.py): a group a<b (a<b<c) of labels in which a tensor is
+// antisymmetric is stored as ONE packed index over the strictly increasing tuples, first label fastest:
+//     p(a<b) = b(b-1)/2 + a,        p(a<b<c) = c(c-1)(c-2)/6 + b(b-1)/2 + a.
+// A packed tensor is an ordinary tensor handle whose packed index has extent n(n-1)/2 (n(n-1)(n-2)/6), so contractions over
+// whole groups are plain tcb_contract calls on the packed indices: the pp ladder R(ab,ij) += V(ab,cd) T(cd,ij) runs at 1/8
+// of the dense flops and with no factor 1/2.
+//
+//   pack   : Dp[.., p, ..] = L[.., a, .., b, ..]            pure data movement, bit-exact; one offset table per packed index
+//   unpack : D[.., a, .., b, ..] (+)= alpha * sign * Lp[.., p(sorted), ..],  sign = parity of the sort, 0 on equal labels
+//
+// Both are HBM-bound streaming kernels: a CTA walks rows along the tensor's unit-stride index; the row's multi-index is
+// decoded once per row, per element only the group that holds the unit-stride index is evaluated.
+#include "kernels.h"
+
+#include <algorithm>
+
+namespace tcb {
+
+namespace {
+
+struct PackParams {
+    int rank;                          // of the packed tensor
+    long long e[kMaxRank];             // packed extents
+    const long long *tab[kMaxRank];    // device: offset into the dense tensor contributed by packed index value i of dim d
+    long long nrows;                   // prod e[1..]
+    const double2 *in;
+    double2 *out;
+};
+
+__global__ void __launch_bounds__(256) pack_kernel(const __grid_constant__ PackParams p)
+{
+    const long long e0 = p.e[0];
+    const long long *t0 = p.tab[0];
+    for (long long row = blockIdx.x; row < p.nrows; row += gridDim.x) {
+        long long r = row, off = 0;
+#pragma unroll
+        for (int d = 1; d < kMaxRank; ++d) {
+            if (d >= p.rank) break;
+            const long long i = r % p.e[d];
+            r /= p.e[d];
+            off += __ldg(p.tab[d] + i);
+        }
+        const double2 *src = p.in + off;
+        double2 *dst = p.out + row * e0;
+        for (long long i = threadIdx.x; i < e0; i += blockDim.x) dst[i] = src[__ldg(t0 + i)];
+    }
+}
+
+struct UnpackParams {
+    int rank;                          // dense rank
+    long long e[kMaxRank];             // dense extents
+    int ngroups;
+    int glen[kMaxRank];                // labels per group (1..3)
+    int gpos[kMaxRank][3];             // dense positions of the group's labels
+    long long pstride[kMaxRank];       // stride of the group's packed index in Lp
+    int g0, g0slot;                    // the group that holds dense position 0, and where in it
+    long long nrows;
+    double ar, ai;
+    int accumulate;
+    const double2 *in;
+    double2 *out;
+};
+
+// packed position of a strictly increasing tuple
+__device__ __forceinline__ long long tuple_pos(int len, long long a, long long b, long long c)
+{
+    if (len == 1) return a;
+    if (len == 2) return b * (b - 1) / 2 + a;
+    return c * (c - 1) * (c - 2) / 6 + b * (b - 1) / 2 + a;
+}
+// sorts (x, y, z) ascending (len of them valid); returns the sign of the sorting permutation, 0 if two coincide
+__device__ __forceinline__ int sort_sign(int len, long long &x, long long &y, long long &z)
+{
+    int s = 1;
+    if (len == 1) return 1;
+    if (len == 2) {
+        if (x == y) return 0;
+        if (x > y) { const long long t = x; x = y; y = t; s = -1; }
+        return s;
+    }
+    if (x == y || y == z || x == z) return 0;
+    if (x > y) { const long long t = x; x = y; y = t; s = -s; }
+    if (y > z) { const long long t = y; y = z; z = t; s = -s; }
+    if (x > y) { const long long t = x; x = y; y = t; s = -s; }
+    return s;
+}
+
+__global__ void __launch_bounds__(256) unpack_kernel(const __grid_constant__ UnpackParams p)
+{
+    const long long e0 = p.e[0];
+    for (long long row = blockIdx.x; row < p.nrows; row += gridDim.x) {
+        long long idx[kMaxRank];
+        long long r = row;
+        idx[0] = 0;
+#pragma unroll
+        for (int d = 1; d < kMaxRank; ++d) {
+            idx[d] = 0;
+            if (d < p.rank) { idx[d] = r % p.e[d]; r /= p.e[d]; }
+        }
+        // groups that do not hold the unit-stride index: one offset and one sign per row
+        long long off = 0;
+        int sign = 1;
+        for (int g = 0; g < p.ngroups; ++g) {
+            if (g == p.g0) continue;
+            long long x = idx[p.gpos[g][0]], y = p.glen[g] > 1 ? idx[p.gpos[g][1]] : 0, z = p.glen[g] > 2 ? idx[p.gpos[g][2]] : 0;
+            sign *= sort_sign(p.glen[g], x, y, z);
+            off += tuple_pos(p.glen[g], x, y, z) * p.pstride[g];
+        }
+        const int len0 = p.glen[p.g0];
+        // the other members of the unit-stride index's group
+        long long m1 = 0, m2 = 0;
+        {
+            int q = 0;
+            for (int s = 0; s < len0; ++s) {
+                if (s == p.g0slot) continue;
+                if (q == 0) m1 = idx[p.gpos[p.g0][s]]; else m2 = idx[p.gpos[p.g0][s]];
+                ++q;
+            }
+        }
+        const long long ps0 = p.pstride[p.g0];
+        double2 *dst = p.out + row * e0;
+        for (long long i = threadIdx.x; i < e0; i += blockDim.x) {
+            // the tuple in the group's own label order: i sits in slot g0slot
+            long long x, y = 0, z = 0;
+            if (len0 == 1) { x = i; }
+            else if (len0 == 2) { x = p.g0slot == 0 ? i : m1; y = p.g0slot == 0 ? m1 : i; }
+            else {
+                x = p.g0slot == 0 ? i : m1;
+                y = p.g0slot == 1 ? i : (p.g0slot == 0 ? m1 : m2);
+                z = p.g0slot == 2 ? i : m2;
+            }
+            const int sg = sign * sort_sign(len0, x, y, z);
+            double2 v = make_double2(0.0, 0.0);
+            if (sg != 0) {
+                const double2 w = p.in[off + tuple_pos(len0, x, y, z) * ps0];
+                // alpha * (sign * w): the sign is an exact negation; products and sums rounded one by one
+                const double wr = sg > 0 ? w.x : -w.x, wi = sg > 0 ? w.y : -w.y;
+                v.x = __dsub_rn(__dmul_rn(p.ar, wr), __dmul_rn(p.ai, wi));
+                v.y = __dadd_rn(__dmul_rn(p.ar, wi), __dmul_rn(p.ai, wr));
+            }
+            if (p.accumulate) {
+                const double2 d = dst[i];
+                v.x = __dadd_rn(d.x, v.x);
+                v.y = __dadd_rn(d.y, v.y);
+            }
+            dst[i] = v;
+        }
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_pack(const PackDesc &d, cudaStream_t stream, int64_t *launches)
+{
+    PackParams p;
+    p.rank = d.rank;
+    p.nrows = 1;
+    for (int k = 0; k < kMaxRank; ++k) {
+        p.e[k] = k < d.rank ? d.extent[k] : 1;
+        p.tab[k] = k < d.rank ? (const long long *)d.tab[k] : nullptr;
+        if (k >= 1) p.nrows *= p.e[k];
+    }
+    p.in = (const double2 *)d.in;
+    p.out = (double2 *)d.out;
+    const int blocks = (int)std::max<long long>(1, std::min<long long>(p.nrows, 16LL * sm_count()));
+    pack_kernel<<<blocks, 256, 0, stream>>>(p);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && launches) ++*launches;
+    return e;
+}
+
+cudaError_t launch_unpack(const UnpackDesc &d, cudaStream_t stream, int64_t *launches)
+{
+    UnpackParams p;
+    p.rank = d.rank;
+    p.nrows = 1;
+    for (int k = 0; k < kMaxRank; ++k) {
+        p.e[k] = k < d.rank ? d.extent[k] : 1;
+        if (k >= 1) p.nrows *= p.e[k];
+    }
+    p.ngroups = d.ngroups;
+    p.g0 = -1; p.g0slot = 0;
+    for (int g = 0; g < kMaxRank; ++g) {
+        p.glen[g] = g < d.ngroups ? d.glen[g] : 1;
+        p.pstride[g] = g < d.ngroups ? d.pstride[g] : 0;
+        for (int s = 0; s < 3; ++s) {
+            p.gpos[g][s] = (g < d.ngroups && s < d.glen[g]) ? d.gpos[g][s] : 0;
+            if (g < d.ngroups && s < d.glen[g] && d.gpos[g][s] == 0) { p.g0 = g; p.g0slot = s; }
+        }
+    }
+    if (p.g0 < 0) return cudaErrorInvalidValue;
+    p.ar = d.alpha_re; p.ai = d.alpha_im;
+    p.accumulate = d.accumulate ? 1 : 0;
+    p.in = (const double2 *)d.in;
+    p.out = (double2 *)d.out;
+    const int blocks = (int)std::max<long long>(1, std::min<long long>(p.nrows, 16LL * sm_count()));
+    unpack_kernel<<<blocks, 256, 0, stream>>>(p);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && launches) ++*launches;
+    return e;
+}
+
+}  // namespace tcb
