@@ -76,8 +76,8 @@ def test_round_trip_of_an_antisymmetric_tensor_is_bit_exact(ctx):
 
 
 def test_bad_specs_are_rejected_and_leave_the_context_usable(ctx):
-    T, P = ctx.tensor_create((5, 5, 3, 3)), ctx.tensor_create((10, 3))
-    for spec, D, L, code in [("Tp(a<b,i<j)=T(a,b,i,j)", P, T, binding.TCB_ESHAPE),              # packed extent of (i<j) is 3, rank ok
+    T, P = ctx.tensor_create((5, 5, 3, 3)), ctx.tensor_create((10, 4))
+    for spec, D, L, code in [("Tp(a<b,i<j)=T(a,b,i,j)", P, T, binding.TCB_ESHAPE),              # packed extent of (i<j) must be 3
                              ("Tp(a,b,i,j)=T(a,b,i,j)", T, T, binding.TCB_EINVAL_EXPR),          # no group
                              ("Tp(a<i,b<j)=T(a,b,i,j)", P, T, binding.TCB_ESHAPE),               # unequal extents in a group
                              ("Tp(a<b,i<j)+=T(a,b,i,j)", P, T, binding.TCB_EINVAL_EXPR),
