@@ -59,6 +59,7 @@ constexpr int B_BYTES = BN * BK * 16;   // 8 KB
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
 constexpr int kGatherAhead = 2;         // k-tiles a gathered operand is fetched ahead (its refill never waits for the
                                         // stage the CTA is still draining: no CTA-wide lock step per k-tile)
+constexpr int kInKernelFixupChunks = 32; // a cut tile with more chunks than this is summed by zgemm_fixup_kernel
 constexpr int kQueue = 8;               // segment queue entries (producer is <= STAGES + 1 segments ahead)
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 128 /*barriers*/ + 256 /*segment queue*/;
 constexpr int NTHREADS = 128;
@@ -673,9 +674,10 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     }
 }
 
-// fix-up of the tiles that were cut along K: sums the tile's partial fragments in k order (deterministic) and
-// applies the same permute-and-accumulate epilogue.  grid = (stream-K tiles, 8): CTA y owns fragment column
-// (j, h) = (y >> 1, y & 1) of every warp, same thread <-> element map as the main kernel.
+// fix-up of the tiles that were cut along K into MANY chunks (skinny M x N, long K: one tile, a chunk per CTA): sums the
+// tile's partial fragments in k order (deterministic) and applies the same permute-and-accumulate epilogue.
+// grid = (stream-K tiles, 32): CTA y owns fragment entry (i, j, h) = (y >> 3, (y >> 1) & 3, y & 1) of every warp, one element
+// per thread, same thread <-> element map as the main kernel; eight chunk loads in flight, additions in chunk order.
 __global__ void __launch_bounds__(NTHREADS) zgemm_fixup_kernel(const __grid_constant__ GemmParams p)
 {
     const long long tl = blockIdx.x;
@@ -683,51 +685,44 @@ __global__ void __launch_bounds__(NTHREADS) zgemm_fixup_kernel(const __grid_cons
     const long long ch_lo = base / p.sk_q, ch_hi = (base + p.ktiles - 1) / p.sk_q;
     if (ch_lo == ch_hi) return;                       // computed whole by one CTA, already in D
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int j = blockIdx.y >> 1, h = blockIdx.y & 1;
+    const int i = blockIdx.y >> 3, j = (blockIdx.y >> 1) & 3, h = blockIdx.y & 1;
     const TileGeom tg = tile_geom(p, (unsigned)(p.dp_tiles + tl));
     const WarpGeom wg = warp_geom(tg, warp & 1, warp >> 1);
-    if (j >= wg.ncnt) return;
-    double sr[4] = {0.0, 0.0, 0.0, 0.0}, si[4] = {0.0, 0.0, 0.0, 0.0};
-    // chunks in k order, four at a time: the 16 loads of a batch are independent, the additions keep their order
-    for (long long ch0 = ch_lo; ch0 <= ch_hi; ch0 += 4) {
-        double2 v[4][4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const long long ch = ch0 + u;
-            const long long first = (ch * p.sk_q) / p.ktiles;
-            const double2 *P = p.partial + (ch * p.sk_slots + (tl - first)) * (32LL * NTHREADS) + tid;
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-                if (ch <= ch_hi && i < wg.mcnt) v[u][i] = P[((i * 4 + j) * 2 + h) * NTHREADS];
-        }
-#pragma unroll
-        for (int u = 0; u < 4; ++u)
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-                if (ch0 + u <= ch_hi && i < wg.mcnt) {
-                    sr[i] += v[u][i].x;
-                    si[i] += v[u][i].y;
-                }
-    }
+    if (i >= wg.mcnt || j >= wg.ncnt) return;
     const int r = lane >> 2, c = lane & 3;
     const int rowmap = (r >> 1) + 4 * (r & 1);
+    const long long m = (long long)tg.m0 + wg.moff * 8 + rowmap + i * 8;
     const long long n = (long long)tg.n0 + wg.noff * 8 + c + j * 8 + h * 4;
-    if (n >= p.N) return;
-    const long long on = p.offN[n];
-    const double ar = p.alpha_re, ai = p.alpha_im;
+    if (m >= p.M || n >= p.N) return;
+    const long long entry = (long long)((i * 4 + j) * 2 + h) * NTHREADS + tid;
+    double sr = 0.0, si = 0.0;
+    for (long long ch0 = ch_lo; ch0 <= ch_hi; ch0 += 8) {
+        double2 v[8];
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const long long m = (long long)tg.m0 + wg.moff * 8 + rowmap + i * 8;
-        if (i >= wg.mcnt || m >= p.M) continue;
-        double2 *dst = p.D + p.offM[m] + on;
-        double2 v = make_double2(ar * sr[i] - ai * si[i], ar * si[i] + ai * sr[i]);
-        if (p.accumulate) {
-            const double2 d = *dst;
-            v.x += d.x;
-            v.y += d.y;
+        for (int u = 0; u < 8; ++u) {
+            const long long ch = ch0 + u;
+            if (ch <= ch_hi) {
+                const long long first = (ch * p.sk_q) / p.ktiles;
+                v[u] = __ldcg(p.partial + (ch * p.sk_slots + (tl - first)) * (32LL * NTHREADS) + entry);
+            }
         }
-        *dst = v;
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            if (ch0 + u <= ch_hi) { sr += v[u].x; si += v[u].y; }
     }
+    // the same arithmetic as store_fragment (alpha = 1: none; real alpha: one product per component; complex: fma pairs)
+    const double ar = p.alpha_re, ai = p.alpha_im;
+    double vx, vy;
+    if (ai != 0.0) { vx = fma(ar, sr, -ai * si); vy = fma(ar, si, ai * sr); }
+    else if (ar != 1.0) { vx = ar * sr; vy = ar * si; }
+    else { vx = sr; vy = si; }
+    double2 *dst = p.D + p.offM[m] + p.offN[n];
+    if (p.accumulate) {
+        const double2 d = *dst;
+        vx += d.x;
+        vy += d.y;
+    }
+    *dst = make_double2(vx, vy);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -885,7 +880,11 @@ cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps
     p.counters = (unsigned long long *)g.counters;      // zero on entry; the last CTA to leave zeroes them again
     if (sc.partial_bytes && !p.partial) return cudaErrorInvalidValue;
     // the in-kernel fix-up needs the dynamic deal's counter block and one arrival counter per cut tile
-    p.tile_cnt = (p.counters && sc.sk_tiles > 0 && sc.sk_tiles <= kGemmTileCounters)
+    // ... and pays when a tile has few chunks (the remainder wave behind whole tiles): the CTA that delivers the last one sums
+    // them one after the other.  A skinny M x N with a chunk per CTA (hundreds per tile) goes to zgemm_fixup_kernel, which
+    // spreads a tile's sum over 32 CTAs (measured: 20 x 20 x 128000 0.41 ms in-kernel, 0.05 + fix-up with the kernel).
+    const long long chunks_per_tile = sc.sk_tiles > 0 ? (sc.ktiles + sc.sk_q - 1) / sc.sk_q + 1 : 0;
+    p.tile_cnt = (p.counters && sc.sk_tiles > 0 && sc.sk_tiles <= kGemmTileCounters && chunks_per_tile <= kInKernelFixupChunks)
                      ? reinterpret_cast<unsigned *>(reinterpret_cast<char *>(p.counters) + kGemmTileCounterOffset) : nullptr;
     p.gA = (const double2 *)g.A; p.gB = (const double2 *)g.B;
     p.gAm = (const long long *)g.gatherAm; p.gAk = (const long long *)g.gatherAk;
@@ -902,7 +901,7 @@ cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps
     if (e != cudaSuccess) return e;
     if (launches) ++*launches;
     if (sc.sk_tiles > 0 && !p.tile_cnt) {
-        zgemm_fixup_kernel<<<dim3((unsigned)sc.sk_tiles, 8), NTHREADS, 0, stream>>>(p);
+        zgemm_fixup_kernel<<<dim3((unsigned)sc.sk_tiles, 32), NTHREADS, 0, stream>>>(p);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
         if (launches) ++*launches;

@@ -85,10 +85,12 @@ def test_twopass_epilogue_option(ctx, expr, ext):
     assert plan["epilogue"] == "twopass" and err <= TOL
 
 
-def test_in_kernel_fixup_and_fixup_kernel_agree_bit_for_bit(ctx):
-    """dynamic deal: the CTA delivering a tile's last chunk sums the chunks in k order inside the GEMM launch; static
-    deal: zgemm_fixup_kernel does.  Same k-ranges, same order: same bits, and one launch fewer."""
-    m, n, k = 150, 150, 9000
+@pytest.mark.parametrize("k,expected_launches", [(2000, [1, 2, 1]), (9000, [2, 2, 2])])
+def test_in_kernel_fixup_and_fixup_kernel_agree_bit_for_bit(ctx, k, expected_launches):
+    """dynamic deal, a cut tile with <= 32 chunks (k = 2000: 29): the CTA delivering the tile's last chunk sums the chunks in
+    k order inside the GEMM launch; static deal, or more chunks per tile (k = 9000: 34): zgemm_fixup_kernel does, 32 CTAs per
+    tile.  Same k-ranges, same order: same bits."""
+    m, n = 150, 150
     rng = np.random.default_rng(5)
     D, L, R = rc(rng, m, n), rc(rng, m, k), rc(rng, k, n)
     dL, dR = ctx.tensor_from_numpy(L), ctx.tensor_from_numpy(R)
@@ -102,7 +104,7 @@ def test_in_kernel_fixup_and_fixup_kernel_agree_bit_for_bit(ctx):
         outs.append(ctx.tensor_download(dD))
         dD.destroy()
     assert outs[0].tobytes() == outs[1].tobytes() == outs[2].tobytes()
-    assert launches == [1, 2, 1]
+    assert launches == expected_launches
     ref, sn = oracle.contract("C(m,n)+=A(m,k)*B(k,n)", D, L, R, 0.5)
     assert parity_error(outs[0], ref, sn) <= TOL
 
