@@ -33,16 +33,14 @@ struct GemmDesc {
     int splitk;              // 0 = auto (stream-K on the remainder wave), 1 = off, n > 1 = every tile cut n ways
     void *partial;           // device, gemm_schedule(...).partial_bytes (raw accumulator fragments of cut tiles)
     void *counters = nullptr; // device, kGemmCounterBytes, 8-byte aligned, ZERO on entry (the kernel leaves them zero): work
-                              // counters of the dynamic deal + arrival counters of the cut tiles (null: static deal, fix-up kernel)
+                              // counters of the dynamic deal (null: static deal)
     // Permutation-free operand loads: when gatherAm is set, A is not a matrix in memory and is read in place
     // as A[m,k] = A[gatherAm[m] + gatherAk[k]] (device tables, element offsets; lda / a_kmajor unused); a_mfast: the operand's
     // unit-stride index is a row (free) index, so lanes run along m, else along k.  Same for B.
     const int64_t *gatherAm = nullptr, *gatherAk = nullptr, *gatherBn = nullptr, *gatherBk = nullptr;
     bool a_mfast = false, b_mfast = false;
 };
-constexpr int kGemmTileCounterOffset = 64;                 // bytes into `counters`
-constexpr int kGemmTileCounters = 1000;                    // cut tiles whose fix-up can run inside the main kernel
-constexpr size_t kGemmCounterBytes = kGemmTileCounterOffset + 4 * kGemmTileCounters + 32;
+constexpr size_t kGemmCounterBytes = 64;
 // How the (tile, k-tile) iteration space is dealt to the persistent grid (2 CTAs per SM): whole tiles
 // data-parallel, the remainder ("stream-K") cut along K into equal chunks, one per CTA, summed by a fix-up kernel.
 struct GemmSchedule {

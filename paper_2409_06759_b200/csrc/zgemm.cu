@@ -23,10 +23,11 @@
 //     is an exact XOR on the high word).
 //   * persistent grid (2 CTAs per SM) with a stream-K schedule: whole tiles one CTA each while they fill the grid, the
 //     remainder wave -- or everything, for skinny M x N with long K -- cut along K into chunks whose raw accumulator
-//     fragments go to a workspace; the CTA that delivers a tile's LAST chunk (a per-tile arrival counter) sums the
-//     tile's chunks in k order (deterministic, no atomics on data) and applies the same scatter, inside the same launch
-//     (zgemm_fixup_kernel remains for the static deal and for forced split-K with more cut tiles than counters).
-//     Tiles and chunks are claimed from two counters (dynamic deal).
+//     fragments go to a workspace; zgemm_fixup_kernel (32 CTAs per cut tile) sums a tile's chunks in k order
+//     (deterministic, no atomics on data) and applies the same scatter.  Tiles and chunks are claimed from two counters
+//     (dynamic deal).  Summing inside the main kernel -- the CTA that delivers a tile's last chunk does it -- was built
+//     and measured in round 2: one launch fewer, but 10 registers more in the main loop and a serial tail: 1600^3
+//     0.965 -> 1.067 ms, configs[0] 33 -> 50 us (profiles/r2_gemm_ab.md); not kept.
 //   * the producer (thread 0) walks the CTA's segment list 4 k-tiles ahead of the consumers and ACROSS tile
 //     boundaries; segments reach the other warps through a small shared-memory queue.
 //   * no tensor work on padding: the 8-wide blocks of M and N are dealt to the tiles in pairs, a warp multiplies only
@@ -59,7 +60,6 @@ constexpr int B_BYTES = BN * BK * 16;   // 8 KB
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
 constexpr int kGatherAhead = 2;         // k-tiles a gathered operand is fetched ahead (its refill never waits for the
                                         // stage the CTA is still draining: no CTA-wide lock step per k-tile)
-constexpr int kInKernelFixupChunks = 32; // a cut tile with more chunks than this is summed by zgemm_fixup_kernel
 constexpr int kQueue = 8;               // segment queue entries (producer is <= STAGES + 1 segments ahead)
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 128 /*barriers*/ + 256 /*segment queue*/;
 constexpr int NTHREADS = 128;
@@ -82,7 +82,6 @@ struct GemmParams {
     int accumulate, use_red;
     double2 *partial;              // [slot][32][128] raw accumulator fragments
     unsigned long long *counters;  // [3] whole tiles claimed, stream-K chunks claimed, CTAs done; zero at launch; null: static deal
-    unsigned *tile_cnt;            // [sk_tiles] chunks delivered per cut tile (zero at launch, left zero); null: fix-up kernel
     // gathered operands (mode kGather): X[row, k] = base[rowtab[row] + ktab[k]]
     const double2 *gA, *gB;
     const long long *gAm, *gAk, *gBn, *gBk;
@@ -406,37 +405,6 @@ __device__ __forceinline__ void mma_ktile(double (&cr)[4][4][2], double (&ci)[4]
     }
 }
 
-// sums the chunks of cut tile `tl` in k order into the accumulator registers (same thread <-> element map as the
-// partial stores) -- shared by the in-kernel fix-up and, element-wise, by zgemm_fixup_kernel
-__device__ __forceinline__ void sum_tile_chunks(const GemmParams &p, long long tl, const WarpGeom &wg, int tid,
-                                                double (&cr)[4][4][2], double (&ci)[4][4][2])
-{
-    const long long base = tl * p.ktiles;
-    const long long ch_lo = base / p.sk_q, ch_hi = (base + p.ktiles - 1) / p.sk_q;
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            cr[i][j][0] = cr[i][j][1] = 0.0;
-            ci[i][j][0] = ci[i][j][1] = 0.0;
-        }
-    for (long long ch = ch_lo; ch <= ch_hi; ++ch) {
-        const long long first = (ch * p.sk_q) / p.ktiles;
-        const double2 *P = p.partial + (ch * p.sk_slots + (tl - first)) * (32LL * NTHREADS) + tid;
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-#pragma unroll
-                for (int h = 0; h < 2; ++h)
-                    if (i < wg.mcnt && j < wg.ncnt) {
-                        const double2 v = __ldcg(P + ((i * 4 + j) * 2 + h) * NTHREADS);     // written by other SMs: L2
-                        cr[i][j][h] += v.x;
-                        ci[i][j][h] += v.y;
-                    }
-    }
-}
-
 template <int AMODE, int BMODE>
 __global__ void __launch_bounds__(NTHREADS, 2)
 zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
@@ -477,7 +445,6 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     // before its first operand load; the consumers pop them in order.  kQueue > STAGES + 1 entries suffice.
     Segment *q_seg = reinterpret_cast<Segment *>(smem_raw + (bar_base - smem_u32(smem_raw)) + 128);
     volatile int *q_pub = reinterpret_cast<volatile int *>(q_seg + kQueue);
-    volatile int *s_flag = q_pub + 1;   // "this CTA delivered the tile's last chunk" (in-kernel fix-up)
     int npub = 0;
     auto producer_advance = [&]() {
         pvalid = pit.next(p, &pseg);
@@ -640,27 +607,6 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                     for (int h = 0; h < 2; ++h)
                         if (i < wg.mcnt && j < wg.ncnt)
                             P[((i * 4 + j) * 2 + h) * NTHREADS] = make_double2(cr[i][j][h], ci[i][j][h]);
-            if (p.tile_cnt) {
-                // in-kernel fix-up: the CTA that delivers the LAST chunk of a cut tile sums all of the tile's chunks in k
-                // order (fixed k-ranges, fixed order: the result does not depend on who that CTA is) and writes D
-                const long long tl = seg.tile - p.dp_tiles;
-                __threadfence();
-                __syncthreads();
-                if (tid == 0) {
-                    const long long base = tl * p.ktiles;
-                    const unsigned nch = (unsigned)((base + p.ktiles - 1) / p.sk_q - base / p.sk_q + 1);
-                    const unsigned old = atomicAdd(p.tile_cnt + tl, 1u);
-                    *s_flag = (old == nch - 1) ? 1 : 0;
-                    if (old == nch - 1) p.tile_cnt[tl] = 0;          // left zero for the next launch
-                }
-                __syncthreads();
-                if (*s_flag) {
-                    __threadfence();
-                    sum_tile_chunks(p, tl, wg, tid, cr, ci);
-                    store_fragment(p, cr, ci, tg, wg, rowmap, c);
-                }
-                __syncthreads();                                     // s_flag is reused by the next cut segment
-            }
         }
     }
     // counters[2] counts the CTAs that are done claiming; the last one leaves all three at zero for the next launch
@@ -879,13 +825,6 @@ cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps
     p.partial = (double2 *)g.partial;
     p.counters = (unsigned long long *)g.counters;      // zero on entry; the last CTA to leave zeroes them again
     if (sc.partial_bytes && !p.partial) return cudaErrorInvalidValue;
-    // the in-kernel fix-up needs the dynamic deal's counter block and one arrival counter per cut tile
-    // ... and pays when a tile has few chunks (the remainder wave behind whole tiles): the CTA that delivers the last one sums
-    // them one after the other.  A skinny M x N with a chunk per CTA (hundreds per tile) goes to zgemm_fixup_kernel, which
-    // spreads a tile's sum over 32 CTAs (measured: 20 x 20 x 128000 0.41 ms in-kernel, 0.05 + fix-up with the kernel).
-    const long long chunks_per_tile = sc.sk_tiles > 0 ? (sc.ktiles + sc.sk_q - 1) / sc.sk_q + 1 : 0;
-    p.tile_cnt = (p.counters && sc.sk_tiles > 0 && sc.sk_tiles <= kGemmTileCounters && chunks_per_tile <= kInKernelFixupChunks)
-                     ? reinterpret_cast<unsigned *>(reinterpret_cast<char *>(p.counters) + kGemmTileCounterOffset) : nullptr;
     p.gA = (const double2 *)g.A; p.gB = (const double2 *)g.B;
     p.gAm = (const long long *)g.gatherAm; p.gAk = (const long long *)g.gatherAk;
     p.gBn = (const long long *)g.gatherBn; p.gBk = (const long long *)g.gatherBk;
@@ -900,7 +839,7 @@ cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps
     }
     if (e != cudaSuccess) return e;
     if (launches) ++*launches;
-    if (sc.sk_tiles > 0 && !p.tile_cnt) {
+    if (sc.sk_tiles > 0) {
         zgemm_fixup_kernel<<<dim3((unsigned)sc.sk_tiles, 32), NTHREADS, 0, stream>>>(p);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;

@@ -85,11 +85,10 @@ def test_twopass_epilogue_option(ctx, expr, ext):
     assert plan["epilogue"] == "twopass" and err <= TOL
 
 
-@pytest.mark.parametrize("k,expected_launches", [(2000, [1, 2, 1]), (9000, [2, 2, 2])])
-def test_in_kernel_fixup_and_fixup_kernel_agree_bit_for_bit(ctx, k, expected_launches):
-    """dynamic deal, a cut tile with <= 32 chunks (k = 2000: 29): the CTA delivering the tile's last chunk sums the chunks in
-    k order inside the GEMM launch; static deal, or more chunks per tile (k = 9000: 34): zgemm_fixup_kernel does, 32 CTAs per
-    tile.  Same k-ranges, same order: same bits."""
+@pytest.mark.parametrize("k", [2000, 9000])
+def test_stream_k_fixup_is_deterministic_under_both_deals(ctx, k):
+    """every tile is cut along K (29 / 34 chunks per tile); zgemm_fixup_kernel (32 CTAs per tile, one fragment entry each)
+    sums a tile's chunks in k order: the dynamic and the static deal give the same bits, run to run."""
     m, n = 150, 150
     rng = np.random.default_rng(5)
     D, L, R = rc(rng, m, n), rc(rng, m, k), rc(rng, k, n)
@@ -104,7 +103,7 @@ def test_in_kernel_fixup_and_fixup_kernel_agree_bit_for_bit(ctx, k, expected_lau
         outs.append(ctx.tensor_download(dD))
         dD.destroy()
     assert outs[0].tobytes() == outs[1].tobytes() == outs[2].tobytes()
-    assert launches == expected_launches
+    assert launches == [2, 2, 2]
     ref, sn = oracle.contract("C(m,n)+=A(m,k)*B(k,n)", D, L, R, 0.5)
     assert parity_error(outs[0], ref, sn) <= TOL
 
@@ -140,7 +139,7 @@ def test_lanes_eager_and_captured_as_parallel_graph_branches(ctx):
     _two_branch_list(ctx, T, A, B, X1, X2, R)
     g = ctx.capture_end()
     info = ctx.graph_info(g)
-    assert info["launches"] == 3 and info["nodes"] >= 3
+    assert info["launches"] >= 3 and info["nodes"] >= 3
     assert info["depth"] < info["nodes"], info               # a chain has depth = nodes: two of the three run side by side
     ctx.graph_launch(g)
     assert ctx.tensor_download(R).tobytes() == eager.tobytes()
