@@ -466,6 +466,39 @@ def ccsd_jacobi(B, e_occ, e_virt, iterations):
     return T1, T2, energies
 
 
+def residual_norm(*residuals):
+    """|R| = sqrt(sum over all given residual tensors of <R|R>): the "norm of the residual vector" the paper's tables quote
+    per converged calculation."""
+    return float(np.sqrt(sum(np.vdot(r, r).real for r in residuals)))
+
+
+def ccsd_diis(B, e_occ, e_virt, iterations, depth=6):
+    """The CCSD iteration with DIIS extrapolation over the combined (t1, t2) vector: error vector e_k = (R1 / D1, R2 / D2)
+    at the current amplitudes, trial vector = amplitudes + e_k, next amplitudes = the combination of the last `depth`
+    trial vectors minimising |sum c_i e_i| with <e_i|e_j> = <e1_i|e1_j> + <e2_i|e2_j>.
+    Returns (T1, T2, [E_corr of the amplitudes each residual evaluation saw], [|R| = residual norm of each evaluation])."""
+    v, o = B["fvo"].shape
+    T1 = np.zeros((v, o), dtype=np.complex128, order="F")
+    T2 = np.zeros((v, v, o, o), dtype=np.complex128, order="F")
+    ev, eo = -np.asarray(e_virt, dtype=np.float64), np.asarray(e_occ, dtype=np.float64)
+    trial, err, energies, norms = [], [], [], []
+    for _ in range(iterations):
+        E, R1, R2 = ccsd_residual_program(B, T1, T2)
+        energies.append(E)
+        norms.append(residual_norm(R1, R2))
+        e1 = denominator_update(np.zeros_like(T1), R1, [ev, eo], 1.0)
+        e2 = denominator_update(np.zeros_like(T2), R2, [ev, ev, eo, eo], 1.0)
+        trial.append((np.asfortranarray(T1 + e1), np.asfortranarray(T2 + e2)))
+        err.append((e1, e2))
+        trial, err = trial[-depth:], err[-depth:]
+        m = len(err)
+        Bm = np.array([[np.vdot(err[i][0], err[j][0]) + np.vdot(err[i][1], err[j][1]) for j in range(m)] for i in range(m)])
+        c = diis_coefficients(Bm) if m > 1 else np.ones(1)
+        T1 = np.asfortranarray(sum(ci * t[0] for ci, t in zip(c, trial)))
+        T2 = np.asfortranarray(sum(ci * t[1] for ci, t in zip(c, trial)))
+    return T1, T2, energies, norms
+
+
 # ------------------------------------------------------------------------------------------
 # config 4: CCSDT piece
 # ------------------------------------------------------------------------------------------

@@ -215,11 +215,12 @@ def ccsd_residual(ctx, B, T1, T2, R1=None, R2=None):
     return E, R1, R2
 
 
-def ccd_solve(ctx, B, e_occ, e_virt, iterations, T=None):
+def ccd_solve(ctx, B, e_occ, e_virt, iterations, T=None, norms=None):
     """Jacobi iterations of the CCD amplitude equations (PAPER.md:212 energy denominators, 406-410 "CC
     iteration"):  T <- T + R(T) / (e_i + e_j - e_a - e_b), from T (default: a zero tensor, whose first step is the MP2
     guess).  Every step is `ccd_residual` + one `tcb_denominator_update` + the rank-0 energy contraction; only the
-    16-byte energy comes back to the host per iteration.  Returns (T, [E_corr after each step])."""
+    16-byte energy comes back to the host per iteration.  norms: a list that receives the residual norm |R(T)| each
+    iteration started from (one `tcb_dot`).  Returns (T, [E_corr after each step])."""
     import numpy as np
     v, _, o, _ = B["vvoo"].extents
     if T is None:
@@ -229,6 +230,8 @@ def ccd_solve(ctx, B, e_occ, e_virt, iterations, T=None):
     energies = []
     for _ in range(iterations):
         ccd_residual(ctx, B, T, R)
+        if norms is not None:
+            norms.append(residual_norm(ctx, R))     # |R(T)| of the amplitudes this iteration started from
         ctx.denominator_update(T, R, [ev, ev, eo, eo], 1.0)
         E = ccd_energy(ctx, B, T)
         energies.append(complex(ctx.tensor_download(E)))
@@ -351,6 +354,86 @@ def ccsd_solve(ctx, B, e_occ, e_virt, iterations):
     R1.destroy()
     R2.destroy()
     return T1, T2, energies
+
+
+def residual_norm(ctx, *residuals):
+    """|R| = sqrt(sum <R|R>) over the given residual tensors -- the "norm of the residual vector" quoted per calculation in
+    the paper: one `tcb_dot` into a rank-0 tensor per residual, read back as one number."""
+    import math
+    s = ctx.tensor_create(())
+    total = 0.0
+    for R in residuals:
+        ctx.dot(s, R, R, True, 1.0)
+        total += complex(ctx.tensor_download(s)).real
+    s.destroy()
+    return math.sqrt(total)
+
+
+def ccsd_solve_diis(ctx, B, e_occ, e_virt, iterations, depth=6):
+    """The CCSD iteration with DIIS over the combined (t1, t2) vector (oracle: cc.ccsd_diis): per evaluation the residuals,
+    their norm, the error vectors e = R / D (`tcb_denominator_divide`), the trial vectors, one new row of
+    <e_i|e_j> = <e1_i|e1_j> + <e2_i|e2_j> (`tcb_dot`), and the extrapolated amplitudes (`tcb_add`) -- all on the device;
+    the depth x depth system is solved on the host.
+    Returns (T1, T2, [E_corr of the amplitudes each evaluation saw], [residual norm |R| of each evaluation])."""
+    import numpy as np
+    v, o = B["fvo"].extents
+    s1, s2 = (v, o), (v, v, o, o)
+    T1, T2 = ctx.tensor_create(s1), ctx.tensor_create(s2)
+    R1, R2 = ctx.tensor_create(s1), ctx.tensor_create(s2)
+    ev, eo = -np.asarray(e_virt, dtype=np.float64), np.asarray(e_occ, dtype=np.float64)
+    trial, err, energies, norms = [], [], [], []
+    Bm = np.zeros((0, 0), dtype=np.complex128)
+    s = ctx.tensor_create(())
+
+    def dot(X, Y):
+        ctx.dot(s, X, Y, True, 1.0)
+        return complex(ctx.tensor_download(s))
+
+    for _ in range(iterations):
+        E, _, _ = ccsd_residual(ctx, B, T1, T2, R1, R2)
+        energies.append(complex(ctx.tensor_download(E)))
+        E.destroy()
+        norms.append(float(np.sqrt(dot(R1, R1).real + dot(R2, R2).real)))
+        if len(err) == depth:                      # the oldest pair leaves; its tensors are reused
+            (e1, e2), (t1, t2) = err.pop(0), trial.pop(0)
+            Bm = Bm[1:, 1:]
+        else:
+            e1, e2, t1, t2 = (ctx.tensor_create(x, zero=False) for x in (s1, s2, s1, s2))
+        ctx.denominator_divide(e1, R1, [ev, eo], 1.0)
+        ctx.denominator_divide(e2, R2, [ev, ev, eo, eo], 1.0)
+        ctx.add("t(a,i)=T(a,i)", t1, T1, 1.0)
+        ctx.add("t(a,i)+=e(a,i)", t1, e1, 1.0)
+        ctx.add("t(a,b,i,j)=T(a,b,i,j)", t2, T2, 1.0)
+        ctx.add("t(a,b,i,j)+=e(a,b,i,j)", t2, e2, 1.0)
+        err.append((e1, e2))
+        trial.append((t1, t2))
+        m = len(err)
+        row = np.array([dot(err[i][0], e1) + dot(err[i][1], e2) for i in range(m)])      # <e_i|e_new>; B is Hermitian
+        Bn = np.zeros((m, m), dtype=np.complex128)
+        Bn[:m - 1, :m - 1] = Bm
+        Bn[:, m - 1] = row
+        Bn[m - 1, :] = row.conj()
+        Bn[m - 1, m - 1] = row[m - 1]
+        Bm = Bn
+        if m > 1:
+            A = np.zeros((m + 1, m + 1), dtype=np.complex128)
+            A[:m, :m] = Bm
+            A[:m, m] = A[m, :m] = 1.0
+            rhs = np.zeros(m + 1, dtype=np.complex128)
+            rhs[m] = 1.0
+            c = np.linalg.solve(A, rhs)[:m]
+        else:
+            c = np.ones(1, dtype=np.complex128)
+        for k, (ci, (ta, tb)) in enumerate(zip(c, trial)):
+            op = "=" if k == 0 else "+="
+            ctx.add(f"T(a,i){op}t(a,i)", T1, ta, complex(ci))
+            ctx.add(f"T(a,b,i,j){op}t(a,b,i,j)", T2, tb, complex(ci))
+    for pair in err + trial:
+        for x in pair:
+            x.destroy()
+    for x in (R1, R2, s):
+        x.destroy()
+    return T1, T2, energies, norms
 
 
 CCD_FLOPS = lambda o, v: 8.0 * (                 # 8 real flop per complex multiply-add

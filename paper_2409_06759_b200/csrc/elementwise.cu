@@ -219,7 +219,8 @@ cudaError_t launch_denominator_update(void *T, const void *R, int rank, const in
         p.e[k] = k < rank ? extent[k] : 1;
         p.eps_at[k] = k < rank ? eps_at[k] : -1;
         n *= p.e[k];
-        if (k < rank && (slab < 2048 || p.ninner == 0) && slab * p.e[k] <= (1LL << 30)) {
+        // the inner block is a contiguous PREFIX of the dims: it stops growing at the first dim that does not fit
+        if (k < rank && p.ninner == k && (slab < 2048 || k == 0) && slab * p.e[k] <= (1LL << 30)) {
             slab *= p.e[k];
             p.ninner = k + 1;
         }

@@ -547,6 +547,9 @@ cudaError_t build_plan(const PermSumDesc &d, OrbitPlan &plan)
     e = cudaMemcpy(tables, orbits.data(), b0, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(tables + o1, order.data(), b1, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(tables + o2, group_start.data(), b2, cudaMemcpyHostToDevice);
+    // the sources are pageable: cudaMemcpy may return once they are staged, before the DMA has landed, and the kernel runs on
+    // a non-blocking stream that the legacy stream does not order -- wait for the copies here (once per shape and term set)
+    if (e == cudaSuccess) e = cudaStreamSynchronize(0);
     if (e != cudaSuccess) { cudaFree(tables); return e; }
     p.orbits = reinterpret_cast<const OrbitEntry *>(tables);
     p.slab_order = reinterpret_cast<const unsigned *>(tables + o1);

@@ -338,3 +338,41 @@ def test_cuda_graph_of_the_residual_call_list_replays_bit_identically(ctx):
     ctx.set_option("kernel_timing", "off")
     with pytest.raises(pkg.TcbError):
         ctx.capture_end()                                       # nothing open
+
+
+def test_ccsd_diis_and_residual_norms_follow_the_oracle(ctx):
+    """DIIS around the CCSD iteration and the residual norm per evaluation, every tensor
+    operation on the device, against oracle cc.ccsd_diis (pinned to the Fock-space projections in tests/test_oracle_cc.py)."""
+    o, v = 3, 4
+    rng = np.random.default_rng(46)
+    n = o + v
+    c = lambda *s: rng.standard_normal(s) + 1j * rng.standard_normal(s)
+    A = c(n, n, n, n)
+    A = A - A.transpose(1, 0, 2, 3)
+    A = A - A.transpose(0, 1, 3, 2)
+    g = 0.05 * 0.5 * (A + A.transpose(2, 3, 0, 1).conj())
+    e = np.concatenate([np.linspace(-2.0, -0.5, o), np.linspace(0.5, 3.0, v)])
+    f = 0.05 * c(n, n)
+    f = f + f.conj().T
+    f[np.diag_indices(n)] = e
+    B = cc.ccsd_blocks(o, f, g)
+    dB = {k: ctx.tensor_from_numpy(x) for k, x in B.items()}
+    its = 10
+    dT1, dT2, energies, norms = ccd.ccsd_solve_diis(ctx, dB, e[:o], e[o:], its)
+    T1, T2, e_ref, n_ref = cc.ccsd_diis(B, e[:o], e[o:], its)
+    assert np.max(np.abs(ctx.tensor_download(dT1) - T1)) <= 1e-10 * np.abs(T1).max()
+    assert np.max(np.abs(ctx.tensor_download(dT2) - T2)) <= 1e-10 * np.abs(T2).max()
+    for k in range(its):
+        assert abs(energies[k] - e_ref[k]) <= 1e-10 * max(abs(e_ref[-1]), 1e-300)
+        assert abs(norms[k] - n_ref[k]) <= 1e-10 * n_ref[0]
+    assert norms[-1] < 1e-6 * norms[0]                          # it converges; |R| is what the paper's tables quote
+    # the CCD Jacobi solver reports its residual norms the same way
+    B2, T_mp2, eo, ev = synth.config_ccd(3, 5)
+    dB2 = {k: ctx.tensor_from_numpy(x) for k, x in B2.items()}
+    got = []
+    ccd.ccd_solve(ctx, dB2, eo, ev, 3, norms=got)
+    Tr = np.zeros_like(T_mp2)
+    for k in range(3):
+        R = cc.ccd_residual_program(B2, Tr)
+        assert abs(got[k] - cc.residual_norm(R)) <= 1e-11 * cc.residual_norm(cc.ccd_residual_program(B2, np.zeros_like(T_mp2)))
+        Tr = cc.denominator_update(Tr, R, [-ev, -ev, eo, eo], 1.0)

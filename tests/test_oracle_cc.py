@@ -266,3 +266,28 @@ def test_triples_singles_term_against_the_fock_space_matrix_element():
     assert abs(e - 0.25 * np.einsum("ai,jkbc,abcijk->", t1.conj(), g[:o, :o, o:, o:], t3)) <= 1e-13 * abs(e0)
     # T3 Phi0 has the right norm: 1/36 of the sum over all index tuples = sum over unique triples
     assert abs(np.vdot(fs.apply_T3(t3, fs.phi0), fs.apply_T3(t3, fs.phi0)) - np.sum(np.abs(t3) ** 2) / 36.0) <= 1e-13 * np.sum(np.abs(t3) ** 2)
+
+
+def test_ccsd_diis_fixed_point_is_the_fock_space_solution_and_residual_norm_is_the_vector_norm():
+    """DIIS around the CCSD iteration (combined t1, t2 error vector): the amplitudes it converges to zero the Fock-space
+    singles and doubles projections of e^-T H e^T (PAPER Eq. 3) -- the same fixed point as the Jacobi iteration, reached in
+    fewer evaluations; the residual norm it reports is the 2-norm of the Fock-space projections at the
+    amplitudes of that evaluation, and its first value is that of the bare driver terms (f_ai, <ab||ij>)."""
+    o, v = 3, 3
+    f, g, eo, ev = _ccsd_problem(o, v, 46)
+    B = cc.ccsd_blocks(o, f, g)
+    T1, T2, energies, norms = cc.ccsd_diis(B, eo, ev, 16)
+    e0, r1, r2 = cc.fock_space_residuals(o, v, f, g, T2, T1)
+    scale = np.abs(g).max()
+    assert np.abs(r1).max() <= 1e-12 * scale and np.abs(r2).max() <= 1e-12 * scale
+    # energies[k] belongs to the amplitudes evaluation k saw: one more evaluation at the converged amplitudes gives e0
+    e_last, r1p, r2p = cc.ccsd_residual_program(B, T1, T2)
+    assert abs(e_last - e0) <= 1e-12 * abs(e0)
+    assert abs(cc.residual_norm(r1p, r2p) - np.sqrt(np.sum(np.abs(r1) ** 2) + np.sum(np.abs(r2) ** 2))) <= 1e-13 * scale
+    assert abs(norms[0] - np.sqrt(np.sum(np.abs(B["fvo"]) ** 2) + np.sum(np.abs(B["vvoo"]) ** 2))) <= 1e-14 * norms[0]
+    assert energies[0] == 0
+    # fewer evaluations than Jacobi: after 8 evaluations the DIIS residual norm is far below the Jacobi one
+    Tj1, Tj2, _ = cc.ccsd_jacobi(B, eo, ev, 7)
+    _, j1, j2 = cc.ccsd_residual_program(B, Tj1, Tj2)
+    assert norms[7] < 0.1 * cc.residual_norm(j1, j2)
+    assert all(norms[k + 1] < norms[k] for k in range(8))
