@@ -638,6 +638,19 @@ int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor
         return TCB_OK;
     }
 
+    if (P.outer) {
+        OuterDesc g;
+        g.M = P.M; g.N = P.N;
+        g.A = TA->ptr; g.B = TB->ptr; g.D = D->ptr;
+        g.offM = cp->d_tables;
+        g.offN = cp->d_tables + P.offM.size();
+        g.rowA = cp->d_aux[0]; g.rowB = cp->d_aux[2];
+        g.alpha_re = alpha.re; g.alpha_im = alpha.im;
+        g.accumulate = P.accumulate;
+        TimedLaunch tl(ctx, kClsZgemm, P.flops, P.bytes);
+        TCB_CUDA(ctx, launch_outer(g, cur_stream(ctx), &ctx->launches));
+        return TCB_OK;
+    }
     const size_t bytesA = P.a.permuted ? align_up((size_t)P.a.elems * 16, 1024) : 0;
     const size_t bytesB = P.b.permuted ? align_up((size_t)P.b.elems * 16, 1024) : 0;
     const size_t bytesP = align_up(P.partial_bytes, 1024);

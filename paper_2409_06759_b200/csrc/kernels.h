@@ -72,6 +72,16 @@ struct GemvDesc {
     void *partial;           // device, gemv_ksplit(M, K, kfast) * M complex128 when the split is > 1
 };
 int gemv_ksplit(int64_t M, int64_t K, bool kfast);
+// regime "outer product" (K = 1):  D[offM[m] + offN[n]] (+)= alpha * A[rowA[m]] * B[rowB[n]]   (device tables, element offsets)
+struct OuterDesc {
+    int64_t M, N;
+    const void *A, *B;
+    void *D;
+    const int64_t *rowA, *rowB, *offM, *offN;
+    double alpha_re, alpha_im;
+    bool accumulate;
+};
+cudaError_t launch_outer(const OuterDesc &g, cudaStream_t stream, int64_t *launches);
 cudaError_t launch_gemv(const GemvDesc &g, cudaStream_t stream, int64_t *launches);
 
 // ---- S3: tensor transposition, and the permuted add built on it ------------------------------------------

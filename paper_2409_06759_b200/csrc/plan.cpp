@@ -221,6 +221,27 @@ int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const 
         return TCB_OK;
     }
 
+    // (vii) regime "outer product": nothing is contracted (tt(a,b,i,j) = T1(a,i) T1(b,j)) -- a store stream, no tensor work:
+    // both operands are read through row tables in D's order of their indices
+    if (P.K == 1 && !opt.permute_always) {
+        std::vector<const Lab *> fa_, fb_;
+        for (const Lab *l : seqD) (posA(l) >= 0 ? fa_ : fb_).push_back(l);
+        P.outer = true;
+        P.offM = offset_table(fa_);
+        P.offN = offset_table(fb_);
+        P.a.gather_row = offset_table(fa_, swapped ? 2 : 1);
+        P.b.gather_row = offset_table(fb_, swapped ? 1 : 2);
+        P.a.rows = P.M; P.b.rows = P.N; P.a.elems = sizeA; P.b.elems = sizeB;
+        for (const Lab *l : fa_) P.m_labels.push_back(l->name);
+        for (const Lab *l : fb_) P.n_labels.push_back(l->name);
+        P.splitk = opt.splitk;
+        P.flops = 8.0 * (double)P.M * (double)P.N;
+        P.bytes = 16.0 * ((double)sizeA + (double)sizeB + (double)sizeD * (e.accumulate ? 2.0 : 1.0));
+        P.est_seconds = P.bytes / 6.0e12 + 4e-6;
+        *out = std::move(P);
+        return TCB_OK;
+    }
+
     // (iii)-(viii) how each operand reaches the GEMM, decided by a cost model.  Per operand three feeds exist:
     //   tma     : read in place by 2-D TMA boxes -- needs a matrix-shaped memory order whose contracted order is the common one;
     //   gather  : read in place through a row table and a column table (any index order);
@@ -364,7 +385,7 @@ int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const 
 std::string ContractPlan::describe() const
 {
     char buf[1280];
-    auto feed = [&](const OperandPlan &o) { return gemv ? "table" : o.permuted ? "permute" : o.gather ? "gather" : "tma"; };
+    auto feed = [&](const OperandPlan &o) { return (gemv || outer) ? "table" : o.permuted ? "permute" : o.gather ? "gather" : "tma"; };
     std::snprintf(buf, sizeof buf,
                   "{\"M\": %lld, \"N\": %lld, \"K\": %lld, \"m_labels\": \"%s\", \"n_labels\": \"%s\", "
                   "\"k_labels\": \"%s\", \"row_operand\": \"%s\", \"permute_A\": %s, \"permute_B\": %s, "
@@ -374,7 +395,7 @@ std::string ContractPlan::describe() const
                   (long long)M, (long long)N, (long long)K, join(m_labels).c_str(), join(n_labels).c_str(),
                   join(k_labels).c_str(), swapped ? "R" : "L", a.permuted ? "true" : "false",
                   b.permuted ? "true" : "false", a.kmajor ? "K-major" : "M-major", b.kmajor ? "K-major" : "M-major",
-                  feed(a), feed(b), splits, gemv ? "gemv" : "gemm", twopass ? "twopass" : "fused-scatter",
+                  feed(a), feed(b), splits, gemv ? "gemv" : outer ? "outer" : "gemm", twopass ? "twopass" : "fused-scatter",
                   accumulate ? "true" : "false", flops, bytes, est_seconds * 1e6);
     return buf;
 }

@@ -51,6 +51,7 @@ struct ContractPlan {
     OperandPlan a, b;
     std::vector<int64_t> offM, offN;
     // GEMV route (N = 1: one operand fully contracted): the other operand is read in place through these tables
+    bool outer = false;      // K = 1 (nothing contracted): the store-stream kernel, rows / columns through a.gather_row / b.gather_row
     bool gemv = false, gemv_kfast = false;
     std::vector<int64_t> offAm, offAk, offBk;
     int splits = 1;          // pieces per tile when every tile is cut along K (skinny shapes), else 1

@@ -195,3 +195,15 @@ def test_graph_launch_is_refused_after_the_workspace_moved(ctx):
     assert ei.value.code == binding.TCB_EINVAL
     ctx.sync()
     ctx.graph_destroy(g)
+
+
+@pytest.mark.parametrize("expr,ext", [
+    ("tt(a,b,i,j)=T1(a,i)*T2(b,j)", dict(a=37, b=29, i=5, j=7)),           # the CCSD outer product
+    ("tt(a,b,i,j)+=T1(a,i)*T2(b,j)", dict(a=300, b=3, i=2, j=41)),
+    ("D(j,a)+=L(a)*R(j)", dict(a=1000, j=33)),
+    ("D(b,a,x)=R(b,x)*L(a)", dict(a=17, b=9, x=1)),                        # D's unit-stride index in the second operand
+])
+def test_outer_product_route(ctx, expr, ext):
+    """K = 1 (nothing contracted): the store-stream kernel of gemv.cu instead of a GEMM with K padded to 4"""
+    err, plan, _ = run(ctx, expr, ext, alpha=0.75 - 0.5j, seed=len(expr))
+    assert plan["route"] == "outer" and plan["K"] == 1 and err <= TOL
