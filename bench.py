@@ -258,11 +258,14 @@ def run_ours(args, rank, world, local_rank):
         upload(0)
         ctx_up.sync()
         for n in range(nsteps):
-            if n + 1 < nsteps:
-                upload((n + 1) % 2)                               # overlaps with this step's kernel
             Vs, Ts = sets[n % 2]
             ctx.tensor_upload_raw(Rt, host_Rin.data_ptr())         # R_in travels too ('+=' reads it)
             ctx.contract(EXPR, Rt, Vs, Ts, 0.5)
+            # the next step's operands are queued on the host->device copy engine AFTER this step's R_in (the engine serves
+            # its queue in order: queued before it, the 26.6 GB would hold the kernel back by 0.5 s) and cross PCIe while
+            # the kernel runs
+            if n + 1 < nsteps:
+                upload((n + 1) % 2)
             ctx.tensor_download_raw(Rt, host_R.data_ptr())         # blocks until R is on the host
             ctx_up.sync()
 
