@@ -21,6 +21,7 @@
 // Terms are added in the caller's order with separately rounded products and sums: bit-identical to the generic
 // kernel and to the oracle.
 #include "kernels.h"
+#include "ptx.cuh"
 
 #include <algorithm>
 #include <cstdlib>
@@ -32,6 +33,8 @@
 namespace tcb {
 
 namespace {
+
+using namespace ptx;
 
 constexpr int T6 = 6;                       // cube edge
 constexpr int kCube = T6 * T6 * T6;         // 216 elements, 3456 bytes = 27 x 128
@@ -66,33 +69,6 @@ struct OrbitParams {
     double2 *D;
 };
 
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "ORB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-        "@P1 bra ORB_DONE;\n"
-        "bra ORB_WAIT;\n"
-        "ORB_DONE:\n"
-        "}\n" ::"r"(bar),
-        "r"(parity)
-        : "memory");
-}
 __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap *tm, int c0, int c1, int c2, int c3,
                                             uint32_t bar)
 {

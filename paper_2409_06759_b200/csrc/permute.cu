@@ -20,6 +20,7 @@
 // (no division in the loop); boundary tiles mask with packed per-dim indices.  All global offsets are 64-bit
 // (V of config 3 is 25.6 GB).
 #include "kernels.h"
+#include "ptx.cuh"
 
 #include <algorithm>
 #include <cstdlib>
@@ -27,6 +28,8 @@
 namespace tcb {
 
 namespace {
+
+using namespace ptx;
 
 constexpr int PT = 256;            // threads per CTA
 constexpr int NW = PT / 32;
@@ -51,44 +54,11 @@ struct PermParams {
     double ar, ai;
 };
 
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "PERM_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-        "@P1 bra PERM_DONE;\n"
-        "bra PERM_WAIT;\n"
-        "PERM_DONE:\n"
-        "}\n" ::"r"(bar),
-        "r"(parity)
-        : "memory");
-}
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
 {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
                  "l"(src), "r"(bytes), "r"(bar)
                  : "memory");
-}
-__device__ __forceinline__ double2 lds128(uint32_t addr)
-{
-    double2 v;
-    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
-    return v;
 }
 
 // tile coordinates of one cursor (the load cursor runs `stages` tiles ahead of the store cursor)

@@ -43,6 +43,7 @@
 //     consumer side does not know the difference.  Lanes run along whichever of m / k is contiguous in memory.
 // Measured history and the ncu evidence for each of these: DESIGN.md 6.2, profiles/r1b_zgemm_ncu_full.md.
 #include "kernels.h"
+#include "ptx.cuh"
 
 #include <algorithm>
 #include <cstdlib>
@@ -52,6 +53,8 @@
 namespace tcb {
 
 namespace {
+
+using namespace ptx;
 
 constexpr int BM = kGemmBM, BN = kGemmBN, BK = kGemmBK;
 constexpr int STAGES = 4;
@@ -89,34 +92,7 @@ struct GemmParams {
 };
 enum { kTmaK = 0, kTmaM = 1, kGather = 2 };   // how an operand reaches shared memory
 
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "LAB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-        "@P1 bra DONE;\n"
-        "bra LAB_WAIT;\n"
-        "DONE:\n"
-        "}\n" ::"r"(bar),
-        "r"(parity)
-        : "memory");
-}
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *tm, int c0, int c1, uint32_t bar)
 {
     asm volatile(
@@ -176,12 +152,6 @@ __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b)
 __device__ __forceinline__ double neg_exact(double x)
 {
     return __hiloint2double(__double2hiint(x) ^ 0x80000000, __double2loint(x));
-}
-__device__ __forceinline__ double2 lds128(uint32_t addr)
-{
-    double2 v;
-    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
-    return v;
 }
 
 // ---- work decomposition ("stream-K": data-parallel full waves, the remainder cut along K) ------------------
