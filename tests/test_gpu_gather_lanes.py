@@ -1,5 +1,6 @@
 """-m gpu: the round-2 paths against the oracle -- permutation-free operand loads, the two-pass epilogue
-option, the in-kernel stream-K fix-up, lanes (8(f)-4) eager and captured, and the capture contract."""
+option, the stream-K fix-up under both deals, the outer-product route, lanes (8(f)-4) eager and captured, and the capture
+contract."""
 import numpy as np
 import pytest
 
@@ -42,7 +43,7 @@ GATHER_CASES = [
     ("D(a,b)+=L(c,a,d)*R(d,b,c)", dict(a=37, b=29, c=19, d=23)),
     # rank 6 x rank 4 (the T3 term with W in a non-matrix order)
     ("X(a,b,c,i,j,k)=W(b,d,c,k)*T(a,d,i,j)", dict(a=6, b=5, c=7, d=9, i=3, j=4, k=2)),
-    # skinny, long K, operand gathered: stream-K chunks + in-kernel fix-up over gathered k-tiles
+    # skinny, long K, operand gathered: stream-K chunks over gathered k-tiles, summed by the fix-up kernel
     ("F(m,i)+=V(m,n,e,f)*T(e,f,i,n)", dict(m=6, i=5, n=7, e=31, f=29)),
     ("F(a,e)+=T(a,f,m,n)*V(m,n,e,f)", dict(a=20, e=18, f=41, m=6, n=5)),
     # extent-1 indices and a K tail of 1
