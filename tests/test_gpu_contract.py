@@ -179,3 +179,38 @@ def test_errors_leave_D_untouched(ctx):
         ctx.contract("D(m,n)+=L(m,k)*R(k,n)", dD, dD, dR, 1.0)
     assert ei.value.code in (pkg.TCB_EALIAS, pkg.TCB_ESHAPE)
     assert np.array_equal(ctx.tensor_download(dD), D)
+
+
+def _random_contraction(rng):
+    """a random valid binary contraction: ranks 0..6 for D, 1..6 for L and R, every label twice, random index orders"""
+    labels = list("abcdefghijkl")
+    for _ in range(1000):
+        nfl, nfr, nc = int(rng.integers(0, 4)), int(rng.integers(0, 4)), int(rng.integers(0, 4))
+        if nfl + nc == 0 or nfr + nc == 0 or nfl + nc > 6 or nfr + nc > 6 or nfl + nfr > 6:
+            continue
+        labs = labels[:nfl + nfr + nc]
+        fl, fr, cc = labs[:nfl], labs[nfl:nfl + nfr], labs[nfl + nfr:]
+        ext = {x: int(rng.choice([1, 2, 3, 5, 7, 9, 16, 23])) for x in labs}
+        if np.prod([ext[x] for x in fl + cc]) > 60000 or np.prod([ext[x] for x in fr + cc]) > 60000:
+            continue
+        d, l, r = list(fl + fr), list(fl + cc), list(fr + cc)
+        rng.shuffle(d); rng.shuffle(l); rng.shuffle(r)
+        op = "+=" if rng.integers(2) else "="
+        return f"D({','.join(d)}){op}L({','.join(l)})*R({','.join(r)})", ext
+    raise RuntimeError("no contraction drawn")
+
+
+@pytest.mark.parametrize("loads", ["auto", "gather", "permute"])
+def test_random_contractions_under_every_operand_feed(ctx, loads):
+    """80 random index patterns (ranks 0..6, extents 1..23, '=' and '+=', complex alpha) per planner setting: whatever the
+    cost model or the forced option picks -- TMA in place, gathered, transposed first, GEMV, outer product -- the result is the
+    oracle's within 1e-11 of each element's own snorm"""
+    rng = np.random.default_rng({"auto": 101, "gather": 102, "permute": 103}[loads])
+    routes = {}
+    for case in range(80):
+        expr, ext = _random_contraction(rng)
+        alpha = complex(rng.choice([1.0, -1.0, 0.5, 0.3 - 0.7j]))
+        plan, _ = run_case(ctx, expr, ext, alpha=alpha, seed=case, options={"operand_loads": loads})
+        key = (plan["route"], plan["feed_A"], plan["feed_B"])
+        routes[key] = routes.get(key, 0) + 1
+    assert len(routes) >= 4, routes               # the draw exercises several routes and feeds
