@@ -182,11 +182,11 @@ def test_errors_leave_D_untouched(ctx):
 
 
 def _random_contraction(rng):
-    """a random valid binary contraction: ranks 0..6 for D, 1..6 for L and R, every label twice, random index orders"""
+    """a random valid binary contraction: ranks 1..6 (a rank-0 D has its own test), every label twice, random index orders"""
     labels = list("abcdefghijkl")
     for _ in range(1000):
         nfl, nfr, nc = int(rng.integers(0, 4)), int(rng.integers(0, 4)), int(rng.integers(0, 4))
-        if nfl + nc == 0 or nfr + nc == 0 or nfl + nc > 6 or nfr + nc > 6 or nfl + nfr > 6:
+        if nfl + nc == 0 or nfr + nc == 0 or nfl + nfr == 0 or nfl + nc > 6 or nfr + nc > 6 or nfl + nfr > 6:
             continue
         labs = labels[:nfl + nfr + nc]
         fl, fr, cc = labs[:nfl], labs[nfl:nfl + nfr], labs[nfl + nfr:]
@@ -202,7 +202,7 @@ def _random_contraction(rng):
 
 @pytest.mark.parametrize("loads", ["auto", "gather", "permute"])
 def test_random_contractions_under_every_operand_feed(ctx, loads):
-    """80 random index patterns (ranks 0..6, extents 1..23, '=' and '+=', complex alpha) per planner setting: whatever the
+    """80 random index patterns (ranks 1..6, extents 1..23, '=' and '+=', complex alpha) per planner setting: whatever the
     cost model or the forced option picks -- TMA in place, gathered, transposed first, GEMV, outer product -- the result is the
     oracle's within 1e-11 of each element's own snorm"""
     rng = np.random.default_rng({"auto": 101, "gather": 102, "permute": 103}[loads])
