@@ -613,3 +613,102 @@ def triples_singles_term(t1, oovv, t3, long_double=True):
     Y = _o.contract("Y(a,i)=T(a,b,c,i,j,k)*W(j,k,b,c)", np.zeros((v, o), dtype=np.complex128, order="F"), t3, oovv, 1.0,
                     long_double=long_double, want_snorm=False)[0]
     return Y, 0.25 * np.vdot(t1, Y)
+
+
+# ------------------------------------------------------------------------------------------
+# CCSDT (next row 8(f)-3: "CCSDT iterations"; the paper's production target beyond CCSD).
+# The paper prints only Eqs. (1)-(4).  The equations below were obtained by enumerating every connected contraction
+# topology of H with T2 and T3 and fitting the coefficients to the Fock-space projections of exp(-T) H exp(T) |Phi0>
+# (Eq. 3) at o = v = 5 with a NON-Hermitian H (fit residual 4e-15, every coefficient a simple rational); they are PINNED
+# to the Fock space in tests/test_oracle_cc.py.  T1 enters through the exact similarity transformation of the integrals
+# (`dress_t1`), so the amplitude equations themselves are written for T = T2 + T3 only.
+# ------------------------------------------------------------------------------------------
+def dress_t1(o, f, g, t1):
+    """(f~, g~) with  sum f~ .. + 1/4 sum g~ .. = exp(-T1) H exp(T1):  exp(-T1) a+_p exp(T1) = sum_q a+_q X[q,p],
+    exp(-T1) a_q exp(T1) = sum_r Y[q,r] a_r with X = 1 - tau, Y = 1 + tau, tau[a,i] = t_i^a (virtual row, occupied column);
+    h~ = X h Y, g~[PQRS] = X[P,p] X[Q,q] g[pqrs] Y[r,R] Y[s,S]; h = f - sum_i <pi||qi> is the bare one-electron part and
+    f~ = h~ + sum_i g~[P i Q i] the Fock matrix of the dressed integrals."""
+    n = f.shape[0]
+    tau = np.zeros((n, n), dtype=np.complex128)
+    tau[o:, :o] = t1
+    X, Y = np.eye(n) - tau, np.eye(n) + tau
+    h = f - np.einsum("piqi->pq", g[:, :o, :, :o])
+    ht = X @ h @ Y
+    gt = np.einsum("Pp,Qq,pqrs,rR,sS->PQRS", X, X, g, Y, Y)
+    ft = ht + np.einsum("piqi->pq", gt[:, :o, :, :o])
+    return ft, gt
+
+
+def _perm_sign(p):
+    s, p = 1, list(p)
+    for i in range(len(p)):
+        while p[i] != i:
+            j = p[i]
+            p[i], p[j] = p[j], p[i]
+            s = -s
+    return s
+
+
+def antisymmetrise_abc_ijk(X):
+    """A3 X = sum over the 36 signed permutations of (a,b,c) x (i,j,k)   (X[a,b,c,i,j,k])"""
+    out = np.zeros_like(X)
+    for pv in itertools.permutations(range(3)):
+        for po in itertools.permutations(range(3)):
+            out = out + _perm_sign(pv) * _perm_sign(po) * X.transpose(list(pv) + [3 + q for q in po])
+    return out
+
+
+# (coefficient, block types of H, einsum) -- R3 = A3 sum_k c_k X_k, T = T2 + T3 (T1 dressed away)
+CCSDT_R3_TERMS = [
+    (+1 / 4, "g", "ovoo", "laij,bclk->abcijk", ("t2",)),
+    (+1 / 4, "g", "vvov", "abid,dcjk->abcijk", ("t2",)),
+    (-1 / 12, "f", "oo", "li,abcljk->abcijk", ("t3",)),
+    (+1 / 12, "f", "vv", "ad,dbcijk->abcijk", ("t3",)),
+    (+1 / 24, "g", "oooo", "lmij,abclmk->abcijk", ("t3",)),
+    (-1 / 4, "g", "ovov", "laid,dbcljk->abcijk", ("t3",)),
+    (+1 / 24, "g", "vvvv", "abde,decijk->abcijk", ("t3",)),
+    (+1 / 4, "f", "ov", "ld,abli,dcjk->abcijk", ("t2", "t2")),
+    (+1 / 8, "g", "ooov", "lmid,ablm,dcjk->abcijk", ("t2", "t2")),
+    (-1 / 2, "g", "ooov", "lmid,dalj,bcmk->abcijk", ("t2", "t2")),
+    (-1 / 2, "g", "ovvv", "lade,dbli,ecjk->abcijk", ("t2", "t2")),
+    (+1 / 8, "g", "ovvv", "lade,bcli,dejk->abcijk", ("t2", "t2")),
+    (-1 / 24, "g", "oovv", "lmde,dalm,ebcijk->abcijk", ("t2", "t3")),
+    (+1 / 48, "g", "oovv", "lmde,ablm,decijk->abcijk", ("t2", "t3")),
+    (-1 / 24, "g", "oovv", "lmde,deli,abcmjk->abcijk", ("t2", "t3")),
+    (+1 / 4, "g", "oovv", "lmde,dali,ebcmjk->abcijk", ("t2", "t3")),
+    (-1 / 8, "g", "oovv", "lmde,abli,decmjk->abcijk", ("t2", "t3")),
+    (+1 / 48, "g", "oovv", "lmde,deij,abclmk->abcijk", ("t2", "t3")),
+    (-1 / 8, "g", "oovv", "lmde,daij,ebclmk->abcijk", ("t2", "t3")),
+]
+
+
+def _blk(o, H, types):
+    return H[tuple(slice(0, o) if t == "o" else slice(o, None) for t in types)]
+
+
+def ccsdt_residual_unfactorised(o, f, g, t1, t2, t3):
+    """(E_corr, R1, R2, R3) of CCSDT: the projections of exp(-T) H exp(T) |Phi0>, T = T1 + T2 + T3 (PAPER Eqs. 2-3), as
+    explicit sums.  With (f~, g~) = dress_t1:
+      R1[a,i]  = f~[a,i] + f~[l,d] t2[d,a,l,i] + 1/2 g~[l,m,i,d] t2[d,a,l,m] + 1/2 g~[l,a,d,e] t2[d,e,l,i]
+                 + 1/4 g~[l,m,d,e] t3[d,e,a,l,m,i]
+      R2       = (the 10-term CCD residual of f~, g~, t2) + f~[l,d] t3[d,a,b,l,i,j]
+                 + 1/2 P(ij) g~[l,m,i,d] t3[d,a,b,l,m,j] + 1/2 P(ab) g~[l,a,d,e] t3[d,e,b,l,i,j]
+      R3       = A3 sum of CCSDT_R3_TERMS (19 terms)
+      E_corr   = f[i,a] t1[a,i] + 1/4 <ij||ab> t2 + 1/2 <ij||ab> t1 t1   (bare integrals; T3 does not enter)"""
+    es = np.einsum
+    ft, gt = dress_t1(o, f, g, t1)
+    B = lambda H, ty: _blk(o, H, ty)
+    r1 = (B(ft, "vo") + es("ld,dali->ai", B(ft, "ov"), t2) + 0.5 * es("lmid,dalm->ai", B(gt, "ooov"), t2)
+          + 0.5 * es("lade,deli->ai", B(gt, "ovvv"), t2) + 0.25 * es("lmde,dealmi->ai", B(gt, "oovv"), t3))
+    r2 = ccd_residual_unfactorised(o, ft, gt, t2)[0]
+    r2 = r2 + es("ld,dablij->abij", B(ft, "ov"), t3)
+    r2 = r2 + 0.5 * _P(es("lmid,dablmj->abij", B(gt, "ooov"), t3), 2, 3)
+    r2 = r2 + 0.5 * _P(es("lade,deblij->abij", B(gt, "ovvv"), t3), 0, 1)
+    amps = {"t2": t2, "t3": t3}
+    x = np.zeros_like(t3)
+    for c, which, types, spec, ts in CCSDT_R3_TERMS:
+        x = x + c * es(spec, B(ft if which == "f" else gt, types), *[amps[t] for t in ts])
+    r3 = antisymmetrise_abc_ijk(x)
+    oovv = B(g, "oovv")
+    e = (es("ia,ai->", B(f, "ov"), t1) + 0.25 * es("ijab,abij->", oovv, t2) + 0.5 * es("ijab,ai,bj->", oovv, t1, t1))
+    return complex(e), r1, r2, r3

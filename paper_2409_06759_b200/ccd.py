@@ -457,3 +457,155 @@ def t3_term(ctx, W, T2, R3, X=None):
     if own:
         X.destroy()
     return R3
+
+
+# ---- CCSDT ("CCSDT iterations"; the paper's production target beyond CCSD: Tables III-IV) --------
+A3_PERMS, A3_SIGNS = [], []
+for _pv, _sv in (((0, 1, 2), 1), ((1, 0, 2), -1), ((2, 1, 0), -1), ((0, 2, 1), -1), ((1, 2, 0), 1), ((2, 0, 1), 1)):
+    for _po, _so in (((0, 1, 2), 1), ((1, 0, 2), -1), ((2, 1, 0), -1), ((0, 2, 1), -1), ((1, 2, 0), 1), ((2, 0, 1), 1)):
+        A3_PERMS.append(list(_pv) + [3 + q for q in _po])
+        A3_SIGNS.append(float(_sv * _so))
+
+
+def t1_dressed_blocks(ctx, o, h, g, T1, names):
+    """The blocks `names` (e.g. "ovvv", "fov") of the T1-similarity-transformed integrals, exp(-T1) H exp(T1), built from the
+    FULL-range bare one-electron matrix h(p,q) and <pq||rs> = g(p,q,r,s) (device tensors over all n = o + v spinors) by binary
+    contractions:  g~[PQRS] = X[P,p] X[Q,q] g[pqrs] Y[r,R] Y[s,S],  X = 1 - tau, Y = 1 + tau, tau[a,i] = t_i^a;
+    f~ = X (h + J) Y with J(p,r) = sum_{i occ} sum_s g(p,i,r,s) Y[s,i].  Only the 16-byte-per-element t1 is read back to
+    build the four row / column slices of X and Y on the host.  Returns {name: Tensor}."""
+    import numpy as np
+    n = g.extents[0]
+    v = n - o
+    t1 = ctx.tensor_download(T1)
+    tau = np.zeros((n, n), dtype=np.complex128)
+    tau[o:, :o] = t1
+    X, Y = np.eye(n) - tau, np.eye(n) + tau
+    ext = {"o": o, "v": v}
+    rng = {"o": slice(0, o), "v": slice(o, n)}
+    Xr = {c: ctx.tensor_from_numpy(np.asfortranarray(X[rng[c], :])) for c in "ov"}      # (|c|, n): rows of X
+    Yc = {c: ctx.tensor_from_numpy(np.asfortranarray(Y[:, rng[c]])) for c in "ov"}      # (n, |c|): columns of Y
+    Yocc = Y.copy()
+    Yocc[:, o:] = 0.0
+    Yp = ctx.tensor_from_numpy(np.asfortranarray(Yocc))
+    new = lambda shape: ctx.tensor_create(shape, zero=False)
+    out = {}
+    # ---- f~ blocks
+    fnames = [x for x in names if x[0] == "f"]
+    if fnames:
+        hJ = new((n, n))
+        ctx.add("hJ(p,r)=h(p,r)", hJ, h, 1.0)
+        ctx.contract("hJ(p,r)+=g(p,q,r,s)*Yp(s,q)", hJ, g, Yp, 1.0)
+        for name in fnames:
+            P, Q = name[1], name[2]
+            F1 = new((n, ext[Q]))
+            ctx.contract("F1(p,Q)=hJ(p,r)*Yc(r,Q)", F1, hJ, Yc[Q], 1.0)
+            out[name] = new((ext[P], ext[Q]))
+            ctx.contract("F(P,Q)=Xr(P,p)*F1(p,Q)", out[name], Xr[P], F1, 1.0)
+            F1.destroy()
+        hJ.destroy()
+    # ---- g~ blocks: index 4, then 3, then 2, then 1; partial transforms shared between the blocks that need them
+    gnames = sorted(x for x in names if x[0] != "f")
+    for S in "ov":
+        needS = [x for x in gnames if x[3] == S]
+        if not needS:
+            continue
+        G1 = new((n, n, n, ext[S]))
+        ctx.contract("G1(p,q,r,S)=g(p,q,r,s)*Yc(s,S)", G1, g, Yc[S], 1.0)
+        for Rr in "ov":
+            needR = [x for x in needS if x[2] == Rr]
+            if not needR:
+                continue
+            G2 = new((n, n, ext[Rr], ext[S]))
+            ctx.contract("G2(p,q,R,S)=G1(p,q,r,S)*Yc(r,R)", G2, G1, Yc[Rr], 1.0)
+            for Q in "ov":
+                needQ = [x for x in needR if x[1] == Q]
+                if not needQ:
+                    continue
+                G3 = new((n, ext[Q], ext[Rr], ext[S]))
+                ctx.contract("G3(p,Q,R,S)=Xr(Q,q)*G2(p,q,R,S)", G3, Xr[Q], G2, 1.0)
+                for name in needQ:
+                    out[name] = new((ext[name[0]], ext[Q], ext[Rr], ext[S]))
+                    ctx.contract("G(P,Q,R,S)=Xr(P,p)*G3(p,Q,R,S)", out[name], Xr[name[0]], G3, 1.0)
+                G3.destroy()
+            G2.destroy()
+        G1.destroy()
+    for t in list(Xr.values()) + list(Yc.values()) + [Yp]:
+        t.destroy()
+    return out
+
+
+CCSDT_BLOCKS = ("foo", "fvv", "fov", "fvo", "vvoo", "oovv", "oooo", "vvvv", "ovvo", "ooov", "ovvv", "ovoo", "vvov", "ovov")
+
+
+def ccsdt_residual(ctx, o, h, g, T1, T2, T3, R1=None, R2=None, R3=None):
+    """Spin-orbital CCSDT residuals R1, R2, R3 = <Phi_mu| exp(-T) H exp(T) |Phi0>, T = T1 + T2 + T3 (PAPER Eqs. 2-3), as binary
+    tensor operations.  T1 is absorbed exactly into the integrals (`t1_dressed_blocks`); with the dressed blocks the
+    equations are those of T = T2 + T3 (oracle: cc.ccsdt_residual_unfactorised, 5 + 13 + 19 terms, pinned to the Fock space):
+      R1 = f~vo + f~ov.T2 + 1/2 g~ooov.T2 + 1/2 g~ovvv.T2 + 1/4 g~oovv.T3
+      R2 = [CCD residual of the dressed blocks] + f~ov.T3 + 1/2 P(ij) g~ooov.T3 + 1/2 P(ab) g~ovvv.T3
+      R3 = A3 X,  X = Wovoo.T2 + Wvvov.T2 + Fo.T3 + Fv.T3 + Woooo.T3 + Wvvvv.T3 + Wr.T3  (seven rank-6 contractions into one X,
+           ONE 36-term antisymmetrisation), the W / F intermediates carrying the quadratic T2 T2 and T2 T3 terms.
+    h (n,n) bare one-electron matrix, g (n,n,n,n) = <pq||rs>, n = o + v.  Returns (R1, R2, R3)."""
+    v = T1.extents[0]
+    B = t1_dressed_blocks(ctx, o, h, g, T1, CCSDT_BLOCKS)
+    new = lambda shape: ctx.tensor_create(shape, zero=False)
+    con, add = ctx.contract, ctx.add
+    # ---- singles
+    if R1 is None:
+        R1 = new((v, o))
+    add("R(a,i)=f(a,i)", R1, B["fvo"], 1.0)
+    con("R(a,i)+=f(l,d)*T(d,a,l,i)", R1, B["fov"], T2, 1.0)
+    con("R(a,i)+=W(l,m,i,d)*T(d,a,l,m)", R1, B["ooov"], T2, 0.5)
+    con("R(a,i)+=W(l,a,d,e)*T(d,e,l,i)", R1, B["ovvv"], T2, 0.5)
+    con("R(a,i)+=T(d,e,a,l,m,i)*W(l,m,d,e)", R1, T3, B["oovv"], 0.25)
+    # ---- doubles: the CCD program on the dressed blocks + the three T3 terms
+    R2 = ccd_residual(ctx, B, T2, R2)
+    con("R(a,b,i,j)+=T(d,a,b,l,i,j)*f(l,d)", R2, T3, B["fov"], 1.0)
+    X2 = new((v, v, o, o))
+    con("X(a,b,i,j)=T(d,a,b,l,m,j)*W(l,m,i,d)", X2, T3, B["ooov"], 1.0)
+    ctx.antisymmetrize("P(ij):R(a,b,i,j)+=X(a,b,i,j)", R2, X2, 0.5)
+    con("X(a,b,i,j)=W(l,a,d,e)*T(d,e,b,l,i,j)", X2, B["ovvv"], T3, 1.0)
+    ctx.antisymmetrize("P(ab):R(a,b,i,j)+=X(a,b,i,j)", R2, X2, 0.5)
+    X2.destroy()
+    # ---- triples: intermediates
+    Wovoo = new((o, v, o, o))
+    add("W(l,a,i,j)=g(l,a,i,j)", Wovoo, B["ovoo"], 0.25)
+    con("W(l,a,i,j)+=f(l,d)*T(d,a,i,j)", Wovoo, B["fov"], T2, 0.25)
+    con("W(m,a,i,j)+=g(l,m,i,d)*T(d,a,l,j)", Wovoo, B["ooov"], T2, -0.5)
+    con("W(l,a,j,k)+=g(l,a,d,e)*T(d,e,j,k)", Wovoo, B["ovvv"], T2, 0.125)
+    con("W(l,a,i,j)+=g(l,m,d,e)*T(d,e,a,m,i,j)", Wovoo, B["oovv"], T3, -0.125)
+    Wvvov = new((v, v, o, v))
+    add("W(a,b,i,d)=g(a,b,i,d)", Wvvov, B["vvov"], 0.25)
+    con("W(a,b,i,d)+=T(a,b,l,m)*g(l,m,i,d)", Wvvov, T2, B["ooov"], 0.125)
+    con("W(a,b,i,e)+=g(l,a,d,e)*T(d,b,l,i)", Wvvov, B["ovvv"], T2, -0.5)
+    con("W(a,b,i,d)+=g(l,m,d,e)*T(e,a,b,l,m,i)", Wvvov, B["oovv"], T3, -0.125)
+    Fo, Fv = new((o, o)), new((v, v))
+    add("F(m,i)=f(m,i)", Fo, B["foo"], -1.0 / 12.0)
+    con("F(m,i)+=g(l,m,d,e)*T(d,e,l,i)", Fo, B["oovv"], T2, -1.0 / 24.0)
+    add("F(a,e)=f(a,e)", Fv, B["fvv"], 1.0 / 12.0)
+    con("F(a,e)+=g(l,m,d,e)*T(d,a,l,m)", Fv, B["oovv"], T2, -1.0 / 24.0)
+    Woooo, Wvvvv, Wr = new((o, o, o, o)), new((v, v, v, v)), new((o, v, o, v))
+    add("W(l,m,i,j)=g(l,m,i,j)", Woooo, B["oooo"], 1.0 / 24.0)
+    con("W(l,m,i,j)+=g(l,m,d,e)*T(d,e,i,j)", Woooo, B["oovv"], T2, 1.0 / 48.0)
+    add("W(a,b,d,e)=g(a,b,d,e)", Wvvvv, B["vvvv"], 1.0 / 24.0)
+    con("W(a,b,d,e)+=T(a,b,l,m)*g(l,m,d,e)", Wvvvv, T2, B["oovv"], 1.0 / 48.0)
+    add("W(m,a,i,e)=g(m,a,i,e)", Wr, B["ovov"], -0.25)
+    con("W(m,a,i,e)+=g(l,m,d,e)*T(d,a,l,i)", Wr, B["oovv"], T2, 0.25)
+    for t in B.values():
+        t.destroy()
+    # ---- triples: seven contractions into one X, one antisymmetrisation
+    X = new((v, v, v, o, o, o))
+    con("X(a,b,c,i,j,k)=W(l,a,i,j)*T(b,c,l,k)", X, Wovoo, T2, 1.0)
+    con("X(a,b,c,i,j,k)+=W(a,b,i,d)*T(d,c,j,k)", X, Wvvov, T2, 1.0)
+    con("X(a,b,c,i,j,k)+=F(m,i)*T(a,b,c,m,j,k)", X, Fo, T3, 1.0)
+    con("X(a,b,c,i,j,k)+=F(a,e)*T(e,b,c,i,j,k)", X, Fv, T3, 1.0)
+    con("X(a,b,c,i,j,k)+=W(l,m,i,j)*T(a,b,c,l,m,k)", X, Woooo, T3, 1.0)
+    con("X(a,b,c,i,j,k)+=W(a,b,d,e)*T(d,e,c,i,j,k)", X, Wvvvv, T3, 1.0)
+    con("X(a,b,c,i,j,k)+=W(m,a,i,e)*T(e,b,c,m,j,k)", X, Wr, T3, 1.0)
+    for t in (Wovoo, Wvvov, Fo, Fv, Woooo, Wvvvv, Wr):
+        t.destroy()
+    if R3 is None:
+        R3 = new((v, v, v, o, o, o))
+    ctx.permsum(R3, X, A3_PERMS, A3_SIGNS, 0.0)
+    X.destroy()
+    return R1, R2, R3

@@ -291,3 +291,96 @@ def test_ccsd_diis_fixed_point_is_the_fock_space_solution_and_residual_norm_is_t
     _, j1, j2 = cc.ccsd_residual_program(B, Tj1, Tj2)
     assert norms[7] < 0.1 * cc.residual_norm(j1, j2)
     assert all(norms[k + 1] < norms[k] for k in range(8))
+
+
+def _ccsdt_problem(o, v, seed, hermitian=False, scale=0.3):
+    rng = np.random.default_rng(seed)
+    n = o + v
+    c = lambda *s: rng.standard_normal(s) + 1j * rng.standard_normal(s)
+    g = c(n, n, n, n)
+    g = g - g.transpose(1, 0, 2, 3)
+    g = scale * (g - g.transpose(0, 1, 3, 2))
+    f = scale * c(n, n)
+    if hermitian:
+        g = 0.5 * (g + g.transpose(2, 3, 0, 1).conj())
+        f = 0.5 * (f + f.conj().T)
+    t1 = scale * c(v, o)
+    t2 = c(v, v, o, o)
+    t2 = t2 - t2.transpose(1, 0, 2, 3)
+    t2 = scale * (t2 - t2.transpose(0, 1, 3, 2))
+    t3 = 0.1 * cc.antisymmetrise_abc_ijk(c(v, v, v, o, o, o))
+    return f, g, t1, t2, t3
+
+
+def _fock_ccsdt(o, v, f, g, t1, t2, t3):
+    """exp(-T) H exp(T) |Phi0> with T = T1 + T2 + T3 on the Fock space: E, singles, doubles, triples projections"""
+    fs = cc.FockSpace(o, v)
+
+    def exp_t(psi, sign):
+        out, term = psi.copy(), psi.copy()
+        for k in range(1, o + v + 2):
+            term = sign * (fs.apply_T(t1, t2, term) + fs.apply_T3(t3, term)) / k
+            if not np.any(term):
+                break
+            out = out + term
+        return out
+    psi = exp_t(fs.apply_H(f, g, exp_t(fs.phi0, 1.0)), -1.0)
+    e = np.vdot(fs.phi0, psi) - np.vdot(fs.phi0, fs.apply_H(f, g, fs.phi0))
+    return e, fs.project_singles(psi), fs.project_doubles(psi), fs.project_triples(psi), fs
+
+
+def test_t1_dressing_is_the_similarity_transformation_on_the_fock_space():
+    """H~ built from dress_t1's integrals IS exp(-T1) H exp(T1) as an operator: applied to a random Fock-space vector"""
+    o, v = 2, 3
+    f, g, t1, _, _ = _ccsdt_problem(o, v, 5)
+    ft, gt = cc.dress_t1(o, f, g, t1)
+    fs = cc.FockSpace(o, v)
+    rng = np.random.default_rng(1)
+    psi = rng.standard_normal(2 ** (o + v)) + 1j * rng.standard_normal(2 ** (o + v))
+    lhs = fs.exp_T(t1, None, fs.apply_H(f, g, fs.exp_T(t1, None, psi)), sign=-1.0)
+    rhs = fs.apply_H(ft, gt, psi)
+    assert np.abs(lhs - rhs).max() <= 1e-12 * np.abs(lhs).max()
+    ft0, gt0 = cc.dress_t1(o, f, g, np.zeros_like(t1))
+    assert np.array_equal(gt0, g) and np.abs(ft0 - f).max() <= 1e-15
+
+
+@pytest.mark.parametrize("o,v,hermitian", [(3, 4, False), (4, 4, False), (3, 5, True)])
+def test_ccsdt_residuals_equal_the_fock_space_projections(o, v, hermitian):
+    """CCSDT: 5 + 13 + 19 terms against Eq. (3) evaluated literally, random complex t1, t2, t3, H general (non-Hermitian: the
+    T1-dressed integrals are not Hermitian either) -- a dropped term, a wrong sign, factor or index placement in any of the
+    three equations fails this (sizes beyond o = 3 matter: at o = 3 the occupied part of T3 is one-dimensional)"""
+    f, g, t1, t2, t3 = _ccsdt_problem(o, v, 10 * o + v, hermitian)
+    e0, s0, d0, t0, _ = _fock_ccsdt(o, v, f, g, t1, t2, t3)
+    e, r1, r2, r3 = cc.ccsdt_residual_unfactorised(o, f, g, t1, t2, t3)
+    assert abs(e - e0) <= 1e-12 * abs(e0)
+    for got, ref in ((r1, s0), (r2, d0), (r3, t0)):
+        assert np.abs(got - ref).max() <= 1e-12 * np.abs(ref).max()
+    assert len(cc.CCSDT_R3_TERMS) == 19
+    # each of the 19 triples terms matters: dropping any one changes R3 by far more than the tolerance (from o = v = 4 on:
+    # with three occupied spinors some topologies vanish under the antisymmetriser)
+    amps = {"t2": t2, "t3": t3}
+    ft, gt = cc.dress_t1(o, f, g, t1)
+    for cf, which, types, spec, ts in (cc.CCSDT_R3_TERMS if min(o, v) >= 4 else []):
+        x = cf * np.einsum(spec, cc._blk(o, ft if which == "f" else gt, types), *[amps[t] for t in ts])
+        assert np.abs(cc.antisymmetrise_abc_ijk(x)).max() >= 1e-6 * np.abs(t0).max(), spec
+    # t3 = 0, t1 = 0: the doubles equation is the CCD tier, the triples equation the (T) driver terms
+    e_, r1_, r2_, r3_ = cc.ccsdt_residual_unfactorised(o, f, g, 0 * t1, t2, 0 * t3)
+    assert np.abs(r2_ - cc.ccd_residual_unfactorised(o, f, g, t2)[0]).max() <= 1e-13 * np.abs(r2_).max()
+
+
+def test_ccsdt_driver_call_list_is_the_unfactorised_equations():
+    """The product's CCSDT driver (ccd.ccsdt_residual: T1 dressing by binary contractions, intermediates, seven rank-6
+    contractions into one X, one 36-term antisymmetrisation) run on the host with every tensor operation done by the oracle:
+    its result is the unfactorised 37-term evaluation (pinned above to the Fock space)."""
+    from oracle_ctx import OracleContext
+    from paper_2409_06759_b200 import ccd
+    o, v = 3, 4
+    f, g, t1, t2, t3 = _ccsdt_problem(o, v, 77)
+    h = f - np.einsum("piqi->pq", g[:, :o, :, :o])
+    oc = OracleContext()
+    W = oc.tensor_from_numpy
+    R1, R2, R3 = ccd.ccsdt_residual(oc, o, W(h), W(g), W(t1), W(t2), W(t3))
+    e, r1, r2, r3 = cc.ccsdt_residual_unfactorised(o, f, g, t1, t2, t3)
+    for got, ref in ((R1.host, r1), (R2.host, r2), (R3.host, r3)):
+        assert np.abs(got - ref).max() <= 1e-12 * np.abs(ref).max()
+    assert oc.calls > 80
