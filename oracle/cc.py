@@ -712,3 +712,24 @@ def ccsdt_residual_unfactorised(o, f, g, t1, t2, t3):
     oovv = B(g, "oovv")
     e = (es("ia,ai->", B(f, "ov"), t1) + 0.25 * es("ijab,abij->", oovv, t2) + 0.5 * es("ijab,ai,bj->", oovv, t1, t1))
     return complex(e), r1, r2, r3
+
+
+def ccsdt_jacobi(o, f, g, iterations):
+    """t1 += R1 / (e_i - e_a), t2 += R2 / (e_i + e_j - e_a - e_b), t3 += R3 / (e_i + e_j + e_k - e_a - e_b - e_c) from zero
+    amplitudes, e = diag f, all three residuals evaluated at the old amplitudes (`ccsdt_residual_unfactorised`).
+    Returns (T1, T2, T3, [E_corr of the amplitudes each evaluation saw], [residual norm of each evaluation])."""
+    v = f.shape[0] - o
+    e = np.real(np.diag(f))
+    eo, ev = e[:o], -e[o:]
+    T1 = np.zeros((v, o), dtype=np.complex128, order="F")
+    T2 = np.zeros((v, v, o, o), dtype=np.complex128, order="F")
+    T3 = np.zeros((v, v, v, o, o, o), dtype=np.complex128, order="F")
+    energies, norms = [], []
+    for _ in range(iterations):
+        E, R1, R2, R3 = ccsdt_residual_unfactorised(o, f, g, T1, T2, T3)
+        energies.append(E)
+        norms.append(residual_norm(R1, R2, R3))
+        T1 = denominator_update(T1, R1, [ev, eo], 1.0)
+        T2 = denominator_update(T2, R2, [ev, ev, eo, eo], 1.0)
+        T3 = denominator_update(T3, R3, [ev, ev, ev, eo, eo, eo], 1.0)
+    return T1, T2, T3, energies, norms

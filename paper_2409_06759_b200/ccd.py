@@ -609,3 +609,38 @@ def ccsdt_residual(ctx, o, h, g, T1, T2, T3, R1=None, R2=None, R3=None):
     ctx.permsum(R3, X, A3_PERMS, A3_SIGNS, 0.0)
     X.destroy()
     return R1, R2, R3
+
+
+def ccsdt_solve(ctx, o, h, g, f_diag, iterations):
+    """Jacobi iterations of the CCSDT amplitude equations from zero amplitudes (oracle: cc.ccsdt_jacobi): per iteration
+    `ccsdt_residual`, the residual norm |R|, the energy of the amplitudes the evaluation saw, and three
+    `tcb_denominator_update`.  f_diag: the n orbital energies (diagonal of the Fock matrix).
+    Returns (T1, T2, T3, [E_corr per evaluation], [|R| per evaluation])."""
+    import numpy as np
+    n = g.extents[0]
+    v = n - o
+    e = np.asarray(f_diag, dtype=np.float64)
+    eo, ev = e[:o], -e[o:]
+    T1, T2, T3 = ctx.tensor_create((v, o)), ctx.tensor_create((v, v, o, o)), ctx.tensor_create((v, v, v, o, o, o))
+    R1, R2, R3 = ctx.tensor_create((v, o)), ctx.tensor_create((v, v, o, o)), ctx.tensor_create((v, v, v, o, o, o), zero=False)
+    # bare blocks for the energy: E = f_ia t_i^a + 1/4 <ij||ab> t_ij^ab + 1/2 <ij||ab> t_i^a t_j^b
+    Bz = t1_dressed_blocks(ctx, o, h, g, T1, ("fov", "oovv"))          # T1 = 0 here: the bare blocks
+    energies, norms = [], []
+    for _ in range(iterations):
+        E = ctx.tensor_create(())
+        Y = ctx.tensor_create((o, v), zero=False)
+        ctx.contract("E()=f(i,a)*T(a,i)", E, Bz["fov"], T1, 1.0)
+        ctx.contract("E()+=W(i,j,a,b)*T(a,b,i,j)", E, Bz["oovv"], T2, 0.25)
+        ctx.contract("Y(i,a)=W(i,j,a,b)*T(b,j)", Y, Bz["oovv"], T1, 1.0)
+        ctx.contract("E()+=Y(i,a)*T(a,i)", E, Y, T1, 0.5)
+        ccsdt_residual(ctx, o, h, g, T1, T2, T3, R1, R2, R3)
+        energies.append(complex(ctx.tensor_download(E)))
+        norms.append(residual_norm(ctx, R1, R2, R3))
+        E.destroy()
+        Y.destroy()
+        ctx.denominator_update(T1, R1, [ev, eo], 1.0)
+        ctx.denominator_update(T2, R2, [ev, ev, eo, eo], 1.0)
+        ctx.denominator_update(T3, R3, [ev, ev, ev, eo, eo, eo], 1.0)
+    for t in list(Bz.values()) + [R1, R2, R3]:
+        t.destroy()
+    return T1, T2, T3, energies, norms

@@ -190,6 +190,19 @@ class ShadowContext:
         sn = abs(alpha) * oracle.add(e_acc, np.zeros_like(base), L.norm, 1.0).real
         self._compare(expr, D, ref, sn + (D.norm if acc else 0.0))
 
+    def tensor_from_numpy(self, host):
+        return self.wrap(host)
+
+    def tensor_download(self, t):
+        return self.ctx.tensor_download(t.gpu)
+
+    def permsum(self, D, X, perms, coefs, beta=1.0):
+        import oracle
+        self.ctx.permsum(D.gpu, X.gpu, perms, coefs, beta)
+        ref = oracle.permsum(D.host, X.host, perms, coefs, beta)
+        sn = oracle.permsum(np.zeros_like(D.host), X.norm, perms, [abs(c) for c in coefs], 0.0).real + abs(beta) * D.norm
+        self._compare("permsum", D, ref, sn)
+
     def antisymmetrize(self, spec, D, X, alpha=1.0):
         import oracle
         self.ctx.antisymmetrize(spec, D.gpu, X.gpu, alpha)

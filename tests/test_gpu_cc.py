@@ -376,3 +376,65 @@ def test_ccsd_diis_and_residual_norms_follow_the_oracle(ctx):
         R = cc.ccd_residual_program(B2, Tr)
         assert abs(got[k] - cc.residual_norm(R)) <= 1e-11 * cc.residual_norm(cc.ccd_residual_program(B2, np.zeros_like(T_mp2)))
         Tr = cc.denominator_update(Tr, R, [-ev, -ev, eo, eo], 1.0)
+
+
+def _ccsdt_inputs(o, v, seed, scale=0.3):
+    rng = np.random.default_rng(seed)
+    n = o + v
+    c = lambda *s: rng.standard_normal(s) + 1j * rng.standard_normal(s)
+    g = c(n, n, n, n)
+    g = g - g.transpose(1, 0, 2, 3)
+    g = scale * (g - g.transpose(0, 1, 3, 2))
+    f = scale * c(n, n)
+    t1 = scale * c(v, o)
+    t2 = c(v, v, o, o)
+    t2 = t2 - t2.transpose(1, 0, 2, 3)
+    t2 = scale * (t2 - t2.transpose(0, 1, 3, 2))
+    t3 = 0.1 * cc.antisymmetrise_abc_ijk(c(v, v, v, o, o, o))
+    h = f - np.einsum("piqi->pq", g[:, :o, :, :o])
+    return f, g, h, t1, t2, t3
+
+
+@pytest.mark.parametrize("o,v", [(3, 4), (4, 6)])
+def test_ccsdt_residual_call_by_call_and_against_the_fock_space_pinned_equations(ctx, o, v):
+    """SURVEY 8(f)-3, CCSDT: the driver's ~120 library calls (T1 dressing of the integrals, CCD program on the dressed blocks,
+    intermediates, seven rank-6 contractions, one 36-term antisymmetrisation), each compared with the oracle's evaluation of
+    the same call under its own carried snorm; the three residuals against cc.ccsdt_residual_unfactorised (pinned to the
+    Fock-space projections in tests/test_oracle_cc.py), H general complex and not Hermitian."""
+    from gpu_util import ShadowContext
+    f, g, h, t1, t2, t3 = _ccsdt_inputs(o, v, 100 * o + v)
+    sh = ShadowContext(ctx)
+    R1, R2, R3 = ccd.ccsdt_residual(sh, o, sh.wrap(h), sh.wrap(g), sh.wrap(t1), sh.wrap(t2), sh.wrap(t3))
+    assert sh.calls >= 100 and sh.worst <= 1e-11
+    e, r1, r2, r3 = cc.ccsdt_residual_unfactorised(o, f, g, t1, t2, t3)
+    for got, ref in ((R1, r1), (R2, r2), (R3, r3)):
+        dev = ctx.tensor_download(got.gpu)
+        assert np.abs(dev - ref).max() <= 1e-11 * np.abs(got.norm).max()
+        assert np.abs(got.host - ref).max() <= 1e-12 * np.abs(got.norm).max()
+    gR3 = ctx.tensor_download(R3.gpu)
+    assert np.abs(gR3 + gR3.transpose(1, 0, 2, 3, 4, 5)).max() <= 1e-12 * np.abs(R3.norm).max()
+
+
+def test_ccsdt_iterations_follow_the_oracle_and_converge(ctx):
+    o, v = 3, 3
+    rng = np.random.default_rng(52)
+    n = o + v
+    c = lambda *s: rng.standard_normal(s) + 1j * rng.standard_normal(s)
+    A = c(n, n, n, n)
+    A = A - A.transpose(1, 0, 2, 3)
+    A = A - A.transpose(0, 1, 3, 2)
+    g = 0.05 * 0.5 * (A + A.transpose(2, 3, 0, 1).conj())
+    e = np.concatenate([np.linspace(-2.0, -0.5, o), np.linspace(0.5, 3.0, v)])
+    f = 0.05 * c(n, n)
+    f = f + f.conj().T
+    f[np.diag_indices(n)] = e
+    h = f - np.einsum("piqi->pq", g[:, :o, :, :o])
+    its = 12
+    dh, dg = ctx.tensor_from_numpy(h), ctx.tensor_from_numpy(g)
+    T1, T2, T3, energies, norms = ccd.ccsdt_solve(ctx, o, dh, dg, e, its)
+    r1, r2, r3, e_ref, n_ref = cc.ccsdt_jacobi(o, f, g, its)
+    for got, ref in ((T1, r1), (T2, r2), (T3, r3)):
+        assert np.abs(ctx.tensor_download(got) - ref).max() <= 1e-10 * max(np.abs(ref).max(), 1e-300)
+    for k in range(its):
+        assert abs(energies[k] - e_ref[k]) <= 1e-10 * abs(e_ref[-1]) and abs(norms[k] - n_ref[k]) <= 1e-10 * n_ref[0]
+    assert norms[-1] < 1e-4 * norms[0]

@@ -384,3 +384,21 @@ def test_ccsdt_driver_call_list_is_the_unfactorised_equations():
     for got, ref in ((R1.host, r1), (R2.host, r2), (R3.host, r3)):
         assert np.abs(got - ref).max() <= 1e-12 * np.abs(ref).max()
     assert oc.calls > 80
+
+
+def test_converged_ccsdt_iteration_zeroes_all_three_fock_space_projections():
+    """Jacobi iterations of the CCSDT equations on a weakly coupled Hermitian problem (non-zero occupied-virtual Fock block,
+    so t1 != 0): at the fixed point the singles, doubles AND triples projections of exp(-T) H exp(T)|Phi0> vanish and the
+    energy is the Fock-space one; the residual norm falls monotonically."""
+    o, v = 3, 3
+    f, g, eo, ev = _ccsd_problem(o, v, 52)
+    T1, T2, T3, energies, norms = cc.ccsdt_jacobi(o, f, g, 45)
+    e0, s0, d0, t0, _ = _fock_ccsdt(o, v, f, g, T1, T2, T3)
+    scale = np.abs(g).max()
+    assert max(np.abs(s0).max(), np.abs(d0).max(), np.abs(t0).max()) <= 1e-12 * scale
+    assert abs(cc.ccsdt_residual_unfactorised(o, f, g, T1, T2, T3)[0] - e0) <= 1e-12 * abs(e0)
+    assert np.abs(T3).max() > 1e-6 and np.abs(T1).max() > 1e-4
+    assert all(norms[k + 1] < norms[k] for k in range(20))
+    # triples change the energy: CCSD's fixed point differs
+    _, _, e_sd = cc.ccsd_jacobi(cc.ccsd_blocks(o, f, g), eo, ev, 45)
+    assert abs(e_sd[-1] - e0) > 1e-9 * abs(e0)
