@@ -675,6 +675,52 @@ def run_extras(ctx):
         ctx.sync()
     except Exception as e:          # noqa: BLE001
         out.append({"workload": "[T] triples correction", "error": str(e)})
+    try:    # next row 8(f)-3: one CCSDT residual evaluation (R1, R2, R3) at the configs[3] size o=12 v=60 (T3, X, R3 of 5.97 GB)
+        from paper_2409_06759_b200 import ccd
+        o, v = 12, 60
+        n = o + v
+        hh, gg = ctx.tensor_create((n, n), zero=False), ctx.tensor_create((n, n, n, n), zero=False)
+        ctx.synth_normal(hh, 20240913, 1, sigma=0.05)
+        ctx.synth_normal(gg, 20240913, 2, antisym=((0, 1), (2, 3)), sigma=0.02)
+        T1, T2, T3 = ctx.tensor_create((v, o), zero=False), ctx.tensor_create((v, v, o, o), zero=False), \
+            ctx.tensor_create((v, v, v, o, o, o), zero=False)
+        ctx.synth_normal(T1, 20240913, 3, sigma=0.05)
+        ctx.synth_normal(T2, 20240913, 4, antisym=((0, 1), (2, 3)), sigma=0.05)
+        ctx.synth_normal(T3, 20240913, 5, sigma=0.01)
+
+        class CountingT:                      # forwards to ctx; adds up the planner's flop count of every contraction
+            flops = 0.0
+            calls = 0
+
+            def __getattr__(self, name):
+                return getattr(ctx, name)
+
+            def contract(self, e, D, L, R, alpha=1.0):
+                CountingT.flops += ctx.plan_describe(e, D, L, R)["flops"]
+                CountingT.calls += 1
+                return ctx.contract(e, D, L, R, alpha)
+
+        Rs = ccd.ccsdt_residual(CountingT(), o, hh, gg, T1, T2, T3)          # warm-up pass, counted
+        ctx.sync()
+        ts = []
+        for _ in range(3):
+            l0 = ctx.launch_count()
+            ctx.timer_start()
+            ccd.ccsdt_residual(ctx, o, hh, gg, T1, T2, T3, *Rs)
+            ts.append(ctx.timer_stop())
+            launches = ctx.launch_count() - l0
+        b = min(ts)
+        out.append({"workload": "next row 8(f)-3: CCSDT residual (R1, R2, R3) o=12 v=60: T1 dressing of the integrals, CCD "
+                                "program on the dressed blocks, 7 rank-6 contractions into one X, one 36-term antisymmetrisation; "
+                                "T3, X, R3 of 5.97 GB each",
+                    "ms": b, "ms_median": float(np.median(ts)), "contractions": CountingT.calls, "launches": launches,
+                    "tflops": CountingT.flops / b * 1e-9,
+                    "frac_fp64_tensor_peak": CountingT.flops / b * 1e-9 / FP64_TENSOR_PEAK_TFLOPS})
+        for t in (hh, gg, T1, T2, T3) + tuple(Rs):
+            t.destroy()
+        ctx.sync()
+    except Exception as e:          # noqa: BLE001
+        out.append({"workload": "CCSDT residual", "error": str(e)})
     try:    # configs[4] transposition samples (the whole sweep: python -m paper_2409_06759_b200.transpose_bench)
         import itertools
         from paper_2409_06759_b200 import transpose_bench as tb
