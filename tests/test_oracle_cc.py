@@ -370,7 +370,7 @@ def test_ccsdt_residuals_equal_the_fock_space_projections(o, v, hermitian):
 
 def test_ccsdt_driver_call_list_is_the_unfactorised_equations():
     """The product's CCSDT driver (ccd.ccsdt_residual: T1 dressing by binary contractions, intermediates, seven rank-6
-    contractions into one X, one 36-term antisymmetrisation) run on the host with every tensor operation done by the oracle:
+    contractions into one X, the antisymmetriser in two passes) run on the host with every tensor operation done by the oracle:
     its result is the unfactorised 37-term evaluation (pinned above to the Fock space)."""
     from oracle_ctx import OracleContext
     from paper_2409_06759_b200 import ccd
@@ -383,7 +383,7 @@ def test_ccsdt_driver_call_list_is_the_unfactorised_equations():
     e, r1, r2, r3 = cc.ccsdt_residual_unfactorised(o, f, g, t1, t2, t3)
     for got, ref in ((R1.host, r1), (R2.host, r2), (R3.host, r3)):
         assert np.abs(got - ref).max() <= 1e-12 * np.abs(ref).max()
-    assert oc.calls == 89
+    assert oc.calls == 90
 
 
 def test_converged_ccsdt_iteration_zeroes_all_three_fock_space_projections():
