@@ -150,6 +150,12 @@ def max_over_ranks(values, dist, device):
     return tt.tolist()
 
 
+def e2e_ranks_at_once(world, host_ram_bytes, pinned_bytes_per_rank):
+    """How many replicas measure their end-to-end step at the same time: all of them when 60 % of the host's memory holds
+    every rank's pinned buffers, otherwise as many as fit (at least one); the others wait their turn."""
+    return max(1, min(world, int(0.6 * host_ram_bytes // pinned_bytes_per_rank)))
+
+
 def job_throughput(world, flops_per_replica_step, ms_per_step):
     """Whole-job GFLOP/s: every rank runs the same step on its own GPU; the job takes the slowest rank's time."""
     return world * flops_per_replica_step / (ms_per_step * 1e-3) * 1e-9
@@ -242,7 +248,7 @@ def run_ours(args, rank, world, local_rank):
     # N replicas on one host each pin 27.6 GB: when the host cannot hold all of them at once the ranks take turns in groups
     # (PCIe links are per GPU; what the turns leave out is contention for host memory bandwidth -- said in the JSON line)
     host_ram = os.sysconf("SC_PAGE_SIZE") * os.sysconf("SC_PHYS_PAGES")
-    group = max(1, min(world, int(0.6 * host_ram // (h2d + d2h + 2 * Rt.nbytes))))
+    group = e2e_ranks_at_once(world, host_ram, h2d + d2h + 2 * Rt.nbytes)
 
     def e2e_measure():
         host_V = torch.empty(Vt.size, dtype=torch.complex128).pin_memory()

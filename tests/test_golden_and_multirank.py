@@ -110,3 +110,14 @@ def test_ccsd_contraction_list_is_well_formed():
                                                 ("R2(b,a,j,i)+", 1.0)]
     kinds = {(p["K"] == 1, p["N"] == 1) for p in (binding.plan_describe_host(e, sd, sl, sr) for e, _, sd, sl, sr in calls)}
     assert (True, False) in kinds and (False, True) in kinds          # the list holds an outer product and N = 1 cases
+
+
+def test_e2e_rank_groups_fit_the_host():
+    """bench.py e2e: N replicas each pin 30.7 GB; on a 196 GB host eight of them do not fit at once"""
+    import bench
+    per = 27_648_000_000 + 1_024_000_000 + 2 * 1_024_000_000
+    assert bench.e2e_ranks_at_once(1, 196 << 30, per) == 1
+    assert bench.e2e_ranks_at_once(4, 196 << 30, per) == 4
+    assert bench.e2e_ranks_at_once(8, 196 << 30, per) == 4
+    assert bench.e2e_ranks_at_once(8, 2048 << 30, per) == 8
+    assert bench.e2e_ranks_at_once(8, 16 << 30, per) == 1
