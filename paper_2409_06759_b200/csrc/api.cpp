@@ -314,6 +314,8 @@ int get_plan(tcb_ctx *ctx, const char *expr, const tcb_tensor *D, const tcb_tens
         cp->d_aux[q] = aux[q]->empty() ? nullptr : cp->d_tables + at;
         TCB_CUDA(ctx, put(*aux[q]));
     }
+    // the tables were enqueued on the CURRENT lane's stream; the plan may next be used on another lane: wait once, here
+    TCB_CUDA(ctx, cudaStreamSynchronize(cur_stream(ctx)));
     *out = cp.get();
     ctx->plans[key] = std::move(cp);
     return TCB_OK;
@@ -1153,6 +1155,7 @@ int tcb_pack(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *L)
         TCB_CUDA(ctx, cudaMalloc((void **)&st->dev, std::max<size_t>(1, st->host.size()) * sizeof(int64_t)));
         TCB_CUDA(ctx, cudaMemcpyAsync(st->dev, st->host.data(), st->host.size() * sizeof(int64_t), cudaMemcpyHostToDevice,
                                       cur_stream(ctx)));
+        TCB_CUDA(ctx, cudaStreamSynchronize(cur_stream(ctx)));     // usable from every lane from here on
         it = ctx->sym_tables.emplace(key, std::move(st)).first;
     }
     PackDesc d;
