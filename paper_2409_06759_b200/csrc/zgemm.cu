@@ -779,7 +779,11 @@ cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps
     const int mpairs = (p.mblocks + 1) / 2, npairs = (p.nblocks + 1) / 2;
     p.mpair_base = mpairs / sc.mt; p.mpair_extra = mpairs % sc.mt;
     p.npair_base = npairs / sc.nt; p.npair_extra = npairs % sc.nt;
-    p.gn = p.nt <= 24 ? p.nt : 16;
+    // width of a tile-column group: every tile column while there are at most 32 (a wave of 296 CTAs then shares each A row
+    // panel among all of them), else 16.  configs[2] (25 tile columns), DRAM read per launch by ncu: 215 GB at 4, 145 GB at 8
+    // and 16, 120 GB at 25 -- same 578 ms (profiles/r2_zgemm_configs2_ncu.md)
+    p.gn = p.nt <= 32 ? p.nt : 16;
+    if (getenv("TCB_GEMM_GN")) p.gn = std::max(1, std::min(p.nt, atoi(getenv("TCB_GEMM_GN"))));
     p.ktiles = sc.ktiles;
     p.klast_steps = (int)((g.K - (int64_t)(sc.ktiles - 1) * BK + 3) / 4);
     p.dp_tiles = sc.dp_tiles; p.sk_tiles = sc.sk_tiles; p.sk_chunks = sc.sk_chunks;
