@@ -320,8 +320,16 @@ cudaError_t launch_permute(const PermuteDesc &pd, cudaStream_t stream, int64_t *
     std::stable_sort(q, q + r, [&](int a, int b) { return pd.ostride[a] < pd.ostride[b]; });
     for (int d = 0; d < kMaxRank; ++d) p.q[d] = q[d];
 
-    const int TI = env_int("TCB_PERM_TI", 32), TO = env_int("TCB_PERM_TO", 32);
-    const int VOL = std::min(env_int("TCB_PERM_VOL", 2048), kMaxVol);
+    // Large tensors (>= 256 MB) whose output-fastest dim is long (>= 256 elements: 2-D-like transpositions such as
+    // (a,b,i,j) -> (i,j,a,b)) take longer output runs and bigger tiles: >= 48 contiguous elements on the store side, ~3200
+    // elements (50 KB) per tile.  Measured (profiles/r2_transpose_sweep.md): that transposition of (200,200,40,40) 5.07 ->
+    // 6.0 TB/s, median of its 24 orders 5.41 -> 5.51 TB/s.  Applied to every large tensor it costs the shapes with short
+    // leading extents (60^3 x 12^3: median 5.99 -> 5.68 TB/s), and the 64-76 MB shapes lose 10 % (too few tiles for 296 CTAs).
+    long long total = 1;
+    for (int d = 0; d < r; ++d) total *= pd.extent[d];
+    const bool big = total >= (1LL << 24) && p.e[q[0]] >= env_int("TCB_PERM_BIGMIN", 256);
+    const int TI = env_int("TCB_PERM_TI", 32), TO = env_int("TCB_PERM_TO", big ? 48 : 32);
+    const int VOL = std::min(env_int("TCB_PERM_VOL", big ? 3200 : 2048), kMaxVol);
     // tile extent for a dim of extent e, between lo and hi: least padding first (ragged last tiles waste a CTA
     // slot), then 128-byte-aligned cuts (multiples of 8 elements: no cache line shared by two tiles), then
     // 32-byte-aligned cuts (even: no half-written sector), then the larger tile
