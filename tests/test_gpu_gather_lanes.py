@@ -208,3 +208,24 @@ def test_outer_product_route(ctx, expr, ext):
     """K = 1 (nothing contracted): the store-stream kernel of gemv.cu instead of a GEMM with K padded to 4"""
     err, plan, _ = run(ctx, expr, ext, alpha=0.75 - 0.5j, seed=len(expr))
     assert plan["route"] == "outer" and plan["K"] == 1 and err <= TOL
+
+
+def test_lane_api_argument_errors_leave_the_context_usable(ctx):
+    for bad in (-1, ctx.lane_count()):
+        with pytest.raises(pkg.TcbError) as ei:
+            ctx.lane_set(bad)
+        assert ei.value.code == binding.TCB_EINVAL
+        with pytest.raises(pkg.TcbError) as ei:
+            ctx.lane_wait(0, bad)
+        assert ei.value.code == binding.TCB_EINVAL
+    ctx.lane_wait(1, 1)                                        # a lane waiting on itself is a no-op
+    ctx.lane_set(1)
+    with pytest.raises(pkg.TcbError) as ei:
+        ctx.capture_begin()                                    # a capture starts on lane 0
+    assert ei.value.code == binding.TCB_EINVAL
+    t = ctx.tensor_create((4, 4))                              # created, filled and destroyed on lane 1
+    ctx.tensor_fill(t, 2.0 - 1.0j)
+    assert np.all(ctx.tensor_download(t) == 2.0 - 1.0j)
+    t.destroy()
+    ctx.lane_set(0)
+    ctx.sync()
