@@ -618,9 +618,135 @@ def ccsdt_residual(ctx, o, h, g, T1, T2, T3, R1=None, R2=None, R3=None):
     return R1, R2, R3
 
 
-def ccsdt_solve(ctx, o, h, g, f_diag, iterations):
+def ccsdt_residual_packed(ctx, o, h, g, T1, T2, T3, R1=None, R2=None, R3=None):
+    """`ccsdt_residual` with every contraction that touches T3 run on index-permutation-symmetric packed storage (SURVEY
+    8(f)-2 applied to 8(f)-3).  T2 and T3 must be antisymmetric within their virtual and within their
+    occupied indices (they are in `ccsdt_solve`: zero start + antisymmetric residuals).  The dense T3 is read by three
+    `tcb_pack` calls only:
+        Tq(d<e, c, i<j<k)      To(a<b<c, l<m, k)      Tr(b<c, j<k, e, m) = T3(b,c,e,j,k,m)
+    (T3(e,b,c,..) = T3(b,c,e,..): a cyclic relabelling has sign +), and the seven rank-6 contractions collapse onto three
+    packed accumulators -- the full antisymmetriser A3 that follows does not care which of a, b, c (of i, j, k) a term calls
+    its "single" index, and only the antisymmetric part of an intermediate survives it:
+        Xq(a<b, c, i<j<k)  = 2 Wvvvv(a<b, d<e) Tq(d<e, c, ijk)          + Tq(a<b, e, ijk) Fv(c, e)
+        Xo(a<b<c, i<j, k)  = 2 To(abc, l<m, k) Woooo(l<m, i<j)          + To(abc, i<j, m) Fo(m, k)
+        Xr(a, i, b<c, j<k) = Wr(m,a,i,e) Tr(b<c, j<k, e, m) + Wvvov(b<c, i, d) T2(d, a, j<k) + Wovoo(l, a, j<k) T2(b<c, l, i)
+    against the dense program: 1/32 of the flops for the vvvv term, 1/4 for the ring term; X is written by three
+    `tcb_unpack` calls and antisymmetrised by ONE 9-term permute-sum.  Same arguments and results as `ccsdt_residual`; needs o >= 3 and v >= 3."""
+    v = T1.extents[0]
+    if o < 3 or v < 3:
+        raise ValueError("ccsdt_residual_packed needs o >= 3 and v >= 3 (a<b<c groups)")
+    B = t1_dressed_blocks(ctx, o, h, g, T1, CCSDT_BLOCKS)
+    new = lambda shape: ctx.tensor_create(shape, zero=False)
+    con, add, pack, unpack = ctx.contract, ctx.add, ctx.pack, ctx.unpack
+    nv2, nv3, no2, no3 = (ctx.packed_extent(v, 2), ctx.packed_extent(v, 3), ctx.packed_extent(o, 2), ctx.packed_extent(o, 3))
+
+    def packed(shape, spec, src):
+        t = new(shape)
+        pack(spec, t, src)
+        return t
+    # ---- the three packed views of T3, the packed views of T2 and of the dressed integrals
+    Tq = packed((nv2, v, no3), "P(d<e,c,i<j<k)=T(d,e,c,i,j,k)", T3)
+    To = packed((nv3, no2, o), "P(a<b<c,l<m,k)=T(a,b,c,l,m,k)", T3)
+    Tr = packed((nv2, no2, v, o), "P(b<c,j<k,e,m)=T(b,c,e,j,k,m)", T3)
+    T2p = packed((nv2, no2), "P(a<b,l<m)=T(a,b,l,m)", T2)
+    T2x = packed((nv2, o, o), "P(b<c,l,i)=T(b,c,l,i)", T2)
+    T2y = packed((v, v, no2), "P(d,a,j<k)=T(d,a,j,k)", T2)
+    gp = packed((no2, nv2), "P(l<m,d<e)=g(l,m,d,e)", B["oovv"])
+    gs = packed((o, o, nv2), "P(l,m,d<e)=g(l,m,d,e)", B["oovv"])
+    gt = packed((no2, v, v), "P(l<m,d,e)=g(l,m,d,e)", B["oovv"])
+    gq = packed((no2, o, v), "P(l<m,i,d)=g(l,m,i,d)", B["ooov"])
+    gr = packed((o, v, nv2), "P(l,a,d<e)=g(l,a,d,e)", B["ovvv"])
+    # ---- singles
+    if R1 is None:
+        R1 = new((v, o))
+    add("R(a,i)=f(a,i)", R1, B["fvo"], 1.0)
+    con("R(a,i)+=f(l,d)*T(d,a,l,i)", R1, B["fov"], T2, 1.0)
+    con("R(a,i)+=W(l,m,i,d)*T(d,a,l,m)", R1, B["ooov"], T2, 0.5)
+    con("R(a,i)+=W(l,a,d,e)*T(d,e,l,i)", R1, B["ovvv"], T2, 0.5)
+    con("R(a,i)+=T(x,y,a,i)*W(y,x)", R1, Tr, gp, 1.0)                  # 1/4 sum_{de,lm} = sum_{d<e,l<m}
+    # ---- doubles: the CCD program on the dressed blocks + the three T3 terms
+    R2 = ccd_residual(ctx, B, T2, R2)
+    R2p = new((nv2, no2))
+    con("R(x,y)=T(x,y,d,l)*f(l,d)", R2p, Tr, B["fov"], 1.0)
+    unpack("R(a,b,i,j)+=P(a<b,i<j)", R2, R2p, 1.0)
+    R2p.destroy()
+    X2, X2a, X2b = new((v, v, o, o)), new((nv2, o, o)), new((v, v, no2))
+    con("X(x,i,j)=T(x,z,d,j)*W(z,i,d)", X2a, Tr, gq, 2.0)
+    unpack("X(a,b,i,j)=P(a<b,i,j)", X2, X2a, 1.0)
+    ctx.antisymmetrize("P(ij):R(a,b,i,j)+=X(a,b,i,j)", R2, X2, 0.5)
+    con("X(a,b,y)=W(l,a,z)*T(z,y,b,l)", X2b, gr, Tr, 2.0)
+    unpack("X(a,b,i,j)=P(a,b,i<j)", X2, X2b, 1.0)
+    ctx.antisymmetrize("P(ab):R(a,b,i,j)+=X(a,b,i,j)", R2, X2, 0.5)
+    for t in (X2, X2a, X2b):
+        t.destroy()
+    # ---- triples: intermediates.  Wovoo and Wvvov: T2 terms dense, their antisymmetric part packed, the T3 term added packed
+    Wd, Wa = new((o, v, o, o)), new((o, v, o, o))
+    add("W(l,a,i,j)=g(l,a,i,j)", Wd, B["ovoo"], 0.25)
+    con("W(l,a,i,j)+=f(l,d)*T(d,a,i,j)", Wd, B["fov"], T2, 0.25)
+    con("W(m,a,i,j)+=g(l,m,i,d)*T(d,a,l,j)", Wd, B["ooov"], T2, -0.5)
+    con("W(l,a,j,k)+=g(l,a,d,e)*T(d,e,j,k)", Wd, B["ovvv"], T2, 0.125)
+    ctx.antisymmetrize("P(ij):A(l,a,i,j)=W(l,a,i,j)", Wa, Wd, 0.5)
+    Wovoo = packed((o, v, no2), "P(l,a,i<j)=W(l,a,i,j)", Wa)
+    con("W(l,a,y)+=g(l,m,z)*T(z,y,a,m)", Wovoo, gs, Tr, -0.25)
+    Wd.destroy()
+    Wa.destroy()
+    Wd, Wa = new((v, v, o, v)), new((v, v, o, v))
+    add("W(a,b,i,d)=g(a,b,i,d)", Wd, B["vvov"], 0.25)
+    con("W(a,b,i,d)+=T(a,b,l,m)*g(l,m,i,d)", Wd, T2, B["ooov"], 0.125)
+    con("W(a,b,i,e)+=g(l,a,d,e)*T(d,b,l,i)", Wd, B["ovvv"], T2, -0.5)
+    ctx.antisymmetrize("P(ab):A(a,b,i,d)=W(a,b,i,d)", Wa, Wd, 0.5)
+    Wvvov = packed((nv2, o, v), "P(a<b,i,d)=W(a,b,i,d)", Wa)
+    con("W(x,i,d)+=T(x,z,e,i)*g(z,d,e)", Wvvov, Tr, gt, -0.25)
+    Wd.destroy()
+    Wa.destroy()
+    Fo, Fv = new((o, o)), new((v, v))
+    add("F(m,i)=f(m,i)", Fo, B["foo"], -1.0 / 12.0)
+    con("F(m,i)+=g(l,m,d,e)*T(d,e,l,i)", Fo, B["oovv"], T2, -1.0 / 24.0)
+    add("F(a,e)=f(a,e)", Fv, B["fvv"], 1.0 / 12.0)
+    con("F(a,e)+=g(l,m,d,e)*T(d,a,l,m)", Fv, B["oovv"], T2, -1.0 / 24.0)
+    Woooo, Wvvvv = new((no2, no2)), new((nv2, nv2))
+    gpk = packed((no2, no2), "P(l<m,i<j)=g(l,m,i,j)", B["oooo"])
+    add("W(z,y)=g(z,y)", Woooo, gpk, 1.0 / 24.0)
+    gpk.destroy()
+    con("W(z,y)+=g(z,x)*T(x,y)", Woooo, gp, T2p, 1.0 / 24.0)           # 1/48 sum_de = 1/24 sum_{d<e}
+    gpk = packed((nv2, nv2), "P(a<b,d<e)=g(a,b,d,e)", B["vvvv"])
+    add("W(x,z)=g(x,z)", Wvvvv, gpk, 1.0 / 24.0)
+    gpk.destroy()
+    con("W(x,z)+=T(x,y)*g(y,z)", Wvvvv, T2p, gp, 1.0 / 24.0)
+    Wr = new((o, v, o, v))
+    add("W(m,a,i,e)=g(m,a,i,e)", Wr, B["ovov"], -0.25)
+    con("W(m,a,i,e)+=g(l,m,d,e)*T(d,a,l,i)", Wr, B["oovv"], T2, 0.25)
+    for t in list(B.values()) + [gp, gs, gt, gq, gr, T2p]:
+        t.destroy()
+    # ---- triples: the three packed accumulators
+    Xq, Xo, Xr = new((nv2, v, no3)), new((nv3, no2, o)), new((v, o, nv2, no2))
+    con("X(x,c,t)=W(x,z)*T(z,c,t)", Xq, Wvvvv, Tq, 2.0)
+    con("X(x,c,t)+=T(x,e,t)*F(c,e)", Xq, Tq, Fv, 1.0)
+    con("X(t,y,k)=T(t,z,k)*W(z,y)", Xo, To, Woooo, 2.0)
+    con("X(t,y,k)+=T(t,y,m)*F(m,k)", Xo, To, Fo, 1.0)
+    con("X(a,i,x,y)=W(m,a,i,e)*T(x,y,e,m)", Xr, Wr, Tr, 1.0)
+    con("X(a,i,x,y)+=W(x,i,d)*T(d,a,y)", Xr, Wvvov, T2y, 1.0)
+    con("X(a,i,x,y)+=W(l,a,y)*T(x,l,i)", Xr, Wovoo, T2x, 1.0)
+    for t in (Wovoo, Wvvov, Fo, Fv, Woooo, Wvvvv, Wr, Tq, To, Tr, T2x, T2y):
+        t.destroy()
+    # Each accumulator is unpacked under the relabelling (cyclic: sign +) that makes it antisymmetric in (b,c) and in (j,k);
+    # on such an X the 36-term A3 is 4 P(a/bc) P(i/jk): one 9-term pass of the orbit kernel, no 4-term pass, no second 6 GB.
+    X = new((v, v, v, o, o, o))
+    unpack("X(a,b,c,i,j,k)=P(a,i,b<c,j<k)", X, Xr, 1.0)
+    unpack("X(a,b,c,i,j,k)+=P(b<c,a,i<j<k)", X, Xq, 1.0)
+    unpack("X(a,b,c,i,j,k)+=P(a<b<c,j<k,i)", X, Xo, 1.0)
+    for t in (Xq, Xo, Xr):
+        t.destroy()
+    if R3 is None:
+        R3 = new((v, v, v, o, o, o))
+    ctx.antisymmetrize("P(a/bc)P(i/jk):R(a,b,c,i,j,k)=X(a,b,c,i,j,k)", R3, X, 4.0)
+    X.destroy()
+    return R1, R2, R3
+
+
+def ccsdt_solve(ctx, o, h, g, f_diag, iterations, packed=False):
     """Jacobi iterations of the CCSDT amplitude equations from zero amplitudes (oracle: cc.ccsdt_jacobi): per iteration
-    `ccsdt_residual`, the residual norm |R|, the energy of the amplitudes the evaluation saw, and three
+    `ccsdt_residual` (`ccsdt_residual_packed` with packed=True), the residual norm |R|, the energy of the amplitudes the evaluation saw, and three
     `tcb_denominator_update`.  f_diag: the n orbital energies (diagonal of the Fock matrix).
     Returns (T1, T2, T3, [E_corr per evaluation], [|R| per evaluation])."""
     import numpy as np
@@ -640,7 +766,7 @@ def ccsdt_solve(ctx, o, h, g, f_diag, iterations):
         ctx.contract("E()+=W(i,j,a,b)*T(a,b,i,j)", E, Bz["oovv"], T2, 0.25)
         ctx.contract("Y(i,a)=W(i,j,a,b)*T(b,j)", Y, Bz["oovv"], T1, 1.0)
         ctx.contract("E()+=Y(i,a)*T(a,i)", E, Y, T1, 0.5)
-        ccsdt_residual(ctx, o, h, g, T1, T2, T3, R1, R2, R3)
+        (ccsdt_residual_packed if packed else ccsdt_residual)(ctx, o, h, g, T1, T2, T3, R1, R2, R3)
         energies.append(complex(ctx.tensor_download(E)))
         norms.append(residual_norm(ctx, R1, R2, R3))
         E.destroy()

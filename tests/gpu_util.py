@@ -210,3 +210,27 @@ class ShadowContext:
         ref = oracle.permsum(D.host, X.host, perms, [alpha * s for s in signs], 1.0 if acc else 0.0)
         sn = abs(alpha) * oracle.permsum(np.zeros_like(D.host), X.norm, perms, [1.0] * len(signs), 0.0).real
         self._compare(spec, D, ref, sn + (D.norm if acc else 0.0))
+
+    def packed_extent(self, n, k):
+        return self.ctx.packed_extent(n, k)
+
+    def pack(self, spec, D, L):
+        """pure data movement: the device result is the oracle's pack of the DEVICE's operand, bit for bit (the operand itself
+        was compared, under its snorm, by the call that produced it); the shadow carries the oracle's own values on"""
+        from oracle import sym
+        self.ctx.pack(spec, D.gpu, L.gpu)
+        self.ctx.sync()
+        ref = np.asfortranarray(sym.pack(spec, np.asarray(self.ctx.tensor_download(L.gpu))))
+        got = np.asarray(self.ctx.tensor_download(D.gpu))
+        assert got.shape == ref.shape and np.array_equal(got.ravel(order="F").view(np.uint64),
+                                                         ref.ravel(order="F").view(np.uint64)), ("pack moves bits", spec)
+        self.calls += 1
+        D.host, D.norm = sym.pack(spec, L.host), sym.pack(spec, L.norm).real
+
+    def unpack(self, spec, D, L, alpha=1.0):
+        from oracle import sym
+        self.ctx.unpack(spec, D.gpu, L.gpu, alpha)
+        acc = "+=" in spec
+        ref = sym.unpack(spec, L.host, D.host, alpha)
+        sn = abs(alpha) * np.abs(sym.unpack(spec.replace("+=", "=", 1), L.norm, np.zeros_like(D.host), 1.0))
+        self._compare(spec, D, ref, sn + (D.norm if acc else 0.0))

@@ -4,6 +4,7 @@ the call list's result with the unfactorised equations.  Test infrastructure onl
 import numpy as np
 
 import oracle
+from oracle import sym
 from gpu_util import expand_antisym_spec
 
 
@@ -46,4 +47,16 @@ class OracleContext:
     def antisymmetrize(self, spec, D, X, alpha=1.0):
         perms, signs, acc = expand_antisym_spec(spec)
         D.host = oracle.permsum(D.host, X.host, perms, [alpha * s for s in signs], 1.0 if acc else 0.0)
+        self.calls += 1
+
+    def packed_extent(self, n, k):
+        return sym.packed_extent(n, k)
+
+    def pack(self, spec, D, L):
+        D.host = sym.pack(spec, L.host)
+        assert D.host.shape == tuple(D.extents), (spec, D.host.shape, D.extents)
+        self.calls += 1
+
+    def unpack(self, spec, D, L, alpha=1.0):
+        D.host = sym.unpack(spec, L.host, D.host, alpha)
         self.calls += 1

@@ -415,7 +415,30 @@ def test_ccsdt_residual_call_by_call_and_against_the_fock_space_pinned_equations
     assert np.abs(gR3 + gR3.transpose(1, 0, 2, 3, 4, 5)).max() <= 1e-12 * np.abs(R3.norm).max()
 
 
-def test_ccsdt_iterations_follow_the_oracle_and_converge(ctx):
+@pytest.mark.parametrize("o,v", [(3, 4), (4, 6), (5, 5)])
+def test_packed_ccsdt_residual_call_by_call_and_against_the_fock_space_pinned_equations(ctx, o, v):
+    """SURVEY 8(f)-2 applied to 8(f)-3: ccd.ccsdt_residual_packed -- every contraction with T3 on a<b / a<b<c packed storage --
+    call by call against the oracle (tcb_pack bit-exact, tcb_unpack and the contractions under their carried snorm), the
+    residuals against the unfactorised equations, and against the dense driver."""
+    from gpu_util import ShadowContext
+    f, g, h, t1, t2, t3 = _ccsdt_inputs(o, v, 100 * o + v)
+    sh = ShadowContext(ctx)
+    R1, R2, R3 = ccd.ccsdt_residual_packed(sh, o, sh.wrap(h), sh.wrap(g), sh.wrap(t1), sh.wrap(t2), sh.wrap(t3))
+    assert sh.calls == 112 and sh.worst <= 1e-11
+    e, r1, r2, r3 = cc.ccsdt_residual_unfactorised(o, f, g, t1, t2, t3)
+    W = ctx.tensor_from_numpy
+    D1, D2, D3 = ccd.ccsdt_residual(ctx, o, W(h), W(g), W(t1), W(t2), W(t3))
+    for got, ref, dense in ((R1, r1, D1), (R2, r2, D2), (R3, r3, D3)):
+        dev = ctx.tensor_download(got.gpu)
+        scale = np.abs(got.norm).max()
+        assert np.abs(dev - ref).max() <= 1e-11 * scale
+        assert np.abs(dev - ctx.tensor_download(dense)).max() <= 1e-11 * scale
+    gR3 = ctx.tensor_download(R3.gpu)
+    assert np.abs(gR3 + gR3.transpose(0, 1, 2, 4, 3, 5)).max() <= 1e-12 * np.abs(R3.norm).max()
+
+
+@pytest.mark.parametrize("packed", [False, True])
+def test_ccsdt_iterations_follow_the_oracle_and_converge(ctx, packed):
     o, v = 3, 3
     rng = np.random.default_rng(52)
     n = o + v
@@ -431,7 +454,7 @@ def test_ccsdt_iterations_follow_the_oracle_and_converge(ctx):
     h = f - np.einsum("piqi->pq", g[:, :o, :, :o])
     its = 12
     dh, dg = ctx.tensor_from_numpy(h), ctx.tensor_from_numpy(g)
-    T1, T2, T3, energies, norms = ccd.ccsdt_solve(ctx, o, dh, dg, e, its)
+    T1, T2, T3, energies, norms = ccd.ccsdt_solve(ctx, o, dh, dg, e, its, packed=packed)
     r1, r2, r3, e_ref, n_ref = cc.ccsdt_jacobi(o, f, g, its)
     for got, ref in ((T1, r1), (T2, r2), (T3, r3)):
         assert np.abs(ctx.tensor_download(got) - ref).max() <= 1e-10 * max(np.abs(ref).max(), 1e-300)

@@ -386,6 +386,26 @@ def test_ccsdt_driver_call_list_is_the_unfactorised_equations():
     assert oc.calls == 90
 
 
+@pytest.mark.parametrize("o,v", [(3, 3), (3, 4), (4, 4)])
+def test_packed_ccsdt_driver_call_list_is_the_unfactorised_equations(o, v):
+    """ccd.ccsdt_residual_packed (every T3 contraction on a<b / a<b<c packed storage: three packed views of T3, three packed
+    accumulators, three unpacks) run on the host with the oracle's contract / add / permsum / sym.pack / sym.unpack: equals
+    the unfactorised 37-term evaluation, and the dense driver."""
+    from oracle_ctx import OracleContext
+    from paper_2409_06759_b200 import ccd
+    f, g, t1, t2, t3 = _ccsdt_problem(o, v, 78 + o + v)
+    h = f - np.einsum("piqi->pq", g[:, :o, :, :o])
+    oc = OracleContext()
+    W = oc.tensor_from_numpy
+    R1, R2, R3 = ccd.ccsdt_residual_packed(oc, o, W(h), W(g), W(t1), W(t2), W(t3))
+    e, r1, r2, r3 = cc.ccsdt_residual_unfactorised(o, f, g, t1, t2, t3)
+    for got, ref in ((R1.host, r1), (R2.host, r2), (R3.host, r3)):
+        assert np.abs(got - ref).max() <= 1e-12 * np.abs(ref).max()
+    assert oc.calls == 112
+    with pytest.raises(ValueError):
+        ccd.ccsdt_residual_packed(oc, 2, W(h), W(g), W(t1[:, :2]), W(t2), W(t3))
+
+
 def test_converged_ccsdt_iteration_zeroes_all_three_fock_space_projections():
     """Jacobi iterations of the CCSDT equations on a weakly coupled Hermitian problem (non-zero occupied-virtual Fock block,
     so t1 != 0): at the fixed point the singles, doubles AND triples projections of exp(-T) H exp(T)|Phi0> vanish and the
