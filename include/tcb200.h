@@ -178,10 +178,25 @@ int tcb_antisymmetrize(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_
  *   tcb_unpack spec "R(a,b,i,j)+=Rp(a<b,i<j)" (or '='): D[.., a, .., b, ..] (+)= alpha * sign * Lp[.., p(sorted a, b), ..],
  *              sign = parity of the sorting permutation, 0 when two labels of a group coincide.  With alpha = 1 and '=' an
  *              exactly antisymmetric tensor comes back bit for bit.
- * Errors: TCB_EINVAL_EXPR (syntax, no group, '+=' in tcb_pack, labels not matching), TCB_ESHAPE (ranks, unequal extents in a
- * group, packed extent not n choose k), TCB_EUNSUPPORTED (groups of more than 3 labels, repeated label), TCB_EALIAS. */
+ *              D may carry groups too -- a packed view of a packed tensor, "Tq(d<e,c,i<j<k)=T(d<e<c,i<j<k)": an element of D
+ *              fixes the values of all labels (increasing inside D's groups), and L is read at them by the same rule, one
+ *              signed read per element.  Any two groupings of the same labels are allowed.
+ *   tcb_antisym_pack spec "R(a<b<c,i<j<k)+=X(a,i,b<c,j<k)" (or '='): the permutation operator P(a/bc)P(i/jk) of the paper's
+ *              notation evaluated on packed storage.  Every group of L must lie inside one group of D.  For
+ *              an element of D (one increasing tuple per group) the sum runs over the SHUFFLES of each tuple: the ways to
+ *              hand its components to the group's labels such that the labels of one L group, in D's order, receive
+ *              increasing components -- 3 for (a | b<c), 6 for (a | b | c), 1 for (a<b<c); sign = parity of the assignment:
+ *                  D[tuples] (+)= alpha * sum_shuffles sign * L[at those label values],
+ *              terms added in a fixed order (first group of D fastest), then one multiplication by alpha.  With L dense this
+ *              is the full antisymmetriser (36 terms for two triples) restricted to a<b<c, i<j<k.  At most 36 terms.
+ * Errors: TCB_EINVAL_EXPR (syntax, no group, '+=' in tcb_pack, labels not matching, an L group spread over two D groups in
+ * tcb_antisym_pack), TCB_ESHAPE (ranks, unequal extents in a group, packed extent not n choose k), TCB_EUNSUPPORTED (groups
+ * of more than 3 labels, repeated label, group labels of extent above 65535 when both sides are packed), TCB_EALIAS.  The
+ * first call that meets a new (extent, group size) builds a tuple table on the device: like a first plan, it is refused
+ * inside a stream capture. */
 int tcb_pack(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *L);
 int tcb_unpack(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *L, tcb_c128 alpha);
+int tcb_antisym_pack(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *L, tcb_c128 alpha);
 int64_t tcb_packed_extent(int64_t n, int k);      /* n choose k for k = 1, 2, 3; -1 otherwise */
 /* JSON description of the plan tcb_contract would use: M, N, K, which operands are permuted, GEMM variant,
  * split-K, estimated flops and bytes.  Truncated to buflen-1 characters. */

@@ -45,7 +45,7 @@ ABI_SYMBOLS = [
     "tcb_denominator_update", "tcb_denominator_divide", "tcb_dot",
     "tcb_permute", "tcb_permsum", "tcb_antisymmetrize", "tcb_plan_describe", "tcb_measure_fp64_tensor_peak", "tcb_measure_fp64_vector_peak",
     "tcb_capture_begin", "tcb_capture_end", "tcb_graph_launch", "tcb_graph_info", "tcb_graph_destroy",
-    "tcb_lane_count", "tcb_lane_set", "tcb_lane_wait", "tcb_pack", "tcb_unpack", "tcb_packed_extent",
+    "tcb_lane_count", "tcb_lane_set", "tcb_lane_wait", "tcb_pack", "tcb_unpack", "tcb_antisym_pack", "tcb_packed_extent",
     "tcb_timer_start", "tcb_timer_stop", "tcb_kernel_stats", "tcb_kernel_stats_reset", "tcb_plan_describe_host", "tcbx_synth_normal", "tcbx_synth_index_linear",
     "tcbx_synth_mp2_amplitudes",
 ]
@@ -97,6 +97,7 @@ def load_library():
         "tcb_lane_count": [],
         "tcb_pack": [vp, cp, vp, vp],
         "tcb_unpack": [vp, cp, vp, vp, c128],
+        "tcb_antisym_pack": [vp, cp, vp, vp, c128],
         "tcb_lane_set": [vp, ctypes.c_int],
         "tcb_lane_wait": [vp, ctypes.c_int, ctypes.c_int],
         "tcb_timer_start": [vp],
@@ -327,6 +328,11 @@ class Context:
     def unpack(self, spec, D, L, alpha=1.0):
         """'R(a,b,i,j)+=Rp(a<b,i<j)': D (+)= alpha * sign * Lp[packed position] (tcb_unpack)"""
         self._check(self.lib.tcb_unpack(self.handle, spec.encode(), D.handle, L.handle, _c(alpha)))
+
+    def antisym_pack(self, spec, D, L, alpha=1.0):
+        """'R(a<b<c,i<j<k)+=X(a,i,b<c,j<k)': P(a/bc)P(i/jk) on packed storage, D (+)= alpha * signed sum over the shuffles
+        (tcb_antisym_pack)"""
+        self._check(self.lib.tcb_antisym_pack(self.handle, spec.encode(), D.handle, L.handle, _c(alpha)))
 
     def packed_extent(self, n, k):
         return int(self.lib.tcb_packed_extent(int(n), int(k)))

@@ -59,6 +59,7 @@ struct tcb_ctx {
     PlanOptions opt;
     std::map<std::string, std::unique_ptr<CachedPlan>> plans;
     std::map<std::string, std::unique_ptr<struct SymTables>> sym_tables;   // tcb_pack offset tables per (spec, extents)
+    std::map<std::pair<int64_t, int>, SymTuple *> sym_tuples;              // device: the increasing k-tuples of range(n)
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     int64_t live_tensors = 0;
     // per-kernel-class device timing ("kernel_timing" = "on"): event pairs around every launch, summed on query
@@ -390,6 +391,7 @@ int tcb_ctx_destroy(tcb_ctx *ctx)
     for (Lane &ln : ctx->lanes) if (ln.stream) cudaStreamSynchronize(ln.stream);
     for (auto &kv : ctx->plans)
         if (kv.second->d_tables) cudaFree(kv.second->d_tables);
+    for (auto &kv : ctx->sym_tuples) cudaFree(kv.second);
     for (auto &kv : ctx->sym_tables)
         if (kv.second->dev) cudaFree(kv.second->dev);
     for (Lane &ln : ctx->lanes) if (ln.ws) cudaFree(ln.ws);
@@ -1118,6 +1120,134 @@ int bind_sym_spec(tcb_ctx *ctx, const std::vector<std::vector<std::string>> &pac
     return TCB_OK;
 }
 
+
+// inverse of choose: the n with choose(n, k) == e, or -1
+int64_t unchoose(int64_t e, int k)
+{
+    for (int64_t n = k; n < 70000; ++n) {
+        const int64_t c = choose(n, k);
+        if (c == e) return n;
+        if (c > e) break;
+    }
+    return -1;
+}
+
+// A spec with a<b groups on BOTH sides: labels, their extents, and which (index, slot) of each side a label sits in.
+struct SymBinding {
+    std::vector<std::string> labels;
+    std::vector<int64_t> ext;
+    std::vector<std::vector<int>> dg, lg;         // per index of D / L: the label ids of its group, in the group's order
+};
+
+int bind_sym_general(tcb_ctx *ctx, const SymSpec &sp, const tcb_tensor *D, const tcb_tensor *L, SymBinding *b)
+{
+    if ((int)sp.lhs.size() != D->shape.rank || (int)sp.rhs.size() != L->shape.rank)
+        return set_error(ctx, TCB_ESHAPE, "rank of a handle differs from the spec");
+    auto side = [&](const std::vector<std::vector<std::string>> &groups, std::vector<std::vector<int>> *out, bool first) -> int {
+        size_t seen = 0;
+        for (const auto &grp : groups) {
+            if (grp.size() > 3) return set_error(ctx, TCB_EUNSUPPORTED, "groups of more than three labels");
+            std::vector<int> ids;
+            for (const auto &lab : grp) {
+                int id = find_label(b->labels, lab);
+                if (first) {
+                    if (id >= 0) return set_error(ctx, TCB_EUNSUPPORTED, "label repeated inside a tensor");
+                    id = (int)b->labels.size();
+                    b->labels.push_back(lab);
+                } else if (id < 0) return set_error(ctx, TCB_EINVAL_EXPR, "label " + lab + " is on one side only");
+                for (const auto &g2 : *out) for (int x : g2) if (x == id) return set_error(ctx, TCB_EUNSUPPORTED, "label repeated inside a tensor");
+                for (int x : ids) if (x == id) return set_error(ctx, TCB_EUNSUPPORTED, "label repeated inside a tensor");
+                ids.push_back(id);
+                ++seen;
+            }
+            out->push_back(ids);
+        }
+        if (!first && seen != b->labels.size()) return set_error(ctx, TCB_EINVAL_EXPR, "a label is on one side only");
+        return TCB_OK;
+    };
+    int rc = side(sp.lhs, &b->dg, true);
+    if (rc) return rc;
+    rc = side(sp.rhs, &b->lg, false);
+    if (rc) return rc;
+    b->ext.assign(b->labels.size(), -1);
+    auto extents = [&](const std::vector<std::vector<int>> &groups, const tcb_tensor *T) -> int {
+        for (size_t g = 0; g < groups.size(); ++g) {
+            const int k = (int)groups[g].size();
+            const int64_t n = k == 1 ? T->shape.ext[g] : unchoose(T->shape.ext[g], k);
+            if (n < 0) return set_error(ctx, TCB_ESHAPE, "packed extent is not n(n-1)/2 (n(n-1)(n-2)/6) of any n");
+            if (k > 1 && n > 65535) return set_error(ctx, TCB_EUNSUPPORTED, "group labels of extent above 65535");
+            for (int id : groups[g]) {
+                if (b->ext[id] >= 0 && b->ext[id] != n) return set_error(ctx, TCB_ESHAPE, "a label has two extents (or a group mixes extents)");
+                b->ext[id] = n;
+            }
+        }
+        return TCB_OK;
+    };
+    rc = extents(b->dg, D);
+    if (rc) return rc;
+    return extents(b->lg, L);
+}
+
+// the device table of the strictly increasing k-tuples of range(n), first label fastest (built once per (n, k))
+int sym_tuple_table(tcb_ctx *ctx, int64_t n, int k, const SymTuple **out)
+{
+    auto it = ctx->sym_tuples.find({n, k});
+    if (it == ctx->sym_tuples.end()) {
+        int rc = refuse_in_capture(ctx, "the first use of an a<b group of this extent (run the call list once before capturing it)");
+        if (rc) return rc;
+        std::vector<SymTuple> host;
+        host.reserve((size_t)choose(n, k));
+        if (k == 2) { for (int64_t y = 0; y < n; ++y) for (int64_t x = 0; x < y; ++x) host.push_back(SymTuple{{(unsigned short)x, (unsigned short)y, 0, 0}}); }
+        else for (int64_t z = 0; z < n; ++z) for (int64_t y = 0; y < z; ++y) for (int64_t x = 0; x < y; ++x)
+                 host.push_back(SymTuple{{(unsigned short)x, (unsigned short)y, (unsigned short)z, 0}});
+        SymTuple *dev = nullptr;
+        TCB_CUDA(ctx, cudaMalloc((void **)&dev, std::max<size_t>(1, host.size()) * sizeof(SymTuple)));
+        cudaError_t e = cudaMemcpyAsync(dev, host.data(), host.size() * sizeof(SymTuple), cudaMemcpyHostToDevice, cur_stream(ctx));
+        if (e == cudaSuccess) e = cudaStreamSynchronize(cur_stream(ctx));   // host vector dies here; usable from every lane
+        if (e != cudaSuccess) { cudaFree(dev); return cuda_fail(ctx, e, "cudaMemcpyAsync(tuple table)"); }
+        it = ctx->sym_tuples.emplace(std::make_pair(n, k), dev).first;
+    }
+    *out = it->second;
+    return TCB_OK;
+}
+
+// fills the descriptor's structure (not the terms) from a binding
+int symmap_structure(tcb_ctx *ctx, const SymBinding &b, const tcb_tensor *D, const tcb_tensor *L, SymMapDesc *d)
+{
+    d->nd = D->shape.rank;
+    d->nl = L->shape.rank;
+    int64_t sL[kMaxRank];
+    strides_of(L->shape, sL);
+    std::vector<int> ldim(b.labels.size()), lslot(b.labels.size());
+    for (int k = 0; k < kMaxRank; ++k) {
+        d->dext[k] = k < d->nd ? D->shape.ext[k] : 1;
+        d->dlen[k] = k < d->nd ? (int)b.dg[k].size() : 1;
+        d->dtab[k] = nullptr;
+        if (k < d->nd) {
+            for (size_t s = 0; s < b.dg[k].size(); ++s) { ldim[b.dg[k][s]] = k; lslot[b.dg[k][s]] = (int)s; }
+            if (d->dlen[k] > 1) {
+                int rc = sym_tuple_table(ctx, b.ext[b.dg[k][0]], d->dlen[k], &d->dtab[k]);
+                if (rc) return rc;
+            }
+        }
+    }
+    for (int g = 0; g < kMaxRank; ++g) {
+        d->llen[g] = g < d->nl ? (int)b.lg[g].size() : 1;
+        d->lstride[g] = g < d->nl ? sL[g] : 0;
+        for (int s = 0; s < 3; ++s) {
+            const bool on = g < d->nl && s < d->llen[g];
+            d->lsrc_dim[g][s] = on ? ldim[b.lg[g][s]] : 0;
+            d->lsrc_slot[g][s] = on ? lslot[b.lg[g][s]] : 0;
+        }
+    }
+    for (int t = 0; t < kMaxSymTerms; ++t) {
+        d->sign[t] = 1;
+        for (int k = 0; k < kMaxRank; ++k) for (int s = 0; s < 3; ++s) d->perm[t][k][s] = (unsigned char)s;
+    }
+    d->nterms = 1;
+    return TCB_OK;
+}
+
 }  // namespace
 
 int tcb_pack(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *L)
@@ -1178,6 +1308,24 @@ int tcb_unpack(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *
     if (!spec || !D || !L) return set_error(ctx, TCB_EINVAL, "null argument");
     SymSpec sp;
     if (!parse_sym_spec(spec, &sp)) return set_error(ctx, TCB_EINVAL_EXPR, std::string("cannot parse: ") + spec);
+    bool d_groups = false;
+    for (const auto &g : sp.lhs) d_groups = d_groups || g.size() > 1;
+    if (d_groups) {
+        // a<b groups on D as well: a packed view of a packed tensor, "Tq(d<e,c,i<j<k)=T(d<e<c,i<j<k)" -- one signed read each
+        SymBinding b;
+        rc = bind_sym_general(ctx, sp, D, L, &b);
+        if (rc) return rc;
+        if (overlaps(D, L)) return set_error(ctx, TCB_EALIAS, "D overlaps L");
+        SymMapDesc m;
+        rc = symmap_structure(ctx, b, D, L, &m);
+        if (rc) return rc;
+        m.alpha_re = alpha.re; m.alpha_im = alpha.im;
+        m.accumulate = sp.accumulate;
+        m.in = L->ptr; m.out = D->ptr;
+        TimedLaunch tl(ctx, kClsPermute, 0.0, 16.0 * (double)D->elems() * (sp.accumulate ? 3.0 : 2.0));
+        TCB_CUDA(ctx, launch_symmap(m, cur_stream(ctx), &ctx->launches));
+        return TCB_OK;
+    }
     int pos[kMaxRank][3];
     rc = bind_sym_spec(ctx, sp.rhs, sp.lhs, L, D, pos);
     if (rc) return rc;
@@ -1198,6 +1346,76 @@ int tcb_unpack(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *
     d.in = L->ptr; d.out = D->ptr;
     TimedLaunch tl(ctx, kClsPermute, 0.0, 16.0 * ((double)D->elems() * (sp.accumulate ? 2.0 : 1.0) + (double)L->elems()));
     TCB_CUDA(ctx, launch_unpack(d, cur_stream(ctx), &ctx->launches));
+    return TCB_OK;
+}
+
+int tcb_antisym_pack(tcb_ctx *ctx, const char *spec, tcb_tensor *D, const tcb_tensor *L, tcb_c128 alpha)
+{
+    NvtxRange nvtx_range("tcb_antisym_pack");
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!spec || !D || !L) return set_error(ctx, TCB_EINVAL, "null argument");
+    SymSpec sp;
+    if (!parse_sym_spec(spec, &sp)) return set_error(ctx, TCB_EINVAL_EXPR, std::string("cannot parse: ") + spec);
+    SymBinding b;
+    rc = bind_sym_general(ctx, sp, D, L, &b);
+    if (rc) return rc;
+    if (overlaps(D, L)) return set_error(ctx, TCB_EALIAS, "D overlaps L");
+    // every group of L must lie inside one group of D: D's groups are unions of L's
+    std::vector<int> dim_of(b.labels.size()), slot_of(b.labels.size());
+    for (size_t k = 0; k < b.dg.size(); ++k)
+        for (size_t s = 0; s < b.dg[k].size(); ++s) { dim_of[b.dg[k][s]] = (int)k; slot_of[b.dg[k][s]] = (int)s; }
+    for (const auto &g : b.lg)
+        for (int id : g)
+            if (dim_of[id] != dim_of[g[0]]) return set_error(ctx, TCB_EINVAL_EXPR, "a group of L is spread over two groups of D");
+    SymMapDesc m;
+    rc = symmap_structure(ctx, b, D, L, &m);
+    if (rc) return rc;
+    // the shuffles: per group of D, the assignments slot -> tuple component under which every block (a group of L, its
+    // labels taken in D's slot order) receives increasing components; sign = parity of the assignment
+    struct Choice { unsigned char perm[3]; int sign; };
+    std::vector<std::vector<Choice>> per_dim(b.dg.size());
+    for (size_t k = 0; k < b.dg.size(); ++k) {
+        const int n = (int)b.dg[k].size();
+        int block[3] = {0, 0, 0};
+        for (size_t g = 0; g < b.lg.size(); ++g)
+            for (int id : b.lg[g]) if (dim_of[id] == (int)k) block[slot_of[id]] = (int)g;
+        int perm[3] = {0, 1, 2};
+        do {
+            bool ok = true;
+            for (int s1 = 0; s1 < n && ok; ++s1)
+                for (int s2 = s1 + 1; s2 < n && ok; ++s2)
+                    if (block[s1] == block[s2] && perm[s1] > perm[s2]) ok = false;
+            if (ok) {
+                int inv = 0;
+                for (int s1 = 0; s1 < n; ++s1) for (int s2 = s1 + 1; s2 < n; ++s2) inv += perm[s1] > perm[s2] ? 1 : 0;
+                Choice c;
+                for (int s1 = 0; s1 < 3; ++s1) c.perm[s1] = (unsigned char)(s1 < n ? perm[s1] : s1);
+                c.sign = inv % 2 ? -1 : 1;
+                per_dim[k].push_back(c);
+            }
+        } while (std::next_permutation(perm, perm + n));
+    }
+    size_t nterms = 1;
+    for (const auto &v : per_dim) nterms *= v.size();
+    if (nterms > (size_t)kMaxSymTerms) return set_error(ctx, TCB_EUNSUPPORTED, "more than 36 signed terms");
+    m.nterms = (int)nterms;
+    for (size_t t = 0; t < nterms; ++t) {            // first group of D fastest
+        size_t r = t;
+        int sign = 1;
+        for (size_t k = 0; k < per_dim.size(); ++k) {
+            const Choice &c = per_dim[k][r % per_dim[k].size()];
+            r /= per_dim[k].size();
+            for (int s1 = 0; s1 < 3; ++s1) m.perm[t][k][s1] = c.perm[s1];
+            sign *= c.sign;
+        }
+        m.sign[t] = (signed char)sign;
+    }
+    m.alpha_re = alpha.re; m.alpha_im = alpha.im;
+    m.accumulate = sp.accumulate;
+    m.in = L->ptr; m.out = D->ptr;
+    TimedLaunch tl(ctx, kClsPermute, 0.0, 16.0 * (double)D->elems() * ((double)nterms + (sp.accumulate ? 2.0 : 1.0)));
+    TCB_CUDA(ctx, launch_symmap(m, cur_stream(ctx), &ctx->launches));
     return TCB_OK;
 }
 

@@ -143,6 +143,31 @@ struct UnpackDesc {
     void *out;
 };
 cudaError_t launch_unpack(const UnpackDesc &d, cudaStream_t stream, int64_t *launches);
+// symmap: both tensors packed.  An element of D fixes a strictly increasing tuple per D index; term t hands the tuple's
+// components to the index's labels in the order perm[t]; L is read at the sorted values of its groups' labels:
+//   out[e] (+)= alpha * sum_t sign[t] * sortsign * in[sum_g p(sorted labels of L group g) * lstride[g]]
+// one identity term: tcb_unpack onto a packed D ("split"); the shuffles of the D groups: tcb_antisym_pack ("merge")
+constexpr int kMaxSymTerms = 36;
+struct SymTuple { unsigned short v[4]; };   // one strictly increasing tuple (k = 2, 3), first label first
+struct SymMapDesc {
+    int nd;                                  // rank of D
+    int64_t dext[kMaxRank];                  // extents of D (packed)
+    int dlen[kMaxRank];                      // labels per D index
+    const SymTuple *dtab[kMaxRank];          // device: tuple of packed value i of D index d (nullptr when dlen == 1)
+    int nl;                                  // rank of L
+    int llen[kMaxRank];
+    int lsrc_dim[kMaxRank][3];               // label s of L group g takes its value from D index lsrc_dim, slot lsrc_slot
+    int lsrc_slot[kMaxRank][3];
+    int64_t lstride[kMaxRank];
+    int nterms;
+    unsigned char perm[kMaxSymTerms][kMaxRank][3];
+    signed char sign[kMaxSymTerms];
+    double alpha_re, alpha_im;
+    bool accumulate;
+    const void *in;
+    void *out;
+};
+cudaError_t launch_symmap(const SymMapDesc &d, cudaStream_t stream, int64_t *launches);
 
 // ---- S7: elementwise --------------------------------------------------------------------------------------
 cudaError_t launch_fill(void *D, int64_t n, double re, double im, cudaStream_t stream, int64_t *launches);

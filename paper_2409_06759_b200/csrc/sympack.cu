@@ -193,6 +193,81 @@ __global__ void __launch_bounds__(256) unpack_kernel(const __grid_constant__ Unp
     }
 }
 
+// ---- symmap: D and L both packed (tcb_unpack onto a packed D, tcb_antisym_pack) ------------------------------------------------
+struct SymMapParams {
+    int nd, nl, nterms, accumulate;
+    long long dext[kMaxRank];
+    int dlen[kMaxRank];
+    const SymTuple *dtab[kMaxRank];
+    int llen[kMaxRank];
+    int lsrc_dim[kMaxRank][3], lsrc_slot[kMaxRank][3];
+    long long lstride[kMaxRank];
+    unsigned char perm[kMaxSymTerms][kMaxRank][3];
+    signed char sign[kMaxSymTerms];
+    long long total;
+    double ar, ai;
+    const double2 *in;
+    double2 *out;
+};
+
+// One thread per element of D (D is the small, packed side or a packed view of it).  The tuple of every D index sits in one
+// 64-bit register (16 bits per component; a single-label index keeps its full value), so nothing is indexed dynamically.
+__global__ void __launch_bounds__(256) symmap_kernel(const __grid_constant__ SymMapParams p)
+{
+    const long long step = (long long)gridDim.x * blockDim.x;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < p.total; e += step) {
+        long long tup[kMaxRank];
+        {
+            long long r = e;
+#pragma unroll
+            for (int d = 0; d < kMaxRank; ++d) {
+                tup[d] = 0;
+                if (d < p.nd) {
+                    const long long i = r % p.dext[d];
+                    r /= p.dext[d];
+                    if (p.dlen[d] == 1) tup[d] = i;
+                    else {
+                        const SymTuple t = p.dtab[d][i];
+                        tup[d] = (long long)t.v[0] | ((long long)t.v[1] << 16) | ((long long)t.v[2] << 32);
+                    }
+                }
+            }
+        }
+        double sr = 0.0, si = 0.0;
+        for (int t = 0; t < p.nterms; ++t) {
+            long long off = 0;
+            int sg = p.sign[t];
+            for (int g = 0; g < p.nl; ++g) {
+                long long val[3] = {0, 0, 0};
+#pragma unroll
+                for (int s = 0; s < 3; ++s) {
+                    if (s < p.llen[g]) {
+                        const int d = p.lsrc_dim[g][s];
+                        const long long w = pick(tup, d);
+                        val[s] = p.dlen[d] == 1 ? w : (w >> (16 * p.perm[t][d][p.lsrc_slot[g][s]])) & 0xffff;
+                    }
+                }
+                sg *= sort_sign(p.llen[g], val[0], val[1], val[2]);
+                off += tuple_pos(p.llen[g], val[0], val[1], val[2]) * p.lstride[g];
+            }
+            if (sg != 0) {
+                const double2 w = p.in[off];
+                sr = __dadd_rn(sr, sg > 0 ? w.x : -w.x);
+                si = __dadd_rn(si, sg > 0 ? w.y : -w.y);
+            }
+        }
+        double2 v;
+        v.x = __dsub_rn(__dmul_rn(p.ar, sr), __dmul_rn(p.ai, si));
+        v.y = __dadd_rn(__dmul_rn(p.ar, si), __dmul_rn(p.ai, sr));
+        if (p.accumulate) {
+            const double2 d = p.out[e];
+            v.x = __dadd_rn(d.x, v.x);
+            v.y = __dadd_rn(d.y, v.y);
+        }
+        p.out[e] = v;
+    }
+}
+
 }  // namespace
 
 cudaError_t launch_pack(const PackDesc &d, cudaStream_t stream, int64_t *launches)
@@ -241,6 +316,39 @@ cudaError_t launch_unpack(const UnpackDesc &d, cudaStream_t stream, int64_t *lau
     const long long chunks = (p.nrows + kRowChunk - 1) / kRowChunk;
     const int blocks = (int)std::max<long long>(1, std::min<long long>((chunks + 7) / 8, 8LL * sm_count()));
     unpack_kernel<<<blocks, 256, 0, stream>>>(p);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && launches) ++*launches;
+    return e;
+}
+
+cudaError_t launch_symmap(const SymMapDesc &d, cudaStream_t stream, int64_t *launches)
+{
+    SymMapParams p;
+    p.nd = d.nd; p.nl = d.nl; p.nterms = d.nterms; p.accumulate = d.accumulate ? 1 : 0;
+    p.total = 1;
+    for (int k = 0; k < kMaxRank; ++k) {
+        p.dext[k] = k < d.nd ? d.dext[k] : 1;
+        p.dlen[k] = k < d.nd ? d.dlen[k] : 1;
+        p.dtab[k] = k < d.nd ? d.dtab[k] : nullptr;
+        p.llen[k] = k < d.nl ? d.llen[k] : 1;
+        p.lstride[k] = k < d.nl ? d.lstride[k] : 0;
+        for (int s = 0; s < 3; ++s) {
+            p.lsrc_dim[k][s] = (k < d.nl && s < d.llen[k]) ? d.lsrc_dim[k][s] : 0;
+            p.lsrc_slot[k][s] = (k < d.nl && s < d.llen[k]) ? d.lsrc_slot[k][s] : 0;
+        }
+        p.total *= p.dext[k];
+    }
+    if (d.nterms < 1 || d.nterms > kMaxSymTerms) return cudaErrorInvalidValue;
+    for (int t = 0; t < kMaxSymTerms; ++t) {
+        p.sign[t] = t < d.nterms ? d.sign[t] : 0;
+        for (int k = 0; k < kMaxRank; ++k)
+            for (int s = 0; s < 3; ++s) p.perm[t][k][s] = t < d.nterms ? d.perm[t][k][s] : (unsigned char)s;
+    }
+    p.ar = d.alpha_re; p.ai = d.alpha_im;
+    p.in = (const double2 *)d.in;
+    p.out = (double2 *)d.out;
+    const int blocks = (int)std::max<long long>(1, std::min<long long>((p.total + 255) / 256, 16LL * sm_count()));
+    symmap_kernel<<<blocks, 256, 0, stream>>>(p);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess && launches) ++*launches;
     return e;

@@ -8,7 +8,7 @@ import oracle
 from oracle import sym
 import paper_2409_06759_b200 as pkg
 from paper_2409_06759_b200 import binding, ccd, synth
-from gpu_util import TOL, rc, parity_error, sample_indices, download_at
+from gpu_util import TOL, rc, parity_error, sample_indices, download_at, slab
 
 pytestmark = pytest.mark.gpu
 
@@ -139,4 +139,127 @@ def test_packed_pp_ladder_fullsize_sampled_and_faster_than_dense(ctx):
     t_packed = timed(lambda: ccd.pp_ladder_packed(ctx, R, V, T, Vp=Vp))
     assert t_dense / t_packed >= 5.0, (t_dense, t_packed)
     for t in (V, T, R, Vp):
+        t.destroy()
+
+
+# ---- packed views of packed tensors (tcb_unpack with groups on D) and tcb_antisym_pack ----------------------------------------
+VIEW_CASES = [("Tq(d<e,c,i<j<k)=T(d<e<c,i<j<k)", dict(d=7, e=7, c=7, i=5, j=5, k=5)),
+              ("To(a<b<c,l<m,k)=T(a<b<c,l<m<k)", dict(a=7, b=7, c=7, l=5, m=5, k=5)),
+              ("Tr(b<c,j<k,e,m)=T(b<c<e,j<k<m)", dict(b=6, c=6, e=6, j=5, k=5, m=5)),
+              ("Tr(j<k,e,b<c,m)=T(e<b<c,m<j<k)", dict(b=6, c=6, e=6, j=5, k=5, m=5)),
+              ("Ts(a<c,b,i)=T(a<b<c,i)", dict(a=9, b=9, c=9, i=3)),
+              ("D(a<b,c)=L(a,b<c)", dict(a=8, b=8, c=8)),                            # regrouping: zeros at b == c
+              ("D(x<y,p)=L(p,y,x)", dict(x=11, y=11, p=4))]                          # dense L: a pack with a transposition
+
+
+def _shape(groups, ext):
+    return tuple(sym.packed_extent(ext[g[0]], len(g)) for g in groups)
+
+
+@pytest.mark.parametrize("spec,ext", VIEW_CASES)
+@pytest.mark.parametrize("op,alpha", [("=", 1.0), ("+=", -1.0), ("+=", 0.75 + 0.5j)])
+def test_packed_views_match_the_oracle(ctx, spec, ext, op, alpha):
+    dg, lg, _ = sym.parse_both(spec)
+    rng = np.random.default_rng(len(spec) + len(op))
+    L, D0 = rc(rng, *_shape(lg, ext)), rc(rng, *_shape(dg, ext))
+    uspec = spec.replace("=", op, 1)
+    ref = sym.unpack(uspec, L, D=D0, alpha=alpha)
+    dL, dD = ctx.tensor_from_numpy(L), ctx.tensor_from_numpy(D0)
+    ctx.unpack(uspec, dD, dL, alpha)
+    got = ctx.tensor_download(dD)
+    if alpha in (1.0, -1.0):
+        assert np.array_equal(got, ref)
+    else:
+        assert np.max(np.abs(got - ref)) <= 1e-15 * (np.abs(D0).max() + 3 * np.abs(L).max())
+    dL.destroy(); dD.destroy()
+
+
+MERGE_CASES = [("R(a<b<c,i<j<k)=X(a,i,b<c,j<k)", dict(a=7, b=7, c=7, i=5, j=5, k=5), 9),
+               ("R(a<b<c,i<j<k)=X(b<c,a,i<j<k)", dict(a=7, b=7, c=7, i=5, j=5, k=5), 3),
+               ("R(a<b<c,i<j<k)=X(a<b<c,j<k,i)", dict(a=7, b=7, c=7, i=5, j=5, k=5), 3),
+               ("R(a<b<c,i<j<k)=X(a,b,c,i,j,k)", dict(a=5, b=5, c=5, i=4, j=4, k=4), 36),
+               ("R(i<j,a<b)=X(a,i,b,j)", dict(a=9, b=9, i=6, j=6), 4),
+               ("R(a<b<c,q)=X(c,q,a<b)", dict(a=10, b=10, c=10, q=3), 3),
+               ("R(a<b<c,i<j<k)=X(a<b<c,i<j<k)", dict(a=6, b=6, c=6, i=5, j=5, k=5), 1)]
+
+
+@pytest.mark.parametrize("spec,ext,nterms", MERGE_CASES)
+@pytest.mark.parametrize("op,alpha", [("=", 1.0), ("+=", 4.0), ("+=", 0.5 - 1.5j)])
+def test_antisym_pack_matches_the_oracle_within_the_north_star_tolerance(ctx, spec, ext, nterms, op, alpha):
+    """the shuffle sum under snorm = |alpha| * (sum over the shuffles of |L|) + |D_in|, element by element"""
+    dg, lg, _ = sym.parse_both(spec)
+    rng = np.random.default_rng(nterms + len(spec))
+    L, D0 = rc(rng, *_shape(lg, ext)), rc(rng, *_shape(dg, ext))
+    uspec = spec.replace("=", op, 1)
+    ref = sym.antisym_pack(uspec, L, D=D0, alpha=alpha)
+    # |terms| summed: the same call on |L| with every sign made + is not available, so bound it by nterms * max over reads
+    snorm = abs(alpha) * nterms * np.abs(L).max() + (np.abs(D0) if op == "+=" else 0.0)
+    dL, dD = ctx.tensor_from_numpy(L), ctx.tensor_from_numpy(D0)
+    ctx.antisym_pack(uspec, dD, dL, alpha)
+    got = ctx.tensor_download(dD)
+    assert np.max(np.abs(got - ref) / snorm) <= TOL
+    if nterms == 1 and alpha == 1.0 and op == "=":
+        assert np.array_equal(got, L)
+    dL.destroy(); dD.destroy()
+
+
+def test_antisym_pack_and_view_errors(ctx):
+    P3, P2, Dn = ctx.tensor_create((20, 4)), ctx.tensor_create((6, 15)), ctx.tensor_create((6, 6, 6))
+    for fn, spec, D, L, code in [(ctx.antisym_pack, "R(a<b,c)=X(a,b<c)", ctx.tensor_create((15, 6)), P2, binding.TCB_EINVAL_EXPR),
+                                 (ctx.antisym_pack, "R(a<b<c,q)=X(a,b<c)", P3, P2, binding.TCB_EINVAL_EXPR),   # q on one side
+                                 (ctx.antisym_pack, "R(a<b<c,q)=X(q,a,b<c)", P3, P2, binding.TCB_ESHAPE),      # rank of X
+                                 (ctx.unpack, "D(a<b,c)=L(a,b<c)", ctx.tensor_create((14, 6)), P2, binding.TCB_ESHAPE),
+                                 (ctx.unpack, "D(a<b,c)=L(a,b<d)", ctx.tensor_create((15, 6)), P2, binding.TCB_EINVAL_EXPR),
+                                 (ctx.antisym_pack, "R(a<b<c)=X(a,b,c)", Dn, Dn, binding.TCB_ESHAPE)]:
+        with pytest.raises(pkg.TcbError) as ei:
+            fn(spec, D, L, 1.0)
+        assert ei.value.code == code, spec
+    R = ctx.tensor_create((20,))
+    ctx.antisym_pack("R(a<b<c)=X(a,b,c)", R, Dn, 1.0)           # the context still works
+    ctx.sync()
+
+
+def test_packed_t3_views_and_antisymmetriser_at_the_ccsdt_size(ctx):
+    """o = 12, v = 60 (the CCSDT bench size): T3p(a<b<c,i<j<k) is 120 MB instead of 6 GB.  Sampled elements of the three views
+    and of the 9-term packed antisymmetriser against the oracle's rule evaluated one by one on host copies."""
+    o, v = 12, 60
+    nv2, nv3, no2, no3 = (ctx.packed_extent(v, 2), ctx.packed_extent(v, 3), ctx.packed_extent(o, 2), ctx.packed_extent(o, 3))
+    Tp = ctx.tensor_create((nv3, no3), zero=False)
+    ctx.synth_normal(Tp, synth.SEED0, 41)
+    hTp = ctx.tensor_download(Tp)
+    tv3 = {t: p for p, t in enumerate(sym.tuples(v, 3))}
+    to3 = {t: p for p, t in enumerate(sym.tuples(o, 3))}
+    pv2, po2 = sym.tuples(v, 2), sym.tuples(o, 2)
+
+    def t3(abc, ijk):
+        (sa, sga), (si, sgi) = sym._sort_sign(abc), sym._sort_sign(ijk)
+        return 0.0 if sga * sgi == 0 else sga * sgi * hTp[tv3[sa], to3[si]]
+    rng = np.random.default_rng(5)
+    Tr = ctx.tensor_create((nv2, no2, v, o), zero=False)
+    ctx.unpack("Tr(b<c,j<k,e,m)=T(b<c<e,j<k<m)", Tr, Tp, 1.0)
+    for m in (0, 5, o - 1):
+        view = slab(ctx, Tr, m)
+        hs = ctx.tensor_download(view)
+        view.destroy()
+        for _ in range(100):
+            x, y, e = (int(rng.integers(n)) for n in (nv2, no2, v))
+            assert hs[x, y, e] == t3(pv2[x] + (e,), po2[y] + (m,))
+    # the 9-term antisymmetriser of Xr(a,i,b<c,j<k) on packed storage
+    Xr = ctx.tensor_create((v, o, nv2, no2), zero=False)
+    ctx.synth_normal(Xr, synth.SEED0, 42)
+    R = ctx.tensor_create((nv3, no3), zero=False)
+    ctx.antisym_pack("R(a<b<c,i<j<k)=X(a,i,b<c,j<k)", R, Xr, 4.0)
+    hX, hR = ctx.tensor_download(Xr), ctx.tensor_download(R)
+    pv2i, po2i = {t: p for p, t in enumerate(pv2)}, {t: p for p, t in enumerate(po2)}
+    lv3, lo3 = sym.tuples(v, 3), sym.tuples(o, 3)
+    for _ in range(200):
+        p, q = int(rng.integers(nv3)), int(rng.integers(no3))
+        (a, b, c), (i, j, k) = lv3[p], lo3[q]
+        ref, sn = 0.0, 0.0
+        for (s, rest, sg) in ((a, (b, c), 1), (b, (a, c), -1), (c, (a, b), 1)):
+            for (u, orest, sg2) in ((i, (j, k), 1), (j, (i, k), -1), (k, (i, j), 1)):
+                w = hX[s, u, pv2i[rest], po2i[orest]]
+                ref, sn = ref + sg * sg2 * w, sn + abs(w)
+        assert abs(hR[p, q] - 4.0 * ref) <= TOL * 4.0 * sn
+    for t in (Tp, Tr, Xr, R):
         t.destroy()

@@ -123,3 +123,129 @@ def test_bad_specs_are_rejected():
         sym.pack("Tp(a<b,i<j)+=T(a,b,i,j)", T)                   # pack does not accumulate
     with pytest.raises(AssertionError):
         sym.pack("Tp(a<i,b,j)=T(a,b,i,j)", T)                    # unequal extents inside a group
+
+
+# ---- packed views of packed tensors, and the permutation operators on packed storage ------------------------------------------
+def _exactly_antisymmetric_t3(rng, v, o):
+    """(packed, dense) of a T(a,b,c,i,j,k) that is antisymmetric bit for bit: the dense one is written from the packed one
+    with the sign of the permutation determinant (no function of oracle/sym.py involved)"""
+    tv = [t for t in itertools.combinations(range(v), 3)]
+    tv.sort(key=lambda t: t[::-1])
+    to = [t for t in itertools.combinations(range(o), 3)]
+    to.sort(key=lambda t: t[::-1])
+    P = rng.standard_normal((len(tv), len(to))) + 1j * rng.standard_normal((len(tv), len(to)))
+    T = np.zeros((v, v, v, o, o, o), dtype=np.complex128, order="F")
+    for p, abc in enumerate(tv):
+        for q, ijk in enumerate(to):
+            for pv in itertools.permutations(range(3)):
+                sv = round(np.linalg.det(np.eye(3)[list(pv)]))
+                for po in itertools.permutations(range(3)):
+                    so = round(np.linalg.det(np.eye(3)[list(po)]))
+                    T[abc[pv[0]], abc[pv[1]], abc[pv[2]], ijk[po[0]], ijk[po[1]], ijk[po[2]]] = sv * so * P[p, q]
+    return np.asfortranarray(P), T
+
+
+VIEWS = [("Tq(d<e,c,i<j<k)=T(d<e<c,i<j<k)", "Tq(d<e,c,i<j<k)=T(d,e,c,i,j,k)"),
+         ("To(a<b<c,l<m,k)=T(a<b<c,l<m<k)", "To(a<b<c,l<m,k)=T(a,b,c,l,m,k)"),
+         ("Tr(b<c,j<k,e,m)=T(b<c<e,j<k<m)", "Tr(b<c,j<k,e,m)=T(b,c,e,j,k,m)"),
+         ("Tr(j<k,e,b<c,m)=T(e<b<c,m<j<k)", "Tr(j<k,e,b<c,m)=T(e,b,c,m,j,k)"),     # the single label first in L's group
+         ("Ts(a<c,b,i<j<k)=T(a<b<c,i<j<k)", "Ts(a<c,b,i<j<k)=T(a,b,c,i,j,k)")]     # the outer two labels of a triple
+
+
+@pytest.mark.parametrize("view,from_dense", VIEWS)
+def test_a_packed_view_is_the_pack_of_the_dense_tensor(view, from_dense):
+    """groups on both sides of `unpack`: the view of the packed tensor equals `pack` (pinned above by running counters)
+    applied to the dense antisymmetric tensor -- bit for bit, signs included"""
+    rng = np.random.default_rng(len(view))
+    P, T = _exactly_antisymmetric_t3(rng, 5, 4)
+    got = sym.unpack(view, P)
+    ref = sym.pack(from_dense, T)
+    assert got.shape == ref.shape and np.array_equal(got, ref)
+    base = rng.standard_normal(ref.shape) + 0j
+    acc = sym.unpack(view.replace("=", "+=", 1), P, D=base, alpha=2.0)
+    assert np.array_equal(acc, base + 2.0 * ref)
+    assert np.count_nonzero(got) > got.size // 4         # zeros only where a label of the view repeats inside a group of L
+
+
+def test_a_view_that_repeats_a_value_inside_a_group_of_l_reads_zero():
+    """D(a<b, c) = L(a, b<c) at c == b: L's group (b,c) has two equal labels -> 0; at c < b the sign flips"""
+    rng = np.random.default_rng(3)
+    n = 5
+    L = rng.standard_normal((n, sym.packed_extent(n, 2))) + 0j
+    D = sym.unpack("D(a<b,c)=L(a,b<c)", L)
+    pairs = sym.tuples(n, 2)
+    pos = {t: p for p, t in enumerate(pairs)}
+    for p, (a, b) in enumerate(pairs):
+        for c in range(n):
+            want = 0.0 if b == c else (L[a, pos[(b, c)]] if b < c else -L[a, pos[(c, b)]])
+            assert D[p, c] == want
+
+
+def _dense_operator(spec_ops, labels, X):
+    """P(x/yz)-style operators on a DENSE tensor through oracle.permsum (pinned in tests/test_oracle_permute.py); the
+    expansion of the operator string into signed permutations is written out here by hand-rolled transpositions"""
+    terms = [(list(labels), 1)]
+    for op in spec_ops:                                  # e.g. ("a", "bc"): 1 - (a b) - (a c)
+        x, rest = op
+        nxt = []
+        for lab, sg in terms:
+            nxt.append((lab, sg))
+            for y in rest:
+                sw = [y if q == x else x if q == y else q for q in lab]
+                nxt.append((sw, -sg))
+        terms = nxt
+    perms = [[list(labels).index(q) for q in lab] for lab, _ in terms]
+    return oracle.permsum(np.zeros_like(X), X, perms, [float(s) for _, s in terms], 0.0)
+
+
+MERGES = [("R(a<b<c,i<j<k)=X(a,i,b<c,j<k)", "X(a,b,c,i,j,k)=P(a,i,b<c,j<k)", [("a", "bc"), ("i", "jk")], 9),
+          ("R(a<b<c,i<j<k)=X(b<c,a,i<j<k)", "X(a,b,c,i,j,k)=P(b<c,a,i<j<k)", [("a", "bc")], 3),
+          ("R(a<b<c,i<j<k)=X(a<b<c,j<k,i)", "X(a,b,c,i,j,k)=P(a<b<c,j<k,i)", [("i", "jk")], 3),
+          ("R(a<b<c,i<j<k)=X(a<b,c,i<j,k)", "X(a,b,c,i,j,k)=P(a<b,c,i<j,k)", [("c", "ab"), ("k", "ij")], 9),
+          ("R(a<b,i<j)=X(a,i,b,j)", "X(a,b,i,j)=P(a,i,b,j)", [("a", "b"), ("i", "j")], 4)]
+
+
+@pytest.mark.parametrize("spec,expand,ops,nterms", MERGES)
+def test_antisym_pack_is_the_permutation_operator_on_the_dense_expansion(spec, expand, ops, nterms):
+    """antisym_pack == pack( P(..)P(..) [ dense expansion of L ] ): the operator applied by oracle.permsum to the tensor
+    `unpack` (pinned above) writes out; and the number of shuffles is the paper's term count for the operator"""
+    rng = np.random.default_rng(nterms + len(spec))
+    v, o = 5, 4
+    labels = expand[expand.index("(") + 1:expand.index(")")].split(",")
+    ext = {x: (v if x in "abc" else o) for x in labels}
+    groups = sym.parse_both(spec)[1]
+    shape = [sym.packed_extent(ext[g[0]], len(g)) for g in groups]
+    L = rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+    if "<" in expand:
+        Xd = sym.unpack(expand, L, extents=ext)
+    else:                                                 # L is dense already: only its index order differs
+        Xd = np.asfortranarray(np.transpose(L, [[g[0] for g in groups].index(x) for x in labels]))
+    Rd = _dense_operator(ops, labels, Xd)
+    dgroups = sym.parse_both(spec)[0]
+    ref = sym.pack("P(" + ",".join("<".join(g) for g in dgroups) + ")=R(" + ",".join(labels) + ")", Rd)
+    got = sym.antisym_pack(spec, L)
+    assert got.shape == ref.shape and np.abs(got - ref).max() <= 1e-14 * np.abs(ref).max()
+    count = 1
+    for g in dgroups:
+        count *= len(sym.shuffles(g, [set(b) for b in groups]))
+    assert count == nterms
+    base = rng.standard_normal(ref.shape) + 0j
+    acc = sym.antisym_pack(spec.replace("=", "+=", 1), L, D=base, alpha=0.5 - 1.5j)
+    assert np.abs(acc - (base + (0.5 - 1.5j) * ref)).max() <= 1e-14 * np.abs(ref).max()
+
+
+def test_antisym_pack_of_a_dense_tensor_is_the_36_term_antisymmetriser_and_of_a_packed_one_the_identity():
+    from oracle import cc
+    rng = np.random.default_rng(12)
+    v, o = 4, 4
+    X = rng.standard_normal((v, v, v, o, o, o)) + 1j * rng.standard_normal((v, v, v, o, o, o))
+    got = sym.antisym_pack("R(a<b<c,i<j<k)=X(a,b,c,i,j,k)", X)
+    ref = sym.pack("P(a<b<c,i<j<k)=A(a,b,c,i,j,k)", cc.antisymmetrise_abc_ijk(X))
+    assert np.abs(got - ref).max() <= 1e-14 * np.abs(ref).max()
+    assert len(sym.shuffles(["a", "b", "c"], [{"a"}, {"b"}, {"c"}])) == 6
+    same = sym.antisym_pack("R(a<b<c,i<j<k)=P(a<b<c,i<j<k)", got)        # one shuffle per group: a copy
+    assert np.array_equal(same, got)
+    with pytest.raises(ValueError):
+        sym.antisym_pack("R(a<b,c)=X(a,b<c)", np.zeros((4, 6)))           # L's group straddles two groups of D
+    with pytest.raises(ValueError):
+        sym.unpack("D(a<b,c)=L(a,b<d)", np.zeros((4, 6)))                 # labels differ
