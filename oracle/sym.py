@@ -214,9 +214,10 @@ def shuffles(group, blocks):
     return out
 
 
-def antisym_pack(spec, L, D=None, alpha=1.0, extents=None):
+def antisym_pack(spec, L, D=None, alpha=1.0, extents=None, magnitudes=False):
     """spec 'R(a<b<c,i<j<k)+=X(a,i,b<c,j<k)': D[tuples] (+)= alpha * sum over the shuffles of sign * L[at the label values];
-    the terms are summed with the FIRST group of D running fastest, then multiplied by alpha once."""
+    the terms are summed with the FIRST group of D running fastest, then multiplied by alpha once.
+    magnitudes=True (for the tests' normaliser): every term enters as |L[..]| with sign +."""
     dg, lg, acc = parse_both(spec)
     for g in lg:
         if not any(all(x in d for x in g) for d in dg):
@@ -244,6 +245,6 @@ def antisym_pack(spec, L, D=None, alpha=1.0, extents=None):
                     val[lab] = t[p][perm[slot]]
             w, s2 = _read(lg, where, val, L)
             if sign * s2 != 0:
-                total = total + w * (sign * s2)
+                total = total + (abs(w) if magnitudes else w * (sign * s2))
         D[pidx] = (D[pidx] if acc else 0.0) + a * total
     return D

@@ -618,11 +618,11 @@ def ccsdt_residual(ctx, o, h, g, T1, T2, T3, R1=None, R2=None, R3=None):
     return R1, R2, R3
 
 
-def ccsdt_residual_packed(ctx, o, h, g, T1, T2, T3, R1=None, R2=None, R3=None):
-    """`ccsdt_residual` with every contraction that touches T3 run on index-permutation-symmetric packed storage (SURVEY
-    8(f)-2 applied to 8(f)-3).  T2 and T3 must be antisymmetric within their virtual and within their
-    occupied indices (they are in `ccsdt_solve`: zero start + antisymmetric residuals).  The dense T3 is read by three
-    `tcb_pack` calls only:
+def ccsdt_residual_packed(ctx, o, h, g, T1, T2, T3p, R1=None, R2=None, R3p=None):
+    """`ccsdt_residual` on index-permutation-symmetric packed storage (SURVEY 8(f)-2 applied to 8(f)-3; PAPER.md:202, 440,
+    452): the triples amplitudes and the triples residual exist only as T3p, R3p(a<b<c, i<j<k) -- 1/36 of the dense tensor
+    (120 MB instead of 6 GB at o = 12, v = 60); no rank-6 dense tensor is ever formed.  T2 must be antisymmetric in (a,b) and
+    in (i,j) (it is in `ccsdt_solve`).  T3p is read by three packed views (`tcb_unpack` with groups on both sides),
         Tq(d<e, c, i<j<k)      To(a<b<c, l<m, k)      Tr(b<c, j<k, e, m) = T3(b,c,e,j,k,m)
     (T3(e,b,c,..) = T3(b,c,e,..): a cyclic relabelling has sign +), and the seven rank-6 contractions collapse onto three
     packed accumulators -- the full antisymmetriser A3 that follows does not care which of a, b, c (of i, j, k) a term calls
@@ -630,8 +630,9 @@ def ccsdt_residual_packed(ctx, o, h, g, T1, T2, T3, R1=None, R2=None, R3=None):
         Xq(a<b, c, i<j<k)  = 2 Wvvvv(a<b, d<e) Tq(d<e, c, ijk)          + Tq(a<b, e, ijk) Fv(c, e)
         Xo(a<b<c, i<j, k)  = 2 To(abc, l<m, k) Woooo(l<m, i<j)          + To(abc, i<j, m) Fo(m, k)
         Xr(a, i, b<c, j<k) = Wr(m,a,i,e) Tr(b<c, j<k, e, m) + Wvvov(b<c, i, d) T2(d, a, j<k) + Wovoo(l, a, j<k) T2(b<c, l, i)
-    against the dense program: 1/32 of the flops for the vvvv term, 1/4 for the ring term; X is written by three
-    `tcb_unpack` calls and antisymmetrised by ONE 9-term permute-sum.  Same arguments and results as `ccsdt_residual`; needs o >= 3 and v >= 3."""
+    against the dense program: 1/32 of the flops for the vvvv term, 1/4 for the ring term.  On an X antisymmetric in (b,c)
+    and (j,k) the 36-term A3 is 4 P(a/bc) P(i/jk), on Xq it is 12 P(c/ab), on Xo 12 P(k/ij): three `tcb_antisym_pack` calls
+    (9 + 3 + 3 signed reads per element of R3p).  Returns (R1, R2, R3p); needs o >= 3 and v >= 3."""
     v = T1.extents[0]
     if o < 3 or v < 3:
         raise ValueError("ccsdt_residual_packed needs o >= 3 and v >= 3 (a<b<c groups)")
@@ -645,9 +646,10 @@ def ccsdt_residual_packed(ctx, o, h, g, T1, T2, T3, R1=None, R2=None, R3=None):
         pack(spec, t, src)
         return t
     # ---- the three packed views of T3, the packed views of T2 and of the dressed integrals
-    Tq = packed((nv2, v, no3), "P(d<e,c,i<j<k)=T(d,e,c,i,j,k)", T3)
-    To = packed((nv3, no2, o), "P(a<b<c,l<m,k)=T(a,b,c,l,m,k)", T3)
-    Tr = packed((nv2, no2, v, o), "P(b<c,j<k,e,m)=T(b,c,e,j,k,m)", T3)
+    Tq, To, Tr = new((nv2, v, no3)), new((nv3, no2, o)), new((nv2, no2, v, o))
+    unpack("Tq(d<e,c,i<j<k)=T(d<e<c,i<j<k)", Tq, T3p, 1.0)
+    unpack("To(a<b<c,l<m,k)=T(a<b<c,l<m<k)", To, T3p, 1.0)
+    unpack("Tr(b<c,j<k,e,m)=T(b<c<e,j<k<m)", Tr, T3p, 1.0)
     T2p = packed((nv2, no2), "P(a<b,l<m)=T(a,b,l,m)", T2)
     T2x = packed((nv2, o, o), "P(b<c,l,i)=T(b,c,l,i)", T2)
     T2y = packed((v, v, no2), "P(d,a,j<k)=T(d,a,j,k)", T2)
@@ -729,33 +731,46 @@ def ccsdt_residual_packed(ctx, o, h, g, T1, T2, T3, R1=None, R2=None, R3=None):
     con("X(a,i,x,y)+=W(l,a,y)*T(x,l,i)", Xr, Wovoo, T2x, 1.0)
     for t in (Wovoo, Wvvov, Fo, Fv, Woooo, Wvvvv, Wr, Tq, To, Tr, T2x, T2y):
         t.destroy()
-    # Each accumulator is unpacked under the relabelling (cyclic: sign +) that makes it antisymmetric in (b,c) and in (j,k);
-    # on such an X the 36-term A3 is 4 P(a/bc) P(i/jk): one 9-term pass of the orbit kernel, no 4-term pass, no second 6 GB.
-    X = new((v, v, v, o, o, o))
-    unpack("X(a,b,c,i,j,k)=P(a,i,b<c,j<k)", X, Xr, 1.0)
-    unpack("X(a,b,c,i,j,k)+=P(b<c,a,i<j<k)", X, Xq, 1.0)
-    unpack("X(a,b,c,i,j,k)+=P(a<b<c,j<k,i)", X, Xo, 1.0)
+    if R3p is None:
+        R3p = new((nv3, no3))
+    ctx.antisym_pack("R(a<b<c,i<j<k)=X(a,i,b<c,j<k)", R3p, Xr, 4.0)
+    ctx.antisym_pack("R(a<b<c,i<j<k)+=X(a<b,c,i<j<k)", R3p, Xq, 12.0)
+    ctx.antisym_pack("R(a<b<c,i<j<k)+=X(a<b<c,i<j,k)", R3p, Xo, 12.0)
     for t in (Xq, Xo, Xr):
         t.destroy()
-    if R3 is None:
-        R3 = new((v, v, v, o, o, o))
-    ctx.antisymmetrize("P(a/bc)P(i/jk):R(a,b,c,i,j,k)=X(a,b,c,i,j,k)", R3, X, 4.0)
-    X.destroy()
-    return R1, R2, R3
+    return R1, R2, R3p
+
+
+def _tuple_sums(e, k):
+    """sum of e over the strictly increasing k-tuples of range(len(e)), first label fastest (the packed order)"""
+    n = len(e)
+    if k == 2:
+        return [e[a] + e[b] for b in range(n) for a in range(b)]
+    return [e[a] + e[b] + e[c] for c in range(n) for b in range(c) for a in range(b)]
 
 
 def ccsdt_solve(ctx, o, h, g, f_diag, iterations, packed=False):
     """Jacobi iterations of the CCSDT amplitude equations from zero amplitudes (oracle: cc.ccsdt_jacobi): per iteration
-    `ccsdt_residual` (`ccsdt_residual_packed` with packed=True), the residual norm |R|, the energy of the amplitudes the evaluation saw, and three
+    `ccsdt_residual`, the residual norm |R|, the energy of the amplitudes the evaluation saw, and three
     `tcb_denominator_update`.  f_diag: the n orbital energies (diagonal of the Fock matrix).
+    packed=True: `ccsdt_residual_packed`; T3 and R3 live as (a<b<c, i<j<k) packed tensors (their denominators are the sums
+    of the orbital energies over the tuples, |R3|^2 = 36 |R3p|^2) and T3 comes back packed.
     Returns (T1, T2, T3, [E_corr per evaluation], [|R| per evaluation])."""
+    import math
     import numpy as np
     n = g.extents[0]
     v = n - o
     e = np.asarray(f_diag, dtype=np.float64)
     eo, ev = e[:o], -e[o:]
-    T1, T2, T3 = ctx.tensor_create((v, o)), ctx.tensor_create((v, v, o, o)), ctx.tensor_create((v, v, v, o, o, o))
-    R1, R2, R3 = ctx.tensor_create((v, o)), ctx.tensor_create((v, v, o, o)), ctx.tensor_create((v, v, v, o, o, o), zero=False)
+    if packed:
+        shape3 = (ctx.packed_extent(v, 3), ctx.packed_extent(o, 3))
+        eps3 = [np.asarray(_tuple_sums(ev, 3)), np.asarray(_tuple_sums(eo, 3))]
+    else:
+        shape3 = (v, v, v, o, o, o)
+        eps3 = [ev, ev, ev, eo, eo, eo]
+    residual = ccsdt_residual_packed if packed else ccsdt_residual
+    T1, T2, T3 = ctx.tensor_create((v, o)), ctx.tensor_create((v, v, o, o)), ctx.tensor_create(shape3)
+    R1, R2, R3 = ctx.tensor_create((v, o)), ctx.tensor_create((v, v, o, o)), ctx.tensor_create(shape3, zero=False)
     # bare blocks for the energy: E = f_ia t_i^a + 1/4 <ij||ab> t_ij^ab + 1/2 <ij||ab> t_i^a t_j^b
     Bz = t1_dressed_blocks(ctx, o, h, g, T1, ("fov", "oovv"))          # T1 = 0 here: the bare blocks
     energies, norms = [], []
@@ -766,14 +781,17 @@ def ccsdt_solve(ctx, o, h, g, f_diag, iterations, packed=False):
         ctx.contract("E()+=W(i,j,a,b)*T(a,b,i,j)", E, Bz["oovv"], T2, 0.25)
         ctx.contract("Y(i,a)=W(i,j,a,b)*T(b,j)", Y, Bz["oovv"], T1, 1.0)
         ctx.contract("E()+=Y(i,a)*T(a,i)", E, Y, T1, 0.5)
-        (ccsdt_residual_packed if packed else ccsdt_residual)(ctx, o, h, g, T1, T2, T3, R1, R2, R3)
+        residual(ctx, o, h, g, T1, T2, T3, R1, R2, R3)
         energies.append(complex(ctx.tensor_download(E)))
-        norms.append(residual_norm(ctx, R1, R2, R3))
+        if packed:
+            norms.append(math.sqrt(residual_norm(ctx, R1, R2) ** 2 + 36.0 * residual_norm(ctx, R3) ** 2))
+        else:
+            norms.append(residual_norm(ctx, R1, R2, R3))
         E.destroy()
         Y.destroy()
         ctx.denominator_update(T1, R1, [ev, eo], 1.0)
         ctx.denominator_update(T2, R2, [ev, ev, eo, eo], 1.0)
-        ctx.denominator_update(T3, R3, [ev, ev, ev, eo, eo, eo], 1.0)
+        ctx.denominator_update(T3, R3, eps3, 1.0)
     for t in list(Bz.values()) + [R1, R2, R3]:
         t.destroy()
     return T1, T2, T3, energies, norms

@@ -234,3 +234,11 @@ class ShadowContext:
         ref = sym.unpack(spec, L.host, D.host, alpha)
         sn = abs(alpha) * np.abs(sym.unpack(spec.replace("+=", "=", 1), L.norm, np.zeros_like(D.host), 1.0))
         self._compare(spec, D, ref, sn + (D.norm if acc else 0.0))
+
+    def antisym_pack(self, spec, D, L, alpha=1.0):
+        from oracle import sym
+        self.ctx.antisym_pack(spec, D.gpu, L.gpu, alpha)
+        acc = "+=" in spec
+        ref = sym.antisym_pack(spec, L.host, D.host, alpha)
+        sn = abs(alpha) * sym.antisym_pack(spec.replace("+=", "=", 1), L.norm, np.zeros_like(D.host), 1.0, magnitudes=True).real
+        self._compare(spec, D, ref, sn + (D.norm if acc else 0.0))

@@ -60,3 +60,7 @@ class OracleContext:
     def unpack(self, spec, D, L, alpha=1.0):
         D.host = sym.unpack(spec, L.host, D.host, alpha)
         self.calls += 1
+
+    def antisym_pack(self, spec, D, L, alpha=1.0):
+        D.host = sym.antisym_pack(spec, L.host, D.host, alpha)
+        self.calls += 1

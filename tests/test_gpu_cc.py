@@ -417,24 +417,28 @@ def test_ccsdt_residual_call_by_call_and_against_the_fock_space_pinned_equations
 
 @pytest.mark.parametrize("o,v", [(3, 4), (4, 6), (5, 5)])
 def test_packed_ccsdt_residual_call_by_call_and_against_the_fock_space_pinned_equations(ctx, o, v):
-    """SURVEY 8(f)-2 applied to 8(f)-3: ccd.ccsdt_residual_packed -- every contraction with T3 on a<b / a<b<c packed storage --
-    call by call against the oracle (tcb_pack bit-exact, tcb_unpack and the contractions under their carried snorm), the
-    residuals against the unfactorised equations, and against the dense driver."""
+    """SURVEY 8(f)-2 applied to 8(f)-3: ccd.ccsdt_residual_packed -- T3 and R3 only as (a<b<c, i<j<k) packed tensors, every
+    contraction with T3 on packed views -- call by call against the oracle (tcb_pack bit-exact; packed views, contractions
+    and tcb_antisym_pack under their carried snorm), the residuals against the unfactorised equations, and against the dense
+    driver."""
     from gpu_util import ShadowContext
+    from oracle import sym
     f, g, h, t1, t2, t3 = _ccsdt_inputs(o, v, 100 * o + v)
+    t3p = sym.pack("P(a<b<c,i<j<k)=T(a,b,c,i,j,k)", t3)
     sh = ShadowContext(ctx)
-    R1, R2, R3 = ccd.ccsdt_residual_packed(sh, o, sh.wrap(h), sh.wrap(g), sh.wrap(t1), sh.wrap(t2), sh.wrap(t3))
-    assert sh.calls == 112 and sh.worst <= 1e-11
+    R1, R2, R3p = ccd.ccsdt_residual_packed(sh, o, sh.wrap(h), sh.wrap(g), sh.wrap(t1), sh.wrap(t2), sh.wrap(t3p))
+    assert sh.calls == 111 and sh.worst <= 1e-11
     e, r1, r2, r3 = cc.ccsdt_residual_unfactorised(o, f, g, t1, t2, t3)
     W = ctx.tensor_from_numpy
     D1, D2, D3 = ccd.ccsdt_residual(ctx, o, W(h), W(g), W(t1), W(t2), W(t3))
-    for got, ref, dense in ((R1, r1, D1), (R2, r2, D2), (R3, r3, D3)):
-        dev = ctx.tensor_download(got.gpu)
-        scale = np.abs(got.norm).max()
+    R3 = ctx.tensor_create((v, v, v, o, o, o), zero=False)
+    ctx.unpack("R(a,b,c,i,j,k)=P(a<b<c,i<j<k)", R3, R3p.gpu, 1.0)
+    scale3 = np.abs(R3p.norm).max()
+    for got, scale, ref, dense in ((R1.gpu, np.abs(R1.norm).max(), r1, D1), (R2.gpu, np.abs(R2.norm).max(), r2, D2), (R3, scale3, r3, D3)):
+        dev = ctx.tensor_download(got)
         assert np.abs(dev - ref).max() <= 1e-11 * scale
         assert np.abs(dev - ctx.tensor_download(dense)).max() <= 1e-11 * scale
-    gR3 = ctx.tensor_download(R3.gpu)
-    assert np.abs(gR3 + gR3.transpose(0, 1, 2, 4, 3, 5)).max() <= 1e-12 * np.abs(R3.norm).max()
+    assert np.abs(R3p.host - sym.pack("P(a<b<c,i<j<k)=R(a,b,c,i,j,k)", r3)).max() <= 1e-12 * scale3
 
 
 @pytest.mark.parametrize("packed", [False, True])
@@ -456,6 +460,9 @@ def test_ccsdt_iterations_follow_the_oracle_and_converge(ctx, packed):
     dh, dg = ctx.tensor_from_numpy(h), ctx.tensor_from_numpy(g)
     T1, T2, T3, energies, norms = ccd.ccsdt_solve(ctx, o, dh, dg, e, its, packed=packed)
     r1, r2, r3, e_ref, n_ref = cc.ccsdt_jacobi(o, f, g, its)
+    if packed:
+        T3p, T3 = T3, ctx.tensor_create((v, v, v, o, o, o), zero=False)
+        ctx.unpack("T(a,b,c,i,j,k)=P(a<b<c,i<j<k)", T3, T3p, 1.0)
     for got, ref in ((T1, r1), (T2, r2), (T3, r3)):
         assert np.abs(ctx.tensor_download(got) - ref).max() <= 1e-10 * max(np.abs(ref).max(), 1e-300)
     for k in range(its):

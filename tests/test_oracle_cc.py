@@ -388,22 +388,25 @@ def test_ccsdt_driver_call_list_is_the_unfactorised_equations():
 
 @pytest.mark.parametrize("o,v", [(3, 3), (3, 4), (4, 4)])
 def test_packed_ccsdt_driver_call_list_is_the_unfactorised_equations(o, v):
-    """ccd.ccsdt_residual_packed (every T3 contraction on a<b / a<b<c packed storage: three packed views of T3, three packed
-    accumulators, three unpacks) run on the host with the oracle's contract / add / permsum / sym.pack / sym.unpack: equals
-    the unfactorised 37-term evaluation, and the dense driver."""
+    """ccd.ccsdt_residual_packed (T3 and R3 exist only packed, (a<b<c, i<j<k); three packed views of T3, three packed
+    accumulators, three packed permutation operators) run on the host with the oracle's contract / add / permsum / sym.*:
+    R3p unpacked equals the unfactorised 37-term evaluation."""
+    from oracle import sym
     from oracle_ctx import OracleContext
     from paper_2409_06759_b200 import ccd
     f, g, t1, t2, t3 = _ccsdt_problem(o, v, 78 + o + v)
     h = f - np.einsum("piqi->pq", g[:, :o, :, :o])
     oc = OracleContext()
     W = oc.tensor_from_numpy
-    R1, R2, R3 = ccd.ccsdt_residual_packed(oc, o, W(h), W(g), W(t1), W(t2), W(t3))
+    t3p = sym.pack("P(a<b<c,i<j<k)=T(a,b,c,i,j,k)", t3)
+    R1, R2, R3p = ccd.ccsdt_residual_packed(oc, o, W(h), W(g), W(t1), W(t2), W(t3p))
     e, r1, r2, r3 = cc.ccsdt_residual_unfactorised(o, f, g, t1, t2, t3)
-    for got, ref in ((R1.host, r1), (R2.host, r2), (R3.host, r3)):
+    R3 = sym.unpack("R(a,b,c,i,j,k)=P(a<b<c,i<j<k)", R3p.host, extents=dict(a=v, b=v, c=v, i=o, j=o, k=o))
+    for got, ref in ((R1.host, r1), (R2.host, r2), (R3, r3)):
         assert np.abs(got - ref).max() <= 1e-12 * np.abs(ref).max()
-    assert oc.calls == 112
+    assert oc.calls == 111
     with pytest.raises(ValueError):
-        ccd.ccsdt_residual_packed(oc, 2, W(h), W(g), W(t1[:, :2]), W(t2), W(t3))
+        ccd.ccsdt_residual_packed(oc, 2, W(h), W(g), W(t1[:, :2]), W(t2), W(t3p))
 
 
 def test_converged_ccsdt_iteration_zeroes_all_three_fock_space_projections():
