@@ -722,9 +722,46 @@ def run_extras(ctx):
                     "ms": b, "ms_median": float(np.median(ts)), "contractions": CountingT.calls, "launches": launches,
                     "tflops": CountingT.flops / b * 1e-9,
                     "frac_fp64_tensor_peak": CountingT.flops / b * 1e-9 / FP64_TENSOR_PEAK_TFLOPS})
+        dense_ms = b
         for t in (hh, gg, T1, T2, T3) + tuple(Rs):
             t.destroy()
         ctx.sync()
+        # the same residual on packed storage (8(f)-2 applied to 8(f)-3): T3, R3 only as (a<b<c, i<j<k); then a size whose
+        # dense T3 (65.5 GB per tensor, four of them live) does not fit one GPU at all
+        for (o, v) in ((12, 60), (16, 100)):
+            n = o + v
+            hh, gg = ctx.tensor_create((n, n), zero=False), ctx.tensor_create((n, n, n, n), zero=False)
+            ctx.synth_normal(hh, 20240913, 1, sigma=0.05)
+            ctx.synth_normal(gg, 20240913, 2, antisym=((0, 1), (2, 3)), sigma=0.02)
+            T1, T2 = ctx.tensor_create((v, o), zero=False), ctx.tensor_create((v, v, o, o), zero=False)
+            T3p = ctx.tensor_create((ctx.packed_extent(v, 3), ctx.packed_extent(o, 3)), zero=False)
+            ctx.synth_normal(T1, 20240913, 3, sigma=0.05)
+            ctx.synth_normal(T2, 20240913, 4, antisym=((0, 1), (2, 3)), sigma=0.05)
+            ctx.synth_normal(T3p, 20240913, 5, sigma=0.01)
+            CountingT.flops, CountingT.calls = 0.0, 0
+            Rs = ccd.ccsdt_residual_packed(CountingT(), o, hh, gg, T1, T2, T3p)
+            ctx.sync()
+            ts = []
+            for _ in range(3):
+                l0 = ctx.launch_count()
+                ctx.timer_start()
+                ccd.ccsdt_residual_packed(ctx, o, hh, gg, T1, T2, T3p, *Rs)
+                ts.append(ctx.timer_stop())
+                launches = ctx.launch_count() - l0
+            b = min(ts)
+            row = {"workload": f"next rows 8(f)-2 + 8(f)-3: CCSDT residual on packed storage o={o} v={v}: T3 and R3 only as "
+                               f"(a<b<c, i<j<k) tensors of {T3p.nbytes / 1e6:.0f} MB (dense: {16e-9 * v ** 3 * o ** 3:.1f} GB each), "
+                               "three packed views of T3, three packed accumulators, tcb_antisym_pack",
+                   "ms": b, "ms_median": float(np.median(ts)), "contractions": CountingT.calls, "launches": launches,
+                   "tflops_executed": CountingT.flops / b * 1e-9,
+                   "frac_fp64_tensor_peak": CountingT.flops / b * 1e-9 / FP64_TENSOR_PEAK_TFLOPS}
+            if (o, v) == (12, 60):
+                row["dense_program_ms"] = dense_ms
+                row["speedup_over_dense_program"] = dense_ms / b
+            out.append(row)
+            for t in (hh, gg, T1, T2, T3p) + tuple(Rs):
+                t.destroy()
+            ctx.sync()
     except Exception as e:          # noqa: BLE001
         out.append({"workload": "CCSDT residual", "error": str(e)})
     try:    # configs[4] transposition samples (the whole sweep: python -m paper_2409_06759_b200.transpose_bench)

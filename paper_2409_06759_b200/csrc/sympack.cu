@@ -205,10 +205,103 @@ struct SymMapParams {
     unsigned char perm[kMaxSymTerms][kMaxRank][3];
     signed char sign[kMaxSymTerms];
     long long total;
+    int touch0[kMaxRank];                   // L group g holds a label of D's index 0
+    long long nrows;                        // total / dext[0]
     double ar, ai;
     const double2 *in;
     double2 *out;
 };
+
+__device__ __forceinline__ long long tuple_word(const SymMapParams &p, int d, long long i)
+{
+    if (p.dlen[d] == 1) return i;
+    const SymTuple t = p.dtab[d][i];
+    return (long long)t.v[0] | ((long long)t.v[1] << 16) | ((long long)t.v[2] << 32);
+}
+
+constexpr int kViewU = 4;                   // elements of D's index 0 per thread and tile
+
+// One signed read per element (tcb_unpack onto a packed D).  A tile = 256 * kViewU consecutive values of D's index 0 at
+// fixed other indices: the 64-bit decode of those, and the L groups fed by them alone, are done once per tile; per element
+// only the groups holding a label of index 0 are sorted.  (The one-thread-per-element kernel below spent its time in 64-bit
+// divisions: 21 ms for a 15 GB view.)
+__global__ void __launch_bounds__(256) symview_kernel(const __grid_constant__ SymMapParams p)
+{
+    const long long e0 = p.dext[0];
+    const long long tiles_per_row = (e0 + 256 * kViewU - 1) / (256 * kViewU);
+    const long long ntiles = p.nrows * tiles_per_row;
+    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const long long row = tile / tiles_per_row, chunk = tile - row * tiles_per_row;
+        long long tup[kMaxRank];
+        {
+            long long r = row;
+            tup[0] = 0;
+#pragma unroll
+            for (int d = 1; d < kMaxRank; ++d) {
+                tup[d] = 0;
+                if (d < p.nd) {
+                    const long long i = r % p.dext[d];
+                    r /= p.dext[d];
+                    tup[d] = tuple_word(p, d, i);
+                }
+            }
+        }
+        long long off_row = 0;
+        int sign_row = 1;
+        for (int g = 0; g < p.nl; ++g) {
+            if (p.touch0[g]) continue;
+            long long val[3] = {0, 0, 0};
+#pragma unroll
+            for (int s = 0; s < 3; ++s) {
+                if (s < p.llen[g]) {
+                    const int d = p.lsrc_dim[g][s];
+                    const long long w = pick(tup, d);
+                    val[s] = p.dlen[d] == 1 ? w : (w >> (16 * p.lsrc_slot[g][s])) & 0xffff;
+                }
+            }
+            sign_row *= sort_sign(p.llen[g], val[0], val[1], val[2]);
+            off_row += tuple_pos(p.llen[g], val[0], val[1], val[2]) * p.lstride[g];
+        }
+        double2 *dst = p.out + row * e0;
+#pragma unroll
+        for (int u = 0; u < kViewU; ++u) {
+            const long long i0 = (chunk * kViewU + u) * 256 + threadIdx.x;
+            if (i0 >= e0) break;
+            int sg = sign_row;
+            double2 v = make_double2(0.0, 0.0);
+            if (sg != 0) {
+                tup[0] = tuple_word(p, 0, i0);
+                long long off = off_row;
+                for (int g = 0; g < p.nl; ++g) {
+                    if (!p.touch0[g]) continue;
+                    long long val[3] = {0, 0, 0};
+#pragma unroll
+                    for (int s = 0; s < 3; ++s) {
+                        if (s < p.llen[g]) {
+                            const int d = p.lsrc_dim[g][s];
+                            const long long w = pick(tup, d);
+                            val[s] = p.dlen[d] == 1 ? w : (w >> (16 * p.lsrc_slot[g][s])) & 0xffff;
+                        }
+                    }
+                    sg *= sort_sign(p.llen[g], val[0], val[1], val[2]);
+                    off += tuple_pos(p.llen[g], val[0], val[1], val[2]) * p.lstride[g];
+                }
+                if (sg != 0) {
+                    const double2 w = p.in[off];
+                    const double wr = sg > 0 ? w.x : -w.x, wi = sg > 0 ? w.y : -w.y;
+                    v.x = __dsub_rn(__dmul_rn(p.ar, wr), __dmul_rn(p.ai, wi));
+                    v.y = __dadd_rn(__dmul_rn(p.ar, wi), __dmul_rn(p.ai, wr));
+                }
+            }
+            if (p.accumulate) {
+                const double2 d = dst[i0];
+                v.x = __dadd_rn(d.x, v.x);
+                v.y = __dadd_rn(d.y, v.y);
+            }
+            dst[i0] = v;
+        }
+    }
+}
 
 // One thread per element of D (D is the small, packed side or a packed view of it).  The tuple of every D index sits in one
 // 64-bit register (16 bits per component; a single-label index keeps its full value), so nothing is indexed dynamically.
@@ -347,6 +440,24 @@ cudaError_t launch_symmap(const SymMapDesc &d, cudaStream_t stream, int64_t *lau
     p.ar = d.alpha_re; p.ai = d.alpha_im;
     p.in = (const double2 *)d.in;
     p.out = (double2 *)d.out;
+    for (int g = 0; g < kMaxRank; ++g) {
+        p.touch0[g] = 0;
+        for (int s2 = 0; s2 < 3; ++s2)
+            if (g < d.nl && s2 < d.llen[g] && d.lsrc_dim[g][s2] == 0) p.touch0[g] = 1;
+    }
+    p.nrows = p.total / p.dext[0];
+    if (d.nterms == 1 && d.sign[0] == 1) {
+        bool identity = true;
+        for (int k = 0; k < kMaxRank; ++k) for (int s2 = 0; s2 < 3; ++s2) identity = identity && d.perm[0][k][s2] == s2;
+        if (identity) {
+            const long long tiles = p.nrows * ((p.dext[0] + 256 * kViewU - 1) / (256 * kViewU));
+            const int vb = (int)std::max<long long>(1, std::min<long long>(tiles, 16LL * sm_count()));
+            symview_kernel<<<vb, 256, 0, stream>>>(p);
+            cudaError_t ve = cudaGetLastError();
+            if (ve == cudaSuccess && launches) ++*launches;
+            return ve;
+        }
+    }
     const int blocks = (int)std::max<long long>(1, std::min<long long>((p.total + 255) / 256, 16LL * sm_count()));
     symmap_kernel<<<blocks, 256, 0, stream>>>(p);
     cudaError_t e = cudaGetLastError();
