@@ -274,6 +274,56 @@ def triples_correction(ctx, W, U, T2, e_occ, e_virt, keep=False, T1=None, oovv=N
     return out[0] if T1 is None else tuple(out)
 
 
+def triples_correction_packed(ctx, W, U, T2, e_occ, e_virt, keep=False, T1=None, oovv=None):
+    """`triples_correction` on index-permutation-symmetric packed storage: R3 and t3
+    exist only on a<b<c, i<j<k.  W(b,c,d,k) is antisymmetric in (b,c), U(l,c,j,k) in (j,k), T2 in (a,b) and (i,j), so
+        X1(a, i<j, b<c, k) = sum_d T2(a,d,i<j) W(b<c,d,k)        X2(a<b, i, c, j<k) = sum_l T2(a<b,i,l) U(l,c,j<k)
+    are 1/4 of the dense contractions, and the two 9-term operators P(a/bc)P(k/ij), P(c/ab)P(i/jk) are `tcb_antisym_pack`
+    calls straight into R3p(a<b<c, i<j<k):  E[T] = <t3p|R3p> (each unordered triple pair once: the factor 1/36 is gone).
+    Singles term: Y(a,i) = 4 sum_{b<c, j<k} t3(b<c, a | j<k, i) <j<k||b<c> on a packed view of t3p, E_ST = 1/4 <t1|Y>.
+    Returns as `triples_correction`; with keep=True R3p and t3p (packed).  Needs o >= 3 and v >= 3."""
+    import numpy as np
+    v, _, o, _ = T2.extents
+    if o < 3 or v < 3:
+        raise ValueError("triples_correction_packed needs o >= 3 and v >= 3 (a<b<c groups)")
+    nv2, nv3, no2, no3 = (ctx.packed_extent(v, 2), ctx.packed_extent(v, 3), ctx.packed_extent(o, 2), ctx.packed_extent(o, 3))
+    new = lambda shape: ctx.tensor_create(shape, zero=False)
+    T2y, Wp, T2z, Up = new((v, v, no2)), new((nv2, v, o)), new((nv2, o, o)), new((o, v, no2))
+    ctx.pack("P(a,d,i<j)=T(a,d,i,j)", T2y, T2)
+    ctx.pack("P(b<c,d,k)=W(b,c,d,k)", Wp, W)
+    ctx.pack("P(a<b,i,l)=T(a,b,i,l)", T2z, T2)
+    ctx.pack("P(l,c,j<k)=U(l,c,j,k)", Up, U)
+    X1, X2 = new((v, no2, nv2, o)), new((nv2, o, v, no2))
+    ctx.contract("X(a,y,x,k)=T(a,d,y)*W(x,d,k)", X1, T2y, Wp, 1.0)
+    ctx.contract("X(x,i,c,y)=T(x,i,l)*U(l,c,y)", X2, T2z, Up, 1.0)
+    R3p = new((nv3, no3))
+    ctx.antisym_pack("R(a<b<c,i<j<k)=X(a,i<j,b<c,k)", R3p, X1, 1.0)
+    ctx.antisym_pack("R(a<b<c,i<j<k)+=X(a<b,i,c,j<k)", R3p, X2, -1.0)
+    for t in (T2y, Wp, T2z, Up, X1, X2):
+        t.destroy()
+    ev, eo = -np.asarray(e_virt, dtype=np.float64), np.asarray(e_occ, dtype=np.float64)
+    t3p = new((nv3, no3))
+    ctx.denominator_divide(t3p, R3p, [np.asarray(_tuple_sums(ev, 3)), np.asarray(_tuple_sums(eo, 3))], 1.0)
+    E = ctx.tensor_create(())
+    ctx.dot(E, t3p, R3p, True, 1.0)
+    out = [E]
+    if T1 is not None:
+        V, gp = new((nv2, no2, v, o)), new((no2, nv2))
+        ctx.unpack("V(b<c,j<k,a,i)=T(b<c<a,j<k<i)", V, t3p, 1.0)
+        ctx.pack("P(j<k,b<c)=g(j,k,b,c)", gp, oovv)
+        Y, Est = ctx.tensor_create((v, o)), ctx.tensor_create(())
+        ctx.contract("Y(a,i)=T(x,y,a,i)*W(y,x)", Y, V, gp, 4.0)
+        ctx.dot(Est, T1, Y, True, 0.25)
+        for t in (V, gp, Y):
+            t.destroy()
+        out.append(Est)
+    if keep:
+        return tuple(out) + (R3p, t3p)
+    R3p.destroy()
+    t3p.destroy()
+    return out[0] if T1 is None else tuple(out)
+
+
 def ccd_solve_diis(ctx, B, e_occ, e_virt, iterations, depth=6):
     """The CCD iteration with DIIS extrapolation (Pulay): error vector e_k = R(T_k) / D, trial vector T_k + e_k, next T =
     the combination of the last `depth` trial vectors minimising |sum c_i e_i|.  Tensors, inner products (`tcb_dot`,
@@ -741,12 +791,32 @@ def ccsdt_residual_packed(ctx, o, h, g, T1, T2, T3p, R1=None, R2=None, R3p=None)
     return R1, R2, R3p
 
 
+_TUPLES = {}
+
+
+def _tuple_members(n, k):
+    """index arrays (a, b[, c]) of the strictly increasing k-tuples of range(n), first label fastest (the packed order);
+    the pairs with b < c are the first c(c-1)/2 pairs, so the triples are prefixes of the pair list, one per c"""
+    import numpy as np
+    if (n, k) not in _TUPLES:
+        b = np.repeat(np.arange(n), np.arange(n))
+        a = np.concatenate([np.arange(x) for x in range(n)]) if n else np.zeros(0, dtype=np.int64)
+        if k == 2:
+            _TUPLES[(n, k)] = (a, b)
+        else:
+            cnt = [c * (c - 1) // 2 for c in range(n)]
+            _TUPLES[(n, k)] = (np.concatenate([a[:m] for m in cnt]), np.concatenate([b[:m] for m in cnt]),
+                               np.repeat(np.arange(n), cnt))
+    return _TUPLES[(n, k)]
+
+
 def _tuple_sums(e, k):
-    """sum of e over the strictly increasing k-tuples of range(len(e)), first label fastest (the packed order)"""
-    n = len(e)
-    if k == 2:
-        return [e[a] + e[b] for b in range(n) for a in range(b)]
-    return [e[a] + e[b] + e[c] for c in range(n) for b in range(c) for a in range(b)]
+    """sum of e over the strictly increasing k-tuples of range(len(e)), in the packed order, members added first to last"""
+    import numpy as np
+    e = np.asarray(e, dtype=np.float64)
+    m = _tuple_members(len(e), k)
+    out = e[m[0]] + e[m[1]]
+    return out if k == 2 else out + e[m[2]]
 
 
 def ccsdt_solve(ctx, o, h, g, f_diag, iterations, packed=False):

@@ -207,6 +207,7 @@ struct SymMapParams {
     long long total;
     int touch0[kMaxRank];                   // L group g holds a label of D's index 0
     long long nrows;                        // total / dext[0]
+    long long rowdiv[kMaxRank];             // product of dext[1 .. d-1]: row / rowdiv[d] % dext[d] = index d of the row
     double ar, ai;
     const double2 *in;
     double2 *out;
@@ -219,80 +220,120 @@ __device__ __forceinline__ long long tuple_word(const SymMapParams &p, int d, lo
     return (long long)t.v[0] | ((long long)t.v[1] << 16) | ((long long)t.v[2] << 32);
 }
 
-constexpr int kViewU = 4;                   // elements of D's index 0 per thread and tile
+constexpr int kTileU = 8;                   // elements of D's index 0 per thread and tile
 
-// One signed read per element (tcb_unpack onto a packed D).  A tile = 256 * kViewU consecutive values of D's index 0 at
-// fixed other indices: the 64-bit decode of those, and the L groups fed by them alone, are done once per tile; per element
-// only the groups holding a label of index 0 are sorted.  (The one-thread-per-element kernel below spent its time in 64-bit
-// divisions: 21 ms for a 15 GB view.)
-__global__ void __launch_bounds__(256) symview_kernel(const __grid_constant__ SymMapParams p)
+__device__ __forceinline__ int sort_sign32(int len, unsigned &x, unsigned &y, unsigned &z)
 {
+    int s = 1;
+    if (len == 1) return 1;
+    if (len == 2) {
+        if (x == y) return 0;
+        if (x > y) { const unsigned t = x; x = y; y = t; s = -1; }
+        return s;
+    }
+    if (x == y || y == z || x == z) return 0;
+    if (x > y) { const unsigned t = x; x = y; y = t; s = -s; }
+    if (y > z) { const unsigned t = y; y = z; z = t; s = -s; }
+    if (x > y) { const unsigned t = x; x = y; y = t; s = -s; }
+    return s;
+}
+// packed position of a strictly increasing tuple; group labels are below 65536 (one label alone: any 32-bit value)
+__device__ __forceinline__ long long tuple_pos32(int len, unsigned a, unsigned b, unsigned c)
+{
+    if (len == 1) return a;
+    const unsigned pb = (b * (b - 1)) >> 1;
+    if (len == 2) return (long long)pb + a;
+    return (long long)((unsigned long long)((c * (c - 1)) >> 1) * (c - 2) / 3) + pb + a;
+}
+
+// The tiled kernel behind tcb_unpack onto a packed D (one identity term) and tcb_antisym_pack (the shuffles).  A tile =
+// 256 * kTileU consecutive values of D's index 0 at fixed other indices ("row").  Per tile, through shared memory: the
+// tuples of the row's indices (one 64-bit division each, by one thread each), the value every L label fed by them takes
+// under every term, and per term the packed offset and sign of the L groups fed by the row alone.  Per element and term only
+// the groups holding a label of D's index 0 are sorted, in 32-bit arithmetic.  (One thread per element with everything
+// recomputed: 358 instructions per element, 21 ms for a 15 GB view; the first tiled version with a per-thread row decode:
+// 12.8 ms.)
+__global__ void __launch_bounds__(256) symtile_kernel(const __grid_constant__ SymMapParams p)
+{
+    __shared__ long long s_tup[kMaxRank];
+    __shared__ unsigned s_val[kMaxSymTerms][kMaxRank][3];
+    __shared__ long long s_off[kMaxSymTerms];
+    __shared__ int s_sgn[kMaxSymTerms];
     const long long e0 = p.dext[0];
-    const long long tiles_per_row = (e0 + 256 * kViewU - 1) / (256 * kViewU);
+    const long long tile_elems = 256 * kTileU;
+    const long long tiles_per_row = (e0 + tile_elems - 1) / tile_elems;
     const long long ntiles = p.nrows * tiles_per_row;
+    const int tid = threadIdx.x;
+    const int len0 = p.dlen[0];
     for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const long long row = tile / tiles_per_row, chunk = tile - row * tiles_per_row;
-        long long tup[kMaxRank];
-        {
-            long long r = row;
-            tup[0] = 0;
-#pragma unroll
-            for (int d = 1; d < kMaxRank; ++d) {
-                tup[d] = 0;
-                if (d < p.nd) {
-                    const long long i = r % p.dext[d];
-                    r /= p.dext[d];
-                    tup[d] = tuple_word(p, d, i);
+        __syncthreads();
+        if (tid >= 1 && tid < p.nd) s_tup[tid] = tuple_word(p, tid, (row / p.rowdiv[tid]) % p.dext[tid]);
+        __syncthreads();
+        for (int q = tid; q < p.nterms * kMaxRank * 3; q += 256) {
+            const int t = q / (kMaxRank * 3), g = (q / 3) % kMaxRank, sl = q % 3;
+            unsigned val = 0;
+            if (g < p.nl && sl < p.llen[g]) {
+                const int d = p.lsrc_dim[g][sl];
+                if (d != 0) {
+                    const long long w = s_tup[d];
+                    val = p.dlen[d] == 1 ? (unsigned)w : (unsigned)(w >> (16 * p.perm[t][d][p.lsrc_slot[g][sl]])) & 0xffffu;
                 }
             }
+            s_val[t][g][sl] = val;
         }
-        long long off_row = 0;
-        int sign_row = 1;
-        for (int g = 0; g < p.nl; ++g) {
-            if (p.touch0[g]) continue;
-            long long val[3] = {0, 0, 0};
-#pragma unroll
-            for (int s = 0; s < 3; ++s) {
-                if (s < p.llen[g]) {
-                    const int d = p.lsrc_dim[g][s];
-                    const long long w = pick(tup, d);
-                    val[s] = p.dlen[d] == 1 ? w : (w >> (16 * p.lsrc_slot[g][s])) & 0xffff;
-                }
+        __syncthreads();
+        if (tid < p.nterms) {
+            long long off = 0;
+            int sg = p.sign[tid];
+            for (int g = 0; g < p.nl; ++g) {
+                if (p.touch0[g]) continue;
+                unsigned x = s_val[tid][g][0], y = s_val[tid][g][1], z = s_val[tid][g][2];
+                sg *= sort_sign32(p.llen[g], x, y, z);
+                off += tuple_pos32(p.llen[g], x, y, z) * p.lstride[g];
             }
-            sign_row *= sort_sign(p.llen[g], val[0], val[1], val[2]);
-            off_row += tuple_pos(p.llen[g], val[0], val[1], val[2]) * p.lstride[g];
+            s_off[tid] = off;
+            s_sgn[tid] = sg;
         }
+        __syncthreads();
         double2 *dst = p.out + row * e0;
-#pragma unroll
-        for (int u = 0; u < kViewU; ++u) {
-            const long long i0 = (chunk * kViewU + u) * 256 + threadIdx.x;
+        for (int u = 0; u < kTileU; ++u) {
+            const long long i0 = chunk * tile_elems + u * 256 + tid;
             if (i0 >= e0) break;
-            int sg = sign_row;
-            double2 v = make_double2(0.0, 0.0);
-            if (sg != 0) {
-                tup[0] = tuple_word(p, 0, i0);
-                long long off = off_row;
+            long long w0 = i0;
+            if (len0 > 1) {
+                const SymTuple t0 = p.dtab[0][i0];
+                w0 = (long long)t0.v[0] | ((long long)t0.v[1] << 16) | ((long long)t0.v[2] << 32);
+            }
+            double sr = 0.0, si = 0.0;
+            for (int t = 0; t < p.nterms; ++t) {
+                int sg = s_sgn[t];
+                if (sg == 0) continue;
+                long long off = s_off[t];
                 for (int g = 0; g < p.nl; ++g) {
                     if (!p.touch0[g]) continue;
-                    long long val[3] = {0, 0, 0};
+                    unsigned val[3] = {0, 0, 0};
 #pragma unroll
-                    for (int s = 0; s < 3; ++s) {
-                        if (s < p.llen[g]) {
-                            const int d = p.lsrc_dim[g][s];
-                            const long long w = pick(tup, d);
-                            val[s] = p.dlen[d] == 1 ? w : (w >> (16 * p.lsrc_slot[g][s])) & 0xffff;
+                    for (int sl = 0; sl < 3; ++sl) {
+                        if (sl < p.llen[g]) {
+                            if (p.lsrc_dim[g][sl] == 0)
+                                val[sl] = len0 == 1 ? (unsigned)w0 : (unsigned)(w0 >> (16 * p.perm[t][0][p.lsrc_slot[g][sl]])) & 0xffffu;
+                            else
+                                val[sl] = s_val[t][g][sl];
                         }
                     }
-                    sg *= sort_sign(p.llen[g], val[0], val[1], val[2]);
-                    off += tuple_pos(p.llen[g], val[0], val[1], val[2]) * p.lstride[g];
+                    sg *= sort_sign32(p.llen[g], val[0], val[1], val[2]);
+                    off += tuple_pos32(p.llen[g], val[0], val[1], val[2]) * p.lstride[g];
                 }
                 if (sg != 0) {
                     const double2 w = p.in[off];
-                    const double wr = sg > 0 ? w.x : -w.x, wi = sg > 0 ? w.y : -w.y;
-                    v.x = __dsub_rn(__dmul_rn(p.ar, wr), __dmul_rn(p.ai, wi));
-                    v.y = __dadd_rn(__dmul_rn(p.ar, wi), __dmul_rn(p.ai, wr));
+                    sr = __dadd_rn(sr, sg > 0 ? w.x : -w.x);
+                    si = __dadd_rn(si, sg > 0 ? w.y : -w.y);
                 }
             }
+            double2 v;
+            v.x = __dsub_rn(__dmul_rn(p.ar, sr), __dmul_rn(p.ai, si));
+            v.y = __dadd_rn(__dmul_rn(p.ar, si), __dmul_rn(p.ai, sr));
             if (p.accumulate) {
                 const double2 d = dst[i0];
                 v.x = __dadd_rn(d.x, v.x);
@@ -303,7 +344,7 @@ __global__ void __launch_bounds__(256) symview_kernel(const __grid_constant__ Sy
     }
 }
 
-// One thread per element of D (D is the small, packed side or a packed view of it).  The tuple of every D index sits in one
+// Fallback (a short index 0 of D, where a tile would be mostly empty): one thread per element of D.  The tuple of every D index sits in one
 // 64-bit register (16 bits per component; a single-label index keeps its full value), so nothing is indexed dynamically.
 __global__ void __launch_bounds__(256) symmap_kernel(const __grid_constant__ SymMapParams p)
 {
@@ -446,17 +487,20 @@ cudaError_t launch_symmap(const SymMapDesc &d, cudaStream_t stream, int64_t *lau
             if (g < d.nl && s2 < d.llen[g] && d.lsrc_dim[g][s2] == 0) p.touch0[g] = 1;
     }
     p.nrows = p.total / p.dext[0];
-    if (d.nterms == 1 && d.sign[0] == 1) {
-        bool identity = true;
-        for (int k = 0; k < kMaxRank; ++k) for (int s2 = 0; s2 < 3; ++s2) identity = identity && d.perm[0][k][s2] == s2;
-        if (identity) {
-            const long long tiles = p.nrows * ((p.dext[0] + 256 * kViewU - 1) / (256 * kViewU));
-            const int vb = (int)std::max<long long>(1, std::min<long long>(tiles, 16LL * sm_count()));
-            symview_kernel<<<vb, 256, 0, stream>>>(p);
-            cudaError_t ve = cudaGetLastError();
-            if (ve == cudaSuccess && launches) ++*launches;
-            return ve;
-        }
+    bool fits32 = true;
+    long long div = 1;
+    for (int k = 0; k < kMaxRank; ++k) {
+        p.rowdiv[k] = div;
+        if (k >= 1) div *= p.dext[k];
+        fits32 = fits32 && p.dext[k] < (1LL << 31);
+    }
+    if (p.dext[0] >= 128 && fits32) {
+        const long long tiles = p.nrows * ((p.dext[0] + 256 * kTileU - 1) / (256 * kTileU));
+        const int vb = (int)std::max<long long>(1, std::min<long long>(tiles, 16LL * sm_count()));
+        symtile_kernel<<<vb, 256, 0, stream>>>(p);
+        cudaError_t ve = cudaGetLastError();
+        if (ve == cudaSuccess && launches) ++*launches;
+        return ve;
     }
     const int blocks = (int)std::max<long long>(1, std::min<long long>((p.total + 255) / 256, 16LL * sm_count()));
     symmap_kernel<<<blocks, 256, 0, stream>>>(p);

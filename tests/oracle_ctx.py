@@ -64,3 +64,18 @@ class OracleContext:
     def antisym_pack(self, spec, D, L, alpha=1.0):
         D.host = sym.antisym_pack(spec, L.host, D.host, alpha)
         self.calls += 1
+
+    def denominator_divide(self, T, R, eps, alpha=1.0):
+        from oracle import cc
+        T.host = cc.denominator_update(np.zeros_like(R.host), R.host, eps, alpha)
+        self.calls += 1
+
+    def denominator_update(self, T, R, eps, alpha=1.0):
+        from oracle import cc
+        T.host = cc.denominator_update(T.host, R.host, eps, alpha)
+        self.calls += 1
+
+    def dot(self, D, X, Y, conjugate_x=True, alpha=1.0):
+        x = np.conj(X.host) if conjugate_x else X.host
+        D.host = np.asfortranarray(np.array(alpha * np.sum(x * Y.host)))
+        self.calls += 1

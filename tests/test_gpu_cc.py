@@ -415,6 +415,39 @@ def test_ccsdt_residual_call_by_call_and_against_the_fock_space_pinned_equations
     assert np.abs(gR3 + gR3.transpose(1, 0, 2, 3, 4, 5)).max() <= 1e-12 * np.abs(R3.norm).max()
 
 
+@pytest.mark.parametrize("o,v", [(3, 4), (4, 12), (6, 9)])
+def test_packed_triples_correction_program(ctx, o, v):
+    """(T) on packed storage: R3p, t3p against the pack of the oracle program's dense R3, t3; E[T] and E_ST against the
+    oracle's and against the dense driver on the same inputs."""
+    from oracle import sym
+    n = o + v
+    g = synth.tensor(synth.SEED0 + 7, 1, [n] * 4, antisym=((0, 1), (2, 3)), sigma=0.3, hermitian=True)
+    rng = np.random.default_rng(o + v)
+    t2 = rng.standard_normal((v, v, o, o)) + 1j * rng.standard_normal((v, v, o, o))
+    t2 = t2 - t2.transpose(1, 0, 2, 3)
+    t2 = np.asfortranarray(t2 - t2.transpose(0, 1, 3, 2))
+    t1 = np.asfortranarray(rng.standard_normal((v, o)) + 1j * rng.standard_normal((v, o)))
+    eo, ev = np.linspace(-2.0, -0.5, o), np.linspace(0.5, 3.0, v)
+    W, U = np.asfortranarray(g[o:, o:, o:, :o]), np.asfortranarray(g[:o, o:, :o, :o])
+    oovv = np.asfortranarray(g[:o, :o, o:, o:])
+    dW, dU, dT, dT1, dV = (ctx.tensor_from_numpy(x) for x in (W, U, t2, t1, oovv))
+    dE, dEst, dR3p, dt3p = ccd.triples_correction_packed(ctx, dW, dU, dT, eo, ev, keep=True, T1=dT1, oovv=dV)
+    R3, t3, E = cc.triples_program(W, U, t2, eo, ev)
+    _, est_ref = cc.triples_singles_term(t1, oovv, t3)
+    assert np.max(np.abs(ctx.tensor_download(dR3p) - sym.pack("P(a<b<c,i<j<k)=R(a,b,c,i,j,k)", R3))) <= 1e-11 * np.abs(R3).max()
+    assert np.max(np.abs(ctx.tensor_download(dt3p) - sym.pack("P(a<b<c,i<j<k)=T(a,b,c,i,j,k)", t3))) <= 1e-11 * np.abs(t3).max()
+    got, got_st = complex(ctx.tensor_download(dE)), complex(ctx.tensor_download(dEst))
+    assert abs(got - E) <= 1e-11 * abs(E) and got.real < 0
+    assert abs(got_st - est_ref) <= 1e-11 * abs(est_ref)
+    eE, eEst = ccd.triples_correction(ctx, dW, dU, dT, eo, ev, T1=dT1, oovv=dV)
+    assert abs(got - complex(ctx.tensor_download(eE))) <= 1e-11 * abs(E)
+    assert abs(got_st - complex(ctx.tensor_download(eEst))) <= 1e-11 * abs(est_ref)
+    with pytest.raises(ValueError):
+        ccd.triples_correction_packed(ctx, dW, dU, ctx.tensor_create((v, v, 2, 2)), eo, ev)
+    for t in (dW, dU, dT, dT1, dV, dE, dEst, dR3p, dt3p, eE, eEst):
+        t.destroy()
+
+
 @pytest.mark.parametrize("o,v", [(3, 4), (4, 6), (5, 5)])
 def test_packed_ccsdt_residual_call_by_call_and_against_the_fock_space_pinned_equations(ctx, o, v):
     """SURVEY 8(f)-2 applied to 8(f)-3: ccd.ccsdt_residual_packed -- T3 and R3 only as (a<b<c, i<j<k) packed tensors, every

@@ -149,7 +149,12 @@ VIEW_CASES = [("Tq(d<e,c,i<j<k)=T(d<e<c,i<j<k)", dict(d=7, e=7, c=7, i=5, j=5, k
               ("Tr(j<k,e,b<c,m)=T(e<b<c,m<j<k)", dict(b=6, c=6, e=6, j=5, k=5, m=5)),
               ("Ts(a<c,b,i)=T(a<b<c,i)", dict(a=9, b=9, c=9, i=3)),
               ("D(a<b,c)=L(a,b<c)", dict(a=8, b=8, c=8)),                            # regrouping: zeros at b == c
-              ("D(x<y,p)=L(p,y,x)", dict(x=11, y=11, p=4))]                          # dense L: a pack with a transposition
+              ("D(x<y,p)=L(p,y,x)", dict(x=11, y=11, p=4)),                          # dense L: a pack with a transposition
+              # index 0 of D >= 128: the tiled kernel; 2080 pairs = one full tile of 2048 + a ragged one
+              ("Tq(d<e,c,q)=T(d<e<c,q)", dict(d=65, e=65, c=65, q=3)),
+              ("Tr(b<c,j<k,e,m)=T(b<c<e,j<k<m)", dict(b=17, c=17, e=17, j=5, k=5, m=5)),
+              ("D(p,x<y)=L(y,x,p)", dict(x=9, y=9, p=130)),                          # a plain index first
+              ("To(a<b<c,l<m,k)=T(a<b<c,l<m<k)", dict(a=12, b=12, c=12, l=5, m=5, k=5))]
 
 
 def _shape(groups, ext):
@@ -180,7 +185,13 @@ MERGE_CASES = [("R(a<b<c,i<j<k)=X(a,i,b<c,j<k)", dict(a=7, b=7, c=7, i=5, j=5, k
                ("R(a<b<c,i<j<k)=X(a,b,c,i,j,k)", dict(a=5, b=5, c=5, i=4, j=4, k=4), 36),
                ("R(i<j,a<b)=X(a,i,b,j)", dict(a=9, b=9, i=6, j=6), 4),
                ("R(a<b<c,q)=X(c,q,a<b)", dict(a=10, b=10, c=10, q=3), 3),
-               ("R(a<b<c,i<j<k)=X(a<b<c,i<j<k)", dict(a=6, b=6, c=6, i=5, j=5, k=5), 1)]
+               ("R(a<b<c,i<j<k)=X(a<b<c,i<j<k)", dict(a=6, b=6, c=6, i=5, j=5, k=5), 1),
+               # index 0 of D >= 128: the tiled kernel
+               ("R(a<b<c,i<j<k)=X(a,i,b<c,j<k)", dict(a=12, b=12, c=12, i=5, j=5, k=5), 9),
+               ("R(a<b<c,i<j<k)=X(a<b,i,c,j<k)", dict(a=12, b=12, c=12, i=5, j=5, k=5), 9),
+               ("R(a<b<c,q)=X(b<c,a,q)", dict(a=13, b=13, c=13, q=4), 3),
+               ("R(a<b,i<j)=X(a,i,b,j)", dict(a=18, b=18, i=4, j=4), 4),
+               ("R(a<b<c,i<j<k)=X(a,b,c,i,j,k)", dict(a=11, b=11, c=11, i=4, j=4, k=4), 36)]
 
 
 @pytest.mark.parametrize("spec,ext,nterms", MERGE_CASES)
@@ -263,3 +274,38 @@ def test_packed_t3_views_and_antisymmetriser_at_the_ccsdt_size(ctx):
         assert abs(hR[p, q] - 4.0 * ref) <= TOL * 4.0 * sn
     for t in (Tp, Tr, Xr, R):
         t.destroy()
+
+
+def test_packed_storage_calls_in_a_capture_cold_refused_warm_replayed():
+    """the first use of an (extent, group size) builds a tuple table (tcb_pack: an offset table): refused inside a capture
+    like a first plan; after one eager pass the same list is captured and the replay is bit-identical"""
+    c = pkg.Context(0)
+    rng = np.random.default_rng(8)
+    n, m = 13, 6                                             # extents no other test of this module uses first
+    Tp = rc(rng, sym.packed_extent(n, 3), m)
+    X = rc(rng, n, m, sym.packed_extent(n, 2))
+    dTp, dX = c.tensor_from_numpy(Tp), c.tensor_from_numpy(X)
+    dV, dR = c.tensor_create((sym.packed_extent(n, 2), n, m)), c.tensor_create((sym.packed_extent(n, 3), m))
+    calls = [lambda: c.unpack("V(a<b,c,q)=T(a<b<c,q)", dV, dTp, 1.0),
+             lambda: c.antisym_pack("R(a<b<c,q)=X(a,q,b<c)", dR, dX, 2.0)]
+    c.capture_begin()
+    for f in calls:
+        with pytest.raises(pkg.TcbError) as ei:
+            f()
+        assert ei.value.code == binding.TCB_EUNSUPPORTED
+    with pytest.raises(pkg.TcbError):
+        c.capture_end()
+    for f in calls:
+        f()
+    want_v, want_r = c.tensor_download(dV), c.tensor_download(dR)
+    assert np.array_equal(want_v, sym.unpack("V(a<b,c,q)=T(a<b<c,q)", Tp))
+    c.capture_begin()
+    for f in calls:
+        f()
+    g = c.capture_end()
+    c.tensor_fill(dV, 0.0)
+    c.tensor_fill(dR, 0.0)
+    c.graph_launch(g)
+    assert np.array_equal(c.tensor_download(dV), want_v) and np.array_equal(c.tensor_download(dR), want_r)
+    c.graph_destroy(g)
+    c.destroy()

@@ -250,6 +250,34 @@ def test_triples_correction_against_the_fock_space_and_unique_triples():
     assert np.abs(t3p + t3p.transpose(0, 1, 2, 3, 5, 4)).max() <= 1e-13 * np.abs(t3p).max()
 
 
+@pytest.mark.parametrize("o,v", [(3, 3), (3, 4), (4, 5)])
+def test_packed_triples_correction_driver_equals_the_unfactorised_sums(o, v):
+    """ccd.triples_correction_packed (R3, t3 only on a<b<c, i<j<k; contractions at 1/4 of the flops; tcb_antisym_pack for both
+    9-term operators; no factor 1/36) run on the host through the oracle's primitives: R3p is the pack of the direct sums,
+    E[T] and the singles term E_ST are those of the dense oracle programs (pinned above and below to the Fock space)."""
+    from oracle import sym
+    from oracle_ctx import OracleContext
+    from paper_2409_06759_b200 import ccd
+    f, g, t2 = rand_inputs(o, v, 50 + o + v)
+    t2 = np.asfortranarray(t2)
+    eo, ev = np.linspace(-2.0, -0.5, o), np.linspace(0.5, 3.0, v)
+    rng = np.random.default_rng(o * v)
+    t1 = np.asfortranarray(rng.standard_normal((v, o)) + 1j * rng.standard_normal((v, o)))
+    W, U = np.asfortranarray(g[o:, o:, o:, :o]), np.asfortranarray(g[:o, o:, :o, :o])
+    oovv = np.asfortranarray(g[:o, :o, o:, o:])
+    oc = OracleContext()
+    Wr = oc.tensor_from_numpy
+    E, Est, R3p, t3p = ccd.triples_correction_packed(oc, Wr(W), Wr(U), Wr(t2), eo, ev, keep=True, T1=Wr(t1), oovv=Wr(oovv))
+    R3u, Eu = cc.triples_unfactorised(o, g, t2, eo, ev)
+    _, t3, _ = cc.triples_program(W, U, t2, eo, ev)
+    _, est_ref = cc.triples_singles_term(t1, oovv, t3)
+    assert np.abs(R3p.host - sym.pack("P(a<b<c,i<j<k)=R(a,b,c,i,j,k)", R3u)).max() <= 1e-13 * np.abs(R3u).max()
+    assert np.abs(t3p.host - sym.pack("P(a<b<c,i<j<k)=T(a,b,c,i,j,k)", t3)).max() <= 1e-13 * np.abs(t3).max()
+    assert abs(E.host.ravel()[0] - Eu) <= 1e-13 * abs(Eu)
+    assert abs(Est.host.ravel()[0] - est_ref) <= 1e-13 * abs(est_ref)
+    assert oc.calls == 14
+
+
 def test_triples_singles_term_against_the_fock_space_matrix_element():
     """E_ST = <T1 Phi0| H |T3 Phi0> on the Fock space (T3 from PAPER Eq. 2) against 1/4 sum conj(t1) <jk||bc> t3."""
     o = v = 3
