@@ -116,12 +116,16 @@ CCSD_BLOCKS = ("vvoo", "oovv", "oooo", "vvvv", "ovvo", "ooov", "ovvv", "vovv", "
                "foo", "fvv", "fov", "fvo")
 
 
-def ccsd_residual(ctx, B, T1, T2, R1=None, R2=None):
+def ccsd_residual(ctx, B, T1, T2, R1=None, R2=None, packed=None):
     """Spin-orbital CCSD residuals (the paper's benchmark iteration) as the binary tensor operations a
     generated driver issues: 35 contractions, 9 permute-sums, 12 adds; intermediates are created and destroyed around
     their use (PAPER.md:212).  B: dict of device tensors `CCSD_BLOCKS` (<pq||rs> blocks in bra-ket order, f blocks);
     T1 (v,o) = t_i^a, T2 (v,v,o,o) = t_ij^ab.  Returns (E rank-0 tensor, R1, R2).  Equations: DESIGN.md / oracle/cc.py
-    `ccsd_residual_unfactorised` (pinned to PAPER Eq. (3) on the Fock space)."""
+    `ccsd_residual_unfactorised` (pinned to PAPER Eq. (3) on the Fock space).
+    packed: a dict (start with {}) switches the particle-particle ladder to index-permutation-symmetric packed storage
+    (SURVEY 8(f)-2): W_abef is built and used only as Wp(a<b, e<f) -- the v^4 o^2 ladder at 1/8 of the flops, its T1 term at
+    1/2, P(ab) as a `tcb_antisym_pack`.  The dict keeps the packed integral blocks (<ab||ef>, <am||ef>, <mn||ef>) between
+    calls; destroy its values when done."""
     v, o = T1.extents
     new = lambda shape: ctx.tensor_create(shape, zero=False)      # every tensor below is first written by an '=' call
     con, add, asym = ctx.contract, ctx.add, ctx.antisymmetrize
@@ -154,12 +158,28 @@ def ccsd_residual(ctx, B, T1, T2, R1=None, R2=None):
     asym("P(ij):W(m,n,i,j)+=X(m,n,i,j)", Wmnij, X, 1.0)
     X.destroy()
     con("W(m,n,i,j)+=V(m,n,e,f)*t(e,f,i,j)", Wmnij, B["oovv"], tau, 0.25)
-    X = new((v, v, v, v))
-    con("X(a,b,e,f)=V(a,m,e,f)*T1(b,m)", X, B["vovv"], T1, 1.0)
-    Wabef = copy(B["vvvv"], (v, v, v, v), "a,b,e,f")
-    asym("P(ab):W(a,b,e,f)+=X(a,b,e,f)", Wabef, X, -1.0)
-    X.destroy()
-    con("W(a,b,e,f)+=t(a,b,m,n)*V(m,n,e,f)", Wabef, tau, B["oovv"], 0.25)
+    if packed is None:
+        X = new((v, v, v, v))
+        con("X(a,b,e,f)=V(a,m,e,f)*T1(b,m)", X, B["vovv"], T1, 1.0)
+        Wabef = copy(B["vvvv"], (v, v, v, v), "a,b,e,f")
+        asym("P(ab):W(a,b,e,f)+=X(a,b,e,f)", Wabef, X, -1.0)
+        X.destroy()
+        con("W(a,b,e,f)+=t(a,b,m,n)*V(m,n,e,f)", Wabef, tau, B["oovv"], 0.25)
+    else:
+        nv2, no2 = ctx.packed_extent(v, 2), ctx.packed_extent(o, 2)
+        for name, shape, spec in (("vvvv", (nv2, nv2), "P(a<b,e<f)=V(a,b,e,f)"), ("vovv", (v, o, nv2), "P(a,m,e<f)=V(a,m,e,f)"),
+                                  ("oovv", (no2, nv2), "P(m<n,e<f)=V(m,n,e,f)")):
+            if name not in packed:
+                packed[name] = new(shape)
+                ctx.pack(spec, packed[name], B[name])
+        X = new((v, v, nv2))
+        con("X(a,b,z)=V(a,m,z)*T1(b,m)", X, packed["vovv"], T1, 1.0)
+        Wabef = copy(packed["vvvv"], (nv2, nv2), "x,z")
+        ctx.antisym_pack("W(a<b,z)+=X(a,b,z)", Wabef, X, -1.0)                 # P(ab) on packed storage
+        X.destroy()
+        taup = new((nv2, no2))
+        ctx.pack("P(a<b,m<n)=t(a,b,m,n)", taup, tau)
+        con("W(x,z)+=t(x,y)*V(y,z)", Wabef, taup, packed["oovv"], 0.5)         # 1/4 sum_mn = 1/2 sum_{m<n}
     Q = new((v, v, o, o))
     add("Q(f,b,j,n)=T2(f,b,j,n)", Q, T2, 0.5)
     add("Q(f,b,j,n)+=t(f,b,j,n)", Q, tt, 1.0)
@@ -192,7 +212,14 @@ def ccsd_residual(ctx, B, T1, T2, R1=None, R2=None):
     Fme.destroy()
     con("R(a,b,i,j)+=t(a,b,m,n)*W(m,n,i,j)", R2, tau, Wmnij, 0.5)
     Wmnij.destroy()
-    con("R(a,b,i,j)+=W(a,b,e,f)*t(e,f,i,j)", R2, Wabef, tau, 0.5)
+    if packed is None:
+        con("R(a,b,i,j)+=W(a,b,e,f)*t(e,f,i,j)", R2, Wabef, tau, 0.5)
+    else:
+        Rp = new((nv2, no2))
+        con("R(x,y)=W(x,z)*t(z,y)", Rp, Wabef, taup, 1.0)                      # 1/2 sum_ef = sum_{e<f}
+        ctx.unpack("R(a,b,i,j)+=P(a<b,i<j)", R2, Rp, 1.0)
+        Rp.destroy()
+        taup.destroy()
     Wabef.destroy()
     tau.destroy()
     con("X(a,b,i,j)=T2(a,e,i,m)*W(m,b,e,j)", X, T2, Wmbej, 1.0)
@@ -381,19 +408,21 @@ def ccd_solve_diis(ctx, B, e_occ, e_virt, iterations, depth=6):
     return T, energies, norms
 
 
-def ccsd_solve(ctx, B, e_occ, e_virt, iterations):
+def ccsd_solve(ctx, B, e_occ, e_virt, iterations, packed=False):
     """Jacobi iterations of the CCSD amplitude equations from zero amplitudes: t1 += R1 / (e_i - e_a),
     t2 += R2 / (e_i + e_j - e_a - e_b), both residuals evaluated at the old amplitudes.  One iteration = `ccsd_residual`
     + two `tcb_denominator_update`; the energy of the updated amplitudes is produced by the next residual evaluation
-    (so `iterations` updates cost iterations + 1 evaluations).  Returns (T1, T2, [E_corr after each step])."""
+    (so `iterations` updates cost iterations + 1 evaluations).  packed=True: the pp ladder on packed storage, the packed
+    integral blocks built once for all iterations.  Returns (T1, T2, [E_corr after each step])."""
     import numpy as np
     v, o = B["fvo"].extents
     T1, T2 = ctx.tensor_create((v, o)), ctx.tensor_create((v, v, o, o))
     R1, R2 = ctx.tensor_create((v, o)), ctx.tensor_create((v, v, o, o))
     ev, eo = -np.asarray(e_virt, dtype=np.float64), np.asarray(e_occ, dtype=np.float64)
     energies = []
+    cache = {} if packed else None
     for it in range(iterations + 1):
-        E, _, _ = ccsd_residual(ctx, B, T1, T2, R1, R2)
+        E, _, _ = ccsd_residual(ctx, B, T1, T2, R1, R2, cache)
         if it > 0:
             energies.append(complex(ctx.tensor_download(E)))
         E.destroy()
@@ -401,8 +430,8 @@ def ccsd_solve(ctx, B, e_occ, e_virt, iterations):
             break
         ctx.denominator_update(T1, R1, [ev, eo], 1.0)
         ctx.denominator_update(T2, R2, [ev, ev, eo, eo], 1.0)
-    R1.destroy()
-    R2.destroy()
+    for t in [R1, R2] + list((cache or {}).values()):
+        t.destroy()
     return T1, T2, energies
 
 

@@ -76,6 +76,15 @@ def test_ccsd_residual_program_call_by_call_with_each_calls_own_snorm(ctx):
     e_ref, r1_ref, r2_ref = cc.ccsd_residual_program(B, t1, t2)
     assert np.max(np.abs(sR2.host - r2_ref)) <= 1e-12 * np.abs(r2_ref).max()
     assert abs(complex(sE.host) - e_ref) <= 1e-12 * abs(e_ref)
+    # the same with the pp ladder on packed storage (W_abef only as Wp(a<b,e<f), P(ab) = tcb_antisym_pack)
+    sh2 = ShadowContext(ctx)
+    sB2 = {k: sh2.wrap(x) for k, x in B.items()}
+    cache = {}
+    pE, pR1, pR2 = ccd.ccsd_residual(sh2, sB2, sh2.wrap(t1), sh2.wrap(t2), packed=cache)
+    assert sh2.calls == 61 and sh2.worst <= 1e-11 and sorted(cache) == ["oovv", "vovv", "vvvv"]
+    assert np.max(np.abs(pR2.host - r2_ref)) <= 1e-12 * np.abs(r2_ref).max()
+    assert np.max(np.abs(ctx.tensor_download(pR2.gpu) - ctx.tensor_download(sR2.gpu))) <= 1e-11 * np.abs(pR2.norm).max()
+    assert np.max(np.abs(ctx.tensor_download(pR1.gpu) - ctx.tensor_download(sR1.gpu))) <= 1e-11 * np.abs(pR1.norm).max()
 
 
 def test_t3_term_program(ctx):

@@ -154,6 +154,32 @@ def test_ccsd_unfactorised_agrees_with_fock_space(o, v):
     assert np.abs(r2_d - cc.ccd_residual_unfactorised(o, f, g, t2)[0]).max() <= 1e-13 * np.abs(r2_d).max()
 
 
+@pytest.mark.parametrize("o,v", [(2, 3), (3, 4), (4, 5)])
+def test_ccsd_driver_with_the_packed_pp_ladder_equals_the_unfactorised_tier(o, v):
+    """ccd.ccsd_residual(packed={}): W_abef only as Wp(a<b, e<f), P(ab) as antisym_pack, the ladder at 1/8 of the flops --
+    run on the host through the oracle's primitives (tests/oracle_ctx.py) against the Fock-space-pinned direct sums, and
+    against the same driver with the dense ladder."""
+    from oracle_ctx import OracleContext
+    from paper_2409_06759_b200 import ccd
+    f, g, t2 = rand_inputs(o, v, 500 * o + v)
+    rng = np.random.default_rng(11 * o + v)
+    t1 = np.asfortranarray(0.3 * (rng.standard_normal((v, o)) + 1j * rng.standard_normal((v, o))))
+    t2 = np.asfortranarray(0.3 * t2)
+    e, r1, r2 = cc.ccsd_residual_unfactorised(o, f, g, t1, t2)
+    out = {}
+    for mode in ("dense", "packed"):
+        oc = OracleContext()
+        B = {k: oc.tensor_from_numpy(x) for k, x in cc.ccsd_blocks(o, f, g).items()}
+        cache = {} if mode == "packed" else None
+        E, R1, R2 = ccd.ccsd_residual(oc, B, oc.tensor_from_numpy(t1), oc.tensor_from_numpy(t2), packed=cache)
+        assert abs(E.host.ravel()[0] - e) <= 1e-13 * abs(e)
+        assert np.abs(R1.host - r1).max() <= 1e-13 * np.abs(r1).max()
+        assert np.abs(R2.host - r2).max() <= 1e-13 * np.abs(r2).max()
+        out[mode] = (oc.calls, cache)
+    assert out["dense"][0] == 56 and out["packed"][0] == 56 + 5      # 3 packs (once per solve), pack tau, unpack Rp
+    assert sorted(out["packed"][1]) == ["oovv", "vovv", "vvvv"]
+
+
 @pytest.mark.parametrize("o,v", [(2, 3), (3, 4)])
 def test_ccsd_program_of_binary_operations_agrees_with_the_unfactorised_tier(o, v):
     f, g, t2 = rand_inputs(o, v, 500 * o + v)
