@@ -632,7 +632,7 @@ def run_extras(ctx):
         E.destroy()
         classes = {k: ctx.kernel_stats(k) for k in ("zgemm", "permute", "permsum", "elementwise")}
         ctx.set_option("kernel_timing", "off")
-        out.append({"workload": "CCSD residual (R1, R2, E) o=30 v=150: 35 contractions + 9 permute-sums + 12 adds, "
+        out.append({"workload": "CCSD residual (R1, R2, E) o=30 v=150: 34 contractions + 9 permute-sums + 12 adds, "
                                 "vvvv and Wabef 8.1 GB each",
                     "ms": b, "ms_median": float(np.median(ts)), "contractions": Counting.calls, "launches": launches,
                     "tflops": Counting.flops / b * 1e-9,

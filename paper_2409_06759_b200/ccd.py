@@ -118,13 +118,13 @@ CCSD_BLOCKS = ("vvoo", "oovv", "oooo", "vvvv", "ovvo", "ooov", "ovvv", "vovv", "
 
 def ccsd_residual(ctx, B, T1, T2, R1=None, R2=None, packed=None):
     """Spin-orbital CCSD residuals (the paper's benchmark iteration) as the binary tensor operations a
-    generated driver issues: 35 contractions, 9 permute-sums, 12 adds; intermediates are created and destroyed around
+    generated driver issues: 34 contractions, 9 permute-sums, 12 adds; intermediates are created and destroyed around
     their use (PAPER.md:212).  B: dict of device tensors `CCSD_BLOCKS` (<pq||rs> blocks in bra-ket order, f blocks);
     T1 (v,o) = t_i^a, T2 (v,v,o,o) = t_ij^ab.  Returns (E rank-0 tensor, R1, R2).  Equations: DESIGN.md / oracle/cc.py
     `ccsd_residual_unfactorised` (pinned to PAPER Eq. (3) on the Fock space).
     packed: a dict (start with {}) switches the particle-particle ladder to index-permutation-symmetric packed storage
     (SURVEY 8(f)-2): W_abef is built and used only as Wp(a<b, e<f) -- the v^4 o^2 ladder at 1/8 of the flops, its T1 term at
-    1/2, P(ab) as a `tcb_antisym_pack`.  The dict keeps the packed integral blocks (<ab||ef>, <am||ef>, <mn||ef>) between
+    1/2, P(ab) as a `tcb_antisym_pack`.  The dict keeps the packed integral blocks (<ab||ef>, <am||ef>) between
     calls; destroy its values when done."""
     v, o = T1.extents
     new = lambda shape: ctx.tensor_create(shape, zero=False)      # every tensor below is first written by an '=' call
@@ -157,18 +157,18 @@ def ccsd_residual(ctx, B, T1, T2, R1=None, R2=None, packed=None):
     Wmnij = copy(B["oooo"], (o, o, o, o), "m,n,i,j")
     asym("P(ij):W(m,n,i,j)+=X(m,n,i,j)", Wmnij, X, 1.0)
     X.destroy()
-    con("W(m,n,i,j)+=V(m,n,e,f)*t(e,f,i,j)", Wmnij, B["oovv"], tau, 0.25)
+    # The quadratic term 1/4 tau V tau of R2 enters through W_mnij alone (coefficient 1/2 here instead of 1/4 here and 1/4
+    # in W_abef): o^4 v^2 work instead of v^4 o^2 -- the same residual; neither intermediate is used anywhere else.
+    con("W(m,n,i,j)+=V(m,n,e,f)*t(e,f,i,j)", Wmnij, B["oovv"], tau, 0.5)
     if packed is None:
         X = new((v, v, v, v))
         con("X(a,b,e,f)=V(a,m,e,f)*T1(b,m)", X, B["vovv"], T1, 1.0)
         Wabef = copy(B["vvvv"], (v, v, v, v), "a,b,e,f")
         asym("P(ab):W(a,b,e,f)+=X(a,b,e,f)", Wabef, X, -1.0)
         X.destroy()
-        con("W(a,b,e,f)+=t(a,b,m,n)*V(m,n,e,f)", Wabef, tau, B["oovv"], 0.25)
     else:
         nv2, no2 = ctx.packed_extent(v, 2), ctx.packed_extent(o, 2)
-        for name, shape, spec in (("vvvv", (nv2, nv2), "P(a<b,e<f)=V(a,b,e,f)"), ("vovv", (v, o, nv2), "P(a,m,e<f)=V(a,m,e,f)"),
-                                  ("oovv", (no2, nv2), "P(m<n,e<f)=V(m,n,e,f)")):
+        for name, shape, spec in (("vvvv", (nv2, nv2), "P(a<b,e<f)=V(a,b,e,f)"), ("vovv", (v, o, nv2), "P(a,m,e<f)=V(a,m,e,f)")):
             if name not in packed:
                 packed[name] = new(shape)
                 ctx.pack(spec, packed[name], B[name])
@@ -178,8 +178,7 @@ def ccsd_residual(ctx, B, T1, T2, R1=None, R2=None, packed=None):
         ctx.antisym_pack("W(a<b,z)+=X(a,b,z)", Wabef, X, -1.0)                 # P(ab) on packed storage
         X.destroy()
         taup = new((nv2, no2))
-        ctx.pack("P(a<b,m<n)=t(a,b,m,n)", taup, tau)
-        con("W(x,z)+=t(x,y)*V(y,z)", Wabef, taup, packed["oovv"], 0.5)         # 1/4 sum_mn = 1/2 sum_{m<n}
+        ctx.pack("P(e<f,i<j)=t(e,f,i,j)", taup, tau)
     Q = new((v, v, o, o))
     add("Q(f,b,j,n)=T2(f,b,j,n)", Q, T2, 0.5)
     add("Q(f,b,j,n)+=t(f,b,j,n)", Q, tt, 1.0)

@@ -231,7 +231,7 @@ def test_every_contraction_of_the_driver_programs_is_planned_on_the_host():
     n_ccd = len(rec.contractions)
     assert (n_ccd, len(rec.antisym), len(rec.adds)) == (11, 5, 3)
     ccd.ccsd_residual(rec, B, T1, T2)
-    assert len(rec.contractions) - n_ccd == 35 and len(rec.antisym) - 5 == 9
+    assert len(rec.contractions) - n_ccd == 34 and len(rec.antisym) - 5 == 9
     n_before = len(rec.contractions)
     ccd.triples_correction(rec, rec._T((v, v, v, o)), rec._T((o, v, o, o)), T2, [0.0] * o, [0.0] * v,
                            T1=T1, oovv=B["oovv"])

@@ -72,7 +72,7 @@ def test_ccsd_residual_program_call_by_call_with_each_calls_own_snorm(ctx):
     sh = ShadowContext(ctx)
     sB = {k: sh.wrap(x) for k, x in B.items()}
     sE, sR1, sR2 = ccd.ccsd_residual(sh, sB, sh.wrap(t1), sh.wrap(t2))
-    assert sh.calls == 56 and sh.worst <= 1e-11
+    assert sh.calls == 55 and sh.worst <= 1e-11
     e_ref, r1_ref, r2_ref = cc.ccsd_residual_program(B, t1, t2)
     assert np.max(np.abs(sR2.host - r2_ref)) <= 1e-12 * np.abs(r2_ref).max()
     assert abs(complex(sE.host) - e_ref) <= 1e-12 * abs(e_ref)
@@ -81,7 +81,7 @@ def test_ccsd_residual_program_call_by_call_with_each_calls_own_snorm(ctx):
     sB2 = {k: sh2.wrap(x) for k, x in B.items()}
     cache = {}
     pE, pR1, pR2 = ccd.ccsd_residual(sh2, sB2, sh2.wrap(t1), sh2.wrap(t2), packed=cache)
-    assert sh2.calls == 61 and sh2.worst <= 1e-11 and sorted(cache) == ["oovv", "vovv", "vvvv"]
+    assert sh2.calls == 59 and sh2.worst <= 1e-11 and sorted(cache) == ["vovv", "vvvv"]
     assert np.max(np.abs(pR2.host - r2_ref)) <= 1e-12 * np.abs(r2_ref).max()
     assert np.max(np.abs(ctx.tensor_download(pR2.gpu) - ctx.tensor_download(sR2.gpu))) <= 1e-11 * np.abs(pR2.norm).max()
     assert np.max(np.abs(ctx.tensor_download(pR1.gpu) - ctx.tensor_download(sR1.gpu))) <= 1e-11 * np.abs(pR1.norm).max()
@@ -183,7 +183,7 @@ def test_ccd_jacobi_iterations_follow_the_oracle(ctx):
 
 @pytest.mark.parametrize("o,v", [(3, 4), (5, 11)])
 def test_ccsd_residual_program(ctx, o, v):
-    """The CCSD residuals (singles, doubles, energy) as 56 ABI calls against the oracle's program of the same binary
+    """The CCSD residuals (singles, doubles, energy) as 55 ABI calls against the oracle's program of the same binary
     operations; at (3,4) also against the unfactorised tier (itself pinned to the Fock space)."""
     n = o + v
     rng = np.random.default_rng(o * 100 + v)
@@ -201,7 +201,7 @@ def test_ccsd_residual_program(ctx, o, v):
     dT1, dT2 = ctx.tensor_from_numpy(t1), ctx.tensor_from_numpy(t2)
     live = ctx.launch_count()
     dE, dR1, dR2 = ccd.ccsd_residual(ctx, dB, dT1, dT2)
-    assert ctx.launch_count() - live >= 56          # 56 ABI calls, at least one launch each
+    assert ctx.launch_count() - live >= 55          # 55 ABI calls, at least one launch each
     E, R1, R2 = complex(ctx.tensor_download(dE)), ctx.tensor_download(dR1), ctx.tensor_download(dR2)
     e_ref, r1_ref, r2_ref = cc.ccsd_residual_program(B, t1, t2)
     assert abs(E - e_ref) <= 1e-11 * abs(e_ref)

@@ -176,8 +176,8 @@ def test_ccsd_driver_with_the_packed_pp_ladder_equals_the_unfactorised_tier(o, v
         assert np.abs(R1.host - r1).max() <= 1e-13 * np.abs(r1).max()
         assert np.abs(R2.host - r2).max() <= 1e-13 * np.abs(r2).max()
         out[mode] = (oc.calls, cache)
-    assert out["dense"][0] == 56 and out["packed"][0] == 56 + 5      # 3 packs (once per solve), pack tau, unpack Rp
-    assert sorted(out["packed"][1]) == ["oovv", "vovv", "vvvv"]
+    assert out["dense"][0] == 55 and out["packed"][0] == 55 + 4      # 2 packs (once per solve), pack tau, unpack Rp
+    assert sorted(out["packed"][1]) == ["vovv", "vvvv"]
 
 
 @pytest.mark.parametrize("o,v", [(2, 3), (3, 4)])
