@@ -207,7 +207,9 @@ struct SymMapParams {
     long long total;
     int touch0[kMaxRank];                   // L group g holds a label of D's index 0
     long long nrows;                        // total / dext[0]
-    long long rowdiv[kMaxRank];             // product of dext[1 .. d-1]: row / rowdiv[d] % dext[d] = index d of the row
+    int tdim[kMaxRank];                     // rows are visited in an order of their own: position k (>= 1) runs D's index tdim[k]
+    long long tdiv[kMaxRank];               // row / tdiv[k] % dext[tdim[k]] = that index
+    long long dstride[kMaxRank];            // element stride of D's index d
     double ar, ai;
     const double2 *in;
     double2 *out;
@@ -256,6 +258,7 @@ __device__ __forceinline__ long long tuple_pos32(int len, unsigned a, unsigned b
 __global__ void __launch_bounds__(256) symtile_kernel(const __grid_constant__ SymMapParams p)
 {
     __shared__ long long s_tup[kMaxRank];
+    __shared__ long long s_idx[kMaxRank];
     __shared__ unsigned s_val[kMaxSymTerms][kMaxRank][3];
     __shared__ long long s_off[kMaxSymTerms];
     __shared__ int s_sgn[kMaxSymTerms];
@@ -268,7 +271,12 @@ __global__ void __launch_bounds__(256) symtile_kernel(const __grid_constant__ Sy
     for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const long long row = tile / tiles_per_row, chunk = tile - row * tiles_per_row;
         __syncthreads();
-        if (tid >= 1 && tid < p.nd) s_tup[tid] = tuple_word(p, tid, (row / p.rowdiv[tid]) % p.dext[tid]);
+        if (tid >= 1 && tid < p.nd) {
+            const int d = p.tdim[tid];
+            const long long i = (row / p.tdiv[tid]) % p.dext[d];
+            s_idx[d] = i;
+            s_tup[d] = tuple_word(p, d, i);
+        }
         __syncthreads();
         for (int q = tid; q < p.nterms * kMaxRank * 3; q += 256) {
             const int t = q / (kMaxRank * 3), g = (q / 3) % kMaxRank, sl = q % 3;
@@ -296,7 +304,11 @@ __global__ void __launch_bounds__(256) symtile_kernel(const __grid_constant__ Sy
             s_sgn[tid] = sg;
         }
         __syncthreads();
-        double2 *dst = p.out + row * e0;
+        long long rowoff = 0;
+#pragma unroll
+        for (int d = 1; d < kMaxRank; ++d)
+            if (d < p.nd) rowoff += s_idx[d] * p.dstride[d];
+        double2 *dst = p.out + rowoff;
         for (int u = 0; u < kTileU; ++u) {
             const long long i0 = chunk * tile_elems + u * 256 + tid;
             if (i0 >= e0) break;
@@ -488,11 +500,28 @@ cudaError_t launch_symmap(const SymMapDesc &d, cudaStream_t stream, int64_t *lau
     }
     p.nrows = p.total / p.dext[0];
     bool fits32 = true;
-    long long div = 1;
-    for (int k = 0; k < kMaxRank; ++k) {
-        p.rowdiv[k] = div;
-        if (k >= 1) div *= p.dext[k];
-        fits32 = fits32 && p.dext[k] < (1LL << 31);
+    {   // Row order: the index of D that feeds the L labels of SMALLEST stride runs fastest, so that consecutive tiles read the
+        // same stretch of L (view Tr(b<c,j<k,e,m) of T3p at o=16, v=100: e before (j<k) keeps one 2.6 MB column of T3p in L2
+        // instead of cycling through 120 of them: DRAM reads 38.7 GB -> see profiles/r2_sympack_ncu.md).
+        long long key[kMaxRank], st = 1;
+        for (int k = 0; k < kMaxRank; ++k) {
+            p.dstride[k] = st;
+            st *= p.dext[k];
+            fits32 = fits32 && p.dext[k] < (1LL << 31);
+            key[k] = 0;
+            for (int g = 0; g < d.nl; ++g)
+                for (int s2 = 0; s2 < d.llen[g]; ++s2)
+                    if (d.lsrc_dim[g][s2] == k) key[k] = std::max<long long>(key[k], d.lstride[g]);
+        }
+        int order[kMaxRank];
+        for (int k = 0; k < kMaxRank; ++k) order[k] = k;
+        if (d.nd > 2) std::stable_sort(order + 1, order + d.nd, [&](int x, int y) { return key[x] < key[y]; });
+        long long div = 1;
+        for (int k = 0; k < kMaxRank; ++k) {
+            p.tdim[k] = order[k];
+            p.tdiv[k] = div;
+            if (k >= 1 && k < d.nd) div *= p.dext[order[k]];
+        }
     }
     if (p.dext[0] >= 128 && fits32) {
         const long long tiles = p.nrows * ((p.dext[0] + 256 * kTileU - 1) / (256 * kTileU));
