@@ -499,7 +499,21 @@ def run_extras(ctx):
                     "one_lane_ms_by_class": {k: c["ms"] for k, c in classes.items()},
                     "one_lane_launches_by_class": {k: c["launches"] for k, c in classes.items()},
                     "one_lane_gbs_by_class": {k: (c["bytes"] / c["ms"] * 1e-6 if c["ms"] > 0 else None) for k, c in classes.items()}})
-        for t in list(B.values()) + [T, R]:
+        cache = {}
+        for _ in range(3):
+            ccd.ccd_residual(ctx, B, T, R, packed=cache)
+        ctx.sync()
+        ctx.capture_begin()
+        ccd.ccd_residual(ctx, B, T, R, packed=cache)
+        g = ctx.capture_end()
+        bp_graph, _ = best_of(lambda: [ctx.graph_launch(g) for _ in range(10)], 5)
+        bp_eager, _ = best_of(lambda: [ccd.ccd_residual(ctx, B, T, R, packed=cache) for _ in range(10)], 3)
+        ctx.graph_destroy(g)
+        out.append({"workload": "next row 8(f)-2: the configs[1] CCD residual with the pp ladder on packed storage (<ab||cd> packed "
+                                "once: 160 MB instead of 655 MB; ladder at 1/8 of the flops)",
+                    "ms_graph_replay": bp_graph / 10, "ms_call_by_call_lanes": bp_eager / 10,
+                    "dense_program_ms_graph_replay": b_graph / 10, "speedup_over_dense_program": b_graph / bp_graph})
+        for t in list(B.values()) + list(cache.values()) + [T, R]:
             t.destroy()
         ctx.sync()
     except Exception as e:          # noqa: BLE001

@@ -20,14 +20,16 @@ I4(a,d)     = oovv(k,l,c,d)*T(a,c,l,k) ; X(a,b,i,j) = I4(a,d)*T(d,b,i,j) ; R -= 
 """
 
 
-def ccd_residual(ctx, B, T, R=None, lanes=True):
+def ccd_residual(ctx, B, T, R=None, lanes=True, packed=None):
     """B: dict name -> Tensor for foo, fvv, vvoo, oovv, oooo, vvvv, ovvo;  T: Tensor (v,v,o,o).
     Returns the residual tensor R (v,v,o,o); all work is enqueued on the context (lane 0 holds the result).
 
     lanes: the intermediates that do not depend on one another are built side by side (DLTC layers,
     PAPER.md:79, instead of the barrier after every operation of PAPER.md:400): lane 1 builds I3, I4 and their X tensors
     (skinny, long-K contractions that leave most of the tensor pipe idle), lane 2 builds I2 and the ring term's X, lane 0
-    does the Fock terms, the two ladders, and every update of R (updates of one tensor stay on one lane, in order)."""
+    does the Fock terms, the two ladders, and every update of R (updates of one tensor stay on one lane, in order).
+    packed: a dict (start with {}) runs the particle-particle ladder on packed storage (`pp_ladder_packed`: 1/8 of the flops)
+    and keeps the packed <ab||cd> under "vvvv" between calls; destroy its values when done."""
     v, _, o, _ = T.extents
     use_lanes = lanes and hasattr(ctx, "lane_set")
     lane = ctx.lane_set if use_lanes else (lambda l: None)
@@ -71,7 +73,10 @@ def ccd_residual(ctx, B, T, R=None, lanes=True):
     ctx.contract("I1(k,l,i,j)+=W(k,l,c,d)*T(c,d,i,j)", I1, B["oovv"], T, 0.5)
     ctx.contract("R(a,b,i,j)+=T(a,b,k,l)*I1(k,l,i,j)", R, T, I1, 0.5)
     I1.destroy()
-    ctx.contract("R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)", R, B["vvvv"], T, 0.5)
+    if packed is None:
+        ctx.contract("R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)", R, B["vvvv"], T, 0.5)
+    else:
+        packed["vvvv"] = pp_ladder_packed(ctx, R, B["vvvv"], T, Vp=packed.get("vvvv"), alpha=0.5)
     wait(0, 2)
     ctx.antisymmetrize("P(ij)P(ab):R(a,b,i,j)+=X(a,b,i,j)", R, X2, 1.0)
     X2.destroy()
@@ -241,12 +246,13 @@ def ccsd_residual(ctx, B, T1, T2, R1=None, R2=None, packed=None):
     return E, R1, R2
 
 
-def ccd_solve(ctx, B, e_occ, e_virt, iterations, T=None, norms=None):
+def ccd_solve(ctx, B, e_occ, e_virt, iterations, T=None, norms=None, packed=False):
     """Jacobi iterations of the CCD amplitude equations (PAPER.md:212 energy denominators, 406-410 "CC
     iteration"):  T <- T + R(T) / (e_i + e_j - e_a - e_b), from T (default: a zero tensor, whose first step is the MP2
     guess).  Every step is `ccd_residual` + one `tcb_denominator_update` + the rank-0 energy contraction; only the
     16-byte energy comes back to the host per iteration.  norms: a list that receives the residual norm |R(T)| each
-    iteration started from (one `tcb_dot`).  Returns (T, [E_corr after each step])."""
+    iteration started from (one `tcb_dot`).  packed=True: the pp ladder on packed storage, <ab||cd>
+    packed once for all iterations.  Returns (T, [E_corr after each step])."""
     import numpy as np
     v, _, o, _ = B["vvoo"].extents
     if T is None:
@@ -254,15 +260,17 @@ def ccd_solve(ctx, B, e_occ, e_virt, iterations, T=None, norms=None):
     ev, eo = -np.asarray(e_virt, dtype=np.float64), np.asarray(e_occ, dtype=np.float64)
     R = ctx.tensor_create((v, v, o, o))
     energies = []
+    cache = {} if packed else None
     for _ in range(iterations):
-        ccd_residual(ctx, B, T, R)
+        ccd_residual(ctx, B, T, R, packed=cache)
         if norms is not None:
             norms.append(residual_norm(ctx, R))     # |R(T)| of the amplitudes this iteration started from
         ctx.denominator_update(T, R, [ev, ev, eo, eo], 1.0)
         E = ccd_energy(ctx, B, T)
         energies.append(complex(ctx.tensor_download(E)))
         E.destroy()
-    R.destroy()
+    for t in [R] + list((cache or {}).values()):
+        t.destroy()
     return T, energies
 
 

@@ -53,6 +53,13 @@ def test_ccd_residual_program_call_by_call_with_each_calls_own_snorm(ctx, o, v, 
     assert sh.calls == 19 and sh.worst <= 1e-11
     ref = cc.ccd_residual_program(B, T)
     assert np.max(np.abs(sR.host - ref)) <= 1e-12 * np.abs(ref).max()     # the shadow's own chain is the oracle program
+    # the pp ladder on packed storage: 2 packs + GEMM on packed indices + unpack instead of the one dense contraction
+    sh2 = ShadowContext(ctx)
+    cache = {}
+    pR = ccd.ccd_residual(sh2, {k: sh2.wrap(x) for k, x in B.items()}, sh2.wrap(T), lanes=lanes, packed=cache)
+    assert sh2.calls == 22 and sh2.worst <= 1e-11 and list(cache) == ["vvvv"]
+    assert np.max(np.abs(pR.host - ref)) <= 1e-12 * np.abs(ref).max()
+    assert np.max(np.abs(ctx.tensor_download(pR.gpu) - ctx.tensor_download(sR.gpu))) <= 1e-11 * np.abs(pR.norm).max()
 
 
 def test_ccsd_residual_program_call_by_call_with_each_calls_own_snorm(ctx):
