@@ -733,3 +733,31 @@ def ccsdt_jacobi(o, f, g, iterations):
         T2 = denominator_update(T2, R2, [ev, ev, eo, eo], 1.0)
         T3 = denominator_update(T3, R3, [ev, ev, ev, eo, eo, eo], 1.0)
     return T1, T2, T3, energies, norms
+
+
+def ccsdt_diis(o, f, g, iterations, depth=6):
+    """The CCSDT iteration with DIIS over the combined (t1, t2, t3) vector (as `ccsd_diis`, one more component): error
+    vector e_k = (R1 / D1, R2 / D2, R3 / D3) at the current amplitudes, trial vector = amplitudes + e_k, next amplitudes =
+    the combination of the last `depth` trial vectors minimising |sum c_i e_i|, <e_i|e_j> summed over the three components
+    (every element of the full antisymmetric tensors counted).
+    Returns (T1, T2, T3, [E_corr of the amplitudes each evaluation saw], [residual norm of each evaluation])."""
+    v = f.shape[0] - o
+    e = np.real(np.diag(f))
+    eo, ev = e[:o], -e[o:]
+    T = [np.zeros((v, o), dtype=np.complex128, order="F"), np.zeros((v, v, o, o), dtype=np.complex128, order="F"),
+         np.zeros((v, v, v, o, o, o), dtype=np.complex128, order="F")]
+    eps = [[ev, eo], [ev, ev, eo, eo], [ev, ev, ev, eo, eo, eo]]
+    trial, err, energies, norms = [], [], [], []
+    for _ in range(iterations):
+        E, R1, R2, R3 = ccsdt_residual_unfactorised(o, f, g, *T)
+        energies.append(E)
+        norms.append(residual_norm(R1, R2, R3))
+        ek = [denominator_update(np.zeros_like(t), r, d, 1.0) for t, r, d in zip(T, (R1, R2, R3), eps)]
+        trial.append([np.asfortranarray(t + x) for t, x in zip(T, ek)])
+        err.append(ek)
+        trial, err = trial[-depth:], err[-depth:]
+        m = len(err)
+        Bm = np.array([[sum(np.vdot(err[i][q], err[j][q]) for q in range(3)) for j in range(m)] for i in range(m)])
+        c = diis_coefficients(Bm) if m > 1 else np.ones(1)
+        T = [np.asfortranarray(sum(ci * t[q] for ci, t in zip(c, trial))) for q in range(3)]
+    return T[0], T[1], T[2], energies, norms

@@ -901,3 +901,90 @@ def ccsdt_solve(ctx, o, h, g, f_diag, iterations, packed=False):
     for t in list(Bz.values()) + [R1, R2, R3]:
         t.destroy()
     return T1, T2, T3, energies, norms
+
+
+def ccsdt_solve_diis(ctx, o, h, g, f_diag, iterations, depth=6, packed=True):
+    """The CCSDT iteration with DIIS over the combined (t1, t2, t3) vector (oracle: cc.ccsdt_diis): per evaluation the three
+    residuals, their norm, the error vectors e = R / D (`tcb_denominator_divide`), the trial vectors, one new row of
+    <e_i|e_j> (three `tcb_dot` per pair), the extrapolated amplitudes (`tcb_add`) -- all on the device; the depth x depth
+    system is solved on the host.  packed=True: t3, R3 and the DIIS history of t3 live as (a<b<c, i<j<k) tensors (each
+    history entry 1/36 of a dense one); an inner product over the full antisymmetric tensor is 36 times the packed one.
+    Returns (T1, T2, T3, [E_corr of the amplitudes each evaluation saw], [residual norm of each evaluation])."""
+    import numpy as np
+    n = g.extents[0]
+    v = n - o
+    e = np.asarray(f_diag, dtype=np.float64)
+    eo, ev = e[:o], -e[o:]
+    if packed:
+        shape3, lab3, w3 = (ctx.packed_extent(v, 3), ctx.packed_extent(o, 3)), "x,y", 36.0
+        eps3 = [np.asarray(_tuple_sums(ev, 3)), np.asarray(_tuple_sums(eo, 3))]
+    else:
+        shape3, lab3, w3 = (v, v, v, o, o, o), "a,b,c,i,j,k", 1.0
+        eps3 = [ev, ev, ev, eo, eo, eo]
+    shapes = [(v, o), (v, v, o, o), shape3]
+    labels = ["a,i", "a,b,i,j", lab3]
+    eps = [[ev, eo], [ev, ev, eo, eo], eps3]
+    weight = [1.0, 1.0, w3]
+    residual = ccsdt_residual_packed if packed else ccsdt_residual
+    T = [ctx.tensor_create(s_) for s_ in shapes]
+    R = [ctx.tensor_create(s_) for s_ in shapes]
+    Bz = t1_dressed_blocks(ctx, o, h, g, T[0], ("fov", "oovv"))        # T1 = 0 here: the bare blocks, for the energy
+    trial, err, energies, norms = [], [], [], []
+    Bm = np.zeros((0, 0), dtype=np.complex128)
+    s = ctx.tensor_create(())
+
+    def dot(X, Y):
+        ctx.dot(s, X, Y, True, 1.0)
+        return complex(ctx.tensor_download(s))
+
+    for _ in range(iterations):
+        E = ctx.tensor_create(())
+        Y = ctx.tensor_create((o, v), zero=False)
+        ctx.contract("E()=f(i,a)*T(a,i)", E, Bz["fov"], T[0], 1.0)
+        ctx.contract("E()+=W(i,j,a,b)*T(a,b,i,j)", E, Bz["oovv"], T[1], 0.25)
+        ctx.contract("Y(i,a)=W(i,j,a,b)*T(b,j)", Y, Bz["oovv"], T[0], 1.0)
+        ctx.contract("E()+=Y(i,a)*T(a,i)", E, Y, T[0], 0.5)
+        residual(ctx, o, h, g, T[0], T[1], T[2], R[0], R[1], R[2])
+        energies.append(complex(ctx.tensor_download(E)))
+        E.destroy()
+        Y.destroy()
+        norms.append(float(np.sqrt(sum(w * dot(r, r).real for w, r in zip(weight, R)))))
+        if len(err) == depth:                      # the oldest entry leaves; its tensors are reused
+            ek, tk = err.pop(0), trial.pop(0)
+            Bm = Bm[1:, 1:]
+        else:
+            ek = [ctx.tensor_create(s_, zero=False) for s_ in shapes]
+            tk = [ctx.tensor_create(s_, zero=False) for s_ in shapes]
+        for q in range(3):
+            ctx.denominator_divide(ek[q], R[q], eps[q], 1.0)
+            ctx.add(f"t({labels[q]})=T({labels[q]})", tk[q], T[q], 1.0)
+            ctx.add(f"t({labels[q]})+=e({labels[q]})", tk[q], ek[q], 1.0)
+        err.append(ek)
+        trial.append(tk)
+        m = len(err)
+        row = np.array([sum(weight[q] * dot(err[i][q], ek[q]) for q in range(3)) for i in range(m)])   # <e_i|e_new>
+        Bn = np.zeros((m, m), dtype=np.complex128)
+        Bn[:m - 1, :m - 1] = Bm
+        Bn[:, m - 1] = row
+        Bn[m - 1, :] = row.conj()
+        Bn[m - 1, m - 1] = row[m - 1]
+        Bm = Bn
+        if m > 1:
+            A = np.zeros((m + 1, m + 1), dtype=np.complex128)
+            A[:m, :m] = Bm
+            A[:m, m] = A[m, :m] = 1.0
+            rhs = np.zeros(m + 1, dtype=np.complex128)
+            rhs[m] = 1.0
+            c = np.linalg.solve(A, rhs)[:m]
+        else:
+            c = np.ones(1, dtype=np.complex128)
+        for k, (ci, tk_) in enumerate(zip(c, trial)):
+            op = "=" if k == 0 else "+="
+            for q in range(3):
+                ctx.add(f"T({labels[q]}){op}t({labels[q]})", T[q], tk_[q], complex(ci))
+    for entry in err + trial:
+        for x in entry:
+            x.destroy()
+    for x in R + [s] + list(Bz.values()):
+        x.destroy()
+    return T[0], T[1], T[2], energies, norms

@@ -517,3 +517,34 @@ def test_ccsdt_iterations_follow_the_oracle_and_converge(ctx, packed):
     for k in range(its):
         assert abs(energies[k] - e_ref[k]) <= 1e-10 * abs(e_ref[-1]) and abs(norms[k] - n_ref[k]) <= 1e-10 * n_ref[0]
     assert norms[-1] < 1e-4 * norms[0]
+
+
+@pytest.mark.parametrize("packed", [False, True])
+def test_ccsdt_diis_follows_the_oracle_and_converges(ctx, packed):
+    """DIIS over (t1, t2, t3) around the CCSDT residual, dense and with t3 / R3 / the t3 history packed (inner products
+    weighted by 36): amplitudes, energies and residual norms of every evaluation against cc.ccsdt_diis."""
+    o, v = 3, 3
+    rng = np.random.default_rng(52)
+    n = o + v
+    c = lambda *s: rng.standard_normal(s) + 1j * rng.standard_normal(s)
+    A = c(n, n, n, n)
+    A = A - A.transpose(1, 0, 2, 3)
+    A = A - A.transpose(0, 1, 3, 2)
+    g = 0.05 * 0.5 * (A + A.transpose(2, 3, 0, 1).conj())
+    e = np.concatenate([np.linspace(-2.0, -0.5, o), np.linspace(0.5, 3.0, v)])
+    f = 0.05 * c(n, n)
+    f = f + f.conj().T
+    f[np.diag_indices(n)] = e
+    h = f - np.einsum("piqi->pq", g[:, :o, :, :o])
+    its = 9
+    dh, dg = ctx.tensor_from_numpy(h), ctx.tensor_from_numpy(g)
+    T1, T2, T3, energies, norms = ccd.ccsdt_solve_diis(ctx, o, dh, dg, e, its, packed=packed)
+    r1, r2, r3, e_ref, n_ref = cc.ccsdt_diis(o, f, g, its)
+    if packed:
+        T3p, T3 = T3, ctx.tensor_create((v, v, v, o, o, o), zero=False)
+        ctx.unpack("T(a,b,c,i,j,k)=P(a<b<c,i<j<k)", T3, T3p, 1.0)
+    for got, ref in ((T1, r1), (T2, r2), (T3, r3)):
+        assert np.abs(ctx.tensor_download(got) - ref).max() <= 1e-9 * max(np.abs(ref).max(), 1e-300)
+    for k in range(its):
+        assert abs(energies[k] - e_ref[k]) <= 1e-9 * abs(e_ref[-1]) and abs(norms[k] - n_ref[k]) <= 1e-9 * n_ref[0]
+    assert norms[-1] < 1e-5 * norms[0]

@@ -479,3 +479,19 @@ def test_converged_ccsdt_iteration_zeroes_all_three_fock_space_projections():
     # triples change the energy: CCSD's fixed point differs
     _, _, e_sd = cc.ccsd_jacobi(cc.ccsd_blocks(o, f, g), eo, ev, 45)
     assert abs(e_sd[-1] - e0) > 1e-9 * abs(e0)
+
+
+def test_ccsdt_diis_reaches_the_fock_space_fixed_point_in_fewer_evaluations():
+    """DIIS over (t1, t2, t3): the amplitudes it converges to zero all three Fock-space projections (the Jacobi fixed point),
+    the first residual norm is that of the driver terms, and after 10 evaluations the norm is far below Jacobi's."""
+    o, v = 3, 3
+    f, g, eo, ev = _ccsd_problem(o, v, 52)
+    T1, T2, T3, energies, norms = cc.ccsdt_diis(o, f, g, 18)
+    e0, s0, d0, t0, _ = _fock_ccsdt(o, v, f, g, T1, T2, T3)
+    scale = np.abs(g).max()
+    assert max(np.abs(s0).max(), np.abs(d0).max(), np.abs(t0).max()) <= 1e-12 * scale
+    assert abs(cc.ccsdt_residual_unfactorised(o, f, g, T1, T2, T3)[0] - e0) <= 1e-12 * abs(e0)
+    _, _, _, ej, nj = cc.ccsdt_jacobi(o, f, g, 11)
+    assert norms[0] == nj[0] and energies[0] == 0 and abs(norms[1] - nj[1]) <= 1e-14 * nj[0]    # the first step is a Jacobi step
+    assert norms[10] < 0.05 * nj[10]
+    assert np.abs(T3).max() > 1e-6
