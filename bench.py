@@ -244,7 +244,7 @@ def run_ours(args, rank, world, local_rank):
     # second context (its own stream) for the uploads: while step n computes on one copy, step n+1's operands cross PCIe
     # into the other.
     h2d, d2h = Vt.nbytes + Tt.nbytes + Rt.nbytes, Rt.nbytes
-    e2e_steps = max(3, min(args.steps, 5))
+    e2e_steps = max(3, min(args.steps, 20))
     # N replicas on one host each pin 27.6 GB: when the host cannot hold all of them at once the ranks take turns in groups
     # (PCIe links are per GPU; what the turns leave out is contention for host memory bandwidth -- said in the JSON line)
     host_ram = os.sysconf("SC_PAGE_SIZE") * os.sysconf("SC_PHYS_PAGES")
