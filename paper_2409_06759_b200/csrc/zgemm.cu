@@ -737,8 +737,32 @@ GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk)
             // by the fix-up, the fewer the better.
             // measured: 6 per CTA behind whole tiles (pp ladder 33.1 -> 33.7 TFLOP/s: the tail is half a chunk), 3 when
             // everything is chunks (more only lengthens the fix-up's sums)
-            const int64_t per_cta = tiles >= slots ? 6 : tiles >= 16 ? 3 : 1;
-            const int64_t chunks = std::max<int64_t>(1, std::min<int64_t>(per_cta * slots, rem * KT / 8));
+            // A handful of tiles (2 ... 15, small M x N with a long K): four chunks per CTA of >= 24 k-tiles.  The tiles of
+            // such a grid are ragged (M = 150 -> 64 + 48 + 38 rows) and a k-tile of a 6 x 6-block tile costs 9/16 of an
+            // 8 x 8 one; with one equal chunk per CTA the CTAs on the small tiles idle while the full tiles finish
+            // (150 x 150 x 135000 took as long as 192 x 192 x 135000: 1.13 ms; dynamic claims of smaller chunks: 0.90 ms).
+            // A single tile has nothing to balance: one chunk per CTA.
+            // Only where the tiles really differ (largest / mean warp work >= 1.25): with equal tiles (128 x 128, 192 x 192)
+            // more chunks only lengthen the fix-up (0.53 -> 0.60 ms).
+            auto warp_rows = [](int64_t blocks, int tiles_dim, int64_t *sum, int64_t *mx) {
+                const int64_t pairs = (blocks + 1) / 2, base = pairs / tiles_dim, extra = pairs % tiles_dim;
+                int64_t at = 0;
+                *sum = 0; *mx = 0;
+                for (int t = 0; t < tiles_dim; ++t) {
+                    const int64_t np = base + (t < extra ? 1 : 0);
+                    const int64_t b = std::min<int64_t>(2 * (at + np), blocks) - 2 * at;
+                    at += np;
+                    *sum += (b + 1) / 2;
+                    *mx = std::max<int64_t>(*mx, (b + 1) / 2);
+                }
+            };
+            int64_t sm_, mm_, sn_, mn_;
+            warp_rows(mblocks, s.mt, &sm_, &mm_);
+            warp_rows(nblocks, s.nt, &sn_, &mn_);
+            const bool ragged = 4 * mm_ * mn_ * tiles >= 5 * sm_ * sn_;          // max >= 1.25 x mean
+            const bool few = tiles > 1 && tiles < 16 && ragged;
+            const int64_t per_cta = tiles >= slots ? 6 : tiles >= 16 ? 3 : few ? 4 : 1;
+            const int64_t chunks = std::max<int64_t>(1, std::min<int64_t>(per_cta * slots, rem * KT / (few ? 24 : 8)));
             s.sk_q = (int)((rem * KT + chunks - 1) / chunks);
             if (s.dp_tiles == 0) s.splits = (int)((KT + s.sk_q - 1) / s.sk_q);
         }
