@@ -151,6 +151,22 @@ int tcb_denominator_divide(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, con
  * X and Y have the same shape (any rank), D has rank 0 and overlaps neither.  Deterministic (fixed summation order).
  * Stream-ordered like every other call: download D to read it.  Errors: TCB_EINVAL, TCB_ESHAPE, TCB_EALIAS, TCB_ECUDA. */
 int tcb_dot(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, const tcb_tensor *Y, int conjugate_x, tcb_c128 alpha);
+/* The same inner product for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): tcb_dot keeps its per-block partial sums in a stream-ordered allocation made for the call; this
+ * entry point keeps them in ONE fixed device array inside the library (131 328 bytes, held by every GPU that loads the
+ * library until the process exits) and calls no cudaMalloc / cudaMallocAsync / cudaFree or allocating routine: one
+ * 4-byte cudaMemsetAsync and one kernel launch on the context's current lane.  Same arguments and checks as tcb_dot.
+ *   Limit: X and Y hold at most TCB_DOT_NOALLOC_MAX_ELEMS = 536 870 912 elements (8.6 GB each); more is refused with
+ *          TCB_EUNSUPPORTED (nothing enqueued, D untouched) -- use tcb_dot.
+ *   Result: deterministic; the grid depends on the element count alone, so the bits do not depend on the GPU model either.
+ *          It differs from tcb_dot's by summation order only (both round every product and sum separately; <x|x> has an
+ *          exactly zero imaginary part).
+ *   Sharing: every call on a device uses the same array, which keeps the last call's contents (the call clears the counter
+ *          it needs at zero itself).  Calls that OVERLAP on the GPU -- other lanes, streams, contexts or host threads on
+ *          the same device -- race on it: keep them on one stream or order them with events.
+ * Errors: TCB_EINVAL, TCB_ESHAPE, TCB_EALIAS, TCB_EUNSUPPORTED (too many elements), TCB_ECUDA. */
+#define TCB_DOT_NOALLOC_MAX_ELEMS 536870912LL
+int tcb_dot_noalloc(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, const tcb_tensor *Y, int conjugate_x, tcb_c128 alpha);
 /* S3, tensor transposition: "D(i,j,a,b)=L(a,b,i,j)", pure data movement, bit-exact. */
 int tcb_permute(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor *L);
 /* S6, fused permute-sum (the generator's unrolled permutation operators):

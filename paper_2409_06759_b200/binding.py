@@ -6,6 +6,7 @@ import os
 
 import numpy as np
 
+DOT_NOALLOC_MAX_ELEMS = 536870912          # TCB_DOT_NOALLOC_MAX_ELEMS of include/tcb200.h
 TCB_OK, TCB_EINVAL_EXPR, TCB_ESHAPE, TCB_ERANK, TCB_EALIAS, TCB_ENOMEM, TCB_ECUDA, TCB_EUNSUPPORTED, TCB_EINVAL = \
     0, -1, -2, -3, -4, -5, -6, -7, -8
 
@@ -42,7 +43,7 @@ ABI_SYMBOLS = [
     "tcb_ctx_create", "tcb_ctx_destroy", "tcb_ctx_set_option", "tcb_sync", "tcb_last_error", "tcb_strerror",
     "tcb_launch_count", "tcb_tensor_create", "tcb_tensor_alloc", "tcb_tensor_wrap", "tcb_tensor_destroy", "tcb_tensor_info",
     "tcb_tensor_upload", "tcb_tensor_download", "tcb_tensor_fill", "tcb_contract", "tcb_add", "tcb_scale",
-    "tcb_denominator_update", "tcb_denominator_divide", "tcb_dot",
+    "tcb_denominator_update", "tcb_denominator_divide", "tcb_dot", "tcb_dot_noalloc",
     "tcb_permute", "tcb_permsum", "tcb_antisymmetrize", "tcb_plan_describe", "tcb_measure_fp64_tensor_peak", "tcb_measure_fp64_vector_peak",
     "tcb_capture_begin", "tcb_capture_end", "tcb_graph_launch", "tcb_graph_info", "tcb_graph_destroy",
     "tcb_lane_count", "tcb_lane_set", "tcb_lane_wait", "tcb_pack", "tcb_unpack", "tcb_antisym_pack", "tcb_packed_extent",
@@ -81,6 +82,7 @@ def load_library():
         "tcb_denominator_update": [vp, vp, vp, ctypes.POINTER(ctypes.POINTER(ctypes.c_double)), c128],
         "tcb_denominator_divide": [vp, vp, vp, ctypes.POINTER(ctypes.POINTER(ctypes.c_double)), c128],
         "tcb_dot": [vp, vp, vp, vp, ctypes.c_int, c128],
+        "tcb_dot_noalloc": [vp, vp, vp, vp, ctypes.c_int, c128],
         "tcb_permute": [vp, cp, vp, vp],
         "tcb_permsum": [vp, vp, vp, ctypes.c_int, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(c128), c128],
         "tcb_antisymmetrize": [vp, cp, vp, vp, c128],
@@ -307,6 +309,11 @@ class Context:
     def dot(self, D, X, Y, conjugate_x=True, alpha=1.0):
         """D (rank 0) = alpha * sum conj?(X) * Y"""
         self._check(self.lib.tcb_dot(self.handle, D.handle, X.handle, Y.handle, int(bool(conjugate_x)), _c(alpha)))
+
+    def dot_noalloc(self, D, X, Y, conjugate_x=True, alpha=1.0):
+        """tcb_dot with its scratch in a fixed device array inside the library: no allocation of any kind; at most
+        DOT_NOALLOC_MAX_ELEMS elements; calls that overlap on the GPU race on the array"""
+        self._check(self.lib.tcb_dot_noalloc(self.handle, D.handle, X.handle, Y.handle, int(bool(conjugate_x)), _c(alpha)))
 
     def permute(self, expr, D, L):
         self._check(self.lib.tcb_permute(self.handle, expr.encode(), D.handle, L.handle))

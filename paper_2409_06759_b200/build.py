@@ -5,7 +5,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtcb200.so")
-SOURCES = ["api.cpp", "device.cpp", "parse.cpp", "plan.cpp", "zgemm.cu", "gemv.cu", "permute.cu", "permsum.cu", "permsum_orbit.cu", "sympack.cu", "elementwise.cu",
+SOURCES = ["api.cpp", "device.cpp", "parse.cpp", "plan.cpp", "zgemm.cu", "gemv.cu", "permute.cu", "permsum.cu", "permsum_orbit.cu", "sympack.cu", "elementwise.cu", "dot_noalloc.cu",
            "peak.cu", "synth.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-x", "cu"]

@@ -924,6 +924,28 @@ int tcb_dot(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, const tcb_tensor *
     return TCB_OK;
 }
 
+static_assert(TCB_DOT_NOALLOC_MAX_ELEMS == kNoAllocMaxElems, "the header states the limit of dot_noalloc.cu");
+
+int tcb_dot_noalloc(tcb_ctx *ctx, tcb_tensor *D, const tcb_tensor *X, const tcb_tensor *Y, int conjugate_x, tcb_c128 alpha)
+{
+    NvtxRange nvtx_range("tcb_dot_noalloc");
+    int rc = enter(ctx);
+    if (rc) return rc;
+    if (!D || !X || !Y) return set_error(ctx, TCB_EINVAL, "null argument");
+    if (D->shape.rank != 0) return set_error(ctx, TCB_ESHAPE, "D must have rank 0");
+    if (X->shape.rank != Y->shape.rank) return set_error(ctx, TCB_ESHAPE, "rank mismatch");
+    for (int k = 0; k < X->shape.rank; ++k)
+        if (X->shape.ext[k] != Y->shape.ext[k]) return set_error(ctx, TCB_ESHAPE, "X and Y differ in shape");
+    if (overlaps(D, X) || overlaps(D, Y)) return set_error(ctx, TCB_EALIAS, "D overlaps X or Y");
+    const int64_t n = X->elems();
+    if (n > kNoAllocMaxElems)
+        return set_error(ctx, TCB_EUNSUPPORTED, "tcb_dot_noalloc: " + std::to_string(n) + " elements exceed the fixed scratch array's " +
+                                                    std::to_string(kNoAllocMaxElems) + " (TCB_DOT_NOALLOC_MAX_ELEMS); use tcb_dot");
+    TimedLaunch tl(ctx, kClsElementwise, 8.0 * (double)n, 32.0 * (double)n);
+    TCB_CUDA(ctx, launch_dot_noalloc(D->ptr, X->ptr, Y->ptr, n, conjugate_x != 0, alpha.re, alpha.im, cur_stream(ctx), &ctx->launches));
+    return TCB_OK;
+}
+
 static int denominator_op(tcb_ctx *ctx, tcb_tensor *T, const tcb_tensor *R, const double *const *eps, tcb_c128 alpha,
                           bool accumulate)
 {

@@ -179,6 +179,12 @@ cudaError_t launch_axpy(void *D, const void *L, int64_t n, double re, double im,
 constexpr int kDotBlocks = 1024;      // upper bound of the first-stage grid (4 blocks per SM)
 cudaError_t launch_dot(void *D, const void *X, const void *Y, int64_t n, bool conj_x, double re, double im, void *partial,
                        int nblocks, cudaStream_t stream, int64_t *launches);
+// The same inner product with its partial sums in a file-scope device array instead of an allocation (dot_noalloc.cu):
+// at most kNoAllocMaxElems elements; launches on `stream`; calls that overlap on the GPU race on the array.
+constexpr int kNoAllocMaxBlocks = 8192;                                  // partial sums the array holds (131 328 bytes with its header)
+constexpr int64_t kNoAllocMaxElems = (int64_t)kNoAllocMaxBlocks * 65536;  // 536 870 912 elements (8.6 GB per operand)
+cudaError_t launch_dot_noalloc(void *D, const void *X, const void *Y, int64_t n, bool conj_x, double re, double im,
+                               cudaStream_t stream, int64_t *launches);
 // T[idx] (+)= alpha * R[idx] / (sum_k eps[eps_at[k] + idx_k]) over the dims with eps_at[k] >= 0 (eps: device doubles)
 cudaError_t launch_denominator_update(void *T, const void *R, int rank, const int64_t *extent, const double *eps_dev,
                                       const int *eps_at, double re, double im, bool accumulate, cudaStream_t stream,
