@@ -183,3 +183,63 @@ def test_configs4_ccsd_contraction_list_fullsize_sampled(ctx):
         worst = max(worst, err)
         seen += 1
     assert seen >= 20 and worst <= TOL
+
+
+PACKED_CCSDT_CALLS = [  # the contractions of ccd.ccsdt_residual_packed that hold >= 100 MB at o=16, v=100, on their packed extents
+    ("X(a,i,x,y)=W(m,a,i,e)*T(x,y,e,m)", 1.0),        # ring term: 1600 x 594000 x 1600, T and X 15.2 GB, operand permuted
+    ("X(x,c,t)=W(x,z)*T(z,c,t)", 2.0),                # vvvv term on a<b, d<e, i<j<k: 4950 x 56000 x 4950
+    ("X(x,c,t)+=T(x,e,t)*F(c,e)", 1.0),               # K = 100 accumulation into 4.4 GB
+    ("X(t,y,k)=T(t,z,k)*W(z,y)", 2.0),                # oooo term on a<b<c, l<m: 2587200 x 120 x 120
+    ("X(t,y,k)+=T(t,y,m)*F(m,k)", 1.0),               # K = 16
+    ("X(a,i,x,y)+=W(x,i,d)*T(d,a,y)", 1.0),           # 12000 x 79200 x 100 accumulation into 15.2 GB
+    ("X(a,i,x,y)+=W(l,a,y)*T(x,l,i)", 1.0),           # K = 16
+    ("W(x,i,d)+=T(x,z,e,i)*g(z,d,e)", -0.25),         # 79200 x 100 x 12000, T3 view gathered
+    ("W(l,a,y)+=g(l,m,z)*T(z,y,a,m)", -0.25),         # 16 x 12000 x 79200
+    ("X(x,i,j)=T(x,z,d,j)*W(z,i,d)", 2.0),            # doubles <- T3: 79200 x 16 x 12000
+    ("X(a,b,y)=W(l,a,z)*T(z,y,b,l)", 2.0),            # doubles <- T3: 100 x 12000 x 79200
+    ("R(x,y)=T(x,y,d,l)*f(l,d)", 1.0),                # GEMV over a 15.2 GB view
+    ("R(a,i)+=T(x,y,a,i)*W(y,x)", 1.0),               # GEMV, K = 594000
+]
+
+
+def test_packed_ccsdt_contractions_at_the_timed_size_sampled(ctx):
+    """bench.py times ccd.ccsdt_residual_packed at o=16, v=100 (dense T3: 65.5 GB per tensor).  Every contraction of that
+    program that touches a packed view of T3 or a packed accumulator, with the packed extents it has there (pairs 4950 / 120,
+    triples 161700 / 560), on sampled outputs: per free label 5 index values, every contracted index value, long-double
+    oracle on host-regenerated operands."""
+    from gpu_util import split_expr
+    o, v = 16, 100
+    nv2, nv3, no2, no3 = v * (v - 1) // 2, v * (v - 1) * (v - 2) // 6, o * (o - 1) // 2, o * (o - 1) * (o - 2) // 6
+    # extents by the role a label plays in the driver's expressions
+    sizes = {"X(a,i,x,y)=W(m,a,i,e)*T(x,y,e,m)": dict(a=v, i=o, x=nv2, y=no2, m=o, e=v),
+             "X(x,c,t)=W(x,z)*T(z,c,t)": dict(x=nv2, z=nv2, c=v, t=no3),
+             "X(x,c,t)+=T(x,e,t)*F(c,e)": dict(x=nv2, c=v, e=v, t=no3),
+             "X(t,y,k)=T(t,z,k)*W(z,y)": dict(t=nv3, y=no2, z=no2, k=o),
+             "X(t,y,k)+=T(t,y,m)*F(m,k)": dict(t=nv3, y=no2, m=o, k=o),
+             "X(a,i,x,y)+=W(x,i,d)*T(d,a,y)": dict(a=v, i=o, x=nv2, y=no2, d=v),
+             "X(a,i,x,y)+=W(l,a,y)*T(x,l,i)": dict(a=v, i=o, x=nv2, y=no2, l=o),
+             "W(x,i,d)+=T(x,z,e,i)*g(z,d,e)": dict(x=nv2, i=o, d=v, z=no2, e=v),
+             "W(l,a,y)+=g(l,m,z)*T(z,y,a,m)": dict(l=o, a=v, y=no2, m=o, z=nv2),
+             "X(x,i,j)=T(x,z,d,j)*W(z,i,d)": dict(x=nv2, i=o, j=o, z=no2, d=v),
+             "X(a,b,y)=W(l,a,z)*T(z,y,b,l)": dict(a=v, b=v, y=no2, l=o, z=nv2),
+             "R(x,y)=T(x,y,d,l)*f(l,d)": dict(x=nv2, y=no2, d=v, l=o),
+             "R(a,i)+=T(x,y,a,i)*W(y,x)": dict(a=v, i=o, x=nv2, y=no2)}
+    rng = np.random.default_rng(16)
+    worst = 0.0
+    for k, (e, alpha) in enumerate(PACKED_CCSDT_CALLS):
+        err, n = sampled_contraction_parity(ctx, e, sizes[e], alpha, synth.SEED0 + 40 + k, rng, nsub=5, sigma=0.5)
+        assert err <= TOL and n >= 25, (e, err, n)
+        worst = max(worst, err)
+    assert worst <= TOL
+
+
+def test_packed_ccsd_ladder_contractions_at_the_timed_size_sampled(ctx):
+    """bench.py times ccd.ccsd_residual(packed={}) at o=30, v=150: its two contractions on packed indices (pairs 11175 / 435)
+    on sampled outputs, as above."""
+    o, v = 30, 150
+    nv2, no2 = v * (v - 1) // 2, o * (o - 1) // 2
+    rng = np.random.default_rng(30)
+    for k, (e, alpha, ext) in enumerate([("R(x,y)=W(x,z)*t(z,y)", 1.0, dict(x=nv2, y=no2, z=nv2)),
+                                         ("X(a,b,z)=V(a,m,z)*T1(b,m)", 1.0, dict(a=v, b=v, z=nv2, m=o))]):
+        err, n = sampled_contraction_parity(ctx, e, ext, alpha, synth.SEED0 + 60 + k, rng, nsub=8, sigma=0.5)
+        assert err <= TOL and n >= 64, (e, err, n)
