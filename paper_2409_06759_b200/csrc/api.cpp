@@ -279,7 +279,8 @@ int get_plan(tcb_ctx *ctx, const char *expr, const tcb_tensor *D, const tcb_tens
 {
     std::string key = std::string(expr) + "|" + shape_key(D->shape) + shape_key(L->shape) + shape_key(R->shape) +
                       "|" + std::to_string(ctx->opt.splitk) + "," + std::to_string(ctx->opt.epilogue) + "," +
-                      (ctx->opt.permute_always ? "1" : "0") + "," + std::to_string(ctx->opt.operand_loads);
+                      (ctx->opt.permute_always ? "1" : "0") + "," + std::to_string(ctx->opt.operand_loads) + "," +
+                      std::to_string(ctx->opt.complex_product);
     auto it = ctx->plans.find(key);
     if (it != ctx->plans.end()) { *out = it->second.get(); return TCB_OK; }
     {
@@ -358,6 +359,10 @@ int tcb_ctx_create(tcb_ctx **out, int device, void *cuda_stream, size_t workspac
     if (cudaSetDevice(device) != cudaSuccess) return TCB_ECUDA;
     std::unique_ptr<tcb_ctx> ctx(new tcb_ctx());
     ctx->device = device;
+    if (const char *cp_env = getenv("TCB_COMPLEX_PRODUCT")) {          // A/B runs of whole test suites: the context's default
+        const std::string v = cp_env;
+        ctx->opt.complex_product = v == "3m" ? 2 : v == "4m" ? 1 : 0;
+    }
     for (int c = 0; c < 4; ++c) ctx->acc[c] = tcb_kernel_stat{0, 0.0, 0.0, 0.0};
     if (cuda_stream) {
         ctx->lanes[0].stream = (cudaStream_t)cuda_stream;
@@ -707,6 +712,7 @@ int tcb_contract(tcb_ctx *ctx, const char *expr, tcb_tensor *D, const tcb_tensor
     g.alpha_re = P.twopass ? 1.0 : alpha.re; g.alpha_im = P.twopass ? 0.0 : alpha.im;
     g.accumulate = P.twopass ? false : P.accumulate;
     g.splitk = P.splitk;
+    g.m3 = P.m3;
     g.partial = bytesP ? ws + bytesA + bytesB : nullptr;
     g.counters = ctx->opt.static_deal ? nullptr : ctx->lanes[ctx->cur].ws;      // the workspace header
     // the two TMA descriptors are kept beside the plan: re-encoded only when an operand sits somewhere else
@@ -770,6 +776,13 @@ static int apply_option(PlanOptions &opt, const std::string &k, const std::strin
         else if (v == "gather") opt.operand_loads = 1;
         else if (v == "permute") opt.operand_loads = 2;
         else { *why = "operand_loads: expected auto, gather or permute"; return TCB_EINVAL; }
+        return TCB_OK;
+    }
+    if (k == "complex_product") {
+        if (v == "auto") opt.complex_product = 0;
+        else if (v == "4m") opt.complex_product = 1;
+        else if (v == "3m") opt.complex_product = 2;
+        else { *why = "complex_product: expected auto, 4m or 3m"; return TCB_EINVAL; }
         return TCB_OK;
     }
     if (k == "gemm_deal") {

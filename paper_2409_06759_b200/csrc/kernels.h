@@ -39,6 +39,7 @@ struct GemmDesc {
     // unit-stride index is a row (free) index, so lanes run along m, else along k.  Same for B.
     const int64_t *gatherAm = nullptr, *gatherAk = nullptr, *gatherBn = nullptr, *gatherBk = nullptr;
     bool a_mfast = false, b_mfast = false;
+    bool m3 = false;         // three real products per complex product, 48 x 48 tiles (zgemm.cu); the maps must be encoded with it
 };
 constexpr size_t kGemmCounterBytes = 64;
 // How the (tile, k-tile) iteration space is dealt to the persistent grid (2 CTAs per SM): whole tiles
@@ -50,7 +51,7 @@ struct GemmSchedule {
     int splits;              // pieces per tile when every tile is cut (reported by the planner), else 1
     size_t partial_bytes;
 };
-GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk);
+GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk, bool m3 = false);
 constexpr int kGemmBM = 64, kGemmBN = 64, kGemmBK = 8;
 cudaError_t launch_zgemm(const GemmDesc &g, cudaStream_t stream, int64_t *launches);
 // Encodes the two TMA descriptors; separated so that the planner can cache them.

@@ -371,8 +371,14 @@ int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const 
 
     // (vii) schedule: whole tiles data-parallel over the persistent grid, the remainder wave (or, for skinny
     // M x N with long K, everything) cut along K -- see gemm_schedule in zgemm.cu
+    // (vii-a) complex products from three real ones (3M) where the GEMM is tensor-bound and TMA-fed: measured +10 ... +18 %
+    // from K = 128 up (profiles/r2_gemm_3m.md); not with a gathered operand (the gather is the bound: -2 ... -5 %) and not with
+    // two M-major operands (12 TMA requests per k-tile: -9 %).  "complex_product" = "3m" / "4m" forces either.
+    constexpr int64_t kM3MinK = 128;
+    P.m3 = opt.complex_product == 2 ||
+           (opt.complex_product == 0 && !P.a.gather && !P.b.gather && (P.a.kmajor || P.b.kmajor) && P.K >= kM3MinK);
     P.splitk = opt.splitk;
-    const GemmSchedule sc = gemm_schedule(P.M, P.N, P.K, opt.splitk);
+    const GemmSchedule sc = gemm_schedule(P.M, P.N, P.K, opt.splitk, P.m3);
     P.splits = sc.splits;
     P.partial_bytes = sc.partial_bytes;
 
@@ -391,12 +397,12 @@ std::string ContractPlan::describe() const
                   "\"k_labels\": \"%s\", \"row_operand\": \"%s\", \"permute_A\": %s, \"permute_B\": %s, "
                   "\"A_layout\": \"%s\", \"B_layout\": \"%s\", \"feed_A\": \"%s\", \"feed_B\": \"%s\", \"splits\": %d, "
                   "\"route\": \"%s\", \"epilogue\": \"%s\", \"accumulate\": %s, \"flops\": %.6g, \"bytes\": %.6g, "
-                  "\"est_us\": %.4g}",
+                  "\"est_us\": %.4g, \"complex_product\": \"%s\"}",
                   (long long)M, (long long)N, (long long)K, join(m_labels).c_str(), join(n_labels).c_str(),
                   join(k_labels).c_str(), swapped ? "R" : "L", a.permuted ? "true" : "false",
                   b.permuted ? "true" : "false", a.kmajor ? "K-major" : "M-major", b.kmajor ? "K-major" : "M-major",
                   feed(a), feed(b), splits, gemv ? "gemv" : outer ? "outer" : "gemm", twopass ? "twopass" : "fused-scatter",
-                  accumulate ? "true" : "false", flops, bytes, est_seconds * 1e6);
+                  accumulate ? "true" : "false", flops, bytes, est_seconds * 1e6, (gemv || outer) ? "fma" : m3 ? "3m" : "4m");
     return buf;
 }
 

@@ -21,6 +21,7 @@ struct PlanOptions {
     int splitk = 0;               // 0 = auto, 1 = off, n > 1 = forced
     int epilogue = 0;             // 0 = auto, 1 = fused, 2 = two-pass (GEMM into workspace + permute-accumulate pass)
     int operand_loads = 0;        // 0 = auto (cost model), 1 = never permute (gather whatever TMA cannot read), 2 = never gather
+    int complex_product = 0;      // 0 = auto, 1 = "4m" (four real products per complex product), 2 = "3m" (three; see zgemm.cu)
     bool permute_always = false;  // A/B testing: permute both operands even when they are matrix-shaped
     bool static_deal = false;     // A/B testing: GEMM work dealt statically (tile c + w * grid) instead of claimed
 };
@@ -60,6 +61,7 @@ struct ContractPlan {
     std::vector<std::string> m_labels, n_labels, k_labels;
     double flops = 0, bytes = 0;
     double est_seconds = 0;   // the cost model's estimate for the chosen candidate
+    bool m3 = false;          // the GEMM forms complex products from three real ones (3M); decided here, see plan.cpp
     bool twopass = false;     // epilogue: GEMM into a plain M x N workspace matrix, then c_perm brings it into D
     PermuteShape c_perm;
     std::string describe() const;

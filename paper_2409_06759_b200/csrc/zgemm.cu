@@ -375,14 +375,54 @@ __device__ __forceinline__ void mma_ktile(double (&cr)[4][4][2], double (&ci)[4]
     }
 }
 
-template <int AMODE, int BMODE>
+// The same k-tile with THREE real products per complex product (the "3M" scheme of xGEMM3M):
+//     P1 = Ar Br,  P2 = Ai Bi,  P3 = (Ar + Ai)(Br + Bi);      Re C = P1 - P2,  Im C = P3 - P1 - P2
+// 3 DMMAs per block pair and k-step instead of 4, three accumulator sets instead of two -- which is why a warp holds at most
+// 3 x 3 blocks here (108 accumulator registers; 4 x 4 would need 192 of the 255).  The operand sums cost MC + NC DADDs per
+// k-step on the pipe DMMA runs on (6 against 27 DMMAs of 16 issue slots each).
+template <int MC, int NC, int KS>
+__device__ __forceinline__ void mma_ktile3(double (&p1)[3][3][2], double (&p2)[3][3][2], double (&p3)[3][3][2], uint32_t sA,
+                                           uint32_t sB, const uint32_t (&offA)[2], const uint32_t (&offB)[2])
+{
+#pragma unroll
+    for (int ks = 0; ks < KS; ++ks) {
+        double2 a[MC], b[NC];
+        double as[MC], bs[NC];
+#pragma unroll
+        for (int i = 0; i < MC; ++i) a[i] = lds128(sA + i * 1024 + offA[ks]);
+#pragma unroll
+        for (int j = 0; j < NC; ++j) b[j] = lds128(sB + j * 1024 + offB[ks]);
+#pragma unroll
+        for (int i = 0; i < MC; ++i) as[i] = __dadd_rn(a[i].x, a[i].y);
+#pragma unroll
+        for (int j = 0; j < NC; ++j) bs[j] = __dadd_rn(b[j].x, b[j].y);
+#pragma unroll
+        for (int i = 0; i < MC; ++i)
+#pragma unroll
+            for (int j = 0; j < NC; ++j) {
+                dmma(p1[i][j][0], p1[i][j][1], a[i].x, b[j].x);
+                dmma(p2[i][j][0], p2[i][j][1], a[i].y, b[j].y);
+                dmma(p3[i][j][0], p3[i][j][1], as[i], bs[j]);
+            }
+    }
+}
+
+template <int AMODE, int BMODE, bool M3>
 __global__ void __launch_bounds__(NTHREADS, 2)
 zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                   const __grid_constant__ GemmParams p)
 {
     constexpr bool kAnyTma = AMODE != kGather || BMODE != kGather;
     constexpr bool kAnyGather = AMODE == kGather || BMODE == kGather;
-    constexpr uint32_t kTmaBytes = (AMODE != kGather ? A_BYTES : 0) + (BMODE != kGather ? B_BYTES : 0);
+    constexpr int TB = M3 ? 6 : 8;                       // 8 x 8 blocks per tile dimension at most (3M: 48 x 48 tiles)
+    // An M-major operand takes one TMA per 8 x 8 atom (6 per operand and k-tile).  With 3M a k-tile is 27 DMMAs per k-step
+    // instead of 64, and thread 0 issuing 12 UTMALDG per k-tile held its warp back (4500^3 M-major: 38 against 41 TFLOP/s
+    // K-major).  So lane 0 of EVERY warp issues the atoms j = warp, warp + 4 of the k-tile, following thread 0's cursor
+    // through the published segment list; thread 0 alone posts the byte count (a stage's barrier completes when its one
+    // arrival is in and the bytes of all four issuers have landed, in whichever order).
+    constexpr bool kSplitIssue = M3 && (AMODE == kTmaM || BMODE == kTmaM);
+    constexpr int kIssuers = kSplitIssue ? NTHREADS / 32 : 1;
+    constexpr uint32_t kTmaBytes = (AMODE != kGather ? TB * 1024 : 0) + (BMODE != kGather ? TB * 1024 : 0);
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;   // full[s] at +8s, empty[s] at +8(STAGES+s)
@@ -438,13 +478,13 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 tma_load_2d(sA, &tmA, 2 * k0, pm0, bar);
             } else if (AMODE == kTmaM) {
 #pragma unroll
-                for (int j = 0; j < BM / 8; ++j) tma_load_2d(sA + j * 1024, &tmA, 2 * (pm0 + 8 * j), k0, bar);
+                for (int j = 0; j < TB; j += kIssuers) tma_load_2d(sA + j * 1024, &tmA, 2 * (pm0 + 8 * j), k0, bar);
             }
             if (BMODE == kTmaK) {
                 tma_load_2d(sB, &tmB, 2 * k0, pn0, bar);
             } else if (BMODE == kTmaM) {
 #pragma unroll
-                for (int j = 0; j < BN / 8; ++j) tma_load_2d(sB + j * 1024, &tmB, 2 * (pn0 + 8 * j), k0, bar);
+                for (int j = 0; j < TB; j += kIssuers) tma_load_2d(sB + j * 1024, &tmB, 2 * (pn0 + 8 * j), k0, bar);
             }
         }
         if (++pstage == STAGES) { pstage = 0; pphase ^= 1; }
@@ -475,10 +515,44 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         if (++gstage == STAGES) { gstage = 0; gphase ^= 1; }
         if (++gk == gke) { ++gq; gather_enter(); }
     };
+    int tq = 0, tk = 0, tke = 0, tstage = 0, tm0 = 0, tn0 = 0;
+    uint32_t tphase = 0;
+    bool tvalid = false;
+    auto follow_enter = [&]() {
+        while (*q_pub <= tq) { }
+        __threadfence_block();
+        const Segment sg = q_seg[tq % kQueue];
+        tvalid = sg.tile >= 0;
+        if (tvalid) {
+            const TileGeom t = tile_geom(p, (unsigned)sg.tile);
+            tm0 = t.m0; tn0 = t.n0; tk = sg.kb; tke = sg.ke;
+        }
+    };
+    auto follow_issue = [&]() {       // this warp's atoms of k-tile tk, into the stage thread 0 fills with the same k-tile
+        const uint32_t bar = bar_base + 8 * tstage;
+        const uint32_t sA = smem_base + tstage * STAGE_BYTES, sB = sA + A_BYTES;
+        const int k0 = tk * BK;
+        if (AMODE == kTmaM) {
+#pragma unroll
+            for (int j = 0; j < TB; ++j)
+                if (j % kIssuers == warp) tma_load_2d(sA + j * 1024, &tmA, 2 * (tm0 + 8 * j), k0, bar);
+        }
+        if (BMODE == kTmaM) {
+#pragma unroll
+            for (int j = 0; j < TB; ++j)
+                if (j % kIssuers == warp) tma_load_2d(sB + j * 1024, &tmB, 2 * (tn0 + 8 * j), k0, bar);
+        }
+        if (++tstage == STAGES) { tstage = 0; tphase ^= 1; }
+        if (++tk == tke) { ++tq; follow_enter(); }
+    };
     if (tid == 0) {
         pit.init(p);
         producer_advance();
         for (int s = 0; s < STAGES && pvalid; ++s) issue();
+    }
+    if (kSplitIssue && lane == 0 && warp != 0) {
+        follow_enter();
+        for (int s = 0; s < STAGES && tvalid; ++s) follow_issue();
     }
     if (kAnyGather) {
         gather_enter();
@@ -512,14 +586,25 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 
         const bool shape44 = wg.mcnt == 4 && wg.ncnt == 4, shape43 = wg.mcnt == 4 && wg.ncnt == 3;
         const bool shape34 = wg.mcnt == 3 && wg.ncnt == 4, shape33 = wg.mcnt == 3 && wg.ncnt == 3;
+        const bool shape32 = wg.mcnt == 3 && wg.ncnt == 2, shape23 = wg.mcnt == 2 && wg.ncnt == 3;
         double cr[4][4][2], ci[4][4][2];
+        double p1[3][3][2], p2[3][3][2], p3[3][3][2];      // 3M only (dead otherwise)
+        if (!M3) {
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
+            for (int i = 0; i < 4; ++i)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                cr[i][j][0] = cr[i][j][1] = 0.0;
-                ci[i][j][0] = ci[i][j][1] = 0.0;
-            }
+                for (int j = 0; j < 4; ++j) {
+                    cr[i][j][0] = cr[i][j][1] = 0.0;
+                    ci[i][j][0] = ci[i][j][1] = 0.0;
+                }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 3; ++i)
+#pragma unroll
+                for (int j = 0; j < 3; ++j)
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) p1[i][j][h] = p2[i][j][h] = p3[i][j][h] = 0.0;
+        }
 
         for (int kt = seg.kb; kt < seg.ke; ++kt, ++done) {
             if (tid == 0 && done >= 1 && pvalid) {
@@ -528,6 +613,10 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 // slower: the wait keeps the four warps of a CTA in step, which the shared DMMA pipe prefers.
                 mbar_wait(bar_base + 8 * (STAGES + pstage), pphase ^ 1);
                 issue();
+            }
+            if (kSplitIssue && lane == 0 && warp != 0 && done >= 1 && tvalid) {
+                mbar_wait(bar_base + 8 * (STAGES + tstage), tphase ^ 1);
+                follow_issue();
             }
             if (kAnyGather && gvalid) {
                 // the gathered part of k-tile done + kGatherAhead goes into the stage that was consumed STAGES - kGatherAhead
@@ -542,6 +631,7 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             const int nks = (kt == p.ktiles - 1) ? p.klast_steps : 2;
             // The common warp shapes are tested directly, per segment flags: the jump table's indirect branch (BRX)
             // per k-tile cost 3 % of the pipe on full tiles (90.7 -> 93.4 % at 6400 x 512 x 6400).
+            if (!M3) {
             if (nks == 2 && shape44) mma_ktile<4, 4, 2>(cr, ci, sA, sB, offA, offB);
             else if (nks == 2 && shape43) mma_ktile<4, 3, 2>(cr, ci, sA, sB, offA, offB);
             else if (nks == 2 && shape34) mma_ktile<3, 4, 2>(cr, ci, sA, sB, offA, offB);
@@ -559,11 +649,44 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 #undef TCB_CASE
                 default: break;                   // a warp without blocks only keeps the barriers moving
             }
+            } else {
+            if (nks == 2 && shape33) mma_ktile3<3, 3, 2>(p1, p2, p3, sA, sB, offA, offB);
+            else if (nks == 2 && shape32) mma_ktile3<3, 2, 2>(p1, p2, p3, sA, sB, offA, offB);
+            else if (nks == 2 && shape23) mma_ktile3<2, 3, 2>(p1, p2, p3, sA, sB, offA, offB);
+            else
+            switch (wg.mcnt * 5 + wg.ncnt) {
+#define TCB_CASE(MC, NC) case MC * 5 + NC:                                              \
+    if (nks == 2) mma_ktile3<MC, NC, 2>(p1, p2, p3, sA, sB, offA, offB);                   \
+    else mma_ktile3<MC, NC, 1>(p1, p2, p3, sA, sB, offA, offB);                            \
+    break;
+                TCB_CASE(3, 3) TCB_CASE(3, 2) TCB_CASE(3, 1)
+                TCB_CASE(2, 3) TCB_CASE(2, 2) TCB_CASE(2, 1)
+                TCB_CASE(1, 3) TCB_CASE(1, 2) TCB_CASE(1, 1)
+#undef TCB_CASE
+                default: break;
+            }
+            }
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + stage));
             if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
 
+        if (M3) {                               // Re C = P1 - P2, Im C = P3 - P1 - P2
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        if (i < 3 && j < 3) {
+                            cr[i][j][h] = __dsub_rn(p1[i][j][h], p2[i][j][h]);
+                            ci[i][j][h] = __dsub_rn(p3[i][j][h], __dadd_rn(p1[i][j][h], p2[i][j][h]));
+                        } else {
+                            cr[i][j][h] = 0.0;
+                            ci[i][j][h] = 0.0;
+                        }
+                    }
+        }
         // ---- epilogue: lane holds C[m = block i, row rowmap][n = block j, column c (+4)] of its warp's blocks -----
         if (seg.slot < 0) {
             store_fragment(p, cr, ci, tg, wg, rowmap, c);
@@ -687,10 +810,10 @@ cudaError_t encode_operand(CUtensorMap *tm, const void *ptr, int64_t rows, int64
 }
 
 
-template <int AM, int BM_>
+template <int AM, int BM_, bool M3>
 cudaError_t launch_variant(const GemmTensorMaps &maps, const GemmParams &p, int grid, cudaStream_t stream)
 {
-    auto kern = zgemm_dmma_kernel<AM, BM_>;
+    auto kern = zgemm_dmma_kernel<AM, BM_, M3>;
     if (first_use_on_device((const void *)kern)) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
         if (e != cudaSuccess) return e;
@@ -699,24 +822,35 @@ cudaError_t launch_variant(const GemmTensorMaps &maps, const GemmParams &p, int 
     return cudaGetLastError();
 }
 
-template <int AM>
+template <int AM, bool M3>
 cudaError_t launch_b(int bmode, const GemmTensorMaps &maps, const GemmParams &p, int grid, cudaStream_t stream)
 {
     switch (bmode) {
-    case kTmaK: return launch_variant<AM, kTmaK>(maps, p, grid, stream);
-    case kTmaM: return launch_variant<AM, kTmaM>(maps, p, grid, stream);
-    default: return launch_variant<AM, kGather>(maps, p, grid, stream);
+    case kTmaK: return launch_variant<AM, kTmaK, M3>(maps, p, grid, stream);
+    case kTmaM: return launch_variant<AM, kTmaM, M3>(maps, p, grid, stream);
+    default: return launch_variant<AM, kGather, M3>(maps, p, grid, stream);
+    }
+}
+template <bool M3>
+cudaError_t launch_a(int amode, int bmode, const GemmTensorMaps &maps, const GemmParams &p, int grid, cudaStream_t stream)
+{
+    switch (amode) {
+    case kTmaK: return launch_b<kTmaK, M3>(bmode, maps, p, grid, stream);
+    case kTmaM: return launch_b<kTmaM, M3>(bmode, maps, p, grid, stream);
+    default: return launch_b<kGather, M3>(bmode, maps, p, grid, stream);
     }
 }
 
+
 }  // namespace
 
-GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk)
+GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk, bool m3)
 {
     GemmSchedule s;
     const int64_t mblocks = (M + 7) / 8, nblocks = (N + 7) / 8;
-    s.mt = (int)((mblocks + 7) / 8);
-    s.nt = (int)((nblocks + 7) / 8);
+    const int tb = m3 ? 6 : 8;                            // blocks per tile dimension (3M: 48 x 48 tiles)
+    s.mt = (int)((mblocks + tb - 1) / tb);
+    s.nt = (int)((nblocks + tb - 1) / tb);
     s.ktiles = (int)((K + BK - 1) / BK);
     const int64_t tiles = (int64_t)s.mt * s.nt, KT = s.ktiles;
     const int64_t slots = 2LL * sm_count();              // resident CTAs: the persistent grid is 2 per SM
@@ -782,18 +916,19 @@ cudaError_t encode_gemm_maps(const GemmDesc &g, GemmTensorMaps *maps)
 {
     // a strided dimension of extent 1 still needs a legal stride: ld >= 1 always holds here; a gathered operand has no map
     std::memset(maps, 0, sizeof *maps);
+    const int box_rows = g.m3 ? 48 : BM;
     if (!g.gatherAm) {
-        cudaError_t e = encode_operand(&maps->a, g.A, g.M, g.K, g.lda, g.a_kmajor, BM);
+        cudaError_t e = encode_operand(&maps->a, g.A, g.M, g.K, g.lda, g.a_kmajor, box_rows);
         if (e != cudaSuccess) return e;
     }
-    if (!g.gatherBn) return encode_operand(&maps->b, g.B, g.N, g.K, g.ldb, g.b_kmajor, BN);
+    if (!g.gatherBn) return encode_operand(&maps->b, g.B, g.N, g.K, g.ldb, g.b_kmajor, box_rows);
     return cudaSuccess;
 }
 
 cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps, cudaStream_t stream,
                                    int64_t *launches)
 {
-    const GemmSchedule sc = gemm_schedule(g.M, g.N, g.K, g.splitk);
+    const GemmSchedule sc = gemm_schedule(g.M, g.N, g.K, g.splitk, g.m3);
     GemmParams p;
     p.M = g.M; p.N = g.N; p.K = g.K;
     p.mblocks = (int)((g.M + 7) / 8);
@@ -829,12 +964,8 @@ cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps
     p.a_mfast = g.a_mfast ? 1 : 0; p.b_mfast = g.b_mfast ? 1 : 0;
     const int amode = g.gatherAm ? kGather : (g.a_kmajor ? kTmaK : kTmaM);
     const int bmode = g.gatherBn ? kGather : (g.b_kmajor ? kTmaK : kTmaM);
-    cudaError_t e;
-    switch (amode) {
-    case kTmaK: e = launch_b<kTmaK>(bmode, maps, p, sc.grid, stream); break;
-    case kTmaM: e = launch_b<kTmaM>(bmode, maps, p, sc.grid, stream); break;
-    default: e = launch_b<kGather>(bmode, maps, p, sc.grid, stream); break;
-    }
+    cudaError_t e = g.m3 ? launch_a<true>(amode, bmode, maps, p, sc.grid, stream)
+                         : launch_a<false>(amode, bmode, maps, p, sc.grid, stream);
     if (e != cudaSuccess) return e;
     if (launches) ++*launches;
     if (sc.sk_tiles > 0) {
