@@ -63,8 +63,10 @@ constexpr int B_BYTES = BN * BK * 16;   // 8 KB
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
 constexpr int kGatherAhead = 2;         // k-tiles a gathered operand is fetched ahead (its refill never waits for the
                                         // stage the CTA is still draining: no CTA-wide lock step per k-tile)
-constexpr int kQueue = 8;               // segment queue entries (producer is <= STAGES + 1 segments ahead)
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 128 /*barriers*/ + 256 /*segment queue*/;
+constexpr int kStages3M = 4;            // ring depth of the 3M kernel (12 KB stages)
+constexpr int kQueue = 16;              // segment queue entries (producer is <= stages + 1 segments ahead)
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 128 /*barriers*/ + 512 /*segment queue*/;
+constexpr int SMEM_BYTES_3M = kStages3M * 12 * 1024 + 1024 + 128 + 512;
 constexpr int NTHREADS = 128;
 
 struct GemmParams {
@@ -415,6 +417,10 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     constexpr bool kAnyTma = AMODE != kGather || BMODE != kGather;
     constexpr bool kAnyGather = AMODE == kGather || BMODE == kGather;
     constexpr int TB = M3 ? 6 : 8;                       // 8 x 8 blocks per tile dimension at most (3M: 48 x 48 tiles)
+    // ring: 4 stages of 16 KB; 3M: 4 stages of 12 KB (8 stages measured the same: 491.7 against 493 ms on configs[2], and
+    // the same 1.1 TB of DRAM reads -- see profiles/r2_gemm_3m.md)
+    constexpr int NST = M3 ? kStages3M : STAGES;
+    constexpr int kAOff = TB * 1024, kStageBytes = 2 * TB * 1024;
     // An M-major operand takes one TMA per 8 x 8 atom (6 per operand and k-tile).  With 3M a k-tile is 27 DMMAs per k-step
     // instead of 64, and thread 0 issuing 12 UTMALDG per k-tile held its warp back (4500^3 M-major: 38 against 41 TFLOP/s
     // K-major).  So lane 0 of EVERY warp issues the atoms j = warp, warp + 4 of the k-tile, following thread 0's cursor
@@ -425,16 +431,16 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     constexpr uint32_t kTmaBytes = (AMODE != kGather ? TB * 1024 : 0) + (BMODE != kGather ? TB * 1024 : 0);
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;   // full[s] at +8s, empty[s] at +8(STAGES+s)
+    const uint32_t bar_base = smem_base + NST * kStageBytes;   // full[s] at +8s, empty[s] at +8(NST+s)
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int warp_m = warp & 1, warp_n = warp >> 1;
 
     if (tid == 0) {
-        for (int s = 0; s < STAGES; ++s) {
+        for (int s = 0; s < NST; ++s) {
             // full: thread 0's expect_tx arrival for the TMA part + one cp.async arrival per thread for the gathered part
             mbar_init(bar_base + 8 * s, (kAnyTma ? 1 : 0) + (kAnyGather ? NTHREADS : 0));
-            mbar_init(bar_base + 8 * (STAGES + s), NTHREADS / 32);
+            mbar_init(bar_base + 8 * (NST + s), NTHREADS / 32);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         if (AMODE != kGather) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
@@ -443,7 +449,7 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     }
     __syncthreads();
 
-    // ---- producer (thread 0): walks the same segment list, STAGES k-tiles ahead of the consumers, ACROSS tile
+    // ---- producer (thread 0): walks the same segment list, NST k-tiles ahead of the consumers, ACROSS tile
     // boundaries -- the next tile's operands are already in flight while this tile's epilogue stores drain
     SegmentIter pit;
     Segment pseg;
@@ -452,7 +458,7 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     int pstage = 0;
     uint32_t pphase = 0;                // parity of the ring round the producer is filling
     // segment queue: the producer decides (or claims) what this CTA computes and publishes every segment here
-    // before its first operand load; the consumers pop them in order.  kQueue > STAGES + 1 entries suffice.
+    // before its first operand load; the consumers pop them in order.  kQueue > NST + 1 entries suffice.
     Segment *q_seg = reinterpret_cast<Segment *>(smem_raw + (bar_base - smem_u32(smem_raw)) + 128);
     volatile int *q_pub = reinterpret_cast<volatile int *>(q_seg + kQueue);
     int npub = 0;
@@ -471,7 +477,7 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     auto issue = [&]() {              // loads k-tile pk of the producer's segment into stage pstage (TMA operands)
         if (kAnyTma) {
             const uint32_t bar = bar_base + 8 * pstage;
-            const uint32_t sA = smem_base + pstage * STAGE_BYTES, sB = sA + A_BYTES;
+            const uint32_t sA = smem_base + pstage * kStageBytes, sB = sA + kAOff;
             const int k0 = pk * BK;
             mbar_expect_tx(bar, kTmaBytes);
             if (AMODE == kTmaK) {
@@ -487,7 +493,7 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 for (int j = 0; j < TB; j += kIssuers) tma_load_2d(sB + j * 1024, &tmB, 2 * (pn0 + 8 * j), k0, bar);
             }
         }
-        if (++pstage == STAGES) { pstage = 0; pphase ^= 1; }
+        if (++pstage == NST) { pstage = 0; pphase ^= 1; }
         if (++pk == pseg.ke) producer_advance();
     };
     // ---- gathered operands: EVERY thread walks the published segment list with its own cursor, in step with thread 0's,
@@ -507,12 +513,12 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         }
     };
     auto gather_issue = [&]() {
-        const uint32_t sA = smem_base + gstage * STAGE_BYTES, sB = sA + A_BYTES;
+        const uint32_t sA = smem_base + gstage * kStageBytes, sB = sA + kAOff;
         const long long k0 = (long long)gk * BK;
         if (AMODE == kGather) gather_ktile(sA, p.gA, p.gAm, gm0, gmr, p.M, p.gAk, k0, p.K, p.a_mfast != 0, tid);
         if (BMODE == kGather) gather_ktile(sB, p.gB, p.gBn, gn0, gnr, p.N, p.gBk, k0, p.K, p.b_mfast != 0, tid);
         cp_async_arrive(bar_base + 8 * gstage);
-        if (++gstage == STAGES) { gstage = 0; gphase ^= 1; }
+        if (++gstage == NST) { gstage = 0; gphase ^= 1; }
         if (++gk == gke) { ++gq; gather_enter(); }
     };
     int tq = 0, tk = 0, tke = 0, tstage = 0, tm0 = 0, tn0 = 0;
@@ -530,7 +536,7 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     };
     auto follow_issue = [&]() {       // this warp's atoms of k-tile tk, into the stage thread 0 fills with the same k-tile
         const uint32_t bar = bar_base + 8 * tstage;
-        const uint32_t sA = smem_base + tstage * STAGE_BYTES, sB = sA + A_BYTES;
+        const uint32_t sA = smem_base + tstage * kStageBytes, sB = sA + kAOff;
         const int k0 = tk * BK;
         if (AMODE == kTmaM) {
 #pragma unroll
@@ -542,17 +548,17 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             for (int j = 0; j < TB; ++j)
                 if (j % kIssuers == warp) tma_load_2d(sB + j * 1024, &tmB, 2 * (tn0 + 8 * j), k0, bar);
         }
-        if (++tstage == STAGES) { tstage = 0; tphase ^= 1; }
+        if (++tstage == NST) { tstage = 0; tphase ^= 1; }
         if (++tk == tke) { ++tq; follow_enter(); }
     };
     if (tid == 0) {
         pit.init(p);
         producer_advance();
-        for (int s = 0; s < STAGES && pvalid; ++s) issue();
+        for (int s = 0; s < NST && pvalid; ++s) issue();
     }
     if (kSplitIssue && lane == 0 && warp != 0) {
         follow_enter();
-        for (int s = 0; s < STAGES && tvalid; ++s) follow_issue();
+        for (int s = 0; s < NST && tvalid; ++s) follow_issue();
     }
     if (kAnyGather) {
         gather_enter();
@@ -611,23 +617,23 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 // refill the stage consumed in the previous iteration (the other warps had a whole k-tile to
                 // release it).  A non-blocking variant (mbarrier.test_wait, refill whatever is free) measured 7 %
                 // slower: the wait keeps the four warps of a CTA in step, which the shared DMMA pipe prefers.
-                mbar_wait(bar_base + 8 * (STAGES + pstage), pphase ^ 1);
+                mbar_wait(bar_base + 8 * (NST + pstage), pphase ^ 1);
                 issue();
             }
             if (kSplitIssue && lane == 0 && warp != 0 && done >= 1 && tvalid) {
-                mbar_wait(bar_base + 8 * (STAGES + tstage), tphase ^ 1);
+                mbar_wait(bar_base + 8 * (NST + tstage), tphase ^ 1);
                 follow_issue();
             }
             if (kAnyGather && gvalid) {
-                // the gathered part of k-tile done + kGatherAhead goes into the stage that was consumed STAGES - kGatherAhead
+                // the gathered part of k-tile done + kGatherAhead goes into the stage that was consumed NST - kGatherAhead
                 // iterations ago: every thread checks that all four warps have left it (they have, unless one lags two
                 // k-tiles; a fresh barrier passes the parity test at once)
-                mbar_wait(bar_base + 8 * (STAGES + gstage), gphase ^ 1);
+                mbar_wait(bar_base + 8 * (NST + gstage), gphase ^ 1);
                 gather_issue();
             }
             mbar_wait(bar_base + 8 * stage, phase);
-            const uint32_t sA = smem_base + stage * STAGE_BYTES + wg.moff * 1024;
-            const uint32_t sB = smem_base + stage * STAGE_BYTES + A_BYTES + wg.noff * 1024;
+            const uint32_t sA = smem_base + stage * kStageBytes + wg.moff * 1024;
+            const uint32_t sB = smem_base + stage * kStageBytes + kAOff + wg.noff * 1024;
             const int nks = (kt == p.ktiles - 1) ? p.klast_steps : 2;
             // The common warp shapes are tested directly, per segment flags: the jump table's indirect branch (BRX)
             // per k-tile cost 3 % of the pipe on full tiles (90.7 -> 93.4 % at 6400 x 512 x 6400).
@@ -667,8 +673,8 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             }
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + stage));
-            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+            if (lane == 0) mbar_arrive(bar_base + 8 * (NST + stage));
+            if (++stage == NST) { stage = 0; phase ^= 1; }
         }
 
         if (M3) {                               // Re C = P1 - P2, Im C = P3 - P1 - P2
@@ -804,7 +810,8 @@ cudaError_t encode_operand(CUtensorMap *tm, const void *ptr, int64_t rows, int64
     }
     strides[0] = (cuuint64_t)ld * 16;
     CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void *>(ptr), dims, strides, box, estr,
-                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                    getenv("TCB_GEMM_PROMO") ? (CUtensorMapL2promotion)atoi(getenv("TCB_GEMM_PROMO")) : CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
@@ -814,11 +821,12 @@ template <int AM, int BM_, bool M3>
 cudaError_t launch_variant(const GemmTensorMaps &maps, const GemmParams &p, int grid, cudaStream_t stream)
 {
     auto kern = zgemm_dmma_kernel<AM, BM_, M3>;
+    constexpr int smem = M3 ? SMEM_BYTES_3M : SMEM_BYTES;
     if (first_use_on_device((const void *)kern)) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
     }
-    kern<<<grid, NTHREADS, SMEM_BYTES, stream>>>(maps.a, maps.b, p);
+    kern<<<grid, NTHREADS, smem, stream>>>(maps.a, maps.b, p);
     return cudaGetLastError();
 }
 
