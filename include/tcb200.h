@@ -78,11 +78,10 @@ int tcb_ctx_destroy(tcb_ctx *ctx);
  *       "permute_operands" = "auto" | "always"  (A/B testing of plans: both operands always permuted);
  *       "complex_product" = "auto" | "4m" | "3m": how the GEMM forms a complex product from real tensor-core products.
  *                    "4m": Re = ArBr - AiBi, Im = ArBi + AiBr (four).  "3m": P1 = ArBr, P2 = AiBi, P3 = (Ar+Ai)(Br+Bi),
- *                    Re = P1 - P2, Im = P3 - P1 - P2 (three: 25 % less tensor work, 10 ... 18 % faster where the GEMM is
- *                    tensor-bound).  Both meet the 1e-11 * snorm tolerance with orders of magnitude to spare; 3m gives up
+ *                    Re = P1 - P2, Im = P3 - P1 - P2 (three: 25 % less tensor work, 8 ... 27 % faster).  Both meet the 1e-11 * snorm tolerance with orders of magnitude to spare; 3m gives up
  *                    bit-exact products of exactly representable operands (a delta tensor returns its partner to within
  *                    2^-52 (|re| + |im|), not bit for bit) -- real operands still give an exactly real result.  "auto": 3m
- *                    when both operands are TMA-fed, at least one is K-major and K >= 128; 4m otherwise;
+ *                    when both operands are TMA-fed (not gathered) and K >= 32; 4m otherwise;
  *       "gemm_deal" = "dynamic" | "static" (how the GEMM's tiles and stream-K chunks reach the CTAs: claimed from a counter,
  *                    or dealt round-robin; the result is the same bit for bit);
  *       "kernel_timing" = "on" | "off" (see tcb_kernel_stats);   unknown key -> TCB_EINVAL. */

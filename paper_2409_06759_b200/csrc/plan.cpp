@@ -371,12 +371,12 @@ int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const 
 
     // (vii) schedule: whole tiles data-parallel over the persistent grid, the remainder wave (or, for skinny
     // M x N with long K, everything) cut along K -- see gemm_schedule in zgemm.cu
-    // (vii-a) complex products from three real ones (3M) where the GEMM is tensor-bound and TMA-fed: measured +10 ... +18 %
-    // from K = 128 up (profiles/r2_gemm_3m.md); not with a gathered operand (the gather is the bound: -2 ... -5 %) and not with
-    // two M-major operands (12 TMA requests per k-tile: -9 %).  "complex_product" = "3m" / "4m" forces either.
-    constexpr int64_t kM3MinK = 128;
-    P.m3 = opt.complex_product == 2 ||
-           (opt.complex_product == 0 && !P.a.gather && !P.b.gather && (P.a.kmajor || P.b.kmajor) && P.K >= kM3MinK);
+    // (vii-a) complex products from three real ones (3M) where both operands are TMA-fed (in place or after a transposition):
+    // measured faster from K = 32 up in every layout pair (+8 % at K = 32, +15 % at 64, +20 ... +27 % from 512 up,
+    // profiles/r2_gemm_3m.md); K = 16 loses 6 % (one 16-deep k-tile: no pipelining), a gathered operand makes the gather the
+    // bound (0 ... -5 %).  "complex_product" = "3m" / "4m" forces either.
+    constexpr int64_t kM3MinK = 32;
+    P.m3 = opt.complex_product == 2 || (opt.complex_product == 0 && !P.a.gather && !P.b.gather && P.K >= kM3MinK);
     P.splitk = opt.splitk;
     const GemmSchedule sc = gemm_schedule(P.M, P.N, P.K, opt.splitk, P.m3);
     P.splits = sc.splits;

@@ -63,10 +63,10 @@ constexpr int B_BYTES = BN * BK * 16;   // 8 KB
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
 constexpr int kGatherAhead = 2;         // k-tiles a gathered operand is fetched ahead (its refill never waits for the
                                         // stage the CTA is still draining: no CTA-wide lock step per k-tile)
-constexpr int kStages3M = 4;            // ring depth of the 3M kernel (12 KB stages)
+constexpr int kStages3M = 4;            // ring depth of the 3M kernel (24 KB stages)
 constexpr int kQueue = 16;              // segment queue entries (producer is <= stages + 1 segments ahead)
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 128 /*barriers*/ + 512 /*segment queue*/;
-constexpr int SMEM_BYTES_3M = kStages3M * 12 * 1024 + 1024 + 128 + 512;
+constexpr int SMEM_BYTES_3M = kStages3M * 24 * 1024 + 1024 + 128 + 512;   // 16-deep stages: 2 x 6 blocks x 2 KB
 constexpr int NTHREADS = 128;
 
 struct GemmParams {
@@ -352,7 +352,7 @@ __device__ __forceinline__ void store_fragment(const GemmParams &p, const double
 // k-step would end the basic block and keep the second step's LDS from being hoisted over the first step's DMMAs.
 template <int MC, int NC, int KS>
 __device__ __forceinline__ void mma_ktile(double (&cr)[4][4][2], double (&ci)[4][4][2], uint32_t sA, uint32_t sB,
-                                          const uint32_t (&offA)[2], const uint32_t (&offB)[2])
+                                          const uint32_t (&offA)[4], const uint32_t (&offB)[4])
 {
 #pragma unroll
     for (int ks = 0; ks < KS; ++ks) {
@@ -382,18 +382,18 @@ __device__ __forceinline__ void mma_ktile(double (&cr)[4][4][2], double (&ci)[4]
 // 3 DMMAs per block pair and k-step instead of 4, three accumulator sets instead of two -- which is why a warp holds at most
 // 3 x 3 blocks here (108 accumulator registers; 4 x 4 would need 192 of the 255).  The operand sums cost MC + NC DADDs per
 // k-step on the pipe DMMA runs on (6 against 27 DMMAs of 16 issue slots each).
-template <int MC, int NC, int KS>
+template <int MC, int NC, int KS, int BLKA, int BLKB>
 __device__ __forceinline__ void mma_ktile3(double (&p1)[3][3][2], double (&p2)[3][3][2], double (&p3)[3][3][2], uint32_t sA,
-                                           uint32_t sB, const uint32_t (&offA)[2], const uint32_t (&offB)[2])
+                                           uint32_t sB, const uint32_t (&offA)[4], const uint32_t (&offB)[4])
 {
 #pragma unroll
     for (int ks = 0; ks < KS; ++ks) {
         double2 a[MC], b[NC];
         double as[MC], bs[NC];
 #pragma unroll
-        for (int i = 0; i < MC; ++i) a[i] = lds128(sA + i * 1024 + offA[ks]);
+        for (int i = 0; i < MC; ++i) a[i] = lds128(sA + i * BLKA + offA[ks]);
 #pragma unroll
-        for (int j = 0; j < NC; ++j) b[j] = lds128(sB + j * 1024 + offB[ks]);
+        for (int j = 0; j < NC; ++j) b[j] = lds128(sB + j * BLKB + offB[ks]);
 #pragma unroll
         for (int i = 0; i < MC; ++i) as[i] = __dadd_rn(a[i].x, a[i].y);
 #pragma unroll
@@ -408,6 +408,21 @@ __device__ __forceinline__ void mma_ktile3(double (&p1)[3][3][2], double (&p2)[3
             }
     }
 }
+// the last k-tile of a K that does not fill it: 1 ... 3 k-steps, once per tile -- a plain loop
+template <int MC, int NC, int BLKA, int BLKB>
+__device__ __forceinline__ void mma_ktile3_tail(double (&p1)[3][3][2], double (&p2)[3][3][2], double (&p3)[3][3][2],
+                                                uint32_t sA, uint32_t sB, const uint32_t (&offA)[4],
+                                                const uint32_t (&offB)[4], int nks)
+{
+    uint32_t oa[4] = {offA[0], offA[1], offA[2], offA[3]}, ob[4] = {offB[0], offB[1], offB[2], offB[3]};
+#pragma unroll 1
+    for (int ks = 0; ks < nks; ++ks) {
+        const uint32_t one_a[4] = {oa[0], 0, 0, 0}, one_b[4] = {ob[0], 0, 0, 0};
+        mma_ktile3<MC, NC, 1, BLKA, BLKB>(p1, p2, p3, sA, sB, one_a, one_b);
+        oa[0] = oa[1]; oa[1] = oa[2]; oa[2] = oa[3];
+        ob[0] = ob[1]; ob[1] = ob[2]; ob[2] = ob[3];
+    }
+}
 
 template <int AMODE, int BMODE, bool M3>
 __global__ void __launch_bounds__(NTHREADS, 2)
@@ -417,10 +432,15 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     constexpr bool kAnyTma = AMODE != kGather || BMODE != kGather;
     constexpr bool kAnyGather = AMODE == kGather || BMODE == kGather;
     constexpr int TB = M3 ? 6 : 8;                       // 8 x 8 blocks per tile dimension at most (3M: 48 x 48 tiles)
-    // ring: 4 stages of 16 KB; 3M: 4 stages of 12 KB (8 stages measured the same: 491.7 against 493 ms on configs[2], and
-    // the same 1.1 TB of DRAM reads -- see profiles/r2_gemm_3m.md)
+    // ring: 4 stages of 16 KB; 3M: 4 stages of 24 KB (with 8-deep stages, 8 stages of 12 KB measured the same as 4: 491.7
+    // against 493 ms on configs[2], and the same 1.1 TB of DRAM reads -- see profiles/r2_gemm_3m.md)
     constexpr int NST = M3 ? kStages3M : STAGES;
-    constexpr int kAOff = TB * 1024, kStageBytes = 2 * TB * 1024;
+    // k-values per stage: 8; 3M: 16 (two 128-byte swizzle rows).  A 3M k-step is 27 DMMAs per warp instead of 64, so with 8-deep
+    // stages the per-stage cost (barrier wait and arrive, refill, queue) weighed twice as much: DMMA pipe 84 % busy on
+    // configs[2] against 95 % for 4M.  An M-major atom becomes one 16 x 8 box of 2 KB: half the TMA requests per flop.
+    constexpr int KB = M3 ? 16 : 8, KH = KB / 8;
+    constexpr int kAOff = TB * 1024 * KH, kStageBytes = 2 * kAOff;
+    constexpr int kBlkA = AMODE == kTmaM ? 1024 * KH : 1024, kBlkB = BMODE == kTmaM ? 1024 * KH : 1024;   // 8-row block stride
     // An M-major operand takes one TMA per 8 x 8 atom (6 per operand and k-tile).  With 3M a k-tile is 27 DMMAs per k-step
     // instead of 64, and thread 0 issuing 12 UTMALDG per k-tile held its warp back (4500^3 M-major: 38 against 41 TFLOP/s
     // K-major).  So lane 0 of EVERY warp issues the atoms j = warp, warp + 4 of the k-tile, following thread 0's cursor
@@ -428,7 +448,7 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     // arrival is in and the bytes of all four issuers have landed, in whichever order).
     constexpr bool kSplitIssue = M3 && (AMODE == kTmaM || BMODE == kTmaM);
     constexpr int kIssuers = kSplitIssue ? NTHREADS / 32 : 1;
-    constexpr uint32_t kTmaBytes = (AMODE != kGather ? TB * 1024 : 0) + (BMODE != kGather ? TB * 1024 : 0);
+    constexpr uint32_t kTmaBytes = (AMODE != kGather ? TB * 1024 * (M3 ? 2 : 1) : 0) + (BMODE != kGather ? TB * 1024 * (M3 ? 2 : 1) : 0);
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar_base = smem_base + NST * kStageBytes;   // full[s] at +8s, empty[s] at +8(NST+s)
@@ -478,19 +498,21 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         if (kAnyTma) {
             const uint32_t bar = bar_base + 8 * pstage;
             const uint32_t sA = smem_base + pstage * kStageBytes, sB = sA + kAOff;
-            const int k0 = pk * BK;
+            const int k0 = pk * KB;
             mbar_expect_tx(bar, kTmaBytes);
             if (AMODE == kTmaK) {
-                tma_load_2d(sA, &tmA, 2 * k0, pm0, bar);
+#pragma unroll
+                for (int h = 0; h < KH; ++h) tma_load_2d(sA + h * TB * 1024, &tmA, 2 * (k0 + 8 * h), pm0, bar);
             } else if (AMODE == kTmaM) {
 #pragma unroll
-                for (int j = 0; j < TB; j += kIssuers) tma_load_2d(sA + j * 1024, &tmA, 2 * (pm0 + 8 * j), k0, bar);
+                for (int j = 0; j < TB; j += kIssuers) tma_load_2d(sA + j * kBlkA, &tmA, 2 * (pm0 + 8 * j), k0, bar);
             }
             if (BMODE == kTmaK) {
-                tma_load_2d(sB, &tmB, 2 * k0, pn0, bar);
+#pragma unroll
+                for (int h = 0; h < KH; ++h) tma_load_2d(sB + h * TB * 1024, &tmB, 2 * (k0 + 8 * h), pn0, bar);
             } else if (BMODE == kTmaM) {
 #pragma unroll
-                for (int j = 0; j < TB; j += kIssuers) tma_load_2d(sB + j * 1024, &tmB, 2 * (pn0 + 8 * j), k0, bar);
+                for (int j = 0; j < TB; j += kIssuers) tma_load_2d(sB + j * kBlkB, &tmB, 2 * (pn0 + 8 * j), k0, bar);
             }
         }
         if (++pstage == NST) { pstage = 0; pphase ^= 1; }
@@ -514,9 +536,14 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     };
     auto gather_issue = [&]() {
         const uint32_t sA = smem_base + gstage * kStageBytes, sB = sA + kAOff;
-        const long long k0 = (long long)gk * BK;
-        if (AMODE == kGather) gather_ktile(sA, p.gA, p.gAm, gm0, gmr, p.M, p.gAk, k0, p.K, p.a_mfast != 0, tid);
-        if (BMODE == kGather) gather_ktile(sB, p.gB, p.gBn, gn0, gnr, p.N, p.gBk, k0, p.K, p.b_mfast != 0, tid);
+        const long long k0 = (long long)gk * KB;
+#pragma unroll
+        for (int h = 0; h < KH; ++h) {
+            if (AMODE == kGather)
+                gather_ktile(sA + h * TB * 1024, p.gA, p.gAm, gm0, gmr, p.M, p.gAk, k0 + 8 * h, p.K, p.a_mfast != 0, tid);
+            if (BMODE == kGather)
+                gather_ktile(sB + h * TB * 1024, p.gB, p.gBn, gn0, gnr, p.N, p.gBk, k0 + 8 * h, p.K, p.b_mfast != 0, tid);
+        }
         cp_async_arrive(bar_base + 8 * gstage);
         if (++gstage == NST) { gstage = 0; gphase ^= 1; }
         if (++gk == gke) { ++gq; gather_enter(); }
@@ -537,16 +564,16 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     auto follow_issue = [&]() {       // this warp's atoms of k-tile tk, into the stage thread 0 fills with the same k-tile
         const uint32_t bar = bar_base + 8 * tstage;
         const uint32_t sA = smem_base + tstage * kStageBytes, sB = sA + kAOff;
-        const int k0 = tk * BK;
+        const int k0 = tk * KB;
         if (AMODE == kTmaM) {
 #pragma unroll
             for (int j = 0; j < TB; ++j)
-                if (j % kIssuers == warp) tma_load_2d(sA + j * 1024, &tmA, 2 * (tm0 + 8 * j), k0, bar);
+                if (j % kIssuers == warp) tma_load_2d(sA + j * kBlkA, &tmA, 2 * (tm0 + 8 * j), k0, bar);
         }
         if (BMODE == kTmaM) {
 #pragma unroll
             for (int j = 0; j < TB; ++j)
-                if (j % kIssuers == warp) tma_load_2d(sB + j * 1024, &tmB, 2 * (tn0 + 8 * j), k0, bar);
+                if (j % kIssuers == warp) tma_load_2d(sB + j * kBlkB, &tmB, 2 * (tn0 + 8 * j), k0, bar);
         }
         if (++tstage == NST) { tstage = 0; tphase ^= 1; }
         if (++tk == tke) { ++tq; follow_enter(); }
@@ -568,12 +595,12 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     // per-lane fragment offsets inside a 1 KB atom, for the two k-steps of a stage
     const int r = lane >> 2, c = lane & 3;
     const int rowmap = (r >> 1) + 4 * (r & 1);
-    uint32_t offA[2], offB[2];
+    uint32_t offA[4], offB[4];
 #pragma unroll
-    for (int ks = 0; ks < 2; ++ks) {
-        const int k = ks * 4 + c;
-        offA[ks] = AMODE != kTmaM ? (rowmap * 128 + ((k ^ rowmap) * 16)) : (k * 128 + ((rowmap ^ k) * 16));
-        offB[ks] = BMODE != kTmaM ? (rowmap * 128 + ((k ^ rowmap) * 16)) : (k * 128 + ((rowmap ^ k) * 16));
+    for (int ks = 0; ks < 4; ++ks) {
+        const int k = ks * 4 + c, kk = k & 7, h = k >> 3;       // 4M: ks < 2, h = 0
+        offA[ks] = AMODE != kTmaM ? (h * TB * 1024 + rowmap * 128 + ((kk ^ rowmap) * 16)) : (k * 128 + ((rowmap ^ kk) * 16));
+        offB[ks] = BMODE != kTmaM ? (h * TB * 1024 + rowmap * 128 + ((kk ^ rowmap) * 16)) : (k * 128 + ((rowmap ^ kk) * 16));
     }
 
     Segment seg;
@@ -632,9 +659,9 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 gather_issue();
             }
             mbar_wait(bar_base + 8 * stage, phase);
-            const uint32_t sA = smem_base + stage * kStageBytes + wg.moff * 1024;
-            const uint32_t sB = smem_base + stage * kStageBytes + kAOff + wg.noff * 1024;
-            const int nks = (kt == p.ktiles - 1) ? p.klast_steps : 2;
+            const uint32_t sA = smem_base + stage * kStageBytes + wg.moff * kBlkA;
+            const uint32_t sB = smem_base + stage * kStageBytes + kAOff + wg.noff * kBlkB;
+            const int nks = (kt == p.ktiles - 1) ? p.klast_steps : 2 * KH;
             // The common warp shapes are tested directly, per segment flags: the jump table's indirect branch (BRX)
             // per k-tile cost 3 % of the pipe on full tiles (90.7 -> 93.4 % at 6400 x 512 x 6400).
             if (!M3) {
@@ -656,14 +683,14 @@ zgemm_dmma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 default: break;                   // a warp without blocks only keeps the barriers moving
             }
             } else {
-            if (nks == 2 && shape33) mma_ktile3<3, 3, 2>(p1, p2, p3, sA, sB, offA, offB);
-            else if (nks == 2 && shape32) mma_ktile3<3, 2, 2>(p1, p2, p3, sA, sB, offA, offB);
-            else if (nks == 2 && shape23) mma_ktile3<2, 3, 2>(p1, p2, p3, sA, sB, offA, offB);
+            if (nks == 4 && shape33) mma_ktile3<3, 3, 4, kBlkA, kBlkB>(p1, p2, p3, sA, sB, offA, offB);
+            else if (nks == 4 && shape32) mma_ktile3<3, 2, 4, kBlkA, kBlkB>(p1, p2, p3, sA, sB, offA, offB);
+            else if (nks == 4 && shape23) mma_ktile3<2, 3, 4, kBlkA, kBlkB>(p1, p2, p3, sA, sB, offA, offB);
             else
             switch (wg.mcnt * 5 + wg.ncnt) {
 #define TCB_CASE(MC, NC) case MC * 5 + NC:                                              \
-    if (nks == 2) mma_ktile3<MC, NC, 2>(p1, p2, p3, sA, sB, offA, offB);                   \
-    else mma_ktile3<MC, NC, 1>(p1, p2, p3, sA, sB, offA, offB);                            \
+    if (nks == 4) mma_ktile3<MC, NC, 4, kBlkA, kBlkB>(p1, p2, p3, sA, sB, offA, offB);     \
+    else mma_ktile3_tail<MC, NC, kBlkA, kBlkB>(p1, p2, p3, sA, sB, offA, offB, nks);       \
     break;
                 TCB_CASE(3, 3) TCB_CASE(3, 2) TCB_CASE(3, 1)
                 TCB_CASE(2, 3) TCB_CASE(2, 2) TCB_CASE(2, 1)
@@ -791,7 +818,7 @@ EncodeTiledFn get_encode_fn()
 
 // one operand: K-major -> dims {2K doubles, rows}, box {16, 64};  M-major -> dims {2*rows doubles, K}, box {16, 8}
 cudaError_t encode_operand(CUtensorMap *tm, const void *ptr, int64_t rows, int64_t K, int64_t ld, bool kmajor,
-                           int box_rows)
+                           int box_rows, int box_k)
 {
     EncodeTiledFn fn = get_encode_fn();
     if (!fn) return cudaErrorNotSupported;
@@ -806,7 +833,7 @@ cudaError_t encode_operand(CUtensorMap *tm, const void *ptr, int64_t rows, int64
         dims[0] = (cuuint64_t)(2 * rows);
         dims[1] = (cuuint64_t)K;
         box[0] = 16;
-        box[1] = 8;
+        box[1] = (cuuint32_t)box_k;
     }
     strides[0] = (cuuint64_t)ld * 16;
     CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void *>(ptr), dims, strides, box, estr,
@@ -859,7 +886,8 @@ GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk, bool m3)
     const int tb = m3 ? 6 : 8;                            // blocks per tile dimension (3M: 48 x 48 tiles)
     s.mt = (int)((mblocks + tb - 1) / tb);
     s.nt = (int)((nblocks + tb - 1) / tb);
-    s.ktiles = (int)((K + BK - 1) / BK);
+    const int kb = m3 ? 16 : BK;                          // k-values per stage
+    s.ktiles = (int)((K + kb - 1) / kb);
     const int64_t tiles = (int64_t)s.mt * s.nt, KT = s.ktiles;
     const int64_t slots = 2LL * sm_count();              // resident CTAs: the persistent grid is 2 per SM
     s.dp_tiles = tiles; s.sk_tiles = 0; s.sk_chunks = 0; s.sk_q = 1; s.sk_slots = 1; s.splits = 1;
@@ -926,10 +954,10 @@ cudaError_t encode_gemm_maps(const GemmDesc &g, GemmTensorMaps *maps)
     std::memset(maps, 0, sizeof *maps);
     const int box_rows = g.m3 ? 48 : BM;
     if (!g.gatherAm) {
-        cudaError_t e = encode_operand(&maps->a, g.A, g.M, g.K, g.lda, g.a_kmajor, box_rows);
+        cudaError_t e = encode_operand(&maps->a, g.A, g.M, g.K, g.lda, g.a_kmajor, box_rows, g.m3 ? 16 : 8);
         if (e != cudaSuccess) return e;
     }
-    if (!g.gatherBn) return encode_operand(&maps->b, g.B, g.N, g.K, g.ldb, g.b_kmajor, box_rows);
+    if (!g.gatherBn) return encode_operand(&maps->b, g.B, g.N, g.K, g.ldb, g.b_kmajor, box_rows, g.m3 ? 16 : 8);
     return cudaSuccess;
 }
 
@@ -952,7 +980,7 @@ cudaError_t launch_zgemm_with_maps(const GemmDesc &g, const GemmTensorMaps &maps
     p.gn = p.nt <= 32 ? p.nt : 16;
     if (getenv("TCB_GEMM_GN")) p.gn = std::max(1, std::min(p.nt, atoi(getenv("TCB_GEMM_GN"))));
     p.ktiles = sc.ktiles;
-    p.klast_steps = (int)((g.K - (int64_t)(sc.ktiles - 1) * BK + 3) / 4);
+    p.klast_steps = (int)((g.K - (int64_t)(sc.ktiles - 1) * (g.m3 ? 16 : BK) + 3) / 4);
     p.dp_tiles = sc.dp_tiles; p.sk_tiles = sc.sk_tiles; p.sk_chunks = sc.sk_chunks;
     p.sk_q = sc.sk_q; p.sk_slots = sc.sk_slots;
     p.D = (double2 *)g.D;

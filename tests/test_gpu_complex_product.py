@@ -1,9 +1,10 @@
 """-m gpu: the GEMM's two ways to form a complex product (context option "complex_product"):
     "4m"  four real DMMAs per block pair and k-step  (Re = ArBr - AiBi, Im = ArBi + AiBr)
     "3m"  three                                       (P1 = ArBr, P2 = AiBi, P3 = (Ar+Ai)(Br+Bi); Re = P1 - P2, Im = P3 - P1 - P2)
-    "auto" 3m where both operands are TMA-fed, not both M-major, and K >= 128 (csrc/plan.cpp).
+    "auto" 3m where both operands are TMA-fed and K >= 32 (csrc/plan.cpp).
 Both against the nested-loop oracle within north_star's 1e-11 * snorm, element by element, over the shapes that exercise the
-3M kernel's own geometry (48 x 48 tiles, warps of up to 3 x 3 blocks, M-major atoms issued by all four warps, stream-K
+3M kernel's own geometry (48 x 48 tiles, 16-deep k-tiles with tails of 1 ... 3 k-steps, warps of up to 3 x 3 blocks, M-major
+atoms issued by all four warps, stream-K
 fragments, gathered operands, K tails); what 3M gives up (bit-exact products with exactly representable operands) is
 asserted as well, with its bound."""
 import numpy as np
@@ -53,7 +54,10 @@ GEOMETRY = [   # (expr, extents): all four TMA layout pairs, ragged tiles, one-b
     ("C(m,n)+=A(k,m)*B(n,k)", dict(m=7, n=300, k=129)),        # K-major A, M-major B, one block of rows
     ("C(m,n)=A(m,k)*B(k,n)", dict(m=2, n=3, k=1000)),          # six outputs in one block (N = 1 would take the GEMV route)
     ("C(m,n)=A(m,k)*B(k,n)", dict(m=96, n=96, k=4)),           # one k-step
-    ("C(m,n)=A(m,k)*B(k,n)", dict(m=96, n=96, k=13)),          # k tail of 5: two k-steps, the second half empty
+    ("C(m,n)=A(m,k)*B(k,n)", dict(m=96, n=96, k=13)),          # one 16-deep k-tile, 4 k-steps, the last with one valid k
+    ("C(m,n)=A(k,m)*B(n,k)", dict(m=50, n=96, k=16 * 5 + 9)),  # tail k-tile of 3 k-steps, K-major A / M-major B
+    ("C(m,n)=A(k,m)*B(k,n)", dict(m=96, n=50, k=16 * 3 + 5)),  # tail k-tile of 2 k-steps
+    ("C(m,n)=A(m,k)*B(n,k)", dict(m=70, n=70, k=16 * 2 + 1)),  # tail k-tile of 1 k-step, both M-major
     ("R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)", dict(a=13, b=13, c=13, d=13, i=5, j=5)),
     ("X(a,b,i,j)=T(a,c,i,k)*I(k,b,c,j)", dict(a=11, b=11, c=11, i=6, j=6, k=6)),      # ring term: transposed or gathered operands
 ]
@@ -90,9 +94,9 @@ def test_auto_takes_3m_where_it_was_measured_faster_and_4m_elsewhere(ctx):
             for t in ts:
                 t.destroy()
     mm = "C(m,n)=A(m,k)*B(k,n)"
-    assert plan_of(mm, [(200, 200), (200, 128), (128, 200)])["complex_product"] == "3m"          # K = 128, TMA-fed
-    assert plan_of(mm, [(200, 200), (200, 127), (127, 200)])["complex_product"] == "4m"          # short K
-    assert plan_of("C(m,n)=A(m,k)*B(n,k)", [(200, 200), (200, 500), (200, 500)])["complex_product"] == "4m"   # both M-major
+    assert plan_of(mm, [(200, 200), (200, 32), (32, 200)])["complex_product"] == "3m"             # K = 32, TMA-fed
+    assert plan_of(mm, [(200, 200), (200, 31), (31, 200)])["complex_product"] == "4m"             # short K
+    assert plan_of("C(m,n)=A(m,k)*B(n,k)", [(200, 200), (200, 500), (200, 500)])["complex_product"] == "3m"   # any layout pair
     ring = "X(a,b,i,j)=T(a,c,i,k)*I(k,b,c,j)"
     shapes = [(40, 40, 10, 10), (40, 40, 10, 10), (10, 40, 40, 10)]
     assert plan_of(ring, shapes, operand_loads="gather")["complex_product"] == "4m"               # a gathered operand
