@@ -297,6 +297,8 @@ int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const 
             for (const Feed &cb : feeds_of(sb, seqB, dorderB, co, false)) {
                 const double wd = (seqD.empty() || (!ca.forder.empty() && ca.forder[0] == seqD[0])) ? 1.0 : 2.0;
                 double fl = flops / kPeak;
+                // TMA-fed candidates run with three real products per complex product (vii-a): measured 0.80 of the 4M time
+                if (opt.complex_product != 1 && ca.kind != 1 && cb.kind != 1 && P.K >= 32) fl *= 0.80;
                 if (ca.kind == 1) fl *= ca.waste > 1.0 ? kGatherScattered : kGatherCost;
                 if (cb.kind == 1) fl *= cb.waste > 1.0 ? kGatherScattered : kGatherCost;
                 const double by = (16.0 * (double)sizeA * ca.waste + 16.0 * (double)sizeB * cb.waste + bytesD * wd) / kBw;

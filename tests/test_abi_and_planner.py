@@ -116,7 +116,12 @@ def test_cost_model_picks_per_operand_feeds():
     # pp ladder: both in place by TMA, cost = the tensor-bound GEMM
     p = plan("R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)", (v, v, o, o), (v, v, v, v), (v, v, o, o))
     assert p["feed_A"] == "tma" and p["feed_B"] == "tma"
-    assert abs(p["est_us"] - 8.0 * 22500 * 900 * 22500 / (37.2e12 * 0.92) * 1e6) < 0.02 * p["est_us"]
+    # ... run with three real products per complex product (0.80 of the four-product time); "4m" costs the full time
+    assert p["complex_product"] == "3m"
+    assert abs(p["est_us"] - 0.80 * 8.0 * 22500 * 900 * 22500 / (37.2e12 * 0.92) * 1e6) < 0.02 * p["est_us"]
+    p4 = plan("R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)", (v, v, o, o), (v, v, v, v), (v, v, o, o), "complex_product=4m")
+    assert p4["complex_product"] == "4m"
+    assert abs(p4["est_us"] - 8.0 * 22500 * 900 * 22500 / (37.2e12 * 0.92) * 1e6) < 0.02 * p4["est_us"]
     # the two-pass epilogue is an option, never the default
     assert p["epilogue"] == "fused-scatter"
     assert plan("R(a,b,i,j)+=V(a,b,c,d)*T(c,d,i,j)", (v, v, o, o), (v, v, v, v), (v, v, o, o), "epilogue=twopass")["epilogue"] == "twopass"
