@@ -330,6 +330,10 @@ def run_ours(args, rank, world, local_rank):
                      # multiply-add on the tensor pipe): frac may exceed 1 against the real-arithmetic peak; frac_issued
                      # is what the pipe does.
                      "complex_product": plan.get("complex_product"),
+                     "frac_note": "achieved and frac count SURVEY 8(d)'s 8 real flop per complex multiply-add; with complex_product = 3m "
+                                  "the kernel forms a complex product from 3 real tensor-core products instead of 4 (6 flop issued per "
+                                  "complex multiply-add), so frac > 1 is the algorithmic gain over the real-arithmetic peak and "
+                                  "frac_issued (= 0.75 frac) is what the tensor pipe executes; ncu: profiles/r2_gemm_3m.md",
                      "issued_tensor_flops_per_launch": zg["flops"] / max(zg["launches"], 1) * (0.75 if plan.get("complex_product") == "3m" else 1.0),
                      "frac_issued": achieved / FP64_TENSOR_PEAK_TFLOPS * (0.75 if plan.get("complex_product") == "3m" else 1.0),
                      "peak_source": "derived FP64 DMMA peak 148 SM x 128 flop/clk x 1.965 GHz (MEASURED_PEAKS.json has no FP64 "
