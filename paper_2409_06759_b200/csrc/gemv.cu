@@ -36,10 +36,10 @@ __device__ __forceinline__ void cmac(double2 &acc, const double2 a, const double
     acc.y = fma(a.x, b.y, fma(a.y, b.x, acc.y));
 }
 
-__device__ __forceinline__ void finish(const GemvParams &p, long long m, double2 acc)
+__device__ __forceinline__ void finish(const GemvParams &p, long long m, double2 acc, long long chunk)
 {
     if (p.ksplit > 1) {
-        p.partial[(long long)blockIdx.y * p.M + m] = acc;
+        p.partial[chunk * p.M + m] = acc;
         return;
     }
     double2 v = make_double2(p.ar * acc.x - p.ai * acc.y, p.ar * acc.y + p.ai * acc.x);
@@ -73,15 +73,18 @@ __global__ void __launch_bounds__(GT) gemv_mfast_kernel(const __grid_constant__ 
             for (; k < nk; ++k) cmac(acc, row[s_o[k]], s_b[k]);
         }
     }
-    if (m < p.M) finish(p, m, acc);
+    if (m < p.M) finish(p, m, acc, blockIdx.y);
 }
 
 __global__ void __launch_bounds__(GT) gemv_kfast_kernel(const __grid_constant__ GemvParams p)
 {
+    // one warp per (row, k-chunk) pair, rows fastest: with few rows (M = 1: a full contraction into a rank-0 tensor) all
+    // eight warps of a CTA still have work (one warp per CTA ran E() = V(i,j,a,b) T(a,b,i,j) at 0.8 TB/s)
     const int lane = threadIdx.x & 31;
-    const long long m = (long long)blockIdx.x * (GT / 32) + (threadIdx.x >> 5);
-    if (m >= p.M) return;
-    const long long k0 = (long long)blockIdx.y * p.kchunk, k1 = min(p.K, k0 + p.kchunk);
+    const long long pair = (long long)blockIdx.x * (GT / 32) + (threadIdx.x >> 5);
+    const long long chunk = pair / p.M, m = pair - chunk * p.M;
+    if (chunk >= p.ksplit) return;
+    const long long k0 = chunk * p.kchunk, k1 = min(p.K, k0 + p.kchunk);
     const double2 *row = p.A + p.offAm[m];
     double2 acc[2] = {make_double2(0.0, 0.0), make_double2(0.0, 0.0)};
     long long k = k0 + lane;
@@ -97,7 +100,7 @@ __global__ void __launch_bounds__(GT) gemv_kfast_kernel(const __grid_constant__ 
         s.x += __shfl_down_sync(0xffffffffu, s.x, d);
         s.y += __shfl_down_sync(0xffffffffu, s.y, d);
     }
-    if (lane == 0) finish(p, m, s);
+    if (lane == 0) finish(p, m, s, chunk);
 }
 
 // chunk partials -> D: one warp per row, lanes stride over the chunks in order, then a fixed shuffle tree (deterministic)
@@ -198,12 +201,16 @@ cudaError_t launch_outer(const OuterDesc &g, cudaStream_t stream, int64_t *launc
 
 int gemv_ksplit(int64_t M, int64_t K, bool kfast)
 {
-    const int64_t ctas_m = kfast ? (M + GT / 32 - 1) / (GT / 32) : (M + GT - 1) / GT;
-    const int64_t min_chunk = kfast ? 512 : 256;
     const int64_t sms = sm_count();
+    if (kfast) {                                  // a warp per (row, chunk): 32 warps per SM wanted, chunks of >= 512
+        const int64_t want = 32 * sms;
+        const int64_t s = std::min<int64_t>((want + M - 1) / M, K / 512);
+        return (int)std::max<int64_t>(1, std::min<int64_t>(s, want));
+    }
+    const int64_t ctas_m = (M + GT - 1) / GT;
     int64_t s = (4 * sms + ctas_m - 1) / ctas_m;
-    s = std::min<int64_t>(s, K / min_chunk);
-    return (int)std::max<int64_t>(1, std::min<int64_t>(s, kfast ? 8 * 4 * sms : 64));   // a dot product: one warp per chunk
+    s = std::min<int64_t>(s, K / 256);
+    return (int)std::max<int64_t>(1, std::min<int64_t>(s, 64));
 }
 
 cudaError_t launch_gemv(const GemvDesc &g, cudaStream_t stream, int64_t *launches)
@@ -222,8 +229,8 @@ cudaError_t launch_gemv(const GemvDesc &g, cudaStream_t stream, int64_t *launche
     p.kchunk = (p.kchunk + 63) / 64 * 64;
     p.ksplit = (int)((g.K + p.kchunk - 1) / p.kchunk);
     if (g.kfast) {
-        dim3 grid((unsigned)((g.M + GT / 32 - 1) / (GT / 32)), (unsigned)p.ksplit);
-        gemv_kfast_kernel<<<grid, GT, 0, stream>>>(p);
+        const long long pairs = (long long)g.M * p.ksplit;
+        gemv_kfast_kernel<<<(unsigned)((pairs + GT / 32 - 1) / (GT / 32)), GT, 0, stream>>>(p);
     } else {
         dim3 grid((unsigned)((g.M + GT - 1) / GT), (unsigned)p.ksplit);
         gemv_mfast_kernel<<<grid, GT, 0, stream>>>(p);
