@@ -281,9 +281,14 @@ int plan_contraction(const ParsedExpr &e, const Shape &D, const Shape &L, const 
     // achievable rates on a B200: 0.92 of the FP64 tensor peak, 5.5 TB/s for a transposition pass
     const double kPeak = 37.2e12 * 0.92, kBw = 6.0e12, kBwPerm = 5.5e12, kLaunch = 4e-6;
     // what a gathered operand costs the tensor pipe (table loads, address arithmetic and 4 x LDGSTS per thread and k-tile
-    // are issued by the warps that also issue the DMMAs), measured on 4500^3 and 1600^3 ring terms (profiles/r2_gather_ab.md):
-    // +4.5 % per operand whose lanes run along contiguous memory, +26 % when every lane fetches its own 32-byte sector
-    const double kGatherCost = 1.045, kGatherScattered = 1.26;
+    // are issued by the warps that also issue the DMMAs; a gathered operand also keeps the GEMM on four real products).
+    // Measured against 0.92 of the peak: 4500^3 and 1600^3 ring terms with both operands gathered 1.34 (1.16 per operand),
+    // 100 x 12000 x 79200 with a gathered 15 GB view of T3 1.28, 79200 x 100 x 12000 1.19 (profiles/r2_gemm_ab.md,
+    // profiles/r2_ccsdt_packed.md): +18 % per operand whose lanes run along contiguous memory, +30 % when every lane
+    // fetches its own 32-byte sector
+    // -- in the tensor-bound regime (K >= 256).  A short-K GEMM leaves the issue slots the gather needs idle anyway: there the
+    // first calibration stands (+4.5 % / +26 %; R2 += vvvo T1, K = 150: 1.51 ms transposed first, 1.20 ms gathered)
+    const double kGatherCost = P.K >= 256 ? 1.18 : 1.045, kGatherScattered = P.K >= 256 ? 1.30 : 1.26;
     const double flops = 8.0 * (double)P.M * (double)P.N * (double)P.K;
     const double bytesD = 16.0 * (double)sizeD * (e.accumulate ? 2.0 : 1.0);
     std::vector<std::vector<const Lab *>> corders;
