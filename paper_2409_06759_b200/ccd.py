@@ -589,29 +589,34 @@ def t1_dressed_blocks(ctx, o, h, g, T1, names):
             ctx.contract("F(P,Q)=Xr(P,p)*F1(p,Q)", out[name], Xr[P], F1, 1.0)
             F1.destroy()
         hJ.destroy()
-    # ---- g~ blocks: index 4, then 3, then 2, then 1; partial transforms shared between the blocks that need them
+    # ---- g~ blocks.  Every step contracts the FIRST (unit-stride) index of its operand and appends the new index last:
+    #     G1(q,r,s,P) = g(p,q,r,s) X(P,p);  G2(r,s,P,Q) = G1(q,..) X(Q,q);  G3(s,P,Q,R) = G2(r,..) Y(r,R);  g~(P,Q,R,S) = G3(s,..) Y(s,S)
+    # so each operand is a K-major matrix as it lies in memory and each result a plain matrix: four TMA-fed GEMMs per block,
+    # no gather tables and no transposition (contracting index 4, 3, 2, 1 in place left the free indices on both sides of the
+    # contracted one: three of the four steps ran on gathered operands).  Partial transforms are shared between the blocks
+    # that need them.
     gnames = sorted(x for x in names if x[0] != "f")
-    for S in "ov":
-        needS = [x for x in gnames if x[3] == S]
-        if not needS:
+    for P in "ov":
+        needP = [x for x in gnames if x[0] == P]
+        if not needP:
             continue
-        G1 = new((n, n, n, ext[S]))
-        ctx.contract("G1(p,q,r,S)=g(p,q,r,s)*Yc(s,S)", G1, g, Yc[S], 1.0)
-        for Rr in "ov":
-            needR = [x for x in needS if x[2] == Rr]
-            if not needR:
+        G1 = new((n, n, n, ext[P]))
+        ctx.contract("G1(q,r,s,P)=g(p,q,r,s)*Xr(P,p)", G1, g, Xr[P], 1.0)
+        for Q in "ov":
+            needQ = [x for x in needP if x[1] == Q]
+            if not needQ:
                 continue
-            G2 = new((n, n, ext[Rr], ext[S]))
-            ctx.contract("G2(p,q,R,S)=G1(p,q,r,S)*Yc(r,R)", G2, G1, Yc[Rr], 1.0)
-            for Q in "ov":
-                needQ = [x for x in needR if x[1] == Q]
-                if not needQ:
+            G2 = new((n, n, ext[P], ext[Q]))
+            ctx.contract("G2(r,s,P,Q)=G1(q,r,s,P)*Xr(Q,q)", G2, G1, Xr[Q], 1.0)
+            for Rr in "ov":
+                needR = [x for x in needQ if x[2] == Rr]
+                if not needR:
                     continue
-                G3 = new((n, ext[Q], ext[Rr], ext[S]))
-                ctx.contract("G3(p,Q,R,S)=Xr(Q,q)*G2(p,q,R,S)", G3, Xr[Q], G2, 1.0)
-                for name in needQ:
-                    out[name] = new((ext[name[0]], ext[Q], ext[Rr], ext[S]))
-                    ctx.contract("G(P,Q,R,S)=Xr(P,p)*G3(p,Q,R,S)", out[name], Xr[name[0]], G3, 1.0)
+                G3 = new((n, ext[P], ext[Q], ext[Rr]))
+                ctx.contract("G3(s,P,Q,R)=G2(r,s,P,Q)*Yc(r,R)", G3, G2, Yc[Rr], 1.0)
+                for name in needR:
+                    out[name] = new((ext[P], ext[Q], ext[Rr], ext[name[3]]))
+                    ctx.contract("G(P,Q,R,S)=G3(s,P,Q,R)*Yc(s,S)", out[name], G3, Yc[name[3]], 1.0)
                 G3.destroy()
             G2.destroy()
         G1.destroy()
