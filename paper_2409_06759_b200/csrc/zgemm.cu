@@ -899,7 +899,7 @@ GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk, bool m3)
         const int64_t rem = tiles % slots;
         // worth it when the remainder wave would leave most of the chip idle for a whole K sweep; a chunk
         // shorter than 8 k-tiles costs more in fix-up traffic than it saves
-        if (rem > 0 && rem * KT / slots + 8 < KT * 9 / 10) {
+        if (rem > 0 && rem * KT / slots + (m3 ? 4 : 8) < KT * 9 / 10) {      // the fix-up costs about 8 k-tiles (4 of the 16-deep ones)
             s.dp_tiles = tiles - rem; s.sk_tiles = rem;
             // three to six chunks per CTA, claimed dynamically: they even out what whole tiles left uneven and what
             // ragged tiles make uneven among the chunks themselves (a 6 x 6-block tile costs half an 8 x 8 one).
@@ -932,7 +932,10 @@ GemmSchedule gemm_schedule(int64_t M, int64_t N, int64_t K, int splitk, bool m3)
             const bool ragged = 4 * mm_ * mn_ * tiles >= 5 * sm_ * sn_;          // max >= 1.25 x mean
             const bool few = tiles > 1 && tiles < 16 && ragged;
             const int64_t per_cta = tiles >= slots ? 6 : tiles >= 16 ? 3 : few ? 4 : 1;
-            const int64_t chunks = std::max<int64_t>(1, std::min<int64_t>(per_cta * slots, rem * KT / (few ? 24 : 8)));
+            // shortest chunk: 8 k-tiles; 5 of the 3M kernel's 16-deep ones (configs[0], 576 x 64 x 576 = 24 tiles of 36 k-tiles:
+            // 5 chunks per tile 19.9 us per call in a graph, 6 chunks 16.7 us, 9 chunks 17.5 us, 18 chunks 20.2 us)
+            const int64_t min_q = few ? 24 : m3 ? 5 : 8;
+            const int64_t chunks = std::max<int64_t>(1, std::min<int64_t>(per_cta * slots, rem * KT / min_q));
             s.sk_q = (int)((rem * KT + chunks - 1) / chunks);
             if (s.dp_tiles == 0) s.splits = (int)((KT + s.sk_q - 1) / s.sk_q);
         }
